@@ -1,0 +1,170 @@
+"""ORACLE — test infrastructure, not the product.
+
+ctypes wrapper around oracle/ajt_oracle.c (plain C: brute-force merge, fp64 loss).  Only tests/,
+__graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import this package.
+It never imports paper_2606_04484_b200 and shares nothing with its CUDA sources.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "ajt_oracle.c")
+_SO = os.path.join(_HERE, "libajt_oracle.so")
+
+OWNER_LONGEST = 0   # BASELINE.json north_star: longest surviving extender, then lowest index
+OWNER_PAPER = 1     # Algorithm 1 taken literally: the latest extender
+DT_BF16 = 0
+DT_F32 = 1
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _SO, _SRC, "-lm"])
+    return _SO
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_SO)
+        _lib.ajt_oracle_merge.restype = C.c_int
+        _lib.ajt_oracle_loss.restype = C.c_int
+        _lib.ajt_oracle_round_bf16.restype = C.c_double
+        _lib.ajt_oracle_round_bf16.argtypes = [C.c_double]
+        _lib.ajt_oracle_num_threads.restype = C.c_int
+        _lib.ajt_oracle_set_threads.argtypes = [C.c_int]
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().ajt_oracle_num_threads())
+
+
+def set_threads(n: int) -> None:
+    lib().ajt_oracle_set_threads(int(n))
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _c(a, dtype):
+    if a is None:
+        return None
+    a = np.ascontiguousarray(a, dtype=dtype)
+    return a
+
+
+@dataclass
+class MergeResult:
+    merged_tokens: np.ndarray    # int32 [N_out]
+    merged_mask: np.ndarray      # uint8 [N_out]
+    merged_src: np.ndarray       # int32 [N_out]
+    merged_old_logp: Optional[np.ndarray]  # float32 [N_out]
+    merged_offsets: np.ndarray   # int64 [M+1]
+    merged_origin: np.ndarray    # int32 [M]
+    merged_traj: np.ndarray      # int32 [M]
+    owner: np.ndarray            # int32 [n]
+    M: int
+    N_out: int
+
+
+def merge_timelines(tokens, offsets, traj_ids, resp_start=None, mask_in=None, old_logp_in=None,
+                    owner_rule: int = OWNER_LONGEST) -> MergeResult:
+    """Definition of the merge (DESIGN.md O-M; Algorithm 1) by brute force."""
+    tokens = _c(tokens, np.int32)
+    offsets = _c(offsets, np.int64)
+    traj_ids = _c(traj_ids, np.int32)
+    resp_start = _c(resp_start, np.int32)
+    mask_in = _c(mask_in, np.uint8)
+    old_logp_in = _c(old_logp_in, np.float32)
+    n = int(traj_ids.shape[0])
+    assert offsets.shape[0] == n + 1
+    N = int(tokens.shape[0])
+    assert n == 0 or int(offsets[-1]) == N
+    mt = np.zeros(max(N, 1), np.int32)
+    mm = np.zeros(max(N, 1), np.uint8)
+    ms = np.zeros(max(N, 1), np.int32)
+    ml = np.zeros(max(N, 1), np.float32) if old_logp_in is not None else None
+    mo = np.zeros(n + 1, np.int64)
+    mor = np.zeros(max(n, 1), np.int32)
+    mtr = np.zeros(max(n, 1), np.int32)
+    ow = np.zeros(max(n, 1), np.int32)
+    cnt = np.zeros(2, np.int64)
+    rc = lib().ajt_oracle_merge(_p(tokens), _p(offsets), _p(traj_ids), _p(resp_start), _p(mask_in), _p(old_logp_in),
+                                C.c_int32(n), C.c_int32(owner_rule), _p(mt), _p(mm), _p(ms), _p(ml), _p(mo),
+                                _p(mor), _p(mtr), _p(ow), _p(cnt))
+    if rc != 0:
+        raise ValueError(f"ajt_oracle_merge: invalid input (rc={rc})")
+    M, No = int(cnt[0]), int(cnt[1])
+    return MergeResult(mt[:No].copy(), mm[:No].copy(), ms[:No].copy(), None if ml is None else ml[:No].copy(),
+                       mo[:M + 1].copy(), mor[:M].copy(), mtr[:M].copy(), ow[:n].copy(), M, No)
+
+
+@dataclass
+class LossResult:
+    loss: float                  # sum over the given rows of w_t L_t (the whole loss when all rows are given)
+    logp: np.ndarray             # float64 [R]
+    w: np.ndarray                # float64 [R]
+    g: np.ndarray                # float64 [R]
+    Lt: np.ndarray               # float64 [R]
+    dlogits: Optional[np.ndarray]  # float64 [R,V], before rounding
+    stats: np.ndarray            # float64 [4]
+
+
+def policy_loss(logits, targets, old_logp, adv, mask, seg_ids, S: int, eps_lo: float, eps_hi: float,
+                seg_denom=None, inv_num_segs: float = 0.0, grad_scale: float = 1.0,
+                row_ids=None, want_dlogits: bool = True, logits_is_bf16_bits: bool = False) -> LossResult:
+    """fp64 loss oracle (DESIGN.md O-L).  `logits` is float32 [R,V], or uint16 [R,V] holding bf16 bit
+    patterns when logits_is_bf16_bits.  Per-token vectors have length T (all tokens of the call);
+    `row_ids` (int64 [R]) says which tokens the given logits rows are (None => R == T)."""
+    if logits_is_bf16_bits:
+        logits = _c(logits, np.uint16)
+        dt = DT_BF16
+    else:
+        logits = _c(logits, np.float32)
+        dt = DT_F32
+    R, V = int(logits.shape[0]), int(logits.shape[1])
+    targets = _c(targets, np.int32)
+    old_logp = _c(old_logp, np.float32)
+    adv = _c(adv, np.float32)
+    mask = _c(mask, np.uint8)
+    seg_ids = _c(seg_ids, np.int32)
+    T = int(targets.shape[0])
+    row_ids = _c(row_ids, np.int64)
+    if row_ids is None:
+        assert R == T
+    seg_denom = _c(seg_denom, np.float32)
+    loss = np.zeros(1, np.float64)
+    logp = np.zeros(max(R, 1), np.float64)
+    w = np.zeros(max(R, 1), np.float64)
+    g = np.zeros(max(R, 1), np.float64)
+    Lt = np.zeros(max(R, 1), np.float64)
+    dl = np.zeros((R, V), np.float64) if want_dlogits else None
+    stats = np.zeros(4, np.float64)
+    rc = lib().ajt_oracle_loss(_p(logits), C.c_int32(dt), C.c_int64(R), C.c_int32(V), C.c_int64(V), _p(row_ids),
+                               _p(targets), _p(old_logp), _p(adv), _p(mask), _p(seg_ids), C.c_int64(T), C.c_int32(S),
+                               C.c_double(eps_lo), C.c_double(eps_hi), _p(seg_denom), C.c_double(inv_num_segs),
+                               C.c_double(grad_scale), _p(loss), _p(logp), _p(w), _p(g), _p(Lt), _p(dl), _p(stats))
+    if rc != 0:
+        raise ValueError(f"ajt_oracle_loss: invalid input (rc={rc})")
+    return LossResult(float(loss[0]), logp[:R], w[:R], g[:R], Lt[:R], dl, stats)
+
+
+def round_bf16(x: np.ndarray) -> np.ndarray:
+    """fp64 -> nearest bf16 (ties to even), as fp64."""
+    a = np.ascontiguousarray(x, np.float64)
+    out = np.empty_like(a)
+    lib().ajt_oracle_round_bf16_array(_p(a), _p(out), C.c_int64(a.size))
+    return out
