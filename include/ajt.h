@@ -1,0 +1,190 @@
+/*
+ * ajt.h — C ABI of libajt.so: B200-native (sm_100a) timeline merging and policy-loss fwd+bwd.
+ *
+ * The two hot-path calls follow the paper's statement of the problem (arxiv/paper_2606_04484,
+ * "AgentJet"; line numbers are /root/reference/PAPER.md):
+ *
+ *   ajt_merge_timelines      Timeline merging, Algorithm 1 (§4.4.2) on flat token
+ *                            streams with token-level Match: every timeline whose token
+ *                            context is a prefix of a LATER timeline of the same episode is absorbed;
+ *                            the survivors carry the OR of the LLM loss masks (eq. (1))
+ *                            and an index map back to the original timelines.
+ *   ajt_policy_loss_fwd_bwd  "policy gradient ... loss terms are computed" (§4.2 step 4),
+ *                            "GRPO-style policy-gradient updates", clip_ratio 0.2
+ *                            (PAPER.md:531).  The formula is BASELINE.json north_star's: fused online
+ *                            log-softmax over V, target gather, importance ratio vs old log-probs,
+ *                            PPO/GRPO clip, masked per-trajectory mean; forward value and gradient
+ *                            w.r.t. the logits, written in bf16 (DESIGN.md "O-L" steps 1-7).
+ *
+ * Conventions (all calls)
+ *   - Plain pointers and sizes; no C++ or framework types.  Pointers marked DEVICE are CUDA device
+ *     memory owned by the caller; the library allocates nothing and frees nothing.
+ *   - Calls enqueue work on `stream` and return WITHOUT synchronising.  The return value reports
+ *     host-detectable errors only (AJT_ERR_*).  Data-dependent faults set bits in a device status
+ *     word inside the workspace (AJT_STATUS_*), read back with ajt_last_status(); outputs are then
+ *     unspecified.  No exceptions, no abort(), no global state; thread-safe for distinct workspaces.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns AJT_ERR_CUDA.
+ *   - The *_host variants take HOST buffers, stage them through a caller-provided device arena with
+ *     cudaMemcpyAsync on `stream`, run the same kernels and copy the results back; they synchronise
+ *     the stream before returning.
+ */
+#ifndef AJT_H_
+#define AJT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct CUstream_st* ajt_stream_t; /* cudaStream_t */
+
+enum {
+    AJT_OK = 0,
+    AJT_ERR_INVALID_ARG = -1,
+    AJT_ERR_WORKSPACE_TOO_SMALL = -2,
+    AJT_ERR_CAPACITY = -3,
+    AJT_ERR_CUDA = -4,
+    AJT_ERR_UNSUPPORTED = -5
+};
+
+/* Owner rule (reading M-3). */
+enum {
+    AJT_OWNER_LONGEST = 0, /* BASELINE.json north_star: longest surviving extender, then lowest index */
+    AJT_OWNER_PAPER = 1    /* Algorithm 1 literally: the latest extender */
+};
+
+enum { AJT_DT_BF16 = 0, AJT_DT_F32 = 1 };
+
+/* ajt_merge_timelines `flags` */
+enum {
+    AJT_MERGE_WEAK_HASH = 1 /* test hook: degrade the prefix hash to 4 bits so that hash-equal,
+                               token-different candidates are common and the exact-verification /
+                               repair path is exercised.  Results are still exact. */
+};
+
+/* Device status bits (ajt_last_status). */
+enum {
+    AJT_STATUS_BAD_TARGET = 1,       /* targets[t] outside [0,V) on a masked-in row */
+    AJT_STATUS_BAD_SEG = 2,          /* seg_ids[t] outside [0,S) on a masked-in row */
+    AJT_STATUS_BAD_OFFSETS = 4,      /* offsets[0] != 0, decreasing, or offsets[n] != n_tokens */
+    AJT_STATUS_ZERO_LEN = 8,         /* a timeline of length 0 (L_j >= 1 required) */
+    AJT_STATUS_PROBE_CAPACITY = 16,  /* more candidate (timeline, earlier-length) pairs than the workspace holds */
+    AJT_STATUS_HASH_COLLISION = 32,  /* informational: a hash-equal candidate failed exact verification and the
+                                        exact repair path produced the outputs (they are still exact) */
+    AJT_STATUS_INTERNAL = 64
+};
+
+int ajt_version(void);                /* major*10000 + minor*100 + patch */
+const char* ajt_strerror(int code);   /* static string for an AJT_ERR_* code */
+
+/* Synchronises `stream`, copies the status word of `workspace` (DEVICE) to *bits.  Returns AJT_OK or AJT_ERR_CUDA. */
+int ajt_last_status(const void* workspace, ajt_stream_t stream, uint32_t* bits);
+
+/* ------------------------------------------------------------------------------------------------
+ * Stage (a): timeline merging.  Algorithm 1; definition restated in DESIGN.md "O-M".
+ *
+ *   i extends j  <=>  traj_ids[i]==traj_ids[j], i>j, L_i>=L_j, tokens_i[0:L_j]==tokens_j
+ *   j survives   <=>  no i extends j; survivors are numbered m=0..M-1 in ascending original index
+ *   owner_tl(j)  =    j if it survives; else per `owner_rule` among the (surviving) extenders of j
+ *   merged seq m =    the survivor's tokens; mask = OR of member masks; src / old_logp from the largest
+ *                     member index whose mask is 1 at that position (Alg. 1 lines 10-17)
+ *
+ * Workspace: ajt_merge_workspace_bytes(n, n_tokens) bytes of DEVICE memory, 256-byte aligned.  It sizes
+ * room for 64*n + 4096 candidate pairs; a batch whose groups are so large that sum_g k_g(k_g+1)/2 exceeds
+ * that sets AJT_STATUS_PROBE_CAPACITY — pass a larger workspace (every extra 32 bytes hold one more pair).
+ *
+ * All integer; outputs are bit-exact with the definition.  Only the first N_out / M entries of the
+ * outputs are written.  `counts` is DEVICE memory: synchronise the stream before reading it.
+ */
+size_t ajt_merge_workspace_bytes(int32_t n, int64_t n_tokens);
+
+int ajt_merge_timelines(
+    /* inputs, DEVICE, read-only */
+    const int32_t* tokens,      /* [n_tokens] packed token ids (opaque 32-bit patterns, compared bitwise) */
+    const int64_t* offsets,     /* [n+1] offsets[0]=0, strictly increasing, offsets[n]=n_tokens */
+    const int32_t* traj_ids,    /* [n] opaque group keys; need not be contiguous or sorted */
+    const int32_t* resp_start,  /* [n] mask_j[p] = (p >= resp_start[j]); may be NULL if mask_in is given */
+    const uint8_t* mask_in,     /* [n_tokens] explicit per-token 0/1 mask, or NULL -> use resp_start */
+    const float* old_logp_in,   /* [n_tokens] per-token log-probs carried on the timelines, or NULL */
+    int32_t n, int64_t n_tokens, int32_t owner_rule, uint32_t flags,
+    /* outputs, DEVICE, caller-allocated with worst-case capacity (n_tokens tokens, n sequences) */
+    int32_t* merged_tokens,     /* [N_out] */
+    uint8_t* merged_mask,       /* [N_out] */
+    int32_t* merged_src,        /* [N_out] original timeline index supplying mask/logp here, -1 if mask 0 */
+    float* merged_old_logp,     /* [N_out], or NULL (must be NULL iff old_logp_in is NULL) */
+    int64_t* merged_offsets,    /* [M+1] */
+    int32_t* merged_origin,     /* [M] original index of the surviving timeline */
+    int32_t* merged_traj,       /* [M] its traj_id */
+    int32_t* owner,             /* [n] merged-sequence index m whose first L_j tokens are timeline j */
+    int64_t* counts,            /* [2] {M, N_out} */
+    void* workspace, size_t workspace_bytes, ajt_stream_t stream);
+
+/* HOST-buffer variant: same arguments but every array pointer is HOST memory (pinned for speed).
+ * `arena` is DEVICE scratch of at least ajt_merge_host_arena_bytes(n, n_tokens) bytes.  Synchronises. */
+size_t ajt_merge_host_arena_bytes(int32_t n, int64_t n_tokens);
+
+int ajt_merge_timelines_host(
+    const int32_t* tokens, const int64_t* offsets, const int32_t* traj_ids, const int32_t* resp_start,
+    const uint8_t* mask_in, const float* old_logp_in, int32_t n, int64_t n_tokens, int32_t owner_rule,
+    uint32_t flags, int32_t* merged_tokens, uint8_t* merged_mask, int32_t* merged_src, float* merged_old_logp,
+    int64_t* merged_offsets, int32_t* merged_origin, int32_t* merged_traj, int32_t* owner,
+    int64_t* counts /* HOST [2] */, uint32_t* status_bits /* HOST [1] or NULL */,
+    void* arena /* DEVICE */, size_t arena_bytes, ajt_stream_t stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Stage (b): token-level clipped policy-gradient loss, forward and backward w.r.t. the logits.
+ * Definition, for t in [0,T):
+ *   lse_t = log sum_v exp(z_tv);  logp_t = z_{t,y_t} - lse_t;  r_t = exp(logp_t - old_logp_t)
+ *   L_t   = -min(r_t A_t, clip(r_t, 1-eps_lo, 1+eps_hi) A_t)
+ *   N_s   = sum_{t: seg_t = s} mask_t  (or seg_denom[s]);  S' = #{s: N_s > 0}  (or 1/inv_num_segs)
+ *   w_t   = mask_t / (N_{seg_t} S');   loss = sum_t w_t L_t
+ *   g_t   = grad_scale w_t (-A_t r_t) [not (A_t>0 and r_t>1+eps_hi)] [not (A_t<0 and r_t<1-eps_lo)]
+ *   dlogits_tv = g_t (1[v = y_t] - exp(z_tv - lse_t))      stored as bf16, round-to-nearest-even
+ * Rows with mask_t = 0 are not read; their dlogits rows are written as zeros.
+ *
+ * Arithmetic: fp32 on chip, the scalar loss accumulated in fp64 in a fixed order (bitwise reproducible).
+ * Fast path (one HBM read of each unmasked row, one write of every row): bf16 logits, V % 8 == 0,
+ * ld_logits % 8 == 0, 16-byte aligned base pointers, V <= 155648.  Everything else (fp32 logits, odd V,
+ * larger V) takes a slower generic kernel with the same results.
+ *
+ * `dlogits` may alias `logits` when logits_dtype is AJT_DT_BF16 (in-place backward).
+ * Workspace: ajt_loss_workspace_bytes(T, V, S) bytes of DEVICE memory, 256-byte aligned.
+ */
+size_t ajt_loss_workspace_bytes(int64_t T, int32_t V, int32_t S);
+
+int ajt_policy_loss_fwd_bwd(
+    const void* logits,         /* DEVICE [T, ld_logits] row-major, logits_dtype; columns [0,V) are used */
+    const int32_t* targets,     /* DEVICE [T] in [0,V) */
+    const float* old_logp,      /* DEVICE [T] */
+    const float* adv,           /* DEVICE [T] per-token advantage */
+    const uint8_t* mask,        /* DEVICE [T] 0/1 */
+    const int32_t* seg_ids,     /* DEVICE [T] in [0,S): trajectory of each token */
+    float eps_lo, float eps_hi,
+    int64_t T, int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype,
+    const float* seg_denom,     /* DEVICE [S] or NULL: override N_s (chunked streaming, reading L-4) */
+    float inv_num_segs,         /* 0 -> compute 1/S' from this call's tokens; else used as given */
+    float grad_scale,           /* upstream dLoss, normally 1.0f */
+    void* dlogits,              /* DEVICE [T, ld_logits] bf16 */
+    float* loss_out,            /* DEVICE [1]: this call's sum_t w_t L_t (the caller sums chunks) */
+    float* logp_out,            /* DEVICE [T] or NULL: logp_t where mask_t = 1, 0 elsewhere */
+    float* stats_out,           /* DEVICE [4] or NULL: {n_masked, n_clipped_hi, n_clipped_lo, sum_t w_t (-log r_t)} */
+    void* workspace, size_t workspace_bytes, ajt_stream_t stream);
+
+/* HOST-buffer variant.  `arena` is DEVICE scratch of at least ajt_loss_host_arena_bytes(T, V, S, ld, dtype)
+ * bytes.  Rows are staged in slabs so that H2D, compute and D2H overlap.  Synchronises. */
+size_t ajt_loss_host_arena_bytes(int64_t T, int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype);
+
+int ajt_policy_loss_fwd_bwd_host(
+    const void* logits, const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
+    const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T, int32_t V, int32_t S, int64_t ld_logits,
+    int32_t logits_dtype, const float* seg_denom, float inv_num_segs, float grad_scale,
+    void* dlogits /* HOST bf16 */, float* loss_out /* HOST [1] */, float* logp_out /* HOST [T] or NULL */,
+    float* stats_out /* HOST [4] or NULL */, uint32_t* status_bits /* HOST [1] or NULL */,
+    void* arena /* DEVICE */, size_t arena_bytes, ajt_stream_t stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AJT_H_ */

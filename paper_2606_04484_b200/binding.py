@@ -1,0 +1,311 @@
+"""ctypes binding of libajt.so: argument marshalling only (include/ajt.h is the contract).
+
+torch is used for device memory and streams; numpy / pinned torch tensors for the *_host variants.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libajt.so")
+
+OWNER_LONGEST, OWNER_PAPER = 0, 1
+DT_BF16, DT_F32 = 0, 1
+MERGE_WEAK_HASH = 1
+STATUS_BAD_TARGET, STATUS_BAD_SEG, STATUS_BAD_OFFSETS, STATUS_ZERO_LEN = 1, 2, 4, 8
+STATUS_PROBE_CAPACITY, STATUS_HASH_COLLISION, STATUS_INTERNAL = 16, 32, 64
+
+_EXPORTS = [
+    "ajt_version", "ajt_strerror", "ajt_last_status",
+    "ajt_merge_workspace_bytes", "ajt_merge_timelines", "ajt_merge_host_arena_bytes", "ajt_merge_timelines_host",
+    "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
+]
+
+_lib = None
+
+
+class AjtError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {strerror(code)} (code {code})")
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def exported_symbols():
+    return list(_EXPORTS)
+
+
+def lib():
+    """Loads libajt.so.  Fails loudly when it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError(f"{_LIB_PATH} is missing: build it with `python -m paper_2606_04484_b200.build` "
+                               "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(_LIB_PATH)
+        L.ajt_version.restype = C.c_int
+        L.ajt_strerror.restype = C.c_char_p
+        L.ajt_strerror.argtypes = [C.c_int]
+        L.ajt_last_status.restype = C.c_int
+        for f in ("ajt_merge_workspace_bytes", "ajt_merge_host_arena_bytes"):
+            getattr(L, f).restype = C.c_size_t
+            getattr(L, f).argtypes = [C.c_int32, C.c_int64]
+        L.ajt_loss_workspace_bytes.restype = C.c_size_t
+        L.ajt_loss_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
+        L.ajt_loss_host_arena_bytes.restype = C.c_size_t
+        L.ajt_loss_host_arena_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32]
+        for f in ("ajt_merge_timelines", "ajt_merge_timelines_host", "ajt_policy_loss_fwd_bwd",
+                  "ajt_policy_loss_fwd_bwd_host"):
+            getattr(L, f).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def version() -> int:
+    return int(lib().ajt_version())
+
+
+def strerror(code: int) -> str:
+    return lib().ajt_strerror(int(code)).decode()
+
+
+def merge_workspace_bytes(n: int, n_tokens: int) -> int:
+    return int(lib().ajt_merge_workspace_bytes(n, n_tokens))
+
+
+def merge_host_arena_bytes(n: int, n_tokens: int) -> int:
+    return int(lib().ajt_merge_host_arena_bytes(n, n_tokens))
+
+
+def loss_workspace_bytes(T: int, V: int, S: int) -> int:
+    return int(lib().ajt_loss_workspace_bytes(T, V, S))
+
+
+def loss_host_arena_bytes(T: int, V: int, S: int, ld: int, dtype: int) -> int:
+    return int(lib().ajt_loss_host_arena_bytes(T, V, S, ld, dtype))
+
+
+def _dp(t: Optional[torch.Tensor]):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _hp(a):
+    if a is None:
+        return None
+    if isinstance(a, torch.Tensor):
+        return C.c_void_p(a.data_ptr())
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _stream(stream: Optional[torch.cuda.Stream] = None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _check_dev(t: Optional[torch.Tensor], dtype, name: str):
+    if t is None:
+        return
+    if not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous CUDA tensor of {dtype}, got {t.dtype} on {t.device}")
+
+
+def _require_cuda():
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2606_04484_b200: no CUDA device; the hot path has no CPU fallback")
+
+
+def last_status(workspace: torch.Tensor, stream=None) -> int:
+    bits = C.c_uint32(0)
+    rc = lib().ajt_last_status(_dp(workspace), _stream(stream), C.byref(bits))
+    if rc != 0:
+        raise AjtError(rc, "ajt_last_status")
+    return int(bits.value)
+
+
+# ------------------------------------------------------------------------------------------- merge
+
+
+@dataclass
+class MergeOutput:
+    """Device tensors at worst-case capacity; only the first N_out / M entries are defined.  `finalize()`
+    synchronises, reads `counts` and returns views of the right length."""
+    merged_tokens: torch.Tensor
+    merged_mask: torch.Tensor
+    merged_src: torch.Tensor
+    merged_old_logp: Optional[torch.Tensor]
+    merged_offsets: torch.Tensor
+    merged_origin: torch.Tensor
+    merged_traj: torch.Tensor
+    owner: torch.Tensor
+    counts: torch.Tensor
+    workspace: torch.Tensor
+    M: int = -1
+    N_out: int = -1
+
+    def finalize(self) -> "MergeOutput":
+        c = self.counts.cpu()
+        M, No = int(c[0]), int(c[1])
+        return MergeOutput(self.merged_tokens[:No], self.merged_mask[:No], self.merged_src[:No],
+                           None if self.merged_old_logp is None else self.merged_old_logp[:No],
+                           self.merged_offsets[:M + 1], self.merged_origin[:M], self.merged_traj[:M], self.owner,
+                           self.counts, self.workspace, M, No)
+
+
+def merge_timelines(tokens: torch.Tensor, offsets: torch.Tensor, traj_ids: torch.Tensor,
+                    resp_start: Optional[torch.Tensor] = None, mask_in: Optional[torch.Tensor] = None,
+                    old_logp_in: Optional[torch.Tensor] = None, owner_rule: int = OWNER_LONGEST, flags: int = 0,
+                    out: Optional[MergeOutput] = None, workspace_bytes: Optional[int] = None,
+                    stream=None) -> MergeOutput:
+    """ajt_merge_timelines (include/ajt.h).  All tensors live on the current CUDA device."""
+    _require_cuda()
+    _check_dev(tokens, torch.int32, "tokens")
+    _check_dev(offsets, torch.int64, "offsets")
+    _check_dev(traj_ids, torch.int32, "traj_ids")
+    _check_dev(resp_start, torch.int32, "resp_start")
+    _check_dev(mask_in, torch.uint8, "mask_in")
+    _check_dev(old_logp_in, torch.float32, "old_logp_in")
+    n, N = int(traj_ids.numel()), int(tokens.numel())
+    dev = tokens.device
+    if out is None:
+        wsb = merge_workspace_bytes(n, N) if workspace_bytes is None else int(workspace_bytes)
+        out = MergeOutput(
+            torch.empty(max(N, 1), dtype=torch.int32, device=dev), torch.empty(max(N, 1), dtype=torch.uint8, device=dev),
+            torch.empty(max(N, 1), dtype=torch.int32, device=dev),
+            None if old_logp_in is None else torch.empty(max(N, 1), dtype=torch.float32, device=dev),
+            torch.empty(n + 1, dtype=torch.int64, device=dev), torch.empty(max(n, 1), dtype=torch.int32, device=dev),
+            torch.empty(max(n, 1), dtype=torch.int32, device=dev), torch.empty(max(n, 1), dtype=torch.int32, device=dev),
+            torch.empty(2, dtype=torch.int64, device=dev), torch.empty(wsb, dtype=torch.uint8, device=dev))
+    rc = lib().ajt_merge_timelines(
+        _dp(tokens), _dp(offsets), _dp(traj_ids), _dp(resp_start), _dp(mask_in), _dp(old_logp_in),
+        C.c_int32(n), C.c_int64(N), C.c_int32(owner_rule), C.c_uint32(flags),
+        _dp(out.merged_tokens), _dp(out.merged_mask), _dp(out.merged_src), _dp(out.merged_old_logp),
+        _dp(out.merged_offsets), _dp(out.merged_origin), _dp(out.merged_traj), _dp(out.owner), _dp(out.counts),
+        _dp(out.workspace), C.c_size_t(out.workspace.numel()), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_merge_timelines")
+    return out
+
+
+def merge_timelines_host(tokens, offsets, traj_ids, resp_start=None, mask_in=None, old_logp_in=None,
+                         owner_rule: int = OWNER_LONGEST, flags: int = 0, arena: Optional[torch.Tensor] = None,
+                         out: Optional[dict] = None, stream=None) -> dict:
+    """ajt_merge_timelines_host: HOST buffers (numpy arrays or CPU torch tensors, pinned for speed)."""
+    _require_cuda()
+    n, N = int(len(traj_ids)), int(len(tokens))
+    if arena is None:
+        arena = torch.empty(merge_host_arena_bytes(n, N), dtype=torch.uint8, device="cuda")
+    if out is None:
+        pin = dict(pin_memory=True)
+        out = dict(merged_tokens=torch.empty(max(N, 1), dtype=torch.int32, **pin),
+                   merged_mask=torch.empty(max(N, 1), dtype=torch.uint8, **pin),
+                   merged_src=torch.empty(max(N, 1), dtype=torch.int32, **pin),
+                   merged_old_logp=None if old_logp_in is None else torch.empty(max(N, 1), dtype=torch.float32, **pin),
+                   merged_offsets=torch.empty(n + 1, dtype=torch.int64, **pin),
+                   merged_origin=torch.empty(max(n, 1), dtype=torch.int32, **pin),
+                   merged_traj=torch.empty(max(n, 1), dtype=torch.int32, **pin),
+                   owner=torch.empty(max(n, 1), dtype=torch.int32, **pin))
+    counts = np.zeros(2, np.int64)
+    status = C.c_uint32(0)
+    rc = lib().ajt_merge_timelines_host(
+        _hp(tokens), _hp(offsets), _hp(traj_ids), _hp(resp_start), _hp(mask_in), _hp(old_logp_in),
+        C.c_int32(n), C.c_int64(N), C.c_int32(owner_rule), C.c_uint32(flags),
+        _hp(out["merged_tokens"]), _hp(out["merged_mask"]), _hp(out["merged_src"]), _hp(out["merged_old_logp"]),
+        _hp(out["merged_offsets"]), _hp(out["merged_origin"]), _hp(out["merged_traj"]), _hp(out["owner"]),
+        _hp(counts), C.byref(status), _dp(arena), C.c_size_t(arena.numel()), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_merge_timelines_host")
+    out = dict(out)
+    out["M"], out["N_out"], out["status"] = int(counts[0]), int(counts[1]), int(status.value)
+    return out
+
+
+# ------------------------------------------------------------------------------------------- loss
+
+
+@dataclass
+class LossOutput:
+    dlogits: torch.Tensor            # bf16 [T, ld]
+    loss: torch.Tensor               # f32 [1] (device)
+    logp: Optional[torch.Tensor]     # f32 [T]
+    stats: Optional[torch.Tensor]    # f32 [4]
+    workspace: torch.Tensor
+
+
+def policy_loss_fwd_bwd(logits: torch.Tensor, targets: torch.Tensor, old_logp: torch.Tensor, adv: torch.Tensor,
+                        mask: torch.Tensor, seg_ids: torch.Tensor, S: int, eps_lo: float, eps_hi: float,
+                        seg_denom: Optional[torch.Tensor] = None, inv_num_segs: float = 0.0, grad_scale: float = 1.0,
+                        V: Optional[int] = None, dlogits: Optional[torch.Tensor] = None, want_logp: bool = False,
+                        want_stats: bool = False, out: Optional[LossOutput] = None, stream=None) -> LossOutput:
+    """ajt_policy_loss_fwd_bwd (include/ajt.h).  logits: CUDA [T, ld] bf16 or f32; V defaults to ld.
+    Pass dlogits=logits (bf16) for the in-place backward."""
+    _require_cuda()
+    if logits.dim() != 2 or not logits.is_cuda or logits.stride(1) != 1:
+        raise TypeError("logits: expected a 2-D CUDA tensor with unit column stride")
+    if logits.dtype == torch.bfloat16:
+        dt = DT_BF16
+    elif logits.dtype == torch.float32:
+        dt = DT_F32
+    else:
+        raise TypeError("logits: bf16 or f32 only")
+    T, ld = int(logits.shape[0]), int(logits.stride(0)) if logits.shape[0] > 1 else int(logits.shape[1])
+    V = int(logits.shape[1]) if V is None else int(V)
+    _check_dev(targets, torch.int32, "targets")
+    _check_dev(old_logp, torch.float32, "old_logp")
+    _check_dev(adv, torch.float32, "adv")
+    _check_dev(mask, torch.uint8, "mask")
+    _check_dev(seg_ids, torch.int32, "seg_ids")
+    _check_dev(seg_denom, torch.float32, "seg_denom")
+    dev = logits.device
+    if out is None:
+        if dlogits is None:
+            dlogits = torch.empty((T, ld), dtype=torch.bfloat16, device=dev)
+        out = LossOutput(dlogits, torch.empty(1, dtype=torch.float32, device=dev),
+                         torch.empty(max(T, 1), dtype=torch.float32, device=dev) if want_logp else None,
+                         torch.empty(4, dtype=torch.float32, device=dev) if want_stats else None,
+                         torch.empty(loss_workspace_bytes(T, V, S), dtype=torch.uint8, device=dev))
+    if out.dlogits.dtype != torch.bfloat16 or not out.dlogits.is_cuda:
+        raise TypeError("dlogits: expected a CUDA bf16 tensor")
+    rc = lib().ajt_policy_loss_fwd_bwd(
+        _dp(logits), _dp(targets), _dp(old_logp), _dp(adv), _dp(mask), _dp(seg_ids),
+        C.c_float(eps_lo), C.c_float(eps_hi), C.c_int64(T), C.c_int32(V), C.c_int32(S), C.c_int64(ld), C.c_int32(dt),
+        _dp(seg_denom), C.c_float(inv_num_segs), C.c_float(grad_scale), _dp(out.dlogits), _dp(out.loss), _dp(out.logp),
+        _dp(out.stats), _dp(out.workspace), C.c_size_t(out.workspace.numel()), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_policy_loss_fwd_bwd")
+    return out
+
+
+def policy_loss_fwd_bwd_host(logits, targets, old_logp, adv, mask, seg_ids, S: int, eps_lo: float, eps_hi: float,
+                             dtype: int, V: Optional[int] = None, seg_denom=None, inv_num_segs: float = 0.0,
+                             grad_scale: float = 1.0, dlogits=None, want_logp: bool = False, want_stats: bool = False,
+                             arena: Optional[torch.Tensor] = None, stream=None) -> dict:
+    """ajt_policy_loss_fwd_bwd_host: HOST buffers.  logits: [T, ld] CPU tensor (bf16 / f32) or numpy
+    (uint16 bit patterns for bf16 / float32)."""
+    _require_cuda()
+    T, ld = int(logits.shape[0]), int(logits.shape[1])
+    V = ld if V is None else int(V)
+    if arena is None:
+        arena = torch.empty(loss_host_arena_bytes(T, V, S, ld, dtype), dtype=torch.uint8, device="cuda")
+    if dlogits is None:
+        dlogits = torch.empty((T, ld), dtype=torch.bfloat16, pin_memory=True)
+    loss = np.zeros(1, np.float32)
+    logp = np.zeros(max(T, 1), np.float32) if want_logp else None
+    stats = np.zeros(4, np.float32) if want_stats else None
+    status = C.c_uint32(0)
+    rc = lib().ajt_policy_loss_fwd_bwd_host(
+        _hp(logits), _hp(targets), _hp(old_logp), _hp(adv), _hp(mask), _hp(seg_ids), C.c_float(eps_lo), C.c_float(eps_hi),
+        C.c_int64(T), C.c_int32(V), C.c_int32(S), C.c_int64(ld), C.c_int32(dtype), _hp(seg_denom), C.c_float(inv_num_segs),
+        C.c_float(grad_scale), _hp(dlogits), _hp(loss), _hp(logp), _hp(stats), C.byref(status), _dp(arena),
+        C.c_size_t(arena.numel()), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_policy_loss_fwd_bwd_host")
+    return dict(dlogits=dlogits, loss=float(loss[0]), logp=logp, stats=stats, status=int(status.value))

@@ -1,0 +1,614 @@
+// Stage (b): token-level clipped policy-gradient loss, forward + backward w.r.t. logits (sm_100a).
+//
+// What is computed: DESIGN.md "O-L" steps 1-7 (BASELINE.json north_star).
+// Kernels:
+//   K6  loss_prep_kernel   per-segment mask counts N_s, 1/S', and the compacted lists of rows to read
+//                          (mask=1) and rows to zero-fill (mask=0)                          [L0]
+//   K7  loss_rows_kernel   the HBM-bound row kernel: each unmasked [V] row is pulled ONCE from HBM by
+//                          1-D TMA bulk copies into a shared-memory ring, parked in registers as packed
+//                          bf16, reduced (max, sum-exp), turned into dlogits and stored ONCE.  A row of
+//                          V=151936 bf16 (304 KB) does not fit one SM, so a 2-CTA cluster holds half a
+//                          row each and exchanges the 16+16 warp partials over DSMEM (st.async +
+//                          mbarrier complete_tx).  Masked rows are zero-filled by the producer warp with
+//                          bulk stores from a zeroed shared buffer, overlapping the math.      [L1-L3]
+//       loss_rows_generic  fallback for fp32 logits / odd V / unaligned / huge V (3 reads via L1/L2).
+//   K8  loss_final_kernel  fixed-order fp64 reduction of the per-row terms -> loss, stats      [L4]
+#include <math.h>
+
+#include "ajt_common.cuh"
+
+namespace {
+
+using namespace ajt;
+
+// 19 consumer warps + 1 producer warp = 20 warps: registers are allocated per 4 warps, so 20 warps x 96
+// registers fill the 64K register file exactly; 64 of the 96 hold the row slice (16 x uint4).
+constexpr int kConsWarps = 19;
+constexpr int kConsumers = kConsWarps * 32;      // 608 consumer threads
+constexpr int kThreads = kConsumers + 32;        // + 1 producer warp = 640
+constexpr int kChunkElems = kConsumers * 8;      // 4864 bf16 per chunk: one 16-byte vector per consumer thread
+constexpr int kChunkBytes = kChunkElems * 2;     // 9728 B
+constexpr int kSlots = 20;                       // 190 KB ring
+constexpr int kMaxCluster = 2;
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr uint32_t kNegInf2 = 0xFF80FF80u;       // packed bf16 (-inf, -inf)
+
+constexpr size_t kRowsSmemBytes = (size_t)kSlots * kChunkBytes + kChunkBytes /* zero buffer */ +
+                                  (2 * kSlots + 2) * sizeof(uint64_t) + 2 * kConsWarps * kMaxCluster * sizeof(float2);
+
+struct LossParams {
+    const void* logits;
+    const int32_t* targets;
+    const float* old_logp;
+    const float* adv;
+    const uint8_t* mask;
+    const int32_t* seg_ids;
+    float eps_lo, eps_hi;
+    int64_t T;
+    int32_t V, S;
+    int64_t ld;
+    int32_t dtype;
+    const float* seg_denom;
+    float inv_num_segs, grad_scale;
+    void* dlogits;
+    float* loss_out;
+    float* logp_out;
+    float* stats_out;
+    // workspace
+    AjtCtrl* ctrl;
+    int32_t* seg_cnt;      // [S]
+    int32_t* list_active;  // [T] rows with mask = 1, ascending
+    int32_t* list_zero;    // [T] rows with mask = 0, ascending
+    double* row_val;       // [T] w_t L_t by compact index
+    double* row_kl;        // [T] w_t (-log r_t) by compact index
+    uint8_t* row_clip;     // [T] bit0 clipped high, bit1 clipped low
+};
+
+struct LossWs {
+    size_t ctrl, seg_cnt, list_active, list_zero, row_val, row_kl, row_clip, total;
+};
+
+__host__ inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+__host__ LossWs loss_ws_layout(int64_t T, int32_t S) {
+    LossWs w;
+    size_t o = 0;
+    w.ctrl = o; o += align256(sizeof(AjtCtrl));
+    w.seg_cnt = o; o += align256((size_t)S * 4);
+    w.list_active = o; o += align256((size_t)T * 4);
+    w.list_zero = o; o += align256((size_t)T * 4);
+    w.row_val = o; o += align256((size_t)T * 8);
+    w.row_kl = o; o += align256((size_t)T * 8);
+    w.row_clip = o; o += align256((size_t)T);
+    w.total = o;
+    return w;
+}
+
+// ------------------------------------------------------------------------------------------------ K6
+
+__global__ void __launch_bounds__(1024) loss_prep_kernel(const LossParams p) {
+    __shared__ int s_cnt[2][2][32];
+    __shared__ int s_live[32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int s = tid; s < p.S; s += 1024) p.seg_cnt[s] = 0;
+    __syncthreads();
+    int base_a = 0, base_z = 0;
+    int buf = 0;
+    for (int64_t t0 = 0; t0 < p.T; t0 += 1024, buf ^= 1) {
+        const int64_t t = t0 + tid;
+        const bool in = t < p.T;
+        bool act = in && p.mask[t] != 0;
+        int sg = act ? p.seg_ids[t] : 0;
+        if (act && (unsigned)sg >= (unsigned)p.S) {
+            atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_BAD_SEG);
+            act = false;  // treated as a masked-out row
+        }
+        // N_s: warp-aggregated atomics (segments are contiguous runs, so lanes mostly share one id)
+        const int key = act ? sg : -1 - lane;
+        const unsigned peers = __match_any_sync(0xffffffffu, key);
+        if (act && lane == __ffs(peers) - 1) atomicAdd(&p.seg_cnt[sg], __popc(peers));
+        // stable compaction into the two row lists
+        const unsigned ba = __ballot_sync(0xffffffffu, act);
+        const unsigned bz = __ballot_sync(0xffffffffu, in && !act);
+        if (lane == 0) {
+            s_cnt[buf][0][warp] = __popc(ba);
+            s_cnt[buf][1][warp] = __popc(bz);
+        }
+        __syncthreads();
+        int pa = 0, pz = 0, ta = 0, tz = 0;
+#pragma unroll
+        for (int w = 0; w < 32; ++w) {
+            const int ca = s_cnt[buf][0][w], cz = s_cnt[buf][1][w];
+            if (w < warp) { pa += ca; pz += cz; }
+            ta += ca; tz += cz;
+        }
+        const unsigned lt = (1u << lane) - 1u;
+        if (act) p.list_active[base_a + pa + __popc(ba & lt)] = (int32_t)t;
+        else if (in) p.list_zero[base_z + pz + __popc(bz & lt)] = (int32_t)t;
+        base_a += ta;
+        base_z += tz;
+    }
+    __syncthreads();
+    // S' = #{s : N_s > 0}
+    int live = 0;
+    for (int s = tid; s < p.S; s += 1024) {
+        const float d = p.seg_denom ? p.seg_denom[s] : (float)p.seg_cnt[s];
+        live += d > 0.f;
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) live += __shfl_xor_sync(0xffffffffu, live, o);
+    if (lane == 0) s_live[warp] = live;
+    __syncthreads();
+    if (tid == 0) {
+        int tot = 0;
+        for (int w = 0; w < 32; ++w) tot += s_live[w];
+        p.ctrl->n_active = base_a;
+        p.ctrl->n_zero = base_z;
+        p.ctrl->n_live_segs = tot;
+        p.ctrl->inv_num_segs = p.inv_num_segs != 0.f ? p.inv_num_segs : (tot > 0 ? 1.0f / (float)tot : 0.f);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ L2
+
+struct TokScalars {
+    float g;       // d(w L)/d logp * grad_scale
+    float logp;
+    float lse;
+    double wl;     // w * L
+    double wkl;    // w * (-(logp - old))
+    int clip;      // bit0 high, bit1 low
+};
+
+// M = max_v z, S = sum_v exp(z_v - M) (so 1 <= S <= V), zy = z[y].  DESIGN.md O-L steps 1-6.
+__device__ __forceinline__ TokScalars token_scalars(float M, float S, float zy, float old, float A, float w,
+                                                    float eps_lo, float eps_hi, float grad_scale) {
+    TokScalars o;
+    const float logS = logf(S);
+    o.lse = M + logS;
+    // (zy - M) is exact for bf16 inputs; subtracting the O(1) terms first keeps the log-ratio's error ~2e-7
+    const float zm = zy - M;
+    o.logp = zm - logS;
+    const float d = (zm - old) - logS;       // logp - old_logp
+    const float r = expf(d);
+    const bool hi = (A > 0.f) && (r > 1.f + eps_hi);
+    const bool lo = (A < 0.f) && (r < 1.f - eps_lo);
+    const float rc = fminf(fmaxf(r, 1.f - eps_lo), 1.f + eps_hi);
+    const float L = -fminf(r * A, rc * A);
+    o.g = (hi || lo) ? 0.f : grad_scale * w * (-A * r);
+    o.wl = (double)w * (double)L;
+    o.wkl = (double)w * (-(double)d);
+    o.clip = (hi ? 1 : 0) | (lo ? 2 : 0);
+    return o;
+}
+
+// ------------------------------------------------------------------------------------------------ K7 (fast)
+
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ float exp_diff(float m, float M) {  // exp(m - M), 0 when m = -inf
+    return m == -INFINITY ? 0.f : ex2((m - M) * kLog2e);
+}
+
+template <int NCH, int CSIZE>
+__global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams p) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* ring = smem;
+    uint8_t* zbuf = smem + (size_t)kSlots * kChunkBytes;
+    uint64_t* full = reinterpret_cast<uint64_t*>(zbuf + kChunkBytes);
+    uint64_t* empty = full + kSlots;
+    uint64_t* pbar = empty + kSlots;
+    float2* part = reinterpret_cast<float2*>(pbar + 2);  // [2][kConsWarps * CSIZE]
+    constexpr int kParts = kConsWarps * CSIZE;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t rank = CSIZE > 1 ? cluster_ctarank() : 0u;
+    const int cid = blockIdx.x / CSIZE, NC = gridDim.x / CSIZE;
+
+    // the slice of the vocabulary this CTA owns: 8-element (16-byte) granularity
+    const int V = p.V;
+    const int h = CSIZE == 1 ? V : (((V + CSIZE - 1) / CSIZE + 7) & ~7);
+    const int sl_begin = (int)rank * h;
+    const int sl_len = max(0, min(h, V - sl_begin));
+    const int nch = (sl_len + kChunkElems - 1) / kChunkElems;
+
+    if (tid == 0) {
+        for (int i = 0; i < kSlots; ++i) {
+            mbar_init(&full[i], 1);
+            mbar_init(&empty[i], kConsWarps);
+        }
+        mbar_init(&pbar[0], kConsWarps);
+        mbar_init(&pbar[1], kConsWarps);
+        fence_mbar_init();
+    }
+    for (int i = tid; i < kChunkBytes / 16; i += kThreads) reinterpret_cast<uint4*>(zbuf)[i] = make_uint4(0, 0, 0, 0);
+    fence_proxy_async_smem();
+    if (CSIZE > 1) cluster_sync_all(); else __syncthreads();
+
+    const int n_active = p.ctrl->n_active, n_zero = p.ctrl->n_zero;
+    const int nrows = n_active > cid ? (n_active - cid + NC - 1) / NC : 0;
+    const __nv_bfloat16* logits = reinterpret_cast<const __nv_bfloat16*>(p.logits);
+    __nv_bfloat16* dlogits = reinterpret_cast<__nv_bfloat16*>(p.dlogits);
+
+    if (warp == kConsWarps) {
+        // ===== producer warp: TMA loads of unmasked rows + bulk zero-fill of masked rows =====
+        if (lane == 0) {
+            const int nzero = n_zero > cid ? (n_zero - cid + NC - 1) / NC : 0;
+            int zdone = 0;
+            auto zero_rows_until = [&](int target) {
+                for (; zdone < target; ++zdone) {
+                    const int64_t row = p.list_zero[cid + (int64_t)zdone * NC];
+                    __nv_bfloat16* dst = dlogits + row * p.ld + sl_begin;
+                    for (int ch = 0; ch < nch; ++ch) {
+                        const uint32_t bytes = (uint32_t)min(kChunkElems, sl_len - ch * kChunkElems) * 2u;
+                        bulk_store(dst + (size_t)ch * kChunkElems, zbuf, bytes);
+                    }
+                    bulk_commit();
+                }
+            };
+            int slot = 0;
+            uint32_t ph = 0;
+            for (int k = 0; k < nrows; ++k) {
+                const int64_t row = p.list_active[cid + (int64_t)k * NC];
+                const __nv_bfloat16* src = logits + row * p.ld + sl_begin;
+                for (int ch = 0; ch < nch; ++ch) {
+                    mbar_wait(&empty[slot], ph ^ 1u);
+                    const uint32_t bytes = (uint32_t)min(kChunkElems, sl_len - ch * kChunkElems) * 2u;
+                    mbar_arrive_expect_tx(&full[slot], bytes);
+                    bulk_load(ring + (size_t)slot * kChunkBytes, src + (size_t)ch * kChunkElems, bytes, &full[slot]);
+                    if (++slot == kSlots) { slot = 0; ph ^= 1u; }
+                }
+                zero_rows_until((int)(((int64_t)(k + 1) * nzero) / nrows));
+            }
+            zero_rows_until(nzero);
+            bulk_wait<0>();
+        }
+    } else {
+        // ===== consumer warps =====
+        const float inv_S = p.ctrl->inv_num_segs;
+        int slot = 0;
+        uint32_t ph = 0;
+        for (int k = 0; k < nrows; ++k) {
+            const int kidx = cid + k * NC;
+            const int64_t row = p.list_active[kidx];
+            const int y = p.targets[row];
+            const float old = p.old_logp[row];
+            const float A = p.adv[row];
+            const int sg = p.seg_ids[row];
+            const float denom = p.seg_denom ? p.seg_denom[sg] : (float)p.seg_cnt[sg];
+            const bool ybad = (unsigned)y >= (unsigned)V;
+            const float w = (denom > 0.f && !ybad) ? inv_S / denom : 0.f;
+            const float zy = ybad ? 0.f : __bfloat162float(logits[row * p.ld + y]);
+
+            // ---- pass 1a: ring -> registers (packed bf16), packed running max
+            uint4 r[NCH];
+            uint32_t mx = kNegInf2;
+#pragma unroll
+            for (int ch = 0; ch < NCH; ++ch) {
+                r[ch] = make_uint4(kNegInf2, kNegInf2, kNegInf2, kNegInf2);
+                if (ch < nch) {
+                    mbar_wait(&full[slot], ph);
+                    if (ch * kChunkElems + tid * 8 < sl_len) r[ch] = lds128(ring + (size_t)slot * kChunkBytes + tid * 16);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&empty[slot]);
+                    if (++slot == kSlots) { slot = 0; ph ^= 1u; }
+                    mx = max_bf16x2(mx, max_bf16x2(max_bf16x2(r[ch].x, r[ch].y), max_bf16x2(r[ch].z, r[ch].w)));
+                }
+            }
+            // ---- pass 1b: thread-local sum of exp(x - m_thread) from registers: one MUFU per element
+            const float m = fmaxf(bf16lo(mx), bf16hi(mx));
+            const float ms = m == -INFINITY ? 0.f : m;
+            float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+#pragma unroll
+            for (int ch = 0; ch < NCH; ++ch) {
+                if (ch < nch) {
+                    s0 += ex2((bf16lo(r[ch].x) - ms) * kLog2e);
+                    s1 += ex2((bf16hi(r[ch].x) - ms) * kLog2e);
+                    s2 += ex2((bf16lo(r[ch].y) - ms) * kLog2e);
+                    s3 += ex2((bf16hi(r[ch].y) - ms) * kLog2e);
+                    s0 += ex2((bf16lo(r[ch].z) - ms) * kLog2e);
+                    s1 += ex2((bf16hi(r[ch].z) - ms) * kLog2e);
+                    s2 += ex2((bf16lo(r[ch].w) - ms) * kLog2e);
+                    s3 += ex2((bf16hi(r[ch].w) - ms) * kLog2e);
+                }
+            }
+            float s = (s0 + s1) + (s2 + s3);
+            // ---- warp partial, published to every CTA of the cluster
+            const float mw = warp_max(m);
+            const float sw = warp_sum(s * exp_diff(m, mw));
+            const int par = k & 1;
+            float2* mypart = part + par * kParts;
+            // z[y] must have landed before the peer can learn our partial and start overwriting the row
+            // (dlogits may alias logits)
+            asm volatile("" ::"f"(zy) : "memory");
+            if (lane == 0) {
+                mypart[rank * kConsWarps + warp] = make_float2(mw, sw);
+                if (CSIZE > 1) {
+                    const uint64_t v = ((uint64_t)__float_as_uint(sw) << 32) | (uint64_t)__float_as_uint(mw);
+                    const uint32_t a = smem_u32(&mypart[rank * kConsWarps + warp]), b = smem_u32(&pbar[par]);
+#pragma unroll
+                    for (uint32_t q = 0; q < (uint32_t)CSIZE; ++q)
+                        if (q != rank) st_async_b64(mapa(a, q), v, mapa(b, q));
+                    if (warp == 0) mbar_arrive_expect_tx(&pbar[par], (uint32_t)((CSIZE - 1) * kConsWarps * 8));
+                    else mbar_arrive(&pbar[par]);
+                } else {
+                    mbar_arrive(&pbar[par]);
+                }
+            }
+            mbar_wait(&pbar[par], (uint32_t)(k >> 1) & 1u);
+            // ---- combine the 16*CSIZE partials (every warp redundantly; 1 MUFU + 10 shuffles)
+            float2 pv = lane < kParts ? mypart[lane] : make_float2(-INFINITY, 0.f);
+            float2 pw = (kParts > 32 && lane + 32 < kParts) ? mypart[lane + 32] : make_float2(-INFINITY, 0.f);
+            const float M = warp_max(fmaxf(pv.x, pw.x));
+            const float S = warp_sum(pv.y * exp_diff(pv.x, M) + pw.y * exp_diff(pw.x, M));
+            const TokScalars ts = token_scalars(M, S, zy, old, A, w, p.eps_lo, p.eps_hi, p.grad_scale);
+            if (tid == 0 && rank == 0) {
+                p.row_val[kidx] = ts.wl;
+                p.row_kl[kidx] = ts.wkl;
+                p.row_clip[kidx] = (uint8_t)(w > 0.f ? ts.clip : 0);
+                if (p.logp_out) p.logp_out[row] = ybad ? 0.f : ts.logp;
+                if (ybad) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_BAD_TARGET);
+            }
+            // ---- pass 2: dlogits = g (1[v=y] - exp(z - lse)), bf16 RNE, one 16-byte store per vector
+            __nv_bfloat16* drow = dlogits + row * p.ld + sl_begin;
+            const float g = ts.g;
+            if (g != 0.f) {
+                const float coef = -g, k2 = -ts.lse * kLog2e;
+#pragma unroll
+                for (int ch = 0; ch < NCH; ++ch) {
+                    if (ch < nch && ch * kChunkElems + tid * 8 < sl_len) {
+                        uint4 o;
+                        o.x = pack_bf16x2(coef * ex2(fmaf(bf16lo(r[ch].x), kLog2e, k2)), coef * ex2(fmaf(bf16hi(r[ch].x), kLog2e, k2)));
+                        o.y = pack_bf16x2(coef * ex2(fmaf(bf16lo(r[ch].y), kLog2e, k2)), coef * ex2(fmaf(bf16hi(r[ch].y), kLog2e, k2)));
+                        o.z = pack_bf16x2(coef * ex2(fmaf(bf16lo(r[ch].z), kLog2e, k2)), coef * ex2(fmaf(bf16hi(r[ch].z), kLog2e, k2)));
+                        o.w = pack_bf16x2(coef * ex2(fmaf(bf16lo(r[ch].w), kLog2e, k2)), coef * ex2(fmaf(bf16hi(r[ch].w), kLog2e, k2)));
+                        stg128_stream(drow + (size_t)ch * kChunkElems + tid * 8, o);
+                    }
+                }
+                // the target column: g (1 - p_y); same thread that stored the vector holding it, so ordered
+                const int yl = y - sl_begin;
+                if ((unsigned)yl < (unsigned)sl_len && ((yl % kChunkElems) >> 3) == tid) {
+                    const float py = ex2(fmaf(zy, kLog2e, k2));
+                    drow[yl] = __float2bfloat16_rn(fmaf(coef, py, g));
+                }
+            } else {
+                const uint4 z4 = make_uint4(0, 0, 0, 0);
+#pragma unroll
+                for (int ch = 0; ch < NCH; ++ch)
+                    if (ch < nch && ch * kChunkElems + tid * 8 < sl_len) stg128_stream(drow + (size_t)ch * kChunkElems + tid * 8, z4);
+            }
+        }
+    }
+    if (CSIZE > 1) cluster_sync_all();  // peers may still be writing into this CTA's shared memory
+}
+
+// ------------------------------------------------------------------------------------------------ K7 (generic)
+
+template <typename TIn>
+__device__ __forceinline__ float ld_logit(const TIn* p, int64_t i);
+template <>
+__device__ __forceinline__ float ld_logit<float>(const float* p, int64_t i) { return p[i]; }
+template <>
+__device__ __forceinline__ float ld_logit<__nv_bfloat16>(const __nv_bfloat16* p, int64_t i) { return __bfloat162float(p[i]); }
+
+// One group of G threads per row (G = 32 or 256).  Three sweeps over the row (max, sum-exp, write); the
+// second and third hit L1/L2.  Used for fp32 logits (config c1), V % 8 != 0, unaligned pointers, V > 155648.
+template <typename TIn, int G>
+__global__ void __launch_bounds__(256) loss_rows_generic(const LossParams p) {
+    constexpr int kGroups = 256 / G;
+    __shared__ float s_red[2][kGroups][8];
+    const int tid = threadIdx.x, gl = tid % G, gi = tid / G, lane = tid & 31, wig = gl >> 5;
+    const TIn* logits = reinterpret_cast<const TIn*>(p.logits);
+    __nv_bfloat16* dlogits = reinterpret_cast<__nv_bfloat16*>(p.dlogits);
+    const float inv_S = p.ctrl->inv_num_segs;
+    const int V = p.V;
+    const int64_t nrow_groups = (p.T + kGroups - 1) / kGroups;
+    for (int64_t rg = blockIdx.x; rg < nrow_groups; rg += gridDim.x) {
+        const int64_t row = rg * kGroups + gi;
+        const bool inrange = row < p.T;
+        const bool act = inrange && p.mask[row] != 0;
+        int y = 0, sg = 0;
+        float old = 0.f, A = 0.f, w = 0.f, zy = 0.f;
+        bool ybad = false;
+        if (act) {
+            y = p.targets[row];
+            sg = p.seg_ids[row];
+            old = p.old_logp[row];
+            A = p.adv[row];
+            ybad = (unsigned)y >= (unsigned)V;
+            const bool sbad = (unsigned)sg >= (unsigned)p.S;
+            const float denom = sbad ? 0.f : (p.seg_denom ? p.seg_denom[sg] : (float)p.seg_cnt[sg]);
+            w = (denom > 0.f && !ybad) ? inv_S / denom : 0.f;
+            zy = ybad ? 0.f : ld_logit<TIn>(logits, row * p.ld + y);
+        }
+        const TIn* zrow = logits + row * p.ld;
+        float m = -INFINITY;
+        if (act)
+            for (int v = gl; v < V; v += G) m = fmaxf(m, ld_logit<TIn>(zrow, v));
+        m = warp_max(m);
+        if (G > 32) {
+            if (lane == 0) s_red[0][gi][wig] = m;
+            __syncthreads();
+            m = s_red[0][gi][0];
+#pragma unroll
+            for (int i = 1; i < G / 32; ++i) m = fmaxf(m, s_red[0][gi][i]);
+        }
+        float s = 0.f;
+        if (act)
+            for (int v = gl; v < V; v += G) s += ex2((ld_logit<TIn>(zrow, v) - m) * kLog2e);
+        s = warp_sum(s);
+        if (G > 32) {
+            if (lane == 0) s_red[1][gi][wig] = s;
+            __syncthreads();
+            s = 0.f;
+#pragma unroll
+            for (int i = 0; i < G / 32; ++i) s += s_red[1][gi][i];
+        }
+        if (inrange) {
+            __nv_bfloat16* drow = dlogits + row * p.ld;
+            float g = 0.f, lse = 0.f;
+            if (act) {
+                const TokScalars ts = token_scalars(m, s, zy, old, A, w, p.eps_lo, p.eps_hi, p.grad_scale);
+                g = ts.g;
+                lse = ts.lse;
+                if (gl == 0) {
+                    p.row_val[row] = ts.wl;
+                    p.row_kl[row] = ts.wkl;
+                    p.row_clip[row] = (uint8_t)(w > 0.f ? ts.clip : 0);
+                    if (p.logp_out) p.logp_out[row] = ybad ? 0.f : ts.logp;
+                    if (ybad) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_BAD_TARGET);
+                }
+            } else if (gl == 0) {
+                p.row_val[row] = 0.0;
+                p.row_kl[row] = 0.0;
+                p.row_clip[row] = 0;
+                if (p.logp_out) p.logp_out[row] = 0.f;
+            }
+            if (g != 0.f) {
+                const float coef = -g, k2 = -lse * kLog2e;
+                for (int v = gl; v < V; v += G) {
+                    const float pv = ex2(fmaf(ld_logit<TIn>(zrow, v), kLog2e, k2));
+                    drow[v] = __float2bfloat16_rn(v == y ? fmaf(coef, pv, g) : coef * pv);
+                }
+            } else {
+                for (int v = gl; v < V; v += G) drow[v] = __float2bfloat16_rn(0.f);
+            }
+        }
+        if (G > 32) __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ K8
+
+// Fixed-order fp64 reduction: thread i sums elements i, i+1024, ...; then a shared-memory tree.
+__global__ void __launch_bounds__(1024) loss_final_kernel(const LossParams p, int by_row) {
+    __shared__ double s_a[1024], s_b[1024];
+    __shared__ int s_c[2][1024];
+    const int tid = threadIdx.x;
+    const int64_t n = by_row ? p.T : (int64_t)p.ctrl->n_active;
+    double a = 0.0, b = 0.0;
+    int c1 = 0, c2 = 0;
+    for (int64_t i = tid; i < n; i += 1024) {
+        a += p.row_val[i];
+        b += p.row_kl[i];
+        const int c = p.row_clip[i];
+        c1 += c & 1;
+        c2 += (c >> 1) & 1;
+    }
+    s_a[tid] = a; s_b[tid] = b; s_c[0][tid] = c1; s_c[1][tid] = c2;
+    __syncthreads();
+    for (int o = 512; o; o >>= 1) {
+        if (tid < o) {
+            s_a[tid] += s_a[tid + o];
+            s_b[tid] += s_b[tid + o];
+            s_c[0][tid] += s_c[0][tid + o];
+            s_c[1][tid] += s_c[1][tid + o];
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        p.loss_out[0] = (float)s_a[0];
+        if (p.stats_out) {
+            p.stats_out[0] = (float)p.ctrl->n_active;
+            p.stats_out[1] = (float)s_c[0][0];
+            p.stats_out[2] = (float)s_c[1][0];
+            p.stats_out[3] = (float)s_b[0];
+        }
+    }
+}
+
+template <int NCH, int CSIZE>
+cudaError_t launch_rows(const LossParams& p, int num_sms, cudaStream_t stream) {
+    auto kern = loss_rows_kernel<NCH, CSIZE>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmemBytes);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)((num_sms / CSIZE) * CSIZE));
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = kRowsSmemBytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CSIZE;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, p);
+}
+
+}  // namespace
+
+extern "C" size_t ajt_loss_workspace_bytes(int64_t T, int32_t V, int32_t S) {
+    (void)V;
+    if (T < 0 || S < 0) return 0;
+    return loss_ws_layout(T, S).total;
+}
+
+extern "C" int ajt_policy_loss_fwd_bwd(const void* logits, const int32_t* targets, const float* old_logp, const float* adv,
+                                       const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T,
+                                       int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype, const float* seg_denom,
+                                       float inv_num_segs, float grad_scale, void* dlogits, float* loss_out, float* logp_out,
+                                       float* stats_out, void* workspace, size_t workspace_bytes, ajt_stream_t stream_) {
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (T < 0 || V <= 0 || S <= 0 || ld_logits < V || T >= ((int64_t)1 << 31)) return AJT_ERR_INVALID_ARG;
+    if (!(eps_lo >= 0.f) || !(eps_hi >= 0.f) || inv_num_segs < 0.f) return AJT_ERR_INVALID_ARG;
+    if (logits_dtype != AJT_DT_BF16 && logits_dtype != AJT_DT_F32) return AJT_ERR_INVALID_ARG;
+    if (!loss_out || !workspace) return AJT_ERR_INVALID_ARG;
+    if (T > 0 && (!logits || !targets || !old_logp || !adv || !mask || !seg_ids || !dlogits)) return AJT_ERR_INVALID_ARG;
+    if ((uintptr_t)workspace & 255) return AJT_ERR_INVALID_ARG;
+    const LossWs ws = loss_ws_layout(T, S);
+    if (workspace_bytes < ws.total) return AJT_ERR_WORKSPACE_TOO_SMALL;
+
+    int dev = 0, num_sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AJT_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || num_sms < 2) return AJT_ERR_CUDA;
+
+    uint8_t* wsb = reinterpret_cast<uint8_t*>(workspace);
+    LossParams p;
+    p.logits = logits; p.targets = targets; p.old_logp = old_logp; p.adv = adv; p.mask = mask; p.seg_ids = seg_ids;
+    p.eps_lo = eps_lo; p.eps_hi = eps_hi; p.T = T; p.V = V; p.S = S; p.ld = ld_logits; p.dtype = logits_dtype;
+    p.seg_denom = seg_denom; p.inv_num_segs = inv_num_segs; p.grad_scale = grad_scale;
+    p.dlogits = dlogits; p.loss_out = loss_out; p.logp_out = logp_out; p.stats_out = stats_out;
+    p.ctrl = reinterpret_cast<AjtCtrl*>(wsb + ws.ctrl);
+    p.seg_cnt = reinterpret_cast<int32_t*>(wsb + ws.seg_cnt);
+    p.list_active = reinterpret_cast<int32_t*>(wsb + ws.list_active);
+    p.list_zero = reinterpret_cast<int32_t*>(wsb + ws.list_zero);
+    p.row_val = reinterpret_cast<double*>(wsb + ws.row_val);
+    p.row_kl = reinterpret_cast<double*>(wsb + ws.row_kl);
+    p.row_clip = wsb + ws.row_clip;
+
+    if (cudaMemsetAsync(p.ctrl, 0, sizeof(AjtCtrl), stream) != cudaSuccess) return AJT_ERR_CUDA;
+    loss_prep_kernel<<<1, 1024, 0, stream>>>(p);
+
+    const bool aligned = (((uintptr_t)logits | (uintptr_t)dlogits) & 15) == 0 && (ld_logits % 8) == 0 && (V % 8) == 0;
+    const bool fast = logits_dtype == AJT_DT_BF16 && aligned && T > 0;
+    cudaError_t e = cudaSuccess;
+    int by_row = 0;
+    if (fast && logp_out && cudaMemsetAsync(logp_out, 0, (size_t)T * sizeof(float), stream) != cudaSuccess) return AJT_ERR_CUDA;
+    if (fast && V <= 8 * kChunkElems) e = launch_rows<8, 1>(p, num_sms, stream);
+    else if (fast && V <= 16 * kChunkElems) e = launch_rows<16, 1>(p, num_sms, stream);
+    else if (fast && V <= 2 * 16 * kChunkElems - 16) e = launch_rows<16, 2>(p, num_sms, stream);
+    else if (T > 0) {
+        by_row = 1;
+        const int grid = num_sms * 8;
+        if (logits_dtype == AJT_DT_F32) {
+            if (V <= 2048) loss_rows_generic<float, 32><<<grid, 256, 0, stream>>>(p);
+            else loss_rows_generic<float, 256><<<grid, 256, 0, stream>>>(p);
+        } else {
+            if (V <= 2048) loss_rows_generic<__nv_bfloat16, 32><<<grid, 256, 0, stream>>>(p);
+            else loss_rows_generic<__nv_bfloat16, 256><<<grid, 256, 0, stream>>>(p);
+        }
+    }
+    if (e != cudaSuccess) return AJT_ERR_CUDA;
+    loss_final_kernel<<<1, 1024, 0, stream>>>(p, by_row);
+    return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
+}
