@@ -69,9 +69,13 @@ def test_generic_path(T, V, S, rho, dtype):
 
 
 def test_grad_scale_makes_literal_tolerance_bite():
-    # reading L-9: with grad_scale = N_s * S' gradients are O(1) and the literal 2e-3 bound is meaningful
-    out, ref, info = run_and_check(400, 151936, 8, 0.7, torch.bfloat16, grad_scale=8 * 35.0)
-    assert np.abs(ref.dlogits).max() > 0.05
+    # reading L-9: scale the upstream gradient so that the largest |dlogits| is just under 1.  A bf16 half-ulp
+    # below 1 is 2^-9 = 1.95e-3, so the literal 2e-3 absolute bound is attainable there and it bites (all-zeros
+    # would fail by ~0.9); above 1 bf16 storage alone exceeds 2e-3.  The oracle is linear in grad_scale.
+    _, ref1, _ = run_and_check(400, 151936, 8, 0.7, torch.bfloat16, grad_scale=1.0)
+    gs = float(np.float32(0.9 / np.abs(ref1.dlogits).max()))
+    out, ref, info = run_and_check(400, 151936, 8, 0.7, torch.bfloat16, grad_scale=gs)
+    assert 0.8 < np.abs(ref.dlogits).max() < 1.0
 
 
 def test_symmetric_clip_and_seeds():
