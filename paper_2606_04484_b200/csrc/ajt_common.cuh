@@ -26,7 +26,9 @@ struct AjtCtrl {
     int64_t N_out;
     int32_t collision;    // set by the fused verify+scatter pass when a hash-equal candidate differs
     int32_t n_tiles;
-    uint32_t reserved[50];
+    int32_t tile_counter; // loss prep: dynamic tile ticket (ordered, so a tile's predecessors have always started)
+    int32_t done_counter; // loss prep: CTAs finished (the last one finalises 1/S')
+    uint32_t reserved[48];
 };
 static_assert(sizeof(AjtCtrl) == 256, "AjtCtrl must be 256 bytes");
 

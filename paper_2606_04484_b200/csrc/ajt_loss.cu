@@ -33,8 +33,18 @@ constexpr int kMaxCluster = 2;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr uint32_t kNegInf2 = 0xFF80FF80u;       // packed bf16 (-inf, -inf)
 
+constexpr int kScalRing = 32;                    // per-row scalar records in flight (> kSlots: the producer is at most kSlots rows ahead)
+struct __align__(16) RowScal {                   // written by the producer, read (broadcast) by every consumer
+    int64_t row;
+    int32_t y;
+    int32_t ybad;
+    float old, A, w, zy;
+};
+static_assert(sizeof(RowScal) == 32, "RowScal is two 16-byte vectors");
+
 constexpr size_t kRowsSmemBytes = (size_t)kSlots * kChunkBytes + kChunkBytes /* zero buffer */ +
-                                  (2 * kSlots + 2) * sizeof(uint64_t) + 2 * kConsWarps * kMaxCluster * sizeof(float2);
+                                  (2 * kSlots + 2) * sizeof(uint64_t) + 2 * kConsWarps * kMaxCluster * sizeof(float2) +
+                                  kScalRing * sizeof(RowScal);
 
 struct LossParams {
     const void* logits;
@@ -56,8 +66,10 @@ struct LossParams {
     float* stats_out;
     // workspace
     AjtCtrl* ctrl;
+    uint64_t* tile_state;  // [ntiles] prep scan: bit 63 valid, bits 32..62 active rows of the tile, bits 0..31 masked rows
     int32_t* seg_cnt;      // [S]
-    int32_t* list_active;  // [T] rows with mask = 1, ascending
+    int4* rec_i;           // [T] compact records of the rows with mask = 1, ascending: {row, target, segment, 0}
+    float2* rec_f;         // [T]   "  : {old_logp, adv}
     int32_t* list_zero;    // [T] rows with mask = 0, ascending
     double* row_val;       // [T] w_t L_t by compact index
     double* row_kl;        // [T] w_t (-log r_t) by compact index
@@ -65,8 +77,9 @@ struct LossParams {
 };
 
 struct LossWs {
-    size_t ctrl, seg_cnt, list_active, list_zero, row_val, row_kl, row_clip, total;
+    size_t ctrl, tile_state, seg_cnt, zero_bytes, rec_i, rec_f, list_zero, row_val, row_kl, row_clip, total;
 };
+constexpr int kPrepTile = 1024;
 
 __host__ inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -74,8 +87,11 @@ __host__ LossWs loss_ws_layout(int64_t T, int32_t S) {
     LossWs w;
     size_t o = 0;
     w.ctrl = o; o += align256(sizeof(AjtCtrl));
+    w.tile_state = o; o += align256((size_t)((T + kPrepTile - 1) / kPrepTile) * 8);
     w.seg_cnt = o; o += align256((size_t)S * 4);
-    w.list_active = o; o += align256((size_t)T * 4);
+    w.zero_bytes = o;  // [ctrl, tile_state, seg_cnt] are cleared by one memset per call
+    w.rec_i = o; o += align256((size_t)T * 16);
+    w.rec_f = o; o += align256((size_t)T * 8);
     w.list_zero = o; o += align256((size_t)T * 4);
     w.row_val = o; o += align256((size_t)T * 8);
     w.row_kl = o; o += align256((size_t)T * 8);
@@ -86,16 +102,22 @@ __host__ LossWs loss_ws_layout(int64_t T, int32_t S) {
 
 // ------------------------------------------------------------------------------------------------ K6
 
-__global__ void __launch_bounds__(1024) loss_prep_kernel(const LossParams p) {
-    __shared__ int s_cnt[2][2][32];
-    __shared__ int s_live[32];
+constexpr uint64_t kTileValid = 1ull << 63;
+
+// Grid-wide stable compaction in one pass.  Tiles of 1024 rows are handed out by an atomic ticket (so every predecessor of
+// a tile has started: no deadlock whatever the grid); a tile publishes its (active, masked) counts, then sums the counts of
+// all its predecessors (1024 at a time, spinning on the valid bit) to get its bases.  The last CTA to finish counts S'.
+__global__ void __launch_bounds__(1024) loss_prep_kernel(const LossParams p, int ntiles) {
+    __shared__ int s_cnt[2][32];
+    __shared__ int s_red[2][32];
+    __shared__ int s_tile, s_last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int s = tid; s < p.S; s += 1024) p.seg_cnt[s] = 0;
-    __syncthreads();
-    int base_a = 0, base_z = 0;
-    int buf = 0;
-    for (int64_t t0 = 0; t0 < p.T; t0 += 1024, buf ^= 1) {
-        const int64_t t = t0 + tid;
+    for (;;) {
+        if (tid == 0) s_tile = atomicAdd(&p.ctrl->tile_counter, 1);
+        __syncthreads();
+        const int tile = s_tile;
+        if (tile >= ntiles) break;
+        const int64_t t = (int64_t)tile * kPrepTile + tid;
         const bool in = t < p.T;
         bool act = in && p.mask[t] != 0;
         int sg = act ? p.seg_ids[t] : 0;
@@ -107,43 +129,75 @@ __global__ void __launch_bounds__(1024) loss_prep_kernel(const LossParams p) {
         const int key = act ? sg : -1 - lane;
         const unsigned peers = __match_any_sync(0xffffffffu, key);
         if (act && lane == __ffs(peers) - 1) atomicAdd(&p.seg_cnt[sg], __popc(peers));
-        // stable compaction into the two row lists
         const unsigned ba = __ballot_sync(0xffffffffu, act);
         const unsigned bz = __ballot_sync(0xffffffffu, in && !act);
         if (lane == 0) {
-            s_cnt[buf][0][warp] = __popc(ba);
-            s_cnt[buf][1][warp] = __popc(bz);
+            s_cnt[0][warp] = __popc(ba);
+            s_cnt[1][warp] = __popc(bz);
         }
         __syncthreads();
         int pa = 0, pz = 0, ta = 0, tz = 0;
 #pragma unroll
         for (int w = 0; w < 32; ++w) {
-            const int ca = s_cnt[buf][0][w], cz = s_cnt[buf][1][w];
+            const int ca = s_cnt[0][w], cz = s_cnt[1][w];
             if (w < warp) { pa += ca; pz += cz; }
             ta += ca; tz += cz;
         }
+        if (tid == 0)
+            atomicExch(reinterpret_cast<unsigned long long*>(&p.tile_state[tile]),
+                       (unsigned long long)(kTileValid | ((uint64_t)ta << 32) | (uint64_t)tz));
+        int sa = 0, sz = 0;
+        for (int i = tid; i < tile; i += 1024) {
+            uint64_t v;
+            do {
+                v = *reinterpret_cast<volatile uint64_t*>(&p.tile_state[i]);
+            } while (!(v & kTileValid));
+            sa += (int)((v >> 32) & 0x7fffffffu);
+            sz += (int)(v & 0xffffffffu);
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+            sa += __shfl_xor_sync(0xffffffffu, sa, o);
+            sz += __shfl_xor_sync(0xffffffffu, sz, o);
+        }
+        if (lane == 0) { s_red[0][warp] = sa; s_red[1][warp] = sz; }
+        __syncthreads();
+        int base_a = 0, base_z = 0;
+#pragma unroll
+        for (int w = 0; w < 32; ++w) { base_a += s_red[0][w]; base_z += s_red[1][w]; }
         const unsigned lt = (1u << lane) - 1u;
-        if (act) p.list_active[base_a + pa + __popc(ba & lt)] = (int32_t)t;
-        else if (in) p.list_zero[base_z + pz + __popc(bz & lt)] = (int32_t)t;
-        base_a += ta;
-        base_z += tz;
+        if (act) {
+            const int idx = base_a + pa + __popc(ba & lt);
+            p.rec_i[idx] = make_int4((int)t, p.targets[t], sg, 0);
+            p.rec_f[idx] = make_float2(p.old_logp[t], p.adv[t]);
+        } else if (in) {
+            p.list_zero[base_z + pz + __popc(bz & lt)] = (int32_t)t;
+        }
+        if (tile == ntiles - 1 && tid == 0) {
+            p.ctrl->n_active = base_a + ta;
+            p.ctrl->n_zero = base_z + tz;
+        }
+        __syncthreads();
     }
+    // the last CTA to get here sees every N_s: S' = #{s : N_s > 0}
+    __threadfence();
     __syncthreads();
-    // S' = #{s : N_s > 0}
+    if (tid == 0) s_last = atomicAdd(&p.ctrl->done_counter, 1) == (int)gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
     int live = 0;
     for (int s = tid; s < p.S; s += 1024) {
-        const float d = p.seg_denom ? p.seg_denom[s] : (float)p.seg_cnt[s];
+        const float d = p.seg_denom ? p.seg_denom[s] : (float)__ldcg(&p.seg_cnt[s]);
         live += d > 0.f;
     }
 #pragma unroll
     for (int o = 16; o; o >>= 1) live += __shfl_xor_sync(0xffffffffu, live, o);
-    if (lane == 0) s_live[warp] = live;
+    if (lane == 0) s_red[0][warp] = live;
     __syncthreads();
     if (tid == 0) {
         int tot = 0;
-        for (int w = 0; w < 32; ++w) tot += s_live[w];
-        p.ctrl->n_active = base_a;
-        p.ctrl->n_zero = base_z;
+        for (int w = 0; w < 32; ++w) tot += s_red[0][w];
         p.ctrl->n_live_segs = tot;
         p.ctrl->inv_num_segs = p.inv_num_segs != 0.f ? p.inv_num_segs : (tot > 0 ? 1.0f / (float)tot : 0.f);
     }
@@ -206,7 +260,8 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
     uint64_t* full = reinterpret_cast<uint64_t*>(zbuf + kChunkBytes);
     uint64_t* empty = full + kSlots;
     uint64_t* pbar = empty + kSlots;
-    float2* part = reinterpret_cast<float2*>(pbar + 2);  // [2][kConsWarps * CSIZE]
+    float2* part = reinterpret_cast<float2*>(pbar + 2);  // [2][kConsWarps * kMaxCluster]
+    RowScal* scal = reinterpret_cast<RowScal*>(part + 2 * kConsWarps * kMaxCluster);
     constexpr int kParts = kConsWarps * CSIZE;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -254,10 +309,48 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
                     bulk_commit();
                 }
             };
+            // Per-row scalars are gathered two rows ahead so that their dependent loads (record -> logits[row, y],
+            // N_s) never sit on anybody's critical path: stage B holds row k+1's record with its two loads in
+            // flight, stage C holds row k complete.  Published through shared memory before the row's first
+            // full-barrier arrive (release) and read by the consumers after their wait (acquire).
+            const float inv_S = p.ctrl->inv_num_segs;
+            struct Stage { int4 ri; float2 rf; float zy, den; };
+            auto load_rec = [&](int k, Stage& st) {
+                if (k < nrows) {
+                    const int64_t idx = cid + (int64_t)k * NC;
+                    st.ri = p.rec_i[idx];
+                    st.rf = p.rec_f[idx];
+                }
+            };
+            auto load_dep = [&](int k, Stage& st) {
+                if (k < nrows) {
+                    const bool ybad = (unsigned)st.ri.y >= (unsigned)V;
+                    st.zy = ybad ? 0.f : __bfloat162float(logits[(int64_t)st.ri.x * p.ld + st.ri.y]);
+                    st.den = p.seg_denom ? p.seg_denom[st.ri.z] : (float)p.seg_cnt[st.ri.z];
+                }
+            };
+            Stage A = {}, B = {}, C = {};
+            load_rec(0, C);
+            load_rec(1, B);
+            load_dep(0, C);
+            load_dep(1, B);
             int slot = 0;
             uint32_t ph = 0;
             for (int k = 0; k < nrows; ++k) {
-                const int64_t row = p.list_active[cid + (int64_t)k * NC];
+                load_rec(k + 2, A);
+                {
+                    const bool ybad = (unsigned)C.ri.y >= (unsigned)V;
+                    RowScal rs;
+                    rs.row = C.ri.x;
+                    rs.y = C.ri.y;
+                    rs.ybad = ybad;
+                    rs.old = C.rf.x;
+                    rs.A = C.rf.y;
+                    rs.w = (C.den > 0.f && !ybad) ? inv_S / C.den : 0.f;
+                    rs.zy = C.zy;
+                    scal[k & (kScalRing - 1)] = rs;
+                }
+                const int64_t row = C.ri.x;
                 const __nv_bfloat16* src = logits + row * p.ld + sl_begin;
                 for (int ch = 0; ch < nch; ++ch) {
                     mbar_wait(&empty[slot], ph ^ 1u);
@@ -267,35 +360,41 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
                     if (++slot == kSlots) { slot = 0; ph ^= 1u; }
                 }
                 zero_rows_until((int)(((int64_t)(k + 1) * nzero) / nrows));
+                C = B;
+                B = A;
+                load_dep(k + 2, B);
             }
             zero_rows_until(nzero);
             bulk_wait<0>();
         }
     } else {
         // ===== consumer warps =====
-        const float inv_S = p.ctrl->inv_num_segs;
         int slot = 0;
         uint32_t ph = 0;
         for (int k = 0; k < nrows; ++k) {
             const int kidx = cid + k * NC;
-            const int64_t row = p.list_active[kidx];
-            const int y = p.targets[row];
-            const float old = p.old_logp[row];
-            const float A = p.adv[row];
-            const int sg = p.seg_ids[row];
-            const float denom = p.seg_denom ? p.seg_denom[sg] : (float)p.seg_cnt[sg];
-            const bool ybad = (unsigned)y >= (unsigned)V;
-            const float w = (denom > 0.f && !ybad) ? inv_S / denom : 0.f;
-            const float zy = ybad ? 0.f : __bfloat162float(logits[row * p.ld + y]);
-
             // ---- pass 1a: ring -> registers (packed bf16), packed running max
             uint4 r[NCH];
             uint32_t mx = kNegInf2;
+            int64_t row = 0;
+            int y = 0;
+            bool ybad = false;
+            float old = 0.f, A = 0.f, w = 0.f, zy = 0.f;
 #pragma unroll
             for (int ch = 0; ch < NCH; ++ch) {
                 r[ch] = make_uint4(kNegInf2, kNegInf2, kNegInf2, kNegInf2);
                 if (ch < nch) {
                     mbar_wait(&full[slot], ph);
+                    if (ch == 0) {  // the producer published this row's scalars before arming the first chunk
+                        const uint4 s0 = lds128(&scal[k & (kScalRing - 1)]), s1 = lds128(&scal[k & (kScalRing - 1)].old);
+                        row = (int64_t)(((uint64_t)s0.y << 32) | s0.x);
+                        y = (int)s0.z;
+                        ybad = s0.w != 0;
+                        old = __uint_as_float(s1.x);
+                        A = __uint_as_float(s1.y);
+                        w = __uint_as_float(s1.z);
+                        zy = __uint_as_float(s1.w);
+                    }
                     if (ch * kChunkElems + tid * 8 < sl_len) r[ch] = lds128(ring + (size_t)slot * kChunkBytes + tid * 16);
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&empty[slot]);
@@ -326,9 +425,6 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
             const float sw = warp_sum(s * exp_diff(m, mw));
             const int par = k & 1;
             float2* mypart = part + par * kParts;
-            // z[y] must have landed before the peer can learn our partial and start overwriting the row
-            // (dlogits may alias logits)
-            asm volatile("" ::"f"(zy) : "memory");
             if (lane == 0) {
                 mypart[rank * kConsWarps + warp] = make_float2(mw, sw);
                 if (CSIZE > 1) {
@@ -579,15 +675,18 @@ extern "C" int ajt_policy_loss_fwd_bwd(const void* logits, const int32_t* target
     p.seg_denom = seg_denom; p.inv_num_segs = inv_num_segs; p.grad_scale = grad_scale;
     p.dlogits = dlogits; p.loss_out = loss_out; p.logp_out = logp_out; p.stats_out = stats_out;
     p.ctrl = reinterpret_cast<AjtCtrl*>(wsb + ws.ctrl);
+    p.tile_state = reinterpret_cast<uint64_t*>(wsb + ws.tile_state);
     p.seg_cnt = reinterpret_cast<int32_t*>(wsb + ws.seg_cnt);
-    p.list_active = reinterpret_cast<int32_t*>(wsb + ws.list_active);
+    p.rec_i = reinterpret_cast<int4*>(wsb + ws.rec_i);
+    p.rec_f = reinterpret_cast<float2*>(wsb + ws.rec_f);
     p.list_zero = reinterpret_cast<int32_t*>(wsb + ws.list_zero);
     p.row_val = reinterpret_cast<double*>(wsb + ws.row_val);
     p.row_kl = reinterpret_cast<double*>(wsb + ws.row_kl);
     p.row_clip = wsb + ws.row_clip;
 
-    if (cudaMemsetAsync(p.ctrl, 0, sizeof(AjtCtrl), stream) != cudaSuccess) return AJT_ERR_CUDA;
-    loss_prep_kernel<<<1, 1024, 0, stream>>>(p);
+    if (cudaMemsetAsync(p.ctrl, 0, ws.zero_bytes, stream) != cudaSuccess) return AJT_ERR_CUDA;
+    const int ntiles = (int)((T + kPrepTile - 1) / kPrepTile);
+    loss_prep_kernel<<<max(1, min(ntiles, num_sms)), 1024, 0, stream>>>(p, ntiles);
 
     const bool aligned = (((uintptr_t)logits | (uintptr_t)dlogits) & 15) == 0 && (ld_logits % 8) == 0 && (V % 8) == 0;
     const bool fast = logits_dtype == AJT_DT_BF16 && aligned && T > 0;
