@@ -32,32 +32,12 @@ METRIC = "merge Gtokens/s and policy-loss fwd+bwd logits GB/s (fraction of B200 
 MB_ROWS = 40960          # loss micro-batch rows (BASELINE.json configs[1]: "~40k merged tokens")
 V = 151936
 EPS = (0.2, 0.28)
-FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
-NOMINAL_HBM_GBS = 8000.0    # BASELINE.json north_star "~8 TB/s"
 
-
-def measured_peak():
-    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(p):
-        try:
-            with open(p) as f:
-                return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
-        except Exception:
-            pass
-    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
-
-
-# ----------------------------------------------------------------------------------------- algorithmic bytes
-
-
-def merge_bytes(n: int, N_in: int, N_out: int, with_logp: bool = True) -> int:
-    """read every input token once, write every output once."""
-    return 4 * N_in + 9 * N_out + (4 * N_out if with_logp else 0) + 20 * n
+from paper_2606_04484_b200.harness import (NOMINAL_HBM_GBS, loss_bytes as _loss_bytes, measured_peak, merge_bytes)  # noqa: E402
 
 
 def loss_bytes(T: int, Vv: int, n_unmasked: int, b_in: int = 2) -> int:
-    """read each UNMASKED row once, write EVERY row once, 17 B/token of side inputs."""
-    return n_unmasked * Vv * b_in + T * Vv * 2 + 17 * T
+    return _loss_bytes(T, Vv, n_unmasked, b_in)
 
 
 # ----------------------------------------------------------------------------------------- clocks sampler
@@ -130,24 +110,14 @@ class ClockSampler:
 # ----------------------------------------------------------------------------------------- workload (harness)
 
 
-def harness_old_logp(torch, logits_t, targets_t, noise: np.ndarray):
-    """INPUT synthesis, not the method: old_logp = (library log-softmax of the row at its target) + N(0, 0.05) noise
-    (BASELINE.json configs: "old_logp = new logp + N(0,0.05)")."""
-    T = logits_t.shape[0]
-    out = torch.empty(T, dtype=torch.float32, device=logits_t.device)
-    step = max(1, (1 << 27) // max(1, logits_t.shape[1]))
-    for a in range(0, T, step):
-        z = logits_t[a:a + step].float()
-        lse = torch.logsumexp(z, dim=-1)
-        out[a:a + step] = z.gather(1, targets_t[a:a + step].long()[:, None])[:, 0] - lse
-    return out + torch.from_numpy(noise).to(out.device)
+def harness_old_logp(torch, logits_t, targets_t, noise):
+    from paper_2606_04484_b200.harness import harness_old_logp as f
+    return f(logits_t, targets_t, noise)
 
 
 def fill_logits(torch, buf, seed: int, sigma: float = 3.0, slab: int = 2048):
-    g = torch.Generator(device=buf.device).manual_seed(seed)
-    for a in range(0, buf.shape[0], slab):
-        b = min(buf.shape[0], a + slab)
-        buf[a:b] = (torch.randn((b - a, buf.shape[1]), generator=g, device=buf.device, dtype=torch.float32) * sigma).to(buf.dtype)
+    from paper_2606_04484_b200.harness import fill_logits as f
+    f(buf, seed, sigma, slab)
 
 
 def loss_side_inputs(W, merged_tokens, merged_mask, merged_old_logp, merged_offsets, merged_traj, seed: int):

@@ -172,6 +172,19 @@ int ajt_policy_loss_fwd_bwd(
     float* stats_out,           /* DEVICE [4] or NULL: {n_masked, n_clipped_hi, n_clipped_lo, sum_t w_t (-log r_t)} */
     void* workspace, size_t workspace_bytes, ajt_stream_t stream);
 
+/* Batch-wide per-trajectory normalisers for callers that stream the batch through several loss calls
+ * (micro-batches, 64k-row chunks, or rows of one trajectory spread over several GPUs; reading L-4;
+ * "masked per-trajectory mean", BASELINE.json north_star):
+ *   seg_denom[s] (+)= #{t in [0,T) : seg_ids[t] = s and mask[t] != 0}
+ * `accumulate` = 0 clears seg_denom (and *status_bits) first; != 0 adds to what is there, so a batch can be
+ * counted chunk by chunk.  Counts are integers held in fp32: exact below 2^24 masked tokens per trajectory.
+ * Pass the result as `seg_denom` to every ajt_policy_loss_fwd_bwd call of the batch with inv_num_segs = 0
+ * (1/S' is then taken from seg_denom) — or all-reduce it across ranks first.
+ * seg_denom: DEVICE [S].  status_bits: DEVICE [1] or NULL (AJT_STATUS_BAD_SEG when a masked-in token has
+ * seg_ids[t] outside [0,S); that token is not counted).  Enqueues on `stream`, does not synchronise. */
+int ajt_segment_counts(const uint8_t* mask /* DEVICE [T] */, const int32_t* seg_ids /* DEVICE [T] */, int64_t T, int32_t S,
+                       int32_t accumulate, float* seg_denom, uint32_t* status_bits, ajt_stream_t stream);
+
 /* HOST-buffer variant.  `arena` is DEVICE scratch of at least ajt_loss_host_arena_bytes(T, V, S, ld, dtype)
  * bytes.  Rows are staged in slabs so that H2D, compute and D2H overlap.  Synchronises. */
 size_t ajt_loss_host_arena_bytes(int64_t T, int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype);

@@ -211,8 +211,10 @@ int ajt_oracle_loss(const void* logits, int32_t dtype, int64_t R, int32_t V, int
     for (int32_t s = 0; s < S; ++s) Sp += (Ns[s] > 0.0);
     double inv_Sp = (inv_num_segs != 0.0) ? inv_num_segs : (Sp > 0.0 ? 1.0 / Sp : 0.0);
 
-    double total = 0.0, st0 = 0, st1 = 0, st2 = 0, st3 = 0;
-#pragma omp parallel for schedule(static) reduction(+ : total, st0, st1, st2, st3) reduction(min : err)
+    /* Per-row terms are stored and summed afterwards in row order, so the scalar does not depend on the
+     * number of threads (step 5 is a plain sum over t). */
+    double* term = (double*)calloc((size_t)(R > 0 ? R : 1) * 5, sizeof(double)); /* {w L, m, clip_hi, clip_lo, w(-log r)} */
+#pragma omp parallel for schedule(static) reduction(min : err)
     for (int64_t r = 0; r < R; ++r) {
         int64_t t = row_ids ? row_ids[r] : r;
         double* drow = dlogits ? dlogits + r * (int64_t)V : NULL;
@@ -258,8 +260,9 @@ int ajt_oracle_loss(const void* logits, int32_t dtype, int64_t R, int32_t V, int
         int clip_lo = (A < 0.0 && ratio < 1.0 - eps_lo);
         double gt = (clip_hi || clip_lo) ? 0.0 : grad_scale * wt * (-A * ratio);
 
-        total += wt * L; /* step 5 */
-        st0 += 1.0; st1 += clip_hi; st2 += clip_lo; st3 += wt * (-(lp - (double)old_logp[t]));
+        term[5 * r + 0] = wt * L; /* step 5 */
+        term[5 * r + 1] = 1.0; term[5 * r + 2] = clip_hi; term[5 * r + 3] = clip_lo;
+        term[5 * r + 4] = wt * (-(lp - (double)old_logp[t]));
         if (logp) logp[r] = lp;
         if (w) w[r] = wt;
         if (g) g[r] = gt;
@@ -271,8 +274,14 @@ int ajt_oracle_loss(const void* logits, int32_t dtype, int64_t R, int32_t V, int
             }
         }
     }
+    double total = 0.0, st0 = 0, st1 = 0, st2 = 0, st3 = 0;
+    for (int64_t r = 0; r < R; ++r) {
+        total += term[5 * r + 0];
+        st0 += term[5 * r + 1]; st1 += term[5 * r + 2]; st2 += term[5 * r + 3]; st3 += term[5 * r + 4];
+    }
     *loss_partial = total;
     if (stats) { stats[0] += st0; stats[1] += st1; stats[2] += st2; stats[3] += st3; }
+    free(term);
     free(Ns);
     return err;
 }

@@ -25,6 +25,7 @@ _EXPORTS = [
     "ajt_version", "ajt_strerror", "ajt_last_status",
     "ajt_merge_workspace_bytes", "ajt_merge_timelines", "ajt_merge_host_arena_bytes", "ajt_merge_timelines_host",
     "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
+    "ajt_segment_counts",
 ]
 
 _lib = None
@@ -64,7 +65,7 @@ def lib():
         L.ajt_loss_host_arena_bytes.restype = C.c_size_t
         L.ajt_loss_host_arena_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32]
         for f in ("ajt_merge_timelines", "ajt_merge_timelines_host", "ajt_policy_loss_fwd_bwd",
-                  "ajt_policy_loss_fwd_bwd_host"):
+                  "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -281,6 +282,24 @@ def policy_loss_fwd_bwd(logits: torch.Tensor, targets: torch.Tensor, old_logp: t
         _dp(out.stats), _dp(out.workspace), C.c_size_t(out.workspace.numel()), _stream(stream))
     if rc != 0:
         raise AjtError(rc, "ajt_policy_loss_fwd_bwd")
+    return out
+
+
+def segment_counts(mask: torch.Tensor, seg_ids: torch.Tensor, S: int, out: Optional[torch.Tensor] = None,
+                   accumulate: bool = False, status: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """ajt_segment_counts (include/ajt.h): seg_denom[s] (+)= number of masked-in tokens of trajectory s."""
+    _require_cuda()
+    _check_dev(mask, torch.uint8, "mask")
+    _check_dev(seg_ids, torch.int32, "seg_ids")
+    if out is None:
+        out = torch.empty(S, dtype=torch.float32, device=mask.device)
+        accumulate = False
+    _check_dev(out, torch.float32, "seg_denom")
+    _check_dev(status, torch.int32, "status")
+    rc = lib().ajt_segment_counts(_dp(mask), _dp(seg_ids), C.c_int64(int(mask.numel())), C.c_int32(S),
+                                  C.c_int32(1 if accumulate else 0), _dp(out), _dp(status), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_segment_counts")
     return out
 
 

@@ -621,6 +621,28 @@ __global__ void __launch_bounds__(1024) loss_final_kernel(const LossParams p, in
     }
 }
 
+// ------------------------------------------------------------------------------------------------ segment counts
+
+// N_s += #{t in this call : seg_t = s, mask_t = 1}.  Counts are integers held in fp32 (exact below 2^24), so the
+// float atomics commute and the result does not depend on the order of arrival.
+__global__ void __launch_bounds__(256) segment_counts_kernel(const uint8_t* __restrict__ mask, const int32_t* __restrict__ seg_ids,
+                                                             int64_t T, int32_t S, float* __restrict__ denom,
+                                                             uint32_t* __restrict__ status) {
+    const int lane = threadIdx.x & 31;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int64_t Tpad = (T + 31) & ~(int64_t)31;   // whole warps stay converged for match.any
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < Tpad; t += stride) {
+        bool act = t < T && mask[t] != 0;
+        const int sg = act ? seg_ids[t] : 0;
+        if (act && (unsigned)sg >= (unsigned)S) {
+            if (status) atomicOr(status, (uint32_t)AJT_STATUS_BAD_SEG);
+            act = false;
+        }
+        const unsigned peers = __match_any_sync(0xffffffffu, act ? sg : -1 - lane);
+        if (act && lane == __ffs(peers) - 1) atomicAdd(&denom[sg], (float)__popc(peers));
+    }
+}
+
 template <int NCH, int CSIZE>
 cudaError_t launch_rows(const LossParams& p, int num_sms, cudaStream_t stream) {
     auto kern = loss_rows_kernel<NCH, CSIZE>;
@@ -709,5 +731,24 @@ extern "C" int ajt_policy_loss_fwd_bwd(const void* logits, const int32_t* target
     }
     if (e != cudaSuccess) return AJT_ERR_CUDA;
     loss_final_kernel<<<1, 1024, 0, stream>>>(p, by_row);
+    return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
+}
+
+extern "C" int ajt_segment_counts(const uint8_t* mask, const int32_t* seg_ids, int64_t T, int32_t S, int32_t accumulate,
+                                  float* seg_denom, uint32_t* status_bits, ajt_stream_t stream_) {
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (T < 0 || S <= 0 || !seg_denom) return AJT_ERR_INVALID_ARG;
+    if (T > 0 && (!mask || !seg_ids)) return AJT_ERR_INVALID_ARG;
+    int dev = 0, num_sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AJT_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || num_sms < 1) return AJT_ERR_CUDA;
+    if (!accumulate) {
+        if (cudaMemsetAsync(seg_denom, 0, (size_t)S * sizeof(float), stream) != cudaSuccess) return AJT_ERR_CUDA;
+        if (status_bits && cudaMemsetAsync(status_bits, 0, sizeof(uint32_t), stream) != cudaSuccess) return AJT_ERR_CUDA;
+    }
+    if (T == 0) return AJT_OK;
+    const int64_t want = (T + 255) / 256;
+    const int grid = (int)(want < (int64_t)num_sms * 8 ? want : (int64_t)num_sms * 8);
+    segment_counts_kernel<<<grid, 256, 0, stream>>>(mask, seg_ids, T, S, seg_denom, status_bits);
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }

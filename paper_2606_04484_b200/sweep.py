@@ -1,0 +1,213 @@
+"""Per-config measurement of the CUDA path on one GPU: `python -m paper_2606_04484_b200.sweep [--configs c1,c2,c3,c4,c5]`.
+
+One JSON line per (config, stage): merge time / merged tokens/s / GB/s / token-reduction factor, loss time / logits GB/s,
+each as a fraction of the measured HBM peak (MEASURED_PEAKS.json) and of the nominal 8 TB/s.
+Inputs are the seeded synthetic workloads of DESIGN.md "Input recipe".  Calls whose inputs fit in L2 are timed cold
+(a 256 MB write between repetitions) and the line says so.  bench.py is the driver's contract; this is the wider table
+behind profiles/*_sweep.md.  The oracle is not used here (parity at these sizes is tests/test_gpu_fullsize.py).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import sys
+import time
+
+import numpy as np
+import torch
+
+import paper_2606_04484_b200 as ajt
+from paper_2606_04484_b200 import harness as H
+from paper_2606_04484_b200 import workloads as W
+
+L2_BYTES = 126 << 20
+
+
+def _stats(ms):
+    a = np.asarray(ms, dtype=np.float64)
+    return float(np.median(a)), float(a.min())
+
+
+def _emit(out, **kw):
+    line = json.dumps(kw)
+    print(line, flush=True)
+    if out:
+        out.write(line + "\n")
+        out.flush()
+
+
+def measure_merge(name: str, mi, dev, stream, reps: int, out, rules=(("longest", ajt.OWNER_LONGEST),)):
+    d = lambda a: torch.from_numpy(a).to(dev)
+    tokens, offsets, traj, rs, lp = d(mi.tokens), d(mi.offsets), d(mi.traj_ids), d(mi.resp_start), d(mi.old_logp)
+    peak, _ = H.measured_peak()
+    fin = None
+    for rname, rule in rules:
+        with torch.cuda.stream(stream):
+            mo = ajt.merge_timelines(tokens, offsets, traj, rs, None, lp, owner_rule=rule, stream=stream)
+            stream.synchronize()
+        status = ajt.last_status(mo.workspace, stream)
+        assert status == 0, status
+        fin = mo.finalize()
+        cold = 4 * mi.n_tokens * 2 < L2_BYTES
+        flush = H.L2Flusher(dev) if cold else None
+        call = lambda: ajt.merge_timelines(tokens, offsets, traj, rs, None, lp, owner_rule=rule, out=mo, stream=stream)
+        med, best = _stats(H.time_calls(call, stream, reps=reps, flush=flush))
+        b = H.merge_bytes(mi.n, mi.n_tokens, fin.N_out)
+        gbs = b / (med * 1e-3) / 1e9
+        _emit(out, stage="merge", config=name, owner_rule=rname, n=mi.n, N_in=mi.n_tokens, N_out=fin.N_out, M=fin.M,
+              token_reduction_factor=mi.n_tokens / max(1, fin.N_out), ms_median=med, ms_best=best,
+              merged_gtokens_per_s=fin.N_out / (med * 1e-3) / 1e9, input_gtokens_per_s=mi.n_tokens / (med * 1e-3) / 1e9,
+              algorithmic_bytes=b, gb_per_s=gbs, frac_of_measured=gbs / peak, frac_of_nominal_8tbs=gbs / H.NOMINAL_HBM_GBS,
+              l2="cold (256 MB flush between calls)" if cold else "input larger than L2", reps=reps)
+    return fin
+
+
+def measure_loss(name: str, logits, targets, old, adv, mask, seg, S, eps, dev, stream, reps, out, seg_denom=None, inv=0.0,
+                 dlogits=None, extra=None):
+    T, V = logits.shape
+    b_in = 2 if logits.dtype == torch.bfloat16 else 4
+    if dlogits is None:
+        dlogits = torch.empty((T, V), dtype=torch.bfloat16, device=dev)
+    lo = None
+
+    def call():
+        nonlocal lo
+        lo = ajt.policy_loss_fwd_bwd(logits, targets, old, adv, mask, seg, S, eps[0], eps[1], seg_denom=seg_denom, inv_num_segs=inv,
+                                     dlogits=dlogits, out=lo, stream=stream)
+
+    cold = T * V * b_in < L2_BYTES
+    flush = H.L2Flusher(dev) if cold else None
+    med, best = _stats(H.time_calls(call, stream, reps=reps, flush=flush))
+    status = ajt.last_status(lo.workspace, stream)
+    assert status == 0, status
+    nu = int(mask.sum().item())
+    b = H.loss_bytes(T, V, nu, b_in)
+    gbs = b / (med * 1e-3) / 1e9
+    peak, _ = H.measured_peak()
+    kw = dict(stage="loss", config=name, T=T, V=V, S=S, dtype="bf16" if b_in == 2 else "f32", mask_density=nu / max(1, T),
+              ms_median=med, ms_best=best, algorithmic_bytes=b, logits_gb_per_s=gbs, frac_of_measured=gbs / peak,
+              frac_of_nominal_8tbs=gbs / H.NOMINAL_HBM_GBS, dense_2TV_gb_per_s=2.0 * T * V * 2 / (med * 1e-3) / 1e9,
+              loss=float(lo.loss.item()), l2="cold (256 MB flush between calls)" if cold else "input larger than L2", reps=reps)
+    if extra:
+        kw.update(extra)
+    _emit(out, **kw)
+    return dlogits
+
+
+def loss_inputs_from_merge(fin, seed, cfg_index, adv_kind, dev):
+    cpu = lambda t: t.cpu().numpy()
+    targets, mask, _ = W.shift_for_next_token(cpu(fin.merged_tokens), cpu(fin.merged_mask), cpu(fin.merged_old_logp),
+                                              cpu(fin.merged_offsets))
+    seg, S, _ = W.seg_ids_from_merged(cpu(fin.merged_offsets), cpu(fin.merged_traj))
+    if adv_kind == "pm1":
+        adv = W.advantages_pm1(seed, cfg_index, S)[seg]
+    else:
+        adv = W.advantages_group_zscore(seed, cfg_index, S)[seg]
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    return d(targets), d(mask), d(seg), S, d(adv.astype(np.float32))
+
+
+def chunked_loss(name, fin, V, eps, seed, cfg_index, adv_kind, rows, n_chunks, dev, stream, reps, out, dtype=torch.bfloat16,
+                 sigma=3.0):
+    targets, mask, seg, S, adv = loss_inputs_from_merge(fin, seed, cfg_index, adv_kind, dev)
+    if V < 151936:   # model B of configs[3]: token ids are already < its vocabulary
+        assert int(targets.max().item()) < V
+    Ns = ajt.segment_counts(mask, seg, S)
+    T_all = int(targets.numel())
+    rows = min(rows, T_all)
+    logits = torch.empty((rows, V), dtype=dtype, device=dev)
+    dlogits = torch.empty((rows, V), dtype=torch.bfloat16, device=dev)
+    n_avail = max(1, T_all // rows)
+    for c in range(min(n_chunks, n_avail)):
+        k = (c * max(1, n_avail // max(1, n_chunks))) % n_avail     # spread the timed chunks over the batch
+        sl = slice(k * rows, (k + 1) * rows)
+        H.fill_logits(logits, seed * 13 + c, sigma)
+        noise = (W.rng_for(seed, cfg_index, 99 + c).standard_normal(rows) * 0.05).astype(np.float32)
+        tg = targets[sl].contiguous()
+        old = H.harness_old_logp(logits, tg, noise)
+        measure_loss(name, logits, tg, old, adv[sl].contiguous(), mask[sl].contiguous(), seg[sl].contiguous(), S, eps, dev, stream,
+                     reps, out, seg_denom=Ns, inv=0.0, dlogits=dlogits,
+                     extra=dict(chunk=k, chunks_in_batch=-(-T_all // rows), batch_rows=T_all))
+    del logits, dlogits
+    torch.cuda.empty_cache()
+
+
+def run_c5(dev, stream, reps, out, quick=False):
+    Ts = (4096, 16384, 65536, 131072)
+    Vs = (32000, 128256, 151936)
+    if quick:
+        Ts, Vs = (4096, 65536), (32000, 151936)
+    cell = 0
+    for V in Vs:
+        for T in Ts:
+            logits = torch.empty((T, V), dtype=torch.bfloat16, device=dev)
+            dlogits = torch.empty((T, V), dtype=torch.bfloat16, device=dev)
+            H.fill_logits(logits, 5000 + cell)
+            for rho in (0.3, 0.7):
+                Ss = (64,) if not (T == 65536 and V == 151936 and rho == 0.7) else (8, 64, 512)
+                for S in Ss:
+                    lv = W.loss_sweep_vectors(T, V, S, rho, cell=cell)
+                    d = lambda a: torch.from_numpy(a).to(dev)
+                    tg = d(lv.targets)
+                    old = H.harness_old_logp(logits, tg, lv.noise)
+                    r = reps if T * V < (1 << 32) else max(5, reps // 2)
+                    measure_loss("c5", logits, tg, old, d(lv.adv), d(lv.mask), d(lv.seg_ids), lv.S, (0.2, 0.28), dev, stream, r, out,
+                                 dlogits=dlogits, extra=dict(rho=rho))
+                cell += 1
+            del logits, dlogits
+            torch.cuda.empty_cache()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--configs", default="c1,c2,c3,c4,c5")
+    ap.add_argument("--reps", type=int, default=20)
+    ap.add_argument("--out", default=None, help="also append the JSON lines to this file")
+    ap.add_argument("--merge-only", action="store_true")
+    ap.add_argument("--quick", action="store_true", help="c5: 2x2 cells instead of 4x3")
+    ap.add_argument("--both-rules", action="store_true")
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("sweep: no CUDA device; the hot path has no CPU fallback")
+    ajt.lib()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.Stream(dev)
+    out = open(args.out, "a") if args.out else None
+    rules = (("longest", ajt.OWNER_LONGEST), ("paper", ajt.OWNER_PAPER)) if args.both_rules else (("longest", ajt.OWNER_LONGEST),)
+    cfgs = [c.strip() for c in args.configs.split(",") if c.strip()]
+    t0 = time.time()
+    for c in cfgs:
+        if c == "c1":
+            mi = W.merge_workload("c1")
+            fin = measure_merge("c1", mi, dev, stream, args.reps, out, rules)
+            if not args.merge_only:   # all merged tokens in one call, fp32 logits, V = 1024
+                chunked_loss("c1", fin, 1024, (0.2, 0.2), W.BASE_SEED, 0, "pm1", fin.N_out, 1, dev, stream, args.reps, out,
+                             dtype=torch.float32, sigma=2.0)
+        elif c == "c2":
+            mi = W.merge_workload("c2", seed=W.BASE_SEED + 1)
+            fin = measure_merge("c2", mi, dev, stream, args.reps, out, rules)
+            if not args.merge_only:
+                chunked_loss("c2", fin, 151936, (0.2, 0.28), W.BASE_SEED + 1, 1, "zscore", 40960, 3, dev, stream, args.reps, out)
+        elif c == "c3":
+            mi = W.merge_workload("c3")
+            fin = measure_merge("c3", mi, dev, stream, args.reps, out, rules)
+            if not args.merge_only:
+                chunked_loss("c3", fin, 151936, (0.2, 0.2), W.BASE_SEED + 2, 2, "zscore", 65536, 8, dev, stream,
+                             max(5, args.reps // 2), out)
+        elif c == "c4":
+            for model, mi in W.merge_workload_c4().items():
+                fin = measure_merge("c4" + model, mi, dev, stream, args.reps, out, rules)
+                if not args.merge_only:
+                    chunked_loss("c4" + model, fin, mi.meta["vocab"], (0.2, 0.2), W.BASE_SEED + 3, 3, "zscore", 65536, 4, dev, stream,
+                                 max(5, args.reps // 2), out)
+        elif c == "c5":
+            if not args.merge_only:
+                run_c5(dev, stream, args.reps, out, quick=args.quick)
+        else:
+            raise SystemExit(f"unknown config {c}")
+    print(f"# sweep done in {time.time() - t0:.1f} s", file=sys.stderr)
+
+
+if __name__ == "__main__":
+    main()

@@ -185,3 +185,28 @@ def test_host_buffer_variant():
     assert torch.equal(h["dlogits"], dev.dlogits.cpu())
     assert h["loss"] == float(dev.loss[0])
     assert np.array_equal(h["logp"], dev.logp.cpu().numpy())
+
+
+def test_segment_counts():
+    # ajt_segment_counts: N_s over a batch, chunk by chunk (accumulate), equals a host bincount; bad ids set the status
+    T, S = 100_003, 37
+    rng = np.random.default_rng(23)
+    mask = (rng.random(T) < 0.4).astype(np.uint8)
+    seg = np.sort(rng.integers(0, S, size=T)).astype(np.int32)
+    seg[rng.integers(0, T, size=500)] = rng.integers(0, S, size=500)        # some out-of-run ids
+    want = np.bincount(seg, weights=mask.astype(np.float64), minlength=S).astype(np.float32)
+    mk, sg = torch.from_numpy(mask).cuda(), torch.from_numpy(seg).cuda()
+    got = ajt.segment_counts(mk, sg, S)
+    assert np.array_equal(got.cpu().numpy(), want)
+    acc = torch.full((S,), 99.0, device="cuda")
+    st = torch.full((1,), 7, dtype=torch.int32, device="cuda")
+    ajt.segment_counts(mk[:40000], sg[:40000], S, out=acc, accumulate=False, status=st)
+    ajt.segment_counts(mk[40000:], sg[40000:], S, out=acc, accumulate=True, status=st)
+    assert np.array_equal(acc.cpu().numpy(), want) and int(st[0]) == 0
+    sg2 = sg.clone()
+    on = int(np.nonzero(mask)[0][10])
+    sg2[on] = S
+    got = ajt.segment_counts(mk, sg2, S, out=acc, status=st)
+    assert int(st[0]) & ajt.STATUS_BAD_SEG
+    assert got.sum().item() == want.sum() - 1
+    assert ajt.segment_counts(mk[:0], sg[:0], 3).cpu().tolist() == [0.0, 0.0, 0.0]
