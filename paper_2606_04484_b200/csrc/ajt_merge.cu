@@ -1,36 +1,57 @@
 // Stage (a): timeline merging (Algorithm 1) on flat token streams, sm_100a.
 //
-// Definition: DESIGN.md "O-M".  Pipeline (rows M1-M7 of the scope table):
-//   K1 merge_group_kernel    M1  stable grouping of timelines by traj_id: LSD radix sort of (traj_id - min, index),
-//                                group ids, rank in group, entry / hash-segment offsets (prefix scans)
-//   K2 merge_hash_kernel     M2  warp-cooperative prefix-hash scan, 128-bit loads.  The hash of the first p tokens of
-//                                timeline i is F_i(p) = sum_{q<p} mix(x_q) B^(q+3) mod 2^64: a sum, hence a monoid, so
-//                                every lane keeps its own partial and lanes are only combined (shuffles) where a key
-//                                is emitted: at each length L_j of an earlier same-group timeline (probe key) and at
-//                                L_i itself (full key)
-//      merge_keys_kernel         per-timeline prefix over hash segments; final (hash, len) keys and 32-bit digests
-//   K3 merge_select_kernel   M3  segmented radix sort: one CTA per group sorts its keys by digest (LSD, 8-bit digits,
-//                                stable warp-match ranking) in shared memory (global ping-pong for huge groups)
+// Definition: DESIGN.md "O-M".  Pipeline (rows M1-M7 of the scope table), 6 launches:
+//   K1 merge_group_kernel    M1  one CTA, shared-memory resident for n <= 8192: validate offsets, stable LSD radix sort of
+//                                (traj_id - min, index), group ids, rank in group, per-timeline record {first hash segment,
+//                                group start, rank, first key slot}, lengths in group order
+//   K2 merge_hash_kernel     M2  warp-cooperative prefix-hash scan, 128-bit loads, 8 vectors in flight per lane.  The hash of
+//                                the first p tokens of timeline i is F_i(p) = sum_{q<p} mix(x_q) B^(q+3) mod 2^64: a sum, hence
+//                                a monoid, so every lane keeps its own partial and lanes are only combined (shuffles) where a
+//                                key is emitted: at each length L_a of an earlier same-group timeline (probe key) and at L_i
+//                                itself (full key)
+//   K3 merge_select_kernel   M2  (one CTA per group) per-timeline prefix over its hash windows -> final (hash, len) keys
+//                            M3  segmented radix sort of the group's keys by a 32-bit digest: one MSD pass on the top 11 bits
+//                                in shared memory (<= 2048 keys: a bucket then holds the equal-key run, mean occupancy < 1,
+//                                and keys inside it are compared exactly); 4 LSD passes through global memory above that
 //   K4   (same kernel)       M4  per full key: walk its equal-key run, pick the extender by the owner rule
-//   K6 merge_compact_kernel  M6  survivors in original order, scans -> merged_offsets/origin/traj, owner, member lists
-//   K5/K7 merge_scatter_kernel M5+M7  fused: every merged sequence is streamed once; each absorbed member is compared
-//                                token-by-token against its owner (exact verification) while tokens / mask-OR / src /
-//                                old_logp are written.  A mismatch (a hash collision) raises ctrl->collision.
-//   Repair (enqueued always, exits at once unless ctrl->collision): K4 with exact comparison of every candidate it
-//   accepts, then K6 and K7 again.  Hash collisions can therefore never change the result.
+//   K6 merge_compact_kernel  M6  one CTA, one fused scan: survivors in original order -> merged_offsets/origin/traj, owner,
+//                                tile table
+//   K5/K7 merge_scatter_kernel M5+M7  fused: every merged sequence is streamed once in 512-token warp tiles; each absorbed
+//                                member is compared token-by-token against its owner (exact verification) while tokens /
+//                                mask-OR / src / old_logp are written with 16-byte stores.  A mismatch (a hash collision)
+//                                raises ctrl->collision.
+//   merge_repair_kernel      M5  one cooperative launch that exits at once unless ctrl->collision: K4 with exact comparison of
+//                                every candidate it accepts, grid barrier, K6, grid barrier, K7.  Hash collisions can therefore
+//                                never change the result.
+#include <cooperative_groups.h>
+
 #include "ajt_common.cuh"
 
 namespace {
 
 using namespace ajt;
+namespace cg = cooperative_groups;
 
 constexpr int kHSeg = 2048;        // hash-scan window: 2048 tokens = 16 steps x 32 lanes x 4 tokens
-constexpr int kTile = 1024;        // scatter tile (positions per warp-task)
+constexpr int kHSegLog = 11;
+constexpr int kTile = 256;         // scatter tile (positions per warp task): 2 steps x 32 lanes x 4 tokens
 constexpr uint64_t kB = 0x9E3779B97F4A7C15ull;       // odd multiplier of the polynomial hash
 constexpr uint64_t kMixAdd = 0x632BE59BD9B4E019ull;  // so that token 0 is not the additive identity
 constexpr uint32_t kFatal = AJT_STATUS_BAD_OFFSETS | AJT_STATUS_ZERO_LEN | AJT_STATUS_PROBE_CAPACITY;
 constexpr int kSelThreads = 256;
 constexpr int kSelSmemKeys = 2048;  // groups with more keys than this sort through global memory
+constexpr int kSelBucketBits = 11;
+constexpr int kSelBuckets = 1 << kSelBucketBits;
+constexpr int kSelCacheK = 256;     // per-timeline facts of groups up to this size are staged in shared memory
+constexpr int kGrpSmemN = 8192;     // batches up to this many timelines are grouped entirely in shared memory
+
+constexpr uint64_t inv64(uint64_t b) {  // b^-1 mod 2^64 (b odd): Newton, 3 correct bits double every step
+    uint64_t x = b;
+    for (int i = 0; i < 6; ++i) x *= 2 - b * x;
+    return x;
+}
+constexpr uint64_t kBinv = inv64(kB);
+static_assert(kB * kBinv == 1ull, "modular inverse");
 
 struct MergeParams {
     const int32_t* tokens;
@@ -54,39 +75,32 @@ struct MergeParams {
     int64_t* counts;
     // workspace
     AjtCtrl* ctrl;
-    uint32_t* skey[2];     // [n] radix ping-pong keys (traj_id - min)
-    uint32_t* sval[2];     // [n] radix ping-pong values (timeline index)
-    int32_t* perm;         // [n] sorted position -> timeline index
-    int32_t* gid_sorted;   // [n] group id of each sorted position
-    int32_t* grp_start;    // [n+1] first sorted position of each group
-    int32_t* grp_ent;      // [n+1] first entry of each group
-    int32_t* t_rank;       // [n] rank of timeline i inside its group (input order)
-    int32_t* t_gid;        // [n]
-    int32_t* t_entbase;    // [n] first entry of timeline i: entries (i, a), a = 0..rank
-    int32_t* seg_base;     // [n+1] first hash segment of timeline i
-    uint64_t* seg_part;    // [nseg_cap] per-segment partial sums, then exclusive prefixes per timeline
-    uint64_t* ent_hash;    // [E_cap]
-    int32_t* ent_len;      // [E_cap] prefix length of the key, -1 if invalid (L_a > L_i)
-    uint32_t* ent_dig;     // [E_cap] 32-bit digest of (hash, len)
-    uint32_t* ent_idx;     // [E_cap] sorted order: local entry index inside the group
+    uint32_t* gbuf[5];     // [n+1] each: global stand-ins for the group kernel's shared arrays when n > kGrpSmemN
+    int32_t* perm;         // [n] sorted position -> timeline index (groups contiguous, input order inside a group)
+    int32_t* glen;         // [n] sorted position -> timeline length
+    int32_t* grp_start;    // [G+1] first sorted position of each group
+    int32_t* grp_ent;      // [G+1] first key slot of each group
+    int4* tl_rec;          // [n] {first hash segment, group start (sorted position), rank in group, first key slot}
+    uint64_t* seg_part;    // [nseg_cap] per-window partial sums, then exclusive prefixes per timeline
+    uint64_t* ent_hash;    // [E_cap] key slot (i, a), a = 0..rank_i: in-window partial, then the final prefix hash
+    uint32_t* ent_dig;     // [E_cap] global sort path: digests / order ping-pong
+    uint32_t* ent_idx;     // [E_cap]
     uint32_t* tmp_dig;     // [E_cap]
     uint32_t* tmp_idx;     // [E_cap]
     uint8_t* absorbed;     // [n]
+    uint8_t* link_bad;     // [n] 1: timeline i was compared with its in-group predecessor (hash pass) and is NOT an extension of it
+    uint8_t* needv;        // [n] 1: absorbed timeline whose owner is not implied by a chain of verified predecessor links
     int32_t* owner_tl;     // [n] owning timeline (itself for survivors)
+    int32_t* cand;         // [n] staging of the LONGEST owner while owner_tl is still being read
     int32_t* midx;         // [n] merged index of survivors, -1 otherwise
-    int32_t* mem_cnt;      // [n] number of absorbed members owned by timeline i
-    int32_t* mem_off;      // [n+1] by merged index
-    int32_t* mem_cur;      // [n] fill cursors by merged index
-    int32_t* mem_list;     // [n] absorbed members, grouped by owner
-    int32_t* tile_base;    // [n+1] by merged index
+    int32_t* tile_base;    // [M+1] first scatter tile of each merged sequence
     int32_t E_cap;
     int32_t nseg_cap;
     int32_t mis;           // (address of tokens / 4) mod 4: element misalignment of the token array vs 16 bytes
 };
 
 struct MergeWs {
-    size_t ctrl, skey0, skey1, sval0, sval1, gid_sorted, grp_start, grp_ent, t_rank, t_gid, t_entbase, seg_base, seg_part,
-        absorbed, owner_tl, midx, mem_cnt, mem_off, mem_cur, mem_list, tile_base, ent, fixed_total;
+    size_t ctrl, gbuf[5], perm, glen, grp_start, grp_ent, tl_rec, seg_part, absorbed, link_bad, needv, owner_tl, cand, midx, tile_base, ent;
 };
 __host__ inline size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
 __host__ inline int32_t nseg_capacity(int32_t n, int64_t N) { return (int32_t)(N / kHSeg + 2 * (int64_t)n + 2); }
@@ -94,20 +108,20 @@ __host__ inline int32_t nseg_capacity(int32_t n, int64_t N) { return (int32_t)(N
 __host__ MergeWs merge_ws_layout(int32_t n, int64_t N) {
     MergeWs w;
     size_t o = 0;
-    const size_t n4 = a256(((size_t)n + 1) * 4);
+    const size_t n4 = a256(((size_t)n + 2) * 4);
     w.ctrl = o; o += 256;
-    w.skey0 = o; o += n4; w.skey1 = o; o += n4; w.sval0 = o; o += n4; w.sval1 = o; o += n4;
-    w.gid_sorted = o; o += n4; w.grp_start = o; o += n4; w.grp_ent = o; o += n4;
-    w.t_rank = o; o += n4; w.t_gid = o; o += n4; w.t_entbase = o; o += n4; w.seg_base = o; o += n4;
+    for (int k = 0; k < 5; ++k) { w.gbuf[k] = o; o += n4; }
+    w.perm = o; o += n4; w.glen = o; o += n4; w.grp_start = o; o += n4; w.grp_ent = o; o += n4;
+    w.tl_rec = o; o += a256(((size_t)n + 1) * 16);
     w.seg_part = o; o += a256((size_t)nseg_capacity(n, N) * 8);
     w.absorbed = o; o += a256((size_t)n + 1);
-    w.owner_tl = o; o += n4; w.midx = o; o += n4; w.mem_cnt = o; o += n4; w.mem_off = o; o += n4; w.mem_cur = o; o += n4;
-    w.mem_list = o; o += n4; w.tile_base = o; o += n4;
+    w.link_bad = o; o += a256((size_t)n + 1);
+    w.needv = o; o += a256((size_t)n + 1);
+    w.owner_tl = o; o += n4; w.cand = o; o += n4; w.midx = o; o += n4; w.tile_base = o; o += n4;
     w.ent = o;
-    w.fixed_total = o;
     return w;
 }
-constexpr size_t kEntBytes = 8 + 4 + 4 + 4 + 4 + 4;  // hash, len, dig, idx, tmp_dig, tmp_idx  (< 32, header promises 32)
+constexpr size_t kEntBytes = 32;  // per key slot: hash 8, dig 4, idx 4, tmp_dig 4, tmp_idx 4 = 24 used; ajt.h promises 32 per pair
 
 __device__ __forceinline__ bool fatal(const MergeParams& p) { return (p.ctrl->status & kFatal) != 0; }
 
@@ -120,7 +134,7 @@ __device__ __forceinline__ uint64_t pow64(uint64_t b, uint64_t e) {
     }
     return r;
 }
-__device__ __forceinline__ uint64_t mix_tok(int32_t x) { return (uint64_t)(uint32_t)x + kMixAdd; }
+__device__ __forceinline__ uint64_t powB(int64_t e) { return e >= 0 ? pow64(kB, (uint64_t)e) : pow64(kBinv, (uint64_t)(-e)); }
 __device__ __forceinline__ uint32_t digest32(uint64_t h, int32_t len) {
     uint64_t z = h ^ ((uint64_t)(uint32_t)len * 0xD6E8FEB86659FD93ull);
     z ^= z >> 32;
@@ -133,39 +147,71 @@ __device__ __forceinline__ uint64_t warp_sum_u64(uint64_t v) {
     for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
+__device__ __forceinline__ int64_t tl_len(const MergeParams& p, int i) { return p.offsets[i + 1] - p.offsets[i]; }
+
+// Last index i in [0, n) with key(i) <= x, for a non-decreasing key with key(0) <= x: warp-cooperative 32-ary search
+// (3 dependent loads for n <= 32768 instead of 15).
+template <class F>
+__device__ __forceinline__ int warp_search_last_le(int n, int64_t x, F key) {
+    const int lane = threadIdx.x & 31;
+    int lo = 0, hi = n;  // key(lo) <= x; hi == n or key(hi) > x
+    while (hi - lo > 1) {
+        const int step = (hi - lo + 31) >> 5;
+        const int idx = lo + (lane + 1) * step;
+        const bool le = idx < hi && (int64_t)key(idx) <= x;
+        const int cnt = __popc(__ballot_sync(0xffffffffu, le));
+        const int nlo = lo + cnt * step;
+        hi = min(hi, nlo + step);
+        lo = nlo;
+    }
+    return lo;
+}
 
 // ---------------------------------------------------------------------------------------- block-level building blocks
 
-// Exclusive scan of f(i), i in [0,n), by one CTA of NT threads; g(i, exclusive_prefix, value) consumes it.  Returns the
-// total to every thread.  One __syncthreads per tile of NT (double-buffered warp totals).
+// Exclusive scan of the pair f(i) = (a, b), i in [0,n), by one CTA of NT threads; g(i, ex_a, ex_b, a, b) consumes it.
+// The loads of the next tile (f) are issued before the current tile is scanned, so their latency overlaps.  Returns the
+// totals to every thread.  One __syncthreads per tile of NT (double-buffered warp totals).
+struct I2 {
+    int64_t a, b;
+};
 template <int NT, class F, class G>
-__device__ __forceinline__ int64_t block_scan(int n, F f, G g, int64_t (*s_w)[NT / 32]) {
+__device__ __forceinline__ I2 block_scan2(int n, F f, G g, int64_t (*s_w)[2][NT / 32]) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    int64_t base = 0;
+    I2 base = {0, 0};
     int buf = 0;
+    I2 nxt = tid < n ? f(tid) : I2{0, 0};
     for (int i0 = 0; i0 < n; i0 += NT, buf ^= 1) {
         const int i = i0 + tid;
-        const int64_t v = i < n ? (int64_t)f(i) : 0;
-        int64_t inc = v;
+        const I2 v = nxt;
+        nxt = i + NT < n ? f(i + NT) : I2{0, 0};
+        int64_t ia = v.a, ib = v.b;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const int64_t t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
+            const int64_t ta = __shfl_up_sync(0xffffffffu, ia, o), tb = __shfl_up_sync(0xffffffffu, ib, o);
+            if (lane >= o) { ia += ta; ib += tb; }
         }
-        if (lane == 31) s_w[buf][warp] = inc;
+        if (lane == 31) { s_w[buf][0][warp] = ia; s_w[buf][1][warp] = ib; }
         __syncthreads();
-        int64_t pre = 0, tot = 0;
+        int64_t pa = 0, pb = 0, ta = 0, tb = 0;
 #pragma unroll
         for (int w = 0; w < NT / 32; ++w) {
-            const int64_t c = s_w[buf][w];
-            if (w < warp) pre += c;
-            tot += c;
+            const int64_t ca = s_w[buf][0][w], cb = s_w[buf][1][w];
+            if (w < warp) { pa += ca; pb += cb; }
+            ta += ca; tb += cb;
         }
-        if (i < n) g(i, base + pre + inc - v, v);
-        base += tot;
+        if (i < n) g(i, base.a + pa + ia - v.a, base.b + pb + ib - v.b, v.a, v.b);
+        base.a += ta; base.b += tb;
     }
     __syncthreads();
     return base;
+}
+template <int NT, class F, class G>
+__device__ __forceinline__ int64_t block_scan(int n, F f, G g, int64_t (*s_w)[2][NT / 32]) {
+    return block_scan2<NT>(
+               n, [&](int i) { return I2{(int64_t)f(i), 0}; }, [&](int i, int64_t ex, int64_t, int64_t v, int64_t) { g(i, ex, v); },
+               s_w)
+        .a;
 }
 
 template <int NW>
@@ -236,14 +282,25 @@ __device__ void radix_pass(const uint32_t* kin, const uint32_t* vin, uint32_t* k
 // ---------------------------------------------------------------------------------------- K1: group (M1)
 
 __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) {
+    extern __shared__ __align__(16) uint8_t g_dyn[];
     __shared__ RadixScratch<32> sc;
-    __shared__ int64_t s_w[2][32];
+    __shared__ int64_t s_w[2][2][32];
     __shared__ int s_min, s_max;
     __shared__ uint32_t s_bad;
     const int tid = threadIdx.x, n = p.n;
+    // five [n+1] work arrays: shared memory for n <= kGrpSmemN, the workspace otherwise
+    uint32_t* buf[5];
+    {
+        const size_t nn = ((size_t)n + 4) & ~(size_t)3;
+        for (int k = 0; k < 5; ++k) buf[k] = n <= kGrpSmemN ? reinterpret_cast<uint32_t*>(g_dyn) + k * nn : p.gbuf[k];
+    }
+    uint32_t* kb[2] = {buf[0], buf[1]};
+    uint32_t* vb[2] = {buf[2], buf[3]};
+    int32_t* nsg = reinterpret_cast<int32_t*>(buf[4]);
+    if (tid < (int)(sizeof(AjtCtrl) / 4)) reinterpret_cast<uint32_t*>(p.ctrl)[tid] = 0;   // fresh control block
     if (tid == 0) { s_min = INT32_MAX; s_max = INT32_MIN; s_bad = 0; }
     __syncthreads();
-    // validate offsets; min / max traj id
+    // validate offsets; min / max traj id; hash windows per timeline
     int lmin = INT32_MAX, lmax = INT32_MIN;
     uint32_t bad = 0;
     for (int i = tid; i < n; i += 1024) {
@@ -253,6 +310,10 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
         const int t = p.traj_ids[i];
         lmin = min(lmin, t);
         lmax = max(lmax, t);
+        kb[0][i] = (uint32_t)t;
+        vb[0][i] = (uint32_t)i;
+        p.link_bad[i] = 0;
+        nsg[i] = (int32_t)(((b - 1 + p.mis) >> kHSegLog) - ((a + p.mis) >> kHSegLog) + 1);
     }
     if (tid == 0 && (p.offsets[0] != 0 || p.offsets[n] != p.N)) bad |= AJT_STATUS_BAD_OFFSETS;
     if (bad) atomicOr(&s_bad, bad);
@@ -264,54 +325,49 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
     }
     const int tmin = s_min;
     const uint32_t range = n ? (uint32_t)s_max - (uint32_t)tmin : 0u;
-    for (int i = tid; i < n; i += 1024) {
-        p.skey[0][i] = (uint32_t)p.traj_ids[i] - (uint32_t)tmin;
-        p.sval[0][i] = (uint32_t)i;
-    }
+    for (int i = tid; i < n; i += 1024) kb[0][i] -= (uint32_t)tmin;
     __syncthreads();
     int cur = 0;
     for (int shift = 0; shift < 32 && (range >> shift) != 0; shift += 8) {
-        radix_pass<32>(p.skey[cur], p.sval[cur], p.skey[cur ^ 1], p.sval[cur ^ 1], n, shift, sc);
+        radix_pass<32>(kb[cur], vb[cur], kb[cur ^ 1], vb[cur ^ 1], n, shift, sc);
         cur ^= 1;
         __syncthreads();
     }
-    const uint32_t* key = p.skey[cur];
-    const uint32_t* val = p.sval[cur];
+    const uint32_t* key = kb[cur];
+    const uint32_t* val = vb[cur];
+    uint32_t* gid = kb[cur ^ 1];    // [pos] group id
+    uint32_t* gsv = vb[cur ^ 1];    // [g]   first sorted position of group g
     // group ids and group starts
     const int G = (int)block_scan<1024>(
         n, [&](int pos) { return (pos == 0 || key[pos] != key[pos - 1]) ? 1 : 0; },
         [&](int pos, int64_t ex, int64_t v) {
             const int g = (int)(ex + v) - 1;
-            p.gid_sorted[pos] = g;
+            gid[pos] = (uint32_t)g;
             p.perm[pos] = (int32_t)val[pos];
-            if (v) p.grp_start[g] = pos;
+            if (v) { gsv[g] = (uint32_t)pos; p.grp_start[g] = pos; }
         },
         s_w);
-    if (tid == 0) p.grp_start[G] = n;
+    if (tid == 0) { gsv[G] = (uint32_t)n; p.grp_start[G] = n; }
     __syncthreads();
-    // rank in group; entries (i, a), a = 0..rank  ->  rank+1 entries per timeline
+    uint32_t* gsz = kb[cur];        // [i] size of the group of timeline i (the sorted keys are no longer needed)
+    int32_t* rec = reinterpret_cast<int32_t*>(p.tl_rec);
+    // rank in group; key slots (i, a), a = 0..rank  ->  rank+1 slots per timeline
     const int64_t E = block_scan<1024>(
-        n, [&](int pos) { return pos - p.grp_start[p.gid_sorted[pos]] + 1; },
+        n, [&](int pos) { return (int)(pos - gsv[gid[pos]]) + 1; },
         [&](int pos, int64_t ex, int64_t v) {
-            const int i = p.perm[pos], g = p.gid_sorted[pos];
-            p.t_rank[i] = (int)v - 1;
-            p.t_gid[i] = g;
-            p.t_entbase[i] = (int32_t)ex;
+            const int i = (int)val[pos], g = (int)gid[pos];
+            rec[4 * i + 1] = (int32_t)gsv[g];
+            rec[4 * i + 2] = (int32_t)v - 1;
+            rec[4 * i + 3] = (int32_t)ex;
+            gsz[i] = gsv[g + 1] - gsv[g];
             if (v == 1) p.grp_ent[g] = (int32_t)ex;
+            p.glen[pos] = (int32_t)tl_len(p, i);
         },
         s_w);
-    // hash segments: aligned windows of kHSeg tokens intersected with each timeline (skipped for singleton groups)
+    // hash segments: aligned windows of kHSeg tokens intersected with each timeline (none for singleton groups)
     const int64_t nseg = block_scan<1024>(
-        n,
-        [&](int i) {
-            const int g = p.t_gid[i];
-            if (p.grp_start[g + 1] - p.grp_start[g] < 2) return 0;
-            const int64_t a = p.offsets[i] + p.mis, b = p.offsets[i + 1] - 1 + p.mis;
-            return (int)(b / kHSeg - a / kHSeg + 1);
-        },
-        [&](int i, int64_t ex, int64_t) { p.seg_base[i] = (int32_t)ex; }, s_w);
+        n, [&](int i) { return gsz[i] < 2 ? 0 : nsg[i]; }, [&](int i, int64_t ex, int64_t) { rec[4 * i] = (int32_t)ex; }, s_w);
     if (tid == 0) {
-        p.seg_base[n] = (int32_t)nseg;
         p.grp_ent[G] = (int32_t)min(E, (int64_t)INT32_MAX);
         p.ctrl->n_groups = G;
         p.ctrl->n_entries = (int32_t)min(E, (int64_t)INT32_MAX);
@@ -322,138 +378,158 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
 
 // ---------------------------------------------------------------------------------------- K2: prefix-hash scan (M2)
 
-__global__ void __launch_bounds__(256) merge_hash_kernel(const MergeParams p) {
+// term of token x at slot e of a 4-token vector, before the vector's weight: mix(x) B^e = x B^e + c B^e.  x is 32 bits, so the
+// product is a 32x64 multiply (2 IMADs) with the constant folded into the addend.
+template <int E>
+__device__ __forceinline__ uint64_t tok_term(int32_t x) {
+    constexpr uint64_t B2 = kB * kB, B3 = B2 * kB;
+    constexpr uint64_t BE = E == 0 ? 1ull : E == 1 ? kB : E == 2 ? B2 : B3;
+    return (uint64_t)(uint32_t)x * BE + kMixAdd * BE;
+}
+
+// Rare path, kept out of line so the streaming loop stays small in the instruction cache: writes the in-window partial of
+// every key whose prefix ends inside step s (positions [win0 + 128 s, +128)).  t0..t3 are this lane's four terms of the step
+// (already zero outside the timeline), acc its sum over the earlier steps, pw the weight of its vector.
+__device__ __noinline__ void hash_emit(uint64_t* __restrict__ ent_hash, const int32_t* __restrict__ gln, int rank, int ebase,
+                                       int64_t win0, int Li, int s, int64_t q, uint64_t t0, uint64_t t1, uint64_t t2, uint64_t t3,
+                                       uint64_t acc, uint64_t pw) {
+    const int lane = threadIdx.x & 31;
+    for (int a0 = 0; a0 <= rank; a0 += 32) {
+        const int a = a0 + lane;
+        int64_t Lp = -1;
+        if (a <= rank) {
+            Lp = gln[a];
+            const int64_t rel = Lp - 1 - win0;
+            if (!(Lp <= Li && rel >= 0 && (rel >> 7) == s)) Lp = -1;
+        }
+        unsigned hits = __ballot_sync(0xffffffffu, Lp >= 0);
+        while (hits) {
+            const int src = __ffs(hits) - 1;
+            hits &= hits - 1;
+            const int64_t P = __shfl_sync(0xffffffffu, Lp, src);
+            const uint64_t part = (q < P ? t0 : 0) + (q + 1 < P ? t1 : 0) + (q + 2 < P ? t2 : 0) + (q + 3 < P ? t3 : 0);
+            const uint64_t tot = warp_sum_u64(acc + part * pw);
+            if (lane == 0) ent_hash[ebase + a0 + src] = tot;
+        }
+    }
+}
+
+// One 2048-token window of timeline i.  Returns the warp-total of the window's terms.  kInterior: the window lies entirely
+// inside the timeline (no masking needed).  kLink: the window also holds positions of the in-group predecessor (length Lprev
+// <= L_i, tokens at tprev): they are compared exactly with this timeline's tokens while both stream by (the predecessor was
+// hashed moments ago, so its tokens come from L2); `diff` collects any difference.  Four batches of four 16-byte loads.
+template <bool kInterior, bool kLink>
+__device__ __forceinline__ uint64_t hash_window(const MergeParams& p, int lane, int64_t off, int Li, int64_t win0, uint64_t pw,
+                                                uint64_t B128, uint32_t stepmask, const int32_t* __restrict__ gln, int rank,
+                                                int ebase, const int32_t* __restrict__ tprev, int Lprev, uint32_t& diff) {
+    const int32_t* __restrict__ tok = p.tokens;
+    const int64_t q0 = win0 + lane * 4;   // timeline position of this lane's first slot in step 0
+    uint64_t acc = 0;
+#pragma unroll 1
+    for (int h = 0; h < 4; ++h) {
+        if (!kInterior && win0 + 512 * (int64_t)h >= Li) break;
+        int4 x[4];
+        int32_t y[4][4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int64_t q = q0 + 128 * (int64_t)(h * 4 + u);
+            const int64_t e = off + q;  // element index; 16-byte aligned address
+            if (kInterior) x[u] = __ldg(reinterpret_cast<const int4*>(tok + e));
+            else {
+                x[u] = make_int4(0, 0, 0, 0);
+                if (q + 3 >= 0 && q < Li) {
+                    if (e >= 0 && e + 3 < p.N) x[u] = __ldg(reinterpret_cast<const int4*>(tok + e));
+                    else {
+                        if (e >= 0 && e < p.N) x[u].x = tok[e];
+                        if (e + 1 >= 0 && e + 1 < p.N) x[u].y = tok[e + 1];
+                        if (e + 2 >= 0 && e + 2 < p.N) x[u].z = tok[e + 2];
+                        if (e + 3 >= 0 && e + 3 < p.N) x[u].w = tok[e + 3];
+                    }
+                }
+            }
+            if (kLink) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) y[u][k] = (q + k >= 0 && q + k < Lprev) ? __ldg(tprev + q + k) : 0;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int s = h * 4 + u;
+            const int64_t q = q0 + 128 * (int64_t)s;
+            if (kLink) {
+                if (q >= 0 && q < Lprev) diff |= (uint32_t)(y[u][0] ^ x[u].x);
+                if (q + 1 >= 0 && q + 1 < Lprev) diff |= (uint32_t)(y[u][1] ^ x[u].y);
+                if (q + 2 >= 0 && q + 2 < Lprev) diff |= (uint32_t)(y[u][2] ^ x[u].z);
+                if (q + 3 >= 0 && q + 3 < Lprev) diff |= (uint32_t)(y[u][3] ^ x[u].w);
+            }
+            uint64_t t0 = tok_term<0>(x[u].x), t1 = tok_term<1>(x[u].y), t2 = tok_term<2>(x[u].z), t3 = tok_term<3>(x[u].w);
+            if (!kInterior) {
+                if (!(q >= 0 && q < Li)) t0 = 0;
+                if (!(q + 1 >= 0 && q + 1 < Li)) t1 = 0;
+                if (!(q + 2 >= 0 && q + 2 < Li)) t2 = 0;
+                if (!(q + 3 >= 0 && q + 3 < Li)) t3 = 0;
+            }
+            if (stepmask & (1u << s)) hash_emit(p.ent_hash, gln, rank, ebase, win0, Li, s, q, t0, t1, t2, t3, acc, pw);
+            acc += ((t0 + t1) + (t2 + t3)) * pw;
+            pw *= B128;
+        }
+    }
+    return warp_sum_u64(acc);
+}
+
+__global__ void __launch_bounds__(256, 2) merge_hash_kernel(const MergeParams p) {
     if (fatal(p)) return;
     const int lane = threadIdx.x & 31;
     const int wglobal = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
     const int nseg = p.ctrl->n_hash_segs, n = p.n;
-    const uint64_t B2 = kB * kB, B3 = B2 * kB, B128 = pow64(kB, 128);
+    // Striped windows: at any moment the grid works on ~nwarps consecutive windows (a front of ~20 MB that sweeps the token
+    // array once), so a timeline's in-group predecessor, hashed a little earlier, is still in L2 when it is compared.
+    const uint64_t LB = pow64(kB, (uint64_t)(4 * lane)), B128 = pow64(kB, 128);
+    auto seg_base = [&](int i) { return reinterpret_cast<const int32_t*>(p.tl_rec)[4 * i]; };
     for (int sidx = wglobal; sidx < nseg; sidx += nwarps) {
-        // timeline of this segment: last i with seg_base[i] <= sidx
-        int lo = 0, hi = n;
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (p.seg_base[mid] <= sidx) lo = mid; else hi = mid;
-        }
-        const int i = lo;
+        const int i = warp_search_last_le(n, sidx, seg_base);
+        const int4 rec = p.tl_rec[i];
         const int64_t off = p.offsets[i];
         const int Li = (int)(p.offsets[i + 1] - off);
-        const int64_t w = (off + p.mis) / kHSeg + (sidx - p.seg_base[i]);   // window index (virtual element space)
-        const int64_t win0 = w * kHSeg - p.mis - off;                        // timeline position of the window's first slot
-        const int g = p.t_gid[i], rank = p.t_rank[i];
-        const int32_t* gl = p.perm + p.grp_start[g];
-        const int ebase = p.t_entbase[i];
+        const int64_t wfirst = (off + p.mis) >> kHSegLog;
+        // the in-group predecessor, if this timeline can extend it (the usual case: each call resends the context)
+        int Lprev = 0;
+        const int32_t* tprev = nullptr;
+        if (rec.z > 0) {
+            const int jp = p.perm[rec.y + rec.z - 1];
+            const int64_t op = p.offsets[jp];
+            const int lp = (int)(p.offsets[jp + 1] - op);
+            if (lp <= Li) { Lprev = lp; tprev = p.tokens + op; }
+        }
+        const int64_t win0 = ((wfirst + (sidx - rec.x)) << kHSegLog) - p.mis - off;   // timeline position of the window's first slot
+        const uint64_t X = powB(win0 + 3);   // B^(win0 + 3)
+        const int rank = rec.z, ebase = rec.w;
+        const int32_t* gln = p.glen + rec.y;
         // which 128-token steps of this window hold the end of a requested prefix (L_a of an earlier member, or L_i)
         uint32_t stepmask = 0;
         for (int a0 = 0; a0 <= rank; a0 += 32) {
             const int a = a0 + lane;
             if (a <= rank) {
-                const int j = gl[a];
-                const int64_t Lp = p.offsets[j + 1] - p.offsets[j];
+                const int64_t Lp = gln[a];
                 const int64_t rel = Lp - 1 - win0;
                 if (Lp <= Li && rel >= 0 && rel < kHSeg) stepmask |= 1u << (int)(rel >> 7);
             }
         }
         stepmask = __reduce_or_sync(0xffffffffu, stepmask);
-
-        // per-lane weight B^(q+3) of its first token slot, from the first step where q + 3 >= 0
-        const int64_t q0 = win0 + lane * 4;
-        const int s0 = q0 + 3 >= 0 ? 0 : (int)((-3 - q0 + 127) >> 7);
-        uint64_t pw = pow64(kB, (uint64_t)(q0 + 128 * (int64_t)s0 + 3));
-        uint64_t acc = 0;
-        const int32_t* tok = p.tokens;
-#pragma unroll 4
-        for (int s = 0; s < kHSeg / 128; ++s) {
-            if (win0 + 128 * (int64_t)s >= Li) break;  // warp-uniform: the whole step lies beyond the timeline
-            const int64_t q = q0 + 128 * (int64_t)s;   // position of this lane's first slot
-            const int64_t e = off + q;                  // element index, 16-byte aligned address
-            int4 x = make_int4(0, 0, 0, 0);
-            if (q + 3 >= 0 && q < Li) {
-                if (e >= 0 && e + 3 < p.N) x = __ldg(reinterpret_cast<const int4*>(tok + e));
-                else {
-                    if (e >= 0 && e < p.N) x.x = tok[e];
-                    if (e + 1 >= 0 && e + 1 < p.N) x.y = tok[e + 1];
-                    if (e + 2 >= 0 && e + 2 < p.N) x.z = tok[e + 2];
-                    if (e + 3 >= 0 && e + 3 < p.N) x.w = tok[e + 3];
-                }
-            }
-            if (s > s0) pw *= B128;
-            const bool v0 = q >= 0 && q < Li, v1 = q + 1 >= 0 && q + 1 < Li, v2 = q + 2 >= 0 && q + 2 < Li,
-                       v3 = q + 3 >= 0 && q + 3 < Li;
-            const uint64_t m0 = v0 ? mix_tok(x.x) : 0, m1 = v1 ? mix_tok(x.y) : 0, m2 = v2 ? mix_tok(x.z) : 0,
-                           m3 = v3 ? mix_tok(x.w) : 0;
-            if (stepmask & (1u << s)) {
-                // emit every key whose prefix ends inside this step
-                for (int a0 = 0; a0 <= rank; a0 += 32) {
-                    const int a = a0 + lane;
-                    int64_t Lp = -1;
-                    if (a <= rank) {
-                        const int j = gl[a];
-                        Lp = p.offsets[j + 1] - p.offsets[j];
-                        const int64_t rel = Lp - 1 - win0;
-                        if (!(Lp <= Li && rel >= 0 && (rel >> 7) == s)) Lp = -1;
-                    }
-                    unsigned hits = __ballot_sync(0xffffffffu, Lp >= 0);
-                    while (hits) {
-                        const int src = __ffs(hits) - 1;
-                        hits &= hits - 1;
-                        const int64_t P = __shfl_sync(0xffffffffu, Lp, src);
-                        uint64_t part = 0;
-                        if (s >= s0) {
-                            const uint64_t t0 = q < P ? m0 : 0, t1 = q + 1 < P ? m1 : 0, t2 = q + 2 < P ? m2 : 0,
-                                           t3 = q + 3 < P ? m3 : 0;
-                            part = (t0 + t1 * kB + t2 * B2 + t3 * B3) * pw;
-                        }
-                        const uint64_t tot = warp_sum_u64(acc + part);
-                        if (lane == 0) p.ent_hash[ebase + a0 + src] = tot;
-                    }
-                }
-            }
-            if (s >= s0) acc += (m0 + m1 * kB + m2 * B2 + m3 * B3) * pw;
-        }
-        const uint64_t tot = warp_sum_u64(acc);
+        const uint64_t pw = X * LB;
+        const bool interior = win0 >= 0 && win0 + kHSeg <= Li, link = win0 < Lprev;
+        uint32_t diff = 0;
+        uint64_t tot;
+        if (interior && link) tot = hash_window<true, true>(p, lane, off, Li, win0, pw, B128, stepmask, gln, rank, ebase, tprev, Lprev, diff);
+        else if (interior) tot = hash_window<true, false>(p, lane, off, Li, win0, pw, B128, stepmask, gln, rank, ebase, tprev, Lprev, diff);
+        else if (link) tot = hash_window<false, true>(p, lane, off, Li, win0, pw, B128, stepmask, gln, rank, ebase, tprev, Lprev, diff);
+        else tot = hash_window<false, false>(p, lane, off, Li, win0, pw, B128, stepmask, gln, rank, ebase, tprev, Lprev, diff);
         if (lane == 0) p.seg_part[sidx] = tot;
+        if (link && __any_sync(0xffffffffu, diff != 0) && lane == 0) p.link_bad[i] = 1;
     }
 }
 
-// per timeline: exclusive prefix over its hash segments, then the final keys of its entries (i, a), a = 0..rank
-__global__ void __launch_bounds__(256) merge_keys_kernel(const MergeParams p) {
-    if (fatal(p)) return;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= p.n) return;
-    const int sb = p.seg_base[i], se = p.seg_base[i + 1];
-    uint64_t run = 0;
-    for (int s = sb; s < se; ++s) {
-        const uint64_t v = p.seg_part[s];
-        p.seg_part[s] = run;
-        run += v;
-    }
-    if (se == sb) return;  // singleton group: no keys needed
-    const int64_t off = p.offsets[i];
-    const int Li = (int)(p.offsets[i + 1] - off);
-    const int64_t w_first = (off + p.mis) / kHSeg;
-    const int g = p.t_gid[i], rank = p.t_rank[i];
-    const int32_t* gl = p.perm + p.grp_start[g];
-    const int ebase = p.t_entbase[i];
-    const bool weak = (p.flags & AJT_MERGE_WEAK_HASH) != 0;
-    for (int a = 0; a <= rank; ++a) {
-        const int j = gl[a];
-        const int64_t Lp = p.offsets[j + 1] - p.offsets[j];
-        const int e = ebase + a;
-        if (Lp > Li) {
-            p.ent_len[e] = -1;
-            p.ent_hash[e] = 0;
-            continue;
-        }
-        const int64_t widx = (off + Lp - 1 + p.mis) / kHSeg - w_first;
-        uint64_t h = p.seg_part[sb + widx] + p.ent_hash[e];
-        if (weak) h &= 0xFull;
-        p.ent_hash[e] = h;
-        p.ent_len[e] = (int32_t)Lp;
-    }
-}
-
-// ---------------------------------------------------------------------------------------- K3 + K4: sort + select (M3, M4)
+// ---------------------------------------------------------------------------------------- K3 + K4: keys, sort, select (M2-M4)
 
 __device__ bool tokens_extend(const MergeParams& p, int i, int j) {  // exact: tokens_i[0:L_j] == tokens_j, L_i >= L_j
     const int64_t oi = p.offsets[i], oj = p.offsets[j];
@@ -464,7 +540,7 @@ __device__ bool tokens_extend(const MergeParams& p, int i, int j) {  // exact: t
     return true;
 }
 
-// local entry index -> rank of the probing timeline: entries of rank b occupy [b(b+1)/2, b(b+1)/2 + b]
+// local key slot -> rank of the probing timeline: slots of rank b occupy [b(b+1)/2, b(b+1)/2 + b]
 __device__ __forceinline__ int rank_of_local(uint32_t l) {
     int b = (int)((sqrtf(8.f * (float)l + 1.f) - 1.f) * 0.5f);
     while ((uint64_t)(b + 1) * (uint64_t)(b + 2) / 2 <= l) ++b;
@@ -472,168 +548,266 @@ __device__ __forceinline__ int rank_of_local(uint32_t l) {
     return b;
 }
 
-// mode 0: trust hash-equal candidates (verified later by the scatter pass); mode 1: repair — runs only if the scatter pass
-// found a collision, and accepts a candidate only after comparing tokens exactly.
-__global__ void __launch_bounds__(kSelThreads) merge_select_kernel(const MergeParams p, int mode) {
-    if (fatal(p)) return;
-    if (mode == 1 && p.ctrl->collision == 0) return;
-    __shared__ RadixScratch<kSelThreads / 32> sc;
-    __shared__ uint32_t s_key[2][kSelSmemKeys];
-    __shared__ uint32_t s_val[2][kSelSmemKeys];
-    const int tid = threadIdx.x;
+struct SelectSmem {
+    RadixScratch<kSelThreads / 32> sc;       // global LSD path
+    uint32_t start[kSelBuckets + 1];         // MSD path: bucket starts, then fill cursors
+    uint32_t sorted[kSelSmemKeys];           // MSD path: key slots grouped by bucket
+    uint32_t dig[kSelSmemKeys];              // MSD path: digest of each key slot (0xFFFFFFFF: invalid)
+    uint32_t wtot[kSelThreads / 32];
+    int64_t t_off[kSelCacheK];               // per group member (by rank): token offset, first hash segment
+    int32_t t_sb[kSelCacheK];
+    uint8_t bad[kSelCacheK];                 // predecessor link of member r is broken (not an exact extension)
+};
+
+// mode 0: trust hash-equal candidates (verified later by the scatter pass); mode 1: repair — accepts a candidate only
+// after comparing tokens exactly.  NT threads per CTA; CTAs stride over the groups.
+template <int NT>
+__device__ void select_body(const MergeParams& p, int mode, SelectSmem& sm) {
+    static_assert(NT == kSelThreads, "select_body is written for kSelThreads");
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = p.ctrl->n_groups;
+    const bool weak = (p.flags & AJT_MERGE_WEAK_HASH) != 0;
     for (int g = blockIdx.x; g < G; g += gridDim.x) {
         const int gs = p.grp_start[g], k = p.grp_start[g + 1] - gs;
         const int32_t* gl = p.perm + gs;
+        const int32_t* gln = p.glen + gs;
         if (k < 2) {
             if (tid == 0) { p.absorbed[gl[0]] = 0; p.owner_tl[gl[0]] = gl[0]; }
             continue;
         }
         const int eb = p.grp_ent[g], c = p.grp_ent[g + 1] - eb;
-        // ---- M3: stable LSD radix sort of the group's keys by digest
-        const uint32_t* sk;
-        const uint32_t* sv;
-        if (c <= kSelSmemKeys) {
-            for (int x = tid; x < c; x += kSelThreads) {
-                const int32_t L = p.ent_len[eb + x];
-                s_key[0][x] = L < 0 ? 0xFFFFFFFFu : digest32(p.ent_hash[eb + x], L);
-                s_val[0][x] = (uint32_t)x;
+        const bool cached = k <= kSelCacheK, small = c <= kSelSmemKeys;
+        // ---- M2 (end): per timeline, exclusive prefix over its hash windows (in place), one warp per timeline
+        // (mode 1 finds seg_part and ent_hash already final)
+        for (int r = warp; r < k; r += NT / 32) {
+            const int i = gl[r];
+            const int sb = p.tl_rec[i].x;
+            const int64_t off = p.offsets[i];
+            const int ns = mode == 0 ? (int)(((off + gln[r] - 1 + p.mis) >> kHSegLog) - ((off + p.mis) >> kHSegLog) + 1) : 0;
+            if (cached && lane == 0) {
+                sm.t_off[r] = off;
+                sm.t_sb[r] = sb;
+                sm.bad[r] = r > 0 && (p.link_bad[i] != 0 || gln[r - 1] > gln[r]);
             }
+            uint64_t carry = 0;
+            for (int s0 = 0; s0 < ns; s0 += 32) {
+                const int s = s0 + lane;
+                const uint64_t v = s < ns ? p.seg_part[sb + s] : 0;
+                uint64_t inc = v;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint64_t t = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += t;
+                }
+                if (s < ns) p.seg_part[sb + s] = carry + inc - v;
+                carry += __shfl_sync(0xffffffffu, inc, 31);
+            }
+        }
+        if (small)
+            for (int b = tid; b <= kSelBuckets; b += NT) sm.start[b] = 0;
+        __syncthreads();
+        // ---- final keys: hash of T_i[0:L_a] = prefix of the windows before the one holding position L_a - 1 + its partial
+        uint32_t* gdig = p.ent_dig + eb;
+        uint32_t* gidx = p.ent_idx + eb;
+        for (int x = tid; x < c; x += NT) {
+            const int r = rank_of_local((uint32_t)x), a = x - r * (r + 1) / 2;
+            const int64_t Lp = gln[a];
+            uint32_t dg = 0xFFFFFFFFu;
+            if (Lp <= gln[r]) {
+                uint64_t h = p.ent_hash[eb + x];
+                if (mode == 0) {
+                    int64_t off;
+                    int sb;
+                    if (cached) { off = sm.t_off[r]; sb = sm.t_sb[r]; }
+                    else { const int i = gl[r]; off = p.offsets[i]; sb = p.tl_rec[i].x; }
+                    const int64_t widx = ((off + Lp - 1 + p.mis) >> kHSegLog) - ((off + p.mis) >> kHSegLog);
+                    h += p.seg_part[sb + widx];
+                    if (weak) h &= 0xFull;
+                    p.ent_hash[eb + x] = h;
+                }
+                dg = digest32(h, (int32_t)Lp);
+                if (dg == 0xFFFFFFFFu) dg = 0xFFFFFFFEu;
+            }
+            if (small) {
+                sm.dig[x] = dg;
+                if (dg != 0xFFFFFFFFu) atomicAdd(&sm.start[dg >> (32 - kSelBucketBits)], 1u);
+            } else {
+                gdig[x] = dg;
+                gidx[x] = (uint32_t)x;
+            }
+        }
+        __syncthreads();
+        // ---- M3: segmented radix sort of the group's keys by digest
+        const uint32_t* sk = nullptr;   // global path: sorted digests / order
+        const uint32_t* sv = nullptr;
+        if (small) {
+            // one MSD pass on the top 11 bits: exclusive scan of the 2048-bin histogram (8 bins per thread), then scatter
+            uint32_t loc[kSelBuckets / NT], s = 0;
+#pragma unroll
+            for (int j = 0; j < kSelBuckets / NT; ++j) { loc[j] = sm.start[tid * (kSelBuckets / NT) + j]; s += loc[j]; }
+            uint32_t inc = s;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            if (lane == 31) sm.wtot[warp] = inc;
             __syncthreads();
-            int cur = 0;
-            for (int shift = 0; shift < 32; shift += 8) {
-                radix_pass<kSelThreads / 32>(s_key[cur], s_val[cur], s_key[cur ^ 1], s_val[cur ^ 1], c, shift, sc);
-                cur ^= 1;
+            uint32_t run = inc - s;
+#pragma unroll
+            for (int w = 0; w < NT / 32; ++w)
+                if (w < warp) run += sm.wtot[w];
+#pragma unroll
+            for (int j = 0; j < kSelBuckets / NT; ++j) { sm.start[tid * (kSelBuckets / NT) + j] = run; run += loc[j]; }
+            if (tid == NT - 1) sm.start[kSelBuckets] = run;
+            __syncthreads();
+            for (int x = tid; x < c; x += NT) {
+                const uint32_t dg = sm.dig[x];
+                if (dg != 0xFFFFFFFFu) sm.sorted[atomicAdd(&sm.start[dg >> (32 - kSelBucketBits)], 1u)] = (uint32_t)x;
             }
-            sk = s_key[cur];
-            sv = s_val[cur];
+            __syncthreads();   // start[b] now holds the END of bucket b (= start of b + 1)
         } else {
-            uint32_t* kk[2] = {p.ent_idx + eb, p.tmp_idx + eb};
-            uint32_t* dd[2] = {p.ent_dig + eb, p.tmp_dig + eb};
-            for (int x = tid; x < c; x += kSelThreads) {
-                const int32_t L = p.ent_len[eb + x];
-                dd[0][x] = L < 0 ? 0xFFFFFFFFu : digest32(p.ent_hash[eb + x], L);
-                kk[0][x] = (uint32_t)x;
-            }
-            __syncthreads();
+            uint32_t* kk[2] = {gidx, p.tmp_idx + eb};
+            uint32_t* dd[2] = {gdig, p.tmp_dig + eb};
             int cur = 0;
             for (int shift = 0; shift < 32; shift += 8) {
-                radix_pass<kSelThreads / 32>(dd[cur], kk[cur], dd[cur ^ 1], kk[cur ^ 1], c, shift, sc);
+                radix_pass<NT / 32>(dd[cur], kk[cur], dd[cur ^ 1], kk[cur ^ 1], c, shift, sm.sc);
                 cur ^= 1;
                 __syncthreads();
             }
             sk = dd[cur];   // after 4 passes cur == 0: digests are back in ent_dig (sorted), order in ent_idx
             sv = kk[cur];
         }
-        __syncthreads();
+        // visit(dg, fn): fn(le) for every key slot of this group whose digest is dg (the equal-key run)
+        auto visit = [&](uint32_t dg, auto fn) {
+            if (small) {
+                const uint32_t b = dg >> (32 - kSelBucketBits);
+                const uint32_t x1 = sm.start[b], x0 = b ? sm.start[b - 1] : 0u;
+                for (uint32_t x = x0; x < x1; ++x) {
+                    const uint32_t le = sm.sorted[x];
+                    if (sm.dig[le] == dg) fn(le);
+                }
+            } else {
+                int lo = 0, hi = c;   // lower bound of dg in the sorted digests
+                while (lo < hi) {
+                    const int mid = (lo + hi) >> 1;
+                    if (sk[mid] < dg) lo = mid + 1; else hi = mid;
+                }
+                for (int x = lo; x < c && sk[x] == dg; ++x) fn(sv[x]);
+            }
+        };
         // ---- M4: survivors and the Algorithm-1 owner (latest extender)
-        for (int b = tid; b < k; b += kSelThreads) {
+        for (int b = tid; b < k; b += NT) {
             const int j = gl[b];
-            const int ef = p.t_entbase[j] + b;          // full key of j
+            const int ef = eb + b * (b + 1) / 2 + b;        // full key of j
             const uint64_t H = p.ent_hash[ef];
-            const int32_t L = p.ent_len[ef];
-            const uint32_t dg = digest32(H, L);
-            int lo = 0, hi = c;                          // lower bound of dg in the sorted digests
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (sk[mid] < dg) lo = mid + 1; else hi = mid;
-            }
-            int best = -1;                               // max rank of an extender
-            for (int x = lo; x < c && sk[x] == dg; ++x) {
-                const uint32_t le = sv[x];
+            const int32_t L = gln[b];
+            uint32_t dg = digest32(H, L);
+            if (dg == 0xFFFFFFFFu) dg = 0xFFFFFFFEu;
+            int best = -1;                                   // max rank of an extender
+            visit(dg, [&](uint32_t le) {
                 const int rb = rank_of_local(le);
-                if (rb <= b || rb <= best) continue;
-                if (p.ent_len[eb + le] != L || p.ent_hash[eb + le] != H) continue;
-                if (mode == 1 && !tokens_extend(p, gl[rb], j)) continue;
+                if (rb <= b || rb <= best) return;
+                const int a = (int)le - rb * (rb + 1) / 2;
+                if (gln[a] != L || p.ent_hash[eb + le] != H) return;
+                if (mode == 1 && !tokens_extend(p, gl[rb], j)) return;
                 best = rb;
-            }
+            });
             p.absorbed[j] = best >= 0;
             p.owner_tl[j] = best >= 0 ? gl[best] : j;
         }
         __syncthreads();
         if (p.owner_rule == AJT_OWNER_LONGEST) {
             // the longest SURVIVING extender, then the lowest index (BASELINE.json north_star; reading M-3)
-            for (int b = tid; b < k; b += kSelThreads) {
+            for (int b = tid; b < k; b += NT) {
                 const int j = gl[b];
                 if (!p.absorbed[j]) continue;
-                const int ef = p.t_entbase[j] + b;
+                const int ef = eb + b * (b + 1) / 2 + b;
                 const uint64_t H = p.ent_hash[ef];
-                const int32_t L = p.ent_len[ef];
-                const uint32_t dg = digest32(H, L);
-                int lo = 0, hi = c;
-                while (lo < hi) {
-                    const int mid = (lo + hi) >> 1;
-                    if (sk[mid] < dg) lo = mid + 1; else hi = mid;
-                }
-                const int paper_rb = p.t_rank[p.owner_tl[j]];   // a surviving, (to be) verified extender: the fallback
-                int best = paper_rb;
-                int64_t bestL = p.offsets[gl[best] + 1] - p.offsets[gl[best]];
-                for (int x = lo; x < c && sk[x] == dg; ++x) {
-                    const uint32_t le = sv[x];
+                const int32_t L = gln[b];
+                uint32_t dg = digest32(H, L);
+                if (dg == 0xFFFFFFFFu) dg = 0xFFFFFFFEu;
+                int best = p.tl_rec[p.owner_tl[j]].z;   // a surviving, (to be) verified extender: the fallback
+                int32_t bestL = gln[best];
+                visit(dg, [&](uint32_t le) {
                     const int rb = rank_of_local(le);
-                    if (rb <= b || rb == best) continue;
-                    if (p.ent_len[eb + le] != L || p.ent_hash[eb + le] != H) continue;
+                    if (rb <= b || rb == best) return;
+                    const int a = (int)le - rb * (rb + 1) / 2;
+                    if (gln[a] != L || p.ent_hash[eb + le] != H) return;
                     const int i = gl[rb];
-                    if (p.absorbed[i]) continue;
-                    const int64_t Li = p.offsets[i + 1] - p.offsets[i];
-                    if (!(Li > bestL || (Li == bestL && rb < best))) continue;
-                    if (mode == 1 && !tokens_extend(p, i, j)) continue;
+                    if (p.absorbed[i]) return;
+                    const int32_t Li = gln[rb];
+                    if (!(Li > bestL || (Li == bestL && rb < best))) return;
+                    if (mode == 1 && !tokens_extend(p, i, j)) return;
                     best = rb;
                     bestL = Li;
-                }
-                p.mem_cur[j] = gl[best];   // staged: owner_tl is still being read by other threads
+                });
+                p.cand[j] = gl[best];   // staged: owner_tl is still being read by other threads
             }
             __syncthreads();
-            for (int b = tid; b < k; b += kSelThreads) {
+            for (int b = tid; b < k; b += NT) {
                 const int j = gl[b];
-                if (p.absorbed[j]) p.owner_tl[j] = p.mem_cur[j];
+                if (p.absorbed[j]) p.owner_tl[j] = p.cand[j];
             }
+        }
+        // ---- M5, first half: T_j is a prefix of its owner T_o for certain if every predecessor link between them was
+        // verified by the hash pass (prefix-of is transitive); only the other members are re-read by the scatter pass
+        for (int b = tid; b < k; b += NT) {
+            const int j = gl[b];
+            bool nv = p.absorbed[j] != 0;
+            if (nv && cached) {
+                const int o = p.tl_rec[p.owner_tl[j]].z;
+                nv = false;
+                for (int r = b + 1; r <= o; ++r) nv |= sm.bad[r] != 0;
+            }
+            p.needv[j] = nv;
         }
         __syncthreads();
     }
 }
 
+__global__ void __launch_bounds__(kSelThreads) merge_select_kernel(const MergeParams p) {
+    __shared__ SelectSmem sm;
+    if (fatal(p)) return;
+    select_body<kSelThreads>(p, 0, sm);
+}
+
 // ---------------------------------------------------------------------------------------- K6: compact (M6)
 
-__global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p, int mode) {
-    if (fatal(p)) return;
-    if (mode == 1 && p.ctrl->collision == 0) return;
-    __shared__ int64_t s_w[2][32];
+template <int NT>
+__device__ void compact_body(const MergeParams& p, int mode, int64_t (*s_w)[2][NT / 32]) {
     const int tid = threadIdx.x, n = p.n;
-    for (int i = tid; i < n; i += 1024) p.mem_cnt[i] = 0;
-    __syncthreads();
-    const int M = (int)block_scan<1024>(
-        n, [&](int i) { return p.absorbed[i] ? 0 : 1; },
-        [&](int i, int64_t ex, int64_t v) {
-            p.midx[i] = v ? (int)ex : -1;
-            if (v) { p.merged_origin[ex] = i; p.merged_traj[ex] = p.traj_ids[i]; }
-            else atomicAdd(&p.mem_cnt[p.owner_tl[i]], 1);
+    // one fused scan over the timelines: survivors (-> merged index), their scatter tiles, their lengths (-> offsets).
+    // A merged sequence starting at merged offset mo is tiled on the 4-element grid of the OUTPUT arrays, so it needs
+    // ceil((L + (mo & 3)) / kTile) tiles; (L + 3) bounds that without knowing mo (an empty extra tile exits at once).
+    const I2 tot = block_scan2<NT>(
+        n,
+        [&](int i) {
+            if (p.absorbed[i]) return I2{0, 0};
+            const int64_t L = tl_len(p, i);
+            return I2{((int64_t)1 << 32) | ((L + 3 + kTile - 1) / kTile), L};
+        },
+        [&](int i, int64_t exa, int64_t exb, int64_t va, int64_t) {
+            if (!va) { p.midx[i] = -1; return; }
+            const int m = (int)(exa >> 32);
+            p.midx[i] = m;
+            p.merged_origin[m] = i;
+            p.merged_traj[m] = p.traj_ids[i];
+            p.merged_offsets[m] = exb;
+            p.tile_base[m] = (int32_t)(exa & 0xffffffff);
         },
         s_w);
-    const int64_t Nout = block_scan<1024>(
-        M, [&](int m) { const int s = p.merged_origin[m]; return p.offsets[s + 1] - p.offsets[s]; },
-        [&](int m, int64_t ex, int64_t) { p.merged_offsets[m] = ex; }, s_w);
-    const int64_t ntiles = block_scan<1024>(
-        M, [&](int m) { const int s = p.merged_origin[m]; return (p.offsets[s + 1] - p.offsets[s] + kTile - 1) / kTile; },
-        [&](int m, int64_t ex, int64_t) { p.tile_base[m] = (int32_t)ex; }, s_w);
-    block_scan<1024>(
-        M, [&](int m) { return p.mem_cnt[p.merged_origin[m]]; },
-        [&](int m, int64_t ex, int64_t) { p.mem_off[m] = (int32_t)ex; p.mem_cur[m] = (int32_t)ex; }, s_w);
-    __syncthreads();
-    for (int i = tid; i < n; i += 1024) {
-        const int m = p.midx[p.owner_tl[i]];
-        p.owner[i] = m;
-        if (p.absorbed[i]) p.mem_list[atomicAdd(&p.mem_cur[m], 1)] = i;
-    }
+    const int M = (int)(tot.a >> 32);
+    const int32_t ntiles = (int32_t)(tot.a & 0xffffffff);
+    for (int i = tid; i < n; i += NT) p.owner[i] = p.midx[p.owner_tl[i]];
     if (tid == 0) {
-        p.merged_offsets[M] = Nout;
-        p.tile_base[M] = (int32_t)ntiles;
-        p.mem_off[M] = n - M;
+        p.merged_offsets[M] = tot.b;
+        p.tile_base[M] = ntiles;
         p.counts[0] = M;
-        p.counts[1] = Nout;
+        p.counts[1] = tot.b;
         p.ctrl->M = M;
-        p.ctrl->N_out = Nout;
-        p.ctrl->n_tiles = (int32_t)ntiles;
+        p.ctrl->N_out = tot.b;
+        p.ctrl->n_tiles = ntiles;
         if (mode == 1) {
             p.ctrl->collision = 2;   // repair in progress: the scatter pass must not find another mismatch
             atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_HASH_COLLISION);
@@ -641,48 +815,284 @@ __global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p
     }
 }
 
+__global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p) {
+    __shared__ int64_t s_w[2][2][32];
+    if (fatal(p)) return;
+    compact_body<1024>(p, 0, s_w);
+}
+
 // ---------------------------------------------------------------------------------------- K5 + K7: verify + scatter (M5, M7)
 
-__global__ void __launch_bounds__(256) merge_scatter_kernel(const MergeParams p, int mode) {
-    if (fatal(p)) return;
-    if (mode == 1 && p.ctrl->collision != 2) return;
+// Warp task = one tile of kTile positions of one merged sequence, laid on the 4-element grid of the OUTPUT arrays so that
+// tokens / src / old_logp leave as 16-byte stores and the mask as 4-byte stores.  Lane l holds positions
+// qbase + 128 u + 4 l + e (u < 4, e < 4).  A warp takes a contiguous run of tiles, so the members of a merged sequence (the
+// absorbed timelines it owns, found among the earlier timelines of its group) are gathered once per sequence into a
+// per-warp shared-memory list {index, length, resp_start, token offset}, ascending.  Each member is compared against the
+// survivor exactly (M5) and painted into the slot map in ascending order; slot 0 = nobody, c + 1 = member c, 33 = survivor.
+constexpr int kMemCap = 32;
+struct MemberList {
+    int64_t jo[kMemCap];
+    int32_t j[kMemCap], L[kMemCap], rs[kMemCap];
+    uint8_t nv[kMemCap];
+};
+
+struct TileCtx {
+    int s, Ls, rs_s, gs, rank_s;
+    int64_t so, mo;
+};
+
+// Slow path for a sequence with more than kMemCap members: walks the group's earlier timelines for every tile.
+template <bool kExplicit>
+__device__ __noinline__ bool scatter_tile_generic(const MergeParams& p, const TileCtx c, int qbase, bool vec_ok) {
+    constexpr int kU = kTile / 128;
+    const int lane = threadIdx.x & 31;
+    const int ql = qbase + 4 * lane;
+    const int s = c.s, Ls = c.Ls;
+    bool mismatch = false;
+    int32_t x[kU][4], src[kU][4];
+#pragma unroll
+    for (int u = 0; u < kU; ++u)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int q = ql + 128 * u + e;
+            const bool v = q >= 0 && q < Ls;
+            x[u][e] = v ? p.tokens[c.so + q] : 0;
+            bool mk = false;
+            if (v) mk = kExplicit ? (p.mask_in[c.so + q] != 0) : (q >= c.rs_s);
+            src[u][e] = mk ? s : -1;
+        }
+    const int qlo = max(qbase, 0);
+    for (int a0 = 0; a0 < c.rank_s; a0 += 32) {
+        const int a = a0 + lane;
+        int j = -1, Lj = 0;
+        if (a < c.rank_s) {
+            Lj = p.glen[c.gs + a];
+            if (Lj > qlo) {
+                j = p.perm[c.gs + a];
+                if (p.owner_tl[j] != s) j = -1;
+            }
+        }
+        unsigned hits = __ballot_sync(0xffffffffu, j >= 0);
+        while (hits) {
+            const int sl = __ffs(hits) - 1;
+            hits &= hits - 1;
+            const int jj = __shfl_sync(0xffffffffu, j, sl), Ljj = __shfl_sync(0xffffffffu, Lj, sl);
+            const int64_t jo = p.offsets[jj];
+            const int rs_j = kExplicit ? 0 : p.resp_start[jj];
+#pragma unroll
+            for (int u = 0; u < kU; ++u) {
+                if (qbase + 128 * u >= Ljj) break;   // warp-uniform: the member ends before this step
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int q = ql + 128 * u + e;
+                    if (q >= 0 && q < Ljj) {
+                        if (p.tokens[jo + q] != x[u][e]) mismatch = true;     // exact verification (M5)
+                        const bool mk = kExplicit ? (p.mask_in[jo + q] != 0) : (q >= rs_j);
+                        if (mk) src[u][e] = max(src[u][e], jj);
+                    }
+                }
+            }
+        }
+    }
+    const int64_t dbase = c.mo + ql;   // multiple of 4
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+        const int q = ql + 128 * u;
+        if (q >= Ls || q + 3 < 0) continue;
+        const int64_t d = dbase + 128 * u;
+        float lp[4] = {0.f, 0.f, 0.f, 0.f};
+        if (p.merged_old_logp) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int sj = src[u][e];
+                if (sj >= 0) lp[e] = p.old_logp_in[(sj == s ? c.so : p.offsets[sj]) + q + e];
+            }
+        }
+        if (vec_ok && q >= 0 && q + 3 < Ls) {
+            *reinterpret_cast<int4*>(p.merged_tokens + d) = make_int4(x[u][0], x[u][1], x[u][2], x[u][3]);
+            *reinterpret_cast<int4*>(p.merged_src + d) = make_int4(src[u][0], src[u][1], src[u][2], src[u][3]);
+            *reinterpret_cast<uint32_t*>(p.merged_mask + d) = (src[u][0] >= 0 ? 1u : 0u) | (src[u][1] >= 0 ? 0x100u : 0u) |
+                                                              (src[u][2] >= 0 ? 0x10000u : 0u) | (src[u][3] >= 0 ? 0x1000000u : 0u);
+            if (p.merged_old_logp) *reinterpret_cast<float4*>(p.merged_old_logp + d) = make_float4(lp[0], lp[1], lp[2], lp[3]);
+        } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                if (q + e >= 0 && q + e < Ls) {
+                    p.merged_tokens[d + e] = x[u][e];
+                    p.merged_src[d + e] = src[u][e];
+                    p.merged_mask[d + e] = src[u][e] >= 0;
+                    if (p.merged_old_logp) p.merged_old_logp[d + e] = lp[e];
+                }
+            }
+        }
+    }
+    return mismatch;
+}
+
+template <bool kExplicit>
+__device__ __forceinline__ bool scatter_tile_fast(const MergeParams& p, const TileCtx& c, int qbase, bool vec_ok,
+                                                  const MemberList& ml, int cnt) {
+    constexpr int kU = kTile / 128;
+    constexpr int kSurv = kMemCap + 1;
+    const int lane = threadIdx.x & 31;
+    const int ql = qbase + 4 * lane;
+    const int s = c.s, Ls = c.Ls;
+    bool mismatch = false;
+    const bool full = qbase >= 0 && qbase + kTile <= Ls;   // warp-uniform: every slot of the tile is a position of the sequence
+    int32_t x[kU][4];
+    int32_t slot[kU][4];
+    const int32_t* __restrict__ tok = p.tokens + c.so;
+#pragma unroll
+    for (int u = 0; u < kU; ++u)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int q = ql + 128 * u + e;
+            const bool v = full || (q >= 0 && q < Ls);
+            x[u][e] = v ? tok[q] : 0;
+            bool mk = false;
+            if (v) mk = kExplicit ? (p.mask_in[c.so + q] != 0) : (q >= c.rs_s);
+            slot[u][e] = mk ? kSurv : 0;
+        }
+    const int qlo = max(qbase, 0);
+    for (int m = 0; m < cnt; ++m) {
+        const int Lj = ml.L[m];
+        if (Lj <= qlo) continue;                 // warp-uniform: the member ends before this tile
+        const int rs_j = ml.rs[m];
+        const int32_t* __restrict__ tj = p.tokens + ml.jo[m];
+        const uint8_t* mkj = kExplicit ? p.mask_in + ml.jo[m] : nullptr;
+        // all of the member's loads first (independent), then the compares: one memory latency per member, not one per element
+        if (kExplicit || ml.nv[m]) {   // warp-uniform
+            int32_t y[kU][4];
+            uint8_t ym[kU][4];
+#pragma unroll
+            for (int u = 0; u < kU; ++u)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int q = ql + 128 * u + e;
+                    const bool in = q >= 0 && q < Lj;
+                    y[u][e] = in ? tj[q] : x[u][e];
+                    if (kExplicit) ym[u][e] = in ? mkj[q] : (uint8_t)0;
+                }
+#pragma unroll
+            for (int u = 0; u < kU; ++u)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int q = ql + 128 * u + e;
+                    mismatch |= y[u][e] != x[u][e];     // exact verification (M5, second half)
+                    const bool mk = kExplicit ? (ym[u][e] != 0) : (q >= rs_j && q < Lj);
+                    if (mk) slot[u][e] = max(slot[u][e], m + 1);
+                }
+        } else {
+#pragma unroll
+            for (int u = 0; u < kU; ++u)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int q = ql + 128 * u + e;
+                    if (q >= rs_j && q < Lj) slot[u][e] = max(slot[u][e], m + 1);
+                }
+        }
+    }
+    // ---- outputs
+    const int64_t dbase = c.mo + ql;   // multiple of 4
+    float lp[kU][4];
+    if (p.merged_old_logp) {
+#pragma unroll
+        for (int u = 0; u < kU; ++u)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int sl = slot[u][e];
+                lp[u][e] = 0.f;
+                if (sl) lp[u][e] = p.old_logp_in[(sl == kSurv ? c.so : ml.jo[sl - 1]) + ql + 128 * u + e];
+            }
+    }
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+        const int q = ql + 128 * u;
+        if (!full && (q >= Ls || q + 3 < 0)) continue;
+        const int64_t d = dbase + 128 * u;
+        int32_t sj[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int sl = slot[u][e];
+            sj[e] = sl == 0 ? -1 : (sl == kSurv ? s : ml.j[sl - 1]);
+        }
+        if (vec_ok && (full || (q >= 0 && q + 3 < Ls))) {
+            *reinterpret_cast<int4*>(p.merged_tokens + d) = make_int4(x[u][0], x[u][1], x[u][2], x[u][3]);
+            *reinterpret_cast<int4*>(p.merged_src + d) = make_int4(sj[0], sj[1], sj[2], sj[3]);
+            *reinterpret_cast<uint32_t*>(p.merged_mask + d) =
+                (sj[0] >= 0 ? 1u : 0u) | (sj[1] >= 0 ? 0x100u : 0u) | (sj[2] >= 0 ? 0x10000u : 0u) | (sj[3] >= 0 ? 0x1000000u : 0u);
+            if (p.merged_old_logp)
+                *reinterpret_cast<float4*>(p.merged_old_logp + d) = make_float4(lp[u][0], lp[u][1], lp[u][2], lp[u][3]);
+        } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                if (q + e >= 0 && q + e < Ls) {
+                    p.merged_tokens[d + e] = x[u][e];
+                    p.merged_src[d + e] = sj[e];
+                    p.merged_mask[d + e] = sj[e] >= 0;
+                    if (p.merged_old_logp) p.merged_old_logp[d + e] = lp[u][e];
+                }
+            }
+        }
+    }
+    return mismatch;
+}
+
+template <bool kExplicit>
+__device__ void scatter_body(const MergeParams& p, int mode, MemberList* lists) {
     const int lane = threadIdx.x & 31;
     const int wglobal = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
     const int ntiles = p.ctrl->n_tiles, M = p.ctrl->M;
+    const int per = (ntiles + nwarps - 1) / nwarps;
+    const int t_begin = wglobal * per, t_end = min(ntiles, t_begin + per);
+    if (t_begin >= t_end) return;
+    MemberList& ml = lists[threadIdx.x >> 5];
+    const bool vec_ok = ((((uintptr_t)p.merged_tokens | (uintptr_t)p.merged_src | (uintptr_t)p.merged_old_logp) & 15) == 0) &&
+                        (((uintptr_t)p.merged_mask & 3) == 0);
     bool mismatch = false;
-    for (int t = wglobal; t < ntiles; t += nwarps) {
-        int lo = 0, hi = M;   // merged sequence of this tile: last m with tile_base[m] <= t
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (p.tile_base[mid] <= t) lo = mid; else hi = mid;
-        }
-        const int m = lo;
-        const int s = p.merged_origin[m];
-        const int64_t so = p.offsets[s];
-        const int Ls = (int)(p.offsets[s + 1] - so);
-        const int64_t mo = p.merged_offsets[m];
-        const int p0 = (t - p.tile_base[m]) * kTile, p1 = min(Ls, p0 + kTile);
-        const int mb = p.mem_off[m], me = p.mem_off[m + 1];
-        const int rs_s = p.resp_start ? p.resp_start[s] : 0;
-        for (int q = p0 + lane; q < p1; q += 32) {
-            const int32_t x = p.tokens[so + q];
-            int src = -1;
-            if (p.mask_in ? (p.mask_in[so + q] != 0) : (q >= rs_s)) src = s;
-            for (int u = mb; u < me; ++u) {
-                const int j = p.mem_list[u];
-                const int64_t jo = p.offsets[j];
-                const int Lj = (int)(p.offsets[j + 1] - jo);
-                if (q < Lj) {
-                    if (p.tokens[jo + q] != x) mismatch = true;     // exact verification (M5)
-                    const bool mk = p.mask_in ? (p.mask_in[jo + q] != 0) : (q >= p.resp_start[j]);
-                    if (mk) src = max(src, j);
+    int m = warp_search_last_le(M, t_begin, [&](int x) { return p.tile_base[x]; });
+    int cur_m = -1, cnt = 0, tb = 0;
+    TileCtx c = {};
+    for (int t = t_begin; t < t_end; ++t) {
+        while (p.tile_base[m + 1] <= t) ++m;
+        if (m != cur_m) {
+            cur_m = m;
+            tb = p.tile_base[m];
+            c.s = p.merged_origin[m];
+            c.mo = p.merged_offsets[m];
+            const int4 rec = p.tl_rec[c.s];
+            c.gs = rec.y;
+            c.rank_s = rec.z;
+            c.so = p.offsets[c.s];
+            c.Ls = (int)(p.offsets[c.s + 1] - c.so);
+            c.rs_s = kExplicit ? 0 : p.resp_start[c.s];
+            // members of s: earlier timelines of its group that it owns, ascending
+            __syncwarp();
+            cnt = 0;
+            for (int a0 = 0; a0 < c.rank_s; a0 += 32) {
+                const int a = a0 + lane;
+                int j = -1;
+                if (a < c.rank_s) {
+                    j = p.perm[c.gs + a];
+                    if (p.owner_tl[j] != c.s) j = -1;
                 }
+                const unsigned bal = __ballot_sync(0xffffffffu, j >= 0);
+                const int pos = cnt + __popc(bal & ((1u << lane) - 1u));
+                if (j >= 0 && pos < kMemCap) {
+                    ml.j[pos] = j;
+                    ml.L[pos] = p.glen[c.gs + a];
+                    ml.rs[pos] = kExplicit ? 0 : p.resp_start[j];
+                    ml.jo[pos] = p.offsets[j];
+                    ml.nv[pos] = p.needv[j];
+                }
+                cnt += __popc(bal);
             }
-            p.merged_tokens[mo + q] = x;
-            p.merged_mask[mo + q] = src >= 0;
-            p.merged_src[mo + q] = src;
-            if (p.merged_old_logp) p.merged_old_logp[mo + q] = src >= 0 ? p.old_logp_in[p.offsets[src] + q] : 0.f;
+            __syncwarp();
         }
+        const int qbase = (t - tb) * kTile - (int)(c.mo & 3);   // position of the tile's first slot (may be -3..-1)
+        if (qbase >= c.Ls) continue;
+        if (cnt <= kMemCap) mismatch |= scatter_tile_fast<kExplicit>(p, c, qbase, vec_ok, ml, cnt);
+        else mismatch |= scatter_tile_generic<kExplicit>(p, c, qbase, vec_ok);
     }
     if (__any_sync(0xffffffffu, mismatch) && lane == 0) {
         if (mode == 0) atomicExch(&p.ctrl->collision, 1);
@@ -690,11 +1100,37 @@ __global__ void __launch_bounds__(256) merge_scatter_kernel(const MergeParams p,
     }
 }
 
+constexpr int kScatThreads = 256;
+__global__ void __launch_bounds__(kScatThreads, 4) merge_scatter_kernel(const MergeParams p) {
+    __shared__ MemberList lists[kScatThreads / 32];
+    if (fatal(p)) return;
+    if (p.mask_in) scatter_body<true>(p, 0, lists);
+    else scatter_body<false>(p, 0, lists);
+}
+
+// ---------------------------------------------------------------------------------------- exact repair (M5)
+
+// Cooperative launch; every CTA returns at once unless the scatter pass saw a hash-equal, token-different pair.
+__global__ void __launch_bounds__(kSelThreads) merge_repair_kernel(const MergeParams p) {
+    __shared__ SelectSmem sm;
+    __shared__ int64_t s_w[2][2][kSelThreads / 32];
+    if (fatal(p) || p.ctrl->collision == 0) return;
+    cg::grid_group grid = cg::this_grid();
+    select_body<kSelThreads>(p, 1, sm);
+    grid.sync();
+    if (blockIdx.x == 0) compact_body<kSelThreads>(p, 1, s_w);
+    grid.sync();
+    MemberList* lists = reinterpret_cast<MemberList*>(&sm);   // the select scratch is free again
+    static_assert(sizeof(SelectSmem) >= sizeof(MemberList) * (kSelThreads / 32), "member lists fit in the select scratch");
+    if (p.mask_in) scatter_body<true>(p, 1, lists);
+    else scatter_body<false>(p, 1, lists);
+}
+
 }  // namespace
 
 extern "C" size_t ajt_merge_workspace_bytes(int32_t n, int64_t n_tokens) {
     if (n < 0 || n_tokens < 0) return 0;
-    return merge_ws_layout(n, n_tokens).fixed_total + a256(((size_t)64 * (size_t)n + 4096) * 32);
+    return merge_ws_layout(n, n_tokens).ent + a256(((size_t)64 * (size_t)n + 4096) * 32);
 }
 
 extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets, const int32_t* traj_ids,
@@ -726,32 +1162,26 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     p.merged_offsets = merged_offsets; p.merged_origin = merged_origin; p.merged_traj = merged_traj; p.owner = owner;
     p.counts = counts;
     p.ctrl = reinterpret_cast<AjtCtrl*>(b + ws.ctrl);
-    p.skey[0] = reinterpret_cast<uint32_t*>(b + ws.skey0); p.skey[1] = reinterpret_cast<uint32_t*>(b + ws.skey1);
-    p.sval[0] = reinterpret_cast<uint32_t*>(b + ws.sval0); p.sval[1] = reinterpret_cast<uint32_t*>(b + ws.sval1);
-    p.gid_sorted = reinterpret_cast<int32_t*>(b + ws.gid_sorted);
+    for (int k = 0; k < 5; ++k) p.gbuf[k] = reinterpret_cast<uint32_t*>(b + ws.gbuf[k]);
+    p.perm = reinterpret_cast<int32_t*>(b + ws.perm);
+    p.glen = reinterpret_cast<int32_t*>(b + ws.glen);
     p.grp_start = reinterpret_cast<int32_t*>(b + ws.grp_start);
     p.grp_ent = reinterpret_cast<int32_t*>(b + ws.grp_ent);
-    p.t_rank = reinterpret_cast<int32_t*>(b + ws.t_rank);
-    p.t_gid = reinterpret_cast<int32_t*>(b + ws.t_gid);
-    p.t_entbase = reinterpret_cast<int32_t*>(b + ws.t_entbase);
-    p.seg_base = reinterpret_cast<int32_t*>(b + ws.seg_base);
+    p.tl_rec = reinterpret_cast<int4*>(b + ws.tl_rec);
     p.seg_part = reinterpret_cast<uint64_t*>(b + ws.seg_part);
     p.absorbed = b + ws.absorbed;
+    p.link_bad = b + ws.link_bad;
+    p.needv = b + ws.needv;
     p.owner_tl = reinterpret_cast<int32_t*>(b + ws.owner_tl);
+    p.cand = reinterpret_cast<int32_t*>(b + ws.cand);
     p.midx = reinterpret_cast<int32_t*>(b + ws.midx);
-    p.mem_cnt = reinterpret_cast<int32_t*>(b + ws.mem_cnt);
-    p.mem_off = reinterpret_cast<int32_t*>(b + ws.mem_off);
-    p.mem_cur = reinterpret_cast<int32_t*>(b + ws.mem_cur);
-    p.mem_list = reinterpret_cast<int32_t*>(b + ws.mem_list);
     p.tile_base = reinterpret_cast<int32_t*>(b + ws.tile_base);
-    // everything after the fixed part holds perm and the per-key arrays; their capacity follows from the size given
+    // everything after the fixed part holds the per-key arrays; their capacity follows from the size given
     size_t eo = ws.ent;
-    p.perm = reinterpret_cast<int32_t*>(b + eo); eo += a256(((size_t)n + 1) * 4);
-    if (workspace_bytes < eo + 6 * 256 + ((size_t)n + 1024) * kEntBytes) return AJT_ERR_WORKSPACE_TOO_SMALL;
-    const size_t ecap = (workspace_bytes - eo - 6 * 256) / kEntBytes;
+    if (workspace_bytes < eo + 5 * 256 + ((size_t)n + 1024) * kEntBytes) return AJT_ERR_WORKSPACE_TOO_SMALL;
+    const size_t ecap = (workspace_bytes - eo - 5 * 256) / kEntBytes;
     p.E_cap = (int32_t)(ecap > (size_t)INT32_MAX ? (size_t)INT32_MAX : ecap);
     p.ent_hash = reinterpret_cast<uint64_t*>(b + eo); eo += a256((size_t)p.E_cap * 8);
-    p.ent_len = reinterpret_cast<int32_t*>(b + eo); eo += a256((size_t)p.E_cap * 4);
     p.ent_dig = reinterpret_cast<uint32_t*>(b + eo); eo += a256((size_t)p.E_cap * 4);
     p.ent_idx = reinterpret_cast<uint32_t*>(b + eo); eo += a256((size_t)p.E_cap * 4);
     p.tmp_dig = reinterpret_cast<uint32_t*>(b + eo); eo += a256((size_t)p.E_cap * 4);
@@ -760,22 +1190,33 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     p.nseg_cap = nseg_capacity(n, n_tokens);
     p.mis = (int32_t)(((uintptr_t)tokens >> 2) & 3);
 
-    if (cudaMemsetAsync(p.ctrl, 0, sizeof(AjtCtrl), stream) != cudaSuccess) return AJT_ERR_CUDA;
     if (n == 0) {
+        if (cudaMemsetAsync(p.ctrl, 0, sizeof(AjtCtrl), stream) != cudaSuccess) return AJT_ERR_CUDA;
         if (cudaMemsetAsync(counts, 0, 2 * sizeof(int64_t), stream) != cudaSuccess) return AJT_ERR_CUDA;
         if (cudaMemsetAsync(merged_offsets, 0, sizeof(int64_t), stream) != cudaSuccess) return AJT_ERR_CUDA;
         return AJT_OK;
     }
-    const int wide = num_sms * 8;
-    merge_group_kernel<<<1, 1024, 0, stream>>>(p);
-    merge_hash_kernel<<<wide, 256, 0, stream>>>(p);
-    merge_keys_kernel<<<(n + 255) / 256, 256, 0, stream>>>(p);
-    merge_select_kernel<<<num_sms * 2, kSelThreads, 0, stream>>>(p, 0);
-    merge_compact_kernel<<<1, 1024, 0, stream>>>(p, 0);
-    merge_scatter_kernel<<<wide, 256, 0, stream>>>(p, 0);
-    // exact repair path: each kernel returns at once unless the scatter pass saw a hash-equal, token-different pair
-    merge_select_kernel<<<num_sms * 2, kSelThreads, 0, stream>>>(p, 1);
-    merge_compact_kernel<<<1, 1024, 0, stream>>>(p, 1);
-    merge_scatter_kernel<<<wide, 256, 0, stream>>>(p, 1);
+    // per-device launch facts (attribute opt-in, co-resident grid of the cooperative repair kernel): looked up once
+    static int s_repair_grid[64] = {0};
+    if (dev < 0 || dev >= 64) return AJT_ERR_UNSUPPORTED;
+    if (s_repair_grid[dev] == 0) {
+        if (cudaFuncSetAttribute(merge_group_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * (kGrpSmemN + 4) * 4) !=
+            cudaSuccess)
+            return AJT_ERR_CUDA;
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, merge_repair_kernel, kSelThreads, 0) != cudaSuccess || per_sm < 1)
+            return AJT_ERR_CUDA;
+        s_repair_grid[dev] = num_sms * (per_sm < 4 ? per_sm : 4);
+    }
+    const size_t grp_dyn = n <= kGrpSmemN ? 5 * (((size_t)n + 4) & ~(size_t)3) * 4 : 0;
+    merge_group_kernel<<<1, 1024, grp_dyn, stream>>>(p);
+    merge_hash_kernel<<<num_sms * 2, 256, 0, stream>>>(p);
+    merge_select_kernel<<<num_sms * 4, kSelThreads, 0, stream>>>(p);
+    merge_compact_kernel<<<1, 1024, 0, stream>>>(p);
+    merge_scatter_kernel<<<num_sms * 4, kScatThreads, 0, stream>>>(p);
+    void* args[] = {(void*)&p};
+    if (cudaLaunchCooperativeKernel((const void*)merge_repair_kernel, dim3((unsigned)s_repair_grid[dev]), dim3(kSelThreads), args, 0,
+                                    stream) != cudaSuccess)
+        return AJT_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }
