@@ -4,8 +4,8 @@
 //   K1 merge_group_kernel    M1  one CTA, shared-memory resident for n <= 8192: validate offsets, stable LSD radix sort of
 //                                (traj_id - min, index), group ids, rank in group, per-timeline record {first hash segment,
 //                                group start, rank, first key slot}, lengths in group order
-//   K2 merge_hash_kernel     M2  warp-cooperative prefix-hash scan, 128-bit loads, 8 vectors in flight per lane.  The hash of
-//                                the first p tokens of timeline i is F_i(p) = sum_{q<p} mix(x_q) B^(q+3) mod 2^64: a sum, hence
+//   K2 merge_hash_kernel     M2  warp-cooperative prefix-hash scan, 128-bit loads, 4 vectors in flight per lane.  The hash of
+//                                the first p tokens of timeline i is F_i(p) = sum_{q<p} x_q w(q) mod 2^64, w(q) = B^(q+3) mod 2^32: a sum, hence
 //                                a monoid, so every lane keeps its own partial and lanes are only combined (shuffles) where a
 //                                key is emitted: at each length L_a of an earlier same-group timeline (probe key) and at L_i
 //                                itself (full key)
@@ -35,8 +35,21 @@ namespace cg = cooperative_groups;
 constexpr int kHSeg = 2048;        // hash-scan window: 2048 tokens = 16 steps x 32 lanes x 4 tokens
 constexpr int kHSegLog = 11;
 constexpr int kTile = 256;         // scatter tile (positions per warp task): 2 steps x 32 lanes x 4 tokens
-constexpr uint64_t kB = 0x9E3779B97F4A7C15ull;       // odd multiplier of the polynomial hash
-constexpr uint64_t kMixAdd = 0x632BE59BD9B4E019ull;  // so that token 0 is not the additive identity
+constexpr uint32_t kW = 0x9E3779B1u;   // odd multiplier of the prefix hash's 32-bit position weights
+constexpr uint32_t inv32(uint32_t b) {  // b^-1 mod 2^32 (b odd): Newton, 3 correct bits double every step
+    uint32_t x = b;
+    for (int i = 0; i < 5; ++i) x *= 2u - b * x;
+    return x;
+}
+constexpr uint32_t cpow32(uint32_t b, uint32_t e) {
+    uint32_t r = 1;
+    for (; e; e >>= 1, b *= b)
+        if (e & 1) r *= b;
+    return r;
+}
+constexpr uint32_t kWinv = inv32(kW);
+constexpr uint32_t kW128 = cpow32(kW, 128);
+static_assert((uint32_t)(kW * kWinv) == 1u, "modular inverse");
 constexpr uint32_t kFatal = AJT_STATUS_BAD_OFFSETS | AJT_STATUS_ZERO_LEN | AJT_STATUS_PROBE_CAPACITY;
 constexpr int kSelThreads = 256;
 constexpr int kSelSmemKeys = 2048;  // groups with more keys than this sort through global memory
@@ -44,14 +57,6 @@ constexpr int kSelBucketBits = 11;
 constexpr int kSelBuckets = 1 << kSelBucketBits;
 constexpr int kSelCacheK = 256;     // per-timeline facts of groups up to this size are staged in shared memory
 constexpr int kGrpSmemN = 8192;     // batches up to this many timelines are grouped entirely in shared memory
-
-constexpr uint64_t inv64(uint64_t b) {  // b^-1 mod 2^64 (b odd): Newton, 3 correct bits double every step
-    uint64_t x = b;
-    for (int i = 0; i < 6; ++i) x *= 2 - b * x;
-    return x;
-}
-constexpr uint64_t kBinv = inv64(kB);
-static_assert(kB * kBinv == 1ull, "modular inverse");
 
 struct MergeParams {
     const int32_t* tokens;
@@ -125,16 +130,6 @@ constexpr size_t kEntBytes = 32;  // per key slot: hash 8, dig 4, idx 4, tmp_dig
 
 __device__ __forceinline__ bool fatal(const MergeParams& p) { return (p.ctrl->status & kFatal) != 0; }
 
-__device__ __forceinline__ uint64_t pow64(uint64_t b, uint64_t e) {
-    uint64_t r = 1;
-    while (e) {
-        if (e & 1) r *= b;
-        b *= b;
-        e >>= 1;
-    }
-    return r;
-}
-__device__ __forceinline__ uint64_t powB(int64_t e) { return e >= 0 ? pow64(kB, (uint64_t)e) : pow64(kBinv, (uint64_t)(-e)); }
 __device__ __forceinline__ uint32_t digest32(uint64_t h, int32_t len) {
     uint64_t z = h ^ ((uint64_t)(uint32_t)len * 0xD6E8FEB86659FD93ull);
     z ^= z >> 32;
@@ -378,113 +373,142 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
 
 // ---------------------------------------------------------------------------------------- K2: prefix-hash scan (M2)
 
-// term of token x at slot e of a 4-token vector, before the vector's weight: mix(x) B^e = x B^e + c B^e.  x is 32 bits, so the
-// product is a 32x64 multiply (2 IMADs) with the constant folded into the addend.
-template <int E>
-__device__ __forceinline__ uint64_t tok_term(int32_t x) {
-    constexpr uint64_t B2 = kB * kB, B3 = B2 * kB;
-    constexpr uint64_t BE = E == 0 ? 1ull : E == 1 ? kB : E == 2 ? B2 : B3;
-    return (uint64_t)(uint32_t)x * BE + kMixAdd * BE;
+// Prefix hash F_i(p) = sum_{q<p} x_q w(q) mod 2^64 with 32-bit weights w(q) = B^(q+3) mod 2^32: one IMAD.WIDE per token
+// (32 x 32 -> 64 with a 64-bit addend).  A sum over positions, hence a monoid: per-lane partials, combined only where a key is
+// emitted.  Weak by design (a 64-bit sum of 50-bit products); every accepted pair is verified exactly (M5).
+__device__ __forceinline__ uint32_t pow32(uint32_t b, uint32_t e) {
+    uint32_t r = 1;
+    while (e) {
+        if (e & 1) r *= b;
+        b *= b;
+        e >>= 1;
+    }
+    return r;
+}
+__device__ __forceinline__ uint32_t cpow_dev(uint32_t b, uint32_t e) { return pow32(b, e); }
+__device__ __forceinline__ uint32_t powW(int64_t e) { return e >= 0 ? pow32(kW, (uint32_t)e) : pow32(kWinv, (uint32_t)(-e)); }
+__device__ __forceinline__ uint64_t mad_wide(uint32_t a, uint32_t b, uint64_t c) { return (uint64_t)a * b + c; }
+
+constexpr int kHashThreads = 256;
+
+// This lane's four tokens of step s of a window (positions q .. q+3), zero outside the timeline.  16-byte aligned address.
+template <bool kInterior>
+__device__ __forceinline__ int4 load_step(const MergeParams& p, int64_t off, int Li, int64_t q) {
+    const int32_t* __restrict__ tok = p.tokens;
+    const int64_t e = off + q;
+    if (kInterior) return __ldg(reinterpret_cast<const int4*>(tok + e));
+    int4 x = make_int4(0, 0, 0, 0);
+    if (q + 3 >= 0 && q < Li) {
+        if (e >= 0 && e + 3 < p.N) x = __ldg(reinterpret_cast<const int4*>(tok + e));
+        else {
+            if (e >= 0 && e < p.N) x.x = tok[e];
+            if (e + 1 >= 0 && e + 1 < p.N) x.y = tok[e + 1];
+            if (e + 2 >= 0 && e + 2 < p.N) x.z = tok[e + 2];
+            if (e + 3 >= 0 && e + 3 < p.N) x.w = tok[e + 3];
+        }
+        if (!(q >= 0 && q < Li)) x.x = 0;
+        if (!(q + 1 >= 0 && q + 1 < Li)) x.y = 0;
+        if (!(q + 2 >= 0 && q + 2 < Li)) x.z = 0;
+        if (!(q + 3 >= 0 && q + 3 < Li)) x.w = 0;
+    }
+    return x;
 }
 
-// Rare path, kept out of line so the streaming loop stays small in the instruction cache: writes the in-window partial of
-// every key whose prefix ends inside step s (positions [win0 + 128 s, +128)).  t0..t3 are this lane's four terms of the step
-// (already zero outside the timeline), acc its sum over the earlier steps, pw the weight of its vector.
-__device__ __noinline__ void hash_emit(uint64_t* __restrict__ ent_hash, const int32_t* __restrict__ gln, int rank, int ebase,
-                                       int64_t win0, int Li, int s, int64_t q, uint64_t t0, uint64_t t1, uint64_t t2, uint64_t t3,
-                                       uint64_t acc, uint64_t pw) {
+// One batch = 4 steps = 512 positions of a window: four 16-byte loads per lane in flight (plus 16 predecessor tokens when
+// linked).  kInterior: the batch lies inside the timeline.  kLink: 0 no predecessor positions here, 1 some, 2 all of them.
+// snap[s * 32] receives this lane's running sum BEFORE step s (the key-emission pass needs it); w are the lane's weights.
+template <bool kInterior, int kLink>
+__device__ __forceinline__ void hash_batch(const MergeParams& p, int64_t off, int Li, int64_t qb, const int32_t* __restrict__ tprev,
+                                           int Lprev, uint32_t (&w)[4], uint64_t& acc, uint32_t& diff, uint64_t* snap) {
+    int4 x[4];
+    int32_t y[4][4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int64_t q = qb + 128 * u;
+        x[u] = load_step<kInterior>(p, off, Li, q);
+        if (kLink == 2) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) y[u][k] = __ldg(tprev + q + k);
+        } else if (kLink == 1) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) y[u][k] = (q + k >= 0 && q + k < Lprev) ? __ldg(tprev + q + k) : 0;
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int64_t q = qb + 128 * u;
+        if (kLink == 2) {
+            diff |= (uint32_t)(y[u][0] ^ x[u].x) | (uint32_t)(y[u][1] ^ x[u].y);
+            diff |= (uint32_t)(y[u][2] ^ x[u].z) | (uint32_t)(y[u][3] ^ x[u].w);
+        } else if (kLink == 1) {
+            if (q >= 0 && q < Lprev) diff |= (uint32_t)(y[u][0] ^ x[u].x);
+            if (q + 1 >= 0 && q + 1 < Lprev) diff |= (uint32_t)(y[u][1] ^ x[u].y);
+            if (q + 2 >= 0 && q + 2 < Lprev) diff |= (uint32_t)(y[u][2] ^ x[u].z);
+            if (q + 3 >= 0 && q + 3 < Lprev) diff |= (uint32_t)(y[u][3] ^ x[u].w);
+        }
+        snap[u * 32] = acc;
+        acc = mad_wide((uint32_t)x[u].x, w[0], acc);
+        acc = mad_wide((uint32_t)x[u].y, w[1], acc);
+        acc = mad_wide((uint32_t)x[u].z, w[2], acc);
+        acc = mad_wide((uint32_t)x[u].w, w[3], acc);
+        w[0] *= kW128; w[1] *= kW128; w[2] *= kW128; w[3] *= kW128;
+    }
+}
+
+// Keys whose prefix ends inside step s of the window: the step's tokens are re-read (L1), the lane's four inclusive prefix
+// values are formed from its snapshot, one warp sum and one warp scan turn them into F at every position of the step, and each
+// key picks its value from the lane that holds its last token.  One pass serves any number of keys ending in the step.
+__device__ __noinline__ void hash_emit_step(const MergeParams& p, int64_t off, int Li, int64_t win0, int s, uint32_t w0_window,
+                                            const uint64_t* snap_s, const int32_t* __restrict__ gln, int rank, int ebase) {
     const int lane = threadIdx.x & 31;
+    const int64_t q = win0 + 128 * (int64_t)s + 4 * lane;
+    const int4 x = load_step<false>(p, off, Li, q);
+    uint32_t w = w0_window * cpow_dev(kW128, (uint32_t)s);
+    uint64_t c0 = (uint64_t)(uint32_t)x.x * w;
+    w *= kW;
+    uint64_t c1 = mad_wide((uint32_t)x.y, w, c0);
+    w *= kW;
+    uint64_t c2 = mad_wide((uint32_t)x.z, w, c1);
+    w *= kW;
+    uint64_t c3 = mad_wide((uint32_t)x.w, w, c2);
+    const uint64_t A = warp_sum_u64(snap_s[lane]);
+    uint64_t inc = c3;   // inclusive scan of the lanes' step sums
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint64_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    const uint64_t base = A + inc - c3;
+    c0 += base; c1 += base; c2 += base; c3 += base;   // F at prefix lengths q+1 .. q+4
     for (int a0 = 0; a0 <= rank; a0 += 32) {
         const int a = a0 + lane;
-        int64_t Lp = -1;
+        int rel = -1;
         if (a <= rank) {
-            Lp = gln[a];
-            const int64_t rel = Lp - 1 - win0;
-            if (!(Lp <= Li && rel >= 0 && (rel >> 7) == s)) Lp = -1;
+            const int64_t Lp = gln[a];
+            const int64_t r = Lp - 1 - win0 - 128 * (int64_t)s;
+            if (Lp <= Li && r >= 0 && r < 128) rel = (int)r;
         }
-        unsigned hits = __ballot_sync(0xffffffffu, Lp >= 0);
-        while (hits) {
-            const int src = __ffs(hits) - 1;
-            hits &= hits - 1;
-            const int64_t P = __shfl_sync(0xffffffffu, Lp, src);
-            const uint64_t part = (q < P ? t0 : 0) + (q + 1 < P ? t1 : 0) + (q + 2 < P ? t2 : 0) + (q + 3 < P ? t3 : 0);
-            const uint64_t tot = warp_sum_u64(acc + part * pw);
-            if (lane == 0) ent_hash[ebase + a0 + src] = tot;
+        if (!__any_sync(0xffffffffu, rel >= 0)) continue;
+        const int sl = rel >= 0 ? rel >> 2 : 0;
+        const uint64_t v0 = __shfl_sync(0xffffffffu, c0, sl), v1 = __shfl_sync(0xffffffffu, c1, sl);
+        const uint64_t v2 = __shfl_sync(0xffffffffu, c2, sl), v3 = __shfl_sync(0xffffffffu, c3, sl);
+        if (rel >= 0) {
+            const int e = rel & 3;
+            p.ent_hash[ebase + a] = e == 0 ? v0 : e == 1 ? v1 : e == 2 ? v2 : v3;
         }
     }
 }
 
-// One 2048-token window of timeline i.  Returns the warp-total of the window's terms.  kInterior: the window lies entirely
-// inside the timeline (no masking needed).  kLink: the window also holds positions of the in-group predecessor (length Lprev
-// <= L_i, tokens at tprev): they are compared exactly with this timeline's tokens while both stream by (the predecessor was
-// hashed moments ago, so its tokens come from L2); `diff` collects any difference.  Four batches of four 16-byte loads.
-template <bool kInterior, bool kLink>
-__device__ __forceinline__ uint64_t hash_window(const MergeParams& p, int lane, int64_t off, int Li, int64_t win0, uint64_t pw,
-                                                uint64_t B128, uint32_t stepmask, const int32_t* __restrict__ gln, int rank,
-                                                int ebase, const int32_t* __restrict__ tprev, int Lprev, uint32_t& diff) {
-    const int32_t* __restrict__ tok = p.tokens;
-    const int64_t q0 = win0 + lane * 4;   // timeline position of this lane's first slot in step 0
-    uint64_t acc = 0;
-#pragma unroll 1
-    for (int h = 0; h < 4; ++h) {
-        if (!kInterior && win0 + 512 * (int64_t)h >= Li) break;
-        int4 x[4];
-        int32_t y[4][4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int64_t q = q0 + 128 * (int64_t)(h * 4 + u);
-            const int64_t e = off + q;  // element index; 16-byte aligned address
-            if (kInterior) x[u] = __ldg(reinterpret_cast<const int4*>(tok + e));
-            else {
-                x[u] = make_int4(0, 0, 0, 0);
-                if (q + 3 >= 0 && q < Li) {
-                    if (e >= 0 && e + 3 < p.N) x[u] = __ldg(reinterpret_cast<const int4*>(tok + e));
-                    else {
-                        if (e >= 0 && e < p.N) x[u].x = tok[e];
-                        if (e + 1 >= 0 && e + 1 < p.N) x[u].y = tok[e + 1];
-                        if (e + 2 >= 0 && e + 2 < p.N) x[u].z = tok[e + 2];
-                        if (e + 3 >= 0 && e + 3 < p.N) x[u].w = tok[e + 3];
-                    }
-                }
-            }
-            if (kLink) {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) y[u][k] = (q + k >= 0 && q + k < Lprev) ? __ldg(tprev + q + k) : 0;
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int s = h * 4 + u;
-            const int64_t q = q0 + 128 * (int64_t)s;
-            if (kLink) {
-                if (q >= 0 && q < Lprev) diff |= (uint32_t)(y[u][0] ^ x[u].x);
-                if (q + 1 >= 0 && q + 1 < Lprev) diff |= (uint32_t)(y[u][1] ^ x[u].y);
-                if (q + 2 >= 0 && q + 2 < Lprev) diff |= (uint32_t)(y[u][2] ^ x[u].z);
-                if (q + 3 >= 0 && q + 3 < Lprev) diff |= (uint32_t)(y[u][3] ^ x[u].w);
-            }
-            uint64_t t0 = tok_term<0>(x[u].x), t1 = tok_term<1>(x[u].y), t2 = tok_term<2>(x[u].z), t3 = tok_term<3>(x[u].w);
-            if (!kInterior) {
-                if (!(q >= 0 && q < Li)) t0 = 0;
-                if (!(q + 1 >= 0 && q + 1 < Li)) t1 = 0;
-                if (!(q + 2 >= 0 && q + 2 < Li)) t2 = 0;
-                if (!(q + 3 >= 0 && q + 3 < Li)) t3 = 0;
-            }
-            if (stepmask & (1u << s)) hash_emit(p.ent_hash, gln, rank, ebase, win0, Li, s, q, t0, t1, t2, t3, acc, pw);
-            acc += ((t0 + t1) + (t2 + t3)) * pw;
-            pw *= B128;
-        }
-    }
-    return warp_sum_u64(acc);
-}
-
-__global__ void __launch_bounds__(256, 2) merge_hash_kernel(const MergeParams p) {
+__global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const MergeParams p) {
+    __shared__ uint64_t s_snap[kHashThreads / 32][16 * 32];   // per warp: running sums before each step of the window
     if (fatal(p)) return;
     const int lane = threadIdx.x & 31;
     const int wglobal = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
     const int nseg = p.ctrl->n_hash_segs, n = p.n;
-    // Striped windows: at any moment the grid works on ~nwarps consecutive windows (a front of ~20 MB that sweeps the token
+    uint64_t* snap = s_snap[threadIdx.x >> 5] + lane;
+    // Striped windows: at any moment the grid works on ~nwarps consecutive windows (a front of ~30 MB that sweeps the token
     // array once), so a timeline's in-group predecessor, hashed a little earlier, is still in L2 when it is compared.
-    const uint64_t LB = pow64(kB, (uint64_t)(4 * lane)), B128 = pow64(kB, 128);
+    const uint32_t LW = cpow_dev(kW, (uint32_t)(4 * lane));
     auto seg_base = [&](int i) { return reinterpret_cast<const int32_t*>(p.tl_rec)[4 * i]; };
     for (int sidx = wglobal; sidx < nseg; sidx += nwarps) {
         const int i = warp_search_last_le(n, sidx, seg_base);
@@ -502,7 +526,7 @@ __global__ void __launch_bounds__(256, 2) merge_hash_kernel(const MergeParams p)
             if (lp <= Li) { Lprev = lp; tprev = p.tokens + op; }
         }
         const int64_t win0 = ((wfirst + (sidx - rec.x)) << kHSegLog) - p.mis - off;   // timeline position of the window's first slot
-        const uint64_t X = powB(win0 + 3);   // B^(win0 + 3)
+        const uint32_t w0 = powW(win0 + 3) * LW;   // weight of this lane's first slot
         const int rank = rec.z, ebase = rec.w;
         const int32_t* gln = p.glen + rec.y;
         // which 128-token steps of this window hold the end of a requested prefix (L_a of an earlier member, or L_i)
@@ -516,16 +540,40 @@ __global__ void __launch_bounds__(256, 2) merge_hash_kernel(const MergeParams p)
             }
         }
         stepmask = __reduce_or_sync(0xffffffffu, stepmask);
-        const uint64_t pw = X * LB;
-        const bool interior = win0 >= 0 && win0 + kHSeg <= Li, link = win0 < Lprev;
+        // ---- streaming pass: four batches of 512 positions
+        uint32_t w[4] = {w0, w0 * kW, w0 * kW * kW, w0 * kW * kW * kW};
         uint32_t diff = 0;
-        uint64_t tot;
-        if (interior && link) tot = hash_window<true, true>(p, lane, off, Li, win0, pw, B128, stepmask, gln, rank, ebase, tprev, Lprev, diff);
-        else if (interior) tot = hash_window<true, false>(p, lane, off, Li, win0, pw, B128, stepmask, gln, rank, ebase, tprev, Lprev, diff);
-        else if (link) tot = hash_window<false, true>(p, lane, off, Li, win0, pw, B128, stepmask, gln, rank, ebase, tprev, Lprev, diff);
-        else tot = hash_window<false, false>(p, lane, off, Li, win0, pw, B128, stepmask, gln, rank, ebase, tprev, Lprev, diff);
+        uint64_t acc = 0;
+        const int64_t q0 = win0 + lane * 4;
+#pragma unroll 1
+        for (int h = 0; h < 4; ++h) {
+            const int64_t b0 = win0 + 512 * h, b1 = b0 + 512;
+            if (b0 >= Li) {   // nothing of the timeline here
+#pragma unroll
+                for (int u = 0; u < 4; ++u) snap[(h * 4 + u) * 32] = acc;
+                continue;
+            }
+            const bool interior = b0 >= 0 && b1 <= Li;
+            const int64_t qb = q0 + 512 * h;
+            uint64_t* sn = snap + h * 4 * 32;
+#define AJT_HB(I, K) hash_batch<I, K>(p, off, Li, qb, tprev, Lprev, w, acc, diff, sn)
+            if (interior && b1 <= Lprev) AJT_HB(true, 2);
+            else if (interior && b0 < Lprev) AJT_HB(true, 1);
+            else if (interior) AJT_HB(true, 0);
+            else if (b0 < Lprev) AJT_HB(false, 1);
+            else AJT_HB(false, 0);
+#undef AJT_HB
+        }
+        const uint64_t tot = warp_sum_u64(acc);
         if (lane == 0) p.seg_part[sidx] = tot;
-        if (link && __any_sync(0xffffffffu, diff != 0) && lane == 0) p.link_bad[i] = 1;
+        if (win0 < Lprev && __any_sync(0xffffffffu, diff != 0) && lane == 0) p.link_bad[i] = 1;
+        // ---- key emission pass: only the steps that hold the end of a requested prefix
+        __syncwarp();
+        for (uint32_t sm = stepmask; sm; sm &= sm - 1) {
+            const int s = __ffs(sm) - 1;
+            hash_emit_step(p, off, Li, win0, s, w0, snap + s * 32 - lane, gln, rank, ebase);
+        }
+        __syncwarp();
     }
 }
 
@@ -1210,7 +1258,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     }
     const size_t grp_dyn = n <= kGrpSmemN ? 5 * (((size_t)n + 4) & ~(size_t)3) * 4 : 0;
     merge_group_kernel<<<1, 1024, grp_dyn, stream>>>(p);
-    merge_hash_kernel<<<num_sms * 2, 256, 0, stream>>>(p);
+    merge_hash_kernel<<<num_sms * 3, 256, 0, stream>>>(p);
     merge_select_kernel<<<num_sms * 4, kSelThreads, 0, stream>>>(p);
     merge_compact_kernel<<<1, 1024, 0, stream>>>(p);
     merge_scatter_kernel<<<num_sms * 4, kScatThreads, 0, stream>>>(p);
