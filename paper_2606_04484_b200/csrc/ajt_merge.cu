@@ -49,6 +49,7 @@ constexpr uint32_t cpow32(uint32_t b, uint32_t e) {
 }
 constexpr uint32_t kWinv = inv32(kW);
 constexpr uint32_t kW128 = cpow32(kW, 128);
+constexpr uint32_t kW2048 = cpow32(kW, 2048);
 static_assert((uint32_t)(kW * kWinv) == 1u, "modular inverse");
 constexpr uint32_t kFatal = AJT_STATUS_BAD_OFFSETS | AJT_STATUS_ZERO_LEN | AJT_STATUS_PROBE_CAPACITY;
 constexpr int kSelThreads = 256;
@@ -142,7 +143,7 @@ __device__ __forceinline__ uint64_t warp_sum_u64(uint64_t v) {
     for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
-__device__ __forceinline__ int64_t tl_len(const MergeParams& p, int i) { return p.offsets[i + 1] - p.offsets[i]; }
+__device__ __forceinline__ int64_t tl_len(const MergeParams& p, int i) { return __ldg(p.offsets + i + 1) - __ldg(p.offsets + i); }
 
 // Last index i in [0, n) with key(i) <= x, for a non-decreasing key with key(0) <= x: warp-cooperative 32-ary search
 // (3 dependent loads for n <= 32768 instead of 15).
@@ -165,22 +166,29 @@ __device__ __forceinline__ int warp_search_last_le(int n, int64_t x, F key) {
 // ---------------------------------------------------------------------------------------- block-level building blocks
 
 // Exclusive scan of the pair f(i) = (a, b), i in [0,n), by one CTA of NT threads; g(i, ex_a, ex_b, a, b) consumes it.
-// The loads of the next tile (f) are issued before the current tile is scanned, so their latency overlaps.  Returns the
-// totals to every thread.  One __syncthreads per tile of NT (double-buffered warp totals).
+// Each thread owns kIpt consecutive items of a tile of NT * kIpt, so a tile costs one warp scan, one __syncthreads and one
+// shuffle scan of the NT / 32 warp totals (double-buffered), whatever kIpt is.  Returns the totals to every thread.
 struct I2 {
     int64_t a, b;
 };
+constexpr int kIpt = 4;
 template <int NT, class F, class G>
 __device__ __forceinline__ I2 block_scan2(int n, F f, G g, int64_t (*s_w)[2][NT / 32]) {
+    static_assert(NT / 32 <= 32, "warp totals are scanned by one warp's lanes");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     I2 base = {0, 0};
     int buf = 0;
-    I2 nxt = tid < n ? f(tid) : I2{0, 0};
-    for (int i0 = 0; i0 < n; i0 += NT, buf ^= 1) {
-        const int i = i0 + tid;
-        const I2 v = nxt;
-        nxt = i + NT < n ? f(i + NT) : I2{0, 0};
-        int64_t ia = v.a, ib = v.b;
+    for (int i0 = 0; i0 < n; i0 += NT * kIpt, buf ^= 1) {
+        const int b0 = i0 + tid * kIpt;
+        I2 v[kIpt];
+        int64_t sa = 0, sb = 0;
+#pragma unroll
+        for (int k = 0; k < kIpt; ++k) {
+            v[k] = b0 + k < n ? f(b0 + k) : I2{0, 0};
+            sa += v[k].a;
+            sb += v[k].b;
+        }
+        int64_t ia = sa, ib = sb;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const int64_t ta = __shfl_up_sync(0xffffffffu, ia, o), tb = __shfl_up_sync(0xffffffffu, ib, o);
@@ -188,14 +196,22 @@ __device__ __forceinline__ I2 block_scan2(int n, F f, G g, int64_t (*s_w)[2][NT 
         }
         if (lane == 31) { s_w[buf][0][warp] = ia; s_w[buf][1][warp] = ib; }
         __syncthreads();
-        int64_t pa = 0, pb = 0, ta = 0, tb = 0;
+        const int64_t wa = lane < NT / 32 ? s_w[buf][0][lane] : 0, wb = lane < NT / 32 ? s_w[buf][1][lane] : 0;
+        int64_t ja = wa, jb = wb;
 #pragma unroll
-        for (int w = 0; w < NT / 32; ++w) {
-            const int64_t ca = s_w[buf][0][w], cb = s_w[buf][1][w];
-            if (w < warp) { pa += ca; pb += cb; }
-            ta += ca; tb += cb;
+        for (int o = 1; o < NT / 32; o <<= 1) {
+            const int64_t ta = __shfl_up_sync(0xffffffffu, ja, o), tb = __shfl_up_sync(0xffffffffu, jb, o);
+            if (lane >= o) { ja += ta; jb += tb; }
         }
-        if (i < n) g(i, base.a + pa + ia - v.a, base.b + pb + ib - v.b, v.a, v.b);
+        const int64_t pa = __shfl_sync(0xffffffffu, ja - wa, warp), pb = __shfl_sync(0xffffffffu, jb - wb, warp);
+        const int64_t ta = __shfl_sync(0xffffffffu, ja, NT / 32 - 1), tb = __shfl_sync(0xffffffffu, jb, NT / 32 - 1);
+        int64_t ra = base.a + pa + ia - sa, rb = base.b + pb + ib - sb;
+#pragma unroll
+        for (int k = 0; k < kIpt; ++k) {
+            if (b0 + k < n) g(b0 + k, ra, rb, v[k].a, v[k].b);
+            ra += v[k].a;
+            rb += v[k].b;
+        }
         base.a += ta; base.b += tb;
     }
     __syncthreads();
@@ -209,26 +225,69 @@ __device__ __forceinline__ int64_t block_scan(int n, F f, G g, int64_t (*s_w)[2]
         .a;
 }
 
+// Lanes of the warp whose 8-bit digit equals this lane's (and that are valid): eight ballots instead of match.any, whose
+// cost grows with the number of distinct values in the warp (32 when trajectory ids arrive round-robin).
+__device__ __forceinline__ unsigned peers8(uint32_t d, bool valid) {
+    unsigned m = __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+        const unsigned v = __ballot_sync(0xffffffffu, (d >> b) & 1u);
+        m &= ((d >> b) & 1u) ? v : ~v;
+    }
+    return valid ? m : 0u;
+}
+
 template <int NW>
 struct RadixScratch {
     uint32_t cnt[NW][256];
     uint32_t off[256];
 };
 
-// One stable LSD pass (8-bit digit at `shift`) of (key, value) pairs by one CTA of NW warps.  Ranking inside a tile of
-// NW*32 keys: lanes with equal digits find each other with match.any; the lowest lane of each peer set posts the set size
-// in cnt[warp][digit]; one thread per digit turns the NW counts into running offsets; position = that + rank in peer set.
+// One stable LSD pass (8-bit digit at `shift`) of (key, value) pairs by one CTA of NW warps.  Warp w owns the w-th
+// contiguous chunk of the input, so "chunk, then round, then lane" is input order.  Count: per round, lanes with equal
+// digits find each other with match.any and the lowest lane of each peer set adds the set size to cnt[w][digit].  Offsets:
+// one thread per digit turns the NW counts into running offsets, one warp scans the 256 digit totals.  Scatter: the same
+// rounds again, position = digit base + warp offset + rank in peer set.  Four __syncthreads per pass, whatever n is.
+#ifdef AJT_TIMING
+__device__ uint64_t g_rt[8];
+#define AJT_RT(k) do { __syncthreads(); if (threadIdx.x == 0) { uint64_t t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_rt[k] = t_; } } while (0)
+#else
+#define AJT_RT(k) do { } while (0)
+#endif
 template <int NW>
 __device__ void radix_pass(const uint32_t* kin, const uint32_t* vin, uint32_t* kout, uint32_t* vout, int n, int shift,
                            RadixScratch<NW>& sc) {
+    AJT_RT(0);
     constexpr int NT = NW * 32;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int d = tid; d < 256; d += NT) sc.off[d] = 0;
     for (int x = tid; x < NW * 256; x += NT) (&sc.cnt[0][0])[x] = 0;
     __syncthreads();
-    for (int i = tid; i < n; i += NT) atomicAdd(&sc.off[(kin[i] >> shift) & 255u], 1u);
+    AJT_RT(1);
+    const int per = ((n + NW - 1) / NW + 31) & ~31;
+    const int c0 = min(n, warp * per), c1 = min(n, c0 + per);
+    for (int base = c0; base < c1; base += 32) {
+        const int i = base + lane;
+        const bool valid = i < c1;
+        const uint32_t d = valid ? (kin[i] >> shift) & 255u : 0u;
+        const unsigned peers = peers8(d, valid);
+        if (valid && lane == __ffs(peers) - 1) sc.cnt[warp][d] += (uint32_t)__popc(peers);
+        __syncwarp();
+    }
     __syncthreads();
-    if (warp == 0) {  // exclusive scan of the 256-bin histogram: 8 bins per lane
+    AJT_RT(2);
+    for (int d2 = tid; d2 < 256; d2 += NT) {
+        uint32_t run = 0;
+#pragma unroll 8
+        for (int w = 0; w < NW; ++w) {
+            const uint32_t c = sc.cnt[w][d2];
+            sc.cnt[w][d2] = run;
+            run += c;
+        }
+        sc.off[d2] = run;
+    }
+    __syncthreads();
+    AJT_RT(3);
+    if (warp == 0) {  // exclusive scan of the 256 digit totals: 8 per lane
         uint32_t loc[8], s = 0;
 #pragma unroll
         for (int j = 0; j < 8; ++j) { loc[j] = sc.off[lane * 8 + j]; s += loc[j]; }
@@ -243,40 +302,41 @@ __device__ void radix_pass(const uint32_t* kin, const uint32_t* vin, uint32_t* k
         for (int j = 0; j < 8; ++j) { sc.off[lane * 8 + j] = run; run += loc[j]; }
     }
     __syncthreads();
-    for (int base = 0; base < n; base += NT) {
-        const int i = base + tid;
-        const bool valid = i < n;
+    AJT_RT(4);
+    for (int base = c0; base < c1; base += 32) {
+        const int i = base + lane;
+        const bool valid = i < c1;
         const uint32_t key = valid ? kin[i] : 0u;
         const uint32_t val = valid ? vin[i] : 0u;
         const uint32_t d = (key >> shift) & 255u;
-        const unsigned peers = __match_any_sync(0xffffffffu, valid ? d : (0x100u | (uint32_t)lane));
+        const unsigned peers = peers8(d, valid);
         const int rk = __popc(peers & ((1u << lane) - 1u));
-        if (valid && rk == 0) sc.cnt[warp][d] = (uint32_t)__popc(peers);
-        __syncthreads();
-        for (int d2 = tid; d2 < 256; d2 += NT) {
-            uint32_t run = sc.off[d2];
-#pragma unroll 8
-            for (int w = 0; w < NW; ++w) {
-                const uint32_t c = sc.cnt[w][d2];
-                if (c) { sc.cnt[w][d2] = run; run += c; }
-            }
-            sc.off[d2] = run;
-        }
-        __syncthreads();
         if (valid) {
-            const uint32_t pos = sc.cnt[warp][d] + (uint32_t)rk;
+            const uint32_t pos = sc.off[d] + sc.cnt[warp][d] + (uint32_t)rk;
             kout[pos] = key;
             vout[pos] = val;
         }
-        __syncthreads();
-        if (valid && rk == 0) sc.cnt[warp][d] = 0;  // leave the table clean for the next tile
-        __syncthreads();
+        __syncwarp();
+        if (valid && rk == 0) sc.cnt[warp][d] += (uint32_t)__popc(peers);
+        __syncwarp();
     }
+    __syncthreads();
+    AJT_RT(5);
 }
 
 // ---------------------------------------------------------------------------------------- K1: group (M1)
 
+#ifdef AJT_TIMING
+#define AJT_TICK(k) do { __syncthreads(); if (threadIdx.x == 0) { uint64_t t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); tick_[k] = t_; } } while (0)
+#else
+#define AJT_TICK(k) do { } while (0)
+#endif
+template <bool kSmem>
 __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) {
+#ifdef AJT_TIMING
+    uint64_t tick_[10] = {0};
+#endif
+    AJT_TICK(0);
     extern __shared__ __align__(16) uint8_t g_dyn[];
     __shared__ RadixScratch<32> sc;
     __shared__ int64_t s_w[2][2][32];
@@ -284,35 +344,40 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
     __shared__ uint32_t s_bad;
     const int tid = threadIdx.x, n = p.n;
     // five [n+1] work arrays: shared memory for n <= kGrpSmemN, the workspace otherwise
-    uint32_t* buf[5];
-    {
-        const size_t nn = ((size_t)n + 4) & ~(size_t)3;
-        for (int k = 0; k < 5; ++k) buf[k] = n <= kGrpSmemN ? reinterpret_cast<uint32_t*>(g_dyn) + k * nn : p.gbuf[k];
-    }
-    uint32_t* kb[2] = {buf[0], buf[1]};
-    uint32_t* vb[2] = {buf[2], buf[3]};
-    int32_t* nsg = reinterpret_cast<int32_t*>(buf[4]);
+    const size_t nn = ((size_t)n + 4) & ~(size_t)3;
+    uint32_t* const sm32 = reinterpret_cast<uint32_t*>(g_dyn);
+    uint32_t* kb[2] = {kSmem ? sm32 : p.gbuf[0], kSmem ? sm32 + nn : p.gbuf[1]};
+    uint32_t* vb[2] = {kSmem ? sm32 + 2 * nn : p.gbuf[2], kSmem ? sm32 + 3 * nn : p.gbuf[3]};
+    int32_t* nsg = reinterpret_cast<int32_t*>(kSmem ? sm32 + 4 * nn : p.gbuf[4]);
     if (tid < (int)(sizeof(AjtCtrl) / 4)) reinterpret_cast<uint32_t*>(p.ctrl)[tid] = 0;   // fresh control block
     if (tid == 0) { s_min = INT32_MAX; s_max = INT32_MIN; s_bad = 0; }
     __syncthreads();
     // validate offsets; min / max traj id; hash windows per timeline
     int lmin = INT32_MAX, lmax = INT32_MIN;
     uint32_t bad = 0;
+#pragma unroll 4
     for (int i = tid; i < n; i += 1024) {
-        const int64_t a = p.offsets[i], b = p.offsets[i + 1];
+        const int64_t a = __ldg(p.offsets + i), b = __ldg(p.offsets + i + 1);
         if (b < a || b - a > (int64_t)INT32_MAX) bad |= AJT_STATUS_BAD_OFFSETS;
         else if (b == a) bad |= AJT_STATUS_ZERO_LEN;
-        const int t = p.traj_ids[i];
+        const int t = __ldg(p.traj_ids + i);
         lmin = min(lmin, t);
         lmax = max(lmax, t);
         kb[0][i] = (uint32_t)t;
         vb[0][i] = (uint32_t)i;
-        p.link_bad[i] = 0;
         nsg[i] = (int32_t)(((b - 1 + p.mis) >> kHSegLog) - ((a + p.mis) >> kHSegLog) + 1);
+        p.link_bad[i] = 0;
     }
+    AJT_TICK(1);
     if (tid == 0 && (p.offsets[0] != 0 || p.offsets[n] != p.N)) bad |= AJT_STATUS_BAD_OFFSETS;
-    if (bad) atomicOr(&s_bad, bad);
-    if (lmin != INT32_MAX) { atomicMin(&s_min, lmin); atomicMax(&s_max, lmax); }
+    lmin = __reduce_min_sync(0xffffffffu, lmin);
+    lmax = __reduce_max_sync(0xffffffffu, lmax);
+    bad = __reduce_or_sync(0xffffffffu, bad);
+    if ((tid & 31) == 0) {
+        if (bad) atomicOr(&s_bad, bad);
+        atomicMin(&s_min, lmin);
+        atomicMax(&s_max, lmax);
+    }
     __syncthreads();
     if (s_bad) {
         if (tid == 0) atomicOr(&p.ctrl->status, s_bad);
@@ -328,40 +393,66 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
         cur ^= 1;
         __syncthreads();
     }
+    AJT_TICK(2);
     const uint32_t* key = kb[cur];
-    const uint32_t* val = vb[cur];
-    uint32_t* gid = kb[cur ^ 1];    // [pos] group id
-    uint32_t* gsv = vb[cur ^ 1];    // [g]   first sorted position of group g
+    const uint32_t* val = vb[cur];   // sorted position -> timeline index
+    uint32_t* gid = kb[cur ^ 1];     // [pos] group id
+    uint32_t* gsv = vb[cur ^ 1];     // [g]   first sorted position of group g
     // group ids and group starts
     const int G = (int)block_scan<1024>(
         n, [&](int pos) { return (pos == 0 || key[pos] != key[pos - 1]) ? 1 : 0; },
         [&](int pos, int64_t ex, int64_t v) {
             const int g = (int)(ex + v) - 1;
             gid[pos] = (uint32_t)g;
-            p.perm[pos] = (int32_t)val[pos];
             if (v) { gsv[g] = (uint32_t)pos; p.grp_start[g] = pos; }
         },
         s_w);
     if (tid == 0) { gsv[G] = (uint32_t)n; p.grp_start[G] = n; }
     __syncthreads();
-    uint32_t* gsz = kb[cur];        // [i] size of the group of timeline i (the sorted keys are no longer needed)
-    int32_t* rec = reinterpret_cast<int32_t*>(p.tl_rec);
-    // rank in group; key slots (i, a), a = 0..rank  ->  rank+1 slots per timeline
+    AJT_TICK(3);
+    // singleton groups need no hashing: no windows
+    for (int pos = tid; pos < n; pos += 1024) {
+        const int g = (int)gid[pos];
+        if (gsv[g + 1] - gsv[g] < 2) nsg[val[pos]] = 0;
+    }
+    // key slots (i, a), a = 0..rank_i: a group of k timelines has k(k+1)/2, the slots of rank r start r(r+1)/2 into it
+    uint32_t* gent = kb[cur];        // [g] first key slot of group g (the sorted keys are no longer needed)
     const int64_t E = block_scan<1024>(
-        n, [&](int pos) { return (int)(pos - gsv[gid[pos]]) + 1; },
-        [&](int pos, int64_t ex, int64_t v) {
-            const int i = (int)val[pos], g = (int)gid[pos];
-            rec[4 * i + 1] = (int32_t)gsv[g];
-            rec[4 * i + 2] = (int32_t)v - 1;
-            rec[4 * i + 3] = (int32_t)ex;
-            gsz[i] = gsv[g + 1] - gsv[g];
-            if (v == 1) p.grp_ent[g] = (int32_t)ex;
-            p.glen[pos] = (int32_t)tl_len(p, i);
+        G, [&](int g) { const int64_t k = gsv[g + 1] - gsv[g]; return k * (k + 1) / 2; },
+        [&](int g, int64_t ex, int64_t) {
+            gent[g] = (uint32_t)min(ex, (int64_t)INT32_MAX);
+            p.grp_ent[g] = (int32_t)min(ex, (int64_t)INT32_MAX);
         },
         s_w);
-    // hash segments: aligned windows of kHSeg tokens intersected with each timeline (none for singleton groups)
+    AJT_TICK(4);
+    // hash segments: aligned windows of kHSeg tokens intersected with each timeline, numbered in timeline order
     const int64_t nseg = block_scan<1024>(
-        n, [&](int i) { return gsz[i] < 2 ? 0 : nsg[i]; }, [&](int i, int64_t ex, int64_t) { rec[4 * i] = (int32_t)ex; }, s_w);
+        n, [&](int i) { return nsg[i]; }, [&](int i, int64_t ex, int64_t) { nsg[i] = (int32_t)ex; }, s_w);
+    AJT_TICK(5);
+    for (int pos0 = 0; pos0 < n; pos0 += 8 * 1024) {   // all loads of 8 items first, then their stores
+        int4 rec[8];
+        int32_t len[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int pos = pos0 + k * 1024 + tid;
+            if (pos < n) {
+                const int i = (int)val[pos], g = (int)gid[pos];
+                const int gs = (int)gsv[g], r = pos - gs;
+                rec[k] = make_int4(nsg[i], gs, r, (int)(gent[g] + (uint32_t)r * (uint32_t)(r + 1) / 2u));
+                len[k] = (int32_t)tl_len(p, i);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int pos = pos0 + k * 1024 + tid;
+            if (pos < n) {
+                const int i = (int)val[pos];
+                p.tl_rec[i] = rec[k];
+                p.perm[pos] = i;
+                p.glen[pos] = len[k];
+            }
+        }
+    }
     if (tid == 0) {
         p.grp_ent[G] = (int32_t)min(E, (int64_t)INT32_MAX);
         p.ctrl->n_groups = G;
@@ -369,6 +460,13 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
         p.ctrl->n_hash_segs = (int32_t)nseg;
         if (E > (int64_t)p.E_cap || nseg > (int64_t)p.nseg_cap) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_PROBE_CAPACITY);
     }
+    AJT_TICK(6);
+#ifdef AJT_TIMING
+    if (tid == 0) {
+        for (int k = 0; k < 7; ++k) reinterpret_cast<uint64_t*>(p.ctrl->reserved)[k] = tick_[k];
+        for (int k = 0; k < 6; ++k) reinterpret_cast<uint64_t*>(p.ctrl->reserved)[8 + k] = g_rt[k];
+    }
+#endif
 }
 
 // ---------------------------------------------------------------------------------------- K2: prefix-hash scan (M2)
@@ -385,26 +483,44 @@ __device__ __forceinline__ uint32_t pow32(uint32_t b, uint32_t e) {
     }
     return r;
 }
-__device__ __forceinline__ uint32_t cpow_dev(uint32_t b, uint32_t e) { return pow32(b, e); }
-__device__ __forceinline__ uint32_t powW(int64_t e) { return e >= 0 ? pow32(kW, (uint32_t)e) : pow32(kWinv, (uint32_t)(-e)); }
+// Power tables (constant memory, warp-uniform reads): W^(win0 + 3) of a window that starts d = -win0 (mod 2048) slots before
+// a multiple of 2048, j windows into its timeline, is W2048^j * Winv^(64 (d >> 6)) * Winv^(d & 63) * W^3.
+template <int N>
+struct PowTab {
+    uint32_t v[N];
+    constexpr PowTab() : v{} {}
+    constexpr PowTab(uint32_t base) : v{} {
+        uint32_t r = 1;
+        for (int i = 0; i < N; ++i) { v[i] = r; r *= base; }
+    }
+};
+__constant__ PowTab<64> c_w2048 = PowTab<64>(cpow32(kW, 2048));
+__constant__ PowTab<32> c_winv64 = PowTab<32>(cpow32(kWinv, 64));
+__constant__ PowTab<64> c_winv1 = PowTab<64>(kWinv);
+__constant__ PowTab<16> c_w128 = PowTab<16>(kW128);
+__constant__ PowTab<32> c_w4 = PowTab<32>(cpow32(kW, 4));
+// weight of the first slot of window j of a timeline whose window grid starts d slots before its first token (0 <= d < 2048)
+__device__ __forceinline__ uint32_t window_weight(int j, int d) {
+    const uint32_t wj = j < 64 ? c_w2048.v[j] : pow32(kW2048, (uint32_t)j);
+    return wj * c_winv64.v[d >> 6] * c_winv1.v[d & 63] * (kW * kW * kW);
+}
 __device__ __forceinline__ uint64_t mad_wide(uint32_t a, uint32_t b, uint64_t c) { return (uint64_t)a * b + c; }
 
 constexpr int kHashThreads = 256;
 
-// This lane's four tokens of step s of a window (positions q .. q+3), zero outside the timeline.  16-byte aligned address.
+// This lane's four tokens of step s of a window (positions q .. q+3 of the timeline whose tokens start at tl), zero outside
+// the timeline.  16-byte aligned address.  lo / hi: how many elements may be read before tl / from tl (array bounds).
 template <bool kInterior>
-__device__ __forceinline__ int4 load_step(const MergeParams& p, int64_t off, int Li, int64_t q) {
-    const int32_t* __restrict__ tok = p.tokens;
-    const int64_t e = off + q;
-    if (kInterior) return __ldg(reinterpret_cast<const int4*>(tok + e));
+__device__ __forceinline__ int4 load_step(const int32_t* __restrict__ tl, int Li, int q, int64_t lo, int64_t hi) {
+    if (kInterior) return __ldg(reinterpret_cast<const int4*>(tl + q));
     int4 x = make_int4(0, 0, 0, 0);
     if (q + 3 >= 0 && q < Li) {
-        if (e >= 0 && e + 3 < p.N) x = __ldg(reinterpret_cast<const int4*>(tok + e));
+        if (q >= -lo && q + 3 < hi) x = __ldg(reinterpret_cast<const int4*>(tl + q));
         else {
-            if (e >= 0 && e < p.N) x.x = tok[e];
-            if (e + 1 >= 0 && e + 1 < p.N) x.y = tok[e + 1];
-            if (e + 2 >= 0 && e + 2 < p.N) x.z = tok[e + 2];
-            if (e + 3 >= 0 && e + 3 < p.N) x.w = tok[e + 3];
+            if (q >= -lo && q < hi) x.x = tl[q];
+            if (q + 1 >= -lo && q + 1 < hi) x.y = tl[q + 1];
+            if (q + 2 >= -lo && q + 2 < hi) x.z = tl[q + 2];
+            if (q + 3 >= -lo && q + 3 < hi) x.w = tl[q + 3];
         }
         if (!(q >= 0 && q < Li)) x.x = 0;
         if (!(q + 1 >= 0 && q + 1 < Li)) x.y = 0;
@@ -418,14 +534,15 @@ __device__ __forceinline__ int4 load_step(const MergeParams& p, int64_t off, int
 // linked).  kInterior: the batch lies inside the timeline.  kLink: 0 no predecessor positions here, 1 some, 2 all of them.
 // snap[s * 32] receives this lane's running sum BEFORE step s (the key-emission pass needs it); w are the lane's weights.
 template <bool kInterior, int kLink>
-__device__ __forceinline__ void hash_batch(const MergeParams& p, int64_t off, int Li, int64_t qb, const int32_t* __restrict__ tprev,
-                                           int Lprev, uint32_t (&w)[4], uint64_t& acc, uint32_t& diff, uint64_t* snap) {
+__device__ __forceinline__ void hash_batch(const int32_t* __restrict__ tl, int Li, int qb, int64_t lo, int64_t hi,
+                                           const int32_t* __restrict__ tprev, int Lprev, uint32_t (&w)[4], uint64_t& acc,
+                                           uint32_t& diff, uint64_t* snap) {
     int4 x[4];
     int32_t y[4][4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-        const int64_t q = qb + 128 * u;
-        x[u] = load_step<kInterior>(p, off, Li, q);
+        const int q = qb + 128 * u;
+        x[u] = load_step<kInterior>(tl, Li, q, lo, hi);
         if (kLink == 2) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) y[u][k] = __ldg(tprev + q + k);
@@ -436,7 +553,7 @@ __device__ __forceinline__ void hash_batch(const MergeParams& p, int64_t off, in
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-        const int64_t q = qb + 128 * u;
+        const int q = qb + 128 * u;
         if (kLink == 2) {
             diff |= (uint32_t)(y[u][0] ^ x[u].x) | (uint32_t)(y[u][1] ^ x[u].y);
             diff |= (uint32_t)(y[u][2] ^ x[u].z) | (uint32_t)(y[u][3] ^ x[u].w);
@@ -458,12 +575,13 @@ __device__ __forceinline__ void hash_batch(const MergeParams& p, int64_t off, in
 // Keys whose prefix ends inside step s of the window: the step's tokens are re-read (L1), the lane's four inclusive prefix
 // values are formed from its snapshot, one warp sum and one warp scan turn them into F at every position of the step, and each
 // key picks its value from the lane that holds its last token.  One pass serves any number of keys ending in the step.
-__device__ __noinline__ void hash_emit_step(const MergeParams& p, int64_t off, int Li, int64_t win0, int s, uint32_t w0_window,
-                                            const uint64_t* snap_s, const int32_t* __restrict__ gln, int rank, int ebase) {
+__device__ __noinline__ void hash_emit_step(uint64_t* __restrict__ ent_hash, const int32_t* __restrict__ tl, int Li, int64_t lo,
+                                            int64_t hi, int win0, int s, uint32_t w0_window, const uint64_t* snap_s,
+                                            const int32_t* __restrict__ gln, int rank, int ebase) {
     const int lane = threadIdx.x & 31;
-    const int64_t q = win0 + 128 * (int64_t)s + 4 * lane;
-    const int4 x = load_step<false>(p, off, Li, q);
-    uint32_t w = w0_window * cpow_dev(kW128, (uint32_t)s);
+    const int q = win0 + 128 * s + 4 * lane;
+    const int4 x = load_step<false>(tl, Li, q, lo, hi);
+    uint32_t w = w0_window * c_w128.v[s];
     uint64_t c0 = (uint64_t)(uint32_t)x.x * w;
     w *= kW;
     uint64_t c1 = mad_wide((uint32_t)x.y, w, c0);
@@ -484,9 +602,9 @@ __device__ __noinline__ void hash_emit_step(const MergeParams& p, int64_t off, i
         const int a = a0 + lane;
         int rel = -1;
         if (a <= rank) {
-            const int64_t Lp = gln[a];
-            const int64_t r = Lp - 1 - win0 - 128 * (int64_t)s;
-            if (Lp <= Li && r >= 0 && r < 128) rel = (int)r;
+            const int Lp = gln[a];
+            const int r = Lp - 1 - win0 - 128 * s;
+            if (Lp <= Li && r >= 0 && r < 128) rel = r;
         }
         if (!__any_sync(0xffffffffu, rel >= 0)) continue;
         const int sl = rel >= 0 ? rel >> 2 : 0;
@@ -494,7 +612,7 @@ __device__ __noinline__ void hash_emit_step(const MergeParams& p, int64_t off, i
         const uint64_t v2 = __shfl_sync(0xffffffffu, c2, sl), v3 = __shfl_sync(0xffffffffu, c3, sl);
         if (rel >= 0) {
             const int e = rel & 3;
-            p.ent_hash[ebase + a] = e == 0 ? v0 : e == 1 ? v1 : e == 2 ? v2 : v3;
+            ent_hash[ebase + a] = e == 0 ? v0 : e == 1 ? v1 : e == 2 ? v2 : v3;
         }
     }
 }
@@ -508,25 +626,28 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
     uint64_t* snap = s_snap[threadIdx.x >> 5] + lane;
     // Striped windows: at any moment the grid works on ~nwarps consecutive windows (a front of ~30 MB that sweeps the token
     // array once), so a timeline's in-group predecessor, hashed a little earlier, is still in L2 when it is compared.
-    const uint32_t LW = cpow_dev(kW, (uint32_t)(4 * lane));
-    auto seg_base = [&](int i) { return reinterpret_cast<const int32_t*>(p.tl_rec)[4 * i]; };
+    const uint32_t LW = c_w4.v[lane];
+    auto seg_base = [&](int i) { return __ldg(reinterpret_cast<const int32_t*>(p.tl_rec) + 4 * i); };
     for (int sidx = wglobal; sidx < nseg; sidx += nwarps) {
         const int i = warp_search_last_le(n, sidx, seg_base);
-        const int4 rec = p.tl_rec[i];
-        const int64_t off = p.offsets[i];
-        const int Li = (int)(p.offsets[i + 1] - off);
-        const int64_t wfirst = (off + p.mis) >> kHSegLog;
+        const int4 rec = __ldg(p.tl_rec + i);
+        const int64_t off = __ldg(p.offsets + i);
+        const int Li = (int)(__ldg(p.offsets + i + 1) - off);
+        const int32_t* tl = p.tokens + off;
+        const int64_t lo = off, hi = p.N - off;   // elements of the token array before / from tl
         // the in-group predecessor, if this timeline can extend it (the usual case: each call resends the context)
         int Lprev = 0;
         const int32_t* tprev = nullptr;
         if (rec.z > 0) {
-            const int jp = p.perm[rec.y + rec.z - 1];
-            const int64_t op = p.offsets[jp];
-            const int lp = (int)(p.offsets[jp + 1] - op);
+            const int jp = __ldg(p.perm + rec.y + rec.z - 1);
+            const int64_t op = __ldg(p.offsets + jp);
+            const int lp = (int)(__ldg(p.offsets + jp + 1) - op);
             if (lp <= Li) { Lprev = lp; tprev = p.tokens + op; }
         }
-        const int64_t win0 = ((wfirst + (sidx - rec.x)) << kHSegLog) - p.mis - off;   // timeline position of the window's first slot
-        const uint32_t w0 = powW(win0 + 3) * LW;   // weight of this lane's first slot
+        const int d = (int)((off + p.mis) & (kHSeg - 1));   // the timeline starts d slots into its first window
+        const int j = sidx - rec.x;                          // window index inside the timeline
+        const int win0 = j * kHSeg - d;                      // timeline position of the window's first slot
+        const uint32_t w0 = window_weight(j, d) * LW;        // weight W^(q+3) of this lane's first slot q = win0 + 4 lane
         const int rank = rec.z, ebase = rec.w;
         const int32_t* gln = p.glen + rec.y;
         // which 128-token steps of this window hold the end of a requested prefix (L_a of an earlier member, or L_i)
@@ -534,9 +655,9 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
         for (int a0 = 0; a0 <= rank; a0 += 32) {
             const int a = a0 + lane;
             if (a <= rank) {
-                const int64_t Lp = gln[a];
-                const int64_t rel = Lp - 1 - win0;
-                if (Lp <= Li && rel >= 0 && rel < kHSeg) stepmask |= 1u << (int)(rel >> 7);
+                const int Lp = __ldg(gln + a);
+                const int rel = Lp - 1 - win0;
+                if (Lp <= Li && rel >= 0 && rel < kHSeg) stepmask |= 1u << (rel >> 7);
             }
         }
         stepmask = __reduce_or_sync(0xffffffffu, stepmask);
@@ -544,19 +665,19 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
         uint32_t w[4] = {w0, w0 * kW, w0 * kW * kW, w0 * kW * kW * kW};
         uint32_t diff = 0;
         uint64_t acc = 0;
-        const int64_t q0 = win0 + lane * 4;
+        const int q0 = win0 + lane * 4;
 #pragma unroll 1
         for (int h = 0; h < 4; ++h) {
-            const int64_t b0 = win0 + 512 * h, b1 = b0 + 512;
+            const int b0 = win0 + 512 * h, b1 = b0 + 512;
+            uint64_t* sn = snap + h * 4 * 32;
             if (b0 >= Li) {   // nothing of the timeline here
 #pragma unroll
-                for (int u = 0; u < 4; ++u) snap[(h * 4 + u) * 32] = acc;
+                for (int u = 0; u < 4; ++u) sn[u * 32] = acc;
                 continue;
             }
             const bool interior = b0 >= 0 && b1 <= Li;
-            const int64_t qb = q0 + 512 * h;
-            uint64_t* sn = snap + h * 4 * 32;
-#define AJT_HB(I, K) hash_batch<I, K>(p, off, Li, qb, tprev, Lprev, w, acc, diff, sn)
+            const int qb = q0 + 512 * h;
+#define AJT_HB(I, K) hash_batch<I, K>(tl, Li, qb, lo, hi, tprev, Lprev, w, acc, diff, sn)
             if (interior && b1 <= Lprev) AJT_HB(true, 2);
             else if (interior && b0 < Lprev) AJT_HB(true, 1);
             else if (interior) AJT_HB(true, 0);
@@ -571,7 +692,7 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
         __syncwarp();
         for (uint32_t sm = stepmask; sm; sm &= sm - 1) {
             const int s = __ffs(sm) - 1;
-            hash_emit_step(p, off, Li, win0, s, w0, snap + s * 32 - lane, gln, rank, ebase);
+            hash_emit_step(p.ent_hash, tl, Li, lo, hi, win0, s, w0, snap + s * 32 - lane, gln, rank, ebase);
         }
         __syncwarp();
     }
@@ -831,7 +952,7 @@ __device__ void compact_body(const MergeParams& p, int mode, int64_t (*s_w)[2][N
     const I2 tot = block_scan2<NT>(
         n,
         [&](int i) {
-            if (p.absorbed[i]) return I2{0, 0};
+            if (mode == 0 ? __ldg(p.absorbed + i) : p.absorbed[i]) return I2{0, 0};   // (mode 1: written earlier in this launch)
             const int64_t L = tl_len(p, i);
             return I2{((int64_t)1 << 32) | ((L + 3 + kTile - 1) / kTile), L};
         },
@@ -840,14 +961,15 @@ __device__ void compact_body(const MergeParams& p, int mode, int64_t (*s_w)[2][N
             const int m = (int)(exa >> 32);
             p.midx[i] = m;
             p.merged_origin[m] = i;
-            p.merged_traj[m] = p.traj_ids[i];
+            p.merged_traj[m] = __ldg(p.traj_ids + i);
             p.merged_offsets[m] = exb;
             p.tile_base[m] = (int32_t)(exa & 0xffffffff);
         },
         s_w);
     const int M = (int)(tot.a >> 32);
     const int32_t ntiles = (int32_t)(tot.a & 0xffffffff);
-    for (int i = tid; i < n; i += NT) p.owner[i] = p.midx[p.owner_tl[i]];
+#pragma unroll 4
+    for (int i = tid; i < n; i += NT) p.owner[i] = p.midx[mode == 0 ? __ldg(p.owner_tl + i) : p.owner_tl[i]];
     if (tid == 0) {
         p.merged_offsets[M] = tot.b;
         p.tile_base[M] = ntiles;
@@ -1248,7 +1370,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     static int s_repair_grid[64] = {0};
     if (dev < 0 || dev >= 64) return AJT_ERR_UNSUPPORTED;
     if (s_repair_grid[dev] == 0) {
-        if (cudaFuncSetAttribute(merge_group_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * (kGrpSmemN + 4) * 4) !=
+        if (cudaFuncSetAttribute(merge_group_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * (kGrpSmemN + 4) * 4) !=
             cudaSuccess)
             return AJT_ERR_CUDA;
         int per_sm = 0;
@@ -1256,8 +1378,8 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
             return AJT_ERR_CUDA;
         s_repair_grid[dev] = num_sms * (per_sm < 4 ? per_sm : 4);
     }
-    const size_t grp_dyn = n <= kGrpSmemN ? 5 * (((size_t)n + 4) & ~(size_t)3) * 4 : 0;
-    merge_group_kernel<<<1, 1024, grp_dyn, stream>>>(p);
+    if (n <= kGrpSmemN) merge_group_kernel<true><<<1, 1024, 5 * (((size_t)n + 4) & ~(size_t)3) * 4, stream>>>(p);
+    else merge_group_kernel<false><<<1, 1024, 0, stream>>>(p);
     merge_hash_kernel<<<num_sms * 3, 256, 0, stream>>>(p);
     merge_select_kernel<<<num_sms * 4, kSelThreads, 0, stream>>>(p);
     merge_compact_kernel<<<1, 1024, 0, stream>>>(p);
