@@ -57,7 +57,7 @@ constexpr int kSelSmemKeys = 2048;  // groups with more keys than this sort thro
 constexpr int kSelBucketBits = 11;
 constexpr int kSelBuckets = 1 << kSelBucketBits;
 constexpr int kSelCacheK = 256;     // per-timeline facts of groups up to this size are staged in shared memory
-constexpr int kGrpSmemN = 8192;     // batches up to this many timelines are grouped entirely in shared memory
+constexpr int kGrpSmemN = 7936;     // batches up to this many timelines are grouped entirely in shared memory
 
 struct MergeParams {
     const int32_t* tokens;
@@ -81,12 +81,13 @@ struct MergeParams {
     int64_t* counts;
     // workspace
     AjtCtrl* ctrl;
-    uint32_t* gbuf[5];     // [n+1] each: global stand-ins for the group kernel's shared arrays when n > kGrpSmemN
+    uint32_t* gbuf[6];     // [n+1] each: global stand-ins for the group kernel's shared arrays when n > kGrpSmemN
     int32_t* perm;         // [n] sorted position -> timeline index (groups contiguous, input order inside a group)
     int32_t* glen;         // [n] sorted position -> timeline length
     int32_t* grp_start;    // [G+1] first sorted position of each group
     int32_t* grp_ent;      // [G+1] first key slot of each group
-    int4* tl_rec;          // [n] {first hash segment, group start (sorted position), rank in group, first key slot}
+    int4* tl_rec;          // [n] BY SORTED POSITION: {first hash segment, group start (sorted position), rank in group, first key slot}
+    int32_t* tl_pos;       // [n] timeline index -> sorted position (written by the select kernel)
     uint64_t* seg_part;    // [nseg_cap] per-window partial sums, then exclusive prefixes per timeline
     uint64_t* ent_hash;    // [E_cap] key slot (i, a), a = 0..rank_i: in-window partial, then the final prefix hash
     uint32_t* ent_dig;     // [E_cap] global sort path: digests / order ping-pong
@@ -106,7 +107,7 @@ struct MergeParams {
 };
 
 struct MergeWs {
-    size_t ctrl, gbuf[5], perm, glen, grp_start, grp_ent, tl_rec, seg_part, absorbed, link_bad, needv, owner_tl, cand, midx, tile_base, ent;
+    size_t ctrl, gbuf[6], perm, glen, grp_start, grp_ent, tl_rec, tl_pos, seg_part, absorbed, link_bad, needv, owner_tl, cand, midx, tile_base, ent;
 };
 __host__ inline size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
 __host__ inline int32_t nseg_capacity(int32_t n, int64_t N) { return (int32_t)(N / kHSeg + 2 * (int64_t)n + 2); }
@@ -116,9 +117,10 @@ __host__ MergeWs merge_ws_layout(int32_t n, int64_t N) {
     size_t o = 0;
     const size_t n4 = a256(((size_t)n + 2) * 4);
     w.ctrl = o; o += 256;
-    for (int k = 0; k < 5; ++k) { w.gbuf[k] = o; o += n4; }
+    for (int k = 0; k < 6; ++k) { w.gbuf[k] = o; o += n4; }
     w.perm = o; o += n4; w.glen = o; o += n4; w.grp_start = o; o += n4; w.grp_ent = o; o += n4;
     w.tl_rec = o; o += a256(((size_t)n + 1) * 16);
+    w.tl_pos = o; o += n4;
     w.seg_part = o; o += a256((size_t)nseg_capacity(n, N) * 8);
     w.absorbed = o; o += a256((size_t)n + 1);
     w.link_bad = o; o += a256((size_t)n + 1);
@@ -225,12 +227,12 @@ __device__ __forceinline__ int64_t block_scan(int n, F f, G g, int64_t (*s_w)[2]
         .a;
 }
 
-// Lanes of the warp whose 8-bit digit equals this lane's (and that are valid): eight ballots instead of match.any, whose
+// Lanes of the warp whose nbits-bit digit equals this lane's (and that are valid): one ballot per bit instead of match.any, whose
 // cost grows with the number of distinct values in the warp (32 when trajectory ids arrive round-robin).
-__device__ __forceinline__ unsigned peers8(uint32_t d, bool valid) {
+__device__ __forceinline__ unsigned peers8(uint32_t d, bool valid, int nbits) {
     unsigned m = __ballot_sync(0xffffffffu, valid);
-#pragma unroll
-    for (int b = 0; b < 8; ++b) {
+#pragma unroll 1
+    for (int b = 0; b < nbits; ++b) {
         const unsigned v = __ballot_sync(0xffffffffu, (d >> b) & 1u);
         m &= ((d >> b) & 1u) ? v : ~v;
     }
@@ -243,7 +245,7 @@ struct RadixScratch {
     uint32_t off[256];
 };
 
-// One stable LSD pass (8-bit digit at `shift`) of (key, value) pairs by one CTA of NW warps.  Warp w owns the w-th
+// One stable LSD pass (digit of nbits <= 8 bits at `shift`) of (key, value) pairs by one CTA of NW warps.  Warp w owns the w-th
 // contiguous chunk of the input, so "chunk, then round, then lane" is input order.  Count: per round, lanes with equal
 // digits find each other with match.any and the lowest lane of each peer set adds the set size to cnt[w][digit].  Offsets:
 // one thread per digit turns the NW counts into running offsets, one warp scans the 256 digit totals.  Scatter: the same
@@ -255,8 +257,9 @@ __device__ uint64_t g_rt[8];
 #define AJT_RT(k) do { } while (0)
 #endif
 template <int NW>
-__device__ void radix_pass(const uint32_t* kin, const uint32_t* vin, uint32_t* kout, uint32_t* vout, int n, int shift,
-                           RadixScratch<NW>& sc) {
+__device__ __forceinline__ void radix_pass(const uint32_t* kin, const uint32_t* vin, uint32_t* kout, uint32_t* vout, int n,
+                                           int shift, RadixScratch<NW>& sc, int nbits = 8) {
+    const uint32_t dmask = (1u << nbits) - 1u;
     AJT_RT(0);
     constexpr int NT = NW * 32;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -268,8 +271,8 @@ __device__ void radix_pass(const uint32_t* kin, const uint32_t* vin, uint32_t* k
     for (int base = c0; base < c1; base += 32) {
         const int i = base + lane;
         const bool valid = i < c1;
-        const uint32_t d = valid ? (kin[i] >> shift) & 255u : 0u;
-        const unsigned peers = peers8(d, valid);
+        const uint32_t d = valid ? (kin[i] >> shift) & dmask : 0u;
+        const unsigned peers = peers8(d, valid, nbits);
         if (valid && lane == __ffs(peers) - 1) sc.cnt[warp][d] += (uint32_t)__popc(peers);
         __syncwarp();
     }
@@ -277,7 +280,7 @@ __device__ void radix_pass(const uint32_t* kin, const uint32_t* vin, uint32_t* k
     AJT_RT(2);
     for (int d2 = tid; d2 < 256; d2 += NT) {
         uint32_t run = 0;
-#pragma unroll 8
+#pragma unroll 4
         for (int w = 0; w < NW; ++w) {
             const uint32_t c = sc.cnt[w][d2];
             sc.cnt[w][d2] = run;
@@ -308,8 +311,8 @@ __device__ void radix_pass(const uint32_t* kin, const uint32_t* vin, uint32_t* k
         const bool valid = i < c1;
         const uint32_t key = valid ? kin[i] : 0u;
         const uint32_t val = valid ? vin[i] : 0u;
-        const uint32_t d = (key >> shift) & 255u;
-        const unsigned peers = peers8(d, valid);
+        const uint32_t d = (key >> shift) & dmask;
+        const unsigned peers = peers8(d, valid, nbits);
         const int rk = __popc(peers & ((1u << lane) - 1u));
         if (valid) {
             const uint32_t pos = sc.off[d] + sc.cnt[warp][d] + (uint32_t)rk;
@@ -344,11 +347,12 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
     __shared__ uint32_t s_bad;
     const int tid = threadIdx.x, n = p.n;
     // five [n+1] work arrays: shared memory for n <= kGrpSmemN, the workspace otherwise
-    const size_t nn = ((size_t)n + 4) & ~(size_t)3;
+    const size_t nn = ((size_t)n + 4) & ~(size_t)3;   // (6 arrays of nn words)
     uint32_t* const sm32 = reinterpret_cast<uint32_t*>(g_dyn);
     uint32_t* kb[2] = {kSmem ? sm32 : p.gbuf[0], kSmem ? sm32 + nn : p.gbuf[1]};
     uint32_t* vb[2] = {kSmem ? sm32 + 2 * nn : p.gbuf[2], kSmem ? sm32 + 3 * nn : p.gbuf[3]};
-    int32_t* nsg = reinterpret_cast<int32_t*>(kSmem ? sm32 + 4 * nn : p.gbuf[4]);
+    int32_t* nsg = reinterpret_cast<int32_t*>(kSmem ? sm32 + 4 * nn : p.gbuf[4]);   // [i] hash windows of timeline i
+    int32_t* tln = reinterpret_cast<int32_t*>(kSmem ? sm32 + 5 * nn : p.gbuf[5]);   // [i] its length
     if (tid < (int)(sizeof(AjtCtrl) / 4)) reinterpret_cast<uint32_t*>(p.ctrl)[tid] = 0;   // fresh control block
     if (tid == 0) { s_min = INT32_MAX; s_max = INT32_MIN; s_bad = 0; }
     __syncthreads();
@@ -366,6 +370,7 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
         kb[0][i] = (uint32_t)t;
         vb[0][i] = (uint32_t)i;
         nsg[i] = (int32_t)(((b - 1 + p.mis) >> kHSegLog) - ((a + p.mis) >> kHSegLog) + 1);
+        tln[i] = (int32_t)(b - a);
         p.link_bad[i] = 0;
     }
     AJT_TICK(1);
@@ -383,10 +388,12 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
         if (tid == 0) atomicOr(&p.ctrl->status, s_bad);
         return;
     }
+    AJT_TICK(7);
     const int tmin = s_min;
     const uint32_t range = n ? (uint32_t)s_max - (uint32_t)tmin : 0u;
     for (int i = tid; i < n; i += 1024) kb[0][i] -= (uint32_t)tmin;
     __syncthreads();
+    AJT_TICK(8);
     int cur = 0;
     for (int shift = 0; shift < 32 && (range >> shift) != 0; shift += 8) {
         radix_pass<32>(kb[cur], vb[cur], kb[cur ^ 1], vb[cur ^ 1], n, shift, sc);
@@ -410,11 +417,6 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
     if (tid == 0) { gsv[G] = (uint32_t)n; p.grp_start[G] = n; }
     __syncthreads();
     AJT_TICK(3);
-    // singleton groups need no hashing: no windows
-    for (int pos = tid; pos < n; pos += 1024) {
-        const int g = (int)gid[pos];
-        if (gsv[g + 1] - gsv[g] < 2) nsg[val[pos]] = 0;
-    }
     // key slots (i, a), a = 0..rank_i: a group of k timelines has k(k+1)/2, the slots of rank r start r(r+1)/2 into it
     uint32_t* gent = kb[cur];        // [g] first key slot of group g (the sorted keys are no longer needed)
     const int64_t E = block_scan<1024>(
@@ -425,34 +427,20 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
         },
         s_w);
     AJT_TICK(4);
-    // hash segments: aligned windows of kHSeg tokens intersected with each timeline, numbered in timeline order
+    // hash segments: aligned windows of kHSeg tokens intersected with each timeline (none for singleton groups), numbered in
+    // GROUP order, so that a timeline is hashed right after its in-group predecessor.  Everything the later kernels need
+    // per timeline goes out by sorted position: coalesced, no scattered access from this one CTA.
     const int64_t nseg = block_scan<1024>(
-        n, [&](int i) { return nsg[i]; }, [&](int i, int64_t ex, int64_t) { nsg[i] = (int32_t)ex; }, s_w);
+        n, [&](int pos) { const int g = (int)gid[pos]; return gsv[g + 1] - gsv[g] < 2 ? 0 : nsg[val[pos]]; },
+        [&](int pos, int64_t ex, int64_t) {
+            const int i = (int)val[pos], g = (int)gid[pos];
+            const int gs = (int)gsv[g], r = pos - gs;
+            p.tl_rec[pos] = make_int4((int)ex, gs, r, (int)(gent[g] + (uint32_t)r * (uint32_t)(r + 1) / 2u));
+            p.perm[pos] = i;
+            p.glen[pos] = tln[i];
+        },
+        s_w);
     AJT_TICK(5);
-    for (int pos0 = 0; pos0 < n; pos0 += 8 * 1024) {   // all loads of 8 items first, then their stores
-        int4 rec[8];
-        int32_t len[8];
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const int pos = pos0 + k * 1024 + tid;
-            if (pos < n) {
-                const int i = (int)val[pos], g = (int)gid[pos];
-                const int gs = (int)gsv[g], r = pos - gs;
-                rec[k] = make_int4(nsg[i], gs, r, (int)(gent[g] + (uint32_t)r * (uint32_t)(r + 1) / 2u));
-                len[k] = (int32_t)tl_len(p, i);
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const int pos = pos0 + k * 1024 + tid;
-            if (pos < n) {
-                const int i = (int)val[pos];
-                p.tl_rec[i] = rec[k];
-                p.perm[pos] = i;
-                p.glen[pos] = len[k];
-            }
-        }
-    }
     if (tid == 0) {
         p.grp_ent[G] = (int32_t)min(E, (int64_t)INT32_MAX);
         p.ctrl->n_groups = G;
@@ -464,8 +452,181 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
 #ifdef AJT_TIMING
     if (tid == 0) {
         for (int k = 0; k < 7; ++k) reinterpret_cast<uint64_t*>(p.ctrl->reserved)[k] = tick_[k];
+        reinterpret_cast<uint64_t*>(p.ctrl->reserved)[14] = tick_[7];
+        reinterpret_cast<uint64_t*>(p.ctrl->reserved)[15] = tick_[8];
         for (int k = 0; k < 6; ++k) reinterpret_cast<uint64_t*>(p.ctrl->reserved)[8 + k] = g_rt[k];
     }
+#endif
+}
+
+// ---- K1 for batches that fit in shared memory (n <= kGrpSmemN): the same steps written for a SMALL CODE FOOTPRINT.  A
+// merge call streams hundreds of MB through L2 between two launches of this kernel, so its instructions come from DRAM every
+// time, and a one-CTA kernel that runs each line once pays for every 128-byte line it touches: loops are not unrolled, and
+// the scans share one out-of-line routine working in place on shared arrays.
+
+// In-place exclusive scan of a[0..n) by the CTA (1024 threads); returns the total to every thread.
+__device__ __noinline__ uint32_t cta_scan_excl(uint32_t* a, int n, uint32_t* s_wt) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint32_t base = 0;
+#pragma unroll 1
+    for (int i0 = 0; i0 < n; i0 += 1024) {
+        const int i = i0 + tid;
+        const uint32_t v = i < n ? a[i] : 0u;
+        uint32_t inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) s_wt[warp] = inc;
+        __syncthreads();
+        const uint32_t wv = s_wt[lane];
+        uint32_t winc = wv;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += t;
+        }
+        const uint32_t pre = __shfl_sync(0xffffffffu, winc - wv, warp), tot = __shfl_sync(0xffffffffu, winc, 31);
+        if (i < n) a[i] = base + pre + inc - v;
+        base += tot;
+        __syncthreads();
+    }
+    return base;
+}
+
+__global__ void __launch_bounds__(1024) merge_group_small_kernel(const MergeParams p) {
+    extern __shared__ __align__(16) uint8_t g_dyn[];
+    __shared__ RadixScratch<32> sc;
+    __shared__ uint32_t s_wt[32];
+    __shared__ int s_min, s_max;
+    __shared__ uint32_t s_bad;
+#ifdef AJT_TIMING
+    uint64_t tick_[10] = {0};
+#endif
+    AJT_TICK(0);
+    const int tid = threadIdx.x, n = p.n;
+    const size_t nn = ((size_t)n + 32) & ~(size_t)31;   // 6 arrays of nn words
+    // arrays read BY TIMELINE INDEX through the sorted order are swizzled: timelines of one group are often a power of two
+    // apart (round-robin collection), which would put a warp's 32 gathers in one bank
+    auto swz = [](int i) { return i ^ ((i >> 5) & 31) ^ ((i >> 10) & 31); };
+    uint32_t* const sm32 = reinterpret_cast<uint32_t*>(g_dyn);
+    uint32_t* kb[2] = {sm32, sm32 + nn};
+    uint32_t* vb[2] = {sm32 + 2 * nn, sm32 + 3 * nn};
+    uint32_t* nsg = sm32 + 4 * nn;   // [i] hash windows of timeline i
+    uint32_t* tln = sm32 + 5 * nn;   // [i] its length; later [pos] windows by sorted position
+    if (tid < (int)(sizeof(AjtCtrl) / 4)) reinterpret_cast<uint32_t*>(p.ctrl)[tid] = 0;   // fresh control block
+    if (tid == 0) { s_min = INT32_MAX; s_max = INT32_MIN; s_bad = 0; }
+    __syncthreads();
+    // validate offsets; min / max traj id; hash windows per timeline
+    int lmin = INT32_MAX, lmax = INT32_MIN;
+    uint32_t bad = 0;
+#pragma unroll 2
+    for (int i = tid; i < n; i += 1024) {
+        const int64_t a = __ldg(p.offsets + i), b = __ldg(p.offsets + i + 1);
+        if (b < a || b - a > (int64_t)INT32_MAX) bad |= AJT_STATUS_BAD_OFFSETS;
+        else if (b == a) bad |= AJT_STATUS_ZERO_LEN;
+        const int t = __ldg(p.traj_ids + i);
+        lmin = min(lmin, t);
+        lmax = max(lmax, t);
+        kb[0][i] = (uint32_t)t;
+        vb[0][i] = (uint32_t)i;
+        nsg[swz(i)] = (uint32_t)(((b - 1 + p.mis) >> kHSegLog) - ((a + p.mis) >> kHSegLog) + 1);
+        tln[swz(i)] = (uint32_t)(b - a);
+        p.link_bad[i] = 0;
+    }
+    if (tid == 0 && (__ldg(p.offsets) != 0 || __ldg(p.offsets + n) != p.N)) bad |= AJT_STATUS_BAD_OFFSETS;
+    AJT_TICK(1);
+    lmin = __reduce_min_sync(0xffffffffu, lmin);
+    lmax = __reduce_max_sync(0xffffffffu, lmax);
+    bad = __reduce_or_sync(0xffffffffu, bad);
+    if ((tid & 31) == 0) {
+        if (bad) atomicOr(&s_bad, bad);
+        atomicMin(&s_min, lmin);
+        atomicMax(&s_max, lmax);
+    }
+    __syncthreads();
+    if (s_bad) {
+        if (tid == 0) atomicOr(&p.ctrl->status, s_bad);
+        return;
+    }
+    const uint32_t tmin = (uint32_t)s_min, range = (uint32_t)s_max - tmin;
+#pragma unroll 1
+    for (int i = tid; i < n; i += 1024) kb[0][i] -= tmin;
+    __syncthreads();
+    AJT_TICK(2);
+    int cur = 0;
+    {   // as few passes as the key range needs, digits of equal width (the ranking costs one ballot per digit bit)
+        const int bits = 32 - __clz(range), npass = (bits + 7) / 8, w = npass ? (bits + npass - 1) / npass : 0;
+#pragma unroll 1
+        for (int shift = 0; shift < bits; shift += w) {
+            radix_pass<32>(kb[cur], vb[cur], kb[cur ^ 1], vb[cur ^ 1], n, shift, sc, w);
+            cur ^= 1;
+        }
+    }
+    AJT_TICK(3);
+    uint32_t* key = kb[cur];          // [pos] sorted keys; later [g] first key slot of group g
+    const uint32_t* val = vb[cur];    // [pos] timeline index
+    uint32_t* gid = kb[cur ^ 1];      // [pos] group id
+    uint32_t* gsv = vb[cur ^ 1];      // [g]   first sorted position of group g
+    // group ids and group starts
+#pragma unroll 1
+    for (int pos = tid; pos < n; pos += 1024) gid[pos] = (pos == 0 || key[pos] != key[pos - 1]) ? 1u : 0u;
+    __syncthreads();
+    const int G = (int)cta_scan_excl(gid, n, s_wt);   // gid[pos] = heads before pos
+#pragma unroll 1
+    for (int pos = tid; pos < n; pos += 1024) {
+        const bool head = pos == 0 || key[pos] != key[pos - 1];
+        const uint32_t g = gid[pos] + (head ? 1u : 0u) - 1u;
+        gid[pos] = g;
+        if (head) { gsv[g] = (uint32_t)pos; p.grp_start[g] = pos; }
+    }
+    if (tid == 0) { gsv[G] = (uint32_t)n; p.grp_start[G] = n; }
+    __syncthreads();
+    AJT_TICK(4);
+    // key slots (i, a), a = 0..rank_i: a group of k timelines has k(k+1)/2 (at most n^2/2 < 2^25 here)
+    uint32_t* gent = key;
+#pragma unroll 1
+    for (int g = tid; g < G; g += 1024) {
+        const uint32_t k = gsv[g + 1] - gsv[g];
+        gent[g] = k * (k + 1) / 2;
+    }
+    __syncthreads();
+    const uint32_t E = cta_scan_excl(gent, G, s_wt);
+    AJT_TICK(5);
+    // lengths by sorted position; then the windows by sorted position (none for singleton groups) in the freed array
+#pragma unroll 1
+    for (int pos = tid; pos < n; pos += 1024) p.glen[pos] = (int32_t)tln[swz((int)val[pos])];
+    __syncthreads();
+    uint32_t* segs = tln;
+#pragma unroll 1
+    for (int pos = tid; pos < n; pos += 1024) {
+        const uint32_t g = gid[pos];
+        segs[pos] = gsv[g + 1] - gsv[g] < 2 ? 0u : nsg[swz((int)val[pos])];
+    }
+    __syncthreads();
+    // hash segments numbered in GROUP order, so that a timeline is hashed right after its in-group predecessor
+    const uint32_t nseg = cta_scan_excl(segs, n, s_wt);
+    AJT_TICK(6);
+#pragma unroll 1
+    for (int pos = tid; pos < n; pos += 1024) {
+        const uint32_t g = gid[pos], gs = gsv[g], r = (uint32_t)pos - gs;
+        p.tl_rec[pos] = make_int4((int)segs[pos], (int)gs, (int)r, (int)(gent[g] + r * (r + 1) / 2u));
+        p.perm[pos] = (int32_t)val[pos];
+        if (r == 0) p.grp_ent[g] = (int32_t)gent[g];
+    }
+    if (tid == 0) {
+        p.grp_ent[G] = (int32_t)E;
+        p.ctrl->n_groups = G;
+        p.ctrl->n_entries = (int32_t)E;
+        p.ctrl->n_hash_segs = (int32_t)nseg;
+        if ((int64_t)E > (int64_t)p.E_cap || (int64_t)nseg > (int64_t)p.nseg_cap)
+            atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_PROBE_CAPACITY);
+    }
+    AJT_TICK(7);
+#ifdef AJT_TIMING
+    if (tid == 0)
+        for (int k = 0; k < 8; ++k) reinterpret_cast<uint64_t*>(p.ctrl->reserved)[k] = tick_[k];
 #endif
 }
 
@@ -629,8 +790,9 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
     const uint32_t LW = c_w4.v[lane];
     auto seg_base = [&](int i) { return __ldg(reinterpret_cast<const int32_t*>(p.tl_rec) + 4 * i); };
     for (int sidx = wglobal; sidx < nseg; sidx += nwarps) {
-        const int i = warp_search_last_le(n, sidx, seg_base);
-        const int4 rec = __ldg(p.tl_rec + i);
+        const int pos = warp_search_last_le(n, sidx, seg_base);   // sorted position of the window's timeline
+        const int4 rec = __ldg(p.tl_rec + pos);
+        const int i = __ldg(p.perm + pos);
         const int64_t off = __ldg(p.offsets + i);
         const int Li = (int)(__ldg(p.offsets + i + 1) - off);
         const int32_t* tl = p.tokens + off;
@@ -639,10 +801,8 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
         int Lprev = 0;
         const int32_t* tprev = nullptr;
         if (rec.z > 0) {
-            const int jp = __ldg(p.perm + rec.y + rec.z - 1);
-            const int64_t op = __ldg(p.offsets + jp);
-            const int lp = (int)(__ldg(p.offsets + jp + 1) - op);
-            if (lp <= Li) { Lprev = lp; tprev = p.tokens + op; }
+            const int lp = __ldg(p.glen + pos - 1);
+            if (lp <= Li) { Lprev = lp; tprev = p.tokens + __ldg(p.offsets + __ldg(p.perm + pos - 1)); }
         }
         const int d = (int)((off + p.mis) & (kHSeg - 1));   // the timeline starts d slots into its first window
         const int j = sidx - rec.x;                          // window index inside the timeline
@@ -741,7 +901,7 @@ __device__ void select_body(const MergeParams& p, int mode, SelectSmem& sm) {
         const int32_t* gl = p.perm + gs;
         const int32_t* gln = p.glen + gs;
         if (k < 2) {
-            if (tid == 0) { p.absorbed[gl[0]] = 0; p.owner_tl[gl[0]] = gl[0]; }
+            if (tid == 0) { p.absorbed[gl[0]] = 0; p.owner_tl[gl[0]] = gl[0]; p.needv[gl[0]] = 0; p.tl_pos[gl[0]] = gs; }
             continue;
         }
         const int eb = p.grp_ent[g], c = p.grp_ent[g + 1] - eb;
@@ -750,7 +910,7 @@ __device__ void select_body(const MergeParams& p, int mode, SelectSmem& sm) {
         // (mode 1 finds seg_part and ent_hash already final)
         for (int r = warp; r < k; r += NT / 32) {
             const int i = gl[r];
-            const int sb = p.tl_rec[i].x;
+            const int sb = p.tl_rec[gs + r].x;
             const int64_t off = p.offsets[i];
             const int ns = mode == 0 ? (int)(((off + gln[r] - 1 + p.mis) >> kHSegLog) - ((off + p.mis) >> kHSegLog) + 1) : 0;
             if (cached && lane == 0) {
@@ -788,7 +948,7 @@ __device__ void select_body(const MergeParams& p, int mode, SelectSmem& sm) {
                     int64_t off;
                     int sb;
                     if (cached) { off = sm.t_off[r]; sb = sm.t_sb[r]; }
-                    else { const int i = gl[r]; off = p.offsets[i]; sb = p.tl_rec[i].x; }
+                    else { const int i = gl[r]; off = p.offsets[i]; sb = p.tl_rec[gs + r].x; }
                     const int64_t widx = ((off + Lp - 1 + p.mis) >> kHSegLog) - ((off + p.mis) >> kHSegLog);
                     h += p.seg_part[sb + widx];
                     if (weak) h &= 0xFull;
@@ -884,6 +1044,7 @@ __device__ void select_body(const MergeParams& p, int mode, SelectSmem& sm) {
             });
             p.absorbed[j] = best >= 0;
             p.owner_tl[j] = best >= 0 ? gl[best] : j;
+            p.tl_pos[j] = gs + b;
         }
         __syncthreads();
         if (p.owner_rule == AJT_OWNER_LONGEST) {
@@ -896,7 +1057,7 @@ __device__ void select_body(const MergeParams& p, int mode, SelectSmem& sm) {
                 const int32_t L = gln[b];
                 uint32_t dg = digest32(H, L);
                 if (dg == 0xFFFFFFFFu) dg = 0xFFFFFFFEu;
-                int best = p.tl_rec[p.owner_tl[j]].z;   // a surviving, (to be) verified extender: the fallback
+                int best = p.tl_pos[p.owner_tl[j]] - gs;   // a surviving, (to be) verified extender: the fallback
                 int32_t bestL = gln[best];
                 visit(dg, [&](uint32_t le) {
                     const int rb = rank_of_local(le);
@@ -925,7 +1086,7 @@ __device__ void select_body(const MergeParams& p, int mode, SelectSmem& sm) {
             const int j = gl[b];
             bool nv = p.absorbed[j] != 0;
             if (nv && cached) {
-                const int o = p.tl_rec[p.owner_tl[j]].z;
+                const int o = p.tl_pos[p.owner_tl[j]] - gs;
                 nv = false;
                 for (int r = b + 1; r <= o; ++r) nv |= sm.bad[r] != 0;
             }
@@ -1230,7 +1391,7 @@ __device__ void scatter_body(const MergeParams& p, int mode, MemberList* lists) 
             tb = p.tile_base[m];
             c.s = p.merged_origin[m];
             c.mo = p.merged_offsets[m];
-            const int4 rec = p.tl_rec[c.s];
+            const int4 rec = p.tl_rec[p.tl_pos[c.s]];
             c.gs = rec.y;
             c.rank_s = rec.z;
             c.so = p.offsets[c.s];
@@ -1332,12 +1493,13 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     p.merged_offsets = merged_offsets; p.merged_origin = merged_origin; p.merged_traj = merged_traj; p.owner = owner;
     p.counts = counts;
     p.ctrl = reinterpret_cast<AjtCtrl*>(b + ws.ctrl);
-    for (int k = 0; k < 5; ++k) p.gbuf[k] = reinterpret_cast<uint32_t*>(b + ws.gbuf[k]);
+    for (int k = 0; k < 6; ++k) p.gbuf[k] = reinterpret_cast<uint32_t*>(b + ws.gbuf[k]);
     p.perm = reinterpret_cast<int32_t*>(b + ws.perm);
     p.glen = reinterpret_cast<int32_t*>(b + ws.glen);
     p.grp_start = reinterpret_cast<int32_t*>(b + ws.grp_start);
     p.grp_ent = reinterpret_cast<int32_t*>(b + ws.grp_ent);
     p.tl_rec = reinterpret_cast<int4*>(b + ws.tl_rec);
+    p.tl_pos = reinterpret_cast<int32_t*>(b + ws.tl_pos);
     p.seg_part = reinterpret_cast<uint64_t*>(b + ws.seg_part);
     p.absorbed = b + ws.absorbed;
     p.link_bad = b + ws.link_bad;
@@ -1370,7 +1532,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     static int s_repair_grid[64] = {0};
     if (dev < 0 || dev >= 64) return AJT_ERR_UNSUPPORTED;
     if (s_repair_grid[dev] == 0) {
-        if (cudaFuncSetAttribute(merge_group_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * (kGrpSmemN + 4) * 4) !=
+        if (cudaFuncSetAttribute(merge_group_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 6 * ((kGrpSmemN + 32) & ~31) * 4) !=
             cudaSuccess)
             return AJT_ERR_CUDA;
         int per_sm = 0;
@@ -1378,7 +1540,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
             return AJT_ERR_CUDA;
         s_repair_grid[dev] = num_sms * (per_sm < 4 ? per_sm : 4);
     }
-    if (n <= kGrpSmemN) merge_group_kernel<true><<<1, 1024, 5 * (((size_t)n + 4) & ~(size_t)3) * 4, stream>>>(p);
+    if (n <= kGrpSmemN) merge_group_small_kernel<<<1, 1024, 6 * (((size_t)n + 32) & ~(size_t)31) * 4, stream>>>(p);
     else merge_group_kernel<false><<<1, 1024, 0, stream>>>(p);
     merge_hash_kernel<<<num_sms * 3, 256, 0, stream>>>(p);
     merge_select_kernel<<<num_sms * 4, kSelThreads, 0, stream>>>(p);
