@@ -40,6 +40,7 @@ def lib():
         _lib = C.CDLL(_SO)
         _lib.ajt_oracle_merge.restype = C.c_int
         _lib.ajt_oracle_loss.restype = C.c_int
+        _lib.ajt_oracle_loss_ex.restype = C.c_int
         _lib.ajt_oracle_round_bf16.restype = C.c_double
         _lib.ajt_oracle_round_bf16.argtypes = [C.c_double]
         _lib.ajt_oracle_num_threads.restype = C.c_int
@@ -121,11 +122,15 @@ class LossResult:
     Lt: np.ndarray               # float64 [R]
     dlogits: Optional[np.ndarray]  # float64 [R,V], before rounding
     stats: np.ndarray            # float64 [4]
+    k3: Optional[np.ndarray] = None    # float64 [R]  low-variance KL estimator per token (extended form)
+    ent: Optional[np.ndarray] = None   # float64 [R]  entropy of the row's softmax (extended form)
+    ext: Optional[np.ndarray] = None   # float64 [2]  {sum w_t k3_t, sum w_t H_t}
 
 
 def policy_loss(logits, targets, old_logp, adv, mask, seg_ids, S: int, eps_lo: float, eps_hi: float,
                 seg_denom=None, inv_num_segs: float = 0.0, grad_scale: float = 1.0,
-                row_ids=None, want_dlogits: bool = True, logits_is_bf16_bits: bool = False) -> LossResult:
+                row_ids=None, want_dlogits: bool = True, logits_is_bf16_bits: bool = False,
+                ref_logp=None, kl_coef: float = 0.0, extended: bool = False) -> LossResult:
     """fp64 loss oracle (DESIGN.md O-L).  `logits` is float32 [R,V], or uint16 [R,V] holding bf16 bit
     patterns when logits_is_bf16_bits.  Per-token vectors have length T (all tokens of the call);
     `row_ids` (int64 [R]) says which tokens the given logits rows are (None => R == T)."""
@@ -159,6 +164,21 @@ def policy_loss(logits, targets, old_logp, adv, mask, seg_ids, S: int, eps_lo: f
                                C.c_double(grad_scale), _p(loss), _p(logp), _p(w), _p(g), _p(Lt), _p(dl), _p(stats))
     if rc != 0:
         raise ValueError(f"ajt_oracle_loss: invalid input (rc={rc})")
+    if extended or ref_logp is not None:
+        # steps 8-9 (KL against a reference policy, entropy): a second call of the extended entry point
+        ref = _c(ref_logp, np.float32)
+        k3 = np.zeros(max(R, 1), np.float64)
+        ent = np.zeros(max(R, 1), np.float64)
+        ext = np.zeros(2, np.float64)
+        stats[:] = 0.0
+        rc = lib().ajt_oracle_loss_ex(_p(logits), C.c_int32(dt), C.c_int64(R), C.c_int32(V), C.c_int64(V), _p(row_ids),
+                                      _p(targets), _p(old_logp), _p(adv), _p(mask), _p(seg_ids), C.c_int64(T), C.c_int32(S),
+                                      C.c_double(eps_lo), C.c_double(eps_hi), _p(seg_denom), C.c_double(inv_num_segs),
+                                      C.c_double(grad_scale), _p(loss), _p(logp), _p(w), _p(g), _p(Lt), _p(dl), _p(stats),
+                                      _p(ref), C.c_double(kl_coef), _p(k3), _p(ent), _p(ext))
+        if rc != 0:
+            raise ValueError(f"ajt_oracle_loss_ex: invalid input (rc={rc})")
+        return LossResult(float(loss[0]), logp[:R], w[:R], g[:R], Lt[:R], dl, stats, k3[:R], ent[:R], ext)
     return LossResult(float(loss[0]), logp[:R], w[:R], g[:R], Lt[:R], dl, stats)
 
 

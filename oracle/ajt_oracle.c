@@ -188,12 +188,21 @@ static double load_logit(const void* logits, int dtype, int64_t idx) {
  * stats[4] += {sum m_t, #clipped high, #clipped low, sum w_t (-log r_t)} over the given rows.
  * Returns 0; -1 invalid argument; -3 target or segment id out of range on a masked-in row.
  */
-int ajt_oracle_loss(const void* logits, int32_t dtype, int64_t R, int32_t V, int64_t ld, const int64_t* row_ids,
-                    const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
-                    const int32_t* seg_ids, int64_t T, int32_t S,
-                    double eps_lo, double eps_hi, const float* seg_denom, double inv_num_segs, double grad_scale,
-                    double* loss_partial, double* logp, double* w, double* g, double* Lt, double* dlogits,
-                    double* stats) {
+/*
+ * Extended form (DESIGN.md "O-L" steps 8-9; the "other loss terms" of PAPER.md:136 that the protocol of PAPER.md:531 names:
+ * kl_loss_coef = 2e-3 with the `low_var_kl` estimator, and the policy entropy the paper monitors):
+ *   step 8  d_t = ref_logp_t - logp_t;  k3_t = min(exp(d_t) - d_t - 1, 10)   (the low-variance "k3" estimator of
+ *           KL(pi || pi_ref), clamped at 10; reading L-16);  loss += kl_coef sum_t w_t k3_t;
+ *           g_t += grad_scale w_t kl_coef (1 - exp(d_t)) [k3_t < 10]
+ *   step 9  H_t = lse_t - sum_v p_tv z_tv  (entropy of the row's softmax; reported, no gradient)
+ * ref_logp NULL or kl_coef 0 switches step 8 off.  k3[R], ent[R] optional; ext[2] += {sum w_t k3_t, sum w_t H_t}.
+ */
+static int loss_impl(const void* logits, int32_t dtype, int64_t R, int32_t V, int64_t ld, const int64_t* row_ids,
+                     const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
+                     const int32_t* seg_ids, int64_t T, int32_t S,
+                     double eps_lo, double eps_hi, const float* seg_denom, double inv_num_segs, double grad_scale,
+                     double* loss_partial, double* logp, double* w, double* g, double* Lt, double* dlogits,
+                     double* stats, const float* ref_logp, double kl_coef, double* k3, double* ent, double* ext) {
     if (R < 0 || T < 0 || V <= 0 || S <= 0 || ld < V || eps_lo < 0 || eps_hi < 0) return -1;
     if (dtype != 0 && dtype != 1) return -1;
 
@@ -213,7 +222,7 @@ int ajt_oracle_loss(const void* logits, int32_t dtype, int64_t R, int32_t V, int
 
     /* Per-row terms are stored and summed afterwards in row order, so the scalar does not depend on the
      * number of threads (step 5 is a plain sum over t). */
-    double* term = (double*)calloc((size_t)(R > 0 ? R : 1) * 5, sizeof(double)); /* {w L, m, clip_hi, clip_lo, w(-log r)} */
+    double* term = (double*)calloc((size_t)(R > 0 ? R : 1) * 7, sizeof(double)); /* {w L, m, clip_hi, clip_lo, w(-log r), w k3, w H} */
 #pragma omp parallel for schedule(static) reduction(min : err)
     for (int64_t r = 0; r < R; ++r) {
         int64_t t = row_ids ? row_ids[r] : r;
@@ -222,6 +231,8 @@ int ajt_oracle_loss(const void* logits, int32_t dtype, int64_t R, int32_t V, int
         if (w) w[r] = 0.0;
         if (g) g[r] = 0.0;
         if (Lt) Lt[r] = 0.0;
+        if (k3) k3[r] = 0.0;
+        if (ent) ent[r] = 0.0;
         if (drow) for (int32_t v = 0; v < V; ++v) drow[v] = 0.0;
         if (t < 0 || t >= T) { err = -1; continue; }
         if (!mask[t]) continue; /* m_t = 0: contributes nothing, dlogits row is zero (L-14) */
@@ -260,9 +271,30 @@ int ajt_oracle_loss(const void* logits, int32_t dtype, int64_t R, int32_t V, int
         int clip_lo = (A < 0.0 && ratio < 1.0 - eps_lo);
         double gt = (clip_hi || clip_lo) ? 0.0 : grad_scale * wt * (-A * ratio);
 
-        term[5 * r + 0] = wt * L; /* step 5 */
-        term[5 * r + 1] = 1.0; term[5 * r + 2] = clip_hi; term[5 * r + 3] = clip_lo;
-        term[5 * r + 4] = wt * (-(lp - (double)old_logp[t]));
+        /* Step 8: low-variance KL estimator against the reference policy's log-prob of the same token. */
+        double k3t = 0.0;
+        if (ref_logp && kl_coef != 0.0) {
+            double d = (double)ref_logp[t] - lp;
+            k3t = exp(d) - d - 1.0;
+            if (k3t < 10.0) gt += grad_scale * wt * kl_coef * (1.0 - exp(d));
+            else k3t = 10.0;
+        }
+
+        /* Step 9: entropy of the row, H = lse - sum_v p_v z_v. */
+        double pz = 0.0;
+        for (int32_t v = 0; v < V; ++v) {
+            double z = load_logit(logits, dtype, base + v);
+            pz += exp(z - lse) * z;
+        }
+        double H = lse - pz;
+        term[7 * r + 5] = wt * k3t;
+        term[7 * r + 6] = wt * H;
+        if (k3) k3[r] = k3t;
+        if (ent) ent[r] = H;
+
+        term[7 * r + 0] = wt * L; /* step 5 */
+        term[7 * r + 1] = 1.0; term[7 * r + 2] = clip_hi; term[7 * r + 3] = clip_lo;
+        term[7 * r + 4] = wt * (-(lp - (double)old_logp[t]));
         if (logp) logp[r] = lp;
         if (w) w[r] = wt;
         if (g) g[r] = gt;
@@ -274,16 +306,38 @@ int ajt_oracle_loss(const void* logits, int32_t dtype, int64_t R, int32_t V, int
             }
         }
     }
-    double total = 0.0, st0 = 0, st1 = 0, st2 = 0, st3 = 0;
+    double total = 0.0, st0 = 0, st1 = 0, st2 = 0, st3 = 0, kl = 0, en = 0;
     for (int64_t r = 0; r < R; ++r) {
-        total += term[5 * r + 0];
-        st0 += term[5 * r + 1]; st1 += term[5 * r + 2]; st2 += term[5 * r + 3]; st3 += term[5 * r + 4];
+        total += term[7 * r + 0];
+        st0 += term[7 * r + 1]; st1 += term[7 * r + 2]; st2 += term[7 * r + 3]; st3 += term[7 * r + 4];
+        kl += term[7 * r + 5]; en += term[7 * r + 6];
     }
-    *loss_partial = total;
+    *loss_partial = total + kl_coef * kl;   /* step 5 (+ step 8) */
     if (stats) { stats[0] += st0; stats[1] += st1; stats[2] += st2; stats[3] += st3; }
+    if (ext) { ext[0] += kl; ext[1] += en; }
     free(term);
     free(Ns);
     return err;
+}
+
+int ajt_oracle_loss(const void* logits, int32_t dtype, int64_t R, int32_t V, int64_t ld, const int64_t* row_ids,
+                    const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
+                    const int32_t* seg_ids, int64_t T, int32_t S,
+                    double eps_lo, double eps_hi, const float* seg_denom, double inv_num_segs, double grad_scale,
+                    double* loss_partial, double* logp, double* w, double* g, double* Lt, double* dlogits,
+                    double* stats) {
+    return loss_impl(logits, dtype, R, V, ld, row_ids, targets, old_logp, adv, mask, seg_ids, T, S, eps_lo, eps_hi, seg_denom,
+                     inv_num_segs, grad_scale, loss_partial, logp, w, g, Lt, dlogits, stats, NULL, 0.0, NULL, NULL, NULL);
+}
+
+int ajt_oracle_loss_ex(const void* logits, int32_t dtype, int64_t R, int32_t V, int64_t ld, const int64_t* row_ids,
+                       const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
+                       const int32_t* seg_ids, int64_t T, int32_t S,
+                       double eps_lo, double eps_hi, const float* seg_denom, double inv_num_segs, double grad_scale,
+                       double* loss_partial, double* logp, double* w, double* g, double* Lt, double* dlogits,
+                       double* stats, const float* ref_logp, double kl_coef, double* k3, double* ent, double* ext) {
+    return loss_impl(logits, dtype, R, V, ld, row_ids, targets, old_logp, adv, mask, seg_ids, T, S, eps_lo, eps_hi, seg_denom,
+                     inv_num_segs, grad_scale, loss_partial, logp, w, g, Lt, dlogits, stats, ref_logp, kl_coef, k3, ent, ext);
 }
 
 /* Round an fp64 value to bf16 (round-to-nearest-even), returned as fp64 (reading L-10:
