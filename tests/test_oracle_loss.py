@@ -288,3 +288,100 @@ def test_loss_merged_equals_unmerged(rule):
     gm = np.zeros_like(lm.dlogits)
     np.add.at(gm, rows, lu.dlogits)
     np.testing.assert_allclose(gm, lm.dlogits, rtol=1e-9, atol=1e-15)
+
+
+# ------------------------------------------------------------------ P-L6..P-L8: steps 8-9 (KL vs reference policy, entropy)
+
+
+def test_k3_closed_forms():
+    """Step 8 (PAPER.md:531 `low_var_kl`, reading L-16): k3(d) = exp(d) - d - 1 with d = ref_logp - logp, clamped at 10."""
+    V, T = 7, 5
+    z = np.zeros((T, V), np.float32)                    # uniform rows: logp = -log V exactly representable enough
+    y = np.arange(T, dtype=np.int32) % V
+    lp = -np.log(V)
+    ds = np.array([0.0, np.log(2.0), -1.0, 1e-3, 3.0])   # k3: 0, 1 - log 2, e^-1, ~d^2/2, clamped (e^3 - 4 = 16.09 > 10)
+    ref = (lp + ds).astype(np.float32)
+    old = np.full(T, lp, np.float32)
+    r = oracle.policy_loss(z, y, old, np.zeros(T, np.float32), np.ones(T, np.uint8), np.zeros(T, np.int32), 1, 0.2, 0.2,
+                           ref_logp=ref, kl_coef=1.0)
+    d = ref.astype(np.float64) - r.logp
+    np.testing.assert_allclose(r.k3[0], 0.0, atol=1e-7)
+    np.testing.assert_allclose(r.k3[1], 1.0 - np.log(2.0), atol=1e-6)
+    np.testing.assert_allclose(r.k3[2], np.exp(-1.0), atol=1e-6)
+    np.testing.assert_allclose(r.k3[3], d[3] ** 2 / 2, rtol=1e-3)
+    assert r.k3[4] == 10.0
+    assert np.all(r.k3 >= 0)
+    # A = 0: the loss is the KL term alone, = kl_coef * mean over the segment's tokens
+    np.testing.assert_allclose(r.loss, r.k3.mean(), rtol=1e-12)
+    np.testing.assert_allclose(r.ext[0], r.k3.mean(), rtol=1e-12)
+    # the clamped token has no KL gradient (A = 0 kills the policy-gradient part): its dlogits row is zero
+    assert np.all(r.dlogits[4] == 0.0) and np.any(r.dlogits[1] != 0.0)
+
+
+def test_k3_is_unbiased_for_kl():
+    """E_{y~pi} k3(y) = KL(pi || pi_ref) exactly (sum_y pi_y [pi_ref_y/pi_y - log(pi_ref_y/pi_y) - 1] = KL): enumerate y."""
+    from scipy.special import rel_entr
+    rng = np.random.default_rng(21)
+    V = 9
+    z = rng.standard_normal(V).astype(np.float32)
+    zr = (z + 0.3 * rng.standard_normal(V)).astype(np.float32)
+    pi = torch.softmax(torch.tensor(z, dtype=torch.float64), -1).numpy()
+    pr = torch.softmax(torch.tensor(zr, dtype=torch.float64), -1).numpy()
+    logits = np.tile(z, (V, 1))                          # one row per possible target
+    y = np.arange(V, dtype=np.int32)
+    ref = np.log(pr).astype(np.float32)
+    r = oracle.policy_loss(logits, y, np.log(pi).astype(np.float32), np.zeros(V, np.float32), np.ones(V, np.uint8),
+                           np.zeros(V, np.int32), 1, 0.2, 0.2, ref_logp=ref, kl_coef=1.0)
+    kl = rel_entr(pi, pr).sum()
+    np.testing.assert_allclose((pi * r.k3).sum(), kl, rtol=2e-6)   # ref_logp is stored in fp32
+
+
+def test_entropy_matches_library():
+    """Step 9: H = lse - sum_v p_v z_v = -sum_v p_v log p_v (torch.distributions / scipy), uniform row -> log V."""
+    from scipy.stats import entropy as sp_entropy
+    rng = np.random.default_rng(22)
+    T, V = 6, 33
+    z = (rng.standard_normal((T, V)) * 3).astype(np.float32)
+    z[0] = 1.25
+    y = rng.integers(0, V, T).astype(np.int32)
+    r = oracle.policy_loss(z, y, np.full(T, -3.0, np.float32), np.ones(T, np.float32), np.ones(T, np.uint8),
+                           np.zeros(T, np.int32), 1, 0.2, 0.2, extended=True)
+    H = torch.distributions.Categorical(logits=torch.tensor(z, dtype=torch.float64)).entropy().numpy()
+    np.testing.assert_allclose(r.ent, H, rtol=1e-12, atol=1e-12)
+    p = torch.softmax(torch.tensor(z, dtype=torch.float64), -1).numpy()
+    np.testing.assert_allclose(r.ent, [sp_entropy(row) for row in p], rtol=1e-10)
+    np.testing.assert_allclose(r.ent[0], np.log(V), rtol=1e-12)
+    np.testing.assert_allclose(r.ext[1], H.mean(), rtol=1e-12)
+    # steps 1-7 are untouched by the extended entry point when kl_coef = 0
+    r0 = oracle.policy_loss(z, y, np.full(T, -3.0, np.float32), np.ones(T, np.float32), np.ones(T, np.uint8),
+                            np.zeros(T, np.int32), 1, 0.2, 0.2)
+    assert r.loss == r0.loss and np.array_equal(r.dlogits, r0.dlogits)
+
+
+@pytest.mark.parametrize("T,V,S", [(9, 14, 3), (20, 40, 4)])
+def test_extended_against_torch_autograd(T, V, S):
+    """Whole extended definition (steps 1-8) vs an independently written torch fp64 graph."""
+    rng = np.random.default_rng(23 + T)
+    z, y, old, adv, mask, seg = rand_case(rng, T, V, S)
+    ref = (old + rng.standard_normal(T) * 0.3).astype(np.float32)
+    kl_coef, eps_lo, eps_hi = 0.37, 0.2, 0.28
+    zt = torch.tensor(z, dtype=torch.float64, requires_grad=True)
+    lp = torch.log_softmax(zt, -1).gather(1, torch.tensor(y, dtype=torch.int64)[:, None])[:, 0]
+    ratio = torch.exp(lp - torch.tensor(old, dtype=torch.float64))
+    A = torch.tensor(adv, dtype=torch.float64)
+    pg = -torch.minimum(ratio * A, torch.clamp(ratio, 1 - eps_lo, 1 + eps_hi) * A)
+    d = torch.tensor(ref, dtype=torch.float64) - lp
+    k3 = torch.clamp(torch.exp(d) - d - 1, max=10.0)
+    m = torch.tensor(mask, dtype=torch.float64)
+    total = torch.zeros((), dtype=torch.float64)
+    live = 0
+    for s_ in range(S):
+        sel = torch.tensor(seg == s_, dtype=torch.float64) * m
+        if sel.sum() > 0:
+            total = total + ((pg + kl_coef * k3) * sel).sum() / sel.sum()
+            live += 1
+    total = total / max(live, 1)
+    total.backward()
+    r = oracle.policy_loss(z, y, old, adv, mask, seg, S, eps_lo, eps_hi, ref_logp=ref, kl_coef=kl_coef)
+    np.testing.assert_allclose(r.loss, float(total), rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(r.dlogits, zt.grad.numpy(), rtol=1e-9, atol=1e-14)
