@@ -172,6 +172,28 @@ int ajt_policy_loss_fwd_bwd(
     float* stats_out,           /* DEVICE [4] or NULL: {n_masked, n_clipped_hi, n_clipped_lo, sum_t w_t (-log r_t)} */
     void* workspace, size_t workspace_bytes, ajt_stream_t stream);
 
+/* Extended form: the same call with the protocol's "other loss terms" fused into the same single
+ * read of each row (DESIGN.md "O-L" steps 8-9, readings L-16, L-17):
+ *   step 8  KL penalty against a reference policy with the low-variance estimator the protocol names
+ *           (`kl_loss_coef = 2e-3`, `low_var_kl`):
+ *             d_t = ref_logp_t - logp_t;   k3_t = min(exp(d_t) - d_t - 1, 10)
+ *             loss = sum_t w_t (L_t + kl_coef k3_t);   g_t += grad_scale w_t kl_coef (1 - exp(d_t)) [k3_t < 10]
+ *           switched off by ref_logp = NULL or kl_coef = 0 (then k3_t = 0).
+ *   step 9  entropy of each unmasked row's softmax (the policy entropy the paper monitors),
+ *             H_t = lse_t - sum_v p_tv z_tv,   reported only (no gradient).
+ * Extra arguments: ref_logp DEVICE [T] or NULL; kl_coef >= 0; k3_out, ent_out DEVICE [T] or NULL (k3_t, H_t where
+ * mask_t = 1, 0 elsewhere); ext_out DEVICE [2], required: {sum_t w_t k3_t, sum_t w_t H_t} of this call.
+ * Everything else (arguments, workspace, layouts, error behaviour, paths) is as for ajt_policy_loss_fwd_bwd; with
+ * ref_logp = NULL the loss, dlogits, logp_out and stats_out are bit-identical to that call's. */
+int ajt_policy_loss_fwd_bwd_ext(
+    const void* logits, const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
+    const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T, int32_t V, int32_t S, int64_t ld_logits,
+    int32_t logits_dtype, const float* seg_denom, float inv_num_segs, float grad_scale,
+    const float* ref_logp, float kl_coef,
+    void* dlogits, float* loss_out, float* logp_out, float* stats_out,
+    float* k3_out, float* ent_out, float* ext_out,
+    void* workspace, size_t workspace_bytes, ajt_stream_t stream);
+
 /* Batch-wide per-trajectory normalisers for callers that stream the batch through several loss calls
  * (micro-batches, 64k-row chunks, or rows of one trajectory spread over several GPUs; reading L-4;
  * "masked per-trajectory mean", BASELINE.json north_star):

@@ -29,6 +29,7 @@ from .binding import (  # noqa: F401
     merge_timelines_host,
     merge_workspace_bytes,
     policy_loss_fwd_bwd,
+    policy_loss_fwd_bwd_ext,
     policy_loss_fwd_bwd_host,
     segment_counts,
     strerror,

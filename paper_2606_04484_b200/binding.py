@@ -25,7 +25,7 @@ _EXPORTS = [
     "ajt_version", "ajt_strerror", "ajt_last_status",
     "ajt_merge_workspace_bytes", "ajt_merge_timelines", "ajt_merge_host_arena_bytes", "ajt_merge_timelines_host",
     "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
-    "ajt_segment_counts",
+    "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext",
 ]
 
 _lib = None
@@ -65,7 +65,7 @@ def lib():
         L.ajt_loss_host_arena_bytes.restype = C.c_size_t
         L.ajt_loss_host_arena_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32]
         for f in ("ajt_merge_timelines", "ajt_merge_timelines_host", "ajt_policy_loss_fwd_bwd",
-                  "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts"):
+                  "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -239,6 +239,9 @@ class LossOutput:
     logp: Optional[torch.Tensor]     # f32 [T]
     stats: Optional[torch.Tensor]    # f32 [4]
     workspace: torch.Tensor
+    k3: Optional[torch.Tensor] = None    # f32 [T]  extended form: low-variance KL estimator per token
+    ent: Optional[torch.Tensor] = None   # f32 [T]  extended form: entropy of each unmasked row
+    ext: Optional[torch.Tensor] = None   # f32 [2]  extended form: {sum w_t k3_t, sum w_t H_t}
 
 
 def policy_loss_fwd_bwd(logits: torch.Tensor, targets: torch.Tensor, old_logp: torch.Tensor, adv: torch.Tensor,
@@ -282,6 +285,56 @@ def policy_loss_fwd_bwd(logits: torch.Tensor, targets: torch.Tensor, old_logp: t
         _dp(out.stats), _dp(out.workspace), C.c_size_t(out.workspace.numel()), _stream(stream))
     if rc != 0:
         raise AjtError(rc, "ajt_policy_loss_fwd_bwd")
+    return out
+
+
+def policy_loss_fwd_bwd_ext(logits: torch.Tensor, targets: torch.Tensor, old_logp: torch.Tensor, adv: torch.Tensor,
+                            mask: torch.Tensor, seg_ids: torch.Tensor, S: int, eps_lo: float, eps_hi: float,
+                            ref_logp: Optional[torch.Tensor] = None, kl_coef: float = 0.0,
+                            seg_denom: Optional[torch.Tensor] = None, inv_num_segs: float = 0.0, grad_scale: float = 1.0,
+                            V: Optional[int] = None, dlogits: Optional[torch.Tensor] = None, want_logp: bool = False,
+                            want_stats: bool = False, want_rows: bool = True, out: Optional[LossOutput] = None,
+                            stream=None) -> LossOutput:
+    """ajt_policy_loss_fwd_bwd_ext (include/ajt.h): the loss call plus the KL term against `ref_logp` (low_var_kl) and
+    the per-row entropy, from the same single read of each row."""
+    _require_cuda()
+    if logits.dim() != 2 or not logits.is_cuda or logits.stride(1) != 1:
+        raise TypeError("logits: expected a 2-D CUDA tensor with unit column stride")
+    if logits.dtype == torch.bfloat16:
+        dt = DT_BF16
+    elif logits.dtype == torch.float32:
+        dt = DT_F32
+    else:
+        raise TypeError("logits: bf16 or f32 only")
+    T, ld = int(logits.shape[0]), int(logits.stride(0)) if logits.shape[0] > 1 else int(logits.shape[1])
+    V = int(logits.shape[1]) if V is None else int(V)
+    _check_dev(targets, torch.int32, "targets")
+    _check_dev(old_logp, torch.float32, "old_logp")
+    _check_dev(adv, torch.float32, "adv")
+    _check_dev(mask, torch.uint8, "mask")
+    _check_dev(seg_ids, torch.int32, "seg_ids")
+    _check_dev(seg_denom, torch.float32, "seg_denom")
+    _check_dev(ref_logp, torch.float32, "ref_logp")
+    dev = logits.device
+    if out is None:
+        if dlogits is None:
+            dlogits = torch.empty((T, ld), dtype=torch.bfloat16, device=dev)
+        f32 = lambda n: torch.empty(n, dtype=torch.float32, device=dev)
+        out = LossOutput(dlogits, f32(1), f32(max(T, 1)) if want_logp else None, f32(4) if want_stats else None,
+                         torch.empty(loss_workspace_bytes(T, V, S), dtype=torch.uint8, device=dev),
+                         f32(max(T, 1)) if want_rows else None, f32(max(T, 1)) if want_rows else None, f32(2))
+    if out.dlogits.dtype != torch.bfloat16 or not out.dlogits.is_cuda:
+        raise TypeError("dlogits: expected a CUDA bf16 tensor")
+    if out.ext is None:
+        raise TypeError("out.ext: the extended call needs a [2] f32 CUDA tensor")
+    rc = lib().ajt_policy_loss_fwd_bwd_ext(
+        _dp(logits), _dp(targets), _dp(old_logp), _dp(adv), _dp(mask), _dp(seg_ids),
+        C.c_float(eps_lo), C.c_float(eps_hi), C.c_int64(T), C.c_int32(V), C.c_int32(S), C.c_int64(ld), C.c_int32(dt),
+        _dp(seg_denom), C.c_float(inv_num_segs), C.c_float(grad_scale), _dp(ref_logp), C.c_float(kl_coef),
+        _dp(out.dlogits), _dp(out.loss), _dp(out.logp), _dp(out.stats), _dp(out.k3), _dp(out.ent), _dp(out.ext),
+        _dp(out.workspace), C.c_size_t(out.workspace.numel()), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_policy_loss_fwd_bwd_ext")
     return out
 
 

@@ -121,6 +121,11 @@ __device__ __forceinline__ void st_async_b64(uint32_t cluster_addr, uint64_t v, 
                  "r"(cluster_bar)
                  : "memory");
 }
+__device__ __forceinline__ void st_async_b32(uint32_t cluster_addr, uint32_t v, uint32_t cluster_bar) {
+    asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(cluster_addr), "r"(v),
+                 "r"(cluster_bar)
+                 : "memory");
+}
 
 // ---- misc -----------------------------------------------------------------------------------------
 __device__ __forceinline__ uint4 lds128(const void* p) {

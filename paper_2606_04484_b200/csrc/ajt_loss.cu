@@ -39,12 +39,13 @@ struct __align__(16) RowScal {                   // written by the producer, rea
     int32_t y;
     int32_t ybad;
     float old, A, w, zy;
+    float ref, pad0, pad1, pad2;                 // extended form only: reference-policy log-prob of the target
 };
-static_assert(sizeof(RowScal) == 32, "RowScal is two 16-byte vectors");
+static_assert(sizeof(RowScal) == 48, "RowScal is three 16-byte vectors");
 
 constexpr size_t kRowsSmemBytes = (size_t)kSlots * kChunkBytes + kChunkBytes /* zero buffer */ +
                                   (2 * kSlots + 2) * sizeof(uint64_t) + 2 * kConsWarps * kMaxCluster * sizeof(float2) +
-                                  kScalRing * sizeof(RowScal);
+                                  kScalRing * sizeof(RowScal) + 2 * kConsWarps * kMaxCluster * sizeof(float);
 
 struct LossParams {
     const void* logits;
@@ -64,20 +65,29 @@ struct LossParams {
     float* loss_out;
     float* logp_out;
     float* stats_out;
+    const float* ref_logp;  // extended form (steps 8-9): reference-policy log-probs [T] or NULL
+    float kl_coef;
+    float* ext_out;         // [2] {sum w_t k3_t, sum w_t H_t} or NULL
+    float* k3_out;          // [T] or NULL
+    float* ent_out;         // [T] or NULL
+    int32_t ext;            // 1: extended kernels (KL term and / or entropy requested)
     // workspace
     AjtCtrl* ctrl;
     uint64_t* tile_state;  // [ntiles] prep scan: bit 63 valid, bits 32..62 active rows of the tile, bits 0..31 masked rows
     int32_t* seg_cnt;      // [S]
     int4* rec_i;           // [T] compact records of the rows with mask = 1, ascending: {row, target, segment, 0}
     float2* rec_f;         // [T]   "  : {old_logp, adv}
+    float* rec_r;          // [T]   "  : ref_logp (extended form)
     int32_t* list_zero;    // [T] rows with mask = 0, ascending
     double* row_val;       // [T] w_t L_t by compact index
     double* row_kl;        // [T] w_t (-log r_t) by compact index
     uint8_t* row_clip;     // [T] bit0 clipped high, bit1 clipped low
+    double* row_k3;        // [T] w_t k3_t by compact index (extended form)
+    double* row_ent;       // [T] w_t H_t   "
 };
 
 struct LossWs {
-    size_t ctrl, tile_state, seg_cnt, zero_bytes, rec_i, rec_f, list_zero, row_val, row_kl, row_clip, total;
+    size_t ctrl, tile_state, seg_cnt, zero_bytes, rec_i, rec_f, rec_r, list_zero, row_val, row_kl, row_clip, row_k3, row_ent, total;
 };
 constexpr int kPrepTile = 1024;
 
@@ -92,10 +102,13 @@ __host__ LossWs loss_ws_layout(int64_t T, int32_t S) {
     w.zero_bytes = o;  // [ctrl, tile_state, seg_cnt] are cleared by one memset per call
     w.rec_i = o; o += align256((size_t)T * 16);
     w.rec_f = o; o += align256((size_t)T * 8);
+    w.rec_r = o; o += align256((size_t)T * 4);
     w.list_zero = o; o += align256((size_t)T * 4);
     w.row_val = o; o += align256((size_t)T * 8);
     w.row_kl = o; o += align256((size_t)T * 8);
     w.row_clip = o; o += align256((size_t)T);
+    w.row_k3 = o; o += align256((size_t)T * 8);
+    w.row_ent = o; o += align256((size_t)T * 8);
     w.total = o;
     return w;
 }
@@ -170,6 +183,7 @@ __global__ void __launch_bounds__(1024) loss_prep_kernel(const LossParams p, int
             const int idx = base_a + pa + __popc(ba & lt);
             p.rec_i[idx] = make_int4((int)t, p.targets[t], sg, 0);
             p.rec_f[idx] = make_float2(p.old_logp[t], p.adv[t]);
+            if (p.ref_logp) p.rec_r[idx] = p.ref_logp[t];
         } else if (in) {
             p.list_zero[base_z + pz + __popc(bz & lt)] = (int32_t)t;
         }
@@ -209,17 +223,22 @@ struct TokScalars {
     float g;       // d(w L)/d logp * grad_scale
     float logp;
     float lse;
+    float logS;    // log sum_v exp(z_v - M)
+    float k3;      // step 8 (extended form)
     double wl;     // w * L
     double wkl;    // w * (-(logp - old))
+    double wk3;    // w * k3 (extended form)
     int clip;      // bit0 high, bit1 low
 };
 
 // M = max_v z, S = sum_v exp(z_v - M) (so 1 <= S <= V), zy = z[y].  DESIGN.md O-L steps 1-6.
 __device__ __forceinline__ TokScalars token_scalars(float M, float S, float zy, float old, float A, float w,
-                                                    float eps_lo, float eps_hi, float grad_scale) {
+                                                    float eps_lo, float eps_hi, float grad_scale, bool use_kl = false,
+                                                    float ref = 0.f, float kl_coef = 0.f) {
     TokScalars o;
     const float logS = logf(S);
     o.lse = M + logS;
+    o.logS = logS;
     // (zy - M) is exact for bf16 inputs; subtracting the O(1) terms first keeps the log-ratio's error ~2e-7
     const float zm = zy - M;
     o.logp = zm - logS;
@@ -233,6 +252,18 @@ __device__ __forceinline__ TokScalars token_scalars(float M, float S, float zy, 
     o.wl = (double)w * (double)L;
     o.wkl = (double)w * (-(double)d);
     o.clip = (hi ? 1 : 0) | (lo ? 2 : 0);
+    o.wk3 = 0.0;
+    o.k3 = 0.f;
+    if (use_kl) {
+        // step 8: k3 = exp(d) - d - 1, d = ref_logp - logp, clamped at 10 (low_var_kl; reading L-16)
+        const float dk = (ref - zm) + logS;
+        const float em1 = expm1f(dk);
+        float k3 = em1 - dk;
+        if (k3 < 10.f) o.g += grad_scale * w * kl_coef * (-em1);
+        else k3 = 10.f;
+        o.k3 = k3;
+        o.wk3 = (double)w * (double)k3;
+    }
     return o;
 }
 
@@ -252,7 +283,24 @@ __device__ __forceinline__ float exp_diff(float m, float M) {  // exp(m - M), 0 
     return m == -INFINITY ? 0.f : ex2((m - M) * kLog2e);
 }
 
-template <int NCH, int CSIZE>
+// t = z - m (clamped so that a -inf logit or a padded lane gives 0 * finite), e = exp(t): s += e, u += e t.
+__device__ __forceinline__ void acc_exp(float x, float ms, float& s, float& u, bool ext) {
+    const float t = x - ms;
+    const float e = ex2(t * kLog2e);
+    s += e;
+    if (ext) u = fmaf(e, fmaxf(t, -1e30f), u);
+}
+// re-base a partial (m, s, u = sum e^{z-m} (z-m)) onto the maximum M: returns the factor, updates s and u
+__device__ __forceinline__ void rebase(float m, float M, float& s, float& u) {
+    const float f = exp_diff(m, M);
+    const float dm = m == -INFINITY ? 0.f : m - M;
+    u = f * fmaf(dm, s, u);
+    s = f * s;
+}
+
+// EXT: the extended form (steps 8-9): reference-policy log-prob per row, and u = sum_v e^{z-M} (z-M) beside the sum-exp so
+// that the row entropy H = log S - u / S comes out of the same single read.
+template <int NCH, int CSIZE, bool EXT>
 __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams p) {
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t* ring = smem;
@@ -262,6 +310,7 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
     uint64_t* pbar = empty + kSlots;
     float2* part = reinterpret_cast<float2*>(pbar + 2);  // [2][kConsWarps * kMaxCluster]
     RowScal* scal = reinterpret_cast<RowScal*>(part + 2 * kConsWarps * kMaxCluster);
+    float* partu = reinterpret_cast<float*>(scal + kScalRing);  // [2][kConsWarps * kMaxCluster], extended form
     constexpr int kParts = kConsWarps * CSIZE;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -314,12 +363,13 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
             // flight, stage C holds row k complete.  Published through shared memory before the row's first
             // full-barrier arrive (release) and read by the consumers after their wait (acquire).
             const float inv_S = p.ctrl->inv_num_segs;
-            struct Stage { int4 ri; float2 rf; float zy, den; };
+            struct Stage { int4 ri; float2 rf; float zy, den, ref; };
             auto load_rec = [&](int k, Stage& st) {
                 if (k < nrows) {
                     const int64_t idx = cid + (int64_t)k * NC;
                     st.ri = p.rec_i[idx];
                     st.rf = p.rec_f[idx];
+                    if (EXT) st.ref = p.ref_logp ? p.rec_r[idx] : 0.f;
                 }
             };
             auto load_dep = [&](int k, Stage& st) {
@@ -348,6 +398,8 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
                     rs.A = C.rf.y;
                     rs.w = (C.den > 0.f && !ybad) ? inv_S / C.den : 0.f;
                     rs.zy = C.zy;
+                    rs.ref = C.ref;
+                    rs.pad0 = rs.pad1 = rs.pad2 = 0.f;
                     scal[k & (kScalRing - 1)] = rs;
                 }
                 const int64_t row = C.ri.x;
@@ -379,7 +431,7 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
             int64_t row = 0;
             int y = 0;
             bool ybad = false;
-            float old = 0.f, A = 0.f, w = 0.f, zy = 0.f;
+            float old = 0.f, A = 0.f, w = 0.f, zy = 0.f, ref = 0.f;
 #pragma unroll
             for (int ch = 0; ch < NCH; ++ch) {
                 r[ch] = make_uint4(kNegInf2, kNegInf2, kNegInf2, kNegInf2);
@@ -394,6 +446,7 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
                         A = __uint_as_float(s1.y);
                         w = __uint_as_float(s1.z);
                         zy = __uint_as_float(s1.w);
+                        if (EXT) ref = scal[k & (kScalRing - 1)].ref;
                     }
                     if (ch * kChunkElems + tid * 8 < sl_len) r[ch] = lds128(ring + (size_t)slot * kChunkBytes + tid * 16);
                     __syncwarp();
@@ -405,35 +458,49 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
             // ---- pass 1b: thread-local sum of exp(x - m_thread) from registers: one MUFU per element
             const float m = fmaxf(bf16lo(mx), bf16hi(mx));
             const float ms = m == -INFINITY ? 0.f : m;
-            float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+            float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f, u0 = 0.f, u1 = 0.f;
 #pragma unroll
             for (int ch = 0; ch < NCH; ++ch) {
                 if (ch < nch) {
-                    s0 += ex2((bf16lo(r[ch].x) - ms) * kLog2e);
-                    s1 += ex2((bf16hi(r[ch].x) - ms) * kLog2e);
-                    s2 += ex2((bf16lo(r[ch].y) - ms) * kLog2e);
-                    s3 += ex2((bf16hi(r[ch].y) - ms) * kLog2e);
-                    s0 += ex2((bf16lo(r[ch].z) - ms) * kLog2e);
-                    s1 += ex2((bf16hi(r[ch].z) - ms) * kLog2e);
-                    s2 += ex2((bf16lo(r[ch].w) - ms) * kLog2e);
-                    s3 += ex2((bf16hi(r[ch].w) - ms) * kLog2e);
+                    acc_exp(bf16lo(r[ch].x), ms, s0, u0, EXT);
+                    acc_exp(bf16hi(r[ch].x), ms, s1, u1, EXT);
+                    acc_exp(bf16lo(r[ch].y), ms, s2, u0, EXT);
+                    acc_exp(bf16hi(r[ch].y), ms, s3, u1, EXT);
+                    acc_exp(bf16lo(r[ch].z), ms, s0, u0, EXT);
+                    acc_exp(bf16hi(r[ch].z), ms, s1, u1, EXT);
+                    acc_exp(bf16lo(r[ch].w), ms, s2, u0, EXT);
+                    acc_exp(bf16hi(r[ch].w), ms, s3, u1, EXT);
                 }
             }
             float s = (s0 + s1) + (s2 + s3);
             // ---- warp partial, published to every CTA of the cluster
             const float mw = warp_max(m);
-            const float sw = warp_sum(s * exp_diff(m, mw));
+            float sw, uw = 0.f;
+            if (EXT) {
+                float u = u0 + u1;
+                rebase(m, mw, s, u);
+                sw = warp_sum(s);
+                uw = warp_sum(u);
+            } else {
+                sw = warp_sum(s * exp_diff(m, mw));
+            }
             const int par = k & 1;
             float2* mypart = part + par * kParts;
+            float* mypartu = partu + par * kParts;
             if (lane == 0) {
                 mypart[rank * kConsWarps + warp] = make_float2(mw, sw);
+                if (EXT) mypartu[rank * kConsWarps + warp] = uw;
                 if (CSIZE > 1) {
                     const uint64_t v = ((uint64_t)__float_as_uint(sw) << 32) | (uint64_t)__float_as_uint(mw);
                     const uint32_t a = smem_u32(&mypart[rank * kConsWarps + warp]), b = smem_u32(&pbar[par]);
+                    const uint32_t au = smem_u32(&mypartu[rank * kConsWarps + warp]);
 #pragma unroll
                     for (uint32_t q = 0; q < (uint32_t)CSIZE; ++q)
-                        if (q != rank) st_async_b64(mapa(a, q), v, mapa(b, q));
-                    if (warp == 0) mbar_arrive_expect_tx(&pbar[par], (uint32_t)((CSIZE - 1) * kConsWarps * 8));
+                        if (q != rank) {
+                            st_async_b64(mapa(a, q), v, mapa(b, q));
+                            if (EXT) st_async_b32(mapa(au, q), __float_as_uint(uw), mapa(b, q));
+                        }
+                    if (warp == 0) mbar_arrive_expect_tx(&pbar[par], (uint32_t)((CSIZE - 1) * kConsWarps * (EXT ? 12 : 8)));
                     else mbar_arrive(&pbar[par]);
                 } else {
                     mbar_arrive(&pbar[par]);
@@ -444,14 +511,32 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
             float2 pv = lane < kParts ? mypart[lane] : make_float2(-INFINITY, 0.f);
             float2 pw = (kParts > 32 && lane + 32 < kParts) ? mypart[lane + 32] : make_float2(-INFINITY, 0.f);
             const float M = warp_max(fmaxf(pv.x, pw.x));
-            const float S = warp_sum(pv.y * exp_diff(pv.x, M) + pw.y * exp_diff(pw.x, M));
-            const TokScalars ts = token_scalars(M, S, zy, old, A, w, p.eps_lo, p.eps_hi, p.grad_scale);
+            float S, U = 0.f;
+            if (EXT) {
+                float uv = lane < kParts ? mypartu[lane] : 0.f;
+                float ux = (kParts > 32 && lane + 32 < kParts) ? mypartu[lane + 32] : 0.f;
+                rebase(pv.x, M, pv.y, uv);
+                rebase(pw.x, M, pw.y, ux);
+                S = warp_sum(pv.y + pw.y);
+                U = warp_sum(uv + ux);
+            } else {
+                S = warp_sum(pv.y * exp_diff(pv.x, M) + pw.y * exp_diff(pw.x, M));
+            }
+            const TokScalars ts = token_scalars(M, S, zy, old, A, w, p.eps_lo, p.eps_hi, p.grad_scale,
+                                                EXT && p.ref_logp != nullptr && p.kl_coef != 0.f, ref, p.kl_coef);
             if (tid == 0 && rank == 0) {
                 p.row_val[kidx] = ts.wl;
                 p.row_kl[kidx] = ts.wkl;
                 p.row_clip[kidx] = (uint8_t)(w > 0.f ? ts.clip : 0);
                 if (p.logp_out) p.logp_out[row] = ybad ? 0.f : ts.logp;
                 if (ybad) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_BAD_TARGET);
+                if (EXT) {
+                    const float H = ybad ? 0.f : ts.logS - U / S;   // step 9: H = lse - sum p z = log S - sum e^{z-M}(z-M) / S
+                    p.row_k3[kidx] = ts.wk3;
+                    p.row_ent[kidx] = (double)w * (double)H;
+                    if (p.k3_out) p.k3_out[row] = ybad ? 0.f : ts.k3;
+                    if (p.ent_out) p.ent_out[row] = H;
+                }
             }
             // ---- pass 2: dlogits = g (1[v=y] - exp(z - lse)), bf16 RNE, one 16-byte store per vector
             __nv_bfloat16* drow = dlogits + row * p.ld + sl_begin;
@@ -500,7 +585,7 @@ __device__ __forceinline__ float ld_logit<__nv_bfloat16>(const __nv_bfloat16* p,
 template <typename TIn, int G>
 __global__ void __launch_bounds__(256) loss_rows_generic(const LossParams p) {
     constexpr int kGroups = 256 / G;
-    __shared__ float s_red[2][kGroups][8];
+    __shared__ float s_red[3][kGroups][8];
     const int tid = threadIdx.x, gl = tid % G, gi = tid / G, lane = tid & 31, wig = gl >> 5;
     const TIn* logits = reinterpret_cast<const TIn*>(p.logits);
     __nv_bfloat16* dlogits = reinterpret_cast<__nv_bfloat16*>(p.dlogits);
@@ -512,9 +597,10 @@ __global__ void __launch_bounds__(256) loss_rows_generic(const LossParams p) {
         const bool inrange = row < p.T;
         const bool act = inrange && p.mask[row] != 0;
         int y = 0, sg = 0;
-        float old = 0.f, A = 0.f, w = 0.f, zy = 0.f;
+        float old = 0.f, A = 0.f, w = 0.f, zy = 0.f, ref = 0.f;
         bool ybad = false;
         if (act) {
+            if (p.ext && p.ref_logp) ref = p.ref_logp[row];
             y = p.targets[row];
             sg = p.seg_ids[row];
             old = p.old_logp[row];
@@ -537,22 +623,31 @@ __global__ void __launch_bounds__(256) loss_rows_generic(const LossParams p) {
 #pragma unroll
             for (int i = 1; i < G / 32; ++i) m = fmaxf(m, s_red[0][gi][i]);
         }
-        float s = 0.f;
+        float s = 0.f, u = 0.f;   // u = sum e^{z-m} (z-m): entropy of the row (extended form)
         if (act)
-            for (int v = gl; v < V; v += G) s += ex2((ld_logit<TIn>(zrow, v) - m) * kLog2e);
+            for (int v = gl; v < V; v += G) acc_exp(ld_logit<TIn>(zrow, v), m, s, u, true);
         s = warp_sum(s);
+        u = warp_sum(u);
         if (G > 32) {
-            if (lane == 0) s_red[1][gi][wig] = s;
+            if (lane == 0) {
+                s_red[1][gi][wig] = s;
+                s_red[2][gi][wig] = u;
+            }
             __syncthreads();
             s = 0.f;
+            u = 0.f;
 #pragma unroll
-            for (int i = 0; i < G / 32; ++i) s += s_red[1][gi][i];
+            for (int i = 0; i < G / 32; ++i) {
+                s += s_red[1][gi][i];
+                u += s_red[2][gi][i];
+            }
         }
         if (inrange) {
             __nv_bfloat16* drow = dlogits + row * p.ld;
             float g = 0.f, lse = 0.f;
             if (act) {
-                const TokScalars ts = token_scalars(m, s, zy, old, A, w, p.eps_lo, p.eps_hi, p.grad_scale);
+                const TokScalars ts = token_scalars(m, s, zy, old, A, w, p.eps_lo, p.eps_hi, p.grad_scale,
+                                                    p.ext && p.ref_logp != nullptr && p.kl_coef != 0.f, ref, p.kl_coef);
                 g = ts.g;
                 lse = ts.lse;
                 if (gl == 0) {
@@ -561,12 +656,25 @@ __global__ void __launch_bounds__(256) loss_rows_generic(const LossParams p) {
                     p.row_clip[row] = (uint8_t)(w > 0.f ? ts.clip : 0);
                     if (p.logp_out) p.logp_out[row] = ybad ? 0.f : ts.logp;
                     if (ybad) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_BAD_TARGET);
+                    if (p.ext) {
+                        const float H = ybad ? 0.f : ts.logS - u / s;
+                        p.row_k3[row] = ts.wk3;
+                        p.row_ent[row] = (double)w * (double)H;
+                        if (p.k3_out) p.k3_out[row] = ybad ? 0.f : ts.k3;
+                        if (p.ent_out) p.ent_out[row] = H;
+                    }
                 }
             } else if (gl == 0) {
                 p.row_val[row] = 0.0;
                 p.row_kl[row] = 0.0;
                 p.row_clip[row] = 0;
                 if (p.logp_out) p.logp_out[row] = 0.f;
+                if (p.ext) {
+                    p.row_k3[row] = 0.0;
+                    p.row_ent[row] = 0.0;
+                    if (p.k3_out) p.k3_out[row] = 0.f;
+                    if (p.ent_out) p.ent_out[row] = 0.f;
+                }
             }
             if (g != 0.f) {
                 const float coef = -g, k2 = -lse * kLog2e;
@@ -610,8 +718,37 @@ __global__ void __launch_bounds__(1024) loss_final_kernel(const LossParams p, in
         }
         __syncthreads();
     }
+    double pg = s_a[0];
+    if (p.ext) {   // steps 8-9: second fixed-order pass over the KL and entropy terms, same tree
+        __syncthreads();
+        a = 0.0;
+        b = 0.0;
+        for (int64_t i = tid; i < n; i += 1024) {
+            a += p.row_k3[i];
+            b += p.row_ent[i];
+        }
+        const double hold = s_b[0];
+        __syncthreads();
+        s_a[tid] = a; s_b[tid] = b;
+        __syncthreads();
+        for (int o = 512; o; o >>= 1) {
+            if (tid < o) {
+                s_a[tid] += s_a[tid + o];
+                s_b[tid] += s_b[tid + o];
+            }
+            __syncthreads();
+        }
+        if (tid == 0) {
+            pg += (double)p.kl_coef * s_a[0];
+            if (p.ext_out) {
+                p.ext_out[0] = (float)s_a[0];
+                p.ext_out[1] = (float)s_b[0];
+            }
+            s_b[0] = hold;
+        }
+    }
     if (tid == 0) {
-        p.loss_out[0] = (float)s_a[0];
+        p.loss_out[0] = (float)pg;
         if (p.stats_out) {
             p.stats_out[0] = (float)p.ctrl->n_active;
             p.stats_out[1] = (float)s_c[0][0];
@@ -643,9 +780,9 @@ __global__ void __launch_bounds__(256) segment_counts_kernel(const uint8_t* __re
     }
 }
 
-template <int NCH, int CSIZE>
-cudaError_t launch_rows(const LossParams& p, int num_sms, cudaStream_t stream) {
-    auto kern = loss_rows_kernel<NCH, CSIZE>;
+template <int NCH, int CSIZE, bool EXT>
+cudaError_t launch_rows_t(const LossParams& p, int num_sms, cudaStream_t stream) {
+    auto kern = loss_rows_kernel<NCH, CSIZE, EXT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmemBytes);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
@@ -663,6 +800,11 @@ cudaError_t launch_rows(const LossParams& p, int num_sms, cudaStream_t stream) {
     return cudaLaunchKernelEx(&cfg, kern, p);
 }
 
+template <int NCH, int CSIZE>
+cudaError_t launch_rows(const LossParams& p, int num_sms, cudaStream_t stream) {
+    return p.ext ? launch_rows_t<NCH, CSIZE, true>(p, num_sms, stream) : launch_rows_t<NCH, CSIZE, false>(p, num_sms, stream);
+}
+
 }  // namespace
 
 extern "C" size_t ajt_loss_workspace_bytes(int64_t T, int32_t V, int32_t S) {
@@ -671,12 +813,21 @@ extern "C" size_t ajt_loss_workspace_bytes(int64_t T, int32_t V, int32_t S) {
     return loss_ws_layout(T, S).total;
 }
 
-extern "C" int ajt_policy_loss_fwd_bwd(const void* logits, const int32_t* targets, const float* old_logp, const float* adv,
-                                       const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T,
-                                       int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype, const float* seg_denom,
-                                       float inv_num_segs, float grad_scale, void* dlogits, float* loss_out, float* logp_out,
-                                       float* stats_out, void* workspace, size_t workspace_bytes, ajt_stream_t stream_) {
+namespace {
+struct LossExt {   // steps 8-9 (ajt_policy_loss_fwd_bwd_ext)
+    int32_t on;
+    const float* ref_logp;
+    float kl_coef;
+    float *k3_out, *ent_out, *ext_out;
+};
+
+int loss_call(const void* logits, const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
+              const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T, int32_t V, int32_t S, int64_t ld_logits,
+              int32_t logits_dtype, const float* seg_denom, float inv_num_segs, float grad_scale, void* dlogits, float* loss_out,
+              float* logp_out, float* stats_out, const LossExt& x, void* workspace, size_t workspace_bytes,
+              ajt_stream_t stream_) {
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (x.on && (!x.ext_out || !(x.kl_coef >= 0.f))) return AJT_ERR_INVALID_ARG;
     if (T < 0 || V <= 0 || S <= 0 || ld_logits < V || T >= ((int64_t)1 << 31)) return AJT_ERR_INVALID_ARG;
     if (!(eps_lo >= 0.f) || !(eps_hi >= 0.f) || inv_num_segs < 0.f) return AJT_ERR_INVALID_ARG;
     if (logits_dtype != AJT_DT_BF16 && logits_dtype != AJT_DT_F32) return AJT_ERR_INVALID_ARG;
@@ -705,6 +856,10 @@ extern "C" int ajt_policy_loss_fwd_bwd(const void* logits, const int32_t* target
     p.row_val = reinterpret_cast<double*>(wsb + ws.row_val);
     p.row_kl = reinterpret_cast<double*>(wsb + ws.row_kl);
     p.row_clip = wsb + ws.row_clip;
+    p.ext = x.on; p.ref_logp = x.ref_logp; p.kl_coef = x.kl_coef; p.k3_out = x.k3_out; p.ent_out = x.ent_out; p.ext_out = x.ext_out;
+    p.rec_r = reinterpret_cast<float*>(wsb + ws.rec_r);
+    p.row_k3 = reinterpret_cast<double*>(wsb + ws.row_k3);
+    p.row_ent = reinterpret_cast<double*>(wsb + ws.row_ent);
 
     if (cudaMemsetAsync(p.ctrl, 0, ws.zero_bytes, stream) != cudaSuccess) return AJT_ERR_CUDA;
     const int ntiles = (int)((T + kPrepTile - 1) / kPrepTile);
@@ -715,6 +870,8 @@ extern "C" int ajt_policy_loss_fwd_bwd(const void* logits, const int32_t* target
     cudaError_t e = cudaSuccess;
     int by_row = 0;
     if (fast && logp_out && cudaMemsetAsync(logp_out, 0, (size_t)T * sizeof(float), stream) != cudaSuccess) return AJT_ERR_CUDA;
+    if (fast && x.on && x.k3_out && cudaMemsetAsync(x.k3_out, 0, (size_t)T * sizeof(float), stream) != cudaSuccess) return AJT_ERR_CUDA;
+    if (fast && x.on && x.ent_out && cudaMemsetAsync(x.ent_out, 0, (size_t)T * sizeof(float), stream) != cudaSuccess) return AJT_ERR_CUDA;
     if (fast && V <= 8 * kChunkElems) e = launch_rows<8, 1>(p, num_sms, stream);
     else if (fast && V <= 16 * kChunkElems) e = launch_rows<16, 1>(p, num_sms, stream);
     else if (fast && V <= 2 * 16 * kChunkElems - 16) e = launch_rows<16, 2>(p, num_sms, stream);
@@ -732,6 +889,29 @@ extern "C" int ajt_policy_loss_fwd_bwd(const void* logits, const int32_t* target
     if (e != cudaSuccess) return AJT_ERR_CUDA;
     loss_final_kernel<<<1, 1024, 0, stream>>>(p, by_row);
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
+}
+}  // namespace
+
+extern "C" int ajt_policy_loss_fwd_bwd(const void* logits, const int32_t* targets, const float* old_logp, const float* adv,
+                                       const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T,
+                                       int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype, const float* seg_denom,
+                                       float inv_num_segs, float grad_scale, void* dlogits, float* loss_out, float* logp_out,
+                                       float* stats_out, void* workspace, size_t workspace_bytes, ajt_stream_t stream) {
+    const LossExt x = {0, nullptr, 0.f, nullptr, nullptr, nullptr};
+    return loss_call(logits, targets, old_logp, adv, mask, seg_ids, eps_lo, eps_hi, T, V, S, ld_logits, logits_dtype, seg_denom,
+                     inv_num_segs, grad_scale, dlogits, loss_out, logp_out, stats_out, x, workspace, workspace_bytes, stream);
+}
+
+extern "C" int ajt_policy_loss_fwd_bwd_ext(const void* logits, const int32_t* targets, const float* old_logp, const float* adv,
+                                           const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T,
+                                           int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype, const float* seg_denom,
+                                           float inv_num_segs, float grad_scale, const float* ref_logp, float kl_coef,
+                                           void* dlogits, float* loss_out, float* logp_out, float* stats_out, float* k3_out,
+                                           float* ent_out, float* ext_out, void* workspace, size_t workspace_bytes,
+                                           ajt_stream_t stream) {
+    const LossExt x = {1, ref_logp, kl_coef, k3_out, ent_out, ext_out};
+    return loss_call(logits, targets, old_logp, adv, mask, seg_ids, eps_lo, eps_hi, T, V, S, ld_logits, logits_dtype, seg_denom,
+                     inv_num_segs, grad_scale, dlogits, loss_out, logp_out, stats_out, x, workspace, workspace_bytes, stream);
 }
 
 extern "C" int ajt_segment_counts(const uint8_t* mask, const int32_t* seg_ids, int64_t T, int32_t S, int32_t accumulate,
