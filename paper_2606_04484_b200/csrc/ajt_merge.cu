@@ -733,49 +733,34 @@ __device__ __forceinline__ void hash_batch(const int32_t* __restrict__ tl, int L
     }
 }
 
-// Keys whose prefix ends inside step s of the window: the step's tokens are re-read (L1), the lane's four inclusive prefix
-// values are formed from its snapshot, one warp sum and one warp scan turn them into F at every position of the step, and each
-// key picks its value from the lane that holds its last token.  One pass serves any number of keys ending in the step.
-__device__ __noinline__ void hash_emit_step(uint64_t* __restrict__ ent_hash, const int32_t* __restrict__ tl, int Li, int64_t lo,
-                                            int64_t hi, int win0, int s, uint32_t w0_window, const uint64_t* snap_s,
-                                            const int32_t* __restrict__ gln, int rank, int ebase) {
+// Sum of a 64-bit value over the warp (mod 2^64) with three REDUX instead of ten shuffles: 22 + 22 + 20-bit slices, whose
+// 32-term sums fit 32 bits.
+__device__ __forceinline__ uint64_t warp_sum_u64_redux(uint64_t v) {
+    const uint32_t a = (uint32_t)v & 0x3fffffu, b = (uint32_t)(v >> 22) & 0x3fffffu, c = (uint32_t)(v >> 44);
+    const uint32_t sa = __reduce_add_sync(0xffffffffu, a), sb = __reduce_add_sync(0xffffffffu, b);
+    const uint32_t sc = __reduce_add_sync(0xffffffffu, c);
+    return (uint64_t)sa + ((uint64_t)sb << 22) + ((uint64_t)sc << 44);
+}
+
+// One key: F at prefix length (position r of the window) + 1.  Every lane adds to its running sum BEFORE step s = r >> 7 (its
+// snapshot) the tokens of that step it holds at positions <= r (re-read: L1), and one warp sum gives the value.  ~40
+// instructions per key; a window holds the end of 0-3 requested prefixes.
+__device__ __forceinline__ uint64_t hash_key_value(const int32_t* __restrict__ tl, int Li, int64_t lo, int64_t hi, int win0, int r,
+                                                   uint32_t w0_window, const uint64_t* snap) {
     const int lane = threadIdx.x & 31;
-    const int q = win0 + 128 * s + 4 * lane;
-    const int4 x = load_step<false>(tl, Li, q, lo, hi);
+    const int s = r >> 7;
+    const int4 x = load_step<false>(tl, Li, win0 + 128 * s + 4 * lane, lo, hi);
+    const int c = (r & 127) - 4 * lane;   // tokens k <= c of this lane lie inside the prefix
     uint32_t w = w0_window * c_w128.v[s];
-    uint64_t c0 = (uint64_t)(uint32_t)x.x * w;
+    uint64_t part = snap[s * 32];
+    if (c >= 0) part = mad_wide((uint32_t)x.x, w, part);
     w *= kW;
-    uint64_t c1 = mad_wide((uint32_t)x.y, w, c0);
+    if (c >= 1) part = mad_wide((uint32_t)x.y, w, part);
     w *= kW;
-    uint64_t c2 = mad_wide((uint32_t)x.z, w, c1);
+    if (c >= 2) part = mad_wide((uint32_t)x.z, w, part);
     w *= kW;
-    uint64_t c3 = mad_wide((uint32_t)x.w, w, c2);
-    const uint64_t A = warp_sum_u64(snap_s[lane]);
-    uint64_t inc = c3;   // inclusive scan of the lanes' step sums
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint64_t t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += t;
-    }
-    const uint64_t base = A + inc - c3;
-    c0 += base; c1 += base; c2 += base; c3 += base;   // F at prefix lengths q+1 .. q+4
-    for (int a0 = 0; a0 <= rank; a0 += 32) {
-        const int a = a0 + lane;
-        int rel = -1;
-        if (a <= rank) {
-            const int Lp = gln[a];
-            const int r = Lp - 1 - win0 - 128 * s;
-            if (Lp <= Li && r >= 0 && r < 128) rel = r;
-        }
-        if (!__any_sync(0xffffffffu, rel >= 0)) continue;
-        const int sl = rel >= 0 ? rel >> 2 : 0;
-        const uint64_t v0 = __shfl_sync(0xffffffffu, c0, sl), v1 = __shfl_sync(0xffffffffu, c1, sl);
-        const uint64_t v2 = __shfl_sync(0xffffffffu, c2, sl), v3 = __shfl_sync(0xffffffffu, c3, sl);
-        if (rel >= 0) {
-            const int e = rel & 3;
-            ent_hash[ebase + a] = e == 0 ? v0 : e == 1 ? v1 : e == 2 ? v2 : v3;
-        }
-    }
+    if (c >= 3) part = mad_wide((uint32_t)x.w, w, part);
+    return warp_sum_u64_redux(part);
 }
 
 __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const MergeParams p) {
@@ -810,17 +795,6 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
         const uint32_t w0 = window_weight(j, d) * LW;        // weight W^(q+3) of this lane's first slot q = win0 + 4 lane
         const int rank = rec.z, ebase = rec.w;
         const int32_t* gln = p.glen + rec.y;
-        // which 128-token steps of this window hold the end of a requested prefix (L_a of an earlier member, or L_i)
-        uint32_t stepmask = 0;
-        for (int a0 = 0; a0 <= rank; a0 += 32) {
-            const int a = a0 + lane;
-            if (a <= rank) {
-                const int Lp = __ldg(gln + a);
-                const int rel = Lp - 1 - win0;
-                if (Lp <= Li && rel >= 0 && rel < kHSeg) stepmask |= 1u << (rel >> 7);
-            }
-        }
-        stepmask = __reduce_or_sync(0xffffffffu, stepmask);
         // ---- streaming pass: four batches of 512 positions
         uint32_t w[4] = {w0, w0 * kW, w0 * kW * kW, w0 * kW * kW * kW};
         uint32_t diff = 0;
@@ -848,11 +822,21 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
         const uint64_t tot = warp_sum_u64(acc);
         if (lane == 0) p.seg_part[sidx] = tot;
         if (win0 < Lprev && __any_sync(0xffffffffu, diff != 0) && lane == 0) p.link_bad[i] = 1;
-        // ---- key emission pass: only the steps that hold the end of a requested prefix
+        // ---- key emission: the requested prefixes (L_a of an earlier member, or L_i) that end inside this window
         __syncwarp();
-        for (uint32_t sm = stepmask; sm; sm &= sm - 1) {
-            const int s = __ffs(sm) - 1;
-            hash_emit_step(p.ent_hash, tl, Li, lo, hi, win0, s, w0, snap + s * 32 - lane, gln, rank, ebase);
+        for (int a0 = 0; a0 <= rank; a0 += 32) {
+            const int a = a0 + lane;
+            int rel = -1;
+            if (a <= rank) {
+                const int Lp = __ldg(gln + a);
+                const int r = Lp - 1 - win0;
+                if (Lp <= Li && r >= 0 && r < kHSeg) rel = r;
+            }
+            for (uint32_t m = __ballot_sync(0xffffffffu, rel >= 0); m; m &= m - 1) {
+                const int b = __ffs(m) - 1;
+                const uint64_t F = hash_key_value(tl, Li, lo, hi, win0, __shfl_sync(0xffffffffu, rel, b), w0, snap);
+                if (lane == b) p.ent_hash[ebase + a] = F;
+            }
         }
         __syncwarp();
     }
