@@ -792,6 +792,9 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
         const int d = (int)((off + p.mis) & (kHSeg - 1));   // the timeline starts d slots into its first window
         const int j = sidx - rec.x;                          // window index inside the timeline
         const int win0 = j * kHSeg - d;                      // timeline position of the window's first slot
+        // pull the whole window (<= 8 KB = 64 lines) towards L2 now: the four batches below then wait on L2, not on DRAM
+        for (int e = max(win0, 0) + 32 * lane; e < min(win0 + kHSeg, Li); e += 1024)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(tl + e));
         const uint32_t w0 = window_weight(j, d) * LW;        // weight W^(q+3) of this lane's first slot q = win0 + 4 lane
         const int rank = rec.z, ebase = rec.w;
         const int32_t* gln = p.glen + rec.y;
