@@ -39,6 +39,7 @@ def lib():
         build()
         _lib = C.CDLL(_SO)
         _lib.ajt_oracle_merge.restype = C.c_int
+        _lib.ajt_oracle_merge_blocks.restype = C.c_int
         _lib.ajt_oracle_loss.restype = C.c_int
         _lib.ajt_oracle_loss_ex.restype = C.c_int
         _lib.ajt_oracle_round_bf16.restype = C.c_double
@@ -111,6 +112,70 @@ def merge_timelines(tokens, offsets, traj_ids, resp_start=None, mask_in=None, ol
     M, No = int(cnt[0]), int(cnt[1])
     return MergeResult(mt[:No].copy(), mm[:No].copy(), ms[:No].copy(), None if ml is None else ml[:No].copy(),
                        mo[:M + 1].copy(), mor[:M].copy(), mtr[:M].copy(), ow[:n].copy(), M, No)
+
+
+AUTHOR_ENV, AUTHOR_USER, AUTHOR_LLM = 0, 1, 2   # author labels of eq. (1)
+MATCH_TEXT = 0    # "text (default)"
+MATCH_TOKEN = 1   # "token"
+
+
+@dataclass
+class BlockMergeResult:
+    merged_tokens: np.ndarray         # int32 [N_out]
+    merged_mask: np.ndarray           # uint8 [N_out]
+    merged_logp: Optional[np.ndarray]  # float32 [N_out]
+    merged_tok_src: np.ndarray        # int32 [N_out]
+    merged_offsets: np.ndarray        # int64 [M+1]   tokens
+    merged_block_offsets: np.ndarray  # int64 [M+1]   blocks
+    merged_block_src: np.ndarray      # int32 [B_out]
+    merged_block_author: np.ndarray   # uint8 [B_out]
+    merged_block_tok_off: np.ndarray  # int64 [B_out+1]
+    merged_origin: np.ndarray         # int32 [M]
+    merged_traj: np.ndarray           # int32 [M]
+    owner: np.ndarray                 # int32 [n]
+    M: int
+    B_out: int
+    N_out: int
+
+
+def merge_blocks(block_ids, block_offsets, traj_ids, author, tok_off, tokens, logp=None, tok_mask=None,
+                 match: int = MATCH_TEXT) -> BlockMergeResult:
+    """Algorithm 1 line by line on timelines of message blocks (DESIGN.md O-B)."""
+    block_ids = _c(block_ids, np.int64)
+    block_offsets = _c(block_offsets, np.int64)
+    traj_ids = _c(traj_ids, np.int32)
+    author = _c(author, np.uint8)
+    tok_off = _c(tok_off, np.int64)
+    tokens = _c(tokens, np.int32)
+    logp = _c(logp, np.float32)
+    tok_mask = _c(tok_mask, np.uint8)
+    n = int(traj_ids.shape[0])
+    B = int(block_ids.shape[0])
+    N = int(tokens.shape[0])
+    assert block_offsets.shape[0] == n + 1 and tok_off.shape[0] == B + 1 and author.shape[0] == B
+    assert n == 0 or (int(block_offsets[-1]) == B and int(tok_off[-1]) == N)
+    mt = np.zeros(max(N, 1), np.int32)
+    mm = np.zeros(max(N, 1), np.uint8)
+    ml = np.zeros(max(N, 1), np.float32) if logp is not None else None
+    ms = np.zeros(max(N, 1), np.int32)
+    mo = np.zeros(n + 1, np.int64)
+    mbo = np.zeros(n + 1, np.int64)
+    mbs = np.zeros(max(B, 1), np.int32)
+    mba = np.zeros(max(B, 1), np.uint8)
+    mbt = np.zeros(B + 1, np.int64)
+    mor = np.zeros(max(n, 1), np.int32)
+    mtr = np.zeros(max(n, 1), np.int32)
+    ow = np.zeros(max(n, 1), np.int32)
+    cnt = np.zeros(3, np.int64)
+    rc = lib().ajt_oracle_merge_blocks(_p(block_ids), _p(block_offsets), _p(traj_ids), _p(author), _p(tok_off), _p(tokens),
+                                       _p(logp), _p(tok_mask), C.c_int32(n), C.c_int32(match), _p(mt), _p(mm), _p(ml), _p(ms),
+                                       _p(mo), _p(mbo), _p(mbs), _p(mba), _p(mbt), _p(mor), _p(mtr), _p(ow), _p(cnt))
+    if rc != 0:
+        raise ValueError(f"ajt_oracle_merge_blocks: invalid input (rc={rc})")
+    M, Bo, No = int(cnt[0]), int(cnt[1]), int(cnt[2])
+    return BlockMergeResult(mt[:No].copy(), mm[:No].copy(), None if ml is None else ml[:No].copy(), ms[:No].copy(),
+                            mo[:M + 1].copy(), mbo[:M + 1].copy(), mbs[:Bo].copy(), mba[:Bo].copy(), mbt[:Bo + 1].copy(),
+                            mor[:M].copy(), mtr[:M].copy(), ow[:n].copy(), M, Bo, No)
 
 
 @dataclass

@@ -374,3 +374,126 @@ void ajt_oracle_set_threads(int n) {
 void ajt_oracle_round_bf16_array(const double* in, double* out, int64_t n) {
     for (int64_t i = 0; i < n; ++i) out[i] = ajt_oracle_round_bf16(in[i]);
 }
+
+/* ------------------------------------------------------------------------------ block-level merge */
+
+#define ORACLE_AUTHOR_LLM 2   /* author labels: 0 env, 1 user, 2 llm (eq. (1)) */
+#define ORACLE_MATCH_TEXT 0   /* "text (default): exact text match at every aligned position" */
+#define ORACLE_MATCH_TOKEN 1  /* "token: exact token-id match at every aligned position" */
+
+/* Match(S^[k], T^[k]) of PAPER.md:182 for block sb of S and block tb of T.  The text m of a block is represented by a
+ * caller-supplied 64-bit id with id equality <=> text equality (reading B-1). */
+static int block_match(const int64_t* block_ids, const int64_t* tok_off, const int32_t* tokens, int64_t sb, int64_t tb,
+                       int32_t match_mode) {
+    if (match_mode == ORACLE_MATCH_TEXT) return block_ids[sb] == block_ids[tb];
+    int64_t ls = tok_off[sb + 1] - tok_off[sb], lt = tok_off[tb + 1] - tok_off[tb];
+    if (ls != lt) return 0;
+    for (int64_t p = 0; p < ls; ++p)
+        if (tokens[tok_off[sb] + p] != tokens[tok_off[tb] + p]) return 0;
+    return 1;
+}
+
+/*
+ * Block-level timeline merging: Algorithm 1 followed line by line on timelines of
+ * message blocks (eq. (1)), per episode (timelines with different traj_ids are never compared, M-4).
+ *
+ * Timeline i = blocks block_offsets[i] .. block_offsets[i+1]; block b = (text id block_ids[b], author[b], tokens /
+ * logp / tok_mask at tok_off[b] .. tok_off[b+1]).  tok_mask NULL => mu = 1 exactly on the tokens of llm blocks
+ * (PAPER.md:176).  logp may be NULL.
+ *
+ * Outputs (caller-allocated at worst-case capacity: all tokens, all blocks, n sequences):
+ *   merged_tokens / merged_mask / merged_logp / merged_tok_src [N_out]  (tok_src = timeline whose block supplied the token
+ *   where the mask is 1, else -1), merged_offsets[M+1] (tokens), merged_block_offsets[M+1] (blocks),
+ *   merged_block_src[B_out] (timeline whose block k stands at block k of the survivor), merged_block_author[B_out],
+ *   merged_block_tok_off[B_out+1], merged_origin[M], merged_traj[M], owner[n], counts[3] = {M, B_out, N_out}.
+ * Returns 0, or -1 on invalid input.
+ */
+int ajt_oracle_merge_blocks(const int64_t* block_ids, const int64_t* block_offsets, const int32_t* traj_ids,
+                            const uint8_t* author, const int64_t* tok_off, const int32_t* tokens, const float* logp,
+                            const uint8_t* tok_mask, int32_t n, int32_t match_mode,
+                            int32_t* merged_tokens, uint8_t* merged_mask, float* merged_logp, int32_t* merged_tok_src,
+                            int64_t* merged_offsets, int64_t* merged_block_offsets, int32_t* merged_block_src,
+                            uint8_t* merged_block_author, int64_t* merged_block_tok_off,
+                            int32_t* merged_origin, int32_t* merged_traj, int32_t* owner, int64_t* counts) {
+    if (n < 0 || (match_mode != ORACLE_MATCH_TEXT && match_mode != ORACLE_MATCH_TOKEN)) return -1;
+    if (block_offsets[0] != 0) return -1;
+    for (int64_t i = 0; i < n; ++i)
+        if (block_offsets[i + 1] - block_offsets[i] < 1) return -1;   /* K_i >= 1 */
+    const int64_t B = block_offsets[n];
+    if (tok_off[0] != 0) return -1;
+    for (int64_t b = 0; b < B; ++b)
+        if (tok_off[b + 1] < tok_off[b]) return -1;
+
+    /* the mutable part of every block: author and where its tokens / logprobs come from (Alg. 1 lines 12-14) */
+    uint8_t* cur_author = (uint8_t*)malloc((size_t)B + 1);
+    int32_t* cur_src = (int32_t*)malloc(sizeof(int32_t) * ((size_t)B + 1));
+    uint8_t* absorbed = (uint8_t*)calloc((size_t)n + 1, 1);            /* the set A, line 1 */
+    int64_t* absorber = (int64_t*)malloc(sizeof(int64_t) * ((size_t)n + 1));
+    for (int64_t i = 0; i < n; ++i) {
+        absorber[i] = i;
+        for (int64_t b = block_offsets[i]; b < block_offsets[i + 1]; ++b) { cur_author[b] = author[b]; cur_src[b] = (int32_t)i; }
+    }
+
+    for (int64_t i = n - 1; i >= 1; --i) {                               /* line 2 */
+        if (absorbed[i]) continue;                                       /* lines 3-5 */
+        const int64_t Ki = block_offsets[i + 1] - block_offsets[i];
+        for (int64_t j = i - 1; j >= 0; --j) {                           /* line 6 */
+            if (absorbed[j]) continue;                                   /* lines 7-8 */
+            if (traj_ids[j] != traj_ids[i]) continue;                    /* one list per episode (M-4) */
+            const int64_t Kj = block_offsets[j + 1] - block_offsets[j];
+            if (Ki < Kj) continue;                                       /* line 9: |T_i| >= |T_j| */
+            int ok = 1;
+            for (int64_t k = 0; k < Kj && ok; ++k)                       /* line 9: Match for all k in [1, |T_j|] */
+                ok = block_match(block_ids, tok_off, tokens, block_offsets[i] + k, block_offsets[j] + k, match_mode);
+            if (!ok) continue;
+            for (int64_t k = 0; k < Kj; ++k) {                           /* line 10 */
+                const int64_t bi = block_offsets[i] + k, bj = block_offsets[j] + k;
+                if (cur_author[bj] == ORACLE_AUTHOR_LLM && cur_author[bi] != ORACLE_AUTHOR_LLM) {   /* line 11 */
+                    cur_author[bi] = ORACLE_AUTHOR_LLM;                  /* line 12 */
+                    cur_src[bi] = cur_src[bj];                           /* lines 13-14: tokens and logprob of T_j^[k] */
+                }
+            }
+            absorbed[j] = 1;                                             /* line 18 */
+            absorber[j] = i;
+        }
+    }
+
+    /* line 22: survivors in original order, flattened */
+    int64_t M = 0, Bout = 0, Nout = 0;
+    int64_t* midx = (int64_t*)malloc(sizeof(int64_t) * ((size_t)n + 1));
+    for (int64_t s = 0; s < n; ++s) {
+        midx[s] = -1;
+        if (absorbed[s]) continue;
+        midx[s] = M;
+        merged_origin[M] = (int32_t)s;
+        merged_traj[M] = traj_ids[s];
+        merged_offsets[M] = Nout;
+        merged_block_offsets[M] = Bout;
+        const int64_t Ks = block_offsets[s + 1] - block_offsets[s];
+        for (int64_t k = 0; k < Ks; ++k) {
+            const int64_t b = block_offsets[s] + k;
+            const int64_t sj = cur_src[b];
+            const int64_t sb = block_offsets[sj] + k;                    /* block k of the supplying timeline */
+            merged_block_src[Bout] = (int32_t)sj;
+            merged_block_author[Bout] = cur_author[b];
+            merged_block_tok_off[Bout] = Nout;
+            for (int64_t q = tok_off[sb]; q < tok_off[sb + 1]; ++q) {
+                const int mk = tok_mask ? (tok_mask[q] != 0) : (cur_author[b] == ORACLE_AUTHOR_LLM);
+                merged_tokens[Nout] = tokens[q];
+                merged_mask[Nout] = (uint8_t)mk;
+                merged_tok_src[Nout] = mk ? (int32_t)sj : -1;
+                if (merged_logp) merged_logp[Nout] = (logp && mk) ? logp[q] : 0.0f;
+                ++Nout;
+            }
+            ++Bout;
+        }
+        ++M;
+    }
+    merged_offsets[M] = Nout;
+    merged_block_offsets[M] = Bout;
+    merged_block_tok_off[Bout] = Nout;
+    for (int64_t j = 0; j < n; ++j) owner[j] = (int32_t)midx[absorber[j]];
+    counts[0] = M; counts[1] = Bout; counts[2] = Nout;
+    free(cur_author); free(cur_src); free(absorbed); free(absorber); free(midx);
+    return 0;
+}

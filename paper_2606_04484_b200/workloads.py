@@ -309,3 +309,113 @@ def small_logits(T: int, V: int, sigma: float, seed: int, key: int = 0) -> np.nd
     large matrices are drawn on the GPU by the harness with a seeded torch.Generator."""
     r = rng_for(seed, 0xA0, key, T & 0xFFFFFFFF, V)
     return (r.standard_normal((T, V), dtype=np.float32) * np.float32(sigma)).astype(np.float32)
+
+
+# --------------------------------------------------------------------------- block-level (text matching) inputs
+
+AUTHOR_ENV, AUTHOR_USER, AUTHOR_LLM = 0, 1, 2   # author labels of eq. (1), PAPER.md:172-176
+
+
+@dataclass
+class BlockSpec:
+    name: str
+    index: int
+    n_traj: int
+    turns: Tuple[int, int]        # LLM calls per trajectory
+    env_blocks: Tuple[int, int]   # env / user blocks appended before each call
+    block_len: Tuple[int, int]    # tokens per block
+    vocab: int
+    p_break: float                # per turn: one earlier block is edited (new text), which breaks the prefix there
+    p_drift: float                # per assistant block re-sent as prompt: re-tokenised differently, same text (Fig. 5)
+
+
+BLOCK_SPECS: Dict[str, BlockSpec] = {
+    # shapes follow configs[0] / configs[1] / configs[2] with their appends split into message blocks
+    "b1": BlockSpec("b1", 10, n_traj=32, turns=(6, 6), env_blocks=(1, 2), block_len=(8, 64), vocab=1024, p_break=0.2, p_drift=0.3),
+    "b2": BlockSpec("b2", 11, n_traj=64, turns=(8, 8), env_blocks=(1, 3), block_len=(64, 512), vocab=151936, p_break=0.1,
+                    p_drift=0.2),
+    "b3": BlockSpec("b3", 12, n_traj=256, turns=(20, 40), env_blocks=(1, 3), block_len=(128, 1024), vocab=151936, p_break=0.1,
+                    p_drift=0.1),
+}
+
+
+@dataclass
+class BlockInputs:
+    block_ids: np.ndarray       # int64 [B]   text id of each block (equal ids <=> equal text)
+    block_offsets: np.ndarray   # int64 [n+1] blocks of timeline i
+    traj_ids: np.ndarray        # int32 [n]
+    author: np.ndarray          # uint8 [B]
+    tok_off: np.ndarray         # int64 [B+1] tokens of block b
+    tokens: np.ndarray          # int32 [N]
+    logp: np.ndarray            # float32 [N]  (log-probs of generated tokens; 0 on prompt blocks)
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def n(self) -> int:
+        return int(self.traj_ids.shape[0])
+
+
+def _block_trajectory(spec: BlockSpec, seed: int, traj: int):
+    """One trajectory: per LLM call a list of blocks (text id, author, tokens, logp).  Within a call the context blocks are
+    the prompt (author env / user; assistant messages of earlier calls come back as env-labelled prompt blocks, possibly
+    re-tokenised) and the last block is the generated answer (author llm)."""
+    rs = rng_for(seed, spec.index, 0, traj, _F_STRUCT)
+    rt = rng_for(seed, spec.index, 0, traj, _F_TOKENS)
+    rl = rng_for(seed, spec.index, 0, traj, _F_LOGP)
+    next_id = [(traj + 1) << 32]
+
+    def new_block(author):
+        L = int(rs.integers(spec.block_len[0], spec.block_len[1] + 1))
+        next_id[0] += 1
+        return dict(id=next_id[0] * 0x9E3779B97F4A7C15 % (1 << 63), author=author, tok=draw_tokens(rt, L, spec.vocab, "uniform"))
+
+    K = int(rs.integers(spec.turns[0], spec.turns[1] + 1))
+    ctx = [new_block(AUTHOR_USER)]      # the task prompt
+    calls = []
+    for k in range(1, K + 1):
+        if k > 1 and rs.random() < spec.p_break:
+            e = int(rs.integers(0, len(ctx)))          # the agent edits / compacts its history from block e on
+            keep = int(rs.integers(1, 3))
+            ctx = ctx[:e] + [new_block(AUTHOR_ENV) for _ in range(keep)]
+        for _ in range(int(rs.integers(spec.env_blocks[0], spec.env_blocks[1] + 1))):
+            ctx.append(new_block(AUTHOR_ENV))
+        ans = new_block(AUTHOR_LLM)
+        ans["logp"] = (-np.abs(rl.standard_normal(ans["tok"].shape[0], dtype=np.float32)) - 0.05).astype(np.float32)
+        calls.append([dict(b) for b in ctx] + [ans])
+        # the answer goes back into the context as a prompt block: same text, not generated any more; the chat template
+        # may strip its thinking part, so the token ids differ although the text id is the same (PAPER.md:236-238)
+        back = dict(id=ans["id"], author=AUTHOR_ENV, tok=ans["tok"])
+        if rs.random() < spec.p_drift and ans["tok"].shape[0] > 4:
+            cut = int(rs.integers(1, ans["tok"].shape[0] // 2 + 1))
+            back["tok"] = ans["tok"][cut:]
+        ctx.append(back)
+    return calls
+
+
+def block_workload(config: str, seed: Optional[int] = None, n_traj: Optional[int] = None, order: str = "round_robin") -> BlockInputs:
+    """Timelines of message blocks for the text-level matching path."""
+    spec = BLOCK_SPECS[config]
+    seed = BASE_SEED + spec.index if seed is None else seed
+    nt = spec.n_traj if n_traj is None else n_traj
+    per_traj = [_block_trajectory(spec, seed, t) for t in range(nt)]
+    keys = [2000 + 5 * t for t in range(nt)]
+    items = []
+    if order == "traj_major":
+        for key, calls in zip(keys, per_traj):
+            items += [(key, c) for c in calls]
+    else:
+        for k in range(max(len(c) for c in per_traj)):
+            items += [(key, calls[k]) for key, calls in zip(keys, per_traj) if k < len(calls)]
+    n = len(items)
+    nb = np.array([len(c) for _, c in items], dtype=np.int64)
+    block_offsets = np.zeros(n + 1, np.int64)
+    np.cumsum(nb, out=block_offsets[1:])
+    blocks = [b for _, c in items for b in c]
+    lens = np.array([b["tok"].shape[0] for b in blocks], dtype=np.int64)
+    tok_off = np.zeros(len(blocks) + 1, np.int64)
+    np.cumsum(lens, out=tok_off[1:])
+    tokens = np.concatenate([b["tok"] for b in blocks]).astype(np.int32)
+    logp = np.concatenate([b.get("logp", np.zeros(b["tok"].shape[0], np.float32)) for b in blocks]).astype(np.float32)
+    return BlockInputs(np.array([b["id"] for b in blocks], dtype=np.int64), block_offsets,
+                       np.array([k for k, _ in items], dtype=np.int32), np.array([b["author"] for b in blocks], dtype=np.uint8),
+                       tok_off, tokens, logp, meta=dict(config=config, seed=seed, vocab=spec.vocab, n_groups=nt))
