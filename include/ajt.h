@@ -121,6 +121,48 @@ int ajt_merge_timelines(
     int64_t* counts,            /* [2] {M, N_out} */
     void* workspace, size_t workspace_bytes, ajt_stream_t stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * Stage (a'), text-level matching: Algorithm 1 on timelines of MESSAGE BLOCKS (eq. (1)) with
+ * Match = text, the paper's default strategy.
+ *
+ * Timeline i = blocks block_offsets[i] .. block_offsets[i+1].  Block b = (text, author, tokens, log-probs, mask): the text
+ * is represented by a caller-supplied 64-bit id with equal ids <=> equal texts (reading B-1); author is AJT_AUTHOR_*;
+ * tokens / logp / tok_mask of block b are elements tok_off[b] .. tok_off[b+1] of the packed arrays.
+ *   i extends j  <=>  traj_ids equal, i > j, K_i >= K_j and block_ids_i[k] == block_ids_j[k] for k < K_j
+ *   j is absorbed by its LATEST extender (the reverse double loop); survivors keep their order (line 22)
+ *   block k of a survivor s: if some member has an llm block at k and s has not, the block takes author llm, tokens and
+ *   log-probs (and mask) from the latest such member (lines 10-17); otherwise it stays s's own
+ * tok_mask NULL -> mu = 1 exactly on the tokens of llm blocks.  Token-level matching of the same data is
+ * ajt_merge_timelines on the flat token streams.
+ *
+ * Outputs (DEVICE, caller-allocated at worst-case capacity: n_tokens tokens, n_blocks blocks, n sequences):
+ *   merged_tokens / merged_mask / merged_logp / merged_tok_src [N_out] (tok_src = supplying timeline where the mask is 1,
+ *   else -1; logp 0 where the mask is 0), merged_offsets [M+1] (tokens), merged_block_offsets [M+1] (blocks),
+ *   merged_block_src [B_out] (timeline whose block k stands at block k of the survivor), merged_block_author [B_out],
+ *   merged_block_tok_off [B_out+1], merged_origin / merged_traj [M], owner [n], counts [3] = {M, B_out, N_out}.
+ * All integer / byte work: bit-exact with the definition.  Workspace: ajt_merge_blocks_workspace_bytes(n, n_blocks) bytes
+ * of DEVICE memory, 256-byte aligned (0 is returned for n_blocks >= 2^30).  Status bits as for ajt_merge_timelines
+ * (AJT_STATUS_BAD_OFFSETS also for a decreasing tok_off); `flags` as there.  Enqueues on `stream`, does not synchronise.
+ */
+enum { AJT_AUTHOR_ENV = 0, AJT_AUTHOR_USER = 1, AJT_AUTHOR_LLM = 2 };
+
+size_t ajt_merge_blocks_workspace_bytes(int32_t n, int64_t n_blocks);
+
+int ajt_merge_blocks(
+    const int64_t* block_ids,      /* DEVICE [n_blocks] text ids */
+    const int64_t* block_offsets,  /* DEVICE [n+1] block_offsets[0]=0, strictly increasing, block_offsets[n]=n_blocks */
+    const int32_t* traj_ids,       /* DEVICE [n] */
+    const uint8_t* author,         /* DEVICE [n_blocks] AJT_AUTHOR_* */
+    const int64_t* tok_off,        /* DEVICE [n_blocks+1] tok_off[0]=0, non-decreasing, tok_off[n_blocks]=n_tokens */
+    const int32_t* tokens,         /* DEVICE [n_tokens] */
+    const float* logp,             /* DEVICE [n_tokens] or NULL */
+    const uint8_t* tok_mask,       /* DEVICE [n_tokens] or NULL */
+    int32_t n, int64_t n_blocks, int64_t n_tokens, uint32_t flags,
+    int32_t* merged_tokens, uint8_t* merged_mask, float* merged_logp /* NULL iff logp is NULL */, int32_t* merged_tok_src,
+    int64_t* merged_offsets, int64_t* merged_block_offsets, int32_t* merged_block_src, uint8_t* merged_block_author,
+    int64_t* merged_block_tok_off, int32_t* merged_origin, int32_t* merged_traj, int32_t* owner, int64_t* counts,
+    void* workspace, size_t workspace_bytes, ajt_stream_t stream);
+
 /* HOST-buffer variant: same arguments but every array pointer is HOST memory (pinned for speed).
  * `arena` is DEVICE scratch of at least ajt_merge_host_arena_bytes(n, n_tokens) bytes.  Synchronises. */
 size_t ajt_merge_host_arena_bytes(int32_t n, int64_t n_tokens);

@@ -5,6 +5,9 @@ argument-marshalling binding with the same names; every step of the path runs in
 There is no CPU fallback: calls raise if the CUDA library is missing or no device is present.
 """
 from .binding import (  # noqa: F401
+    AUTHOR_ENV,
+    AUTHOR_LLM,
+    AUTHOR_USER,
     AjtError,
     DT_BF16,
     DT_F32,
@@ -24,6 +27,8 @@ from .binding import (  # noqa: F401
     library_path,
     loss_host_arena_bytes,
     loss_workspace_bytes,
+    merge_blocks,
+    merge_blocks_workspace_bytes,
     merge_host_arena_bytes,
     merge_timelines,
     merge_timelines_host,

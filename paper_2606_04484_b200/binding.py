@@ -25,7 +25,7 @@ _EXPORTS = [
     "ajt_version", "ajt_strerror", "ajt_last_status",
     "ajt_merge_workspace_bytes", "ajt_merge_timelines", "ajt_merge_host_arena_bytes", "ajt_merge_timelines_host",
     "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
-    "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext",
+    "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks_workspace_bytes", "ajt_merge_blocks",
 ]
 
 _lib = None
@@ -60,12 +60,14 @@ def lib():
         for f in ("ajt_merge_workspace_bytes", "ajt_merge_host_arena_bytes"):
             getattr(L, f).restype = C.c_size_t
             getattr(L, f).argtypes = [C.c_int32, C.c_int64]
+        L.ajt_merge_blocks_workspace_bytes.restype = C.c_size_t
+        L.ajt_merge_blocks_workspace_bytes.argtypes = [C.c_int32, C.c_int64]
         L.ajt_loss_workspace_bytes.restype = C.c_size_t
         L.ajt_loss_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
         L.ajt_loss_host_arena_bytes.restype = C.c_size_t
         L.ajt_loss_host_arena_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32]
         for f in ("ajt_merge_timelines", "ajt_merge_timelines_host", "ajt_policy_loss_fwd_bwd",
-                  "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext"):
+                  "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -193,6 +195,78 @@ def merge_timelines(tokens: torch.Tensor, offsets: torch.Tensor, traj_ids: torch
         _dp(out.workspace), C.c_size_t(out.workspace.numel()), _stream(stream))
     if rc != 0:
         raise AjtError(rc, "ajt_merge_timelines")
+    return out
+
+
+AUTHOR_ENV, AUTHOR_USER, AUTHOR_LLM = 0, 1, 2
+
+
+def merge_blocks_workspace_bytes(n: int, n_blocks: int) -> int:
+    return int(lib().ajt_merge_blocks_workspace_bytes(C.c_int32(n), C.c_int64(n_blocks)))
+
+
+@dataclass
+class BlockMergeOutput:
+    """Device tensors at worst-case capacity; `finalize()` synchronises, reads `counts` and returns views of the right length."""
+    merged_tokens: torch.Tensor
+    merged_mask: torch.Tensor
+    merged_logp: Optional[torch.Tensor]
+    merged_tok_src: torch.Tensor
+    merged_offsets: torch.Tensor
+    merged_block_offsets: torch.Tensor
+    merged_block_src: torch.Tensor
+    merged_block_author: torch.Tensor
+    merged_block_tok_off: torch.Tensor
+    merged_origin: torch.Tensor
+    merged_traj: torch.Tensor
+    owner: torch.Tensor
+    counts: torch.Tensor
+    workspace: torch.Tensor
+    M: int = -1
+    B_out: int = -1
+    N_out: int = -1
+
+    def finalize(self) -> "BlockMergeOutput":
+        c = self.counts.cpu()
+        M, Bo, No = int(c[0]), int(c[1]), int(c[2])
+        return BlockMergeOutput(self.merged_tokens[:No], self.merged_mask[:No],
+                                None if self.merged_logp is None else self.merged_logp[:No], self.merged_tok_src[:No],
+                                self.merged_offsets[:M + 1], self.merged_block_offsets[:M + 1], self.merged_block_src[:Bo],
+                                self.merged_block_author[:Bo], self.merged_block_tok_off[:Bo + 1], self.merged_origin[:M],
+                                self.merged_traj[:M], self.owner, self.counts, self.workspace, M, Bo, No)
+
+
+def merge_blocks(block_ids: torch.Tensor, block_offsets: torch.Tensor, traj_ids: torch.Tensor, author: torch.Tensor,
+                 tok_off: torch.Tensor, tokens: torch.Tensor, logp: Optional[torch.Tensor] = None,
+                 tok_mask: Optional[torch.Tensor] = None, flags: int = 0, out: Optional[BlockMergeOutput] = None,
+                 stream=None) -> BlockMergeOutput:
+    """ajt_merge_blocks (include/ajt.h): Algorithm 1 with text-level matching on timelines of message blocks."""
+    _require_cuda()
+    _check_dev(block_ids, torch.int64, "block_ids")
+    _check_dev(block_offsets, torch.int64, "block_offsets")
+    _check_dev(traj_ids, torch.int32, "traj_ids")
+    _check_dev(author, torch.uint8, "author")
+    _check_dev(tok_off, torch.int64, "tok_off")
+    _check_dev(tokens, torch.int32, "tokens")
+    _check_dev(logp, torch.float32, "logp")
+    _check_dev(tok_mask, torch.uint8, "tok_mask")
+    n, B, N = int(traj_ids.numel()), int(block_ids.numel()), int(tokens.numel())
+    dev = block_ids.device
+    if out is None:
+        e = lambda k, dt: torch.empty(max(k, 1), dtype=dt, device=dev)
+        out = BlockMergeOutput(e(N, torch.int32), e(N, torch.uint8), None if logp is None else e(N, torch.float32),
+                               e(N, torch.int32), e(n + 1, torch.int64), e(n + 1, torch.int64), e(B, torch.int32),
+                               e(B, torch.uint8), e(B + 1, torch.int64), e(n, torch.int32), e(n, torch.int32), e(n, torch.int32),
+                               e(3, torch.int64), e(merge_blocks_workspace_bytes(n, B), torch.uint8))
+    rc = lib().ajt_merge_blocks(
+        _dp(block_ids), _dp(block_offsets), _dp(traj_ids), _dp(author), _dp(tok_off), _dp(tokens), _dp(logp), _dp(tok_mask),
+        C.c_int32(n), C.c_int64(B), C.c_int64(N), C.c_uint32(flags),
+        _dp(out.merged_tokens), _dp(out.merged_mask), _dp(out.merged_logp), _dp(out.merged_tok_src), _dp(out.merged_offsets),
+        _dp(out.merged_block_offsets), _dp(out.merged_block_src), _dp(out.merged_block_author), _dp(out.merged_block_tok_off),
+        _dp(out.merged_origin), _dp(out.merged_traj), _dp(out.owner), _dp(out.counts), _dp(out.workspace),
+        C.c_size_t(out.workspace.numel()), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_merge_blocks")
     return out
 
 

@@ -62,18 +62,53 @@ def measure_merge(name: str, mi, dev, stream, reps: int, out, rules=(("longest",
     return fin
 
 
+def measure_blocks(name: str, bi, dev, stream, reps: int, out):
+    """ajt_merge_blocks (text-level matching) on a seeded block workload."""
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    ids, boff, traj, au, toff, tok, lp = (d(bi.block_ids), d(bi.block_offsets), d(bi.traj_ids), d(bi.author), d(bi.tok_off),
+                                          d(bi.tokens), d(bi.logp))
+    peak, _ = H.measured_peak()
+    with torch.cuda.stream(stream):
+        mo = ajt.merge_blocks(ids, boff, traj, au, toff, tok, lp, stream=stream)
+        stream.synchronize()
+    status = ajt.last_status(mo.workspace, stream)
+    assert status == 0, status
+    fin = mo.finalize()
+    B, N = int(bi.block_ids.shape[0]), int(bi.tokens.shape[0])
+    cold = 4 * N < L2_BYTES
+    flush = H.L2Flusher(dev) if cold else None
+    call = lambda: ajt.merge_blocks(ids, boff, traj, au, toff, tok, lp, out=mo, stream=stream)
+    med, best = _stats(H.time_calls(call, stream, reps=reps, flush=flush))
+    # algorithmic bytes: 9 B per input block (id, author) + 8 B of tok_off per block read; per OUTPUT token 4 (token) + 4 (logp)
+    # read and 4 + 4 + 4 + 1 written; absorbed timelines' tokens are never touched
+    b = 17 * B + 21 * fin.N_out + 25 * fin.B_out + 20 * bi.n
+    gbs = b / (med * 1e-3) / 1e9
+    _emit(out, stage="merge_blocks", config=name, n=bi.n, B_in=B, N_in=N, M=fin.M, B_out=fin.B_out, N_out=fin.N_out,
+          token_reduction_factor=N / max(1, fin.N_out), ms_median=med, ms_best=best,
+          merged_gtokens_per_s=fin.N_out / (med * 1e-3) / 1e9, algorithmic_bytes=b, gb_per_s=gbs, frac_of_measured=gbs / peak,
+          frac_of_nominal_8tbs=gbs / H.NOMINAL_HBM_GBS, l2="cold (256 MB flush between calls)" if cold else "output larger than L2",
+          reps=reps)
+    return fin
+
+
 def measure_loss(name: str, logits, targets, old, adv, mask, seg, S, eps, dev, stream, reps, out, seg_denom=None, inv=0.0,
-                 dlogits=None, extra=None):
+                 dlogits=None, extra=None, ext=False):
     T, V = logits.shape
     b_in = 2 if logits.dtype == torch.bfloat16 else 4
     if dlogits is None:
         dlogits = torch.empty((T, V), dtype=torch.bfloat16, device=dev)
     lo = None
 
+    ref = old + 0.01 if ext else None   # extended form (steps 8-9): KL against a reference policy + row entropy, same read
+
     def call():
         nonlocal lo
-        lo = ajt.policy_loss_fwd_bwd(logits, targets, old, adv, mask, seg, S, eps[0], eps[1], seg_denom=seg_denom, inv_num_segs=inv,
-                                     dlogits=dlogits, out=lo, stream=stream)
+        if ext:
+            lo = ajt.policy_loss_fwd_bwd_ext(logits, targets, old, adv, mask, seg, S, eps[0], eps[1], ref_logp=ref, kl_coef=2e-3,
+                                             seg_denom=seg_denom, inv_num_segs=inv, dlogits=dlogits, out=lo, stream=stream)
+        else:
+            lo = ajt.policy_loss_fwd_bwd(logits, targets, old, adv, mask, seg, S, eps[0], eps[1], seg_denom=seg_denom,
+                                         inv_num_segs=inv, dlogits=dlogits, out=lo, stream=stream)
 
     cold = T * V * b_in < L2_BYTES
     flush = H.L2Flusher(dev) if cold else None
@@ -84,7 +119,7 @@ def measure_loss(name: str, logits, targets, old, adv, mask, seg, S, eps, dev, s
     b = H.loss_bytes(T, V, nu, b_in)
     gbs = b / (med * 1e-3) / 1e9
     peak, _ = H.measured_peak()
-    kw = dict(stage="loss", config=name, T=T, V=V, S=S, dtype="bf16" if b_in == 2 else "f32", mask_density=nu / max(1, T),
+    kw = dict(stage="loss_ext" if ext else "loss", config=name, T=T, V=V, S=S, dtype="bf16" if b_in == 2 else "f32", mask_density=nu / max(1, T),
               ms_median=med, ms_best=best, algorithmic_bytes=b, logits_gb_per_s=gbs, frac_of_measured=gbs / peak,
               frac_of_nominal_8tbs=gbs / H.NOMINAL_HBM_GBS, dense_2TV_gb_per_s=2.0 * T * V * 2 / (med * 1e-3) / 1e9,
               loss=float(lo.loss.item()), l2="cold (256 MB flush between calls)" if cold else "input larger than L2", reps=reps)
@@ -153,6 +188,9 @@ def run_c5(dev, stream, reps, out, quick=False):
                     r = reps if T * V < (1 << 32) else max(5, reps // 2)
                     measure_loss("c5", logits, tg, old, d(lv.adv), d(lv.mask), d(lv.seg_ids), lv.S, (0.2, 0.28), dev, stream, r, out,
                                  dlogits=dlogits, extra=dict(rho=rho))
+                    if S == 64 and T == 65536:   # the extended form beside the plain call on the 64k-row cells
+                        measure_loss("c5", logits, tg, old, d(lv.adv), d(lv.mask), d(lv.seg_ids), lv.S, (0.2, 0.28), dev, stream,
+                                     r, out, dlogits=dlogits, extra=dict(rho=rho), ext=True)
                 cell += 1
             del logits, dlogits
             torch.cuda.empty_cache()
@@ -201,6 +239,8 @@ def main():
                 if not args.merge_only:
                     chunked_loss("c4" + model, fin, mi.meta["vocab"], (0.2, 0.2), W.BASE_SEED + 3, 3, "zscore", 65536, 4, dev, stream,
                                  max(5, args.reps // 2), out)
+        elif c in W.BLOCK_SPECS:
+            measure_blocks(c, W.block_workload(c), dev, stream, args.reps, out)
         elif c == "c5":
             if not args.merge_only:
                 run_c5(dev, stream, args.reps, out, quick=args.quick)
