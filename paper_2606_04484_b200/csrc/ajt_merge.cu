@@ -1257,9 +1257,51 @@ __device__ __forceinline__ bool scatter_tile_fast(const MergeParams& p, const Ti
     const int s = c.s, Ls = c.Ls;
     bool mismatch = false;
     const bool full = qbase >= 0 && qbase + kTile <= Ls;   // warp-uniform: every slot of the tile is a position of the sequence
+    const int32_t* __restrict__ tok = p.tokens + c.so;
+    // ---- uniform tile: every response region [rs_m, L_m) of a member (and the survivor's own) either covers the whole tile
+    // or misses it, and nobody needs verifying here: one source for the whole tile.  Regions are hundreds of tokens long, so
+    // most tiles are of this kind; they cost a plain copy instead of a per-element walk over the members.
+    if (!kExplicit && full && vec_ok) {
+        const int qhi = qbase + kTile;
+        bool covers = false, partial = false;
+        if (lane < cnt) {
+            const int Lm = ml.L[lane], rsm = ml.rs[lane];
+            covers = rsm <= qbase && Lm >= qhi;
+            partial = (!covers && Lm > qbase && rsm < qhi) || (ml.nv[lane] && Lm > qbase);
+        }
+        const bool s_covers = c.rs_s <= qbase;
+        if (!__any_sync(0xffffffffu, partial) && (s_covers || c.rs_s >= qhi)) {
+            const unsigned cb = __ballot_sync(0xffffffffu, covers);
+            const int sl = s_covers ? kSurv : (cb ? 32 - __clz(cb) : 0);
+            const int32_t sj = sl == 0 ? -1 : (sl == kSurv ? s : ml.j[sl - 1]);
+            const float* __restrict__ lps = p.old_logp_in + (sl == kSurv ? c.so : (sl ? ml.jo[sl - 1] : 0));
+            const bool want_lp = p.merged_old_logp != nullptr && sl != 0;
+            const bool tvec = (((uintptr_t)(tok + qbase)) & 15) == 0, lvec = want_lp && (((uintptr_t)(lps + qbase)) & 15) == 0;
+            int4 xv[kU];
+            float4 lv[kU];
+#pragma unroll
+            for (int u = 0; u < kU; ++u) {
+                const int q = ql + 128 * u;
+                if (tvec) xv[u] = __ldg(reinterpret_cast<const int4*>(tok + q));
+                else xv[u] = make_int4(__ldg(tok + q), __ldg(tok + q + 1), __ldg(tok + q + 2), __ldg(tok + q + 3));
+                lv[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (lvec) lv[u] = __ldg(reinterpret_cast<const float4*>(lps + q));
+                else if (want_lp) lv[u] = make_float4(__ldg(lps + q), __ldg(lps + q + 1), __ldg(lps + q + 2), __ldg(lps + q + 3));
+            }
+            const int64_t d0 = c.mo + ql;
+#pragma unroll
+            for (int u = 0; u < kU; ++u) {
+                const int64_t d = d0 + 128 * u;
+                *reinterpret_cast<int4*>(p.merged_tokens + d) = xv[u];
+                *reinterpret_cast<int4*>(p.merged_src + d) = make_int4(sj, sj, sj, sj);
+                *reinterpret_cast<uint32_t*>(p.merged_mask + d) = sl ? 0x01010101u : 0u;
+                if (p.merged_old_logp) *reinterpret_cast<float4*>(p.merged_old_logp + d) = lv[u];
+            }
+            return false;
+        }
+    }
     int32_t x[kU][4];
     int32_t slot[kU][4];
-    const int32_t* __restrict__ tok = p.tokens + c.so;
 #pragma unroll
     for (int u = 0; u < kU; ++u)
 #pragma unroll
