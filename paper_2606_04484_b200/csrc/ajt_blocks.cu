@@ -225,7 +225,24 @@ __global__ void __launch_bounds__(256) blocks_offsets_kernel(const BlockParams p
     }
 }
 
-// Gather: four consecutive output tokens per thread (16-byte stores where the output arrays allow it).
+// Gather: a warp takes a tile of 512 consecutive output tokens (4 steps of 32 lanes x 4 tokens, 16-byte stores where the
+// output arrays allow it).  The block that holds the tile's first token is found once per tile (a binary search whose loads
+// are warp-uniform); from there every lane walks forward over the block boundaries it meets (blocks are tens to thousands
+// of tokens long).  All of a step's loads are issued before its stores.
+constexpr int kCopyTile = 512;
+
+struct BlkCursor {   // the block a lane is in: where it ends, where its tokens come from, who supplied it
+    int64_t b, bend, delta;
+    int32_t sj;
+    bool llm;
+};
+__device__ __forceinline__ void cursor_load(const BlockParams& p, BlkCursor& c) {
+    c.bend = __ldg(p.merged_block_tok_off + c.b + 1);
+    c.delta = __ldg(p.tok_off + __ldg(p.blk_srcblk + c.b)) - __ldg(p.merged_block_tok_off + c.b);   // source = output + delta
+    c.sj = p.merged_block_src[c.b];
+    c.llm = p.merged_block_author[c.b] == kAuthorLlm;
+}
+
 __global__ void __launch_bounds__(256) blocks_copy_kernel(const BlockParams p) {
     int64_t M, Bout;
     merged_counts(p, M, Bout);
@@ -233,53 +250,80 @@ __global__ void __launch_bounds__(256) blocks_copy_kernel(const BlockParams p) {
     const int64_t Nout = p.merged_block_tok_off[Bout];
     const bool vec_ok = ((((uintptr_t)p.merged_tokens | (uintptr_t)p.merged_tok_src | (uintptr_t)p.merged_logp) & 15) == 0) &&
                         (((uintptr_t)p.merged_mask & 3) == 0);
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x * 4;
-    for (int64_t q0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4; q0 < Nout; q0 += stride) {
-        int64_t b = search_last_le(p.merged_block_tok_off, Bout, q0);
-        int64_t bend = __ldg(p.merged_block_tok_off + b + 1);
-        int64_t delta = __ldg(p.blk_srcblk + b);
-        int32_t sj = p.merged_block_src[b];
-        bool llm = p.merged_block_author[b] == kAuthorLlm;
-        delta = __ldg(p.tok_off + delta) - __ldg(p.merged_block_tok_off + b);   // source position = output position + delta
-        int32_t x[4], sr[4];
-        float lp[4];
-        uint32_t mk = 0;
+    const int lane = threadIdx.x & 31;
+    const int64_t wglobal = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    const int64_t ntiles = (Nout + kCopyTile - 1) / kCopyTile;
+    for (int64_t tile = wglobal; tile < ntiles; tile += nwarps) {
+        const int64_t t0 = tile * kCopyTile;
+        BlkCursor c;
+        c.b = search_last_le(p.merged_block_tok_off, Bout, t0);
+        cursor_load(p, c);
+#pragma unroll 2
+        for (int u = 0; u < kCopyTile / 128; ++u) {
+            const int64_t q0 = t0 + 128 * u + 4 * lane;
+            if (q0 >= Nout) break;
+            int32_t x[4], sr[4];
+            float lp[4];
+            uint32_t mk = 0;
+            if (q0 + 3 < c.bend) {   // the four tokens lie in the lane's current block (the usual case)
+                const int64_t sq = q0 + c.delta;
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const int64_t q = q0 + e;
-            x[e] = 0; sr[e] = -1; lp[e] = 0.f;
-            if (q < Nout) {
-                while (q >= bend) {   // next block (blocks may be empty)
-                    ++b;
-                    bend = __ldg(p.merged_block_tok_off + b + 1);
-                    sj = p.merged_block_src[b];
-                    llm = p.merged_block_author[b] == kAuthorLlm;
-                    delta = __ldg(p.tok_off + __ldg(p.blk_srcblk + b)) - __ldg(p.merged_block_tok_off + b);
+                for (int e = 0; e < 4; ++e) x[e] = __ldg(p.tokens + sq + e);
+                uint32_t m4 = c.llm ? 0x01010101u : 0u;
+                if (p.tok_mask) {
+                    m4 = 0;
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) m4 |= (__ldg(p.tok_mask + sq + e) != 0 ? 1u : 0u) << (8 * e);
                 }
-                const int64_t sq = q + delta;
-                x[e] = __ldg(p.tokens + sq);
-                const bool m = p.tok_mask ? (__ldg(p.tok_mask + sq) != 0) : llm;
-                if (m) {
-                    mk |= 1u << (8 * e);
-                    sr[e] = sj;
-                    if (p.logp) lp[e] = __ldg(p.logp + sq);
+                mk = m4;
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const bool m = (m4 >> (8 * e)) & 1u;
+                    sr[e] = m ? c.sj : -1;
+                    lp[e] = (m && p.logp) ? __ldg(p.logp + sq + e) : 0.f;
+                }
+            } else {
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int64_t q = q0 + e;
+                    x[e] = 0; sr[e] = -1; lp[e] = 0.f;
+                    if (q < Nout) {
+                        while (q >= c.bend) {   // next block (blocks may be empty)
+                            ++c.b;
+                            cursor_load(p, c);
+                        }
+                        const int64_t sq = q + c.delta;
+                        x[e] = __ldg(p.tokens + sq);
+                        const bool m = p.tok_mask ? (__ldg(p.tok_mask + sq) != 0) : c.llm;
+                        if (m) {
+                            mk |= 1u << (8 * e);
+                            sr[e] = c.sj;
+                            if (p.logp) lp[e] = __ldg(p.logp + sq);
+                        }
+                    }
                 }
             }
-        }
-        if (vec_ok && q0 + 3 < Nout) {
-            *reinterpret_cast<int4*>(p.merged_tokens + q0) = make_int4(x[0], x[1], x[2], x[3]);
-            *reinterpret_cast<int4*>(p.merged_tok_src + q0) = make_int4(sr[0], sr[1], sr[2], sr[3]);
-            *reinterpret_cast<uint32_t*>(p.merged_mask + q0) = mk;
-            if (p.merged_logp) *reinterpret_cast<float4*>(p.merged_logp + q0) = make_float4(lp[0], lp[1], lp[2], lp[3]);
-        } else {
+            if (vec_ok && q0 + 3 < Nout) {
+                *reinterpret_cast<int4*>(p.merged_tokens + q0) = make_int4(x[0], x[1], x[2], x[3]);
+                *reinterpret_cast<int4*>(p.merged_tok_src + q0) = make_int4(sr[0], sr[1], sr[2], sr[3]);
+                *reinterpret_cast<uint32_t*>(p.merged_mask + q0) = mk;
+                if (p.merged_logp) *reinterpret_cast<float4*>(p.merged_logp + q0) = make_float4(lp[0], lp[1], lp[2], lp[3]);
+            } else {
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                if (q0 + e < Nout) {
-                    p.merged_tokens[q0 + e] = x[e];
-                    p.merged_tok_src[q0 + e] = sr[e];
-                    p.merged_mask[q0 + e] = (uint8_t)((mk >> (8 * e)) & 1u);
-                    if (p.merged_logp) p.merged_logp[q0 + e] = lp[e];
+                for (int e = 0; e < 4; ++e) {
+                    if (q0 + e < Nout) {
+                        p.merged_tokens[q0 + e] = x[e];
+                        p.merged_tok_src[q0 + e] = sr[e];
+                        p.merged_mask[q0 + e] = (uint8_t)((mk >> (8 * e)) & 1u);
+                        if (p.merged_logp) p.merged_logp[q0 + e] = lp[e];
+                    }
                 }
+            }
+            // the lane's next step starts 128 tokens further: catch up with the blocks in between
+            const int64_t qn = q0 + 128;
+            while (qn < Nout && qn >= c.bend) {
+                ++c.b;
+                cursor_load(p, c);
             }
         }
     }
@@ -350,7 +394,7 @@ extern "C" int ajt_merge_blocks(const int64_t* block_ids, const int64_t* block_o
     blocks_info_kernel<<<grid_b, 256, 0, stream>>>(p);
     blocks_scan_kernel<<<max(1, min(ntiles, num_sms)), 256, 0, stream>>>(p);
     blocks_offsets_kernel<<<max(1, min((n + 256) / 256, num_sms)), 256, 0, stream>>>(p);
-    const int64_t wantc = (n_tokens + 1023) / 1024 + 1;
-    blocks_copy_kernel<<<(int)(wantc < (int64_t)num_sms * 16 ? wantc : (int64_t)num_sms * 16), 256, 0, stream>>>(p);
+    const int64_t wantc = (n_tokens + 8 * kCopyTile - 1) / (8 * kCopyTile) + 1;   // 8 warps per CTA, one tile per warp and turn
+    blocks_copy_kernel<<<(int)(wantc < (int64_t)num_sms * 8 ? wantc : (int64_t)num_sms * 8), 256, 0, stream>>>(p);
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }
