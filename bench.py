@@ -269,6 +269,23 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                         seg=d(seg[sl].copy()), n_unmasked=int(mask[sl].sum())))
     dlogits = torch.empty((T, V), dtype=torch.bfloat16, device=dev)
     lout = None
+    # The stages are chained on the device: the merge's outputs feed ajt_pack_loss_inputs (next-token alignment, segment ids,
+    # advantages: reading L-12), ajt_segment_counts gives the batch-wide N_s (reading L-4), and the loss call reads the
+    # micro-batch's rows of those arrays.  Nothing goes through the host inside a step.  (`old` was synthesised in the set-up
+    # from the same targets: input synthesis, BASELINE.json configs.)
+    uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
+    assert int(uniq.shape[0]) == S
+    tl_seg_d = d(tl_seg.astype(np.int32))
+    seg_adv_d = d(W.advantages_group_zscore(seed, 1, S).astype(np.float32))
+    with torch.cuda.stream(stream):
+        pk = ajt.pack_loss_inputs(mout, tl_seg_d, S, seg_adv_d, stream=stream)
+        stream.synchronize()
+    for k in range(n_mb):       # the device chain reproduces the set-up's host arrays bit for bit
+        sl = slice(k * T, (k + 1) * T)
+        assert torch.equal(pk.targets[sl], mbs[k]["targets"]) and torch.equal(pk.mask[sl], mbs[k]["mask"])
+        assert torch.equal(pk.seg_ids[sl], mbs[k]["seg"]) and torch.equal(pk.adv[sl], mbs[k]["adv"])
+        mbs[k].update(targets=pk.targets[sl], mask=pk.mask[sl], seg=pk.seg_ids[sl], adv=pk.adv[sl])
+    pk_mask_all, pk_seg_all = pk.mask[:N_out], pk.seg_ids[:N_out]
 
     def step(k: int, ev=None):
         nonlocal lout
@@ -278,6 +295,10 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         ajt.merge_timelines(tokens, offsets, traj, rs, None, lp, owner_rule=ajt.OWNER_LONGEST, out=mout, stream=stream)
         if ev:
             ev[1].record(stream)
+        ajt.pack_loss_inputs(mout, tl_seg_d, S, seg_adv_d, out=pk, stream=stream)
+        ajt.segment_counts(pk_mask_all, pk_seg_all, S, out=Ns_d, stream=stream)
+        if ev:
+            ev[3].record(stream)
         lout = ajt.policy_loss_fwd_bwd(mb["logits"], mb["targets"], mb["old"], mb["adv"], mb["mask"], mb["seg"], S, EPS[0],
                                        EPS[1], seg_denom=Ns_d, inv_num_segs=inv, dlogits=dlogits, out=lout, stream=stream)
         if ev:
@@ -310,7 +331,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         sampler = ClockSampler(local_rank)
         sampler.start()
         time.sleep(0.3)
-        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         tw0 = time.time()
@@ -322,7 +343,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         tw1 = time.time()
     total_ms = max_over_ranks(e0.elapsed_time(e1))
     merge_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
-    loss_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    bridge_ms = float(np.mean([e[1].elapsed_time(e[3]) for e in evs]))
+    loss_ms = float(np.mean([e[3].elapsed_time(e[2]) for e in evs]))
     assert ajt.last_status(mout.workspace) == 0 and ajt.last_status(lout.workspace) == 0
     clocks = sampler.summary(tw0, tw1)
 
@@ -366,13 +388,15 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                       "input_gtokens_per_s": N_in / (merge_ms * 1e-3) / 1e9, "gb_per_s": mg, "frac_of_measured": mg / peak,
                       "frac_of_nominal_8tbs": mg / NOMINAL_HBM_GBS, "token_reduction_factor": N_in / N_out, "M": M,
                       "algorithmic_bytes": b_merge},
+            "bridge": {"ms": bridge_ms, "what": "ajt_pack_loss_inputs over the N_out merged tokens + ajt_segment_counts "
+                       "(device-resident chain between the stages; its bytes are not counted in `value`)"},
             "loss": {"ms": loss_ms, "logits_gb_per_s": ach, "frac_of_measured": ach / peak,
                      "frac_of_nominal_8tbs": ach / NOMINAL_HBM_GBS, "algorithmic_bytes": loss_b,
                      "dense_2TV_gb_per_s": 4.0 * T * V / (loss_ms * 1e-3) / 1e9},
             "roofline": {"bound": "hbm", "kernel": "loss_rows_kernel (timed as the ajt_policy_loss_fwd_bwd call: prep + rows + "
                          "final launches; rows is >99% of it, profiles/)", "achieved": ach, "peak": peak, "unit": "GB/s",
                          "frac": ach / peak, "traffic": traffic, "peak_source": peak_src},
-            "clocks": clocks, "gpu_launches": K * (9 + 3),
+            "clocks": clocks, "gpu_launches": K * (6 + 1 + 1 + 3),   # merge 6, pack 1, segment counts 1, loss 3 (prep, rows, final)
             "e2e": e2e, "cpu_baseline": cpu_baseline,
             "paper_context": "paper reports only end-to-end actor-update 2160 s -> 346 s (6.25x) with merging on AppWorld, "
                              "8-GPU node at most, GPU model and precision not stated (PAPER.md:373,395); not comparable",

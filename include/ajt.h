@@ -176,6 +176,25 @@ int ajt_merge_timelines_host(
     void* arena /* DEVICE */, size_t arena_bytes, ajt_stream_t stream);
 
 /* ------------------------------------------------------------------------------------------------
+ * Bridge (a) -> (b): per-token loss inputs from the merge outputs, on the device ("the packed merged sequences",
+ * BASELINE.json north_star; reading L-12).  For position q of merged sequence m:
+ *   targets[q] = merged_tokens[q+1], mask[q] = merged_mask[q+1], old_logp[q] = merged_old_logp[q+1]
+ *   (next-token alignment inside the sequence); at the LAST position of every sequence all three are 0
+ *   seg_ids[q] = tl_seg[merged_origin[m]];   adv[q] = seg_adv[seg_ids[q]]
+ * tl_seg [n]: caller's dense trajectory id in [0,S) of every ORIGINAL timeline (the traj_ids renumbered on the host);
+ * seg_adv [S]: one advantage per trajectory (GRPO).  counts = the merge call's {M, N_out} (DEVICE): nothing is
+ * read back to the host between the merge, this call and the loss.  Only the first N_out entries of the outputs are
+ * written; a micro-batch is then any row range of them (rows are independent given ajt_segment_counts, reading L-4).
+ * merged_old_logp / old_logp and seg_adv / adv may be NULL in pairs.  status_bits DEVICE [1] or NULL: AJT_STATUS_BAD_SEG
+ * when a tl_seg value is outside [0,S) (segment 0 is used).  All pointers DEVICE; enqueues on `stream`. */
+int ajt_pack_loss_inputs(
+    const int32_t* merged_tokens, const uint8_t* merged_mask, const float* merged_old_logp, const int64_t* merged_offsets,
+    const int32_t* merged_origin, const int32_t* tl_seg, const float* seg_adv, const int64_t* counts,
+    int64_t capacity_tokens /* size of the token arrays (>= N_out) */, int32_t S,
+    int32_t* targets, uint8_t* mask, float* old_logp, int32_t* seg_ids, float* adv,
+    uint32_t* status_bits, ajt_stream_t stream);
+
+/* ------------------------------------------------------------------------------------------------
  * Stage (b): token-level clipped policy-gradient loss, forward and backward w.r.t. the logits.
  * Definition, for t in [0,T):
  *   lse_t = log sum_v exp(z_tv);  logp_t = z_{t,y_t} - lse_t;  r_t = exp(logp_t - old_logp_t)

@@ -33,6 +33,7 @@ from .binding import (  # noqa: F401
     merge_timelines,
     merge_timelines_host,
     merge_workspace_bytes,
+    pack_loss_inputs,
     policy_loss_fwd_bwd,
     policy_loss_fwd_bwd_ext,
     policy_loss_fwd_bwd_host,

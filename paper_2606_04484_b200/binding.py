@@ -26,6 +26,7 @@ _EXPORTS = [
     "ajt_merge_workspace_bytes", "ajt_merge_timelines", "ajt_merge_host_arena_bytes", "ajt_merge_timelines_host",
     "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
     "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks_workspace_bytes", "ajt_merge_blocks",
+    "ajt_pack_loss_inputs",
 ]
 
 _lib = None
@@ -67,7 +68,8 @@ def lib():
         L.ajt_loss_host_arena_bytes.restype = C.c_size_t
         L.ajt_loss_host_arena_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32]
         for f in ("ajt_merge_timelines", "ajt_merge_timelines_host", "ajt_policy_loss_fwd_bwd",
-                  "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks"):
+                  "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks",
+                  "ajt_pack_loss_inputs"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -267,6 +269,45 @@ def merge_blocks(block_ids: torch.Tensor, block_offsets: torch.Tensor, traj_ids:
         C.c_size_t(out.workspace.numel()), _stream(stream))
     if rc != 0:
         raise AjtError(rc, "ajt_merge_blocks")
+    return out
+
+
+@dataclass
+class PackedLossInputs:
+    """Device tensors at the capacity of the merge outputs; the first N_out entries are defined."""
+    targets: torch.Tensor
+    mask: torch.Tensor
+    old_logp: Optional[torch.Tensor]
+    seg_ids: torch.Tensor
+    adv: Optional[torch.Tensor]
+    status: torch.Tensor
+
+
+def pack_loss_inputs(mo, tl_seg: torch.Tensor, S: int, seg_adv: Optional[torch.Tensor] = None,
+                     out: Optional[PackedLossInputs] = None, stream=None) -> PackedLossInputs:
+    """ajt_pack_loss_inputs (include/ajt.h).  `mo`: an un-finalized MergeOutput / BlockMergeOutput (capacity-sized tensors and
+    the device `counts`); nothing is read back to the host."""
+    _require_cuda()
+    _check_dev(tl_seg, torch.int32, "tl_seg")
+    _check_dev(seg_adv, torch.float32, "seg_adv")
+    logp = getattr(mo, "merged_old_logp", None) if hasattr(mo, "merged_old_logp") else getattr(mo, "merged_logp", None)
+    counts = mo.counts
+    if counts.numel() == 3:       # block-level merge: {M, B_out, N_out}
+        counts = torch.stack((counts[0], counts[2]))
+    cap = int(mo.merged_tokens.numel())
+    dev = mo.merged_tokens.device
+    if out is None:
+        out = PackedLossInputs(torch.empty(cap, dtype=torch.int32, device=dev), torch.empty(cap, dtype=torch.uint8, device=dev),
+                               None if logp is None else torch.empty(cap, dtype=torch.float32, device=dev),
+                               torch.empty(cap, dtype=torch.int32, device=dev),
+                               None if seg_adv is None else torch.empty(cap, dtype=torch.float32, device=dev),
+                               torch.empty(1, dtype=torch.int32, device=dev))
+    rc = lib().ajt_pack_loss_inputs(_dp(mo.merged_tokens), _dp(mo.merged_mask), _dp(logp), _dp(mo.merged_offsets),
+                                    _dp(mo.merged_origin), _dp(tl_seg), _dp(seg_adv), _dp(counts), C.c_int64(cap), C.c_int32(S),
+                                    _dp(out.targets), _dp(out.mask), _dp(out.old_logp), _dp(out.seg_ids), _dp(out.adv),
+                                    _dp(out.status), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_pack_loss_inputs")
     return out
 
 

@@ -196,6 +196,31 @@ def run_c5(dev, stream, reps, out, quick=False):
             torch.cuda.empty_cache()
 
 
+def stock_bandwidth(dev, out):
+    """Context for the rooflines: what stock library kernels (torch fill_ / copy_, cudaMemset) reach on this box when they move
+    the bytes of the loss step (12.9 GB arrays; the bench micro-batch reads 27 % of the rows and writes all of them)."""
+    n = 6 * (1 << 30)
+    a = torch.empty(n, dtype=torch.bfloat16, device=dev)
+    b = torch.empty(n, dtype=torch.bfloat16, device=dev)
+    k = int(n * 0.27)
+
+    def run(f, name, nbytes):
+        ts = []
+        for _ in range(6):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); f(); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        t = float(np.min(ts))
+        _emit(out, stage="stock_bandwidth", what=name, ms_best=t, bytes=nbytes, gb_per_s=nbytes / t / 1e6)
+
+    run(lambda: a.zero_(), "zero_ 12.9 GB (write only)", 2 * n)
+    run(lambda: a.fill_(1.0), "fill_ 12.9 GB (write only)", 2 * n)
+    run(lambda: b.copy_(a), "copy_ 12.9 GB -> 12.9 GB (read + write)", 4 * n)
+    run(lambda: (b[:k].copy_(a[:k]), b[k:].fill_(0.0)), "27 % copied + 73 % filled: the bench step's read / write mix, 2 kernels",
+        4 * k + 2 * (n - k))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", default="c1,c2,c3,c4,c5")
@@ -204,6 +229,7 @@ def main():
     ap.add_argument("--merge-only", action="store_true")
     ap.add_argument("--quick", action="store_true", help="c5: 2x2 cells instead of 4x3")
     ap.add_argument("--both-rules", action="store_true")
+    ap.add_argument("--stock-bandwidth", action="store_true", help="time torch fill_ / copy_ on 12.9 GB arrays and exit")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("sweep: no CUDA device; the hot path has no CPU fallback")
@@ -212,6 +238,9 @@ def main():
     torch.cuda.set_device(dev)
     stream = torch.cuda.Stream(dev)
     out = open(args.out, "a") if args.out else None
+    if args.stock_bandwidth:
+        stock_bandwidth(dev, out)
+        return
     rules = (("longest", ajt.OWNER_LONGEST), ("paper", ajt.OWNER_PAPER)) if args.both_rules else (("longest", ajt.OWNER_LONGEST),)
     cfgs = [c.strip() for c in args.configs.split(",") if c.strip()]
     t0 = time.time()

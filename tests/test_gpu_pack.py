@@ -1,0 +1,93 @@
+"""GPU parity: ajt_pack_loss_inputs (merge outputs -> per-token loss inputs on the device) vs oracle.pack_loss_inputs, bit-exact;
+and the whole device-resident chain merge -> pack -> segment counts -> loss against the oracle chain."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2606_04484_b200 as ajt
+from paper_2606_04484_b200 import workloads as W
+from helpers import check_loss, harness_old_logp
+
+pytestmark = pytest.mark.gpu
+
+
+def device_merge(mi, rule=ajt.OWNER_LONGEST):
+    d = lambda a: torch.from_numpy(a).cuda()
+    return ajt.merge_timelines(d(mi.tokens), d(mi.offsets), d(mi.traj_ids), d(mi.resp_start), None, d(mi.old_logp), owner_rule=rule)
+
+
+@pytest.mark.parametrize("config,n_traj", [("c1", None), ("c2", None), ("c3", 12)])
+def test_pack_matches_oracle(config, n_traj):
+    mi = W.merge_workload(config, n_traj=n_traj)
+    uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
+    S = int(uniq.shape[0])
+    adv = W.advantages_group_zscore(W.BASE_SEED, 1, S)
+    mo = device_merge(mi)                                     # not finalized: counts stay on the device
+    pk = ajt.pack_loss_inputs(mo, torch.from_numpy(tl_seg.astype(np.int32)).cuda(), S, torch.from_numpy(adv).cuda())
+    torch.cuda.synchronize()
+    assert int(pk.status[0]) == 0
+    r = oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp)
+    t, m, o, s, a = oracle.pack_loss_inputs(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets, r.merged_origin,
+                                            tl_seg.astype(np.int32), adv)
+    N = r.N_out
+    assert np.array_equal(pk.targets[:N].cpu().numpy(), t) and np.array_equal(pk.mask[:N].cpu().numpy(), m)
+    assert np.array_equal(pk.old_logp[:N].cpu().numpy().view(np.uint32), o.view(np.uint32))
+    assert np.array_equal(pk.seg_ids[:N].cpu().numpy(), s) and np.array_equal(pk.adv[:N].cpu().numpy().view(np.uint32), a.view(np.uint32))
+
+
+def test_pack_without_optional_arrays_and_bad_segment():
+    mi = W.merge_workload("c1")
+    d = lambda a: torch.from_numpy(a).cuda()
+    mo = ajt.merge_timelines(d(mi.tokens), d(mi.offsets), d(mi.traj_ids), d(mi.resp_start))
+    uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
+    pk = ajt.pack_loss_inputs(mo, d(tl_seg.astype(np.int32)), int(uniq.shape[0]))
+    torch.cuda.synchronize()
+    assert pk.old_logp is None and pk.adv is None and int(pk.status[0]) == 0
+    bad = tl_seg.astype(np.int32).copy()
+    bad[:] = 99999
+    pk = ajt.pack_loss_inputs(mo, d(bad), int(uniq.shape[0]))
+    torch.cuda.synchronize()
+    assert int(pk.status[0]) & ajt.STATUS_BAD_SEG
+
+
+def test_pack_after_block_merge():
+    bi = W.block_workload("b1")
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    mo = ajt.merge_blocks(d(bi.block_ids), d(bi.block_offsets), d(bi.traj_ids), d(bi.author), d(bi.tok_off), d(bi.tokens), d(bi.logp))
+    uniq, tl_seg = np.unique(bi.traj_ids, return_inverse=True)
+    pk = ajt.pack_loss_inputs(mo, d(tl_seg.astype(np.int32)), int(uniq.shape[0]))
+    torch.cuda.synchronize()
+    r = oracle.merge_blocks(bi.block_ids, bi.block_offsets, bi.traj_ids, bi.author, bi.tok_off, bi.tokens, bi.logp)
+    t, m, o, s, _ = oracle.pack_loss_inputs(r.merged_tokens, r.merged_mask, r.merged_logp, r.merged_offsets, r.merged_origin,
+                                            tl_seg.astype(np.int32))
+    N = r.N_out
+    assert np.array_equal(pk.targets[:N].cpu().numpy(), t) and np.array_equal(pk.mask[:N].cpu().numpy(), m)
+    assert np.array_equal(pk.old_logp[:N].cpu().numpy().view(np.uint32), o.view(np.uint32))
+    assert np.array_equal(pk.seg_ids[:N].cpu().numpy(), s)
+
+
+def test_device_resident_chain_c1():
+    """configs[0] end to end with no host round trip between the stages: merge -> pack -> segment counts -> loss."""
+    mi = W.merge_workload("c1")
+    uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
+    S = int(uniq.shape[0])
+    advt = W.advantages_pm1(W.BASE_SEED, 0, S)
+    mo = device_merge(mi)
+    pk = ajt.pack_loss_inputs(mo, torch.from_numpy(tl_seg.astype(np.int32)).cuda(), S, torch.from_numpy(advt).cuda())
+    N = int(mo.counts.cpu()[1])              # only to size the synthetic logits of this test
+    V = 1024
+    g = torch.Generator(device="cuda").manual_seed(W.BASE_SEED)
+    logits = torch.randn((N, V), generator=g, device="cuda") * 2.0
+    noise = (W.rng_for(W.BASE_SEED, 0, 99).standard_normal(N) * 0.05).astype(np.float32)
+    old = harness_old_logp(logits, pk.targets[:N], noise)
+    Ns = ajt.segment_counts(pk.mask[:N], pk.seg_ids[:N], S)
+    out = ajt.policy_loss_fwd_bwd(logits, pk.targets[:N], old, pk.adv[:N], pk.mask[:N], pk.seg_ids[:N], S, 0.2, 0.2, seg_denom=Ns,
+                                  want_logp=True, want_stats=True)
+    torch.cuda.synchronize()
+    # oracle chain
+    r = oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp)
+    t, m, _, s, a = oracle.pack_loss_inputs(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets, r.merged_origin,
+                                            tl_seg.astype(np.int32), advt)
+    ref = oracle.policy_loss(logits.cpu().numpy(), t, old.cpu().numpy(), a, m, s, S, float(np.float32(0.2)), float(np.float32(0.2)))
+    check_loss(out, ref, m, 0.2, 0.2, a, old.cpu().numpy(), 1.0, V)
