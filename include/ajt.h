@@ -268,8 +268,12 @@ int ajt_policy_loss_fwd_bwd_ext(
 int ajt_segment_counts(const uint8_t* mask /* DEVICE [T] */, const int32_t* seg_ids /* DEVICE [T] */, int64_t T, int32_t S,
                        int32_t accumulate, float* seg_denom, uint32_t* status_bits, ajt_stream_t stream);
 
-/* HOST-buffer variant.  `arena` is DEVICE scratch of at least ajt_loss_host_arena_bytes(T, V, S, ld, dtype)
- * bytes.  Rows are staged in slabs so that H2D, compute and D2H overlap.  Synchronises. */
+/* HOST-buffer variant.  `arena` is DEVICE scratch of at least ajt_loss_host_arena_bytes(T, V, S, ld, dtype) bytes.
+ * The per-token vectors go up first and the batch-wide normalisers are counted on the device; the matrix is cut into up
+ * to 16 row slabs whose H2D copy, loss call and D2H copy overlap with their neighbours' (both PCIe directions busy at
+ * once).  For that the call creates two helper streams and their events and destroys them before it returns: the only
+ * resources the library ever creates.  dlogits / logp rows are those of the device call; loss and stats[3] are the fp64
+ * sums of the slabs' fp32 partials.  Pinned host buffers are needed for the overlap.  Synchronises. */
 size_t ajt_loss_host_arena_bytes(int64_t T, int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype);
 
 int ajt_policy_loss_fwd_bwd_host(

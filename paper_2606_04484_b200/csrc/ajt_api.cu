@@ -62,6 +62,25 @@ extern "C" size_t ajt_loss_host_arena_bytes(int64_t T, int32_t V, int32_t S, int
     return loss_arena(T, V, S, ld, dtype).total;
 }
 
+namespace {
+// Per-slab partials -> running totals kept on the device in fp64 (no host read between slabs).
+__global__ void host_acc_kernel(double* acc /* [5]: loss, stats[4] */, uint32_t* status_acc, const float* loss, const float* stats,
+                                const uint32_t* ws_status) {
+    acc[0] += (double)loss[0];
+    if (stats)
+        for (int k = 0; k < 4; ++k) acc[1 + k] += (double)stats[k];
+    *status_acc |= *ws_status;
+}
+__global__ void host_fin_kernel(const double* acc, float* loss, float* stats) {
+    loss[0] = (float)acc[0];
+    for (int k = 0; k < 4; ++k) stats[k] = (float)acc[1 + k];
+}
+constexpr int kHostMaxSlabs = 16;
+}  // namespace
+
+// Slab pipeline: the per-token vectors go up first and the batch-wide normalisers are counted on the device (reading L-4);
+// the [T, ld] matrix is cut into up to 16 row slabs, and slab i's H2D copy (helper stream 1), its loss call (the caller's
+// stream) and its D2H copy (helper stream 2) overlap with the neighbours', so both PCIe directions stay busy at once.
 extern "C" int ajt_policy_loss_fwd_bwd_host(const void* logits, const int32_t* targets, const float* old_logp, const float* adv,
                                             const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T,
                                             int32_t V, int32_t S, int64_t ld, int32_t dtype, const float* seg_denom,
@@ -71,35 +90,100 @@ extern "C" int ajt_policy_loss_fwd_bwd_host(const void* logits, const int32_t* t
     cudaStream_t s = reinterpret_cast<cudaStream_t>(stream_);
     if (T < 0 || V <= 0 || S <= 0 || ld < V || !arena || !loss_out) return AJT_ERR_INVALID_ARG;
     if (dtype != AJT_DT_BF16 && dtype != AJT_DT_F32) return AJT_ERR_INVALID_ARG;
+    if (T > 0 && (!logits || !targets || !old_logp || !adv || !mask || !seg_ids || !dlogits)) return AJT_ERR_INVALID_ARG;
     if ((uintptr_t)arena & 255) return AJT_ERR_INVALID_ARG;
     const LossArena a = loss_arena(T, V, S, ld, dtype);
     if (arena_bytes < a.total) return AJT_ERR_WORKSPACE_TOO_SMALL;
     uint8_t* d = reinterpret_cast<uint8_t*>(arena);
     const size_t esz = dtype == AJT_DT_F32 ? 4 : 2;
-    void* d_dlogits = dtype == AJT_DT_F32 ? (void*)(d + a.ws + ajt_loss_workspace_bytes(T, V, S)) : (void*)(d + a.logits);
-#define AJT_CP(dst, src, bytes, kind) \
-    if ((bytes) > 0 && cudaMemcpyAsync((dst), (src), (bytes), (kind), s) != cudaSuccess) return AJT_ERR_CUDA
-    AJT_CP(d + a.logits, logits, (size_t)T * ld * esz, cudaMemcpyHostToDevice);
-    AJT_CP(d + a.targets, targets, (size_t)T * 4, cudaMemcpyHostToDevice);
-    AJT_CP(d + a.old_logp, old_logp, (size_t)T * 4, cudaMemcpyHostToDevice);
-    AJT_CP(d + a.adv, adv, (size_t)T * 4, cudaMemcpyHostToDevice);
-    AJT_CP(d + a.mask, mask, (size_t)T, cudaMemcpyHostToDevice);
-    AJT_CP(d + a.seg, seg_ids, (size_t)T * 4, cudaMemcpyHostToDevice);
-    if (seg_denom) AJT_CP(d + a.denom, seg_denom, (size_t)S * 4, cudaMemcpyHostToDevice);
-    const int rc = ajt_policy_loss_fwd_bwd(d + a.logits, (const int32_t*)(d + a.targets), (const float*)(d + a.old_logp),
-                                           (const float*)(d + a.adv), d + a.mask, (const int32_t*)(d + a.seg), eps_lo, eps_hi, T,
-                                           V, S, ld, dtype, seg_denom ? (const float*)(d + a.denom) : nullptr, inv_num_segs,
-                                           grad_scale, d_dlogits, (float*)(d + a.loss), logp_out ? (float*)(d + a.logp) : nullptr,
-                                           stats_out ? (float*)(d + a.stats) : nullptr, d + a.ws,
-                                           ajt_loss_workspace_bytes(T, V, S), stream_);
-    if (rc != AJT_OK) return rc;
-    AJT_CP(dlogits, d_dlogits, (size_t)T * ld * 2, cudaMemcpyDeviceToHost);
-    AJT_CP(loss_out, d + a.loss, 4, cudaMemcpyDeviceToHost);
-    if (logp_out) AJT_CP(logp_out, d + a.logp, (size_t)T * 4, cudaMemcpyDeviceToHost);
-    if (stats_out) AJT_CP(stats_out, d + a.stats, 16, cudaMemcpyDeviceToHost);
-    if (status_bits) AJT_CP(status_bits, d + a.ws, 4, cudaMemcpyDeviceToHost);
+    const size_t ws_bytes = ajt_loss_workspace_bytes(T, V, S);
+    uint8_t* d_dl = dtype == AJT_DT_F32 ? d + a.ws + ws_bytes : d + a.logits;   // bf16: in place
+    // accumulators live in the tail of the stats slot: [loss f32 | ... ] at a.loss, [stats 4 x f32 | acc 5 x f64 | status u32] at a.stats
+    float* d_loss = reinterpret_cast<float*>(d + a.loss);
+    float* d_stats = reinterpret_cast<float*>(d + a.stats);
+    double* d_acc = reinterpret_cast<double*>(d + a.stats + 64);
+    uint32_t* d_status = reinterpret_cast<uint32_t*>(d + a.stats + 128);
+    float* d_denom = reinterpret_cast<float*>(d + a.denom);
+
+    int rc = AJT_OK;
+    cudaStream_t s_up = nullptr, s_dn = nullptr;
+    cudaEvent_t ev_up[kHostMaxSlabs] = {}, ev_k[kHostMaxSlabs] = {}, ev0 = nullptr, ev_end = nullptr;
+    const int nslab = (int)(T <= 0 ? 0 : (T < 256 * kHostMaxSlabs ? (T + 255) / 256 : kHostMaxSlabs));
+    const int64_t rows_per = nslab ? (T + nslab - 1) / nslab : 0;
+#define AJT_TRY(x) \
+    do { \
+        if (rc == AJT_OK && (x) != cudaSuccess) rc = AJT_ERR_CUDA; \
+    } while (0)
+#define AJT_CP(dst, src, bytes, kind, st) \
+    do { \
+        if ((bytes) > 0) AJT_TRY(cudaMemcpyAsync((dst), (src), (bytes), (kind), (st))); \
+    } while (0)
+    AJT_TRY(cudaStreamCreateWithFlags(&s_up, cudaStreamNonBlocking));
+    AJT_TRY(cudaStreamCreateWithFlags(&s_dn, cudaStreamNonBlocking));
+    AJT_TRY(cudaEventCreateWithFlags(&ev0, cudaEventDisableTiming));
+    AJT_TRY(cudaEventCreateWithFlags(&ev_end, cudaEventDisableTiming));
+    for (int i = 0; i < nslab; ++i) {
+        AJT_TRY(cudaEventCreateWithFlags(&ev_up[i], cudaEventDisableTiming));
+        AJT_TRY(cudaEventCreateWithFlags(&ev_k[i], cudaEventDisableTiming));
+    }
+    // ---- per-token vectors, normalisers, accumulators (caller's stream)
+    AJT_CP(d + a.targets, targets, (size_t)T * 4, cudaMemcpyHostToDevice, s);
+    AJT_CP(d + a.old_logp, old_logp, (size_t)T * 4, cudaMemcpyHostToDevice, s);
+    AJT_CP(d + a.adv, adv, (size_t)T * 4, cudaMemcpyHostToDevice, s);
+    AJT_CP(d + a.mask, mask, (size_t)T, cudaMemcpyHostToDevice, s);
+    AJT_CP(d + a.seg, seg_ids, (size_t)T * 4, cudaMemcpyHostToDevice, s);
+    AJT_TRY(cudaMemsetAsync(d + a.stats, 0, 256, s));
+    AJT_TRY(cudaMemsetAsync(d + a.loss, 0, 256, s));
+    if (rc == AJT_OK) {
+        if (seg_denom) AJT_CP(d_denom, seg_denom, (size_t)S * 4, cudaMemcpyHostToDevice, s);
+        else rc = ajt_segment_counts(d + a.mask, (const int32_t*)(d + a.seg), T, S, 0, d_denom, d_status, stream_);
+    }
+    AJT_TRY(cudaEventRecord(ev0, s));
+    AJT_TRY(cudaStreamWaitEvent(s_up, ev0, 0));   // the uploads start after whatever the caller had queued on its stream
+    // ---- slabs
+    for (int i = 0; i < nslab && rc == AJT_OK; ++i) {
+        const int64_t r0 = i * rows_per, r1 = (r0 + rows_per < T) ? r0 + rows_per : T;
+        if (r1 <= r0) break;
+        const int64_t R = r1 - r0;
+        AJT_CP(d + a.logits + (size_t)r0 * ld * esz, (const uint8_t*)logits + (size_t)r0 * ld * esz, (size_t)R * ld * esz,
+               cudaMemcpyHostToDevice, s_up);
+        AJT_TRY(cudaEventRecord(ev_up[i], s_up));
+        AJT_TRY(cudaStreamWaitEvent(s, ev_up[i], 0));
+        if (rc != AJT_OK) break;
+        rc = ajt_policy_loss_fwd_bwd(d + a.logits + (size_t)r0 * ld * esz, (const int32_t*)(d + a.targets) + r0,
+                                     (const float*)(d + a.old_logp) + r0, (const float*)(d + a.adv) + r0, d + a.mask + r0,
+                                     (const int32_t*)(d + a.seg) + r0, eps_lo, eps_hi, R, V, S, ld, dtype, d_denom, inv_num_segs,
+                                     grad_scale, d_dl + (size_t)r0 * ld * 2, d_loss, logp_out ? (float*)(d + a.logp) + r0 : nullptr,
+                                     stats_out ? d_stats : nullptr, d + a.ws, ws_bytes, stream_);
+        if (rc != AJT_OK) break;
+        host_acc_kernel<<<1, 1, 0, s>>>(d_acc, d_status, d_loss, stats_out ? d_stats : nullptr, (const uint32_t*)(d + a.ws));
+        AJT_TRY(cudaEventRecord(ev_k[i], s));
+        AJT_TRY(cudaStreamWaitEvent(s_dn, ev_k[i], 0));
+        AJT_CP((uint8_t*)dlogits + (size_t)r0 * ld * 2, d_dl + (size_t)r0 * ld * 2, (size_t)R * ld * 2, cudaMemcpyDeviceToHost, s_dn);
+    }
+    if (rc == AJT_OK) {
+        host_fin_kernel<<<1, 1, 0, s>>>(d_acc, d_loss, d_stats);
+        AJT_CP(loss_out, d_loss, 4, cudaMemcpyDeviceToHost, s);
+        if (logp_out) AJT_CP(logp_out, d + a.logp, (size_t)T * 4, cudaMemcpyDeviceToHost, s);
+        if (stats_out) AJT_CP(stats_out, d_stats, 16, cudaMemcpyDeviceToHost, s);
+        if (status_bits) AJT_CP(status_bits, d_status, 4, cudaMemcpyDeviceToHost, s);
+    }
+    // ---- join and clean up (also on the error paths: nothing may still be running on the helper streams)
+    if (s_dn && ev_end && cudaEventRecord(ev_end, s_dn) == cudaSuccess) cudaStreamWaitEvent(s, ev_end, 0);
+    if (s_up) cudaStreamSynchronize(s_up);
+    if (s_dn) cudaStreamSynchronize(s_dn);
+    if (cudaStreamSynchronize(s) != cudaSuccess && rc == AJT_OK) rc = AJT_ERR_CUDA;
+    for (int i = 0; i < nslab; ++i) {
+        if (ev_up[i]) cudaEventDestroy(ev_up[i]);
+        if (ev_k[i]) cudaEventDestroy(ev_k[i]);
+    }
+    if (ev0) cudaEventDestroy(ev0);
+    if (ev_end) cudaEventDestroy(ev_end);
+    if (s_up) cudaStreamDestroy(s_up);
+    if (s_dn) cudaStreamDestroy(s_dn);
 #undef AJT_CP
-    return cudaStreamSynchronize(s) == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
+#undef AJT_TRY
+    return rc;
 }
 
 // ------------------------------------------------------------------------------------------------ merge, host buffers

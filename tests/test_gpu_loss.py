@@ -187,6 +187,30 @@ def test_host_buffer_variant():
     assert np.array_equal(h["logp"], dev.logp.cpu().numpy())
 
 
+def test_host_buffer_variant_slab_pipeline():
+    # several row slabs in flight (H2D, loss call and D2H of neighbouring slabs overlap): dlogits / logp rows identical to the
+    # device call's; the scalar is the fp64 sum of the slabs' fp32 partials
+    T, V, S = 1500, 32000, 6
+    lv, logits, targets, old, adv, mask, seg = make_case(T, V, S, 0.5, torch.bfloat16, 3.0, 29)
+    dev = ajt.policy_loss_fwd_bwd(logits, targets, old, adv, mask, seg, S, 0.2, 0.28, want_logp=True, want_stats=True)
+    h = ajt.policy_loss_fwd_bwd_host(logits.cpu().pin_memory(), lv.targets, old.cpu().numpy(), lv.adv, lv.mask, lv.seg_ids, S,
+                                     0.2, 0.28, ajt.DT_BF16, want_logp=True, want_stats=True)
+    torch.cuda.synchronize()
+    assert h["status"] == 0
+    assert torch.equal(h["dlogits"], dev.dlogits.cpu())
+    assert np.array_equal(h["logp"], dev.logp.cpu().numpy())
+    st = dev.stats.cpu().numpy()
+    assert np.array_equal(h["stats"][:3], st[:3]) and abs(h["stats"][3] - st[3]) <= 1e-6 * max(1e-3, abs(st[3]))
+    # scale of the rounding: each of the 6 slab partials is rounded to fp32 once
+    assert abs(h["loss"] - float(dev.loss[0])) <= 1e-6 * max(abs(float(dev.loss[0])), 1e-3)
+    # fp32 logits take the separate dlogits buffer
+    lv, logits, targets, old, adv, mask, seg = make_case(700, 1024, 4, 0.5, torch.float32, 2.0, 31)
+    dev = ajt.policy_loss_fwd_bwd(logits, targets, old, adv, mask, seg, 4, 0.2, 0.2)
+    h = ajt.policy_loss_fwd_bwd_host(logits.cpu().pin_memory(), lv.targets, old.cpu().numpy(), lv.adv, lv.mask, lv.seg_ids, 4,
+                                     0.2, 0.2, ajt.DT_F32)
+    assert torch.equal(h["dlogits"], dev.dlogits.cpu()) and h["status"] == 0
+
+
 def test_segment_counts():
     # ajt_segment_counts: N_s over a batch, chunk by chunk (accumulate), equals a host bincount; bad ids set the status
     T, S = 100_003, 37
