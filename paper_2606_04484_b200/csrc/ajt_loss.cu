@@ -283,12 +283,13 @@ __device__ __forceinline__ float exp_diff(float m, float M) {  // exp(m - M), 0 
     return m == -INFINITY ? 0.f : ex2((m - M) * kLog2e);
 }
 
-// t = z - m (clamped so that a -inf logit or a padded lane gives 0 * finite), e = exp(t): s += e, u += e t.
+// t = z - m, e = exp(t): s += e, u += e t.  (The extended kernels never feed padding here; a -inf logit makes the entropy
+// NaN, as it does in the definition: the domain is finite logits, reading L-7.)
 __device__ __forceinline__ void acc_exp(float x, float ms, float& s, float& u, bool ext) {
     const float t = x - ms;
     const float e = ex2(t * kLog2e);
     s += e;
-    if (ext) u = fmaf(e, fmaxf(t, -1e30f), u);
+    if (ext) u = fmaf(e, t, u);
 }
 // re-base a partial (m, s, u = sum e^{z-m} (z-m)) onto the maximum M: returns the factor, updates s and u
 __device__ __forceinline__ void rebase(float m, float M, float& s, float& u) {
@@ -461,7 +462,7 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
             float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f, u0 = 0.f, u1 = 0.f;
 #pragma unroll
             for (int ch = 0; ch < NCH; ++ch) {
-                if (ch < nch) {
+                if (ch < nch && (!EXT || ch * kChunkElems + tid * 8 < sl_len)) {   // EXT: no -inf padding in e * t
                     acc_exp(bf16lo(r[ch].x), ms, s0, u0, EXT);
                     acc_exp(bf16hi(r[ch].x), ms, s1, u1, EXT);
                     acc_exp(bf16lo(r[ch].y), ms, s2, u0, EXT);
