@@ -291,6 +291,12 @@ __device__ __forceinline__ void acc_exp(float x, float ms, float& s, float& u, b
     s += e;
     if (ext) u = fmaf(e, t, u);
 }
+// The same with the subtraction folded into one FFMA (k = -m log2(e)); u then collects e z, and the caller takes m s off.
+__device__ __forceinline__ void acc_exp_fma(float x, float k, float& s, float& u, bool ext) {
+    const float e = ex2(fmaf(x, kLog2e, k));
+    s += e;
+    if (ext) u = fmaf(e, x, u);
+}
 // re-base a partial (m, s, u = sum e^{z-m} (z-m)) onto the maximum M: returns the factor, updates s and u
 __device__ __forceinline__ void rebase(float m, float M, float& s, float& u) {
     const float f = exp_diff(m, M);
@@ -460,17 +466,18 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
             const float m = fmaxf(bf16lo(mx), bf16hi(mx));
             const float ms = m == -INFINITY ? 0.f : m;
             float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f, u0 = 0.f, u1 = 0.f;
+            const float kms = -ms * kLog2e;
 #pragma unroll
             for (int ch = 0; ch < NCH; ++ch) {
                 if (ch < nch && (!EXT || ch * kChunkElems + tid * 8 < sl_len)) {   // EXT: no -inf padding in e * t
-                    acc_exp(bf16lo(r[ch].x), ms, s0, u0, EXT);
-                    acc_exp(bf16hi(r[ch].x), ms, s1, u1, EXT);
-                    acc_exp(bf16lo(r[ch].y), ms, s2, u0, EXT);
-                    acc_exp(bf16hi(r[ch].y), ms, s3, u1, EXT);
-                    acc_exp(bf16lo(r[ch].z), ms, s0, u0, EXT);
-                    acc_exp(bf16hi(r[ch].z), ms, s1, u1, EXT);
-                    acc_exp(bf16lo(r[ch].w), ms, s2, u0, EXT);
-                    acc_exp(bf16hi(r[ch].w), ms, s3, u1, EXT);
+                    acc_exp_fma(bf16lo(r[ch].x), kms, s0, u0, EXT);
+                    acc_exp_fma(bf16hi(r[ch].x), kms, s1, u1, EXT);
+                    acc_exp_fma(bf16lo(r[ch].y), kms, s2, u0, EXT);
+                    acc_exp_fma(bf16hi(r[ch].y), kms, s3, u1, EXT);
+                    acc_exp_fma(bf16lo(r[ch].z), kms, s0, u0, EXT);
+                    acc_exp_fma(bf16hi(r[ch].z), kms, s1, u1, EXT);
+                    acc_exp_fma(bf16lo(r[ch].w), kms, s2, u0, EXT);
+                    acc_exp_fma(bf16hi(r[ch].w), kms, s3, u1, EXT);
                 }
             }
             float s = (s0 + s1) + (s2 + s3);
@@ -478,7 +485,7 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
             const float mw = warp_max(m);
             float sw, uw = 0.f;
             if (EXT) {
-                float u = u0 + u1;
+                float u = fmaf(-ms, s, u0 + u1);   // sum e (z - m)
                 rebase(m, mw, s, u);
                 sw = warp_sum(s);
                 uw = warp_sum(u);
