@@ -1412,9 +1412,14 @@ __device__ void scatter_body(const MergeParams& p, int mode, MemberList* lists) 
     bool mismatch = false;
     int m = warp_search_last_le(M, t_begin, [&](int x) { return p.tile_base[x]; });
     int cur_m = -1, cnt = 0, tb = 0;
+    int tb_next = p.tile_base[m + 1];   // first tile of the next sequence: kept in a register, so that a tile inside a
+                                        // sequence does not start with a dependent global load
     TileCtx c = {};
     for (int t = t_begin; t < t_end; ++t) {
-        while (p.tile_base[m + 1] <= t) ++m;
+        while (tb_next <= t) {
+            ++m;
+            tb_next = p.tile_base[m + 1];
+        }
         if (m != cur_m) {
             cur_m = m;
             tb = p.tile_base[m];
