@@ -273,6 +273,32 @@ def pack_loss_inputs(merged_tokens, merged_mask, merged_old_logp, merged_offsets
     return targets, mask, olp, seg, adv
 
 
+def lm_head_logp(hidden_bits, weight_bits, targets, mask=None):
+    """Log-prob and entropy of the target token under an LM head, without the method's tiling (the step before
+    the loss in the actor update, forward half):
+        z_t = W h_t  (fp64 from the exact bf16 inputs);  logp_t = z_{t,y_t} - logsumexp(z_t);  H_t = lse_t - sum_v p_tv z_tv
+    hidden_bits uint16 [T,d], weight_bits uint16 [V,d] (bf16 bit patterns).  Rows with mask 0 give 0, 0."""
+    def f64(bits):
+        b = np.ascontiguousarray(bits, np.uint16).astype(np.uint32) << 16
+        return b.view(np.float32).astype(np.float64)
+    H, W = f64(hidden_bits), f64(weight_bits)
+    T = H.shape[0]
+    logp = np.zeros(T, np.float64)
+    ent = np.zeros(T, np.float64)
+    for a in range(0, T, 256):
+        z = H[a:a + 256] @ W.T                      # library matmul as a step
+        m = z.max(axis=1, keepdims=True)
+        lse = m[:, 0] + np.log(np.exp(z - m).sum(axis=1))
+        p = np.exp(z - lse[:, None])
+        rows = np.arange(z.shape[0])
+        logp[a:a + 256] = z[rows, np.asarray(targets[a:a + 256], np.int64)] - lse
+        ent[a:a + 256] = lse - (p * z).sum(axis=1)
+    if mask is not None:
+        on = np.asarray(mask) != 0
+        logp, ent = np.where(on, logp, 0.0), np.where(on, ent, 0.0)
+    return logp, ent
+
+
 def round_bf16(x: np.ndarray) -> np.ndarray:
     """fp64 -> nearest bf16 (ties to even), as fp64."""
     a = np.ascontiguousarray(x, np.float64)
