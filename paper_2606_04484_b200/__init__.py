@@ -25,6 +25,7 @@ from .binding import (  # noqa: F401
     last_status,
     lib,
     library_path,
+    lm_head_logp,
     loss_host_arena_bytes,
     loss_workspace_bytes,
     merge_blocks,

@@ -26,7 +26,7 @@ _EXPORTS = [
     "ajt_merge_workspace_bytes", "ajt_merge_timelines", "ajt_merge_host_arena_bytes", "ajt_merge_timelines_host",
     "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
     "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks_workspace_bytes", "ajt_merge_blocks",
-    "ajt_pack_loss_inputs",
+    "ajt_pack_loss_inputs", "ajt_lm_head_workspace_bytes", "ajt_lm_head_logp",
 ]
 
 _lib = None
@@ -61,6 +61,8 @@ def lib():
         for f in ("ajt_merge_workspace_bytes", "ajt_merge_host_arena_bytes"):
             getattr(L, f).restype = C.c_size_t
             getattr(L, f).argtypes = [C.c_int32, C.c_int64]
+        L.ajt_lm_head_workspace_bytes.restype = C.c_size_t
+        L.ajt_lm_head_workspace_bytes.argtypes = [C.c_int64, C.c_int32]
         L.ajt_merge_blocks_workspace_bytes.restype = C.c_size_t
         L.ajt_merge_blocks_workspace_bytes.argtypes = [C.c_int32, C.c_int64]
         L.ajt_loss_workspace_bytes.restype = C.c_size_t
@@ -69,7 +71,7 @@ def lib():
         L.ajt_loss_host_arena_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32]
         for f in ("ajt_merge_timelines", "ajt_merge_timelines_host", "ajt_policy_loss_fwd_bwd",
                   "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks",
-                  "ajt_pack_loss_inputs"):
+                  "ajt_pack_loss_inputs", "ajt_lm_head_logp"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -451,6 +453,30 @@ def policy_loss_fwd_bwd_ext(logits: torch.Tensor, targets: torch.Tensor, old_log
     if rc != 0:
         raise AjtError(rc, "ajt_policy_loss_fwd_bwd_ext")
     return out
+
+
+def lm_head_logp(hidden: torch.Tensor, weight: torch.Tensor, targets: torch.Tensor, mask: Optional[torch.Tensor] = None,
+                 want_entropy: bool = True, workspace: Optional[torch.Tensor] = None, stream=None):
+    """ajt_lm_head_logp (include/ajt.h): (logp f32 [T], entropy f32 [T] | None) from hidden [T, d] and weight [V, d] (bf16)."""
+    _require_cuda()
+    _check_dev(hidden, torch.bfloat16, "hidden")
+    _check_dev(weight, torch.bfloat16, "weight")
+    _check_dev(targets, torch.int32, "targets")
+    _check_dev(mask, torch.uint8, "mask")
+    if hidden.dim() != 2 or weight.dim() != 2 or hidden.stride(1) != 1 or weight.stride(1) != 1 or hidden.shape[1] != weight.shape[1]:
+        raise TypeError("hidden [T, d] and weight [V, d] with unit column stride")
+    T, d, V = int(hidden.shape[0]), int(hidden.shape[1]), int(weight.shape[0])
+    dev = hidden.device
+    logp = torch.empty(max(T, 1), dtype=torch.float32, device=dev)
+    ent = torch.empty(max(T, 1), dtype=torch.float32, device=dev) if want_entropy else None
+    if workspace is None:
+        workspace = torch.empty(int(lib().ajt_lm_head_workspace_bytes(C.c_int64(T), C.c_int32(V))) + 256, dtype=torch.uint8, device=dev)
+    rc = lib().ajt_lm_head_logp(_dp(hidden), _dp(weight), _dp(targets), _dp(mask), C.c_int64(T), C.c_int32(d), C.c_int32(V),
+                                C.c_int64(int(hidden.stride(0)) if T > 1 else d), C.c_int64(int(weight.stride(0)) if V > 1 else d),
+                                _dp(logp), _dp(ent), _dp(workspace), C.c_size_t(workspace.numel()), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_lm_head_logp")
+    return logp[:T], (None if ent is None else ent[:T])
 
 
 def segment_counts(mask: torch.Tensor, seg_ids: torch.Tensor, S: int, out: Optional[torch.Tensor] = None,

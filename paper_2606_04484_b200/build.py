@@ -7,7 +7,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["ajt_api.cu", "ajt_loss.cu", "ajt_merge.cu", "ajt_blocks.cu", "ajt_pack.cu"]
+SOURCES = ["ajt_api.cu", "ajt_loss.cu", "ajt_merge.cu", "ajt_blocks.cu", "ajt_pack.cu", "ajt_lmhead.cu"]
 HEADERS = ["ajt_common.cuh", os.path.join("..", "..", "include", "ajt.h")]
 LIB = os.path.join(HERE, "libajt.so")
 

@@ -1,0 +1,330 @@
+// Log-prob and entropy of the target token straight from the hidden states: logits = H W^T are produced tile by tile on the
+// 5th-generation tensor cores (tcgen05.mma, bf16 x bf16 -> fp32 in TMEM) and reduced on the fly (online max / sum-exp /
+// sum e (z - m) / target gather), so the [T, V] logits never reach HBM.  This is the forward half of SURVEY.md §8(f) f3: the pass
+// that produces the old / reference log-probs the loss consumes.  DESIGN.md "O-H".
+//
+// Work item = (128 rows of H) x (one of VS vocabulary ranges).  Inside an item the CTA walks the range in tiles of 256
+// columns; per tile the K loop streams 64-wide slabs of H and W through a 4-stage TMA ring (SWIZZLE_128B, K-major), one
+// elected thread issues 4 x tcgen05.mma (128 x 256 x 16) per slab, and the two 256-column TMEM accumulators alternate so that
+// the epilogue warps (one row per thread: tcgen05.ld 32 columns at a time) reduce tile n while the tensor cores fill tile n+1.
+// The CTAs that run at the same time share the W ranges (L2) and own different row blocks.
+// Per (row, range) the epilogue leaves {m, s, u, z_y}; lm_head_combine_kernel folds the VS partials of a row.
+#include <cuda.h>
+
+#include "ajt_common.cuh"
+
+namespace {
+
+using namespace ajt;
+
+constexpr int kBM = 128, kBN = 256, kBK = 64, kStages = 4, kVS = 4;
+constexpr int kABytes = kBM * kBK * 2, kBBytes = kBN * kBK * 2, kStageBytes = kABytes + kBBytes;
+constexpr int kLmThreads = 192;   // warp 0: TMA producer, warp 1: MMA issuer + TMEM owner, warps 2-5: epilogue
+constexpr size_t kLmSmem = (size_t)kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
+constexpr float kLog2e = 1.4426950408889634f;
+// instruction descriptor (kind::f16): D = F32, A = B = BF16, both K-major, N = 256, M = 128
+constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kBN >> 3) << 17) | ((uint32_t)(kBM >> 4) << 24);
+
+struct LmParams {
+    const int32_t* targets;
+    const uint8_t* mask;
+    int64_t T;
+    int32_t d, V, vs_len, n_mtiles, mgroup;   // vs_len: columns per vocabulary range (multiple of kBN); mgroup: row blocks per wave
+    float4* part;                             // [T][kVS] {m, s, u, z_y (or -inf)}
+    float* logp_out;
+    float* ent_out;
+};
+
+__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+                 : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// K-major operand tile, rows of 128 bytes (64 bf16), 8-row groups 1024 bytes apart, SWIZZLE_128B
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr) {
+    const uint64_t lo = (uint64_t)((addr >> 4) & 0x3FFFu);
+    const uint64_t hi = (uint64_t)((1024u >> 4) & 0x3FFFu) | (1ull << 14) /* descriptor version */ | (2ull << 29) /* SWIZZLE_128B */;
+    return lo | (hi << 32);
+}
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+        "l"(da), "l"(db), "r"(kIdesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+          "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+          "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// item i of CTA b: row block (i * mgroup + b / kVS), vocabulary range b % kVS
+__device__ __forceinline__ bool item_of(const LmParams& p, int it, int& mt, int& vs) {
+    mt = it * p.mgroup + (int)blockIdx.x / kVS;
+    vs = (int)blockIdx.x % kVS;
+    return (int)blockIdx.x / kVS < p.mgroup && mt < p.n_mtiles;
+}
+
+__global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_constant__ CUtensorMap map_h,
+                                                                const __grid_constant__ CUtensorMap map_w, const LmParams p) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)kStages * kStageBytes);
+    uint64_t* empty = full + kStages;
+    uint64_t* tfull = empty + kStages;    // [2] accumulator ready
+    uint64_t* tempty = tfull + 2;         // [2] accumulator drained
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nk = p.d / kBK;
+    const int n_items = (p.n_mtiles + p.mgroup - 1) / p.mgroup;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < kStages; ++i) {
+            mbar_init(&full[i], 1);
+            mbar_init(&empty[i], 1);
+        }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(&tfull[i], 1);
+            mbar_init(&tempty[i], 4);
+        }
+        fence_mbar_init();
+    }
+    if (warp == 1) {   // TMEM: all 512 columns (two 128 x 256 fp32 accumulators)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t ph = 0;
+            for (int it = 0; it < n_items; ++it) {
+                int mt, vs;
+                if (!item_of(p, it, mt, vs)) continue;
+                const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
+                for (int n0 = v0; n0 < v1; n0 += kBN) {
+                    for (int k = 0; k < nk; ++k) {
+                        mbar_wait(&empty[stage], ph ^ 1u);
+                        uint8_t* sa = smem + (size_t)stage * kStageBytes;
+                        mbar_arrive_expect_tx(&full[stage], kStageBytes);
+                        tma_load_2d(sa, &map_h, k * kBK, mt * kBM, &full[stage]);
+                        tma_load_2d(sa + kABytes, &map_w, k * kBK, n0, &full[stage]);
+                        if (++stage == kStages) { stage = 0; ph ^= 1u; }
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        int stage = 0, as = 0;
+        uint32_t ph = 0, aph = 0;
+        for (int it = 0; it < n_items; ++it) {
+            int mt, vs;
+            if (!item_of(p, it, mt, vs)) continue;
+            const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
+            for (int n0 = v0; n0 < v1; n0 += kBN) {
+                mbar_wait(&tempty[as], aph ^ 1u);
+                tc_fence_after();
+                const uint32_t tacc = tmem_base + (uint32_t)(as * kBN);
+                for (int k = 0; k < nk; ++k) {
+                    mbar_wait(&full[stage], ph);
+                    tc_fence_after();
+                    if (lane == 0) {
+                        const uint32_t sa = smem_u32(smem + (size_t)stage * kStageBytes), sb = sa + kABytes;
+#pragma unroll
+                        for (int kk = 0; kk < kBK / 16; ++kk)   // 16 bf16 = 32 bytes along K inside the 128-byte swizzled row
+                            umma_bf16(tacc, smem_desc(sa + kk * 32), smem_desc(sb + kk * 32), (uint32_t)((k | kk) != 0));
+                        tc_commit(&empty[stage]);               // frees the smem slot when these MMAs have read it
+                        if (k == nk - 1) tc_commit(&tfull[as]); // accumulator complete
+                    }
+                    __syncwarp();
+                    if (++stage == kStages) { stage = 0; ph ^= 1u; }
+                }
+                if (++as == 2) { as = 0; aph ^= 1u; }
+            }
+        }
+    } else {
+        // ===== epilogue: thread <-> one row of the block (TMEM lane); warp w may touch lanes 32 (w % 4) .. +31 =====
+        const int quad = warp & 3;
+        const int rloc = quad * 32 + lane;
+        int as = 0;
+        uint32_t aph = 0;
+        for (int it = 0; it < n_items; ++it) {
+            int mt, vs;
+            if (!item_of(p, it, mt, vs)) continue;
+            const int64_t row = (int64_t)mt * kBM + rloc;
+            const bool live = row < p.T;
+            const int y = live ? p.targets[row] : -1;
+            float m = -INFINITY, s = 0.f, u = 0.f, zy = -INFINITY;
+            const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
+            for (int n0 = v0; n0 < v1; n0 += kBN) {
+                mbar_wait(&tfull[as], aph);
+                tc_fence_after();
+                const uint32_t tacc = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * kBN);
+#pragma unroll 1
+                for (int c = 0; c < kBN; c += 32) {
+                    uint32_t v[32];
+                    tmem_ld32(tacc + (uint32_t)c, v);
+                    const int col0 = n0 + c;
+                    if (col0 >= v1) continue;
+                    const int nval = min(32, v1 - col0);
+                    float cm = -INFINITY;
+#pragma unroll
+                    for (int e = 0; e < 32; ++e)
+                        if (e < nval) cm = fmaxf(cm, __uint_as_float(v[e]));
+                    if (cm > m) {   // re-base the running partial onto the new maximum
+                        const float f = m == -INFINITY ? 0.f : ex2((m - cm) * kLog2e);
+                        const float dm = m == -INFINITY ? 0.f : m - cm;
+                        u = f * fmaf(dm, s, u);
+                        s = f * s;
+                        m = cm;
+                    }
+                    const float km = -m * kLog2e;
+                    float es = 0.f, eu = 0.f;
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) {
+                        if (e < nval) {
+                            const float x = __uint_as_float(v[e]);
+                            const float ex = ex2(fmaf(x, kLog2e, km));
+                            es += ex;
+                            eu = fmaf(ex, x - m, eu);
+                        }
+                    }
+                    s += es;
+                    u += eu;
+                    if (y >= col0 && y < col0 + nval) {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e)
+                            if (e == y - col0) zy = __uint_as_float(v[e]);
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&tempty[as]);
+                if (++as == 2) { as = 0; aph ^= 1u; }
+            }
+            if (live) p.part[row * kVS + vs] = make_float4(m, s, u, zy);
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+    }
+}
+
+__global__ void __launch_bounds__(256) lm_head_combine_kernel(const LmParams p, int nvs) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < p.T; t += stride) {
+        float lp = 0.f, H = 0.f;
+        if (!p.mask || p.mask[t] != 0) {
+            float4 q[kVS];
+            float M = -INFINITY, zy = -INFINITY;
+            for (int k = 0; k < nvs; ++k) {
+                q[k] = p.part[t * kVS + k];
+                M = fmaxf(M, q[k].x);
+                zy = fmaxf(zy, q[k].w);   // exactly one range holds the target; the others left -inf
+            }
+            float S = 0.f, U = 0.f;
+            for (int k = 0; k < nvs; ++k) {
+                const float f = q[k].x == -INFINITY ? 0.f : ex2((q[k].x - M) * kLog2e);
+                const float dm = q[k].x == -INFINITY ? 0.f : q[k].x - M;
+                U += f * fmaf(dm, q[k].y, q[k].z);
+                S += f * q[k].y;
+            }
+            const float logS = logf(S);
+            lp = (zy - M) - logS;
+            H = logS - U / S;
+        }
+        p.logp_out[t] = lp;
+        if (p.ent_out) p.ent_out[t] = H;
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// [rows, d] row-major bf16 with row stride ld (elements); box = 64 columns x box_rows rows, 128-byte swizzle
+bool make_map(EncodeTiledFn fn, CUtensorMap* map, const void* base, int64_t rows, int32_t d, int64_t ld, int box_rows) {
+    const cuuint64_t dims[2] = {(cuuint64_t)d, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
+    const cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    return fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+extern "C" size_t ajt_lm_head_workspace_bytes(int64_t T, int32_t V) {
+    if (T < 0 || V <= 0) return 0;
+    return (((size_t)T * kVS * sizeof(float4)) + 255) & ~(size_t)255;
+}
+
+extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const int32_t* targets, const uint8_t* mask, int64_t T,
+                                int32_t d, int32_t V, int64_t ld_hidden, int64_t ld_weight, float* logp_out, float* ent_out,
+                                void* workspace, size_t workspace_bytes, ajt_stream_t stream_) {
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (T < 0 || d <= 0 || V <= 0 || ld_hidden < d || ld_weight < d) return AJT_ERR_INVALID_ARG;
+    if (!logp_out || !workspace) return AJT_ERR_INVALID_ARG;
+    if (T > 0 && (!hidden || !weight || !targets)) return AJT_ERR_INVALID_ARG;
+    if (d % kBK != 0 || (ld_hidden % 8) != 0 || (ld_weight % 8) != 0 || (((uintptr_t)hidden | (uintptr_t)weight) & 15) ||
+        T >= ((int64_t)1 << 31))
+        return AJT_ERR_UNSUPPORTED;   // K slabs of 64, 16-byte aligned rows (TMA)
+    if (((uintptr_t)workspace & 255) || workspace_bytes < ajt_lm_head_workspace_bytes(T, V)) return AJT_ERR_WORKSPACE_TOO_SMALL;
+    if (T == 0) return AJT_OK;
+
+    int dev = 0, num_sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AJT_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || num_sms < kVS) return AJT_ERR_CUDA;
+    static EncodeTiledFn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return AJT_ERR_CUDA;
+        encode = reinterpret_cast<EncodeTiledFn>(fn);
+    }
+    CUtensorMap map_h, map_w;
+    if (!make_map(encode, &map_h, hidden, T, d, ld_hidden, kBM) || !make_map(encode, &map_w, weight, V, d, ld_weight, kBN))
+        return AJT_ERR_CUDA;
+
+    LmParams p;
+    p.targets = targets; p.mask = mask; p.T = T; p.d = d; p.V = V;
+    p.n_mtiles = (int)((T + kBM - 1) / kBM);
+    const int nvs = V >= kVS * kBN ? kVS : 1;   // small vocabularies: one range
+    p.vs_len = (((V + nvs - 1) / nvs + kBN - 1) / kBN) * kBN;
+    p.mgroup = num_sms / kVS;
+    if (p.mgroup > p.n_mtiles) p.mgroup = p.n_mtiles;
+    p.part = reinterpret_cast<float4*>(workspace);
+    p.logp_out = logp_out; p.ent_out = ent_out;
+    if (nvs == 1) p.vs_len = ((V + kBN - 1) / kBN) * kBN;
+
+    if (cudaFuncSetAttribute(lm_head_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLmSmem) != cudaSuccess) return AJT_ERR_CUDA;
+    // ranges beyond nvs are empty (v0 >= V): their CTAs have nothing to do, and the combine reads nvs partials per row
+    lm_head_kernel<<<p.mgroup * kVS, kLmThreads, kLmSmem, stream>>>(map_h, map_w, p);
+    const int64_t want = (T + 255) / 256;
+    lm_head_combine_kernel<<<(int)(want < (int64_t)num_sms * 4 ? want : (int64_t)num_sms * 4), 256, 0, stream>>>(p, nvs);
+    return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
+}
