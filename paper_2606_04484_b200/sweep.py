@@ -196,6 +196,30 @@ def run_c5(dev, stream, reps, out, quick=False):
             torch.cuda.empty_cache()
 
 
+def measure_lm_head(name: str, T: int, d: int, V: int, dev, stream, reps: int, out):
+    """ajt_lm_head_logp (forward half): dense contraction on the tensor cores, reported in TFLOP/s against
+    the measured bf16 matmul throughput of MEASURED_PEAKS.json (burst figure: the kernel is timed alone)."""
+    g = torch.Generator(device=dev).manual_seed(17)
+    Hh = torch.randn((T, d), generator=g, device=dev).to(torch.bfloat16)
+    Ww = (torch.randn((V, d), generator=g, device=dev) * 0.02).to(torch.bfloat16)
+    y = torch.randint(0, V, (T,), generator=g, device=dev, dtype=torch.int32)
+    ws = torch.empty(int(ajt.lib().ajt_lm_head_workspace_bytes(T, V)) + 256, dtype=torch.uint8, device=dev)
+    call = lambda: ajt.lm_head_logp(Hh, Ww, y, None, workspace=ws, stream=stream)
+    med, best = _stats(H.time_calls(call, stream, reps=reps, flush=None))
+    flops = 2.0 * T * d * V
+    tf = flops / (med * 1e-3) / 1e12
+    peak = None
+    try:
+        import json as _j, os as _o
+        with open(_o.path.join(H.ROOT, "MEASURED_PEAKS.json")) as f:
+            peak = float(_j.load(f)["bf16_tflops"])
+    except Exception:
+        peak = 2250.0 * 0.7   # B200_PROFILING.md fallback: nominal dense bf16 x typical cuBLAS fraction
+    _emit(out, stage="lm_head_logp", config=name, T=T, d=d, V=V, ms_median=med, ms_best=best, flops=flops, tflop_per_s=tf,
+          peak_tflops=peak, frac_of_measured=tf / peak, frac_of_nominal_2250=tf / 2250.0,
+          logits_bytes_not_written=2.0 * T * V, reps=reps)
+
+
 def stock_bandwidth(dev, out):
     """Context for the rooflines: what stock library kernels (torch fill_ / copy_, cudaMemset) reach on this box when they move
     the bytes of the loss step (12.9 GB arrays; the bench micro-batch reads 27 % of the rows and writes all of them)."""
@@ -270,6 +294,10 @@ def main():
                                  max(5, args.reps // 2), out)
         elif c in W.BLOCK_SPECS:
             measure_blocks(c, W.block_workload(c), dev, stream, args.reps, out)
+        elif c == "h1":   # Qwen3-8B-like head (d = 4096, V = 151936) over the bench micro-batch's rows
+            measure_lm_head("h1", 40960, 4096, 151936, dev, stream, max(3, args.reps // 4), out)
+        elif c == "h0":
+            measure_lm_head("h0", 8192, 2048, 32000, dev, stream, args.reps, out)
         elif c == "c5":
             if not args.merge_only:
                 run_c5(dev, stream, args.reps, out, quick=args.quick)
