@@ -17,13 +17,25 @@ namespace {
 
 using namespace ajt;
 
-constexpr int kBM = 128, kBN = 256, kBK = 64, kStages = 4, kVS = 4;
-constexpr int kABytes = kBM * kBK * 2, kBBytes = kBN * kBK * 2, kStageBytes = kABytes + kBBytes;
+constexpr int kBM = 128, kBN = 256, kBK = 64, kVS = 4;
+constexpr int kABytes = kBM * kBK * 2;
 constexpr int kLmThreads = 192;   // warp 0: TMA producer, warp 1: MMA issuer + TMEM owner, warps 2-5: epilogue
-constexpr size_t kLmSmem = (size_t)kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
 constexpr float kLog2e = 1.4426950408889634f;
-// instruction descriptor (kind::f16): D = F32, A = B = BF16, both K-major, N = 256, M = 128
-constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kBN >> 3) << 17) | ((uint32_t)(kBM >> 4) << 24);
+// NCTA = 1: one CTA per 128-row block, the whole 256-column W tile in its shared memory (16 + 32 KB per slab, 4 stages).
+// NCTA = 2: a CTA pair (cluster of 2, tcgen05 cta_group::2) per 256-row block: each CTA stages its own 128 rows of H and
+// HALF of the W tile (16 + 16 KB per slab, 6 stages); the leader issues 256 x 256 x 16 MMAs that read both CTAs' shared
+// memory and fill both CTAs' tensor memory.  Less shared-memory traffic per flop and a deeper ring.
+template <int NCTA> struct LmCfg {
+    static constexpr int kBRows = kBN / NCTA;                      // W rows (vocabulary columns) staged per CTA
+    static constexpr int kBBytes = kBRows * kBK * 2;
+    static constexpr int kStageBytes = kABytes + kBBytes;
+    static constexpr int kStages = NCTA == 1 ? 4 : 6;
+    static constexpr size_t kSmem = (size_t)kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
+    // instruction descriptor (kind::f16): D = F32, A = B = BF16, both K-major, N = 256, M = 128 per CTA
+    static constexpr uint32_t kIdesc =
+        (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kBN >> 3) << 17) | ((uint32_t)((kBM * NCTA) >> 4) << 24);
+};
+constexpr uint32_t kPeerBitMask = 0xFEFFFFFFu;   // shared::cluster address of the same location in the pair's CTA 0
 
 struct LmParams {
     const int32_t* targets;
@@ -43,8 +55,27 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// pair: the copy lands in this CTA's shared memory, its bytes are counted on CTA 0's barrier
+__device__ __forceinline__ void tma_load_2d_pair(void* smem_dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+            smem_u32(smem_dst)),
+        "l"(map), "r"(smem_u32(bar) & kPeerBitMask), "r"(c0), "r"(c1)
+        : "memory");
+}
+template <int NCTA>
 __device__ __forceinline__ void tc_commit(uint64_t* bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+    if (NCTA == 1)
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+    else   // arrives on the barrier at this offset in BOTH CTAs of the pair
+        asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(
+                         smem_u32(bar)),
+                     "h"((uint16_t)3)
+                     : "memory");
+}
+// arrive on the barrier at this offset in CTA `rank` of the cluster
+__device__ __forceinline__ void mbar_arrive_remote(uint64_t* bar, uint32_t rank) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(mapa(smem_u32(bar), rank)) : "memory");
 }
 // K-major operand tile, rows of 128 bytes (64 bf16), 8-row groups 1024 bytes apart, SWIZZLE_128B
 __device__ __forceinline__ uint64_t smem_desc(uint32_t addr) {
@@ -52,12 +83,20 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t addr) {
     const uint64_t hi = (uint64_t)((1024u >> 4) & 0x3FFFu) | (1ull << 14) /* descriptor version */ | (2ull << 29) /* SWIZZLE_128B */;
     return lo | (hi << 32);
 }
+template <int NCTA>
 __device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
-        "l"(da), "l"(db), "r"(kIdesc), "r"(accumulate)
-        : "memory");
+    if (NCTA == 1)
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+            "l"(da), "l"(db), "r"(LmCfg<1>::kIdesc), "r"(accumulate)
+            : "memory");
+    else
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+            "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+            "l"(da), "l"(db), "r"(LmCfg<2>::kIdesc), "r"(accumulate)
+            : "memory");
 }
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
     asm volatile(
@@ -73,23 +112,30 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
-// item i of CTA b: row block (i * mgroup + b / kVS), vocabulary range b % kVS
+// item i of work group g (a CTA, or a CTA pair): row block (i * mgroup + g / kVS), vocabulary range g % kVS
+template <int NCTA>
 __device__ __forceinline__ bool item_of(const LmParams& p, int it, int& mt, int& vs) {
-    mt = it * p.mgroup + (int)blockIdx.x / kVS;
-    vs = (int)blockIdx.x % kVS;
-    return (int)blockIdx.x / kVS < p.mgroup && mt < p.n_mtiles;
+    const int g = (int)blockIdx.x / NCTA;
+    mt = it * p.mgroup + g / kVS;
+    vs = g % kVS;
+    return g / kVS < p.mgroup && mt < p.n_mtiles;
 }
 
+// p.n_mtiles counts row blocks of 128 * NCTA rows.
+template <int NCTA>
 __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_constant__ CUtensorMap map_h,
                                                                 const __grid_constant__ CUtensorMap map_w, const LmParams p) {
+    using Cfg = LmCfg<NCTA>;
+    constexpr int kStages = Cfg::kStages, kStageBytes = Cfg::kStageBytes;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)kStages * kStageBytes);
     uint64_t* empty = full + kStages;
     uint64_t* tfull = empty + kStages;    // [2] accumulator ready
-    uint64_t* tempty = tfull + 2;         // [2] accumulator drained
+    uint64_t* tempty = tfull + 2;         // [2] accumulator drained (pair: CTA 0's counts both CTAs' epilogue warps)
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = NCTA > 1 ? cluster_ctarank() : 0u;
     const int nk = p.d / kBK;
     const int n_items = (p.n_mtiles + p.mgroup - 1) / p.mgroup;
 
@@ -100,79 +146,93 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(&tfull[i], 1);
-            mbar_init(&tempty[i], 4);
+            mbar_init(&tempty[i], 4 * NCTA);
         }
         fence_mbar_init();
     }
-    if (warp == 1) {   // TMEM: all 512 columns (two 128 x 256 fp32 accumulators)
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (warp == 1) {   // TMEM: all 512 columns (two 256-column fp32 accumulators of this CTA's 128 rows)
+        if (NCTA == 1) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+        }
     }
     tc_fence_before();
-    __syncthreads();
+    if (NCTA > 1) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
     if (warp == 0) {
-        // ===== TMA producer =====
+        // ===== TMA producer (every CTA: its own rows of H, its share of the W tile) =====
         if (lane == 0) {
             int stage = 0;
             uint32_t ph = 0;
             for (int it = 0; it < n_items; ++it) {
                 int mt, vs;
-                if (!item_of(p, it, mt, vs)) continue;
+                if (!item_of<NCTA>(p, it, mt, vs)) continue;
                 const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
+                const int row0 = (mt * NCTA + (int)rank) * kBM;
                 for (int n0 = v0; n0 < v1; n0 += kBN) {
                     for (int k = 0; k < nk; ++k) {
                         mbar_wait(&empty[stage], ph ^ 1u);
                         uint8_t* sa = smem + (size_t)stage * kStageBytes;
-                        mbar_arrive_expect_tx(&full[stage], kStageBytes);
-                        tma_load_2d(sa, &map_h, k * kBK, mt * kBM, &full[stage]);
-                        tma_load_2d(sa + kABytes, &map_w, k * kBK, n0, &full[stage]);
+                        if (NCTA == 1) {
+                            mbar_arrive_expect_tx(&full[stage], kStageBytes);
+                            tma_load_2d(sa, &map_h, k * kBK, row0, &full[stage]);
+                            tma_load_2d(sa + kABytes, &map_w, k * kBK, n0, &full[stage]);
+                        } else {
+                            if (rank == 0) mbar_arrive_expect_tx(&full[stage], 2 * kStageBytes);   // both CTAs' bytes land on CTA 0's barrier
+                            tma_load_2d_pair(sa, &map_h, k * kBK, row0, &full[stage]);
+                            tma_load_2d_pair(sa + kABytes, &map_w, k * kBK, n0 + (int)rank * Cfg::kBRows, &full[stage]);
+                        }
                         if (++stage == kStages) { stage = 0; ph ^= 1u; }
                     }
                 }
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer =====
-        int stage = 0, as = 0;
-        uint32_t ph = 0, aph = 0;
-        for (int it = 0; it < n_items; ++it) {
-            int mt, vs;
-            if (!item_of(p, it, mt, vs)) continue;
-            const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
-            for (int n0 = v0; n0 < v1; n0 += kBN) {
-                mbar_wait(&tempty[as], aph ^ 1u);
-                tc_fence_after();
-                const uint32_t tacc = tmem_base + (uint32_t)(as * kBN);
-                for (int k = 0; k < nk; ++k) {
-                    mbar_wait(&full[stage], ph);
+        // ===== MMA issuer (pair: the leader CTA only) =====
+        if (rank == 0) {
+            int stage = 0, as = 0;
+            uint32_t ph = 0, aph = 0;
+            for (int it = 0; it < n_items; ++it) {
+                int mt, vs;
+                if (!item_of<NCTA>(p, it, mt, vs)) continue;
+                const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
+                for (int n0 = v0; n0 < v1; n0 += kBN) {
+                    mbar_wait(&tempty[as], aph ^ 1u);
                     tc_fence_after();
-                    if (lane == 0) {
-                        const uint32_t sa = smem_u32(smem + (size_t)stage * kStageBytes), sb = sa + kABytes;
+                    const uint32_t tacc = tmem_base + (uint32_t)(as * kBN);
+                    for (int k = 0; k < nk; ++k) {
+                        mbar_wait(&full[stage], ph);
+                        tc_fence_after();
+                        if (lane == 0) {
+                            const uint32_t sa = smem_u32(smem + (size_t)stage * kStageBytes), sb = sa + kABytes;
 #pragma unroll
-                        for (int kk = 0; kk < kBK / 16; ++kk)   // 16 bf16 = 32 bytes along K inside the 128-byte swizzled row
-                            umma_bf16(tacc, smem_desc(sa + kk * 32), smem_desc(sb + kk * 32), (uint32_t)((k | kk) != 0));
-                        tc_commit(&empty[stage]);               // frees the smem slot when these MMAs have read it
-                        if (k == nk - 1) tc_commit(&tfull[as]); // accumulator complete
+                            for (int kk = 0; kk < kBK / 16; ++kk)   // 16 bf16 = 32 bytes along K inside the 128-byte swizzled row
+                                umma_bf16<NCTA>(tacc, smem_desc(sa + kk * 32), smem_desc(sb + kk * 32), (uint32_t)((k | kk) != 0));
+                            tc_commit<NCTA>(&empty[stage]);               // frees the smem slot (in both CTAs) once read
+                            if (k == nk - 1) tc_commit<NCTA>(&tfull[as]); // accumulator complete
+                        }
+                        __syncwarp();
+                        if (++stage == kStages) { stage = 0; ph ^= 1u; }
                     }
-                    __syncwarp();
-                    if (++stage == kStages) { stage = 0; ph ^= 1u; }
+                    if (++as == 2) { as = 0; aph ^= 1u; }
                 }
-                if (++as == 2) { as = 0; aph ^= 1u; }
             }
         }
     } else {
-        // ===== epilogue: thread <-> one row of the block (TMEM lane); warp w may touch lanes 32 (w % 4) .. +31 =====
+        // ===== epilogue: thread <-> one row of this CTA's 128 (TMEM lane); warp w may touch lanes 32 (w % 4) .. +31 =====
         const int quad = warp & 3;
         const int rloc = quad * 32 + lane;
         int as = 0;
         uint32_t aph = 0;
         for (int it = 0; it < n_items; ++it) {
             int mt, vs;
-            if (!item_of(p, it, mt, vs)) continue;
-            const int64_t row = (int64_t)mt * kBM + rloc;
+            if (!item_of<NCTA>(p, it, mt, vs)) continue;
+            const int64_t row = (int64_t)(mt * NCTA + (int)rank) * kBM + rloc;
             const bool live = row < p.T;
             const int y = live ? p.targets[row] : -1;
             float m = -INFINITY, s = 0.f, u = 0.f, zy = -INFINITY;
@@ -220,17 +280,21 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&tempty[as]);
+                if (lane == 0) {
+                    if (NCTA == 1) mbar_arrive(&tempty[as]);
+                    else mbar_arrive_remote(&tempty[as], 0);   // the leader's MMA warp waits for both CTAs' epilogues
+                }
                 if (++as == 2) { as = 0; aph ^= 1u; }
             }
             if (live) p.part[row * kVS + vs] = make_float4(m, s, u, zy);
         }
     }
     tc_fence_before();
-    __syncthreads();
+    if (NCTA > 1) cluster_sync_all(); else __syncthreads();
     if (warp == 1) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+        if (NCTA == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+        else asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
     }
 }
 
@@ -306,24 +370,44 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return AJT_ERR_CUDA;
         encode = reinterpret_cast<EncodeTiledFn>(fn);
     }
+    const int ncta = T > kBM ? 2 : 1;   // CTA pairs (256-row blocks) unless a single 128-row block holds everything
     CUtensorMap map_h, map_w;
-    if (!make_map(encode, &map_h, hidden, T, d, ld_hidden, kBM) || !make_map(encode, &map_w, weight, V, d, ld_weight, kBN))
+    if (!make_map(encode, &map_h, hidden, T, d, ld_hidden, kBM) || !make_map(encode, &map_w, weight, V, d, ld_weight, kBN / ncta))
         return AJT_ERR_CUDA;
 
     LmParams p;
     p.targets = targets; p.mask = mask; p.T = T; p.d = d; p.V = V;
-    p.n_mtiles = (int)((T + kBM - 1) / kBM);
+    p.n_mtiles = (int)((T + kBM * ncta - 1) / (kBM * ncta));   // row blocks of 128 * ncta rows
     const int nvs = V >= kVS * kBN ? kVS : 1;   // small vocabularies: one range
     p.vs_len = (((V + nvs - 1) / nvs + kBN - 1) / kBN) * kBN;
-    p.mgroup = num_sms / kVS;
+    p.mgroup = (num_sms / ncta) / kVS;
     if (p.mgroup > p.n_mtiles) p.mgroup = p.n_mtiles;
     p.part = reinterpret_cast<float4*>(workspace);
     p.logp_out = logp_out; p.ent_out = ent_out;
     if (nvs == 1) p.vs_len = ((V + kBN - 1) / kBN) * kBN;
 
-    if (cudaFuncSetAttribute(lm_head_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLmSmem) != cudaSuccess) return AJT_ERR_CUDA;
     // ranges beyond nvs are empty (v0 >= V): their CTAs have nothing to do, and the combine reads nvs partials per row
-    lm_head_kernel<<<p.mgroup * kVS, kLmThreads, kLmSmem, stream>>>(map_h, map_w, p);
+    if (ncta == 1) {
+        if (cudaFuncSetAttribute(lm_head_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<1>::kSmem) != cudaSuccess)
+            return AJT_ERR_CUDA;
+        lm_head_kernel<1><<<p.mgroup * kVS, kLmThreads, LmCfg<1>::kSmem, stream>>>(map_h, map_w, p);
+    } else {
+        if (cudaFuncSetAttribute(lm_head_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<2>::kSmem) != cudaSuccess)
+            return AJT_ERR_CUDA;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(p.mgroup * kVS * 2));
+        cfg.blockDim = dim3(kLmThreads);
+        cfg.dynamicSmemBytes = LmCfg<2>::kSmem;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        if (cudaLaunchKernelEx(&cfg, lm_head_kernel<2>, map_h, map_w, p) != cudaSuccess) return AJT_ERR_CUDA;
+    }
     const int64_t want = (T + 255) / 256;
     lm_head_combine_kernel<<<(int)(want < (int64_t)num_sms * 4 ? want : (int64_t)num_sms * 4), 256, 0, stream>>>(p, nvs);
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
