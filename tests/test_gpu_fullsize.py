@@ -207,3 +207,33 @@ def test_c3_chunk_with_real_merge_vectors():
     ref = oracle.policy_loss(bits, tg, old, av, mk, sg, S, e, e, seg_denom=Ns, inv_num_segs=inv, row_ids=rows, logits_is_bf16_bits=True)
     check_loss(out, ref, mk, 0.2, 0.2, av, old, 1.0, V, row_ids=rows, check_scalar=False)
     anysize_properties(out, d(mk), V)
+
+
+def test_lm_head_full_size_sampled_rows():
+    """ajt_lm_head_logp at the size sweep `h1` times (40,960 x 4,096 x 151,936: CTA pairs, 9 waves of row blocks, 4 vocabulary
+    ranges of 149 tiles): sampled rows against the fp64 oracle computed row by row; every row finite and a valid log-prob."""
+    T, d, V = 40960, 4096, 151936
+    g = torch.Generator(device="cuda").manual_seed(41)
+    Hh = torch.randn((T, d), generator=g, device="cuda").to(torch.bfloat16)
+    Ww = (torch.randn((V, d), generator=g, device="cuda") * 0.02).to(torch.bfloat16)
+    y = torch.randint(0, V, (T,), generator=g, device="cuda", dtype=torch.int32)
+    logp, ent = ajt.lm_head_logp(Hh, Ww, y)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(logp).all()) and bool(torch.isfinite(ent).all())
+    assert float(logp.max()) <= 1e-6 and float(ent.min()) >= 0.0 and float(ent.max()) <= np.log(V) + 1e-4
+    rng = np.random.default_rng(2)
+    rows = np.unique(np.concatenate([[0, 127, 128, 255, 256, T - 1], rng.choice(T, size=48, replace=False)]))
+    rt = torch.from_numpy(rows).cuda()
+    wb = bf16_bits(Ww)
+    rl, re = oracle.lm_head_logp(bf16_bits(Hh[rt]), wb, y[rt].cpu().numpy())
+    # |z| ~ 1.3 here and d = 4096: fp32 accumulation error ~ sqrt(d) 2^-24 |z| ~ 5e-6; 5e-5 absolute leaves room for the tails
+    assert np.abs(logp[rt].cpu().numpy().astype(np.float64) - rl).max() <= 5e-5
+    assert np.abs(ent[rt].cpu().numpy().astype(np.float64) - re).max() <= 5e-5
+
+
+def test_merge_blocks_full_size_b3():
+    """ajt_merge_blocks on the full b3 workload (7,805 timelines, 253,556 blocks, 145.6 M tokens), bit-exact in every output."""
+    from test_gpu_blocks import as_dict, run
+    bi = W.block_workload("b3")
+    g, r, _ = run(as_dict(bi))
+    assert g.N_out > 20_000_000 and g.M < bi.n // 5
