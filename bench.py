@@ -447,7 +447,8 @@ def run_e2e(torch, ajt, mi, mb, S, Ns, inv, T, dev, stream, K, Wm, step_bytes, b
     ms = max_over_ranks(e0.elapsed_time(e1)) / Ke
     assert res["merge"]["status"] == 0 and res["loss"]["status"] == 0
     No, M, n, N = res["merge"]["N_out"], res["merge"]["M"], mi.n, mi.n_tokens
-    h2d = 4 * N + 8 * (n + 1) + 4 * n + 4 * n + 4 * N + T * V * 2 + 17 * T + 4 * S
+    n_up = int(mb["n_unmasked"])   # the host call uploads only the rows the kernel reads (mask != 0)
+    h2d = 4 * N + 8 * (n + 1) + 4 * n + 4 * n + 4 * N + n_up * V * 2 + 17 * T + 4 * S
     d2h = No * (4 + 1 + 4 + 4) + 8 * (M + 1) + 4 * M + 4 * M + 4 * n + 16 + 4 + T * V * 2 + 4 + 4
     return {"value": sum_over_ranks(float(step_bytes)) / (ms * 1e-3) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": int(h2d),
             "d2h_bytes_per_step": int(d2h), "ms_per_step": ms, "steps": Ke,

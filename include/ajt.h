@@ -287,7 +287,7 @@ int ajt_segment_counts(const uint8_t* mask /* DEVICE [T] */, const int32_t* seg_
 /* HOST-buffer variant.  `arena` is DEVICE scratch of at least ajt_loss_host_arena_bytes(T, V, S, ld, dtype) bytes.
  * The per-token vectors go up first and the batch-wide normalisers are counted on the device; the matrix is cut into up
  * to 16 row slabs whose H2D copy, loss call and D2H copy overlap with their neighbours' (both PCIe directions busy at
- * once).  For that the call creates two helper streams and their events and destroys them before it returns: the only
+ * once); rows with mask 0 are not copied up, since the kernel never reads them.  For that the call creates two helper streams and their events and destroys them before it returns: the only
  * resources the library ever creates.  dlogits / logp rows are those of the device call; loss and stats[3] are the fp64
  * sums of the slabs' fp32 partials.  Pinned host buffers are needed for the overlap.  Synchronises. */
 size_t ajt_loss_host_arena_bytes(int64_t T, int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype);

@@ -145,8 +145,16 @@ extern "C" int ajt_policy_loss_fwd_bwd_host(const void* logits, const int32_t* t
         const int64_t r0 = i * rows_per, r1 = (r0 + rows_per < T) ? r0 + rows_per : T;
         if (r1 <= r0) break;
         const int64_t R = r1 - r0;
-        AJT_CP(d + a.logits + (size_t)r0 * ld * esz, (const uint8_t*)logits + (size_t)r0 * ld * esz, (size_t)R * ld * esz,
-               cudaMemcpyHostToDevice, s_up);
+        // only the rows the kernel reads go up: runs of consecutive rows with mask != 0 (the mask is host memory here)
+        for (int64_t r = r0; r < r1;) {
+            while (r < r1 && mask[r] == 0) ++r;
+            int64_t e = r;
+            while (e < r1 && mask[e] != 0) ++e;
+            if (e > r)
+                AJT_CP(d + a.logits + (size_t)r * ld * esz, (const uint8_t*)logits + (size_t)r * ld * esz, (size_t)(e - r) * ld * esz,
+                       cudaMemcpyHostToDevice, s_up);
+            r = e;
+        }
         AJT_TRY(cudaEventRecord(ev_up[i], s_up));
         AJT_TRY(cudaStreamWaitEvent(s, ev_up[i], 0));
         if (rc != AJT_OK) break;
