@@ -356,6 +356,28 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     value = sum_over_ranks(step_bytes) / (ms_per_step * 1e-3) / 1e9
     peak, peak_src = measured_peak()
 
+    # ---- HBM ceilings of this box, measured now with the library's probe kernels; dlogits is scratch here
+    ceilings = None
+    if rank == 0:
+        nb = (int(dlogits.numel()) * 2) & ~15
+        sink = torch.zeros(4, dtype=torch.int32, device=dev)
+
+        def probe(mode, dst, src, moved):
+            best = 1e30
+            with torch.cuda.stream(stream):
+                for _ in range(4):
+                    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a0.record(stream)
+                    ajt.hbm_probe(dst, src, nb, mode, stream=stream)
+                    a1.record(stream)
+                    stream.synchronize()
+                    best = min(best, a0.elapsed_time(a1))
+            return moved / (best * 1e-3) / 1e9
+
+        ceilings = {"read_gb_per_s": probe(0, sink, mbs[0]["logits"], nb), "write_gb_per_s": probe(1, dlogits, None, nb),
+                    "memset_gb_per_s": probe(3, dlogits, None, nb), "copy_gb_per_s": probe(2, dlogits, mbs[0]["logits"], 2 * nb),
+                    "bytes": nb, "how": "ajt_hbm_probe (16-byte loads / stores over the 12.4 GB logits / dlogits buffers, best of 4)"}
+
     # ---- e2e: the *_host C-ABI calls, pinned HOST buffers, H2D + D2H inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -396,7 +418,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             "roofline": {"bound": "hbm", "kernel": "loss_rows_kernel (timed as the ajt_policy_loss_fwd_bwd call: prep + rows + "
                          "final launches; rows is >99% of it, profiles/)", "achieved": ach, "peak": peak, "unit": "GB/s",
                          "frac": ach / peak, "traffic": traffic, "peak_source": peak_src},
-            "clocks": clocks, "gpu_launches": K * (6 + 1 + 1 + 3),   # merge 6, pack 1, segment counts 1, loss 3 (prep, rows, final)
+            "hbm_ceilings": ceilings, "clocks": clocks, "gpu_launches": K * (6 + 1 + 1 + 3),   # merge 6, pack 1, segment counts 1, loss 3 (prep, rows, final)
             "e2e": e2e, "cpu_baseline": cpu_baseline,
             "paper_context": "paper reports only end-to-end actor-update 2160 s -> 346 s (6.25x) with merging on AppWorld, "
                              "8-GPU node at most, GPU model and precision not stated (PAPER.md:373,395); not comparable",

@@ -300,6 +300,12 @@ int ajt_policy_loss_fwd_bwd_host(
     float* stats_out /* HOST [4] or NULL */, uint32_t* status_bits /* HOST [1] or NULL */,
     void* arena /* DEVICE */, size_t arena_bytes, ajt_stream_t stream);
 
+/* Measurement helper ("a micro-benchmark for read-only, write-only and copy HBM ceilings on the same box"):
+ * streams `bytes` (multiple of 16, 16-byte aligned DEVICE buffers) with 16-byte accesses.  mode 0: read `src` (dst = a DEVICE
+ * word that is practically never written, may alias anything), 1: write zeros to `dst`, 2: copy src -> dst, 3: cudaMemsetAsync
+ * of `dst`.  Not part of the method. */
+int ajt_hbm_probe(void* dst, const void* src, size_t bytes, int32_t mode, ajt_stream_t stream);
+
 #ifdef __cplusplus
 }
 #endif

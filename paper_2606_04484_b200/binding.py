@@ -27,6 +27,7 @@ _EXPORTS = [
     "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
     "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks_workspace_bytes", "ajt_merge_blocks",
     "ajt_pack_loss_inputs", "ajt_lm_head_workspace_bytes", "ajt_lm_head_logp",
+    "ajt_hbm_probe",
 ]
 
 _lib = None
@@ -71,7 +72,7 @@ def lib():
         L.ajt_loss_host_arena_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32]
         for f in ("ajt_merge_timelines", "ajt_merge_timelines_host", "ajt_policy_loss_fwd_bwd",
                   "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks",
-                  "ajt_pack_loss_inputs", "ajt_lm_head_logp"):
+                  "ajt_pack_loss_inputs", "ajt_lm_head_logp", "ajt_hbm_probe"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -477,6 +478,14 @@ def lm_head_logp(hidden: torch.Tensor, weight: torch.Tensor, targets: torch.Tens
     if rc != 0:
         raise AjtError(rc, "ajt_lm_head_logp")
     return logp[:T], (None if ent is None else ent[:T])
+
+
+def hbm_probe(dst: Optional[torch.Tensor], src: Optional[torch.Tensor], nbytes: int, mode: int, stream=None) -> None:
+    """ajt_hbm_probe (include/ajt.h): 0 read src, 1 write dst, 2 copy src -> dst, 3 cudaMemsetAsync(dst)."""
+    _require_cuda()
+    rc = lib().ajt_hbm_probe(_dp(dst), _dp(src), C.c_size_t(nbytes), C.c_int32(mode), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_hbm_probe")
 
 
 def segment_counts(mask: torch.Tensor, seg_ids: torch.Tensor, S: int, out: Optional[torch.Tensor] = None,

@@ -28,6 +28,50 @@ extern "C" int ajt_last_status(const void* workspace, ajt_stream_t stream, uint3
     return AJT_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ HBM ceilings (measurement)
+
+namespace {
+__global__ void __launch_bounds__(256) probe_read_kernel(const uint4* __restrict__ src, size_t n16, uint32_t* sink) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    uint32_t acc = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) {
+        uint4 v;
+        asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(src + i));
+        acc ^= v.x ^ v.y ^ v.z ^ v.w;
+    }
+    if (acc == 0x9E3779B9u) *sink = acc;   // keeps the loads alive; practically never taken
+}
+__global__ void __launch_bounds__(256) probe_write_kernel(uint4* __restrict__ dst, size_t n16) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) ajt::stg128_stream(dst + i, make_uint4(0, 0, 0, 0));
+}
+__global__ void __launch_bounds__(256) probe_copy_kernel(uint4* __restrict__ dst, const uint4* __restrict__ src, size_t n16) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) {
+        uint4 v;
+        asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(src + i));
+        ajt::stg128_stream(dst + i, v);
+    }
+}
+}  // namespace
+
+extern "C" int ajt_hbm_probe(void* dst, const void* src, size_t bytes, int32_t mode, ajt_stream_t stream_) {
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(stream_);
+    if (mode < 0 || mode > 3 || (bytes & 15) || ((mode != 0) && (!dst || ((uintptr_t)dst & 15))) ||
+        ((mode == 0 || mode == 2) && (!src || ((uintptr_t)src & 15))))
+        return AJT_ERR_INVALID_ARG;
+    int dev = 0, num_sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AJT_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || num_sms < 1) return AJT_ERR_CUDA;
+    const size_t n16 = bytes / 16;
+    const int grid = num_sms * 32;
+    if (mode == 0) probe_read_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<const uint4*>(src), n16, reinterpret_cast<uint32_t*>(dst));
+    else if (mode == 1) probe_write_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<uint4*>(dst), n16);
+    else if (mode == 2) probe_copy_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<uint4*>(dst), reinterpret_cast<const uint4*>(src), n16);
+    else if (cudaMemsetAsync(dst, 0, bytes, s) != cudaSuccess) return AJT_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
+}
+
 // ------------------------------------------------------------------------------------------------ loss, host buffers
 
 namespace {

@@ -238,6 +238,11 @@ def stock_bandwidth(dev, out):
         t = float(np.min(ts))
         _emit(out, stage="stock_bandwidth", what=name, ms_best=t, bytes=nbytes, gb_per_s=nbytes / t / 1e6)
 
+    sink = torch.zeros(4, dtype=torch.int32, device=dev)
+    run(lambda: ajt.hbm_probe(sink, a, 2 * n, 0), "ajt_hbm_probe read 12.9 GB (ld.global.v4)", 2 * n)
+    run(lambda: ajt.hbm_probe(a, None, 2 * n, 1), "ajt_hbm_probe write 12.9 GB (st.global.v4)", 2 * n)
+    run(lambda: ajt.hbm_probe(a, None, 2 * n, 3), "cudaMemsetAsync 12.9 GB", 2 * n)
+    run(lambda: ajt.hbm_probe(b, a, 2 * n, 2), "ajt_hbm_probe copy 12.9 GB -> 12.9 GB", 4 * n)
     run(lambda: a.zero_(), "zero_ 12.9 GB (write only)", 2 * n)
     run(lambda: a.fill_(1.0), "fill_ 12.9 GB (write only)", 2 * n)
     run(lambda: b.copy_(a), "copy_ 12.9 GB -> 12.9 GB (read + write)", 4 * n)
