@@ -6,9 +6,10 @@
 //                                group start, rank, first key slot}, lengths in group order
 //   K2 merge_hash_kernel     M2  warp-cooperative prefix-hash scan, 128-bit loads, 4 vectors in flight per lane.  The hash of
 //                                the first p tokens of timeline i is F_i(p) = sum_{q<p} x_q w(q) mod 2^64, w(q) = B^(q+3) mod 2^32: a sum, hence
-//                                a monoid, so every lane keeps its own partial and lanes are only combined (shuffles) where a
-//                                key is emitted: at each length L_a of an earlier same-group timeline (probe key) and at L_i
-//                                itself (full key)
+//                                a monoid, so every lane keeps its own partial and lanes are only combined (three REDUX)
+//                                where a key is emitted: at each length L_a of an earlier same-group timeline (probe key)
+//                                and at L_i itself (full key).  The positions shared with the in-group predecessor are
+//                                compared exactly on the way (the predecessor was just hashed: L2 hits)
 //   K3 merge_select_kernel   M2  (one CTA per group) per-timeline prefix over its hash windows -> final (hash, len) keys
 //                            M3  segmented radix sort of the group's keys by a 32-bit digest: one MSD pass on the top 11 bits
 //                                in shared memory (<= 2048 keys: a bucket then holds the equal-key run, mean occupancy < 1,
@@ -16,10 +17,12 @@
 //   K4   (same kernel)       M4  per full key: walk its equal-key run, pick the extender by the owner rule
 //   K6 merge_compact_kernel  M6  one CTA, one fused scan: survivors in original order -> merged_offsets/origin/traj, owner,
 //                                tile table
-//   K5/K7 merge_scatter_kernel M5+M7  fused: every merged sequence is streamed once in 512-token warp tiles; each absorbed
-//                                member is compared token-by-token against its owner (exact verification) while tokens /
-//                                mask-OR / src / old_logp are written with 16-byte stores.  A mismatch (a hash collision)
-//                                raises ctrl->collision.
+//   K5/K7 merge_scatter_kernel M5+M7  fused: every merged sequence is streamed once in 256-position warp tiles; a member whose
+//                                containment is not already implied by verified predecessor links (K2) is compared
+//                                token-by-token against its owner (exact verification) while tokens / mask-OR / src /
+//                                old_logp are written with 16-byte stores; tiles that every response region covers or
+//                                misses are plain copies from one source.  A mismatch (a hash collision) raises
+//                                ctrl->collision.
 //   merge_repair_kernel      M5  one cooperative launch that exits at once unless ctrl->collision: K4 with exact comparison of
 //                                every candidate it accepts, grid barrier, K6, grid barrier, K7.  Hash collisions can therefore
 //                                never change the result.
