@@ -259,9 +259,10 @@ int ajt_policy_loss_fwd_bwd_ext(
  * Log-prob and entropy of the target token straight from the hidden states (the forward half of fusing the LM head
  * with the loss; the pass that yields the old / reference log-probs the loss consumes, PAPER.md:136,
  * 172-176):
- *   z_t = W h_t;   logp_out[t] = z_{t,y_t} - logsumexp_v z_tv;   ent_out[t] = logsumexp_v z_tv - sum_v softmax(z_t)_v z_tv
+ *   z_t = W h_t;   lse_t = logsumexp_v z_tv;   logp_out[t] = z_{t,y_t} - lse_t;   ent_out[t] = lse_t - sum_v softmax(z_t)_v z_tv;
+ *   lse_out[t] = lse_t (what a later backward pass needs to recompute softmax tiles)
  * hidden DEVICE [T, ld_hidden] bf16 (columns [0,d)), weight DEVICE [V, ld_weight] bf16, targets DEVICE [T] in [0,V),
- * mask DEVICE [T] or NULL (rows with mask 0 give 0, 0).  The [T, V] logits are never written: tiles of 128 x 256 are
+ * mask DEVICE [T] or NULL (rows with mask 0 give 0, 0, 0).  The [T, V] logits are never written: tiles of 128 x 256 are
  * produced by tcgen05.mma (bf16 x bf16 -> fp32 in tensor memory) and reduced on the fly.  Arithmetic: fp32.
  * Requires d % 64 == 0, ld % 8 == 0 and 16-byte aligned bases (AJT_ERR_UNSUPPORTED otherwise).
  * Workspace: ajt_lm_head_workspace_bytes(T, V) bytes of DEVICE memory, 256-byte aligned. */
@@ -269,7 +270,7 @@ size_t ajt_lm_head_workspace_bytes(int64_t T, int32_t V);
 
 int ajt_lm_head_logp(const void* hidden, const void* weight, const int32_t* targets, const uint8_t* mask, int64_t T, int32_t d,
                      int32_t V, int64_t ld_hidden, int64_t ld_weight, float* logp_out, float* ent_out /* or NULL */,
-                     void* workspace, size_t workspace_bytes, ajt_stream_t stream);
+                     float* lse_out /* or NULL */, void* workspace, size_t workspace_bytes, ajt_stream_t stream);
 
 /* Batch-wide per-trajectory normalisers for callers that stream the batch through several loss calls
  * (micro-batches, 64k-row chunks, or rows of one trajectory spread over several GPUs; reading L-4;

@@ -457,8 +457,9 @@ def policy_loss_fwd_bwd_ext(logits: torch.Tensor, targets: torch.Tensor, old_log
 
 
 def lm_head_logp(hidden: torch.Tensor, weight: torch.Tensor, targets: torch.Tensor, mask: Optional[torch.Tensor] = None,
-                 want_entropy: bool = True, workspace: Optional[torch.Tensor] = None, stream=None):
-    """ajt_lm_head_logp (include/ajt.h): (logp f32 [T], entropy f32 [T] | None) from hidden [T, d] and weight [V, d] (bf16)."""
+                 want_entropy: bool = True, workspace: Optional[torch.Tensor] = None, stream=None, want_lse: bool = False):
+    """ajt_lm_head_logp (include/ajt.h): (logp f32 [T], entropy f32 [T] | None) from hidden [T, d] and weight [V, d] (bf16);
+    with want_lse also the row log-sum-exps as a third element."""
     _require_cuda()
     _check_dev(hidden, torch.bfloat16, "hidden")
     _check_dev(weight, torch.bfloat16, "weight")
@@ -470,13 +471,16 @@ def lm_head_logp(hidden: torch.Tensor, weight: torch.Tensor, targets: torch.Tens
     dev = hidden.device
     logp = torch.empty(max(T, 1), dtype=torch.float32, device=dev)
     ent = torch.empty(max(T, 1), dtype=torch.float32, device=dev) if want_entropy else None
+    lse = torch.empty(max(T, 1), dtype=torch.float32, device=dev) if want_lse else None
     if workspace is None:
         workspace = torch.empty(int(lib().ajt_lm_head_workspace_bytes(C.c_int64(T), C.c_int32(V))) + 256, dtype=torch.uint8, device=dev)
     rc = lib().ajt_lm_head_logp(_dp(hidden), _dp(weight), _dp(targets), _dp(mask), C.c_int64(T), C.c_int32(d), C.c_int32(V),
                                 C.c_int64(int(hidden.stride(0)) if T > 1 else d), C.c_int64(int(weight.stride(0)) if V > 1 else d),
-                                _dp(logp), _dp(ent), _dp(workspace), C.c_size_t(workspace.numel()), _stream(stream))
+                                _dp(logp), _dp(ent), _dp(lse), _dp(workspace), C.c_size_t(workspace.numel()), _stream(stream))
     if rc != 0:
         raise AjtError(rc, "ajt_lm_head_logp")
+    if want_lse:
+        return logp[:T], (None if ent is None else ent[:T]), lse[:T]
     return logp[:T], (None if ent is None else ent[:T])
 
 

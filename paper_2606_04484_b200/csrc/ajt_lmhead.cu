@@ -45,6 +45,7 @@ struct LmParams {
     float4* part;                             // [T][kVS] {m, s, u, z_y (or -inf)}
     float* logp_out;
     float* ent_out;
+    float* lse_out;
 };
 
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
@@ -301,7 +302,7 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
 __global__ void __launch_bounds__(256) lm_head_combine_kernel(const LmParams p, int nvs) {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < p.T; t += stride) {
-        float lp = 0.f, H = 0.f;
+        float lp = 0.f, H = 0.f, lse = 0.f;
         if (!p.mask || p.mask[t] != 0) {
             float4 q[kVS];
             float M = -INFINITY, zy = -INFINITY;
@@ -320,9 +321,11 @@ __global__ void __launch_bounds__(256) lm_head_combine_kernel(const LmParams p, 
             const float logS = logf(S);
             lp = (zy - M) - logS;
             H = logS - U / S;
+            lse = M + logS;
         }
         p.logp_out[t] = lp;
         if (p.ent_out) p.ent_out[t] = H;
+        if (p.lse_out) p.lse_out[t] = lse;
     }
 }
 
@@ -349,7 +352,7 @@ extern "C" size_t ajt_lm_head_workspace_bytes(int64_t T, int32_t V) {
 
 extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const int32_t* targets, const uint8_t* mask, int64_t T,
                                 int32_t d, int32_t V, int64_t ld_hidden, int64_t ld_weight, float* logp_out, float* ent_out,
-                                void* workspace, size_t workspace_bytes, ajt_stream_t stream_) {
+                                float* lse_out, void* workspace, size_t workspace_bytes, ajt_stream_t stream_) {
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
     if (T < 0 || d <= 0 || V <= 0 || ld_hidden < d || ld_weight < d) return AJT_ERR_INVALID_ARG;
     if (!logp_out || !workspace) return AJT_ERR_INVALID_ARG;
@@ -383,7 +386,7 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
     p.mgroup = (num_sms / ncta) / kVS;
     if (p.mgroup > p.n_mtiles) p.mgroup = p.n_mtiles;
     p.part = reinterpret_cast<float4*>(workspace);
-    p.logp_out = logp_out; p.ent_out = ent_out;
+    p.logp_out = logp_out; p.ent_out = ent_out; p.lse_out = lse_out;
     if (nvs == 1) p.vs_len = ((V + kBN - 1) / kBN) * kBN;
 
     // ranges beyond nvs are empty (v0 >= V): their CTAs have nothing to do, and the combine reads nvs partials per row

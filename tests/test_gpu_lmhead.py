@@ -53,6 +53,20 @@ def test_peaked_rows():
     run(256, 256, 4096, seed=9, wscale=0.5)                          # |z| up to ~30: the online re-basing matters
 
 
+def test_row_lse_output():
+    g = torch.Generator(device="cuda").manual_seed(3)
+    H = torch.randn((200, 128), generator=g, device="cuda").to(torch.bfloat16)
+    W = (torch.randn((3000, 128), generator=g, device="cuda") * 0.1).to(torch.bfloat16)
+    y = torch.randint(0, 3000, (200,), generator=g, device="cuda", dtype=torch.int32)
+    logp, ent, lse = ajt.lm_head_logp(H, W, y, want_lse=True)
+    torch.cuda.synchronize()
+    z = H.double() @ W.double().T
+    want = torch.logsumexp(z, dim=-1)
+    assert float((lse.double() - want).abs().max()) <= 3e-5
+    zy = z.gather(1, y.long()[:, None])[:, 0]
+    assert float((logp.double() - (zy - want)).abs().max()) <= 3e-5
+
+
 def test_unsupported_shapes_are_rejected():
     H = torch.zeros((8, 48), dtype=torch.bfloat16, device="cuda")
     W = torch.zeros((16, 48), dtype=torch.bfloat16, device="cuda")
