@@ -37,6 +37,9 @@ def run(T, d, V, seed=0, mask_frac=None, wscale=0.05):
 
 @pytest.mark.parametrize("T,d,V", [
     (128, 64, 256),        # one row block, one K slab, one tile
+    (1, 64, 8),            # a single row, a vocabulary smaller than any tile (TMA boxes larger than the tensors)
+    (50, 64, 100),         # one CTA, ragged everywhere
+    (129, 128, 257),       # CTA pair with one live row in the second CTA, one column in the second tile
     (300, 256, 1000),      # ragged rows and columns, a single vocabulary range
     (257, 128, 5000),      # four vocabulary ranges, ragged last tile
     (1000, 1024, 32000),   # 8 row blocks x 4 ranges, 16 K slabs: the smem ring and both accumulators wrap many times
