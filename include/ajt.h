@@ -141,7 +141,8 @@ int ajt_merge_timelines(
  *   merged_block_src [B_out] (timeline whose block k stands at block k of the survivor), merged_block_author [B_out],
  *   merged_block_tok_off [B_out+1], merged_origin / merged_traj [M], owner [n], counts [3] = {M, B_out, N_out}.
  * All integer / byte work: bit-exact with the definition.  Workspace: ajt_merge_blocks_workspace_bytes(n, n_blocks) bytes
- * of DEVICE memory, 256-byte aligned (0 is returned for n_blocks >= 2^30).  Status bits as for ajt_merge_timelines
+ * of DEVICE memory, 256-byte aligned (0 is returned for n_blocks >= 2^30); like ajt_merge_timelines it holds 64*n + 4096
+ * candidate pairs and every extra 32 bytes the caller provides hold one more.  Status bits as for ajt_merge_timelines
  * (AJT_STATUS_BAD_OFFSETS also for a decreasing tok_off); `flags` as there.  Enqueues on `stream`, does not synchronise.
  */
 enum { AJT_AUTHOR_ENV = 0, AJT_AUTHOR_USER = 1, AJT_AUTHOR_LLM = 2 };

@@ -244,7 +244,7 @@ class BlockMergeOutput:
 def merge_blocks(block_ids: torch.Tensor, block_offsets: torch.Tensor, traj_ids: torch.Tensor, author: torch.Tensor,
                  tok_off: torch.Tensor, tokens: torch.Tensor, logp: Optional[torch.Tensor] = None,
                  tok_mask: Optional[torch.Tensor] = None, flags: int = 0, out: Optional[BlockMergeOutput] = None,
-                 stream=None) -> BlockMergeOutput:
+                 stream=None, extra_workspace_bytes: int = 0) -> BlockMergeOutput:
     """ajt_merge_blocks (include/ajt.h): Algorithm 1 with text-level matching on timelines of message blocks."""
     _require_cuda()
     _check_dev(block_ids, torch.int64, "block_ids")
@@ -262,7 +262,7 @@ def merge_blocks(block_ids: torch.Tensor, block_offsets: torch.Tensor, traj_ids:
         out = BlockMergeOutput(e(N, torch.int32), e(N, torch.uint8), None if logp is None else e(N, torch.float32),
                                e(N, torch.int32), e(n + 1, torch.int64), e(n + 1, torch.int64), e(B, torch.int32),
                                e(B, torch.uint8), e(B + 1, torch.int64), e(n, torch.int32), e(n, torch.int32), e(n, torch.int32),
-                               e(3, torch.int64), e(merge_blocks_workspace_bytes(n, B), torch.uint8))
+                               e(3, torch.int64), e(merge_blocks_workspace_bytes(n, B) + int(extra_workspace_bytes), torch.uint8))
     rc = lib().ajt_merge_blocks(
         _dp(block_ids), _dp(block_offsets), _dp(traj_ids), _dp(author), _dp(tok_off), _dp(tokens), _dp(logp), _dp(tok_mask),
         C.c_int32(n), C.c_int64(B), C.c_int64(N), C.c_uint32(flags),

@@ -63,10 +63,13 @@ struct BlockWs {
 
 __host__ inline size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-__host__ BlockWs block_ws_layout(int32_t n, int64_t B) {
+// The id-level merge's workspace comes first (its status word is the call's status word) and takes whatever the caller
+// provides beyond the minimum: more room for candidate pairs (AJT_STATUS_PROBE_CAPACITY), as for ajt_merge_timelines.
+__host__ BlockWs block_ws_layout(int32_t n, int64_t B, size_t inner_bytes = 0) {
     BlockWs w;
     size_t o = 0;
-    w.inner = o; o += a256(ajt_merge_workspace_bytes(n, 2 * B));
+    const size_t inner_min = a256(ajt_merge_workspace_bytes(n, 2 * B));
+    w.inner = o; o += inner_bytes > inner_min ? (inner_bytes & ~(size_t)255) : inner_min;
     w.offsets2 = o; o += a256(((size_t)n + 1) * 8);
     w.mask2 = o; o += a256((size_t)2 * B + 16);
     w.ids_out = o; o += a256((size_t)2 * B * 4 + 16);
@@ -212,6 +215,14 @@ __global__ void __launch_bounds__(256) blocks_scan_kernel(const BlockParams p) {
 __global__ void __launch_bounds__(256) blocks_offsets_kernel(const BlockParams p) {
     int64_t M, Bout;
     merged_counts(p, M, Bout);
+    if (fatal(p)) {   // the id-level merge stopped: its outputs are unspecified and must not be used as indices
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            p.merged_offsets[0] = 0;
+            p.merged_block_offsets[0] = 0;
+            p.counts[0] = p.counts[1] = p.counts[2] = 0;
+        }
+        return;
+    }
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t m = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; m <= M; m += stride) {
         const int64_t bo = p.offs2_out[m] >> 1;
@@ -354,8 +365,9 @@ extern "C" int ajt_merge_blocks(const int64_t* block_ids, const int64_t* block_o
     if (n_tokens > 0 && (!tokens || !merged_tokens || !merged_mask || !merged_tok_src)) return AJT_ERR_INVALID_ARG;
     if ((logp == nullptr) != (merged_logp == nullptr)) return AJT_ERR_INVALID_ARG;
     if (((uintptr_t)workspace & 255) || ((uintptr_t)block_ids & 7)) return AJT_ERR_INVALID_ARG;
-    const BlockWs ws = block_ws_layout(n, n_blocks);
-    if (workspace_bytes < ws.total) return AJT_ERR_WORKSPACE_TOO_SMALL;
+    const BlockWs ws0 = block_ws_layout(n, n_blocks);
+    if (workspace_bytes < ws0.total) return AJT_ERR_WORKSPACE_TOO_SMALL;
+    const BlockWs ws = block_ws_layout(n, n_blocks, ws0.offsets2 + (workspace_bytes - ws0.total));   // the surplus goes to the pairs
 
     int dev = 0, num_sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return AJT_ERR_CUDA;

@@ -110,6 +110,22 @@ def test_empty_blocks_and_single_timeline():
     run(pack([[[1, 2, [3]]]], [0]))
 
 
+def test_probe_capacity_and_larger_workspace():
+    # one group of 220 timelines: 24,310 (timeline, earlier length) pairs > the 64 n + 4096 the default workspace holds
+    tls = [[[7, 1, [1]]] + [[100 + k, 2 if k == j else 0, [k]] for k in range(j + 1)] for j in range(220)]
+    from test_oracle_blocks import pack
+    x = pack(tls, [3] * 220)
+    g, status = gpu_blocks(x)
+    assert status & ajt.STATUS_PROBE_CAPACITY
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    out = ajt.merge_blocks(d(x["block_ids"]), d(x["block_offsets"]), d(x["traj_ids"]), d(x["author"]), d(x["tok_off"]), d(x["tokens"]),
+                           d(x["logp"]), extra_workspace_bytes=32 * 24310)
+    assert ajt.last_status(out.workspace) == 0
+    r = oracle.merge_blocks(x["block_ids"], x["block_offsets"], x["traj_ids"], x["author"], x["tok_off"], x["tokens"], x["logp"])
+    assert_equal(out.finalize(), r)
+    assert r.M == 1
+
+
 def test_bad_offsets_set_status():
     bi = W.block_workload("b1")
     x = as_dict(bi)
