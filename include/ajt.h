@@ -96,7 +96,9 @@ int ajt_last_status(const void* workspace, ajt_stream_t stream, uint32_t* bits);
  * that sets AJT_STATUS_PROBE_CAPACITY — pass a larger workspace (every extra 32 bytes hold one more pair).
  *
  * All integer; outputs are bit-exact with the definition.  Only the first N_out / M entries of the
- * outputs are written.  `counts` is DEVICE memory: synchronise the stream before reading it.
+ * outputs are written.  `counts` is DEVICE memory: synchronise the stream before reading it.  After a fatal status
+ * (bad offsets, zero-length timeline, pair capacity) the outputs are unspecified except counts = {0, 0}, so that a chained
+ * call (ajt_pack_loss_inputs) does nothing.
  */
 size_t ajt_merge_workspace_bytes(int32_t n, int64_t n_tokens);
 

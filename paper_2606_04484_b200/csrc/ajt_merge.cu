@@ -1138,7 +1138,10 @@ __device__ void compact_body(const MergeParams& p, int mode, int64_t (*s_w)[2][N
 
 __global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p) {
     __shared__ int64_t s_w[2][2][32];
-    if (fatal(p)) return;
+    if (fatal(p)) {   // outputs are unspecified after a fatal status, but the counts a caller may chain on are not garbage
+        if (threadIdx.x == 0) { p.counts[0] = 0; p.counts[1] = 0; }
+        return;
+    }
     compact_body<1024>(p, 0, s_w);
 }
 

@@ -22,6 +22,7 @@ struct PackParams {
     const int32_t* tl_seg;
     const float* seg_adv;
     const int64_t* counts;
+    int64_t cap;
     int32_t S;
     int32_t* targets;
     uint8_t* mask;
@@ -43,7 +44,7 @@ __device__ __forceinline__ int64_t last_le(const int64_t* __restrict__ a, int64_
 
 __global__ void __launch_bounds__(256) pack_loss_inputs_kernel(const PackParams p) {
     const int64_t M = p.counts[0], N = p.counts[1];
-    if (M <= 0 || N <= 0) return;
+    if (M <= 0 || N <= 0 || N > p.cap) return;   // nothing merged, or counts that cannot belong to these arrays
     const int lane = threadIdx.x & 31;
     const int64_t wglobal = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
     const int64_t ntiles = (N + kPackTile - 1) / kPackTile;
@@ -140,7 +141,7 @@ extern "C" int ajt_pack_loss_inputs(const int32_t* merged_tokens, const uint8_t*
     PackParams p;
     p.merged_tokens = merged_tokens; p.merged_mask = merged_mask; p.merged_old_logp = merged_old_logp;
     p.merged_offsets = merged_offsets; p.merged_origin = merged_origin; p.tl_seg = tl_seg; p.seg_adv = seg_adv; p.counts = counts;
-    p.S = S; p.targets = targets; p.mask = mask; p.old_logp = old_logp; p.seg_ids = seg_ids; p.adv = adv; p.status = status_bits;
+    p.cap = capacity_tokens; p.S = S; p.targets = targets; p.mask = mask; p.old_logp = old_logp; p.seg_ids = seg_ids; p.adv = adv; p.status = status_bits;
     const int64_t want = (capacity_tokens + 8 * kPackTile - 1) / (8 * kPackTile);
     const int grid = (int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8);
     pack_loss_inputs_kernel<<<grid, 256, 0, stream>>>(p);

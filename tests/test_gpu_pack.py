@@ -91,3 +91,17 @@ def test_device_resident_chain_c1():
                                             tl_seg.astype(np.int32), advt)
     ref = oracle.policy_loss(logits.cpu().numpy(), t, old.cpu().numpy(), a, m, s, S, float(np.float32(0.2)), float(np.float32(0.2)))
     check_loss(out, ref, m, 0.2, 0.2, a, old.cpu().numpy(), 1.0, V)
+
+
+def test_fatal_merge_status_leaves_zero_counts_and_pack_does_nothing():
+    mi = W.merge_workload("c1")
+    off = mi.offsets.copy()
+    off[5] = off[4]                      # a zero-length timeline
+    d = lambda a: torch.from_numpy(a).cuda()
+    mo = ajt.merge_timelines(d(mi.tokens), d(off), d(mi.traj_ids), d(mi.resp_start), None, d(mi.old_logp))
+    assert ajt.last_status(mo.workspace) & (ajt.STATUS_ZERO_LEN | ajt.STATUS_BAD_OFFSETS)
+    assert mo.counts.cpu().tolist() == [0, 0]
+    uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
+    pk = ajt.pack_loss_inputs(mo, d(tl_seg.astype(np.int32)), int(uniq.shape[0]))
+    torch.cuda.synchronize()
+    assert int(pk.status[0]) == 0
