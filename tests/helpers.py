@@ -83,8 +83,10 @@ def check_loss(out, ref: "oracle.LossResult", logits_rows_mask, eps_lo, eps_hi, 
            ((A < 0) & (np.abs(ratio - (1 - float(np.float32(eps_lo)))) < 1e-5))
     ok = m & ~near
     err = np.abs(d_gpu[ok] - d_ref[ok])
-    # (a) the literal north_star bound
-    assert err.size == 0 or err.max() <= 2e-3, err.max()
+    # (a) the literal north_star bound, where bf16 storage can meet it at all: |dlogits| < 1 (a bf16 half-ulp is 2^-9 = 1.95e-3
+    # just below 1 and doubles with every binade above it; reading L-9)
+    lit = err[np.abs(d_ref[ok]) < 1.0]
+    assert lit.size == 0 or lit.max() <= 2e-3, lit.max()
     # (b) the bound with teeth (reading L-9): half-ulp bf16 rounding + fp32 slack, relative
     tol = 2.0 ** -8 * np.abs(d_ref[ok]) + 1e-10 * max(1.0, abs(grad_scale))
     if err.size:
@@ -107,5 +109,9 @@ def check_loss(out, ref: "oracle.LossResult", logits_rows_mask, eps_lo, eps_hi, 
             assert st[0] == ref.stats[0]
             n_near = int(near.sum())
             assert abs(st[1] - ref.stats[1]) <= n_near and abs(st[2] - ref.stats[2]) <= n_near
-            assert abs(st[3] - ref.stats[3]) <= 1e-5 * max(1e-3, float(np.sum(ref.w * np.abs(ref.logp - old_logp[rows]))))
+            # sum_t w_t (-(logp_t - old_t)): every log-ratio carries the fp32 error of logp_t itself (the 2e-6 max(1, |logp|)
+            # bound checked above), which does not average out when few rows are unmasked
+            tol3 = float(np.sum(ref.w * 2e-6 * np.maximum(1.0, np.abs(ref.logp)))) + \
+                1e-5 * max(1e-3, float(np.sum(ref.w * np.abs(ref.logp - old_logp[rows]))))
+            assert abs(st[3] - ref.stats[3]) <= tol3, (st[3], ref.stats[3], tol3)
     return dict(max_err=float(err.max()) if err.size else 0.0, n_near=int(near.sum()))

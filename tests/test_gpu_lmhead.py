@@ -28,7 +28,10 @@ def run(T, d, V, seed=0, mask_frac=None, wscale=0.05):
     rl, re = oracle.lm_head_logp(bits(H), bits(W), y.cpu().numpy(), None if mask is None else mask.cpu().numpy())
     el = np.abs(logp.cpu().numpy().astype(np.float64) - rl).max()
     ee = np.abs(ent.cpu().numpy().astype(np.float64) - re).max()
-    assert el <= 3e-5 and ee <= 3e-5, (el, ee)
+    # fp32 accumulation error of a logit ~ sqrt(d) 2^-24 |z| with |z| ~ wscale sqrt(d) (a few times that in the tails, which
+    # is where the maximum and usually the target sit): 3e-5 absolute while wscale sqrt(d) <= 2, proportionally more above
+    tol = 3e-5 * max(1.0, wscale * np.sqrt(d) / 2.0)
+    assert el <= tol and ee <= tol, (el, ee, tol)
     if mask is not None:
         off = mask.cpu().numpy() == 0
         assert np.all(logp.cpu().numpy()[off] == 0) and np.all(ent.cpu().numpy()[off] == 0)
