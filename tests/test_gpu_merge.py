@@ -165,6 +165,29 @@ def test_one_giant_group_uses_global_sort_path():
             assert_merge_equal(g, oracle_merge(mi, rule))
 
 
+def test_many_timelines_uses_the_global_memory_group_kernel():
+    # n > 7,936 timelines: grouping no longer fits one CTA's shared memory (merge_group_kernel<false>, arrays in the workspace)
+    rng = np.random.default_rng(21)
+    for n, ngroups in ((9000, 600), (20000, 4000)):
+        gs = [int(rng.integers(0, ngroups)) for _ in range(n)]
+        tls = [None] * n
+        last = {}
+        for j in range(n):
+            g = gs[j]
+            if g in last and rng.random() < 0.7:
+                t = last[g] + [int(x) for x in rng.integers(0, 9, size=int(rng.integers(0, 12)))]
+            else:
+                t = [int(x) for x in rng.integers(0, 9, size=int(rng.integers(1, 30)))]
+            tls[j] = t
+            last[g] = t
+        mi = from_lists(tls, [7 * g - 11 for g in gs], [int(rng.integers(0, len(t) + 1)) for t in tls])
+        for rule in RULES:
+            g, st = gpu_merge(mi, rule)
+            assert st == 0, st
+            assert_merge_equal(g, oracle_merge(mi, rule))
+        assert g.M < n
+
+
 def test_empty_and_invalid():
     dev = "cuda"
     z32 = torch.zeros(1, dtype=torch.int32, device=dev)
