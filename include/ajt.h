@@ -268,8 +268,9 @@ int ajt_policy_loss_fwd_bwd_ext(
  * mask DEVICE [T] or NULL (rows with mask 0 give 0, 0, 0).  The [T, V] logits are never written: tiles of 128 x 256 are
  * produced by tcgen05.mma (bf16 x bf16 -> fp32 in tensor memory) and reduced on the fly.  Arithmetic: fp32.
  * Requires d % 64 == 0, ld % 8 == 0 and 16-byte aligned bases (AJT_ERR_UNSUPPORTED otherwise).
- * Workspace: ajt_lm_head_workspace_bytes(T, V) bytes of DEVICE memory, 256-byte aligned. */
-size_t ajt_lm_head_workspace_bytes(int64_t T, int32_t V);
+ * With a mask the unmasked rows are compacted first (their hidden rows gathered into the workspace), so masked rows cost
+ * no flops.  Workspace: ajt_lm_head_workspace_bytes(T, d, V) bytes of DEVICE memory, 256-byte aligned. */
+size_t ajt_lm_head_workspace_bytes(int64_t T, int32_t d, int32_t V);
 
 int ajt_lm_head_logp(const void* hidden, const void* weight, const int32_t* targets, const uint8_t* mask, int64_t T, int32_t d,
                      int32_t V, int64_t ld_hidden, int64_t ld_weight, float* logp_out, float* ent_out /* or NULL */,

@@ -63,7 +63,7 @@ def lib():
             getattr(L, f).restype = C.c_size_t
             getattr(L, f).argtypes = [C.c_int32, C.c_int64]
         L.ajt_lm_head_workspace_bytes.restype = C.c_size_t
-        L.ajt_lm_head_workspace_bytes.argtypes = [C.c_int64, C.c_int32]
+        L.ajt_lm_head_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
         L.ajt_merge_blocks_workspace_bytes.restype = C.c_size_t
         L.ajt_merge_blocks_workspace_bytes.argtypes = [C.c_int32, C.c_int64]
         L.ajt_loss_workspace_bytes.restype = C.c_size_t
@@ -473,7 +473,8 @@ def lm_head_logp(hidden: torch.Tensor, weight: torch.Tensor, targets: torch.Tens
     ent = torch.empty(max(T, 1), dtype=torch.float32, device=dev) if want_entropy else None
     lse = torch.empty(max(T, 1), dtype=torch.float32, device=dev) if want_lse else None
     if workspace is None:
-        workspace = torch.empty(int(lib().ajt_lm_head_workspace_bytes(C.c_int64(T), C.c_int32(V))) + 256, dtype=torch.uint8, device=dev)
+        workspace = torch.empty(int(lib().ajt_lm_head_workspace_bytes(C.c_int64(T), C.c_int32(d), C.c_int32(V))) + 256, dtype=torch.uint8,
+                                device=dev)
     rc = lib().ajt_lm_head_logp(_dp(hidden), _dp(weight), _dp(targets), _dp(mask), C.c_int64(T), C.c_int32(d), C.c_int32(V),
                                 C.c_int64(int(hidden.stride(0)) if T > 1 else d), C.c_int64(int(weight.stride(0)) if V > 1 else d),
                                 _dp(logp), _dp(ent), _dp(lse), _dp(workspace), C.c_size_t(workspace.numel()), _stream(stream))

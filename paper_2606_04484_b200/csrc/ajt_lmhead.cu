@@ -38,8 +38,10 @@ template <int NCTA> struct LmCfg {
 constexpr uint32_t kPeerBitMask = 0xFEFFFFFFu;   // shared::cluster address of the same location in the pair's CTA 0
 
 struct LmParams {
-    const int32_t* targets;
+    const int32_t* targets;     // per row of the (possibly compacted) hidden matrix the kernel sees
     const uint8_t* mask;
+    const int32_t* n_rows;      // DEVICE: rows to process when the masked rows were compacted away, else NULL (then T)
+    const int32_t* row_idx;     // [n_rows] original row of compacted row k, or NULL
     int64_t T;
     int32_t d, V, vs_len, n_mtiles, mgroup;   // vs_len: columns per vocabulary range (multiple of kBN); mgroup: row blocks per wave
     float4* part;                             // [T][kVS] {m, s, u, z_y (or -inf)}
@@ -115,11 +117,11 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
 
 // item i of work group g (a CTA, or a CTA pair): row block (i * mgroup + g / kVS), vocabulary range g % kVS
 template <int NCTA>
-__device__ __forceinline__ bool item_of(const LmParams& p, int it, int& mt, int& vs) {
+__device__ __forceinline__ bool item_of(const LmParams& p, int n_mtiles, int it, int& mt, int& vs) {
     const int g = (int)blockIdx.x / NCTA;
     mt = it * p.mgroup + g / kVS;
     vs = g % kVS;
-    return g / kVS < p.mgroup && mt < p.n_mtiles;
+    return g / kVS < p.mgroup && mt < n_mtiles;
 }
 
 // p.n_mtiles counts row blocks of 128 * NCTA rows.
@@ -138,7 +140,9 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = NCTA > 1 ? cluster_ctarank() : 0u;
     const int nk = p.d / kBK;
-    const int n_items = (p.n_mtiles + p.mgroup - 1) / p.mgroup;
+    const int64_t Teff = p.n_rows ? (int64_t)*p.n_rows : p.T;   // rows actually present (masked rows compacted away)
+    const int n_mtiles = (int)((Teff + kBM * NCTA - 1) / (kBM * NCTA));
+    const int n_items = (n_mtiles + p.mgroup - 1) / p.mgroup;
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < kStages; ++i) {
@@ -172,7 +176,7 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
             uint32_t ph = 0;
             for (int it = 0; it < n_items; ++it) {
                 int mt, vs;
-                if (!item_of<NCTA>(p, it, mt, vs)) continue;
+                if (!item_of<NCTA>(p, n_mtiles, it, mt, vs)) continue;
                 const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
                 const int row0 = (mt * NCTA + (int)rank) * kBM;
                 for (int n0 = v0; n0 < v1; n0 += kBN) {
@@ -200,7 +204,7 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
             uint32_t ph = 0, aph = 0;
             for (int it = 0; it < n_items; ++it) {
                 int mt, vs;
-                if (!item_of<NCTA>(p, it, mt, vs)) continue;
+                if (!item_of<NCTA>(p, n_mtiles, it, mt, vs)) continue;
                 const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
                 for (int n0 = v0; n0 < v1; n0 += kBN) {
                     mbar_wait(&tempty[as], aph ^ 1u);
@@ -232,9 +236,9 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
         uint32_t aph = 0;
         for (int it = 0; it < n_items; ++it) {
             int mt, vs;
-            if (!item_of<NCTA>(p, it, mt, vs)) continue;
+            if (!item_of<NCTA>(p, n_mtiles, it, mt, vs)) continue;
             const int64_t row = (int64_t)(mt * NCTA + (int)rank) * kBM + rloc;
-            const bool live = row < p.T;
+            const bool live = row < Teff;
             const int y = live ? p.targets[row] : -1;
             float m = -INFINITY, s = 0.f, u = 0.f, zy = -INFINITY;
             const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
@@ -299,11 +303,14 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
     }
 }
 
+// Folds the range partials of every processed row and writes the outputs at the row's ORIGINAL position (the outputs of
+// masked rows were zeroed beforehand when the rows were compacted).
 __global__ void __launch_bounds__(256) lm_head_combine_kernel(const LmParams p, int nvs) {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < p.T; t += stride) {
+    const int64_t Teff = p.n_rows ? (int64_t)*p.n_rows : p.T;
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < Teff; t += stride) {
         float lp = 0.f, H = 0.f, lse = 0.f;
-        if (!p.mask || p.mask[t] != 0) {
+        {
             float4 q[kVS];
             float M = -INFINITY, zy = -INFINITY;
             for (int k = 0; k < nvs; ++k) {
@@ -323,9 +330,91 @@ __global__ void __launch_bounds__(256) lm_head_combine_kernel(const LmParams p, 
             H = logS - U / S;
             lse = M + logS;
         }
-        p.logp_out[t] = lp;
-        if (p.ent_out) p.ent_out[t] = H;
-        if (p.lse_out) p.lse_out[t] = lse;
+        const int64_t o = p.row_idx ? (int64_t)p.row_idx[t] : t;
+        p.logp_out[o] = lp;
+        if (p.ent_out) p.ent_out[o] = H;
+        if (p.lse_out) p.lse_out[o] = lse;
+    }
+}
+
+// ---- masked rows are not worth a single flop: compact the unmasked rows first (stable, one pass: tiles of 1,024 rows handed out
+// by an atomic ticket, each publishes its count and adds up its predecessors'), gather their hidden rows and targets into a
+// dense matrix, run the tiles on that, scatter the results back.
+constexpr int kCompactTile = 1024;
+__global__ void __launch_bounds__(256) lm_compact_kernel(const uint8_t* __restrict__ mask, int64_t T, uint64_t* tile_state, int32_t* ticket,
+                                                         int32_t* row_idx, int32_t* n_rows) {
+    __shared__ int s_w[8];
+    __shared__ int s_tile, s_base;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int ntiles = (int)((T + kCompactTile - 1) / kCompactTile);
+    for (;;) {
+        if (tid == 0) s_tile = atomicAdd(ticket, 1);
+        __syncthreads();
+        const int tile = s_tile;
+        if (tile >= ntiles) break;
+        const int64_t t0 = (int64_t)tile * kCompactTile + tid * 4;
+        bool on[4];
+        int cnt = 0;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            on[e] = t0 + e < T && mask[t0 + e] != 0;
+            cnt += on[e];
+        }
+        int inc = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += v;
+        }
+        if (lane == 31) s_w[warp] = inc;
+        __syncthreads();
+        int wbase = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) {
+            if (w < warp) wbase += s_w[w];
+            total += s_w[w];
+        }
+        if (tid == 0) {
+            __threadfence();
+            atomicExch(reinterpret_cast<unsigned long long*>(&tile_state[tile]), (1ull << 63) | (unsigned long long)total);
+        }
+        int pre = 0;
+        for (int t = tid; t < tile; t += 256) {
+            unsigned long long st;
+            do {
+                st = *reinterpret_cast<volatile unsigned long long*>(&tile_state[t]);
+            } while (!(st >> 63));
+            pre += (int)(st & 0x7fffffffull);
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) pre += __shfl_xor_sync(0xffffffffu, pre, o);
+        __syncthreads();
+        if (lane == 0) s_w[warp] = pre;
+        __syncthreads();
+        if (tid == 0) {
+            int b = 0;
+            for (int w = 0; w < 8; ++w) b += s_w[w];
+            s_base = b;
+        }
+        __syncthreads();
+        int k = s_base + wbase + inc - cnt;
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+            if (on[e]) row_idx[k++] = (int32_t)(t0 + e);
+        if (tile == ntiles - 1 && tid == 255) *n_rows = s_base + total;
+        __syncthreads();
+    }
+}
+__global__ void __launch_bounds__(256) lm_gather_kernel(const uint4* __restrict__ hidden, int64_t ld16, int32_t d16, const int32_t* __restrict__ targets,
+                                                        const int32_t* __restrict__ row_idx, const int32_t* __restrict__ n_rows, uint4* hidden_c,
+                                                        int32_t* targets_c) {
+    const int64_t n = (int64_t)*n_rows * d16, stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const int64_t k = i / d16;
+        const int c = (int)(i - k * d16);
+        const int64_t r = row_idx[k];
+        hidden_c[i] = __ldg(hidden + r * ld16 + c);
+        if (c == 0) targets_c[k] = targets[r];
     }
 }
 
@@ -345,9 +434,26 @@ bool make_map(EncodeTiledFn fn, CUtensorMap* map, const void* base, int64_t rows
 
 }  // namespace
 
-extern "C" size_t ajt_lm_head_workspace_bytes(int64_t T, int32_t V) {
-    if (T < 0 || V <= 0) return 0;
-    return (((size_t)T * kVS * sizeof(float4)) + 255) & ~(size_t)255;
+namespace {
+struct LmWs { size_t part, n_rows, tile_state, row_idx, targets_c, hidden_c, total; };
+inline size_t lm_a256(size_t x) { return (x + 255) & ~(size_t)255; }
+LmWs lm_ws_layout(int64_t T, int32_t d) {
+    LmWs w;
+    size_t o = 0;
+    w.part = o; o += lm_a256((size_t)T * kVS * sizeof(float4));
+    w.n_rows = o; o += 256;                                  // {n_rows, ticket}
+    w.tile_state = o; o += lm_a256((size_t)((T + kCompactTile - 1) / kCompactTile + 1) * 8);
+    w.row_idx = o; o += lm_a256((size_t)T * 4);
+    w.targets_c = o; o += lm_a256((size_t)T * 4);
+    w.hidden_c = o; o += lm_a256((size_t)T * d * 2);
+    w.total = o;
+    return w;
+}
+}  // namespace
+
+extern "C" size_t ajt_lm_head_workspace_bytes(int64_t T, int32_t d, int32_t V) {
+    if (T < 0 || d <= 0 || V <= 0) return 0;
+    return lm_ws_layout(T, d).total;
 }
 
 extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const int32_t* targets, const uint8_t* mask, int64_t T,
@@ -360,8 +466,10 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
     if (d % kBK != 0 || (ld_hidden % 8) != 0 || (ld_weight % 8) != 0 || (((uintptr_t)hidden | (uintptr_t)weight) & 15) ||
         T >= ((int64_t)1 << 31))
         return AJT_ERR_UNSUPPORTED;   // K slabs of 64, 16-byte aligned rows (TMA)
-    if (((uintptr_t)workspace & 255) || workspace_bytes < ajt_lm_head_workspace_bytes(T, V)) return AJT_ERR_WORKSPACE_TOO_SMALL;
+    if (((uintptr_t)workspace & 255) || workspace_bytes < ajt_lm_head_workspace_bytes(T, d, V)) return AJT_ERR_WORKSPACE_TOO_SMALL;
     if (T == 0) return AJT_OK;
+    const LmWs ws = lm_ws_layout(T, d);
+    uint8_t* wsb = reinterpret_cast<uint8_t*>(workspace);
 
     int dev = 0, num_sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return AJT_ERR_CUDA;
@@ -374,18 +482,38 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
         encode = reinterpret_cast<EncodeTiledFn>(fn);
     }
     const int ncta = T > kBM ? 2 : 1;   // CTA pairs (256-row blocks) unless a single 128-row block holds everything
-    CUtensorMap map_h, map_w;
-    if (!make_map(encode, &map_h, hidden, T, d, ld_hidden, kBM) || !make_map(encode, &map_w, weight, V, d, ld_weight, kBN / ncta))
-        return AJT_ERR_CUDA;
-
     LmParams p;
     p.targets = targets; p.mask = mask; p.T = T; p.d = d; p.V = V;
+    p.n_rows = nullptr; p.row_idx = nullptr;
+    const void* h_src = hidden;
+    int64_t h_ld = ld_hidden;
+    if (mask) {
+        int32_t* n_rows = reinterpret_cast<int32_t*>(wsb + ws.n_rows);
+        int32_t* row_idx = reinterpret_cast<int32_t*>(wsb + ws.row_idx);
+        int32_t* targets_c = reinterpret_cast<int32_t*>(wsb + ws.targets_c);
+        if (cudaMemsetAsync(wsb + ws.n_rows, 0, ws.row_idx - ws.n_rows, stream) != cudaSuccess) return AJT_ERR_CUDA;   // count, ticket, tile states
+        if (cudaMemsetAsync(logp_out, 0, (size_t)T * 4, stream) != cudaSuccess) return AJT_ERR_CUDA;
+        if (ent_out && cudaMemsetAsync(ent_out, 0, (size_t)T * 4, stream) != cudaSuccess) return AJT_ERR_CUDA;
+        if (lse_out && cudaMemsetAsync(lse_out, 0, (size_t)T * 4, stream) != cudaSuccess) return AJT_ERR_CUDA;
+        const int ntiles = (int)((T + kCompactTile - 1) / kCompactTile);
+        lm_compact_kernel<<<ntiles < num_sms ? ntiles : num_sms, 256, 0, stream>>>(mask, T, reinterpret_cast<uint64_t*>(wsb + ws.tile_state),
+                                                                                 n_rows + 1, row_idx, n_rows);
+        lm_gather_kernel<<<num_sms * 8, 256, 0, stream>>>(reinterpret_cast<const uint4*>(hidden), ld_hidden / 8, d / 8, targets, row_idx, n_rows,
+                                                         reinterpret_cast<uint4*>(wsb + ws.hidden_c), targets_c);
+        p.targets = targets_c; p.n_rows = n_rows; p.row_idx = row_idx;
+        h_src = wsb + ws.hidden_c;
+        h_ld = d;
+    }
+    CUtensorMap map_h, map_w;
+    if (!make_map(encode, &map_h, h_src, T, d, h_ld, kBM) || !make_map(encode, &map_w, weight, V, d, ld_weight, kBN / ncta))
+        return AJT_ERR_CUDA;
+
     p.n_mtiles = (int)((T + kBM * ncta - 1) / (kBM * ncta));   // row blocks of 128 * ncta rows
     const int nvs = V >= kVS * kBN ? kVS : 1;   // small vocabularies: one range
     p.vs_len = (((V + nvs - 1) / nvs + kBN - 1) / kBN) * kBN;
     p.mgroup = (num_sms / ncta) / kVS;
     if (p.mgroup > p.n_mtiles) p.mgroup = p.n_mtiles;
-    p.part = reinterpret_cast<float4*>(workspace);
+    p.part = reinterpret_cast<float4*>(wsb + ws.part);
     p.logp_out = logp_out; p.ent_out = ent_out; p.lse_out = lse_out;
     if (nvs == 1) p.vs_len = ((V + kBN - 1) / kBN) * kBN;
 

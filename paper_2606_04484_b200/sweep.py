@@ -196,17 +196,21 @@ def run_c5(dev, stream, reps, out, quick=False):
             torch.cuda.empty_cache()
 
 
-def measure_lm_head(name: str, T: int, d: int, V: int, dev, stream, reps: int, out):
+def measure_lm_head(name: str, T: int, d: int, V: int, dev, stream, reps: int, out, rho: float = 1.0):
     """ajt_lm_head_logp (forward half): dense contraction on the tensor cores, reported in TFLOP/s against
     the measured bf16 matmul throughput of MEASURED_PEAKS.json (burst figure: the kernel is timed alone)."""
     g = torch.Generator(device=dev).manual_seed(17)
     Hh = torch.randn((T, d), generator=g, device=dev).to(torch.bfloat16)
     Ww = (torch.randn((V, d), generator=g, device=dev) * 0.02).to(torch.bfloat16)
     y = torch.randint(0, V, (T,), generator=g, device=dev, dtype=torch.int32)
-    ws = torch.empty(int(ajt.lib().ajt_lm_head_workspace_bytes(T, V)) + 256, dtype=torch.uint8, device=dev)
-    call = lambda: ajt.lm_head_logp(Hh, Ww, y, None, workspace=ws, stream=stream)
+    ws = torch.empty(int(ajt.lib().ajt_lm_head_workspace_bytes(T, d, V)) + 256, dtype=torch.uint8, device=dev)
+    mask = None
+    if rho < 1.0:   # response / env runs as in the loss sweep: only the unmasked rows are worth a log-prob
+        mask = torch.from_numpy(W.loss_sweep_vectors(T, V, 64, rho, cell=7).mask).to(dev)
+    call = lambda: ajt.lm_head_logp(Hh, Ww, y, mask, workspace=ws, stream=stream)
     med, best = _stats(H.time_calls(call, stream, reps=reps, flush=None))
-    flops = 2.0 * T * d * V
+    n_rows = T if mask is None else int(mask.sum().item())
+    flops = 2.0 * n_rows * d * V
     tf = flops / (med * 1e-3) / 1e12
     peak = None
     try:
@@ -216,7 +220,7 @@ def measure_lm_head(name: str, T: int, d: int, V: int, dev, stream, reps: int, o
     except Exception:
         peak = 2250.0 * 0.7   # B200_PROFILING.md fallback: nominal dense bf16 x typical cuBLAS fraction
     _emit(out, stage="lm_head_logp", config=name, T=T, d=d, V=V, ms_median=med, ms_best=best, flops=flops, tflop_per_s=tf,
-          peak_tflops=peak, frac_of_measured=tf / peak, frac_of_nominal_2250=tf / 2250.0,
+          rows_unmasked=n_rows, mask_density=n_rows / T, peak_tflops=peak, frac_of_measured=tf / peak, frac_of_nominal_2250=tf / 2250.0,
           logits_bytes_not_written=2.0 * T * V, reps=reps)
 
 
@@ -301,6 +305,7 @@ def main():
             measure_blocks(c, W.block_workload(c), dev, stream, args.reps, out)
         elif c == "h1":   # Qwen3-8B-like head (d = 4096, V = 151936) over the bench micro-batch's rows
             measure_lm_head("h1", 40960, 4096, 151936, dev, stream, max(3, args.reps // 4), out)
+            measure_lm_head("h1", 40960, 4096, 151936, dev, stream, max(3, args.reps // 4), out, rho=0.3)
         elif c == "h0":
             measure_lm_head("h0", 8192, 2048, 32000, dev, stream, args.reps, out)
         elif c == "c5":
