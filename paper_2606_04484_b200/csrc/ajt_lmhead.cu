@@ -43,7 +43,7 @@ struct LmParams {
     const int32_t* n_rows;      // DEVICE: rows to process when the masked rows were compacted away, else NULL (then T)
     const int32_t* row_idx;     // [n_rows] original row of compacted row k, or NULL
     int64_t T;
-    int32_t d, V, vs_len, n_mtiles, mgroup;   // vs_len: columns per vocabulary range (multiple of kBN); mgroup: row blocks per wave
+    int32_t d, V, vs_len, nvs;   // vs_len: columns per vocabulary range (multiple of kBN); nvs: ranges in use (<= kVS)
     float4* part;                             // [T][kVS] {m, s, u, z_y (or -inf)}
     float* logp_out;
     float* ent_out;
@@ -115,16 +115,18 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
-// item i of work group g (a CTA, or a CTA pair): row block (i * mgroup + g / kVS), vocabulary range g % kVS
+// Work unit u = (row block u / nvs, vocabulary range u % nvs); work group g (a CTA, or a CTA pair) takes units g, g + G, ...
+// Groups that run together hold neighbouring units: a few row blocks times all ranges, so the W ranges are shared through L2.
 template <int NCTA>
 __device__ __forceinline__ bool item_of(const LmParams& p, int n_mtiles, int it, int& mt, int& vs) {
-    const int g = (int)blockIdx.x / NCTA;
-    mt = it * p.mgroup + g / kVS;
-    vs = g % kVS;
-    return g / kVS < p.mgroup && mt < n_mtiles;
+    const int G = (int)gridDim.x / NCTA, g = (int)blockIdx.x / NCTA;
+    const int64_t u = (int64_t)it * G + g;
+    mt = (int)(u / p.nvs);
+    vs = (int)(u % p.nvs);
+    return mt < n_mtiles;
 }
 
-// p.n_mtiles counts row blocks of 128 * NCTA rows.
+// Row blocks are 128 * NCTA rows.
 template <int NCTA>
 __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_constant__ CUtensorMap map_h,
                                                                 const __grid_constant__ CUtensorMap map_w, const LmParams p) {
@@ -142,7 +144,8 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
     const int nk = p.d / kBK;
     const int64_t Teff = p.n_rows ? (int64_t)*p.n_rows : p.T;   // rows actually present (masked rows compacted away)
     const int n_mtiles = (int)((Teff + kBM * NCTA - 1) / (kBM * NCTA));
-    const int n_items = (n_mtiles + p.mgroup - 1) / p.mgroup;
+    const int n_groups = (int)gridDim.x / NCTA;
+    const int n_items = (int)(((int64_t)n_mtiles * p.nvs + n_groups - 1) / n_groups);
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < kStages; ++i) {
@@ -508,25 +511,25 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
     if (!make_map(encode, &map_h, h_src, T, d, h_ld, kBM) || !make_map(encode, &map_w, weight, V, d, ld_weight, kBN / ncta))
         return AJT_ERR_CUDA;
 
-    p.n_mtiles = (int)((T + kBM * ncta - 1) / (kBM * ncta));   // row blocks of 128 * ncta rows
+    const int64_t n_mtiles = (T + kBM * ncta - 1) / (kBM * ncta);   // row blocks of 128 * ncta rows (upper bound when rows are compacted)
     const int nvs = V >= kVS * kBN ? kVS : 1;   // small vocabularies: one range
+    p.nvs = nvs;
     p.vs_len = (((V + nvs - 1) / nvs + kBN - 1) / kBN) * kBN;
-    p.mgroup = (num_sms / ncta) / kVS;
-    if (p.mgroup > p.n_mtiles) p.mgroup = p.n_mtiles;
+    int groups = num_sms / ncta;                // one work group per SM (pair of SMs)
+    if ((int64_t)groups > n_mtiles * nvs) groups = (int)(n_mtiles * nvs);
     p.part = reinterpret_cast<float4*>(wsb + ws.part);
     p.logp_out = logp_out; p.ent_out = ent_out; p.lse_out = lse_out;
-    if (nvs == 1) p.vs_len = ((V + kBN - 1) / kBN) * kBN;
 
     // ranges beyond nvs are empty (v0 >= V): their CTAs have nothing to do, and the combine reads nvs partials per row
     if (ncta == 1) {
         if (cudaFuncSetAttribute(lm_head_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<1>::kSmem) != cudaSuccess)
             return AJT_ERR_CUDA;
-        lm_head_kernel<1><<<p.mgroup * kVS, kLmThreads, LmCfg<1>::kSmem, stream>>>(map_h, map_w, p);
+        lm_head_kernel<1><<<groups, kLmThreads, LmCfg<1>::kSmem, stream>>>(map_h, map_w, p);
     } else {
         if (cudaFuncSetAttribute(lm_head_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<2>::kSmem) != cudaSuccess)
             return AJT_ERR_CUDA;
         cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)(p.mgroup * kVS * 2));
+        cfg.gridDim = dim3((unsigned)(groups * 2));
         cfg.blockDim = dim3(kLmThreads);
         cfg.dynamicSmemBytes = LmCfg<2>::kSmem;
         cfg.stream = stream;
