@@ -211,3 +211,20 @@ def test_rejects_bad_input():
     x = pack([[[1, 1, [1]]], []], [0, 0])     # the second timeline has no block: K_i >= 1 is required
     with pytest.raises(ValueError):
         oracle.merge_blocks(**x)
+
+
+def test_explicit_token_mask_travels_with_the_tokens():
+    """Reading B-2: when block k of the survivor takes tokens and log-probs from an absorbed timeline (lines 12-14), the per-token
+    mask it carries is the supplier's; blocks the survivor keeps carry its own mask.  Hand example."""
+    tls = [[[1, 1, [10, 11]], [2, 2, [20, 21, 22]]],                       # T_0: user, llm (generated here)
+           [[1, 1, [10, 11]], [2, 0, [21, 22]], [3, 2, [30, 31]]]]         # T_1: the answer comes back re-tokenised, then a new answer
+    x = pack(tls, [4, 4])
+    #            T_0: u  u  l  l  l   T_1: u  u  e  e  l  l
+    tok_mask = np.array([0, 1, 1, 0, 1,       1, 0, 1, 1, 0, 1], np.uint8)   # arbitrary per-token masks, not derived from authors
+    r = oracle.merge_blocks(**x, tok_mask=tok_mask)
+    assert r.M == 1 and r.merged_block_src.tolist() == [1, 0, 1]
+    assert r.merged_tokens.tolist() == [10, 11, 20, 21, 22, 30, 31]
+    assert r.merged_mask.tolist() == [1, 0, 1, 0, 1, 0, 1]               # T_1's own mask, T_0's for the replaced block, T_1's own
+    assert r.merged_tok_src.tolist() == [1, -1, 0, -1, 0, -1, 1]
+    want_lp = np.where(np.array(r.merged_mask) != 0, x["logp"][[5, 6, 2, 3, 4, 9, 10]], 0).astype(np.float32)
+    assert np.array_equal(r.merged_logp, want_lp)
