@@ -3,12 +3,13 @@
 // sum e (z - m) / target gather), so the [T, V] logits never reach HBM.  This is the forward half of SURVEY.md §8(f) f3: the pass
 // that produces the old / reference log-probs the loss consumes.  DESIGN.md "O-H".
 //
-// Work item = (128 rows of H) x (one of VS vocabulary ranges).  Inside an item the CTA walks the range in tiles of 256
-// columns; per tile the K loop streams 64-wide slabs of H and W through a 4-stage TMA ring (SWIZZLE_128B, K-major), one
-// elected thread issues 4 x tcgen05.mma (128 x 256 x 16) per slab, and the two 256-column TMEM accumulators alternate so that
-// the epilogue warps (one row per thread: tcgen05.ld 32 columns at a time) reduce tile n while the tensor cores fill tile n+1.
-// The CTAs that run at the same time share the W ranges (L2) and own different row blocks.
-// Per (row, range) the epilogue leaves {m, s, u, z_y}; lm_head_combine_kernel folds the VS partials of a row.
+// Work unit = (a block of 128 or 256 rows of H) x (one of 4 vocabulary ranges), striped over the SMs (one CTA, or one CTA pair, per
+// SM / pair of SMs).  Inside a unit the range is walked in tiles of 256 columns; per tile the K loop streams 64-wide slabs of H
+// and W through a TMA ring (SWIZZLE_128B, K-major), one elected thread issues 4 x tcgen05.mma per slab, and the two 256-column
+// TMEM accumulators alternate so that the epilogue warps (one row per thread: tcgen05.ld 32 columns at a time) reduce tile n
+// while the tensor cores fill tile n+1.  The work groups that run at the same time share the W ranges (L2).
+// Per (row, range) the epilogue leaves {m, s, u, z_y}; lm_head_combine_kernel folds the range partials of a row.
+// With a mask, the unmasked rows are compacted first (lm_compact_kernel, lm_gather_kernel) so that masked rows cost no flops.
 #include <cuda.h>
 
 #include "ajt_common.cuh"
