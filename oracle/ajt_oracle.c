@@ -6,12 +6,15 @@
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
  * load this file.  It shares no code, header, table or helper with paper_2606_04484_b200/csrc/.
  *
- *   - merge : the DEFINITION, by brute-force pairwise prefix comparison (no hashing, no sorting).
- *   - loss  : fp64 throughout, from the exact stored input values.
+ *   - merge        : the DEFINITION, by brute-force pairwise prefix comparison (no hashing, no sorting).
+ *   - block merge  : Algorithm 1 line by line on timelines of message blocks (Match = text | token).
+ *   - loss         : fp64 throughout, from the exact stored input values (steps 1-7; steps 8-9 in the extended entry).
+ * (oracle/__init__.py adds, in plain numpy: pack_loss_inputs, the next-token alignment sequence by sequence, and
+ *  lm_head_logp, log-probs / entropy from hidden states with an fp64 matmul as a library step.)
  *
- * Parity status: every function here is pinned by tests/test_oracle_*.py (hand traces of
- * Algorithm 1, a second independent formulation, invariants, closed forms, finite differences,
- * torch fp64 autograd).  Nothing is "parity unpinned".
+ * Parity status: every function here and in oracle/__init__.py is pinned by tests/test_oracle_*.py (hand traces of
+ * Algorithm 1 on tokens and on blocks, second independent formulations, invariants, closed forms, finite differences,
+ * torch fp64 autograd, library routines).  Nothing is "parity unpinned".
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC -o oracle/libajt_oracle.so oracle/ajt_oracle.c -lm
  * OpenMP only parallelises independent outer loops (timelines j, rows t); no blocking, fusion or
