@@ -270,11 +270,19 @@ int ajt_policy_loss_fwd_bwd_ext(
  * Requires d % 64 == 0, ld % 8 == 0 and 16-byte aligned bases (AJT_ERR_UNSUPPORTED otherwise).
  * With a mask the unmasked rows are compacted first (their hidden rows gathered into the workspace), so masked rows cost
  * no flops.  Workspace: ajt_lm_head_workspace_bytes(T, d, V) bytes of DEVICE memory, 256-byte aligned. */
+enum {
+    AJT_LM_ROUND_LOGITS_BF16 = 1 /* round every logit to bf16 (RNE) before the softmax: the log-probs then agree with what
+                                    ajt_policy_loss_fwd_bwd computes from the same logits STORED in bf16 (to fp32 rounding of
+                                    the reductions), so that old / new log-prob ratios start at 1 (the train / inference
+                                    consistency the paper is concerned with) */
+};
+
 size_t ajt_lm_head_workspace_bytes(int64_t T, int32_t d, int32_t V);
 
 int ajt_lm_head_logp(const void* hidden, const void* weight, const int32_t* targets, const uint8_t* mask, int64_t T, int32_t d,
                      int32_t V, int64_t ld_hidden, int64_t ld_weight, float* logp_out, float* ent_out /* or NULL */,
-                     float* lse_out /* or NULL */, void* workspace, size_t workspace_bytes, ajt_stream_t stream);
+                     float* lse_out /* or NULL */, uint32_t flags /* AJT_LM_* */, void* workspace, size_t workspace_bytes,
+                     ajt_stream_t stream);
 
 /* Batch-wide per-trajectory normalisers for callers that stream the batch through several loss calls
  * (micro-batches, 64k-row chunks, or rows of one trajectory spread over several GPUs; reading L-4;

@@ -273,7 +273,7 @@ def pack_loss_inputs(merged_tokens, merged_mask, merged_old_logp, merged_offsets
     return targets, mask, olp, seg, adv
 
 
-def lm_head_logp(hidden_bits, weight_bits, targets, mask=None):
+def lm_head_logp(hidden_bits, weight_bits, targets, mask=None, round_logits_bf16: bool = False):
     """Log-prob and entropy of the target token under an LM head, without the method's tiling (the step before
     the loss in the actor update, forward half):
         z_t = W h_t  (fp64 from the exact bf16 inputs);  logp_t = z_{t,y_t} - logsumexp(z_t);  H_t = lse_t - sum_v p_tv z_tv
@@ -287,6 +287,8 @@ def lm_head_logp(hidden_bits, weight_bits, targets, mask=None):
     ent = np.zeros(T, np.float64)
     for a in range(0, T, 256):
         z = H[a:a + 256] @ W.T                      # library matmul as a step
+        if round_logits_bf16:                       # the logits as a bf16-storing forward pass would hand them to the loss
+            z = round_bf16(z)
         m = z.max(axis=1, keepdims=True)
         lse = m[:, 0] + np.log(np.exp(z - m).sum(axis=1))
         p = np.exp(z - lse[:, None])

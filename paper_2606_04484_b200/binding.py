@@ -457,7 +457,8 @@ def policy_loss_fwd_bwd_ext(logits: torch.Tensor, targets: torch.Tensor, old_log
 
 
 def lm_head_logp(hidden: torch.Tensor, weight: torch.Tensor, targets: torch.Tensor, mask: Optional[torch.Tensor] = None,
-                 want_entropy: bool = True, workspace: Optional[torch.Tensor] = None, stream=None, want_lse: bool = False):
+                 want_entropy: bool = True, workspace: Optional[torch.Tensor] = None, stream=None, want_lse: bool = False,
+                 round_logits_bf16: bool = False):
     """ajt_lm_head_logp (include/ajt.h): (logp f32 [T], entropy f32 [T] | None) from hidden [T, d] and weight [V, d] (bf16);
     with want_lse also the row log-sum-exps as a third element."""
     _require_cuda()
@@ -477,7 +478,8 @@ def lm_head_logp(hidden: torch.Tensor, weight: torch.Tensor, targets: torch.Tens
                                 device=dev)
     rc = lib().ajt_lm_head_logp(_dp(hidden), _dp(weight), _dp(targets), _dp(mask), C.c_int64(T), C.c_int32(d), C.c_int32(V),
                                 C.c_int64(int(hidden.stride(0)) if T > 1 else d), C.c_int64(int(weight.stride(0)) if V > 1 else d),
-                                _dp(logp), _dp(ent), _dp(lse), _dp(workspace), C.c_size_t(workspace.numel()), _stream(stream))
+                                _dp(logp), _dp(ent), _dp(lse), C.c_uint32(1 if round_logits_bf16 else 0), _dp(workspace),
+                                C.c_size_t(workspace.numel()), _stream(stream))
     if rc != 0:
         raise AjtError(rc, "ajt_lm_head_logp")
     if want_lse:

@@ -44,6 +44,7 @@ struct LmParams {
     const int32_t* n_rows;      // DEVICE: rows to process when the masked rows were compacted away, else NULL (then T)
     const int32_t* row_idx;     // [n_rows] original row of compacted row k, or NULL
     int64_t T;
+    int32_t round_bf16;          // AJT_LM_ROUND_LOGITS_BF16: logits rounded to bf16 (RNE) before the softmax
     int32_t d, V, vs_len, nvs;   // vs_len: columns per vocabulary range (multiple of kBN); nvs: ranges in use (<= kVS)
     float4* part;                             // [T][kVS] {m, s, u, z_y (or -inf)}
     float* logp_out;
@@ -254,6 +255,10 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
                 for (int c = 0; c < kBN; c += 32) {
                     uint32_t v[32];
                     tmem_ld32(tacc + (uint32_t)c, v);
+                    if (p.round_bf16) {   // what a forward pass that stores bf16 logits (the loss call's input) would see
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) v[e] = __float_as_uint(__bfloat162float(__float2bfloat16_rn(__uint_as_float(v[e]))));
+                    }
                     const int col0 = n0 + c;
                     if (col0 >= v1) continue;
                     const int nval = min(32, v1 - col0);
@@ -462,7 +467,7 @@ extern "C" size_t ajt_lm_head_workspace_bytes(int64_t T, int32_t d, int32_t V) {
 
 extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const int32_t* targets, const uint8_t* mask, int64_t T,
                                 int32_t d, int32_t V, int64_t ld_hidden, int64_t ld_weight, float* logp_out, float* ent_out,
-                                float* lse_out, void* workspace, size_t workspace_bytes, ajt_stream_t stream_) {
+                                float* lse_out, uint32_t flags, void* workspace, size_t workspace_bytes, ajt_stream_t stream_) {
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
     if (T < 0 || d <= 0 || V <= 0 || ld_hidden < d || ld_weight < d) return AJT_ERR_INVALID_ARG;
     if (!logp_out || !workspace) return AJT_ERR_INVALID_ARG;
@@ -489,6 +494,7 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
     LmParams p;
     p.targets = targets; p.mask = mask; p.T = T; p.d = d; p.V = V;
     p.n_rows = nullptr; p.row_idx = nullptr;
+    p.round_bf16 = (flags & AJT_LM_ROUND_LOGITS_BF16) ? 1 : 0;
     const void* h_src = hidden;
     int64_t h_ld = ld_hidden;
     if (mask) {

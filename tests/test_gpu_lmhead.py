@@ -73,6 +73,28 @@ def test_row_lse_output():
     assert float((logp.double() - (zy - want)).abs().max()) <= 3e-5
 
 
+def test_rounded_logits_agree_with_the_loss_call_on_stored_logits():
+    # AJT_LM_ROUND_LOGITS_BF16: log-probs from hidden states == log-probs the loss call computes from the bf16 logits a forward
+    # pass would store (same rounded values, fp32 reductions in a different order)
+    g = torch.Generator(device="cuda").manual_seed(11)
+    T, d, V = 300, 256, 32000
+    H = torch.randn((T, d), generator=g, device="cuda").to(torch.bfloat16)
+    W = (torch.randn((V, d), generator=g, device="cuda") * 0.1).to(torch.bfloat16)
+    y = torch.randint(0, V, (T,), generator=g, device="cuda", dtype=torch.int32)
+    logp, ent = ajt.lm_head_logp(H, W, y, round_logits_bf16=True)
+    rl, re = oracle.lm_head_logp(bits(H), bits(W), y.cpu().numpy(), round_logits_bf16=True)
+    # a logit whose fp32 value lies within rounding error of a bf16 tie may round the other way: compare in bulk, not per row
+    el = np.abs(logp.cpu().numpy().astype(np.float64) - rl)
+    assert np.median(el) <= 3e-6 and np.quantile(el, 0.99) <= 2e-3
+    logits = (H.float() @ W.float().T).to(torch.bfloat16)
+    one = torch.ones(T, device="cuda")
+    out = ajt.policy_loss_fwd_bwd(logits, y, torch.zeros(T, device="cuda"), one, torch.ones(T, dtype=torch.uint8, device="cuda"),
+                                  torch.zeros(T, dtype=torch.int32, device="cuda"), 1, 0.2, 0.2, want_logp=True)
+    torch.cuda.synchronize()
+    dl = (logp - out.logp).abs().cpu().numpy()
+    assert np.median(dl) <= 3e-6 and np.quantile(dl, 0.99) <= 2e-3
+
+
 def test_unsupported_shapes_are_rejected():
     H = torch.zeros((8, 48), dtype=torch.bfloat16, device="cuda")
     W = torch.zeros((16, 48), dtype=torch.bfloat16, device="cuda")

@@ -48,3 +48,19 @@ def test_consistent_with_the_loss_oracle():
                            0.2, 0.2, extended=True)
     np.testing.assert_allclose(logp, r.logp, atol=2e-6)       # fp32 rounding of the materialised logits
     np.testing.assert_allclose(ent, r.ent, atol=2e-6)
+
+
+def test_rounded_logits_match_the_loss_oracle_on_stored_bf16_logits():
+    # with the logits rounded to bf16 first, lm_head_logp is exactly the loss oracle's log-prob of the stored bf16 matrix
+    rng = np.random.default_rng(5)
+    T, d, V = 12, 64, 150
+    hb, wb = bf16_bits(rng.standard_normal((T, d))), bf16_bits(rng.standard_normal((V, d)) * 0.3)
+    y = rng.integers(0, V, size=T).astype(np.int32)
+    logp, ent = oracle.lm_head_logp(hb, wb, y, round_logits_bf16=True)
+    H = torch.from_numpy(hb.view(np.int16)).view(torch.bfloat16).double()
+    W = torch.from_numpy(wb.view(np.int16)).view(torch.bfloat16).double()
+    zb = bf16_bits((H @ W.T).numpy())            # torch's own fp64 -> bf16 rounding of the same products
+    r = oracle.policy_loss(zb, y, np.zeros(T, np.float32), np.zeros(T, np.float32), np.ones(T, np.uint8), np.zeros(T, np.int32), 1,
+                           0.2, 0.2, extended=True, logits_is_bf16_bits=True)
+    np.testing.assert_allclose(logp, r.logp, atol=1e-12)
+    np.testing.assert_allclose(ent, r.ent, atol=1e-12)
