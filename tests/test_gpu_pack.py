@@ -105,3 +105,21 @@ def test_fatal_merge_status_leaves_zero_counts_and_pack_does_nothing():
     pk = ajt.pack_loss_inputs(mo, d(tl_seg.astype(np.int32)), int(uniq.shape[0]))
     torch.cuda.synchronize()
     assert int(pk.status[0]) == 0
+
+
+def test_hbm_probe_modes():
+    # the measurement helper really moves the bytes it is timed on: write zeros, copy, memset; read leaves everything alone
+    n = 1 << 20
+    a = torch.arange(n, dtype=torch.int32, device="cuda")
+    b = torch.full((n,), 7, dtype=torch.int32, device="cuda")
+    sink = torch.zeros(4, dtype=torch.int32, device="cuda")
+    ajt.hbm_probe(sink, a, 4 * n, 0)
+    ajt.hbm_probe(b, a, 4 * n, 2)
+    torch.cuda.synchronize()
+    assert torch.equal(a, torch.arange(n, dtype=torch.int32, device="cuda")) and torch.equal(b, a) and int(sink.sum()) == 0
+    ajt.hbm_probe(b, None, 4 * n, 1)
+    ajt.hbm_probe(a, None, 4 * n, 3)
+    torch.cuda.synchronize()
+    assert not bool(b.any()) and not bool(a.any())
+    with pytest.raises(ajt.AjtError):
+        ajt.hbm_probe(b, None, 4 * n + 4, 1)      # not a multiple of 16 bytes
