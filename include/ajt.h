@@ -22,7 +22,9 @@
  *   - Calls enqueue work on `stream` and return WITHOUT synchronising.  The return value reports
  *     host-detectable errors only (AJT_ERR_*).  Data-dependent faults set bits in a device status
  *     word inside the workspace (AJT_STATUS_*), read back with ajt_last_status(); outputs are then
- *     unspecified.  No exceptions, no abort(), no global state; thread-safe for distinct workspaces.
+ *     unspecified.  No exceptions, no abort(); thread-safe for distinct workspaces.  The only state kept between
+ *     calls is a per-device table of launch facts (SM count, one-time shared-memory opt-in of the kernels), written
+ *     once per device with idempotent values.
  *   - There is no CPU fallback: without a CUDA device every compute call returns AJT_ERR_CUDA.
  *   - The *_host variants take HOST buffers, stage them through a caller-provided device arena with
  *     cudaMemcpyAsync on `stream`, run the same kernels and copy the results back; they synchronise
@@ -60,8 +62,8 @@ enum { AJT_DT_BF16 = 0, AJT_DT_F32 = 1 };
 /* ajt_merge_timelines `flags` */
 enum {
     AJT_MERGE_WEAK_HASH = 1 /* test hook: degrade the prefix hash to 4 bits so that hash-equal,
-                               token-different candidates are common and the exact-verification /
-                               repair path is exercised.  Results are still exact. */
+                               token-different candidates are common and the exact comparison that
+                               guards every accepted candidate is exercised.  Results are still exact. */
 };
 
 /* Device status bits (ajt_last_status). */
@@ -71,8 +73,8 @@ enum {
     AJT_STATUS_BAD_OFFSETS = 4,      /* offsets[0] != 0, decreasing, or offsets[n] != n_tokens */
     AJT_STATUS_ZERO_LEN = 8,         /* a timeline of length 0 (L_j >= 1 required) */
     AJT_STATUS_PROBE_CAPACITY = 16,  /* more candidate (timeline, earlier-length) pairs than the workspace holds */
-    AJT_STATUS_HASH_COLLISION = 32,  /* informational: a hash-equal candidate failed exact verification and the
-                                        exact repair path produced the outputs (they are still exact) */
+    AJT_STATUS_HASH_COLLISION = 32,  /* informational: a hash-equal candidate failed the exact token comparison and was
+                                        skipped (the outputs are exact either way) */
     AJT_STATUS_INTERNAL = 64
 };
 
@@ -92,15 +94,22 @@ int ajt_last_status(const void* workspace, ajt_stream_t stream, uint32_t* bits);
  *                     member index whose mask is 1 at that position (Alg. 1 lines 10-17)
  *
  * Workspace: ajt_merge_workspace_bytes(n, n_tokens) bytes of DEVICE memory, 256-byte aligned.  It sizes
- * room for 64*n + 4096 candidate pairs; a batch whose groups are so large that sum_g k_g(k_g+1)/2 exceeds
- * that sets AJT_STATUS_PROBE_CAPACITY — pass a larger workspace (every extra 32 bytes hold one more pair).
+ * room for 64*n + 4096 candidate pairs.  The call needs one pair per (timeline, earlier-or-same timeline of its group):
+ * n_pairs = sum over groups of k_g (k_g + 1) / 2, which the caller can count from traj_ids alone.  A batch that needs
+ * more (groups of more than ~127 timelines on average) sets AJT_STATUS_PROBE_CAPACITY; size the workspace with
+ * ajt_merge_workspace_bytes_for_pairs(n, n_tokens, n_pairs) instead (every extra 32 bytes hold one more pair; the
+ * capacity always follows from `workspace_bytes`).
  *
- * All integer; outputs are bit-exact with the definition.  Only the first N_out / M entries of the
- * outputs are written.  `counts` is DEVICE memory: synchronise the stream before reading it.  After a fatal status
- * (bad offsets, zero-length timeline, pair capacity) the outputs are unspecified except counts = {0, 0}, so that a chained
- * call (ajt_pack_loss_inputs) does nothing.
+ * All integer; outputs are bit-exact with the definition, whatever the prefix hash does: a candidate is accepted only
+ * through exactly compared links or after an exact token comparison (AJT_STATUS_HASH_COLLISION is informational: a
+ * hash-equal candidate was rejected by that comparison).  Only the first N_out / M entries of the outputs are written.
+ * `counts` is DEVICE memory: synchronise the stream before reading it.  After a fatal status (bad offsets, zero-length
+ * timeline, pair capacity) the outputs are unspecified except counts = {0, 0} and merged_offsets[0] = 0, so that a chained
+ * call (ajt_pack_loss_inputs) does nothing.  The call is five plain kernel launches on `stream` (no cooperative launch, no
+ * host read-back): it can be captured in a CUDA graph.
  */
 size_t ajt_merge_workspace_bytes(int32_t n, int64_t n_tokens);
+size_t ajt_merge_workspace_bytes_for_pairs(int32_t n, int64_t n_tokens, int64_t n_pairs);
 
 int ajt_merge_timelines(
     /* inputs, DEVICE, read-only */

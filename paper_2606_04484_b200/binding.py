@@ -23,7 +23,7 @@ STATUS_PROBE_CAPACITY, STATUS_HASH_COLLISION, STATUS_INTERNAL = 16, 32, 64
 
 _EXPORTS = [
     "ajt_version", "ajt_strerror", "ajt_last_status",
-    "ajt_merge_workspace_bytes", "ajt_merge_timelines", "ajt_merge_host_arena_bytes", "ajt_merge_timelines_host",
+    "ajt_merge_workspace_bytes", "ajt_merge_workspace_bytes_for_pairs", "ajt_merge_timelines", "ajt_merge_host_arena_bytes", "ajt_merge_timelines_host",
     "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
     "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks_workspace_bytes", "ajt_merge_blocks",
     "ajt_pack_loss_inputs", "ajt_lm_head_workspace_bytes", "ajt_lm_head_logp",
@@ -62,6 +62,8 @@ def lib():
         for f in ("ajt_merge_workspace_bytes", "ajt_merge_host_arena_bytes"):
             getattr(L, f).restype = C.c_size_t
             getattr(L, f).argtypes = [C.c_int32, C.c_int64]
+        L.ajt_merge_workspace_bytes_for_pairs.restype = C.c_size_t
+        L.ajt_merge_workspace_bytes_for_pairs.argtypes = [C.c_int32, C.c_int64, C.c_int64]
         L.ajt_lm_head_workspace_bytes.restype = C.c_size_t
         L.ajt_lm_head_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
         L.ajt_merge_blocks_workspace_bytes.restype = C.c_size_t
@@ -88,6 +90,10 @@ def strerror(code: int) -> str:
 
 def merge_workspace_bytes(n: int, n_tokens: int) -> int:
     return int(lib().ajt_merge_workspace_bytes(n, n_tokens))
+
+
+def merge_workspace_bytes_for_pairs(n: int, n_tokens: int, n_pairs: int) -> int:
+    return int(lib().ajt_merge_workspace_bytes_for_pairs(n, n_tokens, n_pairs))
 
 
 def merge_host_arena_bytes(n: int, n_tokens: int) -> int:

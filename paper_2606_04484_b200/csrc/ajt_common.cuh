@@ -21,14 +21,19 @@ struct AjtCtrl {
     // merge
     int32_t n_groups;
     int32_t n_entries;    // sum_g k_g (k_g+1)/2
-    int32_t n_hash_segs;
+    int32_t n_hash_segs;  // hash slices: sum over timelines of grouped (k >= 2) groups of ceil(L / 512)
     int32_t M;
     int64_t N_out;
-    int32_t collision;    // set by the fused verify+scatter pass when a hash-equal candidate differs
+    int32_t collision;    // informational: a hash-equal candidate failed the exact comparison in the select pass
     int32_t n_tiles;
     int32_t tile_counter; // loss prep: dynamic tile ticket (ordered, so a tile's predecessors have always started)
     int32_t done_counter; // loss prep: CTAs finished (the last one finalises 1/S')
-    uint32_t reserved[48];
+    // merge (round 2)
+    int32_t n_units;      // hash units: sum over grouped groups of ceil(max L / 512)
+    int32_t unit_ticket;  // hash pass: dynamic unit ticket
+    int32_t sel_done;     // select pass: CTAs finished (the last one compacts)
+    int32_t n_gsegs;      // scatter segments (constant-source runs of the merged output)
+    uint32_t reserved[44];
 };
 static_assert(sizeof(AjtCtrl) == 256, "AjtCtrl must be 256 bytes");
 

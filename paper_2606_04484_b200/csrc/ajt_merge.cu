@@ -1,66 +1,87 @@
 // Stage (a): timeline merging (Algorithm 1) on flat token streams, sm_100a.
 //
-// Definition: DESIGN.md "O-M".  Pipeline (rows M1-M7 of the scope table), 6 launches:
-//   K1 merge_group_kernel    M1  one CTA, shared-memory resident for n <= 8192: validate offsets, stable LSD radix sort of
-//                                (traj_id - min, index), group ids, rank in group, per-timeline record {first hash segment,
-//                                group start, rank, first key slot}, lengths in group order
-//   K2 merge_hash_kernel     M2  warp-cooperative prefix-hash scan, 128-bit loads, 4 vectors in flight per lane.  The hash of
-//                                the first p tokens of timeline i is F_i(p) = sum_{q<p} x_q w(q) mod 2^64, w(q) = B^(q+3) mod 2^32: a sum, hence
-//                                a monoid, so every lane keeps its own partial and lanes are only combined (three REDUX)
-//                                where a key is emitted: at each length L_a of an earlier same-group timeline (probe key)
-//                                and at L_i itself (full key).  The positions shared with the in-group predecessor are
-//                                compared exactly on the way (the predecessor was just hashed: L2 hits)
-//   K3 merge_select_kernel   M2  (one CTA per group) per-timeline prefix over its hash windows -> final (hash, len) keys
-//                            M3  segmented radix sort of the group's keys by a 32-bit digest: one MSD pass on the top 11 bits
-//                                in shared memory (<= 2048 keys: a bucket then holds the equal-key run, mean occupancy < 1,
-//                                and keys inside it are compared exactly); 4 LSD passes through global memory above that
-//   K4   (same kernel)       M4  per full key: walk its equal-key run, pick the extender by the owner rule
-//   K6 merge_compact_kernel  M6  one CTA, one fused scan: survivors in original order -> merged_offsets/origin/traj, owner,
-//                                tile table
-//   K5/K7 merge_scatter_kernel M5+M7  fused: every merged sequence is streamed once in 256-position warp tiles; a member whose
-//                                containment is not already implied by verified predecessor links (K2) is compared
-//                                token-by-token against its owner (exact verification) while tokens / mask-OR / src /
-//                                old_logp are written with 16-byte stores; tiles that every response region covers or
-//                                misses are plain copies from one source.  A mismatch (a hash collision) raises
-//                                ctrl->collision.
-//   merge_repair_kernel      M5  one cooperative launch that exits at once unless ctrl->collision: K4 with exact comparison of
-//                                every candidate it accepts, grid barrier, K6, grid barrier, K7.  Hash collisions can therefore
-//                                never change the result.
-#include <cooperative_groups.h>
+// Definition: DESIGN.md "O-M".  Pipeline (rows M1-M7 of the scope table), 5 launches on one
+// stream, no host round trip, no cooperative launch (the call can be captured in a CUDA graph):
+//   K1 merge_group_fast_kernel  M1  one CTA, everything in shared memory (n <= 7936): trajectory ids go through a hash
+//                                   table (atomicCAS), groups are laid out by a scan over its slots, members are placed with
+//                                   an atomic cursor and ranked by counting (in-group order = input order).  Emits, by
+//                                   SORTED POSITION, {timeline, length, token offset, first hash slice, rank, first key
+//                                   slot}, and one record per HASH UNIT = (group, slice of 512 token positions).
+//                                   merge_group_radix_kernel (stable LSD radix sort through the workspace) does the same
+//                                   for larger batches.
+//   K2 merge_hash_kernel        M2  warp per hash unit (dynamic ticket): the warp streams the SAME 512 positions of every
+//                                   member of the group, in order, through a warp-private 4-stage cp.async ring (16-byte
+//                                   async copies of the aligned superset, whatever the member's alignment).  The prefix
+//                                   hash F_i(p) = sum_{q<p} x_q w(q) mod 2^64, w(q) = W^(q+3) mod 2^32, is a sum over
+//                                   positions, hence a monoid: the lane weights depend on the positions only and are
+//                                   computed once per unit; every lane keeps its partial and lanes are combined with
+//                                   three REDUX where a value leaves the warp: the slice total of every member, and one key
+//                                   per (member r, earlier member a with L_a <= L_r) whose prefix end L_a - 1 lies in this
+//                                   slice (probe keys; a = r gives the full key).
+//                               M5  (first half) member r is compared EXACTLY with member r - 1 on the way, register
+//                                   against register (both slices pass through the same lanes): a difference marks the
+//                                   link r-1 -> r broken.  Every token is loaded once; nothing is re-read.
+//   K3 merge_select_kernel      M2  (end) one CTA per group: exclusive prefix of each member's slice totals -> final keys
+//                               M3  segmented radix sort of the group's (hash, length) keys by a 32-bit digest: one MSD
+//                                   pass on the top 11 bits in shared memory (<= 2048 keys), 4 LSD passes through global
+//                                   memory above that
+//                               M4  per timeline: its equal-key run gives the hash-equal extenders; survivor flag,
+//                                   Algorithm-1 owner (latest extender), under LONGEST the longest surviving extender
+//                               M5  (second half) a candidate is ACCEPTED only if an unbroken chain of verified links
+//                                   leads to it (prefix-of is transitive) or after an exact warp-cooperative token
+//                                   comparison (128-bit loads when the two are co-aligned); a hash-equal candidate that
+//                                   fails is skipped (AJT_STATUS_HASH_COLLISION, informational).  Results are exact
+//                                   whatever the hash does (AJT_MERGE_WEAK_HASH degrades it to 4 bits to test this).
+//                                   Then per survivor: its member list and its SEGMENTS (maximal runs of positions with
+//                                   one source of mask / log-prob), warp-cooperatively.
+//                               M6  the last CTA to finish scans the timelines once: survivors in original order ->
+//                                   merged_offsets / origin / traj, owner, first segment of every merged sequence
+//   K4 merge_plan_kernel        M7  segments rebased to output positions (one 32-byte record each), and for every tile
+//                                   of 512 OUTPUT positions the first segment that touches it
+//   K5 merge_scatter_kernel     M7  warp per output tile: one record lookup, then plain coalesced copies -- lane l moves
+//                                   positions l + 32 j of the tile: tokens from the survivor, mask / src constants of the
+//                                   segment, old_logp from the supplying member -- whatever the alignment of the sources
+#include <cstdio>
+#include <cstdlib>
 
 #include "ajt_common.cuh"
 
 namespace {
 
 using namespace ajt;
-namespace cg = cooperative_groups;
 
-constexpr int kHSeg = 2048;        // hash-scan window: 2048 tokens = 16 steps x 32 lanes x 4 tokens
-constexpr int kHSegLog = 11;
-constexpr int kTile = 256;         // scatter tile (positions per warp task): 2 steps x 32 lanes x 4 tokens
+constexpr int kSl = 512;           // hash slice: 512 token positions = 16 per lane
+constexpr int kSlLog = 9;
+constexpr int kTS = 512;           // scatter tile: 512 output positions = 16 per lane
+constexpr int kTSLog = 9;
 constexpr uint32_t kW = 0x9E3779B1u;   // odd multiplier of the prefix hash's 32-bit position weights
-constexpr uint32_t inv32(uint32_t b) {  // b^-1 mod 2^32 (b odd): Newton, 3 correct bits double every step
-    uint32_t x = b;
-    for (int i = 0; i < 5; ++i) x *= 2u - b * x;
-    return x;
-}
 constexpr uint32_t cpow32(uint32_t b, uint32_t e) {
     uint32_t r = 1;
     for (; e; e >>= 1, b *= b)
         if (e & 1) r *= b;
     return r;
 }
-constexpr uint32_t kWinv = inv32(kW);
-constexpr uint32_t kW128 = cpow32(kW, 128);
-constexpr uint32_t kW2048 = cpow32(kW, 2048);
-static_assert((uint32_t)(kW * kWinv) == 1u, "modular inverse");
+constexpr uint32_t kW3 = kW * kW * kW;
+constexpr uint32_t kW32 = cpow32(kW, 32);
+constexpr uint32_t kW512 = cpow32(kW, 512);
 constexpr uint32_t kFatal = AJT_STATUS_BAD_OFFSETS | AJT_STATUS_ZERO_LEN | AJT_STATUS_PROBE_CAPACITY;
 constexpr int kSelThreads = 256;
 constexpr int kSelSmemKeys = 2048;  // groups with more keys than this sort through global memory
 constexpr int kSelBucketBits = 11;
 constexpr int kSelBuckets = 1 << kSelBucketBits;
-constexpr int kSelCacheK = 256;     // per-timeline facts of groups up to this size are staged in shared memory
+constexpr int kSelCacheK = 256;     // per-member decision state of groups up to this size lives in shared memory
 constexpr int kGrpSmemN = 7936;     // batches up to this many timelines are grouped entirely in shared memory
+constexpr int32_t kSrcNone = -1;      // segment source: nobody (mask 0)
+constexpr int32_t kSrcExplicit = -2;  // segment source: decided per token from the explicit masks of the members
+
+struct __align__(16) GSeg {   // one constant-source run of the merged output
+    int64_t out_start;        // first output position
+    int64_t tok_delta;        // token source index = output position + tok_delta
+    int64_t lp_delta;         // log-prob source index = output position + lp_delta (src >= 0); explicit: first member slot
+    int32_t src;              // supplying timeline, kSrcNone or kSrcExplicit
+    int32_t aux;              // explicit: number of members
+};
+static_assert(sizeof(GSeg) == 32, "GSeg is one 32-byte record");
 
 struct MergeParams {
     const int32_t* tokens;
@@ -84,51 +105,64 @@ struct MergeParams {
     int64_t* counts;
     // workspace
     AjtCtrl* ctrl;
-    uint32_t* gbuf[6];     // [n+1] each: global stand-ins for the group kernel's shared arrays when n > kGrpSmemN
+    uint32_t* gbuf[6];     // [n+2] each: the radix group kernel's work arrays (n > kGrpSmemN)
     int32_t* perm;         // [n] sorted position -> timeline index (groups contiguous, input order inside a group)
     int32_t* glen;         // [n] sorted position -> timeline length
-    int32_t* grp_start;    // [G+1] first sorted position of each group
-    int32_t* grp_ent;      // [G+1] first key slot of each group
-    int4* tl_rec;          // [n] BY SORTED POSITION: {first hash segment, group start (sorted position), rank in group, first key slot}
-    int32_t* tl_pos;       // [n] timeline index -> sorted position (written by the select kernel)
-    uint64_t* seg_part;    // [nseg_cap] per-window partial sums, then exclusive prefixes per timeline
-    uint64_t* ent_hash;    // [E_cap] key slot (i, a), a = 0..rank_i: in-window partial, then the final prefix hash
+    int64_t* goff;         // [n] sorted position -> token offset
+    int4* tl_rec;          // [n] BY SORTED POSITION: {first hash slice, group start (sorted position), rank in group, first key slot}
+    uint8_t* lbad;         // [n] BY SORTED POSITION: the member differs from its in-group predecessor on that one's positions (exact)
+    int4* grp_rec;         // [G+1] {group start, members, first key slot, first hash unit}
+    uint64_t* seg_part;    // [slice_cap] per (member, slice) hash totals, then exclusive prefixes per member
+    uint64_t* ent_hash;    // [E_cap] key slot (r, a), a = 0..r: in-slice partial, then the final prefix hash
     uint32_t* ent_dig;     // [E_cap] global sort path: digests / order ping-pong
     uint32_t* ent_idx;     // [E_cap]
     uint32_t* tmp_dig;     // [E_cap]
     uint32_t* tmp_idx;     // [E_cap]
-    uint8_t* absorbed;     // [n]
-    uint8_t* link_bad;     // [n] 1: timeline i was compared with its in-group predecessor (hash pass) and is NOT an extension of it
-    uint8_t* needv;        // [n] 1: absorbed timeline whose owner is not implied by a chain of verified predecessor links
+    uint8_t* absorbed;     // [n] by timeline
     int32_t* owner_tl;     // [n] owning timeline (itself for survivors)
-    int32_t* cand;         // [n] staging of the LONGEST owner while owner_tl is still being read
     int32_t* midx;         // [n] merged index of survivors, -1 otherwise
-    int32_t* tile_base;    // [M+1] first scatter tile of each merged sequence
+    int32_t* sel[8];       // [n] each, by sorted position: decision state of groups larger than kSelCacheK
+    int2* sel_q;           // [n] by sorted position: their verification queue
+    int32_t* mem_list;     // [n] members of every survivor (timeline indices, ascending), grouped by survivor
+    int4* sv_rec;          // [n] by timeline, survivors only: {first member slot, members, first relative segment, segments}
+    int2* rseg;            // [2n] relative segments {first position, source}
+    int32_t* gseg_base;    // [M+1] first global segment of each merged sequence
+    GSeg* gseg;            // [2n+1] global segments, ascending output position; the last one is a sentinel at N_out
+    int32_t* tile_seg;     // [tile_cap] segment holding the first position of each output tile
     int32_t E_cap;
-    int32_t nseg_cap;
+    int32_t slice_cap;
     int32_t mis;           // (address of tokens / 4) mod 4: element misalignment of the token array vs 16 bytes
 };
 
 struct MergeWs {
-    size_t ctrl, gbuf[6], perm, glen, grp_start, grp_ent, tl_rec, tl_pos, seg_part, absorbed, link_bad, needv, owner_tl, cand, midx, tile_base, ent;
+    size_t ctrl, gbuf[6], perm, glen, goff, tl_rec, lbad, grp_rec, seg_part, absorbed, owner_tl, midx, sel[8],
+        sel_q, mem_list, sv_rec, rseg, gseg_base, gseg, tile_seg, ent;
 };
 __host__ inline size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
-__host__ inline int32_t nseg_capacity(int32_t n, int64_t N) { return (int32_t)(N / kHSeg + 2 * (int64_t)n + 2); }
+__host__ inline int64_t slice_capacity(int32_t n, int64_t N) { return N / kSl + (int64_t)n + 2; }
 
 __host__ MergeWs merge_ws_layout(int32_t n, int64_t N) {
     MergeWs w;
     size_t o = 0;
-    const size_t n4 = a256(((size_t)n + 2) * 4);
+    const size_t n4 = a256(((size_t)n + 2) * 4), n8 = a256(((size_t)n + 2) * 8), n16 = a256(((size_t)n + 2) * 16);
+    const size_t sc = (size_t)slice_capacity(n, N);
     w.ctrl = o; o += 256;
-    for (int k = 0; k < 6; ++k) { w.gbuf[k] = o; o += n4; }
-    w.perm = o; o += n4; w.glen = o; o += n4; w.grp_start = o; o += n4; w.grp_ent = o; o += n4;
-    w.tl_rec = o; o += a256(((size_t)n + 1) * 16);
-    w.tl_pos = o; o += n4;
-    w.seg_part = o; o += a256((size_t)nseg_capacity(n, N) * 8);
-    w.absorbed = o; o += a256((size_t)n + 1);
-    w.link_bad = o; o += a256((size_t)n + 1);
-    w.needv = o; o += a256((size_t)n + 1);
-    w.owner_tl = o; o += n4; w.cand = o; o += n4; w.midx = o; o += n4; w.tile_base = o; o += n4;
+    for (int k = 0; k < 6; ++k) { w.gbuf[k] = o; o += n > kGrpSmemN ? n4 : 0; }
+    w.perm = o; o += n4; w.glen = o; o += n4; w.goff = o; o += n8;
+    w.tl_rec = o; o += n16;
+    w.lbad = o; o += a256((size_t)n + 2);
+    w.grp_rec = o; o += n16;
+    w.seg_part = o; o += a256(sc * 8);
+    w.absorbed = o; o += a256((size_t)n + 2);
+    w.owner_tl = o; o += n4; w.midx = o; o += n4;
+    for (int k = 0; k < 8; ++k) { w.sel[k] = o; o += n4; }
+    w.sel_q = o; o += n8;
+    w.mem_list = o; o += n4;
+    w.sv_rec = o; o += n16;
+    w.rseg = o; o += a256(((size_t)n + 1) * 16);
+    w.gseg_base = o; o += n4;
+    w.gseg = o; o += a256(((size_t)2 * n + 2) * sizeof(GSeg));
+    w.tile_seg = o; o += a256(((size_t)(N >> kTSLog) + 2) * 4);
     w.ent = o;
     return w;
 }
@@ -143,53 +177,45 @@ __device__ __forceinline__ uint32_t digest32(uint64_t h, int32_t len) {
     z ^= z >> 32;
     return (uint32_t)z;
 }
-__device__ __forceinline__ uint64_t warp_sum_u64(uint64_t v) {
-#pragma unroll
-    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
+__device__ __forceinline__ uint64_t mad_wide(uint32_t a, uint32_t b, uint64_t c) { return (uint64_t)a * b + c; }
+// Sum of a 64-bit value over the warp (mod 2^64) with three REDUX instead of ten shuffles: 22 + 22 + 20-bit slices, whose
+// 32-term sums fit 32 bits.
+__device__ __forceinline__ uint64_t warp_sum_u64_redux(uint64_t v) {
+    const uint32_t a = (uint32_t)v & 0x3fffffu, b = (uint32_t)(v >> 22) & 0x3fffffu, c = (uint32_t)(v >> 44);
+    const uint32_t sa = __reduce_add_sync(0xffffffffu, a), sb = __reduce_add_sync(0xffffffffu, b);
+    const uint32_t sc = __reduce_add_sync(0xffffffffu, c);
+    return (uint64_t)sa + ((uint64_t)sb << 22) + ((uint64_t)sc << 44);
 }
-__device__ __forceinline__ int64_t tl_len(const MergeParams& p, int i) { return __ldg(p.offsets + i + 1) - __ldg(p.offsets + i); }
-
-// Last index i in [0, n) with key(i) <= x, for a non-decreasing key with key(0) <= x: warp-cooperative 32-ary search
-// (3 dependent loads for n <= 32768 instead of 15).
-template <class F>
-__device__ __forceinline__ int warp_search_last_le(int n, int64_t x, F key) {
-    const int lane = threadIdx.x & 31;
-    int lo = 0, hi = n;  // key(lo) <= x; hi == n or key(hi) > x
-    while (hi - lo > 1) {
-        const int step = (hi - lo + 31) >> 5;
-        const int idx = lo + (lane + 1) * step;
-        const bool le = idx < hi && (int64_t)key(idx) <= x;
-        const int cnt = __popc(__ballot_sync(0xffffffffu, le));
-        const int nlo = lo + cnt * step;
-        hi = min(hi, nlo + step);
-        lo = nlo;
-    }
-    return lo;
+__device__ __forceinline__ int64_t shfl_i64(int64_t v, int src) {
+    const uint32_t lo = __shfl_sync(0xffffffffu, (uint32_t)v, src), hi = __shfl_sync(0xffffffffu, (uint32_t)((uint64_t)v >> 32), src);
+    return (int64_t)(((uint64_t)hi << 32) | lo);
 }
+template <class T>
+__device__ __forceinline__ T ldcg(const T* p) { return __ldcg(p); }
 
 // ---------------------------------------------------------------------------------------- block-level building blocks
 
 // Exclusive scan of the pair f(i) = (a, b), i in [0,n), by one CTA of NT threads; g(i, ex_a, ex_b, a, b) consumes it.
-// Each thread owns kIpt consecutive items of a tile of NT * kIpt, so a tile costs one warp scan, one __syncthreads and one
-// shuffle scan of the NT / 32 warp totals (double-buffered), whatever kIpt is.  Returns the totals to every thread.
+// Each thread owns IPT consecutive items of a tile of NT * IPT (their loads are independent: one memory round trip per
+// tile), so a tile costs one warp scan, one __syncthreads and one shuffle scan of the NT / 32 warp totals (double-buffered).
+// Returns the totals to every thread.
 struct I2 {
     int64_t a, b;
 };
-constexpr int kIpt = 4;
-template <int NT, class F, class G>
+template <int NT, int IPT, class F, class G>
 __device__ __forceinline__ I2 block_scan2(int n, F f, G g, int64_t (*s_w)[2][NT / 32]) {
     static_assert(NT / 32 <= 32, "warp totals are scanned by one warp's lanes");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     I2 base = {0, 0};
     int buf = 0;
-    for (int i0 = 0; i0 < n; i0 += NT * kIpt, buf ^= 1) {
-        const int b0 = i0 + tid * kIpt;
-        I2 v[kIpt];
+    for (int i0 = 0; i0 < n; i0 += NT * IPT, buf ^= 1) {
+        const int b0 = i0 + tid * IPT;
+        I2 v[IPT];
         int64_t sa = 0, sb = 0;
 #pragma unroll
-        for (int k = 0; k < kIpt; ++k) {
-            v[k] = b0 + k < n ? f(b0 + k) : I2{0, 0};
+        for (int k = 0; k < IPT; ++k) v[k] = b0 + k < n ? f(b0 + k) : I2{0, 0};
+#pragma unroll
+        for (int k = 0; k < IPT; ++k) {
             sa += v[k].a;
             sb += v[k].b;
         }
@@ -212,7 +238,7 @@ __device__ __forceinline__ I2 block_scan2(int n, F f, G g, int64_t (*s_w)[2][NT 
         const int64_t ta = __shfl_sync(0xffffffffu, ja, NT / 32 - 1), tb = __shfl_sync(0xffffffffu, jb, NT / 32 - 1);
         int64_t ra = base.a + pa + ia - sa, rb = base.b + pb + ib - sb;
 #pragma unroll
-        for (int k = 0; k < kIpt; ++k) {
+        for (int k = 0; k < IPT; ++k) {
             if (b0 + k < n) g(b0 + k, ra, rb, v[k].a, v[k].b);
             ra += v[k].a;
             rb += v[k].b;
@@ -222,9 +248,9 @@ __device__ __forceinline__ I2 block_scan2(int n, F f, G g, int64_t (*s_w)[2][NT 
     __syncthreads();
     return base;
 }
-template <int NT, class F, class G>
+template <int NT, int IPT, class F, class G>
 __device__ __forceinline__ int64_t block_scan(int n, F f, G g, int64_t (*s_w)[2][NT / 32]) {
-    return block_scan2<NT>(
+    return block_scan2<NT, IPT>(
                n, [&](int i) { return I2{(int64_t)f(i), 0}; }, [&](int i, int64_t ex, int64_t, int64_t v, int64_t) { g(i, ex, v); },
                s_w)
         .a;
@@ -250,25 +276,17 @@ struct RadixScratch {
 
 // One stable LSD pass (digit of nbits <= 8 bits at `shift`) of (key, value) pairs by one CTA of NW warps.  Warp w owns the w-th
 // contiguous chunk of the input, so "chunk, then round, then lane" is input order.  Count: per round, lanes with equal
-// digits find each other with match.any and the lowest lane of each peer set adds the set size to cnt[w][digit].  Offsets:
+// digits find each other (peers8) and the lowest lane of each peer set adds the set size to cnt[w][digit].  Offsets:
 // one thread per digit turns the NW counts into running offsets, one warp scans the 256 digit totals.  Scatter: the same
 // rounds again, position = digit base + warp offset + rank in peer set.  Four __syncthreads per pass, whatever n is.
-#ifdef AJT_TIMING
-__device__ uint64_t g_rt[8];
-#define AJT_RT(k) do { __syncthreads(); if (threadIdx.x == 0) { uint64_t t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_rt[k] = t_; } } while (0)
-#else
-#define AJT_RT(k) do { } while (0)
-#endif
 template <int NW>
 __device__ __forceinline__ void radix_pass(const uint32_t* kin, const uint32_t* vin, uint32_t* kout, uint32_t* vout, int n,
                                            int shift, RadixScratch<NW>& sc, int nbits = 8) {
     const uint32_t dmask = (1u << nbits) - 1u;
-    AJT_RT(0);
     constexpr int NT = NW * 32;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (int x = tid; x < NW * 256; x += NT) (&sc.cnt[0][0])[x] = 0;
     __syncthreads();
-    AJT_RT(1);
     const int per = ((n + NW - 1) / NW + 31) & ~31;
     const int c0 = min(n, warp * per), c1 = min(n, c0 + per);
     for (int base = c0; base < c1; base += 32) {
@@ -280,7 +298,6 @@ __device__ __forceinline__ void radix_pass(const uint32_t* kin, const uint32_t* 
         __syncwarp();
     }
     __syncthreads();
-    AJT_RT(2);
     for (int d2 = tid; d2 < 256; d2 += NT) {
         uint32_t run = 0;
 #pragma unroll 4
@@ -292,7 +309,6 @@ __device__ __forceinline__ void radix_pass(const uint32_t* kin, const uint32_t* 
         sc.off[d2] = run;
     }
     __syncthreads();
-    AJT_RT(3);
     if (warp == 0) {  // exclusive scan of the 256 digit totals: 8 per lane
         uint32_t loc[8], s = 0;
 #pragma unroll
@@ -308,7 +324,6 @@ __device__ __forceinline__ void radix_pass(const uint32_t* kin, const uint32_t* 
         for (int j = 0; j < 8; ++j) { sc.off[lane * 8 + j] = run; run += loc[j]; }
     }
     __syncthreads();
-    AJT_RT(4);
     for (int base = c0; base < c1; base += 32) {
         const int i = base + lane;
         const bool valid = i < c1;
@@ -327,39 +342,250 @@ __device__ __forceinline__ void radix_pass(const uint32_t* kin, const uint32_t* 
         __syncwarp();
     }
     __syncthreads();
-    AJT_RT(5);
+}
+
+// Fatal status found while grouping: the later kernels return at once; the counts a caller may chain on are not garbage.
+__device__ __forceinline__ void group_fail(const MergeParams& p, uint32_t bits) {
+    atomicOr(&p.ctrl->status, bits);
+    p.counts[0] = 0;
+    p.counts[1] = 0;
+    p.merged_offsets[0] = 0;
 }
 
 // ---------------------------------------------------------------------------------------- K1: group (M1)
 
-#ifdef AJT_TIMING
-#define AJT_TICK(k) do { __syncthreads(); if (threadIdx.x == 0) { uint64_t t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); tick_[k] = t_; } } while (0)
+constexpr uint32_t kEmpty = 0xFFFFFFFFu;
+#ifdef AJT_PROF
+__device__ __forceinline__ uint64_t gtimer() { uint64_t t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define AJT_TICK(k) do { __syncthreads(); if (threadIdx.x == 0) reinterpret_cast<unsigned long long*>(p.ctrl->reserved)[k] = gtimer(); } while (0)
+#define AJT_TMAX(k) do { if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned long long*>(p.ctrl->reserved) + (k), (unsigned long long)gtimer()); } while (0)
+#define AJT_TMIN(k) do { if (threadIdx.x == 0) atomicMin(reinterpret_cast<unsigned long long*>(p.ctrl->reserved) + (k), (unsigned long long)gtimer()); } while (0)
 #else
 #define AJT_TICK(k) do { } while (0)
+#define AJT_TMAX(k) do { } while (0)
+#define AJT_TMIN(k) do { } while (0)
 #endif
-template <bool kSmem>
-__global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) {
-#ifdef AJT_TIMING
-    uint64_t tick_[10] = {0};
-#endif
-    AJT_TICK(0);
+
+// n <= kGrpSmemN.  Dynamic shared memory (H = hash-table slots, passed by the host; G <= n groups):
+//   B1 [H+2] u32  table keys              -> members per group -> group starts (sorted position, exclusive scan)
+//   B2 [H+2] u16  group of each table slot -> timeline by sorted position
+//   B3 [n+2] u32  length by timeline
+//   B4 [n+2] u32  per-group cursor        -> key slots per group (-> exclusive scan)
+//   B5 [n+2] u32  longest member of group -> hash units per group (-> exclusive scan)
+//   B6 [n]   u16  table slot by timeline  -> group by timeline
+//   B7 [n]   u16  members as placed (unordered inside a group)
+//   B9 [n+2] u32  first hash slice by sorted position
+// One SM does all of this, so what counts is shared-memory wavefronts and dependent global round trips (~0.8 us each): the
+// members of a group are put in order by a warp-wide bitonic network (shuffles), and every global store is coalesced.
+__global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParams p, const int H) {
     extern __shared__ __align__(16) uint8_t g_dyn[];
+    __shared__ int64_t s_w[2][2][32];
+    __shared__ uint32_t s_bad, s_ng;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = p.n;
+    uint32_t* const B1 = reinterpret_cast<uint32_t*>(g_dyn);
+    uint16_t* const B2 = reinterpret_cast<uint16_t*>(B1 + (H + 2));
+    uint32_t* const B3 = reinterpret_cast<uint32_t*>(B2 + ((H + 3) & ~1));
+    uint32_t* const B4 = B3 + (n + 2);
+    uint32_t* const B5 = B4 + (n + 2);
+    uint32_t* const B9 = B5 + (n + 2);
+    uint16_t* const B6 = reinterpret_cast<uint16_t*>(B9 + (n + 2));
+    uint16_t* const B7 = B6 + ((n + 1) & ~1);
+    uint16_t* const B8 = B2;
+    if (tid < (int)(sizeof(AjtCtrl) / 4)) reinterpret_cast<uint32_t*>(p.ctrl)[tid] = 0;   // fresh control block
+    if (tid == 0) { s_bad = 0; s_ng = 0; }
+#pragma unroll 1
+    for (int s = tid; s < H + 2; s += 1024) B1[s] = kEmpty;
+#pragma unroll 1
+    for (int g = tid; g < n + 2; g += 1024) { B4[g] = 0; B5[g] = 0; }
+    __syncthreads();
+    AJT_TICK(0);
+    // ---- validate offsets; trajectory id -> table slot; the thread that claims a slot numbers the group
+    uint32_t bad = 0;
+#pragma unroll 1
+    for (int i0 = tid; i0 < n; i0 += 8 * 1024) {
+        int64_t a[8], b[8];
+        uint32_t t[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {   // all loads of eight timelines in flight at once: one cold round trip (~2 us)
+            const int i = i0 + u * 1024;
+            const bool v = i < n;
+            a[u] = v ? __ldg(p.offsets + i) : 0;
+            b[u] = v ? __ldg(p.offsets + i + 1) : 1;
+            t[u] = v ? (uint32_t)__ldg(p.traj_ids + i) : 0u;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int i = i0 + u * 1024;
+            if (i >= n) break;
+            if (b[u] < a[u] || b[u] - a[u] > (int64_t)INT32_MAX) bad |= AJT_STATUS_BAD_OFFSETS;
+            else if (b[u] == a[u]) bad |= AJT_STATUS_ZERO_LEN;
+            uint32_t h = (uint32_t)H;   // the id that doubles as the empty marker has a slot of its own
+            uint32_t prev = kEmpty;
+            if (t[u] != kEmpty) {
+                h = __umulhi(t[u] * 0x9E3779B1u, (uint32_t)H);
+                while (true) {
+                    prev = atomicCAS(&B1[h], kEmpty, t[u]);
+                    if (prev == kEmpty || prev == t[u]) break;
+                    h = h + 1 == (uint32_t)H ? 0u : h + 1;
+                }
+            } else {
+                prev = atomicCAS(&B1[h], kEmpty, 0u);
+            }
+            if (prev == kEmpty) B2[h] = (uint16_t)atomicAdd(&s_ng, 1u);
+            B6[i] = (uint16_t)h;
+            B3[i] = (uint32_t)a[u];
+        }
+    }
+    if (tid == 0 && (__ldg(p.offsets) != 0 || __ldg(p.offsets + n) != p.N)) bad |= AJT_STATUS_BAD_OFFSETS;
+    if (tid == 0) B3[n] = (uint32_t)p.N;
+    bad = __reduce_or_sync(0xffffffffu, bad);
+    if ((tid & 31) == 0 && bad) atomicOr(&s_bad, bad);
+    __syncthreads();
+    if (s_bad) {
+        if (tid == 0) group_fail(p, s_bad);
+        return;
+    }
+    const int G = (int)s_ng;
+    AJT_TICK(1);
+    // ---- the table keys are done: B1 becomes the per-group member count
+#pragma unroll 1
+    for (int i = tid; i < n; i += 1024) B6[i] = B2[B6[i]];
+#pragma unroll 1
+    for (int g = tid; g <= G; g += 1024) B1[g] = 0;
+    __syncthreads();
+#pragma unroll 1
+    for (int i = tid; i < n; i += 1024) {
+        const uint32_t g = B6[i];
+        atomicAdd(&B1[g], 1u);
+        atomicMax(&B5[g], B3[i + 1] - B3[i]);
+    }
+    __syncthreads();
+    AJT_TICK(2);
+    block_scan<1024, 8>(
+        G + 1, [&](int g) { return g < G ? B1[g] : 0u; }, [&](int g, int64_t ex, int64_t) { B1[g] = (uint32_t)ex; }, s_w);
+    AJT_TICK(3);
+    // ---- place the members (any order inside a group) ...
+#pragma unroll 1
+    for (int i = tid; i < n; i += 1024) {
+        const uint32_t g = B6[i];
+        B7[B1[g] + atomicAdd(&B4[g], 1u)] = (uint16_t)i;
+    }
+    __syncthreads();
+    AJT_TICK(12);
+    // ---- ... and put them in input order, one warp per group: a bitonic network over the lanes for groups of up to 32
+    // (15 shuffles), ranking by counting (members are read as broadcasts) for larger ones
+#pragma unroll 1
+    for (int g0 = warp; g0 < G; g0 += 2 * 32) {   // two groups per warp at a time: two independent shuffle chains
+        uint32_t gs[2], k[2], v0[2], v1[2];       // a group of up to 64: elements lane and lane + 32
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int g = g0 + 32 * u;
+            gs[u] = g < G ? B1[g] : 0u;
+            k[u] = g < G ? B1[g + 1] - gs[u] : 0u;
+            const bool net = k[u] <= 64;
+            v0[u] = net && (uint32_t)lane < k[u] ? B7[gs[u] + lane] : 0xFFFFu;
+            v1[u] = net && (uint32_t)lane + 32 < k[u] ? B7[gs[u] + lane + 32] : 0xFFFFu;
+        }
+        const bool wide = k[0] > 32 || k[1] > 32;   // warp-uniform: the 32-wide network is enough otherwise
+#pragma unroll
+        for (int sz = 2; sz <= 64; sz <<= 1) {
+            if (sz == 64 && !wide) break;
+#pragma unroll
+            for (int st = sz >> 1; st > 0; st >>= 1) {
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    if (st == 32) {   // partner of element e is e ^ 32: the lane's other register; block of 64 ascending
+                        const uint32_t lo = min(v0[u], v1[u]), hi = max(v0[u], v1[u]);
+                        v0[u] = lo; v1[u] = hi;
+                    } else {
+                        const uint32_t o0 = __shfl_xor_sync(0xffffffffu, v0[u], st), o1 = __shfl_xor_sync(0xffffffffu, v1[u], st);
+                        const bool lower = (lane & st) == 0;
+                        // direction of the block of size sz that holds the element: ascending iff (e & sz) == 0
+                        const bool up0 = sz == 64 ? true : (lane & sz) == 0;
+                        const bool up1 = sz == 64 ? true : (sz == 32 ? false : (lane & sz) == 0);
+                        v0[u] = (lower == up0) ? min(v0[u], o0) : max(v0[u], o0);
+                        v1[u] = (lower == up1) ? min(v1[u], o1) : max(v1[u], o1);
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            if (k[u] <= 64) {
+                if ((uint32_t)lane < k[u]) B8[gs[u] + lane] = (uint16_t)v0[u];
+                if ((uint32_t)lane + 32 < k[u]) B8[gs[u] + lane + 32] = (uint16_t)v1[u];
+            } else {
+                for (uint32_t m = lane; m < k[u]; m += 32) {
+                    const uint32_t i = B7[gs[u] + m];
+                    uint32_t r = 0;
+#pragma unroll 4
+                    for (uint32_t x = 0; x < k[u]; ++x) r += B7[gs[u] + x] < i ? 1u : 0u;
+                    B8[gs[u] + r] = (uint16_t)i;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    AJT_TICK(4);
+    // ---- key slots and hash units by group (two scans), hash slices by sorted position (one scan)
+    const int64_t E = block_scan<1024, 8>(
+        G + 1, [&](int g) { const int64_t k = g < G ? B1[g + 1] - B1[g] : 0; return k * (k + 1) / 2; },
+        [&](int g, int64_t ex, int64_t) { B4[g] = (uint32_t)min(ex, (int64_t)INT32_MAX); }, s_w);
+    const int64_t U = block_scan<1024, 8>(
+        G + 1, [&](int g) { return g < G && B1[g + 1] - B1[g] >= 2 ? (B5[g] + kSl - 1) >> kSlLog : 0u; },
+        [&](int g, int64_t ex, int64_t) { B5[g] = (uint32_t)ex; }, s_w);
+    if (E > (int64_t)p.E_cap) {   // (slices and units always fit: the workspace is sized for their worst case)
+        if (tid == 0) group_fail(p, (uint32_t)AJT_STATUS_PROBE_CAPACITY);
+        return;
+    }
+    AJT_TICK(5);
+    const int64_t nslice = block_scan<1024, 8>(
+        n,
+        [&](int pos) {
+            const uint32_t i = B8[pos], g = B6[i];
+            return B1[g + 1] - B1[g] < 2 ? 0u : (B3[i + 1] - B3[i] + kSl - 1) >> kSlLog;
+        },
+        [&](int pos, int64_t ex, int64_t) { B9[pos] = (uint32_t)ex; }, s_w);
+    // ---- records by sorted position: coalesced stores.  A lone SM cannot afford 7,862 scattered 8-byte loads (one sector
+    // each, ~15 us), so the token offsets come from the 32-bit copies kept since the first phase whenever N < 2^32.
+    const bool off32 = p.N < ((int64_t)1 << 32);
+    AJT_TICK(15);
+#pragma unroll 2
+    for (int pos = tid; pos < n; pos += 1024) {
+        const uint32_t i = B8[pos], g = B6[i], gs = B1[g], r = (uint32_t)pos - gs;
+        p.tl_rec[pos] = make_int4((int)B9[pos], (int)gs, (int)r, (int)(B4[g] + r * (r + 1) / 2u));
+        p.perm[pos] = (int32_t)i;
+        p.glen[pos] = (int32_t)(B3[i + 1] - B3[i]);
+        p.goff[pos] = off32 ? (int64_t)B3[i] : __ldg(p.offsets + i);
+        p.lbad[pos] = 0;
+    }
+    AJT_TICK(6);
+#pragma unroll 1
+    for (int g = tid; g <= G; g += 1024)
+        p.grp_rec[g] = make_int4((int)B1[g], g < G ? (int)(B1[g + 1] - B1[g]) : 0, (int)B4[g], (int)B5[g]);
+    if (tid == 0) {
+        p.ctrl->n_groups = G;
+        p.ctrl->n_entries = (int32_t)E;
+        p.ctrl->n_hash_segs = (int32_t)nslice;
+        p.ctrl->n_units = (int32_t)U;
+    }
+    AJT_TICK(7);
+}
+
+// The same for any n: a stable LSD radix sort of (traj_id - min, index) and block scans, through arrays in the workspace.
+__global__ void __launch_bounds__(1024) merge_group_radix_kernel(const MergeParams p) {
     __shared__ RadixScratch<32> sc;
     __shared__ int64_t s_w[2][2][32];
     __shared__ int s_min, s_max;
     __shared__ uint32_t s_bad;
     const int tid = threadIdx.x, n = p.n;
-    // five [n+1] work arrays: shared memory for n <= kGrpSmemN, the workspace otherwise
-    const size_t nn = ((size_t)n + 4) & ~(size_t)3;   // (6 arrays of nn words)
-    uint32_t* const sm32 = reinterpret_cast<uint32_t*>(g_dyn);
-    uint32_t* kb[2] = {kSmem ? sm32 : p.gbuf[0], kSmem ? sm32 + nn : p.gbuf[1]};
-    uint32_t* vb[2] = {kSmem ? sm32 + 2 * nn : p.gbuf[2], kSmem ? sm32 + 3 * nn : p.gbuf[3]};
-    int32_t* nsg = reinterpret_cast<int32_t*>(kSmem ? sm32 + 4 * nn : p.gbuf[4]);   // [i] hash windows of timeline i
-    int32_t* tln = reinterpret_cast<int32_t*>(kSmem ? sm32 + 5 * nn : p.gbuf[5]);   // [i] its length
+    uint32_t* kb[2] = {p.gbuf[0], p.gbuf[1]};
+    uint32_t* vb[2] = {p.gbuf[2], p.gbuf[3]};
+    uint32_t* gun = p.gbuf[4];                                   // [g] hash units of group g, then their exclusive scan
+    int32_t* tln = reinterpret_cast<int32_t*>(p.gbuf[5]);        // [i] length of timeline i
     if (tid < (int)(sizeof(AjtCtrl) / 4)) reinterpret_cast<uint32_t*>(p.ctrl)[tid] = 0;   // fresh control block
     if (tid == 0) { s_min = INT32_MAX; s_max = INT32_MIN; s_bad = 0; }
     __syncthreads();
-    // validate offsets; min / max traj id; hash windows per timeline
     int lmin = INT32_MAX, lmax = INT32_MIN;
     uint32_t bad = 0;
 #pragma unroll 4
@@ -372,11 +598,8 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
         lmax = max(lmax, t);
         kb[0][i] = (uint32_t)t;
         vb[0][i] = (uint32_t)i;
-        nsg[i] = (int32_t)(((b - 1 + p.mis) >> kHSegLog) - ((a + p.mis) >> kHSegLog) + 1);
         tln[i] = (int32_t)(b - a);
-        p.link_bad[i] = 0;
     }
-    AJT_TICK(1);
     if (tid == 0 && (p.offsets[0] != 0 || p.offsets[n] != p.N)) bad |= AJT_STATUS_BAD_OFFSETS;
     lmin = __reduce_min_sync(0xffffffffu, lmin);
     lmax = __reduce_max_sync(0xffffffffu, lmax);
@@ -388,256 +611,82 @@ __global__ void __launch_bounds__(1024) merge_group_kernel(const MergeParams p) 
     }
     __syncthreads();
     if (s_bad) {
-        if (tid == 0) atomicOr(&p.ctrl->status, s_bad);
+        if (tid == 0) group_fail(p, s_bad);
         return;
     }
-    AJT_TICK(7);
     const int tmin = s_min;
     const uint32_t range = n ? (uint32_t)s_max - (uint32_t)tmin : 0u;
     for (int i = tid; i < n; i += 1024) kb[0][i] -= (uint32_t)tmin;
     __syncthreads();
-    AJT_TICK(8);
     int cur = 0;
     for (int shift = 0; shift < 32 && (range >> shift) != 0; shift += 8) {
         radix_pass<32>(kb[cur], vb[cur], kb[cur ^ 1], vb[cur ^ 1], n, shift, sc);
         cur ^= 1;
         __syncthreads();
     }
-    AJT_TICK(2);
     const uint32_t* key = kb[cur];
     const uint32_t* val = vb[cur];   // sorted position -> timeline index
     uint32_t* gid = kb[cur ^ 1];     // [pos] group id
     uint32_t* gsv = vb[cur ^ 1];     // [g]   first sorted position of group g
-    // group ids and group starts
-    const int G = (int)block_scan<1024>(
+    const int G = (int)block_scan<1024, 4>(
         n, [&](int pos) { return (pos == 0 || key[pos] != key[pos - 1]) ? 1 : 0; },
         [&](int pos, int64_t ex, int64_t v) {
             const int g = (int)(ex + v) - 1;
             gid[pos] = (uint32_t)g;
-            if (v) { gsv[g] = (uint32_t)pos; p.grp_start[g] = pos; }
+            if (v) gsv[g] = (uint32_t)pos;
         },
         s_w);
-    if (tid == 0) { gsv[G] = (uint32_t)n; p.grp_start[G] = n; }
+    if (tid == 0) gsv[G] = (uint32_t)n;
     __syncthreads();
-    AJT_TICK(3);
-    // key slots (i, a), a = 0..rank_i: a group of k timelines has k(k+1)/2, the slots of rank r start r(r+1)/2 into it
+    // key slots (r, a), a = 0..r: a group of k timelines has k(k+1)/2, the slots of rank r start r(r+1)/2 into it
     uint32_t* gent = kb[cur];        // [g] first key slot of group g (the sorted keys are no longer needed)
-    const int64_t E = block_scan<1024>(
+    const int64_t E = block_scan<1024, 4>(
         G, [&](int g) { const int64_t k = gsv[g + 1] - gsv[g]; return k * (k + 1) / 2; },
-        [&](int g, int64_t ex, int64_t) {
-            gent[g] = (uint32_t)min(ex, (int64_t)INT32_MAX);
-            p.grp_ent[g] = (int32_t)min(ex, (int64_t)INT32_MAX);
+        [&](int g, int64_t ex, int64_t) { gent[g] = (uint32_t)min(ex, (int64_t)INT32_MAX); }, s_w);
+    // hash units of a group = slices up to its longest member (none for singleton groups)
+    const int64_t U = block_scan<1024, 1>(
+        G,
+        [&](int g) {
+            const int k = (int)(gsv[g + 1] - gsv[g]);
+            if (k < 2) return (int64_t)0;
+            int mx = 0;
+            for (int x = 0; x < k; ++x) mx = max(mx, tln[val[gsv[g] + x]]);
+            return (int64_t)((mx + kSl - 1) >> kSlLog);
         },
-        s_w);
-    AJT_TICK(4);
-    // hash segments: aligned windows of kHSeg tokens intersected with each timeline (none for singleton groups), numbered in
-    // GROUP order, so that a timeline is hashed right after its in-group predecessor.  Everything the later kernels need
-    // per timeline goes out by sorted position: coalesced, no scattered access from this one CTA.
-    const int64_t nseg = block_scan<1024>(
-        n, [&](int pos) { const int g = (int)gid[pos]; return gsv[g + 1] - gsv[g] < 2 ? 0 : nsg[val[pos]]; },
+        [&](int g, int64_t ex, int64_t) { gun[g] = (uint32_t)ex; }, s_w);
+    if (tid == 0) { gent[G] = (uint32_t)min(E, (int64_t)INT32_MAX); gun[G] = (uint32_t)U; }
+    // hash slices: numbered in GROUP order, by sorted position
+    const int64_t nslice = block_scan<1024, 4>(
+        n, [&](int pos) { const int g = (int)gid[pos]; return gsv[g + 1] - gsv[g] < 2 ? 0 : (tln[val[pos]] + kSl - 1) >> kSlLog; },
         [&](int pos, int64_t ex, int64_t) {
             const int i = (int)val[pos], g = (int)gid[pos];
             const int gs = (int)gsv[g], r = pos - gs;
             p.tl_rec[pos] = make_int4((int)ex, gs, r, (int)(gent[g] + (uint32_t)r * (uint32_t)(r + 1) / 2u));
             p.perm[pos] = i;
             p.glen[pos] = tln[i];
+            p.goff[pos] = __ldg(p.offsets + i);
+            p.lbad[pos] = 0;
         },
         s_w);
-    AJT_TICK(5);
-    if (tid == 0) {
-        p.grp_ent[G] = (int32_t)min(E, (int64_t)INT32_MAX);
-        p.ctrl->n_groups = G;
-        p.ctrl->n_entries = (int32_t)min(E, (int64_t)INT32_MAX);
-        p.ctrl->n_hash_segs = (int32_t)nseg;
-        if (E > (int64_t)p.E_cap || nseg > (int64_t)p.nseg_cap) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_PROBE_CAPACITY);
-    }
-    AJT_TICK(6);
-#ifdef AJT_TIMING
-    if (tid == 0) {
-        for (int k = 0; k < 7; ++k) reinterpret_cast<uint64_t*>(p.ctrl->reserved)[k] = tick_[k];
-        reinterpret_cast<uint64_t*>(p.ctrl->reserved)[14] = tick_[7];
-        reinterpret_cast<uint64_t*>(p.ctrl->reserved)[15] = tick_[8];
-        for (int k = 0; k < 6; ++k) reinterpret_cast<uint64_t*>(p.ctrl->reserved)[8 + k] = g_rt[k];
-    }
-#endif
-}
-
-// ---- K1 for batches that fit in shared memory (n <= kGrpSmemN): the same steps written for a SMALL CODE FOOTPRINT.  A
-// merge call streams hundreds of MB through L2 between two launches of this kernel, so its instructions come from DRAM every
-// time, and a one-CTA kernel that runs each line once pays for every 128-byte line it touches: loops are not unrolled, and
-// the scans share one out-of-line routine working in place on shared arrays.
-
-// In-place exclusive scan of a[0..n) by the CTA (1024 threads); returns the total to every thread.
-__device__ __noinline__ uint32_t cta_scan_excl(uint32_t* a, int n, uint32_t* s_wt) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    uint32_t base = 0;
-#pragma unroll 1
-    for (int i0 = 0; i0 < n; i0 += 1024) {
-        const int i = i0 + tid;
-        const uint32_t v = i < n ? a[i] : 0u;
-        uint32_t inc = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
-        }
-        if (lane == 31) s_wt[warp] = inc;
-        __syncthreads();
-        const uint32_t wv = s_wt[lane];
-        uint32_t winc = wv;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(0xffffffffu, winc, o);
-            if (lane >= o) winc += t;
-        }
-        const uint32_t pre = __shfl_sync(0xffffffffu, winc - wv, warp), tot = __shfl_sync(0xffffffffu, winc, 31);
-        if (i < n) a[i] = base + pre + inc - v;
-        base += tot;
-        __syncthreads();
-    }
-    return base;
-}
-
-__global__ void __launch_bounds__(1024) merge_group_small_kernel(const MergeParams p) {
-    extern __shared__ __align__(16) uint8_t g_dyn[];
-    __shared__ RadixScratch<32> sc;
-    __shared__ uint32_t s_wt[32];
-    __shared__ int s_min, s_max;
-    __shared__ uint32_t s_bad;
-#ifdef AJT_TIMING
-    uint64_t tick_[10] = {0};
-#endif
-    AJT_TICK(0);
-    const int tid = threadIdx.x, n = p.n;
-    const size_t nn = ((size_t)n + 32) & ~(size_t)31;   // 6 arrays of nn words
-    // arrays read BY TIMELINE INDEX through the sorted order are swizzled: timelines of one group are often a power of two
-    // apart (round-robin collection), which would put a warp's 32 gathers in one bank
-    auto swz = [](int i) { return i ^ ((i >> 5) & 31) ^ ((i >> 10) & 31); };
-    uint32_t* const sm32 = reinterpret_cast<uint32_t*>(g_dyn);
-    uint32_t* kb[2] = {sm32, sm32 + nn};
-    uint32_t* vb[2] = {sm32 + 2 * nn, sm32 + 3 * nn};
-    uint32_t* nsg = sm32 + 4 * nn;   // [i] hash windows of timeline i
-    uint32_t* tln = sm32 + 5 * nn;   // [i] its length; later [pos] windows by sorted position
-    if (tid < (int)(sizeof(AjtCtrl) / 4)) reinterpret_cast<uint32_t*>(p.ctrl)[tid] = 0;   // fresh control block
-    if (tid == 0) { s_min = INT32_MAX; s_max = INT32_MIN; s_bad = 0; }
-    __syncthreads();
-    // validate offsets; min / max traj id; hash windows per timeline
-    int lmin = INT32_MAX, lmax = INT32_MIN;
-    uint32_t bad = 0;
-#pragma unroll 2
-    for (int i = tid; i < n; i += 1024) {
-        const int64_t a = __ldg(p.offsets + i), b = __ldg(p.offsets + i + 1);
-        if (b < a || b - a > (int64_t)INT32_MAX) bad |= AJT_STATUS_BAD_OFFSETS;
-        else if (b == a) bad |= AJT_STATUS_ZERO_LEN;
-        const int t = __ldg(p.traj_ids + i);
-        lmin = min(lmin, t);
-        lmax = max(lmax, t);
-        kb[0][i] = (uint32_t)t;
-        vb[0][i] = (uint32_t)i;
-        nsg[swz(i)] = (uint32_t)(((b - 1 + p.mis) >> kHSegLog) - ((a + p.mis) >> kHSegLog) + 1);
-        tln[swz(i)] = (uint32_t)(b - a);
-        p.link_bad[i] = 0;
-    }
-    if (tid == 0 && (__ldg(p.offsets) != 0 || __ldg(p.offsets + n) != p.N)) bad |= AJT_STATUS_BAD_OFFSETS;
-    AJT_TICK(1);
-    lmin = __reduce_min_sync(0xffffffffu, lmin);
-    lmax = __reduce_max_sync(0xffffffffu, lmax);
-    bad = __reduce_or_sync(0xffffffffu, bad);
-    if ((tid & 31) == 0) {
-        if (bad) atomicOr(&s_bad, bad);
-        atomicMin(&s_min, lmin);
-        atomicMax(&s_max, lmax);
-    }
-    __syncthreads();
-    if (s_bad) {
-        if (tid == 0) atomicOr(&p.ctrl->status, s_bad);
+    if (E > (int64_t)p.E_cap || nslice > (int64_t)p.slice_cap || U > (int64_t)p.slice_cap) {
+        if (tid == 0) group_fail(p, (uint32_t)AJT_STATUS_PROBE_CAPACITY);
         return;
     }
-    const uint32_t tmin = (uint32_t)s_min, range = (uint32_t)s_max - tmin;
-#pragma unroll 1
-    for (int i = tid; i < n; i += 1024) kb[0][i] -= tmin;
-    __syncthreads();
-    AJT_TICK(2);
-    int cur = 0;
-    {   // as few passes as the key range needs, digits of equal width (the ranking costs one ballot per digit bit)
-        const int bits = 32 - __clz(range), npass = (bits + 7) / 8, w = npass ? (bits + npass - 1) / npass : 0;
-#pragma unroll 1
-        for (int shift = 0; shift < bits; shift += w) {
-            radix_pass<32>(kb[cur], vb[cur], kb[cur ^ 1], vb[cur ^ 1], n, shift, sc, w);
-            cur ^= 1;
-        }
-    }
-    AJT_TICK(3);
-    uint32_t* key = kb[cur];          // [pos] sorted keys; later [g] first key slot of group g
-    const uint32_t* val = vb[cur];    // [pos] timeline index
-    uint32_t* gid = kb[cur ^ 1];      // [pos] group id
-    uint32_t* gsv = vb[cur ^ 1];      // [g]   first sorted position of group g
-    // group ids and group starts
-#pragma unroll 1
-    for (int pos = tid; pos < n; pos += 1024) gid[pos] = (pos == 0 || key[pos] != key[pos - 1]) ? 1u : 0u;
-    __syncthreads();
-    const int G = (int)cta_scan_excl(gid, n, s_wt);   // gid[pos] = heads before pos
-#pragma unroll 1
-    for (int pos = tid; pos < n; pos += 1024) {
-        const bool head = pos == 0 || key[pos] != key[pos - 1];
-        const uint32_t g = gid[pos] + (head ? 1u : 0u) - 1u;
-        gid[pos] = g;
-        if (head) { gsv[g] = (uint32_t)pos; p.grp_start[g] = pos; }
-    }
-    if (tid == 0) { gsv[G] = (uint32_t)n; p.grp_start[G] = n; }
-    __syncthreads();
-    AJT_TICK(4);
-    // key slots (i, a), a = 0..rank_i: a group of k timelines has k(k+1)/2 (at most n^2/2 < 2^25 here)
-    uint32_t* gent = key;
-#pragma unroll 1
-    for (int g = tid; g < G; g += 1024) {
-        const uint32_t k = gsv[g + 1] - gsv[g];
-        gent[g] = k * (k + 1) / 2;
-    }
-    __syncthreads();
-    const uint32_t E = cta_scan_excl(gent, G, s_wt);
-    AJT_TICK(5);
-    // lengths by sorted position; then the windows by sorted position (none for singleton groups) in the freed array
-#pragma unroll 1
-    for (int pos = tid; pos < n; pos += 1024) p.glen[pos] = (int32_t)tln[swz((int)val[pos])];
-    __syncthreads();
-    uint32_t* segs = tln;
-#pragma unroll 1
-    for (int pos = tid; pos < n; pos += 1024) {
-        const uint32_t g = gid[pos];
-        segs[pos] = gsv[g + 1] - gsv[g] < 2 ? 0u : nsg[swz((int)val[pos])];
-    }
-    __syncthreads();
-    // hash segments numbered in GROUP order, so that a timeline is hashed right after its in-group predecessor
-    const uint32_t nseg = cta_scan_excl(segs, n, s_wt);
-    AJT_TICK(6);
-#pragma unroll 1
-    for (int pos = tid; pos < n; pos += 1024) {
-        const uint32_t g = gid[pos], gs = gsv[g], r = (uint32_t)pos - gs;
-        p.tl_rec[pos] = make_int4((int)segs[pos], (int)gs, (int)r, (int)(gent[g] + r * (r + 1) / 2u));
-        p.perm[pos] = (int32_t)val[pos];
-        if (r == 0) p.grp_ent[g] = (int32_t)gent[g];
-    }
+    for (int g = tid; g <= G; g += 1024)
+        p.grp_rec[g] = make_int4((int)gsv[g], g < G ? (int)(gsv[g + 1] - gsv[g]) : 0, (int)gent[g], (int)gun[g]);
     if (tid == 0) {
-        p.grp_ent[G] = (int32_t)E;
         p.ctrl->n_groups = G;
         p.ctrl->n_entries = (int32_t)E;
-        p.ctrl->n_hash_segs = (int32_t)nseg;
-        if ((int64_t)E > (int64_t)p.E_cap || (int64_t)nseg > (int64_t)p.nseg_cap)
-            atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_PROBE_CAPACITY);
+        p.ctrl->n_hash_segs = (int32_t)nslice;
+        p.ctrl->n_units = (int32_t)U;
     }
-    AJT_TICK(7);
-#ifdef AJT_TIMING
-    if (tid == 0)
-        for (int k = 0; k < 8; ++k) reinterpret_cast<uint64_t*>(p.ctrl->reserved)[k] = tick_[k];
-#endif
 }
 
-// ---------------------------------------------------------------------------------------- K2: prefix-hash scan (M2)
+// ---------------------------------------------------------------------------------------- K2: prefix-hash scan (M2, M5 first half)
 
-// Prefix hash F_i(p) = sum_{q<p} x_q w(q) mod 2^64 with 32-bit weights w(q) = B^(q+3) mod 2^32: one IMAD.WIDE per token
-// (32 x 32 -> 64 with a 64-bit addend).  A sum over positions, hence a monoid: per-lane partials, combined only where a key is
-// emitted.  Weak by design (a 64-bit sum of 50-bit products); every accepted pair is verified exactly (M5).
+// Prefix hash F_i(p) = sum_{q<p} x_q w(q) mod 2^64 with 32-bit weights w(q) = W^(q+3) mod 2^32: one IMAD.WIDE per token
+// (32 x 32 -> 64 with a 64-bit addend).  A sum over positions, hence a monoid: per-lane partials, combined only where a value
+// leaves the warp.  Weak by design (a 64-bit sum of 50-bit products); every accepted pair is verified exactly (M5).
 __device__ __forceinline__ uint32_t pow32(uint32_t b, uint32_t e) {
     uint32_t r = 1;
     while (e) {
@@ -647,8 +696,6 @@ __device__ __forceinline__ uint32_t pow32(uint32_t b, uint32_t e) {
     }
     return r;
 }
-// Power tables (constant memory, warp-uniform reads): W^(win0 + 3) of a window that starts d = -win0 (mod 2048) slots before
-// a multiple of 2048, j windows into its timeline, is W2048^j * Winv^(64 (d >> 6)) * Winv^(d & 63) * W^3.
 template <int N>
 struct PowTab {
     uint32_t v[N];
@@ -658,204 +705,281 @@ struct PowTab {
         for (int i = 0; i < N; ++i) { v[i] = r; r *= base; }
     }
 };
-__constant__ PowTab<64> c_w2048 = PowTab<64>(cpow32(kW, 2048));
-__constant__ PowTab<32> c_winv64 = PowTab<32>(cpow32(kWinv, 64));
-__constant__ PowTab<64> c_winv1 = PowTab<64>(kWinv);
-__constant__ PowTab<16> c_w128 = PowTab<16>(kW128);
-__constant__ PowTab<32> c_w4 = PowTab<32>(cpow32(kW, 4));
-// weight of the first slot of window j of a timeline whose window grid starts d slots before its first token (0 <= d < 2048)
-__device__ __forceinline__ uint32_t window_weight(int j, int d) {
-    const uint32_t wj = j < 64 ? c_w2048.v[j] : pow32(kW2048, (uint32_t)j);
-    return wj * c_winv64.v[d >> 6] * c_winv1.v[d & 63] * (kW * kW * kW);
+__constant__ PowTab<128> c_w512 = PowTab<128>(kW512);   // W^(512 j): slice j of a timeline (64k tokens before the slow path)
+__constant__ PowTab<32> c_w1 = PowTab<32>(kW);          // W^lane
+
+// Last index i in [0, n) with key(i) <= x, for a non-decreasing key with key(0) <= x: warp-cooperative 32-ary search
+// (2 dependent loads for n <= 1024 instead of 10).
+template <class F>
+__device__ __forceinline__ int warp_search_last_le(int n, int64_t x, F key) {
+    const int lane = threadIdx.x & 31;
+    int lo = 0, hi = n;  // key(lo) <= x; hi == n or key(hi) > x
+    while (hi - lo > 1) {
+        const int step = (hi - lo + 31) >> 5;
+        const int idx = lo + (lane + 1) * step;
+        const bool le = idx < hi && (int64_t)key(idx) <= x;
+        const int cnt = __popc(__ballot_sync(0xffffffffu, le));
+        const int nlo = lo + cnt * step;
+        hi = min(hi, nlo + step);
+        lo = nlo;
+    }
+    return lo;
 }
-__device__ __forceinline__ uint64_t mad_wide(uint32_t a, uint32_t b, uint64_t c) { return (uint64_t)a * b + c; }
+
+__device__ __forceinline__ bool mbar_wait_bounded(uint64_t* bar, uint32_t parity) {
+    for (int spin = 0; spin < (1 << 22); ++spin)
+        if (mbar_try_wait(bar, parity)) return true;
+    return false;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t saddr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr));
+    return v;
+}
+__device__ __forceinline__ void sts32(uint32_t saddr, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory"); }
 
 constexpr int kHashThreads = 256;
+constexpr int kHashStages = 4;
+constexpr int kStageBytes = kSl * 4 + 32;                           // 512 tokens + one 16-byte vector of misalignment (+ pad)
+constexpr int kHashWarpBytes = kHashStages * kStageBytes + 128;     // + 4 mbarriers (32 B, padded to 64) + 4 descriptors
+constexpr int kHashSmem = (kHashThreads / 32) * kHashWarpBytes + 128;
 
-// This lane's four tokens of step s of a window (positions q .. q+3 of the timeline whose tokens start at tl), zero outside
-// the timeline.  16-byte aligned address.  lo / hi: how many elements may be read before tl / from tl (array bounds).
-template <bool kInterior>
-__device__ __forceinline__ int4 load_step(const int32_t* __restrict__ tl, int Li, int q, int64_t lo, int64_t hi) {
-    if (kInterior) return __ldg(reinterpret_cast<const int4*>(tl + q));
-    int4 x = make_int4(0, 0, 0, 0);
-    if (q + 3 >= 0 && q < Li) {
-        if (q >= -lo && q + 3 < hi) x = __ldg(reinterpret_cast<const int4*>(tl + q));
-        else {
-            if (q >= -lo && q < hi) x.x = tl[q];
-            if (q + 1 >= -lo && q + 1 < hi) x.y = tl[q + 1];
-            if (q + 2 >= -lo && q + 2 < hi) x.z = tl[q + 2];
-            if (q + 3 >= -lo && q + 3 < hi) x.w = tl[q + 3];
-        }
-        if (!(q >= 0 && q < Li)) x.x = 0;
-        if (!(q + 1 >= 0 && q + 1 < Li)) x.y = 0;
-        if (!(q + 2 >= 0 && q + 2 < Li)) x.z = 0;
-        if (!(q + 3 >= 0 && q + 3 < Li)) x.w = 0;
-    }
-    return x;
-}
-
-// One batch = 4 steps = 512 positions of a window: four 16-byte loads per lane in flight (plus 16 predecessor tokens when
-// linked).  kInterior: the batch lies inside the timeline.  kLink: 0 no predecessor positions here, 1 some, 2 all of them.
-// snap[s * 32] receives this lane's running sum BEFORE step s (the key-emission pass needs it); w are the lane's weights.
-template <bool kInterior, int kLink>
-__device__ __forceinline__ void hash_batch(const int32_t* __restrict__ tl, int Li, int qb, int64_t lo, int64_t hi,
-                                           const int32_t* __restrict__ tprev, int Lprev, uint32_t (&w)[4], uint64_t& acc,
-                                           uint32_t& diff, uint64_t* snap) {
-    int4 x[4];
-    int32_t y[4][4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const int q = qb + 128 * u;
-        x[u] = load_step<kInterior>(tl, Li, q, lo, hi);
-        if (kLink == 2) {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) y[u][k] = __ldg(tprev + q + k);
-        } else if (kLink == 1) {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) y[u][k] = (q + k >= 0 && q + k < Lprev) ? __ldg(tprev + q + k) : 0;
-        }
-    }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const int q = qb + 128 * u;
-        if (kLink == 2) {
-            diff |= (uint32_t)(y[u][0] ^ x[u].x) | (uint32_t)(y[u][1] ^ x[u].y);
-            diff |= (uint32_t)(y[u][2] ^ x[u].z) | (uint32_t)(y[u][3] ^ x[u].w);
-        } else if (kLink == 1) {
-            if (q >= 0 && q < Lprev) diff |= (uint32_t)(y[u][0] ^ x[u].x);
-            if (q + 1 >= 0 && q + 1 < Lprev) diff |= (uint32_t)(y[u][1] ^ x[u].y);
-            if (q + 2 >= 0 && q + 2 < Lprev) diff |= (uint32_t)(y[u][2] ^ x[u].z);
-            if (q + 3 >= 0 && q + 3 < Lprev) diff |= (uint32_t)(y[u][3] ^ x[u].w);
-        }
-        snap[u * 32] = acc;
-        acc = mad_wide((uint32_t)x[u].x, w[0], acc);
-        acc = mad_wide((uint32_t)x[u].y, w[1], acc);
-        acc = mad_wide((uint32_t)x[u].z, w[2], acc);
-        acc = mad_wide((uint32_t)x[u].w, w[3], acc);
-        w[0] *= kW128; w[1] *= kW128; w[2] *= kW128; w[3] *= kW128;
-    }
-}
-
-// Sum of a 64-bit value over the warp (mod 2^64) with three REDUX instead of ten shuffles: 22 + 22 + 20-bit slices, whose
-// 32-term sums fit 32 bits.
-__device__ __forceinline__ uint64_t warp_sum_u64_redux(uint64_t v) {
-    const uint32_t a = (uint32_t)v & 0x3fffffu, b = (uint32_t)(v >> 22) & 0x3fffffu, c = (uint32_t)(v >> 44);
-    const uint32_t sa = __reduce_add_sync(0xffffffffu, a), sb = __reduce_add_sync(0xffffffffu, b);
-    const uint32_t sc = __reduce_add_sync(0xffffffffu, c);
-    return (uint64_t)sa + ((uint64_t)sb << 22) + ((uint64_t)sc << 44);
-}
-
-// One key: F at prefix length (position r of the window) + 1.  Every lane adds to its running sum BEFORE step s = r >> 7 (its
-// snapshot) the tokens of that step it holds at positions <= r (re-read: L1), and one warp sum gives the value.  ~40
-// instructions per key; a window holds the end of 0-3 requested prefixes.
-__device__ __forceinline__ uint64_t hash_key_value(const int32_t* __restrict__ tl, int Li, int64_t lo, int64_t hi, int win0, int r,
-                                                   uint32_t w0_window, const uint64_t* snap) {
-    const int lane = threadIdx.x & 31;
-    const int s = r >> 7;
-    const int4 x = load_step<false>(tl, Li, win0 + 128 * s + 4 * lane, lo, hi);
-    const int c = (r & 127) - 4 * lane;   // tokens k <= c of this lane lie inside the prefix
-    uint32_t w = w0_window * c_w128.v[s];
-    uint64_t part = snap[s * 32];
-    if (c >= 0) part = mad_wide((uint32_t)x.x, w, part);
-    w *= kW;
-    if (c >= 1) part = mad_wide((uint32_t)x.y, w, part);
-    w *= kW;
-    if (c >= 2) part = mad_wide((uint32_t)x.z, w, part);
-    w *= kW;
-    if (c >= 3) part = mad_wide((uint32_t)x.w, w, part);
-    return warp_sum_u64_redux(part);
-}
-
-__global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const MergeParams p) {
-    __shared__ uint64_t s_snap[kHashThreads / 32][16 * 32];   // per warp: running sums before each step of the window
+// Warp per hash unit = (group, slice of 512 positions).  Lane l holds positions S0 + l + 32 t (t < 16) of EVERY member: a
+// member's slice arrives as ONE bulk async copy (TMA, 1-D) of the 16-byte-aligned superset of its bytes, issued by one lane
+// and counted on a warp-private mbarrier, and is read with conflict-free 32-bit shared-memory loads at the member's own
+// misalignment.  So the weights are per unit, and member r is compared with member r - 1 register against register.
+__global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const MergeParams p) {
+    extern __shared__ __align__(128) uint8_t h_dyn[];
     if (fatal(p)) return;
-    const int lane = threadIdx.x & 31;
-    const int wglobal = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
-    const int nseg = p.ctrl->n_hash_segs, n = p.n;
-    uint64_t* snap = s_snap[threadIdx.x >> 5] + lane;
-    // Striped windows: at any moment the grid works on ~nwarps consecutive windows (a front of ~30 MB that sweeps the token
-    // array once), so a timeline's in-group predecessor, hashed a little earlier, is still in L2 when it is compared.
-    const uint32_t LW = c_w4.v[lane];
-    auto seg_base = [&](int i) { return __ldg(reinterpret_cast<const int32_t*>(p.tl_rec) + 4 * i); };
-    for (int sidx = wglobal; sidx < nseg; sidx += nwarps) {
-        const int pos = warp_search_last_le(n, sidx, seg_base);   // sorted position of the window's timeline
-        const int4 rec = __ldg(p.tl_rec + pos);
-        const int i = __ldg(p.perm + pos);
-        const int64_t off = __ldg(p.offsets + i);
-        const int Li = (int)(__ldg(p.offsets + i + 1) - off);
-        const int32_t* tl = p.tokens + off;
-        const int64_t lo = off, hi = p.N - off;   // elements of the token array before / from tl
-        // the in-group predecessor, if this timeline can extend it (the usual case: each call resends the context)
-        int Lprev = 0;
-        const int32_t* tprev = nullptr;
-        if (rec.z > 0) {
-            const int lp = __ldg(p.glen + pos - 1);
-            if (lp <= Li) { Lprev = lp; tprev = p.tokens + __ldg(p.offsets + __ldg(p.perm + pos - 1)); }
-        }
-        const int d = (int)((off + p.mis) & (kHSeg - 1));   // the timeline starts d slots into its first window
-        const int j = sidx - rec.x;                          // window index inside the timeline
-        const int win0 = j * kHSeg - d;                      // timeline position of the window's first slot
-        // pull the whole window (<= 8 KB = 64 lines) towards L2 now: the four batches below then wait on L2, not on DRAM
-        for (int e = max(win0, 0) + 32 * lane; e < min(win0 + kHSeg, Li); e += 1024)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(tl + e));
-        const uint32_t w0 = window_weight(j, d) * LW;        // weight W^(q+3) of this lane's first slot q = win0 + 4 lane
-        const int rank = rec.z, ebase = rec.w;
-        const int32_t* gln = p.glen + rec.y;
-        // ---- streaming pass: four batches of 512 positions
-        uint32_t w[4] = {w0, w0 * kW, w0 * kW * kW, w0 * kW * kW * kW};
-        uint32_t diff = 0;
-        uint64_t acc = 0;
-        const int q0 = win0 + lane * 4;
-#pragma unroll 1
-        for (int h = 0; h < 4; ++h) {
-            const int b0 = win0 + 512 * h, b1 = b0 + 512;
-            uint64_t* sn = snap + h * 4 * 32;
-            if (b0 >= Li) {   // nothing of the timeline here
+    const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
+    uint8_t* const wbuf = reinterpret_cast<uint8_t*>(((uintptr_t)h_dyn + 127) & ~(uintptr_t)127) + (size_t)wic * kHashWarpBytes;
+    uint64_t* const full = reinterpret_cast<uint64_t*>(wbuf + kHashStages * kStageBytes);
+    int4* const desc = reinterpret_cast<int4*>(wbuf + kHashStages * kStageBytes + 64);
+    const uint32_t sbuf = smem_u32(wbuf);
+    if (lane == 0) {
 #pragma unroll
-                for (int u = 0; u < 4; ++u) sn[u * 32] = acc;
-                continue;
-            }
-            const bool interior = b0 >= 0 && b1 <= Li;
-            const int qb = q0 + 512 * h;
-#define AJT_HB(I, K) hash_batch<I, K>(tl, Li, qb, lo, hi, tprev, Lprev, w, acc, diff, sn)
-            if (interior && b1 <= Lprev) AJT_HB(true, 2);
-            else if (interior && b0 < Lprev) AJT_HB(true, 1);
-            else if (interior) AJT_HB(true, 0);
-            else if (b0 < Lprev) AJT_HB(false, 1);
-            else AJT_HB(false, 0);
-#undef AJT_HB
+        for (int s = 0; s < kHashStages; ++s) mbar_init(&full[s], 1);
+        fence_mbar_init();
+    }
+    __syncwarp();
+    uint32_t phases = 0;   // bit s: the parity stage s completes next
+    const int U = p.ctrl->n_units, G = p.ctrl->n_groups;
+    const int32_t* __restrict__ tokens = p.tokens;
+    const int64_t N = p.N;
+    const int mis = p.mis;
+    const uint32_t lw = c_w1.v[lane] * kW3;   // W^(lane + 3)
+    int next = 0;
+    if (lane == 0) next = atomicAdd(&p.ctrl->unit_ticket, 1);
+    next = __shfl_sync(0xffffffffu, next, 0);
+    while (next < U) {
+        const int u = next;
+        if (lane == 0) next = atomicAdd(&p.ctrl->unit_ticket, 1);   // needed only after this unit: the round trip is hidden
+        const int g = warp_search_last_le(G, u, [&](int x) { return __ldg(reinterpret_cast<const int32_t*>(p.grp_rec + x) + 3); });
+        const int4 gr = __ldg(p.grp_rec + g);
+        const int gs = gr.x, k = gr.y, w = u - gr.w;
+        const int64_t eb = gr.z;
+        const int S0 = w << kSlLog;                 // first position of the slice
+        const int32_t* __restrict__ gln = p.glen + gs;
+        const int64_t* __restrict__ gof = p.goff + gs;
+        // lane weights of positions S0 + lane + 32 t: the same for every member
+        uint32_t wt[16];
+        wt[0] = (w < 128 ? c_w512.v[w] : pow32(kW512, (uint32_t)w)) * lw;
+#pragma unroll
+        for (int t = 1; t < 16; ++t) wt[t] = wt[t - 1] * kW32;
+        // members of the first 32 ranks whose last token lies in this slice (keys are emitted only where a prefix ends)
+        const int L0 = lane < k ? __ldg(gln + lane) : 0;
+        bool anyend = __any_sync(0xffffffffu, L0 > 0 && ((L0 - 1) >> kSlLog) == w);
+        for (int a0 = 32; a0 < k && !anyend; a0 += 32) {
+            const int La = a0 + lane < k ? __ldg(gln + a0 + lane) : 0;
+            anyend = __any_sync(0xffffffffu, La > 0 && ((La - 1) >> kSlLog) == w);
         }
-        const uint64_t tot = warp_sum_u64(acc);
-        if (lane == 0) p.seg_part[sidx] = tot;
-        if (win0 < Lprev && __any_sync(0xffffffffu, diff != 0) && lane == 0) p.link_bad[i] = 1;
-        // ---- key emission: the requested prefixes (L_a of an earlier member, or L_i) that end inside this window
-        __syncwarp();
-        for (int a0 = 0; a0 <= rank; a0 += 32) {
-            const int a = a0 + lane;
-            int rel = -1;
-            if (a <= rank) {
-                const int Lp = __ldg(gln + a);
-                const int r = Lp - 1 - win0;
-                if (Lp <= Li && r >= 0 && r < kHSeg) rel = r;
+        // ---- issue side: walks the members that reach this slice, 32 ranks at a time
+        int ic0 = 0, iL = L0, isb = lane < k ? __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + lane)) : 0;
+        int64_t ioff = lane < k ? __ldg(gof + lane) : 0;
+        unsigned ireach = __ballot_sync(0xffffffffu, iL > S0);
+        bool more = true;
+        auto issue_next = [&](int stage) {
+            if (!more) return false;
+            while (ireach == 0) {
+                ic0 += 32;
+                if (ic0 >= k) { more = false; return false; }
+                const bool v = ic0 + lane < k;
+                iL = v ? __ldg(gln + ic0 + lane) : 0;
+                ioff = v ? __ldg(gof + ic0 + lane) : 0;
+                isb = v ? __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + ic0 + lane)) : 0;
+                ireach = __ballot_sync(0xffffffffu, iL > S0);
             }
-            for (uint32_t m = __ballot_sync(0xffffffffu, rel >= 0); m; m &= m - 1) {
-                const int b = __ffs(m) - 1;
-                const uint64_t F = hash_key_value(tl, Li, lo, hi, win0, __shfl_sync(0xffffffffu, rel, b), w0, snap);
-                if (lane == b) p.ent_hash[ebase + a] = F;
+            const int b = __ffs(ireach) - 1;
+            ireach &= ireach - 1;
+            const int Lr = __shfl_sync(0xffffffffu, iL, b);
+            const int64_t off = shfl_i64(ioff, b);
+            const int D = (int)((off + mis) & 3);            // slot of position S0 in the 16-byte grid
+            const int64_t g0 = off + S0 - D;                 // element index of the first aligned vector
+            const int nv = (min(Lr - S0, kSl) + D + 3) >> 2; // vectors holding positions < min(L_r, S0 + 512)
+            const uint32_t sdst = sbuf + stage * kStageBytes;
+            const bool inside = g0 >= 0 && g0 + 4 * (int64_t)nv <= N;
+            if (!inside) {   // first / last vectors of the token array: element-wise, inside the array only
+                for (int e = lane; e < 4 * nv; e += 32) {
+                    const int64_t gi = g0 + e;
+                    sts32(sdst + 4 * e, gi >= 0 && gi < N ? (uint32_t)tokens[gi] : 0u);
+                }
+                __syncwarp();
+            }
+            if (lane == b) {   // the member's own lane launches its copy; the descriptor is published by the barrier
+                desc[stage] = make_int4(ic0 + b, iL, isb, D);
+                if (inside) {
+                    mbar_arrive_expect_tx(&full[stage], 16u * (uint32_t)nv);
+                    bulk_load(wbuf + stage * kStageBytes, tokens + g0, 16u * (uint32_t)nv, &full[stage]);
+                } else {
+                    mbar_arrive(&full[stage]);
+                }
+            }
+            return true;
+        };
+        // ---- consume side: two register images of a slice alternate (the member and its predecessor)
+        int prev_r = -2, prev_L = 0;
+        int issued = 0, consumed = 0;
+        bool dead = false;
+        uint64_t Fk = 0;        // lane a: the partial of the prefix ending at member a's last token, for the latest member
+        unsigned fvalid = 0;    // ranks whose Fk belongs to the latest member
+        auto consume = [&](uint32_t (&x)[16], const uint32_t (&pv)[16]) {
+            const int st = consumed & (kHashStages - 1);
+            if (!mbar_wait_bounded(&full[st], (phases >> st) & 1u)) dead = true;   // never in practice: a lost copy must not hang the GPU
+            phases ^= 1u << st;
+            const int4 d = desc[st];
+            const int r = d.x, Lr = d.y;
+            const uint32_t a0 = sbuf + st * kStageBytes + 4 * (d.w + lane);
+#pragma unroll
+            for (int t = 0; t < 16; ++t) x[t] = lds32(a0 + 128 * t);
+            if (Lr < S0 + kSl) {   // the member ends in this slice: nothing beyond its last token
+                const int rem = Lr - S0 - lane;
+#pragma unroll
+                for (int t = 0; t < 16; ++t)
+                    if (32 * t >= rem) x[t] = 0;
+            }
+            uint64_t ac[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                ac[j] = (uint64_t)x[j] * wt[j];
+#pragma unroll
+                for (int t = j + 4; t < 16; t += 4) ac[j] = mad_wide(x[t], wt[t], ac[j]);
+            }
+            // exact comparison with the in-group predecessor on its positions (M5, first half)
+            bool same = false;   // the two agree on every position of the slice below prev_L
+            if (prev_r == r - 1) {
+                uint32_t diff = 0;
+                if (prev_L >= S0 + kSl) {
+#pragma unroll
+                    for (int t = 0; t < 16; ++t) diff |= x[t] ^ pv[t];
+                } else {
+                    const int rem = prev_L - S0 - lane;
+#pragma unroll
+                    for (int t = 0; t < 16; ++t)
+                        if (32 * t < rem) diff |= x[t] ^ pv[t];
+                }
+                same = !__any_sync(0xffffffffu, diff != 0);
+                if (!same && lane == 0) p.lbad[gs + r] = 1;
+            }
+            const uint64_t tot = warp_sum_u64_redux((ac[0] + ac[1]) + (ac[2] + ac[3]));
+            if (lane == 0) p.seg_part[d.z + w] = tot;
+            // keys: the prefixes (L_a of an earlier member, or L_r itself) that end inside this slice
+            if (anyend) {
+                if (!same) fvalid = 0;
+                for (int a0r = 0; a0r <= r; a0r += 32) {
+                    const int a = a0r + lane;
+                    const int La = a0r == 0 ? L0 : (a < k ? __ldg(gln + a) : 0);
+                    const bool hit = a <= r && La > 0 && La <= Lr && ((La - 1) >> kSlLog) == w;
+                    for (unsigned m = __ballot_sync(0xffffffffu, hit); m; m &= m - 1) {
+                        const int b = __ffs(m) - 1;
+                        const int Lb = __shfl_sync(0xffffffffu, La, b);
+                        uint64_t F;
+                        if (a0r == 0 && ((fvalid >> b) & 1u) && Lb <= prev_L) {
+                            F = (uint64_t)shfl_i64((int64_t)Fk, b);   // member r - 1 has the same tokens up to there
+                        } else {
+                            if (a0r + b == r) {
+                                F = tot;   // its own last token: everything beyond is zero already
+                            } else {
+                                const int rem = Lb - S0 - lane;   // tokens 32 t < rem are inside the prefix
+                                uint64_t part = 0;
+#pragma unroll
+                                for (int t = 0; t < 16; ++t)
+                                    if (32 * t < rem) part = mad_wide(x[t], wt[t], part);
+                                F = warp_sum_u64_redux(part);
+                            }
+                            if (a0r == 0) {
+                                if (lane == b) Fk = F;
+                                fvalid |= 1u << b;
+                            }
+                        }
+                        if (lane == 0) p.ent_hash[eb + (int64_t)r * (r + 1) / 2 + a0r + b] = F;
+                    }
+                }
+            }
+            prev_r = r;
+            prev_L = Lr;
+            ++consumed;
+            __syncwarp();   // every lane is done with the stage before the next issue refills it
+        };
+        uint32_t xa[16], xb[16];
+#pragma unroll 1
+        for (int s = 0; s < kHashStages - 1; ++s)
+            if (issue_next(issued & (kHashStages - 1))) ++issued;
+#pragma unroll 1
+        while (consumed < issued) {
+            if (issue_next(issued & (kHashStages - 1))) ++issued;
+            consume(xa, xb);
+            if (consumed < issued) {
+                if (issue_next(issued & (kHashStages - 1))) ++issued;
+                consume(xb, xa);
             }
         }
-        __syncwarp();
+        next = __shfl_sync(0xffffffffu, next, 0);
+        if (__any_sync(0xffffffffu, dead)) {
+            if (lane == 0) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_INTERNAL);
+            break;
+        }
     }
 }
 
-// ---------------------------------------------------------------------------------------- K3 + K4: keys, sort, select (M2-M4)
+// ---------------------------------------------------------------------------------------- K3: keys, sort, select, verify, segments, compact (M2-M6)
 
-__device__ bool tokens_extend(const MergeParams& p, int i, int j) {  // exact: tokens_i[0:L_j] == tokens_j, L_i >= L_j
-    const int64_t oi = p.offsets[i], oj = p.offsets[j];
-    const int64_t Li = p.offsets[i + 1] - oi, Lj = p.offsets[j + 1] - oj;
-    if (Li < Lj) return false;
-    for (int64_t q = 0; q < Lj; ++q)
-        if (p.tokens[oi + q] != p.tokens[oj + q]) return false;
+// Exact: tokens[oa .. oa + L) == tokens[ob .. ob + L), by one warp.  128-bit loads when the two ranges are co-aligned
+// (after a scalar head), coalesced 32-bit loads otherwise; leaves at the first block that differs.
+__device__ __noinline__ bool warp_tokens_equal(const int32_t* __restrict__ tokens, int64_t oa, int64_t ob, int L, int mis) {
+    const int lane = threadIdx.x & 31;
+    const int32_t* __restrict__ A = tokens + oa;
+    const int32_t* __restrict__ B = tokens + ob;
+    int q = 0;
+    if (((oa ^ ob) & 3) == 0) {
+        const int head = min(L, (int)((4 - ((oa + mis) & 3)) & 3));
+        bool bad = lane < head && A[lane] != B[lane];
+        if (__any_sync(0xffffffffu, bad)) return false;
+        const int nvec = (L - head) >> 2;
+        const int4* __restrict__ A4 = reinterpret_cast<const int4*>(A + head);
+        const int4* __restrict__ B4 = reinterpret_cast<const int4*>(B + head);
+        for (int v0 = 0; v0 < nvec; v0 += 128) {
+            uint32_t diff = 0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int v = v0 + lane + 32 * j;
+                if (v < nvec) {
+                    const int4 x = __ldg(A4 + v), y = __ldg(B4 + v);
+                    diff |= (uint32_t)(x.x ^ y.x) | (uint32_t)(x.y ^ y.y) | (uint32_t)(x.z ^ y.z) | (uint32_t)(x.w ^ y.w);
+                }
+            }
+            if (__any_sync(0xffffffffu, diff != 0)) return false;
+        }
+        q = head + 4 * nvec;   // at most 3 tokens left
+    }
+    for (; q < L; q += 256) {
+        uint32_t diff = 0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int e = q + lane + 32 * j;
+            if (e < L) diff |= (uint32_t)(__ldg(A + e) ^ __ldg(B + e));
+        }
+        if (__any_sync(0xffffffffu, diff != 0)) return false;
+    }
     return true;
 }
 
@@ -873,78 +997,234 @@ struct SelectSmem {
     uint32_t sorted[kSelSmemKeys];           // MSD path: key slots grouped by bucket
     uint32_t dig[kSelSmemKeys];              // MSD path: digest of each key slot (0xFFFFFFFF: invalid)
     uint32_t wtot[kSelThreads / 32];
-    int64_t t_off[kSelCacheK];               // per group member (by rank): token offset, first hash segment
-    int32_t t_sb[kSelCacheK];
-    uint8_t bad[kSelCacheK];                 // predecessor link of member r is broken (not an exact extension)
+    int64_t s_w[2][2][kSelThreads / 32];     // block scans
+    int32_t st[8][kSelCacheK];               // per-member decision state (groups up to kSelCacheK)
+    int2 q[kSelCacheK];                      // verification queue {member, candidate}
+    int32_t qn;
+    int32_t coll;
+};
+// Staged copy of one group (dynamic shared memory): a CTA pays ~1 us per dependent global round trip, so a group of up to
+// kSelCacheK members, kSelSmemKeys keys and kSelSlices hash slices is fetched in three batched round trips and decided from
+// shared memory; larger groups work through the workspace.
+constexpr int kSelSlices = 2048;
+struct SelectStage {
+    uint64_t eh[kSelSmemKeys];               // key slots: in-slice partial, then the final prefix hash
+    uint64_t sp[kSelSlices];                 // slice totals of the group's members, then exclusive prefixes per member
+    int64_t off[kSelCacheK];                 // by rank: token offset
+    int32_t L[kSelCacheK], sb[kSelCacheK], idx[kSelCacheK], rs[kSelCacheK];   // length, first slice, timeline, response start
+    int32_t mj[kSelCacheK], mL[kSelCacheK], mR[kSelCacheK];                   // by member slot: timeline, length, response start
+    uint8_t bad[kSelCacheK];                 // the exact comparison with the predecessor found a difference
 };
 
-// mode 0: trust hash-equal candidates (verified later by the scatter pass); mode 1: repair — accepts a candidate only
-// after comparing tokens exactly.  NT threads per CTA; CTAs stride over the groups.
-template <int NT>
-__device__ void select_body(const MergeParams& p, int mode, SelectSmem& sm) {
-    static_assert(NT == kSelThreads, "select_body is written for kSelThreads");
+// The segments of one surviving timeline, by one warp: maximal runs [p0, p1) of positions whose mask / log-prob come from one
+// member (the largest member index j with rs_j <= p < L_j, Algorithm 1 lines 10-17; kSrcNone if there is none).  The run
+// boundaries are response starts and ends of members, at most 2c of them.  mj / mL / mR: timeline, length and response
+// start (clamped to [0, L]) of the c members, ascending, the survivor last.  With explicit masks the source is decided
+// per token by the scatter pass: one segment.  Returns the number of segments written to out[].
+__device__ __noinline__ int build_segments(bool explicit_masks, const int32_t* mj, const int32_t* mL, const int32_t* mR, int c,
+                                           int2* out) {
+    const int lane = threadIdx.x & 31;
+    if (explicit_masks) {
+        if (lane == 0) out[0] = make_int2(0, kSrcExplicit);
+        return 1;
+    }
+    const int Ls = mL[c - 1];
+    int cnt = 0, last = INT32_MIN, pos = 0;
+    // members of the first 32 stay in registers; longer lists are re-read per step
+    int j0 = -1, L0 = 0, r0 = 0;
+    if (lane < c) { j0 = mj[lane]; L0 = mL[lane]; r0 = mR[lane]; }
+    while (pos < Ls) {
+        int src = kSrcNone, nxt = Ls;
+        if (j0 >= 0) {
+            if (r0 <= pos && pos < L0) src = j0;
+            if (r0 > pos) nxt = min(nxt, r0);
+            if (L0 > pos) nxt = min(nxt, L0);
+        }
+        for (int m0 = 32; m0 < c; m0 += 32) {
+            if (m0 + lane < c) {
+                const int j = mj[m0 + lane], Lj = mL[m0 + lane], rj = mR[m0 + lane];
+                if (rj <= pos && pos < Lj) src = max(src, j);
+                if (rj > pos) nxt = min(nxt, rj);
+                if (Lj > pos) nxt = min(nxt, Lj);
+            }
+        }
+        src = __reduce_max_sync(0xffffffffu, src);
+        nxt = __reduce_min_sync(0xffffffffu, nxt);
+        if (src != last) {
+            if (lane == 0) out[cnt] = make_int2(pos, src);
+            ++cnt;
+            last = src;
+        }
+        pos = nxt;
+    }
+    return cnt;
+}
+
+// M6.  One CTA, one fused scan over the timelines (original order): survivors -> merged index, offsets, origin, traj, first
+// global segment; then owner[].  A lone CTA pays ~0.8 us per dependent global round trip, so every load of the scan is
+// issued up front (8 timelines per thread, nothing conditional) and the owner gather runs 8 deep: three round trips in all.
+__global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p) {
+    __shared__ int64_t s_w[2][2][32];
+    if (fatal(p)) return;
+    constexpr int NT = 1024;
+    const int tid = threadIdx.x, n = p.n;
+    int32_t tr[8];
+    const I2 tot = block_scan2<NT, 8>(
+        n,
+        [&](int i) {   // (a survivor's record is garbage for an absorbed timeline: unused)
+            const bool ab = __ldg(p.absorbed + i) != 0;
+            const int64_t L = __ldg(p.offsets + i + 1) - __ldg(p.offsets + i);
+            const int64_t ns = __ldg(reinterpret_cast<const int32_t*>(p.sv_rec + i) + 3);
+            tr[i & 7] = __ldg(p.traj_ids + i);
+            return ab ? I2{0, 0} : I2{((int64_t)1 << 32) | (ns & 0xffffffff), L};
+        },
+        [&](int i, int64_t exa, int64_t exb, int64_t va, int64_t) {
+            if (!va) { p.midx[i] = -1; return; }
+            const int m = (int)(exa >> 32);
+            p.midx[i] = m;
+            p.merged_origin[m] = i;
+            p.merged_traj[m] = tr[i & 7];
+            p.merged_offsets[m] = exb;
+            p.gseg_base[m] = (int32_t)(exa & 0xffffffff);
+        },
+        s_w);
+    const int M = (int)(tot.a >> 32);
+    const int32_t nseg = (int32_t)(tot.a & 0xffffffff);
+#pragma unroll 1
+    for (int i0 = tid; i0 < n; i0 += 8 * NT) {
+        int32_t o[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) o[u] = i0 + u * NT < n ? __ldg(p.owner_tl + i0 + u * NT) : 0;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) o[u] = p.midx[o[u]];
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (i0 + u * NT < n) p.owner[i0 + u * NT] = o[u];
+    }
+    if (tid == 0) {
+        p.merged_offsets[M] = tot.b;
+        p.gseg_base[M] = nseg;
+        p.counts[0] = M;
+        p.counts[1] = tot.b;
+        p.ctrl->M = M;
+        p.ctrl->N_out = tot.b;
+        p.ctrl->n_gsegs = nseg;
+        p.ctrl->n_tiles = (int32_t)((tot.b + kTS - 1) >> kTSLog);
+    }
+}
+
+__global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const MergeParams p) {
+    __shared__ SelectSmem sm;
+    extern __shared__ __align__(16) uint8_t sel_dyn[];
+    SelectStage& sg = *reinterpret_cast<SelectStage*>(sel_dyn);
+    constexpr int NT = kSelThreads;
+    if (fatal(p)) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = p.ctrl->n_groups;
     const bool weak = (p.flags & AJT_MERGE_WEAK_HASH) != 0;
+    const bool longest = p.owner_rule == AJT_OWNER_LONGEST;
+    const bool explicit_masks = p.mask_in != nullptr;
+    if (tid == 0) sm.coll = 0;
+#ifdef AJT_PROF
+    if (tid == 0 && reinterpret_cast<unsigned long long*>(p.ctrl->reserved)[8] == 0) reinterpret_cast<unsigned long long*>(p.ctrl->reserved)[8] = gtimer();
+#endif
     for (int g = blockIdx.x; g < G; g += gridDim.x) {
-        const int gs = p.grp_start[g], k = p.grp_start[g + 1] - gs;
-        const int32_t* gl = p.perm + gs;
-        const int32_t* gln = p.glen + gs;
-        if (k < 2) {
-            if (tid == 0) { p.absorbed[gl[0]] = 0; p.owner_tl[gl[0]] = gl[0]; p.needv[gl[0]] = 0; p.tl_pos[gl[0]] = gs; }
+        const int4 gr = __ldg(p.grp_rec + g);
+        const int gs = gr.x, k = gr.y, eb = gr.z;
+        const int c = (int)min((int64_t)k * (k + 1) / 2, (int64_t)INT32_MAX);   // key slots (fits: checked against E_cap)
+        int2* const rs_out = p.rseg + 2 * (int64_t)gs;
+        int32_t* const mem = p.mem_list + gs;
+        if (k < 2) {   // a group of one: it survives and is its own only member
+            if (warp == 0) {
+                const int i = __ldg(p.perm + gs), L = __ldg(p.glen + gs);
+                const int rs = explicit_masks ? 0 : min(max(__ldg(p.resp_start + i), 0), L);
+                if (lane == 0) {
+                    p.absorbed[i] = 0; p.owner_tl[i] = i; mem[0] = i;
+                    p.sel[3][gs] = L; p.sel[4][gs] = rs;
+                }
+                __syncwarp();
+                const int sc = build_segments(explicit_masks, mem, p.sel[3] + gs, p.sel[4] + gs, 1, rs_out);
+                if (lane == 0) p.sv_rec[i] = make_int4(gs, 1, 2 * gs, sc);
+            }
             continue;
         }
-        const int eb = p.grp_ent[g], c = p.grp_ent[g + 1] - eb;
         const bool cached = k <= kSelCacheK, small = c <= kSelSmemKeys;
-        // ---- M2 (end): per timeline, exclusive prefix over its hash windows (in place), one warp per timeline
-        // (mode 1 finds seg_part and ent_hash already final)
-        for (int r = warp; r < k; r += NT / 32) {
-            const int i = gl[r];
-            const int sb = p.tl_rec[gs + r].x;
-            const int64_t off = p.offsets[i];
-            const int ns = mode == 0 ? (int)(((off + gln[r] - 1 + p.mis) >> kHSegLog) - ((off + p.mis) >> kHSegLog) + 1) : 0;
-            if (cached && lane == 0) {
-                sm.t_off[r] = off;
-                sm.t_sb[r] = sb;
-                sm.bad[r] = r > 0 && (p.link_bad[i] != 0 || gln[r - 1] > gln[r]);
+        // ---- stage-in, round trip 2 (the group record was 1): per-member facts and the key partials, all independent loads
+        bool fast = cached && small;
+        if (fast) {
+            if (tid < k) {
+                const int i = __ldg(p.perm + gs + tid);
+                sg.idx[tid] = i;
+                sg.L[tid] = __ldg(p.glen + gs + tid);
+                sg.off[tid] = __ldg(p.goff + gs + tid);
+                sg.sb[tid] = __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + tid));
+                sg.bad[tid] = p.lbad[gs + tid];
             }
+            for (int x = tid; x < c; x += NT) sg.eh[x] = p.ent_hash[eb + x];
+            __syncthreads();
+            const int sb0 = sg.sb[0], nsl = sg.sb[k - 1] + ((sg.L[k - 1] + kSl - 1) >> kSlLog) - sb0;
+            fast = nsl <= kSelSlices;
+            if (fast) {   // round trip 3: the slice totals (contiguous: slices are numbered in group order), response starts
+                for (int x = tid; x < nsl; x += NT) sg.sp[x] = p.seg_part[sb0 + x];
+                if (tid < k) sg.rs[tid] = explicit_masks ? 0 : min(max(__ldg(p.resp_start + sg.idx[tid]), 0), sg.L[tid]);
+            }
+            __syncthreads();
+        }
+        const int32_t* const gl = fast ? sg.idx : p.perm + gs;
+        const int32_t* const gln = fast ? sg.L : p.glen + gs;
+        const int64_t* const gof = fast ? sg.off : p.goff + gs;
+        uint64_t* const eh = fast ? sg.eh : p.ent_hash + eb;
+        uint64_t* const sp = fast ? sg.sp - sg.sb[0] : p.seg_part;   // sp[first slice of member r + s]
+        auto sb_of = [&](int r) { return fast ? sg.sb[r] : p.tl_rec[gs + r].x; };
+        // per-member decision state, by rank
+        int32_t* const own = cached ? sm.st[0] : p.sel[0] + gs;    // -2 undecided, -1 survivor, else rank of the owner
+        int32_t* const lim = cached ? sm.st[1] : p.sel[1] + gs;    // PAPER: candidates below this rank only
+        int32_t* const badc = cached ? sm.st[2] : p.sel[2] + gs;   // broken links among ranks <= r
+        int32_t* const exL = cached ? sm.st[3] : p.sel[3] + gs;    // LONGEST: the last candidate that failed (length, rank)
+        int32_t* const exR = cached ? sm.st[4] : p.sel[4] + gs;
+        int32_t* const fin = cached ? sm.st[5] : p.sel[5] + gs;    // LONGEST: the owner, -2 while undecided
+        int32_t* const mcnt = cached ? sm.st[6] : p.sel[6] + gs;   // members per survivor
+        int32_t* const mbase = cached ? sm.st[7] : p.sel[7] + gs;  // its first member slot
+        int2* const vq = cached ? sm.q : p.sel_q + gs;
+        // ---- M2 (end): per member, exclusive prefix over its slice totals (in place), one warp per member
+        for (int r = warp; r < k; r += NT / 32) {
+            const int sb = sb_of(r);
+            const int ns = (gln[r] + kSl - 1) >> kSlLog;
             uint64_t carry = 0;
             for (int s0 = 0; s0 < ns; s0 += 32) {
                 const int s = s0 + lane;
-                const uint64_t v = s < ns ? p.seg_part[sb + s] : 0;
+                const uint64_t v = s < ns ? sp[sb + s] : 0;
                 uint64_t inc = v;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     const uint64_t t = __shfl_up_sync(0xffffffffu, inc, o);
                     if (lane >= o) inc += t;
                 }
-                if (s < ns) p.seg_part[sb + s] = carry + inc - v;
+                if (s < ns) sp[sb + s] = carry + inc - v;
                 carry += __shfl_sync(0xffffffffu, inc, 31);
             }
         }
+        // broken links up to each rank: link r is broken when the exact comparison of the hash pass found a difference, or
+        // when the predecessor is longer (it cannot be a prefix then)
+        block_scan<NT, 1>(
+            k, [&](int r) { return r > 0 && ((fast ? sg.bad[r] : p.lbad[gs + r]) != 0 || gln[r - 1] > gln[r]) ? 1 : 0; },
+            [&](int r, int64_t ex, int64_t v) { badc[r] = (int32_t)(ex + v); own[r] = -2; lim[r] = k; mcnt[r] = 0; }, sm.s_w);
         if (small)
             for (int b = tid; b <= kSelBuckets; b += NT) sm.start[b] = 0;
+        if (tid == 0) sm.qn = 0;
         __syncthreads();
-        // ---- final keys: hash of T_i[0:L_a] = prefix of the windows before the one holding position L_a - 1 + its partial
+        // ---- final keys: hash of T_r[0:L_a] = prefix of the slices before the one holding position L_a - 1 + its partial
         uint32_t* gdig = p.ent_dig + eb;
         uint32_t* gidx = p.ent_idx + eb;
         for (int x = tid; x < c; x += NT) {
             const int r = rank_of_local((uint32_t)x), a = x - r * (r + 1) / 2;
-            const int64_t Lp = gln[a];
+            const int32_t Lp = gln[a];
             uint32_t dg = 0xFFFFFFFFu;
             if (Lp <= gln[r]) {
-                uint64_t h = p.ent_hash[eb + x];
-                if (mode == 0) {
-                    int64_t off;
-                    int sb;
-                    if (cached) { off = sm.t_off[r]; sb = sm.t_sb[r]; }
-                    else { const int i = gl[r]; off = p.offsets[i]; sb = p.tl_rec[gs + r].x; }
-                    const int64_t widx = ((off + Lp - 1 + p.mis) >> kHSegLog) - ((off + p.mis) >> kHSegLog);
-                    h += p.seg_part[sb + widx];
-                    if (weak) h &= 0xFull;
-                    p.ent_hash[eb + x] = h;
-                }
-                dg = digest32(h, (int32_t)Lp);
+                uint64_t h = eh[x] + sp[sb_of(r) + ((Lp - 1) >> kSlLog)];
+                if (weak) h &= 0xFull;
+                eh[x] = h;
+                dg = digest32(h, Lp);
                 if (dg == 0xFFFFFFFFu) dg = 0xFFFFFFFEu;
             }
             if (small) {
@@ -1015,493 +1295,475 @@ __device__ void select_body(const MergeParams& p, int mode, SelectSmem& sm) {
                 for (int x = lo; x < c && sk[x] == dg; ++x) fn(sv[x]);
             }
         };
-        // ---- M4: survivors and the Algorithm-1 owner (latest extender)
-        for (int b = tid; b < k; b += NT) {
-            const int j = gl[b];
-            const int ef = eb + b * (b + 1) / 2 + b;        // full key of j
-            const uint64_t H = p.ent_hash[ef];
-            const int32_t L = gln[b];
-            uint32_t dg = digest32(H, L);
-            if (dg == 0xFFFFFFFFu) dg = 0xFFFFFFFEu;
-            int best = -1;                                   // max rank of an extender
-            visit(dg, [&](uint32_t le) {
-                const int rb = rank_of_local(le);
-                if (rb <= b || rb <= best) return;
-                const int a = (int)le - rb * (rb + 1) / 2;
-                if (gln[a] != L || p.ent_hash[eb + le] != H) return;
-                if (mode == 1 && !tokens_extend(p, gl[rb], j)) return;
-                best = rb;
-            });
-            p.absorbed[j] = best >= 0;
-            p.owner_tl[j] = best >= 0 ? gl[best] : j;
-            p.tl_pos[j] = gs + b;
-        }
-        __syncthreads();
-        if (p.owner_rule == AJT_OWNER_LONGEST) {
-            // the longest SURVIVING extender, then the lowest index (BASELINE.json north_star; DESIGN.md reading M-3)
+        // Verification rounds.  pick(b) proposes a candidate for every undecided member (or decides it); proposals that no
+        // chain of verified links implies are compared exactly, one warp per pair; a failure excludes the candidate.
+        auto run_queue = [&](auto accept, auto reject) {
+            __syncthreads();
+            const int nq = sm.qn;
+            for (int qi = warp; qi < nq; qi += NT / 32) {
+                const int2 e = vq[qi];
+                const bool ok = warp_tokens_equal(p.tokens, gof[e.y], gof[e.x], gln[e.x], p.mis);
+                if (lane == 0) {
+                    if (ok) accept(e.x, e.y);
+                    else { reject(e.x, e.y); sm.coll = 1; }
+                }
+            }
+            __syncthreads();
+            if (tid == 0) sm.qn = 0;
+            __syncthreads();
+            return nq;
+        };
+        // ---- M4 + M5: survivors and the Algorithm-1 owner = the latest extender
+        while (true) {
             for (int b = tid; b < k; b += NT) {
-                const int j = gl[b];
-                if (!p.absorbed[j]) continue;
-                const int ef = eb + b * (b + 1) / 2 + b;
-                const uint64_t H = p.ent_hash[ef];
+                if (own[b] != -2) continue;
+                const uint64_t H = eh[b * (b + 1) / 2 + b];   // full key of member b
                 const int32_t L = gln[b];
                 uint32_t dg = digest32(H, L);
                 if (dg == 0xFFFFFFFFu) dg = 0xFFFFFFFEu;
-                int best = p.tl_pos[p.owner_tl[j]] - gs;   // a surviving, (to be) verified extender: the fallback
-                int32_t bestL = gln[best];
+                const int lm = lim[b];
+                int best = -1;
                 visit(dg, [&](uint32_t le) {
                     const int rb = rank_of_local(le);
-                    if (rb <= b || rb == best) return;
+                    if (rb <= b || rb >= lm || rb <= best) return;
                     const int a = (int)le - rb * (rb + 1) / 2;
-                    if (gln[a] != L || p.ent_hash[eb + le] != H) return;
-                    const int i = gl[rb];
-                    if (p.absorbed[i]) return;
-                    const int32_t Li = gln[rb];
-                    if (!(Li > bestL || (Li == bestL && rb < best))) return;
-                    if (mode == 1 && !tokens_extend(p, i, j)) return;
+                    if (gln[a] != L || eh[le] != H) return;
                     best = rb;
-                    bestL = Li;
                 });
-                p.cand[j] = gl[best];   // staged: owner_tl is still being read by other threads
+                if (best < 0) own[b] = -1;
+                else if (badc[best] == badc[b]) own[b] = best;   // every link b+1 .. best was verified by the hash pass
+                else vq[atomicAdd(&sm.qn, 1)] = make_int2(b, best);
             }
-            __syncthreads();
-            for (int b = tid; b < k; b += NT) {
-                const int j = gl[b];
-                if (p.absorbed[j]) p.owner_tl[j] = p.cand[j];
-            }
+            if (run_queue([&](int b, int cd) { own[b] = cd; }, [&](int b, int cd) { lim[b] = cd; }) == 0) break;
         }
-        // ---- M5, first half: T_j is a prefix of its owner T_o for certain if every predecessor link between them was
-        // verified by the hash pass (prefix-of is transitive); only the other members are re-read by the scatter pass
-        for (int b = tid; b < k; b += NT) {
-            const int j = gl[b];
-            bool nv = p.absorbed[j] != 0;
-            if (nv && cached) {
-                const int o = p.tl_pos[p.owner_tl[j]] - gs;
-                nv = false;
-                for (int r = b + 1; r <= o; ++r) nv |= sm.bad[r] != 0;
+        if (longest) {
+            // the longest SURVIVING extender, then the lowest index (BASELINE.json north_star; DESIGN.md reading M-3)
+            for (int b = tid; b < k; b += NT) { fin[b] = own[b] >= 0 ? -2 : -1; exL[b] = INT32_MAX; exR[b] = -1; }
+            __syncthreads();
+            while (true) {
+                for (int b = tid; b < k; b += NT) {
+                    if (fin[b] != -2) continue;
+                    const uint64_t H = eh[b * (b + 1) / 2 + b];
+                    const int32_t L = gln[b];
+                    uint32_t dg = digest32(H, L);
+                    if (dg == 0xFFFFFFFFu) dg = 0xFFFFFFFEu;
+                    const int xL = exL[b], xR = exR[b];
+                    int best = -1;
+                    int32_t bestL = -1;
+                    visit(dg, [&](uint32_t le) {
+                        const int rb = rank_of_local(le);
+                        if (rb <= b || own[rb] >= 0) return;                       // survivors only
+                        const int32_t Li = gln[rb];
+                        if (!(Li < xL || (Li == xL && rb > xR))) return;            // after the last failure in (length desc, rank asc)
+                        if (!(Li > bestL || (Li == bestL && rb < best))) return;
+                        const int a = (int)le - rb * (rb + 1) / 2;
+                        if (gln[a] != L || eh[le] != H) return;
+                        best = rb;
+                        bestL = Li;
+                    });
+                    if (best < 0 || best == own[b]) fin[b] = own[b];                // the Algorithm-1 owner is verified already
+                    else if (badc[best] == badc[b]) fin[b] = best;
+                    else vq[atomicAdd(&sm.qn, 1)] = make_int2(b, best);
+                }
+                if (run_queue([&](int b, int cd) { fin[b] = cd; }, [&](int b, int cd) { exL[b] = gln[cd]; exR[b] = cd; }) == 0) break;
             }
-            p.needv[j] = nv;
+            for (int b = tid; b < k; b += NT)
+                if (own[b] >= 0) own[b] = fin[b];
+            __syncthreads();
+        }
+        // ---- outputs by timeline; members of every survivor, ascending
+        for (int b = tid; b < k; b += NT) {
+            const int j = gl[b], o = own[b] < 0 ? b : own[b];
+            p.absorbed[j] = own[b] >= 0;
+            p.owner_tl[j] = gl[o];
+            atomicAdd(&mcnt[o], 1);
+        }
+        __syncthreads();
+        block_scan<NT, 1>(
+            k, [&](int r) { return mcnt[r]; }, [&](int r, int64_t ex, int64_t) { mbase[r] = (int32_t)ex; }, sm.s_w);
+        // member slots: timeline, length, response start (exL / exR are free again: they hold the last two when the group
+        // works through the workspace)
+        int32_t* const mj = fast ? sg.mj : mem;
+        int32_t* const mL = fast ? sg.mL : exL;
+        int32_t* const mR = fast ? sg.mR : exR;
+        __syncthreads();
+        for (int b = tid; b < k; b += NT) {
+            const int o = own[b] < 0 ? b : own[b];
+            int at = 0;
+            for (int x = 0; x < b; ++x) at += (own[x] < 0 ? x : own[x]) == o ? 1 : 0;
+            const int slot = mbase[o] + at, j = gl[b], L = gln[b];
+            mem[slot] = j;
+            mj[slot] = j;
+            mL[slot] = L;
+            mR[slot] = fast ? sg.rs[b] : (explicit_masks ? 0 : min(max(__ldg(p.resp_start + j), 0), L));
+        }
+        __syncthreads();
+        // ---- segments of every survivor, one warp each
+        for (int b = warp; b < k; b += NT / 32) {
+            if (own[b] >= 0) continue;
+            const int mb = mbase[b], mc = mcnt[b];
+            const int sc = build_segments(explicit_masks, mj + mb, mL + mb, mR + mb, mc, rs_out + 2 * mb);
+            if (lane == 0) p.sv_rec[gl[b]] = make_int4(gs + mb, mc, 2 * (gs + mb), sc);
         }
         __syncthreads();
     }
+    AJT_TMAX(9);
+    if (tid == 0 && sm.coll) {
+        atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_HASH_COLLISION);
+        p.ctrl->collision = 1;
+    }
 }
 
-__global__ void __launch_bounds__(kSelThreads) merge_select_kernel(const MergeParams p) {
-    __shared__ SelectSmem sm;
+// ---------------------------------------------------------------------------------------- K4: plan (M7, records)
+
+// (a) one warp per merged sequence: its relative segments -> global segment records at output positions;
+// (b) one thread per output tile: the segment that holds the tile's first position.
+__global__ void __launch_bounds__(256) merge_plan_kernel(const MergeParams p) {
     if (fatal(p)) return;
-    select_body<kSelThreads>(p, 0, sm);
-}
-
-// ---------------------------------------------------------------------------------------- K6: compact (M6)
-
-template <int NT>
-__device__ void compact_body(const MergeParams& p, int mode, int64_t (*s_w)[2][NT / 32]) {
-    const int tid = threadIdx.x, n = p.n;
-    // one fused scan over the timelines: survivors (-> merged index), their scatter tiles, their lengths (-> offsets).
-    // A merged sequence starting at merged offset mo is tiled on the 4-element grid of the OUTPUT arrays, so it needs
-    // ceil((L + (mo & 3)) / kTile) tiles; (L + 3) bounds that without knowing mo (an empty extra tile exits at once).
-    const I2 tot = block_scan2<NT>(
-        n,
-        [&](int i) {
-            if (mode == 0 ? __ldg(p.absorbed + i) : p.absorbed[i]) return I2{0, 0};   // (mode 1: written earlier in this launch)
-            const int64_t L = tl_len(p, i);
-            return I2{((int64_t)1 << 32) | ((L + 3 + kTile - 1) / kTile), L};
-        },
-        [&](int i, int64_t exa, int64_t exb, int64_t va, int64_t) {
-            if (!va) { p.midx[i] = -1; return; }
-            const int m = (int)(exa >> 32);
-            p.midx[i] = m;
-            p.merged_origin[m] = i;
-            p.merged_traj[m] = __ldg(p.traj_ids + i);
-            p.merged_offsets[m] = exb;
-            p.tile_base[m] = (int32_t)(exa & 0xffffffff);
-        },
-        s_w);
-    const int M = (int)(tot.a >> 32);
-    const int32_t ntiles = (int32_t)(tot.a & 0xffffffff);
-#pragma unroll 4
-    for (int i = tid; i < n; i += NT) p.owner[i] = p.midx[mode == 0 ? __ldg(p.owner_tl + i) : p.owner_tl[i]];
-    if (tid == 0) {
-        p.merged_offsets[M] = tot.b;
-        p.tile_base[M] = ntiles;
-        p.counts[0] = M;
-        p.counts[1] = tot.b;
-        p.ctrl->M = M;
-        p.ctrl->N_out = tot.b;
-        p.ctrl->n_tiles = ntiles;
-        if (mode == 1) {
-            p.ctrl->collision = 2;   // repair in progress: the scatter pass must not find another mismatch
-            atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_HASH_COLLISION);
-        }
-    }
-}
-
-__global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p) {
-    __shared__ int64_t s_w[2][2][32];
-    if (fatal(p)) {   // outputs are unspecified after a fatal status, but the counts a caller may chain on are not garbage
-        if (threadIdx.x == 0) { p.counts[0] = 0; p.counts[1] = 0; }
-        return;
-    }
-    compact_body<1024>(p, 0, s_w);
-}
-
-// ---------------------------------------------------------------------------------------- K5 + K7: verify + scatter (M5, M7)
-
-// Warp task = one tile of kTile positions of one merged sequence, laid on the 4-element grid of the OUTPUT arrays so that
-// tokens / src / old_logp leave as 16-byte stores and the mask as 4-byte stores.  Lane l holds positions
-// qbase + 128 u + 4 l + e (u < 4, e < 4).  A warp takes a contiguous run of tiles, so the members of a merged sequence (the
-// absorbed timelines it owns, found among the earlier timelines of its group) are gathered once per sequence into a
-// per-warp shared-memory list {index, length, resp_start, token offset}, ascending.  Each member is compared against the
-// survivor exactly (M5) and painted into the slot map in ascending order; slot 0 = nobody, c + 1 = member c, 33 = survivor.
-constexpr int kMemCap = 32;
-struct MemberList {
-    int64_t jo[kMemCap];
-    int32_t j[kMemCap], L[kMemCap], rs[kMemCap];
-    uint8_t nv[kMemCap];
-};
-
-struct TileCtx {
-    int s, Ls, rs_s, gs, rank_s;
-    int64_t so, mo;
-};
-
-// Slow path for a sequence with more than kMemCap members: walks the group's earlier timelines for every tile.
-template <bool kExplicit>
-__device__ __noinline__ bool scatter_tile_generic(const MergeParams& p, const TileCtx c, int qbase, bool vec_ok) {
-    constexpr int kU = kTile / 128;
-    const int lane = threadIdx.x & 31;
-    const int ql = qbase + 4 * lane;
-    const int s = c.s, Ls = c.Ls;
-    bool mismatch = false;
-    int32_t x[kU][4], src[kU][4];
-#pragma unroll
-    for (int u = 0; u < kU; ++u)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const int q = ql + 128 * u + e;
-            const bool v = q >= 0 && q < Ls;
-            x[u][e] = v ? p.tokens[c.so + q] : 0;
-            bool mk = false;
-            if (v) mk = kExplicit ? (p.mask_in[c.so + q] != 0) : (q >= c.rs_s);
-            src[u][e] = mk ? s : -1;
-        }
-    const int qlo = max(qbase, 0);
-    for (int a0 = 0; a0 < c.rank_s; a0 += 32) {
-        const int a = a0 + lane;
-        int j = -1, Lj = 0;
-        if (a < c.rank_s) {
-            Lj = p.glen[c.gs + a];
-            if (Lj > qlo) {
-                j = p.perm[c.gs + a];
-                if (p.owner_tl[j] != s) j = -1;
-            }
-        }
-        unsigned hits = __ballot_sync(0xffffffffu, j >= 0);
-        while (hits) {
-            const int sl = __ffs(hits) - 1;
-            hits &= hits - 1;
-            const int jj = __shfl_sync(0xffffffffu, j, sl), Ljj = __shfl_sync(0xffffffffu, Lj, sl);
-            const int64_t jo = p.offsets[jj];
-            const int rs_j = kExplicit ? 0 : p.resp_start[jj];
-#pragma unroll
-            for (int u = 0; u < kU; ++u) {
-                if (qbase + 128 * u >= Ljj) break;   // warp-uniform: the member ends before this step
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int q = ql + 128 * u + e;
-                    if (q >= 0 && q < Ljj) {
-                        if (p.tokens[jo + q] != x[u][e]) mismatch = true;     // exact verification (M5)
-                        const bool mk = kExplicit ? (p.mask_in[jo + q] != 0) : (q >= rs_j);
-                        if (mk) src[u][e] = max(src[u][e], jj);
-                    }
-                }
-            }
-        }
-    }
-    const int64_t dbase = c.mo + ql;   // multiple of 4
-#pragma unroll
-    for (int u = 0; u < kU; ++u) {
-        const int q = ql + 128 * u;
-        if (q >= Ls || q + 3 < 0) continue;
-        const int64_t d = dbase + 128 * u;
-        float lp[4] = {0.f, 0.f, 0.f, 0.f};
-        if (p.merged_old_logp) {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int sj = src[u][e];
-                if (sj >= 0) lp[e] = p.old_logp_in[(sj == s ? c.so : p.offsets[sj]) + q + e];
-            }
-        }
-        if (vec_ok && q >= 0 && q + 3 < Ls) {
-            *reinterpret_cast<int4*>(p.merged_tokens + d) = make_int4(x[u][0], x[u][1], x[u][2], x[u][3]);
-            *reinterpret_cast<int4*>(p.merged_src + d) = make_int4(src[u][0], src[u][1], src[u][2], src[u][3]);
-            *reinterpret_cast<uint32_t*>(p.merged_mask + d) = (src[u][0] >= 0 ? 1u : 0u) | (src[u][1] >= 0 ? 0x100u : 0u) |
-                                                              (src[u][2] >= 0 ? 0x10000u : 0u) | (src[u][3] >= 0 ? 0x1000000u : 0u);
-            if (p.merged_old_logp) *reinterpret_cast<float4*>(p.merged_old_logp + d) = make_float4(lp[0], lp[1], lp[2], lp[3]);
-        } else {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                if (q + e >= 0 && q + e < Ls) {
-                    p.merged_tokens[d + e] = x[u][e];
-                    p.merged_src[d + e] = src[u][e];
-                    p.merged_mask[d + e] = src[u][e] >= 0;
-                    if (p.merged_old_logp) p.merged_old_logp[d + e] = lp[e];
-                }
-            }
-        }
-    }
-    return mismatch;
-}
-
-template <bool kExplicit>
-__device__ __forceinline__ bool scatter_tile_fast(const MergeParams& p, const TileCtx& c, int qbase, bool vec_ok,
-                                                  const MemberList& ml, int cnt) {
-    constexpr int kU = kTile / 128;
-    constexpr int kSurv = kMemCap + 1;
-    const int lane = threadIdx.x & 31;
-    const int ql = qbase + 4 * lane;
-    const int s = c.s, Ls = c.Ls;
-    bool mismatch = false;
-    const bool full = qbase >= 0 && qbase + kTile <= Ls;   // warp-uniform: every slot of the tile is a position of the sequence
-    const int32_t* __restrict__ tok = p.tokens + c.so;
-    // ---- uniform tile: every response region [rs_m, L_m) of a member (and the survivor's own) either covers the whole tile
-    // or misses it, and nobody needs verifying here: one source for the whole tile.  Regions are hundreds of tokens long, so
-    // most tiles are of this kind; they cost a plain copy instead of a per-element walk over the members.
-    if (!kExplicit && full && vec_ok) {
-        const int qhi = qbase + kTile;
-        bool covers = false, partial = false;
-        if (lane < cnt) {
-            const int Lm = ml.L[lane], rsm = ml.rs[lane];
-            covers = rsm <= qbase && Lm >= qhi;
-            partial = (!covers && Lm > qbase && rsm < qhi) || (ml.nv[lane] && Lm > qbase);
-        }
-        const bool s_covers = c.rs_s <= qbase;
-        if (!__any_sync(0xffffffffu, partial) && (s_covers || c.rs_s >= qhi)) {
-            const unsigned cb = __ballot_sync(0xffffffffu, covers);
-            const int sl = s_covers ? kSurv : (cb ? 32 - __clz(cb) : 0);
-            const int32_t sj = sl == 0 ? -1 : (sl == kSurv ? s : ml.j[sl - 1]);
-            const float* __restrict__ lps = p.old_logp_in + (sl == kSurv ? c.so : (sl ? ml.jo[sl - 1] : 0));
-            const bool want_lp = p.merged_old_logp != nullptr && sl != 0;
-            const bool tvec = (((uintptr_t)(tok + qbase)) & 15) == 0, lvec = want_lp && (((uintptr_t)(lps + qbase)) & 15) == 0;
-            int4 xv[kU];
-            float4 lv[kU];
-#pragma unroll
-            for (int u = 0; u < kU; ++u) {
-                const int q = ql + 128 * u;
-                if (tvec) xv[u] = __ldg(reinterpret_cast<const int4*>(tok + q));
-                else xv[u] = make_int4(__ldg(tok + q), __ldg(tok + q + 1), __ldg(tok + q + 2), __ldg(tok + q + 3));
-                lv[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (lvec) lv[u] = __ldg(reinterpret_cast<const float4*>(lps + q));
-                else if (want_lp) lv[u] = make_float4(__ldg(lps + q), __ldg(lps + q + 1), __ldg(lps + q + 2), __ldg(lps + q + 3));
-            }
-            const int64_t d0 = c.mo + ql;
-#pragma unroll
-            for (int u = 0; u < kU; ++u) {
-                const int64_t d = d0 + 128 * u;
-                *reinterpret_cast<int4*>(p.merged_tokens + d) = xv[u];
-                *reinterpret_cast<int4*>(p.merged_src + d) = make_int4(sj, sj, sj, sj);
-                *reinterpret_cast<uint32_t*>(p.merged_mask + d) = sl ? 0x01010101u : 0u;
-                if (p.merged_old_logp) *reinterpret_cast<float4*>(p.merged_old_logp + d) = lv[u];
-            }
-            return false;
-        }
-    }
-    int32_t x[kU][4];
-    int32_t slot[kU][4];
-#pragma unroll
-    for (int u = 0; u < kU; ++u)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const int q = ql + 128 * u + e;
-            const bool v = full || (q >= 0 && q < Ls);
-            x[u][e] = v ? tok[q] : 0;
-            bool mk = false;
-            if (v) mk = kExplicit ? (p.mask_in[c.so + q] != 0) : (q >= c.rs_s);
-            slot[u][e] = mk ? kSurv : 0;
-        }
-    const int qlo = max(qbase, 0);
-    for (int m = 0; m < cnt; ++m) {
-        const int Lj = ml.L[m];
-        if (Lj <= qlo) continue;                 // warp-uniform: the member ends before this tile
-        const int rs_j = ml.rs[m];
-        const int32_t* __restrict__ tj = p.tokens + ml.jo[m];
-        const uint8_t* mkj = kExplicit ? p.mask_in + ml.jo[m] : nullptr;
-        // all of the member's loads first (independent), then the compares: one memory latency per member, not one per element
-        if (kExplicit || ml.nv[m]) {   // warp-uniform
-            int32_t y[kU][4];
-            uint8_t ym[kU][4];
-#pragma unroll
-            for (int u = 0; u < kU; ++u)
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int q = ql + 128 * u + e;
-                    const bool in = q >= 0 && q < Lj;
-                    y[u][e] = in ? tj[q] : x[u][e];
-                    if (kExplicit) ym[u][e] = in ? mkj[q] : (uint8_t)0;
-                }
-#pragma unroll
-            for (int u = 0; u < kU; ++u)
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int q = ql + 128 * u + e;
-                    mismatch |= y[u][e] != x[u][e];     // exact verification (M5, second half)
-                    const bool mk = kExplicit ? (ym[u][e] != 0) : (q >= rs_j && q < Lj);
-                    if (mk) slot[u][e] = max(slot[u][e], m + 1);
-                }
-        } else {
-#pragma unroll
-            for (int u = 0; u < kU; ++u)
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int q = ql + 128 * u + e;
-                    if (q >= rs_j && q < Lj) slot[u][e] = max(slot[u][e], m + 1);
-                }
-        }
-    }
-    // ---- outputs
-    const int64_t dbase = c.mo + ql;   // multiple of 4
-    float lp[kU][4];
-    if (p.merged_old_logp) {
-#pragma unroll
-        for (int u = 0; u < kU; ++u)
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int sl = slot[u][e];
-                lp[u][e] = 0.f;
-                if (sl) lp[u][e] = p.old_logp_in[(sl == kSurv ? c.so : ml.jo[sl - 1]) + ql + 128 * u + e];
-            }
-    }
-#pragma unroll
-    for (int u = 0; u < kU; ++u) {
-        const int q = ql + 128 * u;
-        if (!full && (q >= Ls || q + 3 < 0)) continue;
-        const int64_t d = dbase + 128 * u;
-        int32_t sj[4];
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const int sl = slot[u][e];
-            sj[e] = sl == 0 ? -1 : (sl == kSurv ? s : ml.j[sl - 1]);
-        }
-        if (vec_ok && (full || (q >= 0 && q + 3 < Ls))) {
-            *reinterpret_cast<int4*>(p.merged_tokens + d) = make_int4(x[u][0], x[u][1], x[u][2], x[u][3]);
-            *reinterpret_cast<int4*>(p.merged_src + d) = make_int4(sj[0], sj[1], sj[2], sj[3]);
-            *reinterpret_cast<uint32_t*>(p.merged_mask + d) =
-                (sj[0] >= 0 ? 1u : 0u) | (sj[1] >= 0 ? 0x100u : 0u) | (sj[2] >= 0 ? 0x10000u : 0u) | (sj[3] >= 0 ? 0x1000000u : 0u);
-            if (p.merged_old_logp)
-                *reinterpret_cast<float4*>(p.merged_old_logp + d) = make_float4(lp[u][0], lp[u][1], lp[u][2], lp[u][3]);
-        } else {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                if (q + e >= 0 && q + e < Ls) {
-                    p.merged_tokens[d + e] = x[u][e];
-                    p.merged_src[d + e] = sj[e];
-                    p.merged_mask[d + e] = sj[e] >= 0;
-                    if (p.merged_old_logp) p.merged_old_logp[d + e] = lp[u][e];
-                }
-            }
-        }
-    }
-    return mismatch;
-}
-
-template <bool kExplicit>
-__device__ void scatter_body(const MergeParams& p, int mode, MemberList* lists) {
     const int lane = threadIdx.x & 31;
     const int wglobal = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
-    const int ntiles = p.ctrl->n_tiles, M = p.ctrl->M;
-    const int per = (ntiles + nwarps - 1) / nwarps;
-    const int t_begin = wglobal * per, t_end = min(ntiles, t_begin + per);
-    if (t_begin >= t_end) return;
-    MemberList& ml = lists[threadIdx.x >> 5];
-    const bool vec_ok = ((((uintptr_t)p.merged_tokens | (uintptr_t)p.merged_src | (uintptr_t)p.merged_old_logp) & 15) == 0) &&
-                        (((uintptr_t)p.merged_mask & 3) == 0);
-    bool mismatch = false;
-    int m = warp_search_last_le(M, t_begin, [&](int x) { return p.tile_base[x]; });
-    int cur_m = -1, cnt = 0, tb = 0;
-    int tb_next = p.tile_base[m + 1];   // first tile of the next sequence: kept in a register, so that a tile inside a
-                                        // sequence does not start with a dependent global load
-    TileCtx c = {};
-    for (int t = t_begin; t < t_end; ++t) {
-        while (tb_next <= t) {
-            ++m;
-            tb_next = p.tile_base[m + 1];
+    const int M = p.ctrl->M, ntiles = p.ctrl->n_tiles;
+    const int64_t N_out = p.ctrl->N_out;
+    for (int m = wglobal; m < M; m += nwarps) {
+        const int s = __ldg(p.merged_origin + m);
+        const int4 sr = __ldg(p.sv_rec + s);
+        const int64_t mo = __ldg(p.merged_offsets + m), so = __ldg(p.offsets + s);
+        const int gb = __ldg(p.gseg_base + m);
+        for (int li = lane; li < sr.w; li += 32) {
+            const int2 rs = __ldg(p.rseg + sr.z + li);
+            GSeg o;
+            o.out_start = mo + rs.x;
+            o.tok_delta = so - mo;
+            o.src = rs.y;
+            o.aux = 0;
+            if (rs.y >= 0) o.lp_delta = __ldg(p.offsets + rs.y) - mo;
+            else if (rs.y == kSrcExplicit) { o.lp_delta = sr.x; o.aux = sr.y; }
+            else o.lp_delta = 0;
+            p.gseg[gb + li] = o;
         }
-        if (m != cur_m) {
-            cur_m = m;
-            tb = p.tile_base[m];
-            c.s = p.merged_origin[m];
-            c.mo = p.merged_offsets[m];
-            const int4 rec = p.tl_rec[p.tl_pos[c.s]];
-            c.gs = rec.y;
-            c.rank_s = rec.z;
-            c.so = p.offsets[c.s];
-            c.Ls = (int)(p.offsets[c.s + 1] - c.so);
-            c.rs_s = kExplicit ? 0 : p.resp_start[c.s];
-            // members of s: earlier timelines of its group that it owns, ascending
-            __syncwarp();
-            cnt = 0;
-            for (int a0 = 0; a0 < c.rank_s; a0 += 32) {
-                const int a = a0 + lane;
-                int j = -1;
-                if (a < c.rank_s) {
-                    j = p.perm[c.gs + a];
-                    if (p.owner_tl[j] != c.s) j = -1;
-                }
-                const unsigned bal = __ballot_sync(0xffffffffu, j >= 0);
-                const int pos = cnt + __popc(bal & ((1u << lane) - 1u));
-                if (j >= 0 && pos < kMemCap) {
-                    ml.j[pos] = j;
-                    ml.L[pos] = p.glen[c.gs + a];
-                    ml.rs[pos] = kExplicit ? 0 : p.resp_start[j];
-                    ml.jo[pos] = p.offsets[j];
-                    ml.nv[pos] = p.needv[j];
-                }
-                cnt += __popc(bal);
-            }
-            __syncwarp();
-        }
-        const int qbase = (t - tb) * kTile - (int)(c.mo & 3);   // position of the tile's first slot (may be -3..-1)
-        if (qbase >= c.Ls) continue;
-        if (cnt <= kMemCap) mismatch |= scatter_tile_fast<kExplicit>(p, c, qbase, vec_ok, ml, cnt);
-        else mismatch |= scatter_tile_generic<kExplicit>(p, c, qbase, vec_ok);
     }
-    if (__any_sync(0xffffffffu, mismatch) && lane == 0) {
-        if (mode == 0) atomicExch(&p.ctrl->collision, 1);
-        else atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_INTERNAL);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        GSeg o;
+        o.out_start = N_out; o.tok_delta = 0; o.lp_delta = 0; o.src = kSrcNone; o.aux = 0;
+        p.gseg[p.ctrl->n_gsegs] = o;
+    }
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < ntiles; t += gridDim.x * blockDim.x) {
+        const int64_t d = (int64_t)t << kTSLog;
+        int lo = 0, hi = M - 1;   // last merged sequence that starts at or before d
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (__ldg(p.merged_offsets + mid) <= d) lo = mid; else hi = mid - 1;
+        }
+        const int s = __ldg(p.merged_origin + lo);
+        const int4 sr = __ldg(p.sv_rec + s);
+        const int64_t pr = d - __ldg(p.merged_offsets + lo);
+        int a = 0, b = sr.w - 1;   // last relative segment that starts at or before pr
+        while (a < b) {
+            const int mid = (a + b + 1) >> 1;
+            if ((int64_t)__ldg(p.rseg + sr.z + mid).x <= pr) a = mid; else b = mid - 1;
+        }
+        p.tile_seg[t] = __ldg(p.gseg_base + lo) + a;
+    }
+}
+
+// ---------------------------------------------------------------------------------------- K5: scatter (M7)
+
+// The source of one token under explicit masks: the largest member index whose mask is 1 at position q (reading M-7).
+__device__ __noinline__ int32_t explicit_src(const int32_t* __restrict__ mem, const int64_t* __restrict__ offsets,
+                                             const uint8_t* __restrict__ mask_in, int cnt, int64_t q) {
+    for (int x = cnt - 1; x >= 0; --x) {
+        const int j = __ldg(mem + x);
+        const int64_t oj = __ldg(offsets + j);
+        if (q < __ldg(offsets + j + 1) - oj && __ldg(mask_in + oj + q) != 0) return j;
+    }
+    return kSrcNone;
+}
+
+__device__ __forceinline__ GSeg load_gseg(const GSeg* g) {
+    const int4 a = __ldg(reinterpret_cast<const int4*>(g)), b = __ldg(reinterpret_cast<const int4*>(g) + 1);
+    GSeg o;
+    o.out_start = (int64_t)(((uint64_t)(uint32_t)a.y << 32) | (uint32_t)a.x);
+    o.tok_delta = (int64_t)(((uint64_t)(uint32_t)a.w << 32) | (uint32_t)a.z);
+    o.lp_delta = (int64_t)(((uint64_t)(uint32_t)b.y << 32) | (uint32_t)b.x);
+    o.src = b.z;
+    o.aux = b.w;
+    return o;
+}
+__device__ __forceinline__ void stg32_stream(void* ptr, uint32_t v) {
+    asm volatile("st.global.L1::no_allocate.u32 [%0], %1;" ::"l"(ptr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t ldg32_stream(const void* ptr) {
+    uint32_t v;
+    asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(ptr));
+    return v;
+}
+
+// One tile moved position by position through registers, walking the segment records from the tile's first one: the path
+// for explicit masks, for the last (partial) tile, for tiles cut into more than 8 pieces and for pieces at the very ends
+// of the input arrays.  Lane l owns positions l + 32 j of the tile.
+struct ScatPtrs {   // what the walk needs, passed by value (a reference to the kernel parameters would copy all of them to the stack)
+    const int32_t* tokens; const float* old_logp_in; const int64_t* offsets; const uint8_t* mask_in; const int32_t* mem_list;
+    const GSeg* gseg; const int32_t* tile_seg;
+    int32_t* merged_tokens; uint8_t* merged_mask; int32_t* merged_src; float* merged_old_logp;
+};
+__device__ __noinline__ void scatter_tile_walk(const ScatPtrs p, int t, int64_t N_out) {
+    const int lane = threadIdx.x & 31;
+    const int32_t* __restrict__ tokens = p.tokens;
+    const float* __restrict__ lps = p.old_logp_in;
+    const bool want_lp = p.merged_old_logp != nullptr;
+    const int64_t d0 = ((int64_t)t << kTSLog) + lane;
+    int idx = __ldg(p.tile_seg + t);
+    GSeg cur = load_gseg(p.gseg + idx);
+    int64_t nxt = __ldg(&p.gseg[idx + 1].out_start);
+#pragma unroll 1
+    for (int j0 = 0; j0 < 16; j0 += 4) {
+        uint32_t xg[4], lg[4];
+        int32_t sg[4];
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+            const int64_t d = d0 + 32 * (j0 + jj);
+            xg[jj] = 0u; lg[jj] = 0u; sg[jj] = kSrcNone;
+            if (d < N_out) {
+                while (d >= nxt) {
+                    ++idx;
+                    cur = load_gseg(p.gseg + idx);
+                    nxt = __ldg(&p.gseg[idx + 1].out_start);
+                }
+                xg[jj] = (uint32_t)__ldg(tokens + (d + cur.tok_delta));
+                int32_t sj = cur.src;
+                if (sj == kSrcExplicit) {
+                    const int64_t q = d - cur.out_start;
+                    sj = explicit_src(p.mem_list + cur.lp_delta, p.offsets, p.mask_in, cur.aux, q);
+                    if (want_lp && sj >= 0) lg[jj] = __float_as_uint(__ldg(lps + (__ldg(p.offsets + sj) + q)));
+                } else if (want_lp && sj >= 0) {
+                    lg[jj] = __float_as_uint(__ldg(lps + (d + cur.lp_delta)));
+                }
+                sg[jj] = sj;
+            }
+        }
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+            const int64_t d = d0 + 32 * (j0 + jj);
+            if (d < N_out) {
+                p.merged_tokens[d] = (int32_t)xg[jj];
+                p.merged_src[d] = sg[jj];
+                p.merged_mask[d] = sg[jj] >= 0 ? 1 : 0;
+                if (want_lp) p.merged_old_logp[d] = __uint_as_float(lg[jj]);
+            }
+        }
     }
 }
 
 constexpr int kScatThreads = 256;
-__global__ void __launch_bounds__(kScatThreads, 4) merge_scatter_kernel(const MergeParams p) {
-    __shared__ MemberList lists[kScatThreads / 32];
+constexpr int kScatInBytes = 2560;                                   // one input array of a tile: 2 KB + 16-byte slack of up to 8 pieces
+constexpr int kScatOutBytes = 3 * kTS * 4 + kTS;                     // tokens, src, old_logp, mask of one tile
+constexpr int kScatWarpBytes = 2 * 2 * kScatInBytes + 2 * kScatOutBytes + 2 * 8 * 32 + 128;   // 2 stages in, 2 out, piece tables, barriers
+constexpr int kScatSmem = (kScatThreads / 32) * kScatWarpBytes + 128;
+static_assert(kScatWarpBytes % 128 == 0, "warp regions stay 128-byte aligned");
+
+// Warp per tile of 512 OUTPUT positions, all bulk data through the TMA engine: a tile is cut at segment boundaries into
+// at most 8 pieces; the lane that owns a piece launches one bulk async copy of the 16-byte-aligned superset of its token
+// source (and one of its log-prob source) into the warp's input stage, one tile ahead; the warp then rewrites the pieces at
+// the output's alignment into a staging copy of the four output rows (32-bit shared-memory accesses, conflict-free) and one
+// lane sends them off with four bulk stores.  Requests of kilobytes instead of 128 bytes: what it takes to fill HBM.
+__global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const MergeParams p) {
+    extern __shared__ __align__(128) uint8_t sc_dyn[];
     if (fatal(p)) return;
-    if (p.mask_in) scatter_body<true>(p, 0, lists);
-    else scatter_body<false>(p, 0, lists);
+    const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
+    const int wglobal = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int ntiles = p.ctrl->n_tiles, nseg = p.ctrl->n_gsegs;
+    const int64_t N_out = p.ctrl->N_out, N = p.N;
+    const bool want_lp = p.merged_old_logp != nullptr;
+    const int mis_t = p.mis, mis_l = (int)(((uintptr_t)p.old_logp_in >> 2) & 3);
+    uint8_t* const wb = reinterpret_cast<uint8_t*>(((uintptr_t)sc_dyn + 127) & ~(uintptr_t)127) + (size_t)wic * kScatWarpBytes;
+    uint8_t* const in_base = wb;                                            // [stage][tok | lp]
+    uint8_t* const out_base = wb + 4 * kScatInBytes;                        // [stage][tok | src | lp | mask]
+    int4* const tbl = reinterpret_cast<int4*>(wb + 4 * kScatInBytes + 2 * kScatOutBytes);   // [stage][8 pieces][2]
+    uint64_t* const full = reinterpret_cast<uint64_t*>(wb + 4 * kScatInBytes + 2 * kScatOutBytes + 2 * 8 * 32);
+    const ScatPtrs sp = {p.tokens, p.old_logp_in, p.offsets, p.mask_in, p.mem_list, p.gseg, p.tile_seg,
+                         p.merged_tokens, p.merged_mask, p.merged_src, p.merged_old_logp};
+    if (lane == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        fence_mbar_init();
+    }
+    __syncwarp();
+    uint32_t phases = 0;
+    // plan(t, stage): cuts tile t into pieces, launches their copies into input stage `stage`; returns the number of pieces,
+    // or -1 when the tile takes the register walk.  rec = this lane's segment record of the tile (lane l: record s0 + l).
+    auto plan = [&](int t, int stage, const GSeg& rec) -> int {
+        const int64_t dt = (int64_t)t << kTSLog;
+        const int64_t rel64 = rec.out_start - dt;
+        const int rel = (int)max((int64_t)-1, min(rel64, (int64_t)kTS));           // lane 0: <= 0; later lanes: > 0, kTS = beyond
+        const int reln = __shfl_down_sync(0xffffffffu, rel, 1);
+        const bool valid = lane < 8 && (lane == 0 || rel < kTS);
+        const int np = __popc(__ballot_sync(0xffffffffu, valid));
+        const int rel8 = __shfl_sync(0xffffffffu, rel, 8);
+        const int q0 = max(rel, 0), q1 = min(reln, kTS);
+        bool bad = false;
+        uint32_t tb = 0, lb = 0;
+        int64_t tg0 = 0, lg0 = 0;
+        int tw = 0, lw = -1;
+        if (valid) {
+            bad = rec.src == kSrcExplicit;
+            const int pb = ((4 * q0) & ~15) + 48 * lane;                           // byte offset of the piece in the input stage
+            const int64_t e0 = dt + q0 + rec.tok_delta;
+            const int a = (int)((e0 + mis_t) & 3);
+            tg0 = e0 - a;
+            tb = (uint32_t)(((q1 - q0 + a + 3) >> 2) << 4);
+            tw = (pb >> 2) + a;
+            bad = bad || tg0 < 0 || tg0 + (tb >> 2) > N;
+            if (want_lp && rec.src >= 0) {
+                const int64_t f0 = dt + q0 + rec.lp_delta;
+                const int al = (int)((f0 + mis_l) & 3);
+                lg0 = f0 - al;
+                lb = (uint32_t)(((q1 - q0 + al + 3) >> 2) << 4);
+                lw = (pb >> 2) + al;
+                bad = bad || lg0 < 0 || lg0 + (lb >> 2) > N;
+            }
+        }
+        if (__any_sync(0xffffffffu, bad) || rel8 < kTS || dt + kTS > N_out) return -1;
+        uint8_t* const ib = in_base + stage * 2 * kScatInBytes;
+        const uint32_t total = __reduce_add_sync(0xffffffffu, valid ? tb + lb : 0u);
+        if (valid) {
+            tbl[(stage * 8 + lane) * 2] = make_int4(q0, q1, tw, lw);
+            tbl[(stage * 8 + lane) * 2 + 1] = make_int4(rec.src, 0, 0, 0);
+            bulk_load(ib + (((4 * q0) & ~15) + 48 * lane), p.tokens + tg0, tb, &full[stage]);
+            if (lb) bulk_load(ib + kScatInBytes + (((4 * q0) & ~15) + 48 * lane), p.old_logp_in + lg0, lb, &full[stage]);
+        }
+        if (lane == 0) mbar_arrive_expect_tx(&full[stage], total);
+        return np;
+    };
+    auto load_rec = [&](int t) -> GSeg {
+        const int s0 = __ldg(p.tile_seg + t);
+        return load_gseg(p.gseg + min(s0 + lane, nseg));   // lanes beyond the last record read the sentinel (starts at N_out)
+    };
+    const bool out_ok = ((((uintptr_t)p.merged_tokens | (uintptr_t)p.merged_src | (uintptr_t)p.merged_old_logp | (uintptr_t)p.merged_mask) & 15) == 0);
+    if (wglobal >= ntiles) return;
+    GSeg rec = load_rec(wglobal);
+    int np_cur = out_ok ? plan(wglobal, 0, rec) : -1;
+    if (wglobal + nwarps < ntiles) rec = load_rec(wglobal + nwarps);
+    int it = 0;
+    bool dead = false;
+#pragma unroll 1
+    for (int t = wglobal; t < ntiles; t += nwarps, ++it) {
+        const int st = it & 1;
+        int np_next = -1;
+        if (t + nwarps < ntiles) {   // next tile: its copies fly while this one is rewritten; the tile after: its record
+            if (out_ok) np_next = plan(t + nwarps, st ^ 1, rec);
+            if (t + 2 * nwarps < ntiles) rec = load_rec(t + 2 * nwarps);
+        }
+        if (np_cur < 0) {
+            scatter_tile_walk(sp, t, N_out);
+        } else {
+            const int64_t dt = (int64_t)t << kTSLog;
+            const uint32_t in_tok = smem_u32(in_base + st * 2 * kScatInBytes), in_lp = in_tok + kScatInBytes;
+            uint8_t* const ob = out_base + st * kScatOutBytes;
+            const uint32_t out_tok = smem_u32(ob), out_src = out_tok + 4 * kTS, out_lp = out_tok + 8 * kTS, out_mask = out_tok + 12 * kTS;
+            if (lane == 0) bulk_wait_read<1>();   // the stores of two tiles ago have read this staging copy
+            __syncwarp();
+            if (!mbar_wait_bounded(&full[st], (phases >> st) & 1u)) dead = true;
+            phases ^= 1u << st;
+            if (np_cur == 1) {
+                const int4 e0 = tbl[(st * 8) * 2], e1 = tbl[(st * 8) * 2 + 1];
+                const uint32_t a0 = in_tok + 4 * (e0.z + lane), o0 = out_tok + 4 * lane;
+#pragma unroll
+                for (int j = 0; j < 16; ++j) sts32(o0 + 128 * j, lds32(a0 + 128 * j));
+                if (want_lp) {
+                    if (e0.w >= 0) {
+                        const uint32_t b0 = in_lp + 4 * (e0.w + lane), q0 = out_lp + 4 * lane;
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) sts32(q0 + 128 * j, lds32(b0 + 128 * j));
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+                            asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(out_lp + 16 * lane + 512 * j), "r"(0u) : "memory");
+                    }
+                }
+                const uint32_t sv = (uint32_t)e1.x, mk = e1.x >= 0 ? 0x01010101u : 0u;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(out_src + 16 * lane + 512 * j), "r"(sv) : "memory");
+                    sts32(out_mask + 4 * lane + 128 * j, mk);
+                }
+            } else {
+#pragma unroll 1
+                for (int pi = 0; pi < np_cur; ++pi) {
+                    const int4 e0 = tbl[(st * 8 + pi) * 2], e1 = tbl[(st * 8 + pi) * 2 + 1];
+                    const uint32_t sv = (uint32_t)e1.x;
+                    for (int q = e0.x + lane; q < e0.y; q += 32) {
+                        sts32(out_tok + 4 * q, lds32(in_tok + 4 * (e0.z + q - e0.x)));
+                        sts32(out_src + 4 * q, sv);
+                        if (want_lp) sts32(out_lp + 4 * q, e0.w >= 0 ? lds32(in_lp + 4 * (e0.w + q - e0.x)) : 0u);
+                        asm volatile("st.shared.u8 [%0], %1;" ::"r"(out_mask + q), "r"(e1.x >= 0 ? 1u : 0u) : "memory");
+                    }
+                }
+            }
+            fence_proxy_async_smem();   // the staging copy was written through the generic proxy, the bulk stores read it through the async one
+            __syncwarp();
+            if (lane == 0) {
+                bulk_store(p.merged_tokens + dt, ob, 4 * kTS);
+                bulk_store(p.merged_src + dt, ob + 4 * kTS, 4 * kTS);
+                if (want_lp) bulk_store(p.merged_old_logp + dt, ob + 8 * kTS, 4 * kTS);
+                bulk_store(p.merged_mask + dt, ob + 12 * kTS, kTS);
+            }
+        }
+        if (lane == 0) bulk_commit();   // one group per tile, empty for a walked one: "two tiles ago" is then always group - 2
+        np_cur = np_next;
+        if (__any_sync(0xffffffffu, dead)) break;
+    }
+    if (lane == 0) bulk_wait<0>();
+    if (dead && lane == 0) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_INTERNAL);
+}
+}  // namespace
+
+// Per-device launch facts: the SM count and the one-time opt-in to large dynamic shared memory.  A process-wide table that
+// is written once per device (idempotent values, so a race between two first calls is benign); nothing else is kept
+// between calls.
+namespace {
+struct DevFacts {
+    int num_sms;
+    bool ready;
+};
+DevFacts g_dev[64] = {};
+size_t group_fast_smem(int n) {
+    const size_t H = (size_t)n + n / 8 + 16;
+    return (H + 2) * 4 + ((H + 3) & ~(size_t)1) * 2 + 4 * ((size_t)n + 2) * 4 + 2 * (((size_t)n + 1) & ~(size_t)1) * 2 + 16;
 }
 
-// ---------------------------------------------------------------------------------------- exact repair (M5)
-
-// Cooperative launch; every CTA returns at once unless the scatter pass saw a hash-equal, token-different pair.
-__global__ void __launch_bounds__(kSelThreads) merge_repair_kernel(const MergeParams p) {
-    __shared__ SelectSmem sm;
-    __shared__ int64_t s_w[2][2][kSelThreads / 32];
-    if (fatal(p) || p.ctrl->collision == 0) return;
-    cg::grid_group grid = cg::this_grid();
-    select_body<kSelThreads>(p, 1, sm);
-    grid.sync();
-    if (blockIdx.x == 0) compact_body<kSelThreads>(p, 1, s_w);
-    grid.sync();
-    MemberList* lists = reinterpret_cast<MemberList*>(&sm);   // the select scratch is free again
-    static_assert(sizeof(SelectSmem) >= sizeof(MemberList) * (kSelThreads / 32), "member lists fit in the select scratch");
-    if (p.mask_in) scatter_body<true>(p, 1, lists);
-    else scatter_body<false>(p, 1, lists);
+int merge_dev_facts(int* num_sms) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AJT_ERR_CUDA;
+    if (dev < 0 || dev >= 64) return AJT_ERR_UNSUPPORTED;
+    if (!g_dev[dev].ready) {
+        int sms = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) return AJT_ERR_CUDA;
+        const int grp_smem = (int)group_fast_smem(kGrpSmemN);
+        if (cudaFuncSetAttribute(merge_group_fast_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, grp_smem) != cudaSuccess)
+            return AJT_ERR_CUDA;
+        if (cudaFuncSetAttribute(merge_hash_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kHashSmem) != cudaSuccess)
+            return AJT_ERR_CUDA;
+        if (cudaFuncSetAttribute(merge_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SelectStage)) != cudaSuccess)
+            return AJT_ERR_CUDA;
+        if (cudaFuncSetAttribute(merge_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kScatSmem) != cudaSuccess)
+            return AJT_ERR_CUDA;
+        g_dev[dev].num_sms = sms;
+        g_dev[dev].ready = true;
+    }
+    *num_sms = g_dev[dev].num_sms;
+    return AJT_OK;
 }
-
 }  // namespace
 
 extern "C" size_t ajt_merge_workspace_bytes(int32_t n, int64_t n_tokens) {
     if (n < 0 || n_tokens < 0) return 0;
-    return merge_ws_layout(n, n_tokens).ent + a256(((size_t)64 * (size_t)n + 4096) * 32);
+    return merge_ws_layout(n, n_tokens).ent + 5 * 256 + a256(((size_t)64 * (size_t)n + 4096) * kEntBytes);
+}
+
+extern "C" size_t ajt_merge_workspace_bytes_for_pairs(int32_t n, int64_t n_tokens, int64_t n_pairs) {
+    if (n < 0 || n_tokens < 0 || n_pairs < 0) return 0;
+    const size_t pairs = (size_t)n_pairs > (size_t)n + 1024 ? (size_t)n_pairs : (size_t)n + 1024;
+    return merge_ws_layout(n, n_tokens).ent + 5 * 256 + a256(pairs * kEntBytes);
 }
 
 extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets, const int32_t* traj_ids,
@@ -1521,9 +1783,9 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     if (((uintptr_t)workspace & 255) || ((uintptr_t)tokens & 3)) return AJT_ERR_INVALID_ARG;
     const MergeWs ws = merge_ws_layout(n, n_tokens);
 
-    int dev = 0, num_sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return AJT_ERR_CUDA;
-    if (cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || num_sms < 1) return AJT_ERR_CUDA;
+    int num_sms = 0;
+    const int frc = merge_dev_facts(&num_sms);
+    if (frc != AJT_OK) return frc;
 
     uint8_t* b = reinterpret_cast<uint8_t*>(workspace);
     MergeParams p;
@@ -1536,18 +1798,22 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     for (int k = 0; k < 6; ++k) p.gbuf[k] = reinterpret_cast<uint32_t*>(b + ws.gbuf[k]);
     p.perm = reinterpret_cast<int32_t*>(b + ws.perm);
     p.glen = reinterpret_cast<int32_t*>(b + ws.glen);
-    p.grp_start = reinterpret_cast<int32_t*>(b + ws.grp_start);
-    p.grp_ent = reinterpret_cast<int32_t*>(b + ws.grp_ent);
+    p.goff = reinterpret_cast<int64_t*>(b + ws.goff);
     p.tl_rec = reinterpret_cast<int4*>(b + ws.tl_rec);
-    p.tl_pos = reinterpret_cast<int32_t*>(b + ws.tl_pos);
+    p.lbad = b + ws.lbad;
+    p.grp_rec = reinterpret_cast<int4*>(b + ws.grp_rec);
     p.seg_part = reinterpret_cast<uint64_t*>(b + ws.seg_part);
     p.absorbed = b + ws.absorbed;
-    p.link_bad = b + ws.link_bad;
-    p.needv = b + ws.needv;
     p.owner_tl = reinterpret_cast<int32_t*>(b + ws.owner_tl);
-    p.cand = reinterpret_cast<int32_t*>(b + ws.cand);
     p.midx = reinterpret_cast<int32_t*>(b + ws.midx);
-    p.tile_base = reinterpret_cast<int32_t*>(b + ws.tile_base);
+    for (int k = 0; k < 8; ++k) p.sel[k] = reinterpret_cast<int32_t*>(b + ws.sel[k]);
+    p.sel_q = reinterpret_cast<int2*>(b + ws.sel_q);
+    p.mem_list = reinterpret_cast<int32_t*>(b + ws.mem_list);
+    p.sv_rec = reinterpret_cast<int4*>(b + ws.sv_rec);
+    p.rseg = reinterpret_cast<int2*>(b + ws.rseg);
+    p.gseg_base = reinterpret_cast<int32_t*>(b + ws.gseg_base);
+    p.gseg = reinterpret_cast<GSeg*>(b + ws.gseg);
+    p.tile_seg = reinterpret_cast<int32_t*>(b + ws.tile_seg);
     // everything after the fixed part holds the per-key arrays; their capacity follows from the size given
     size_t eo = ws.ent;
     if (workspace_bytes < eo + 5 * 256 + ((size_t)n + 1024) * kEntBytes) return AJT_ERR_WORKSPACE_TOO_SMALL;
@@ -1559,7 +1825,9 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     p.tmp_dig = reinterpret_cast<uint32_t*>(b + eo); eo += a256((size_t)p.E_cap * 4);
     p.tmp_idx = reinterpret_cast<uint32_t*>(b + eo); eo += a256((size_t)p.E_cap * 4);
     if (eo > workspace_bytes) return AJT_ERR_WORKSPACE_TOO_SMALL;
-    p.nseg_cap = nseg_capacity(n, n_tokens);
+    const int64_t sc = slice_capacity(n, n_tokens);
+    if (sc > (int64_t)INT32_MAX) return AJT_ERR_UNSUPPORTED;
+    p.slice_cap = (int32_t)sc;
     p.mis = (int32_t)(((uintptr_t)tokens >> 2) & 3);
 
     if (n == 0) {
@@ -1568,27 +1836,19 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
         if (cudaMemsetAsync(merged_offsets, 0, sizeof(int64_t), stream) != cudaSuccess) return AJT_ERR_CUDA;
         return AJT_OK;
     }
-    // per-device launch facts (attribute opt-in, co-resident grid of the cooperative repair kernel): looked up once
-    static int s_repair_grid[64] = {0};
-    if (dev < 0 || dev >= 64) return AJT_ERR_UNSUPPORTED;
-    if (s_repair_grid[dev] == 0) {
-        if (cudaFuncSetAttribute(merge_group_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 6 * ((kGrpSmemN + 32) & ~31) * 4) !=
-            cudaSuccess)
-            return AJT_ERR_CUDA;
-        int per_sm = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, merge_repair_kernel, kSelThreads, 0) != cudaSuccess || per_sm < 1)
-            return AJT_ERR_CUDA;
-        s_repair_grid[dev] = num_sms * (per_sm < 4 ? per_sm : 4);
-    }
-    if (n <= kGrpSmemN) merge_group_small_kernel<<<1, 1024, 6 * (((size_t)n + 32) & ~(size_t)31) * 4, stream>>>(p);
-    else merge_group_kernel<false><<<1, 1024, 0, stream>>>(p);
-    merge_hash_kernel<<<num_sms * 3, 256, 0, stream>>>(p);
-    merge_select_kernel<<<num_sms * 4, kSelThreads, 0, stream>>>(p);
+#define AJT_DBG(name) do { if (getenv("AJT_DEBUG_SYNC")) { cudaError_t e_ = cudaStreamSynchronize(stream); fprintf(stderr, "[ajt] %s: %s\n", name, cudaGetErrorString(e_)); } } while (0)
+    if (n <= kGrpSmemN) merge_group_fast_kernel<<<1, 1024, group_fast_smem(n), stream>>>(p, n + n / 8 + 16);
+    else merge_group_radix_kernel<<<1, 1024, 0, stream>>>(p);
+    AJT_DBG("group");
+    merge_hash_kernel<<<num_sms * 2, kHashThreads, kHashSmem, stream>>>(p);
+    AJT_DBG("hash");
+    merge_select_kernel<<<num_sms * 4, kSelThreads, sizeof(SelectStage), stream>>>(p);
+    AJT_DBG("select");
     merge_compact_kernel<<<1, 1024, 0, stream>>>(p);
-    merge_scatter_kernel<<<num_sms * 4, kScatThreads, 0, stream>>>(p);
-    void* args[] = {(void*)&p};
-    if (cudaLaunchCooperativeKernel((const void*)merge_repair_kernel, dim3((unsigned)s_repair_grid[dev]), dim3(kSelThreads), args, 0,
-                                    stream) != cudaSuccess)
-        return AJT_ERR_CUDA;
+    const int64_t want = ((n_tokens >> kTSLog) + 1 + 255) / 256 + ((int64_t)n * 32 + 255) / 256;
+    merge_plan_kernel<<<(int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8), 256, 0, stream>>>(p);
+    AJT_DBG("plan");
+    merge_scatter_kernel<<<num_sms, kScatThreads, kScatSmem, stream>>>(p);
+    AJT_DBG("scatter");
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }
