@@ -112,6 +112,7 @@ struct MergeParams {
     int4* tl_rec;          // [n] BY SORTED POSITION: {first hash slice, group start (sorted position), rank in group, first key slot}
     uint8_t* lbad;         // [n] BY SORTED POSITION: the member differs from its in-group predecessor on that one's positions (exact)
     int4* grp_rec;         // [G+1] {group start, members, first key slot, first hash unit}
+    int2* unit_rec;        // [slice_cap] hash units {group, slice}, the largest (lowest slices) first
     uint64_t* seg_part;    // [slice_cap] per (member, slice) hash totals, then exclusive prefixes per member
     uint64_t* ent_hash;    // [E_cap] key slot (r, a), a = 0..r: in-slice partial, then the final prefix hash
     uint32_t* ent_dig;     // [E_cap] global sort path: digests / order ping-pong
@@ -135,7 +136,7 @@ struct MergeParams {
 };
 
 struct MergeWs {
-    size_t ctrl, gbuf[6], perm, glen, goff, tl_rec, lbad, grp_rec, seg_part, absorbed, owner_tl, midx, sel[8],
+    size_t ctrl, gbuf[6], perm, glen, goff, tl_rec, lbad, grp_rec, unit_rec, seg_part, absorbed, owner_tl, midx, sel[8],
         sel_q, mem_list, sv_rec, rseg, gseg_base, gseg, tile_seg, ent;
 };
 __host__ inline size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -152,6 +153,7 @@ __host__ MergeWs merge_ws_layout(int32_t n, int64_t N) {
     w.tl_rec = o; o += n16;
     w.lbad = o; o += a256((size_t)n + 2);
     w.grp_rec = o; o += n16;
+    w.unit_rec = o; o += a256(sc * 8);
     w.seg_part = o; o += a256(sc * 8);
     w.absorbed = o; o += a256((size_t)n + 2);
     w.owner_tl = o; o += n4; w.midx = o; o += n4;
@@ -352,6 +354,74 @@ __device__ __forceinline__ void group_fail(const MergeParams& p, uint32_t bits) 
     p.merged_offsets[0] = 0;
 }
 
+// Hash units in the order the hash pass takes them: slice 0 of every group, then slice 1, ... (a unit's work is the number
+// of members that reach its slice, so the longest units go first and the tail of the pass is made of short ones); slices
+// from 128 on follow group by group.  ub[g] = first unit of group g in group-major numbering (exclusive scan, ub[G] = U).
+// One CTA of 1024 threads; s_cnt / s_C: 130 words of shared scratch each.
+constexpr int kUnitRows = 128;
+__device__ __forceinline__ void emit_units(int2* unit_rec, const uint32_t* ub, int G, uint32_t* s_cnt, uint32_t* s_C) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int w = tid; w <= kUnitRows + 1; w += 1024) { s_cnt[w] = 0; s_C[w] = 0; }
+    __syncthreads();
+    for (int g = tid; g < G; g += 1024) {
+        const uint32_t un = ub[g + 1] - ub[g];
+        if (un) atomicAdd(&s_cnt[min(un, (uint32_t)kUnitRows)], 1u);   // histogram of units per group, capped
+        if (un > (uint32_t)kUnitRows) s_cnt[kUnitRows + 1] = 1;        // some group has slices beyond the rows
+    }
+    __syncthreads();
+    if (warp == 0) {   // row w holds the groups with more than w units: suffix sums of the histogram, then their running total
+        uint32_t h[4], c[4], sfx = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) h[j] = s_cnt[4 * lane + j + 1];   // groups with exactly 4 lane + j + 1 units
+#pragma unroll
+        for (int j = 3; j >= 0; --j) { sfx += h[j]; c[j] = sfx; }      // within the lane
+        uint32_t inc = sfx;                                            // + the lanes above
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_down_sync(0xffffffffu, inc, o);
+            if (lane + o < 32) inc += t;
+        }
+        const uint32_t above = inc - sfx;
+        uint32_t rowsum = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { c[j] += above; rowsum += c[j]; }   // c[j] = groups with more than 4 lane + j units
+        uint32_t pre = rowsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, pre, o);
+            if (lane >= o) pre += t;
+        }
+        uint32_t run = pre - rowsum;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { s_C[4 * lane + j] = run; run += c[j]; }
+        if (lane == 31) s_C[kUnitRows] = run;
+    }
+    __syncthreads();
+    for (int w = warp; w < kUnitRows; w += 32) {
+        const uint32_t base = s_C[w];
+        if (s_C[w + 1] == base) break;   // no group has more than w units, nor any later row
+        uint32_t run = 0;
+        for (int g0 = 0; g0 < G; g0 += 32) {
+            const int g = g0 + lane;
+            const bool has = g < G && ub[g + 1] - ub[g] > (uint32_t)w;
+            const unsigned bal = __ballot_sync(0xffffffffu, has);
+            if (has) unit_rec[base + run + __popc(bal & ((1u << lane) - 1u))] = make_int2(g, w);
+            run += __popc(bal);
+        }
+    }
+    // slices from kUnitRows on (timelines beyond 64k tokens): group-major after the rows; one warp, running offset
+    if (warp == 0 && s_cnt[kUnitRows + 1]) {
+        uint32_t run = s_C[kUnitRows];
+        for (int g = 0; g < G; ++g) {
+            const uint32_t un = ub[g + 1] - ub[g];
+            if (un > (uint32_t)kUnitRows) {
+                for (uint32_t x = kUnitRows + lane; x < un; x += 32) unit_rec[run + x - kUnitRows] = make_int2(g, (int)x);
+                run += un - kUnitRows;
+            }
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------- K1: group (M1)
 
 constexpr uint32_t kEmpty = 0xFFFFFFFFu;
@@ -381,6 +451,7 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
     extern __shared__ __align__(16) uint8_t g_dyn[];
     __shared__ int64_t s_w[2][2][32];
     __shared__ uint32_t s_bad, s_ng;
+    __shared__ uint32_t s_cnt[kUnitRows + 2], s_C[kUnitRows + 2];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = p.n;
     uint32_t* const B1 = reinterpret_cast<uint32_t*>(g_dyn);
     uint16_t* const B2 = reinterpret_cast<uint16_t*>(B1 + (H + 2));
@@ -563,6 +634,7 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
 #pragma unroll 1
     for (int g = tid; g <= G; g += 1024)
         p.grp_rec[g] = make_int4((int)B1[g], g < G ? (int)(B1[g + 1] - B1[g]) : 0, (int)B4[g], (int)B5[g]);
+    emit_units(p.unit_rec, B5, G, s_cnt, s_C);
     if (tid == 0) {
         p.ctrl->n_groups = G;
         p.ctrl->n_entries = (int32_t)E;
@@ -578,6 +650,7 @@ __global__ void __launch_bounds__(1024) merge_group_radix_kernel(const MergePara
     __shared__ int64_t s_w[2][2][32];
     __shared__ int s_min, s_max;
     __shared__ uint32_t s_bad;
+    __shared__ uint32_t s_cnt[kUnitRows + 2], s_C[kUnitRows + 2];
     const int tid = threadIdx.x, n = p.n;
     uint32_t* kb[2] = {p.gbuf[0], p.gbuf[1]};
     uint32_t* vb[2] = {p.gbuf[2], p.gbuf[3]};
@@ -674,6 +747,8 @@ __global__ void __launch_bounds__(1024) merge_group_radix_kernel(const MergePara
     }
     for (int g = tid; g <= G; g += 1024)
         p.grp_rec[g] = make_int4((int)gsv[g], g < G ? (int)(gsv[g + 1] - gsv[g]) : 0, (int)gent[g], (int)gun[g]);
+    __syncthreads();
+    emit_units(p.unit_rec, gun, G, s_cnt, s_C);
     if (tid == 0) {
         p.ctrl->n_groups = G;
         p.ctrl->n_entries = (int32_t)E;
@@ -745,16 +820,18 @@ constexpr int kHashWarpBytes = kHashStages * kStageBytes + 128;     // + 4 mbarr
 constexpr int kHashSmem = (kHashThreads / 32) * kHashWarpBytes + 128;
 
 // Warp per hash unit = (group, slice of 512 positions).  Lane l holds positions S0 + l + 32 t (t < 16) of EVERY member: a
-// member's slice arrives as ONE bulk async copy (TMA, 1-D) of the 16-byte-aligned superset of its bytes, issued by one lane
-// and counted on a warp-private mbarrier, and is read with conflict-free 32-bit shared-memory loads at the member's own
-// misalignment.  So the weights are per unit, and member r is compared with member r - 1 register against register.
+// member's slice arrives as ONE bulk async copy (TMA, 1-D) of the 16-byte-aligned superset of its bytes, launched by the
+// lane that holds the member's facts and counted on a warp-private mbarrier, and is read with conflict-free 32-bit
+// shared-memory loads at the member's own misalignment.  So the weights are per unit, and member r is compared with member
+// r - 1 stage against stage (a stage is refilled two members behind).  The kernel is bound by instruction issue (~200 per
+// member-slice), not by memory: everything per member that can be computed 32 members at a time is.
 __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const MergeParams p) {
     extern __shared__ __align__(128) uint8_t h_dyn[];
     if (fatal(p)) return;
     const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
     uint8_t* const wbuf = reinterpret_cast<uint8_t*>(((uintptr_t)h_dyn + 127) & ~(uintptr_t)127) + (size_t)wic * kHashWarpBytes;
     uint64_t* const full = reinterpret_cast<uint64_t*>(wbuf + kHashStages * kStageBytes);
-    int4* const desc = reinterpret_cast<int4*>(wbuf + kHashStages * kStageBytes + 64);
+    const uint32_t sdesc = smem_u32(wbuf + kHashStages * kStageBytes + 64);
     const uint32_t sbuf = smem_u32(wbuf);
     if (lane == 0) {
 #pragma unroll
@@ -763,20 +840,28 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
     }
     __syncwarp();
     uint32_t phases = 0;   // bit s: the parity stage s completes next
-    const int U = p.ctrl->n_units, G = p.ctrl->n_groups;
+#ifdef AJT_PROF
+    long long c_wait = 0, c_setup = 0, c_keys = 0, c_issue = 0; const long long c_begin = clock64();
+#define HP(x) x
+#else
+#define HP(x)
+#endif
+    const int U = p.ctrl->n_units;
     const int32_t* __restrict__ tokens = p.tokens;
     const int64_t N = p.N;
     const int mis = p.mis;
     const uint32_t lw = c_w1.v[lane] * kW3;   // W^(lane + 3)
+    bool dead = false;
     int next = 0;
     if (lane == 0) next = atomicAdd(&p.ctrl->unit_ticket, 1);
     next = __shfl_sync(0xffffffffu, next, 0);
     while (next < U) {
         const int u = next;
+        HP(const long long c_u0 = clock64();)
         if (lane == 0) next = atomicAdd(&p.ctrl->unit_ticket, 1);   // needed only after this unit: the round trip is hidden
-        const int g = warp_search_last_le(G, u, [&](int x) { return __ldg(reinterpret_cast<const int32_t*>(p.grp_rec + x) + 3); });
-        const int4 gr = __ldg(p.grp_rec + g);
-        const int gs = gr.x, k = gr.y, w = u - gr.w;
+        const int2 ur = __ldg(p.unit_rec + u);                      // {group, slice}: largest units first
+        const int4 gr = __ldg(p.grp_rec + ur.x);
+        const int gs = gr.x, k = gr.y, w = ur.y;
         const int64_t eb = gr.z;
         const int S0 = w << kSlLog;                 // first position of the slice
         const int32_t* __restrict__ gln = p.glen + gs;
@@ -786,69 +871,82 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
         wt[0] = (w < 128 ? c_w512.v[w] : pow32(kW512, (uint32_t)w)) * lw;
 #pragma unroll
         for (int t = 1; t < 16; ++t) wt[t] = wt[t - 1] * kW32;
-        // members of the first 32 ranks whose last token lies in this slice (keys are emitted only where a prefix ends)
-        const int L0 = lane < k ? __ldg(gln + lane) : 0;
-        bool anyend = __any_sync(0xffffffffu, L0 > 0 && ((L0 - 1) >> kSlLog) == w);
-        for (int a0 = 32; a0 < k && !anyend; a0 += 32) {
-            const int La = a0 + lane < k ? __ldg(gln + a0 + lane) : 0;
-            anyend = __any_sync(0xffffffffu, La > 0 && ((La - 1) >> kSlLog) == w);
-        }
-        // ---- issue side: walks the members that reach this slice, 32 ranks at a time
-        int ic0 = 0, iL = L0, isb = lane < k ? __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + lane)) : 0;
-        int64_t ioff = lane < k ? __ldg(gof + lane) : 0;
-        unsigned ireach = __ballot_sync(0xffffffffu, iL > S0);
+        // ---- the members, 32 ranks at a time; each lane works out its own member's copy once
+        int ic0 = 0, iL = 0, isb = 0, iD = 0, inv = 0;
+        int64_t ig0 = 0;
+        unsigned ireach = 0, iedge = 0;
+        auto load_chunk = [&]() {
+            const bool v = ic0 + lane < k;
+            iL = v ? __ldg(gln + ic0 + lane) : 0;
+            const int64_t off = v ? __ldg(gof + ic0 + lane) : 0;
+            isb = v ? __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + ic0 + lane)) : 0;
+            iD = (int)((off + mis) & 3);                    // slot of position S0 in the 16-byte grid
+            ig0 = off + S0 - iD;                             // element index of the first aligned vector
+            inv = (min(iL - S0, kSl) + iD + 3) >> 2;         // vectors holding positions < min(L, S0 + 512)
+            ireach = __ballot_sync(0xffffffffu, iL > S0);
+            iedge = __ballot_sync(0xffffffffu, iL > S0 && !(ig0 >= 0 && ig0 + 4 * (int64_t)inv <= N));
+        };
+        load_chunk();
+        const int L0 = iL;   // lengths of the first 32 ranks: where prefixes end
+        const unsigned end0 = __ballot_sync(0xffffffffu, L0 > 0 && ((L0 - 1) >> kSlLog) == w);
         bool more = true;
-        auto issue_next = [&](int stage) {
-            if (!more) return false;
+        int issued = 0, consumed = 0;
+        // launches the next member's copy into stage `issued & 3` (if there is one)
+        auto issue_next = [&]() {
             while (ireach == 0) {
+                if (!more) return;
                 ic0 += 32;
-                if (ic0 >= k) { more = false; return false; }
-                const bool v = ic0 + lane < k;
-                iL = v ? __ldg(gln + ic0 + lane) : 0;
-                ioff = v ? __ldg(gof + ic0 + lane) : 0;
-                isb = v ? __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + ic0 + lane)) : 0;
-                ireach = __ballot_sync(0xffffffffu, iL > S0);
+                if (ic0 >= k) { more = false; return; }
+                load_chunk();
             }
             const int b = __ffs(ireach) - 1;
             ireach &= ireach - 1;
-            const int Lr = __shfl_sync(0xffffffffu, iL, b);
-            const int64_t off = shfl_i64(ioff, b);
-            const int D = (int)((off + mis) & 3);            // slot of position S0 in the 16-byte grid
-            const int64_t g0 = off + S0 - D;                 // element index of the first aligned vector
-            const int nv = (min(Lr - S0, kSl) + D + 3) >> 2; // vectors holding positions < min(L_r, S0 + 512)
-            const uint32_t sdst = sbuf + stage * kStageBytes;
-            const bool inside = g0 >= 0 && g0 + 4 * (int64_t)nv <= N;
-            if (!inside) {   // first / last vectors of the token array: element-wise, inside the array only
+            const int stage = issued & (kHashStages - 1);
+            if ((iedge >> b) & 1u) {   // first / last vectors of the token array: element-wise, inside the array only
+                const int64_t g0 = shfl_i64(ig0, b);
+                const int nv = __shfl_sync(0xffffffffu, inv, b);
                 for (int e = lane; e < 4 * nv; e += 32) {
                     const int64_t gi = g0 + e;
-                    sts32(sdst + 4 * e, gi >= 0 && gi < N ? (uint32_t)tokens[gi] : 0u);
+                    sts32(sbuf + stage * kStageBytes + 4 * e, gi >= 0 && gi < N ? (uint32_t)tokens[gi] : 0u);
                 }
                 __syncwarp();
             }
-            if (lane == b) {   // the member's own lane launches its copy; the descriptor is published by the barrier
-                desc[stage] = make_int4(ic0 + b, iL, isb, D);
-                if (inside) {
-                    mbar_arrive_expect_tx(&full[stage], 16u * (uint32_t)nv);
-                    bulk_load(wbuf + stage * kStageBytes, tokens + g0, 16u * (uint32_t)nv, &full[stage]);
-                } else {
+            if (lane == b) {   // the descriptor is published by the barrier's release / acquire
+                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(sdesc + 16 * stage), "r"(ic0 + b), "r"(iL), "r"(isb), "r"(iD) : "memory");
+                if ((iedge >> b) & 1u) {
                     mbar_arrive(&full[stage]);
+                } else {
+                    mbar_arrive_expect_tx(&full[stage], 16u * (uint32_t)inv);
+                    bulk_load(wbuf + stage * kStageBytes, tokens + ig0, 16u * (uint32_t)inv, &full[stage]);
                 }
             }
-            return true;
+            ++issued;
         };
-        // ---- consume side: two register images of a slice alternate (the member and its predecessor)
-        int prev_r = -2, prev_L = 0;
-        int issued = 0, consumed = 0;
-        bool dead = false;
+        bool end_hi = false;   // does a member of rank >= 32 end in this slice?  (groups of more than 32 only)
+        for (int a0 = 32; a0 < k && !end_hi; a0 += 32) {
+            const int La = a0 + lane < k ? __ldg(gln + a0 + lane) : 0;
+            end_hi = __any_sync(0xffffffffu, La > 0 && ((La - 1) >> kSlLog) == w);
+        }
+        int prev_r = -2, prev_L = 0, prev_D = 0;
         uint64_t Fk = 0;        // lane a: the partial of the prefix ending at member a's last token, for the latest member
         unsigned fvalid = 0;    // ranks whose Fk belongs to the latest member
-        auto consume = [&](uint32_t (&x)[16], const uint32_t (&pv)[16]) {
+        issue_next();
+        issue_next();           // two members ahead: the predecessor's stage stays intact while a member is compared with it
+        HP(c_setup += clock64() - c_u0;)
+#pragma unroll 1
+        while (consumed < issued) {
+            HP(const long long c_i0 = clock64();)
+            issue_next();
+            HP(c_issue += clock64() - c_i0;)
             const int st = consumed & (kHashStages - 1);
+            HP(const long long c_w0 = clock64();)
             if (!mbar_wait_bounded(&full[st], (phases >> st) & 1u)) dead = true;   // never in practice: a lost copy must not hang the GPU
+            HP(c_wait += clock64() - c_w0;)
             phases ^= 1u << st;
-            const int4 d = desc[st];
-            const int r = d.x, Lr = d.y;
-            const uint32_t a0 = sbuf + st * kStageBytes + 4 * (d.w + lane);
+            int r, Lr, sbr, D;
+            asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r), "=r"(Lr), "=r"(sbr), "=r"(D) : "r"(sdesc + 16 * st));
+            const uint32_t a0 = sbuf + st * kStageBytes + 4 * (D + lane);
+            uint32_t x[16];
 #pragma unroll
             for (int t = 0; t < 16; ++t) x[t] = lds32(a0 + 128 * t);
             if (Lr < S0 + kSl) {   // the member ends in this slice: nothing beyond its last token
@@ -857,88 +955,96 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
                 for (int t = 0; t < 16; ++t)
                     if (32 * t >= rem) x[t] = 0;
             }
-            uint64_t ac[4];
+            uint64_t ac0 = (uint64_t)x[0] * wt[0], ac1 = (uint64_t)x[1] * wt[1];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                ac[j] = (uint64_t)x[j] * wt[j];
-#pragma unroll
-                for (int t = j + 4; t < 16; t += 4) ac[j] = mad_wide(x[t], wt[t], ac[j]);
+            for (int t = 2; t < 16; t += 2) {
+                ac0 = mad_wide(x[t], wt[t], ac0);
+                ac1 = mad_wide(x[t + 1], wt[t + 1], ac1);
             }
             // exact comparison with the in-group predecessor on its positions (M5, first half)
             bool same = false;   // the two agree on every position of the slice below prev_L
             if (prev_r == r - 1) {
                 uint32_t diff = 0;
+                const uint32_t pa0 = sbuf + ((consumed - 1) & (kHashStages - 1)) * kStageBytes + 4 * (prev_D + lane);
                 if (prev_L >= S0 + kSl) {
 #pragma unroll
-                    for (int t = 0; t < 16; ++t) diff |= x[t] ^ pv[t];
+                    for (int t = 0; t < 16; ++t) diff |= x[t] ^ lds32(pa0 + 128 * t);
                 } else {
                     const int rem = prev_L - S0 - lane;
 #pragma unroll
                     for (int t = 0; t < 16; ++t)
-                        if (32 * t < rem) diff |= x[t] ^ pv[t];
+                        if (32 * t < rem) diff |= x[t] ^ lds32(pa0 + 128 * t);
                 }
                 same = !__any_sync(0xffffffffu, diff != 0);
                 if (!same && lane == 0) p.lbad[gs + r] = 1;
             }
-            const uint64_t tot = warp_sum_u64_redux((ac[0] + ac[1]) + (ac[2] + ac[3]));
-            if (lane == 0) p.seg_part[d.z + w] = tot;
+            const uint64_t tot = warp_sum_u64_redux(ac0 + ac1);
+            if (lane == 0) p.seg_part[sbr + w] = tot;
             // keys: the prefixes (L_a of an earlier member, or L_r itself) that end inside this slice
-            if (anyend) {
-                if (!same) fvalid = 0;
-                for (int a0r = 0; a0r <= r; a0r += 32) {
+            HP(const long long c_k0 = clock64();)
+            if (!same) fvalid = 0;
+            unsigned m0 = end0 & (r >= 31 ? 0xffffffffu : (2u << r) - 1u);
+            if (m0) m0 &= __ballot_sync(0xffffffffu, L0 <= Lr);
+            for (; m0; m0 &= m0 - 1) {
+                const int b = __ffs(m0) - 1;
+                const int Lb = __shfl_sync(0xffffffffu, L0, b);
+                uint64_t F;
+                if (((fvalid >> b) & 1u) && Lb <= prev_L) {
+                    F = (uint64_t)shfl_i64((int64_t)Fk, b);   // member r - 1 has the same tokens up to there
+                } else {
+                    if (b == r) {
+                        F = tot;   // its own last token: everything beyond is zero already
+                    } else {
+                        const int rem = Lb - S0 - lane;   // tokens 32 t < rem are inside the prefix
+                        uint64_t part = 0;
+#pragma unroll
+                        for (int t = 0; t < 16; ++t)
+                            if (32 * t < rem) part = mad_wide(x[t], wt[t], part);
+                        F = warp_sum_u64_redux(part);
+                    }
+                    if (lane == b) Fk = F;
+                    fvalid |= 1u << b;
+                }
+                if (lane == 0) p.ent_hash[eb + (int64_t)r * (r + 1) / 2 + b] = F;
+            }
+            if (end_hi && r >= 32) {   // groups of more than 32: ends of ranks >= 32, no caching
+                for (int a0r = 32; a0r <= r; a0r += 32) {
                     const int a = a0r + lane;
-                    const int La = a0r == 0 ? L0 : (a < k ? __ldg(gln + a) : 0);
+                    const int La = a < k ? __ldg(gln + a) : 0;
                     const bool hit = a <= r && La > 0 && La <= Lr && ((La - 1) >> kSlLog) == w;
                     for (unsigned m = __ballot_sync(0xffffffffu, hit); m; m &= m - 1) {
                         const int b = __ffs(m) - 1;
-                        const int Lb = __shfl_sync(0xffffffffu, La, b);
-                        uint64_t F;
-                        if (a0r == 0 && ((fvalid >> b) & 1u) && Lb <= prev_L) {
-                            F = (uint64_t)shfl_i64((int64_t)Fk, b);   // member r - 1 has the same tokens up to there
-                        } else {
-                            if (a0r + b == r) {
-                                F = tot;   // its own last token: everything beyond is zero already
-                            } else {
-                                const int rem = Lb - S0 - lane;   // tokens 32 t < rem are inside the prefix
-                                uint64_t part = 0;
+                        const int rem = __shfl_sync(0xffffffffu, La, b) - S0 - lane;
+                        uint64_t part = 0;
 #pragma unroll
-                                for (int t = 0; t < 16; ++t)
-                                    if (32 * t < rem) part = mad_wide(x[t], wt[t], part);
-                                F = warp_sum_u64_redux(part);
-                            }
-                            if (a0r == 0) {
-                                if (lane == b) Fk = F;
-                                fvalid |= 1u << b;
-                            }
-                        }
+                        for (int t = 0; t < 16; ++t)
+                            if (32 * t < rem) part = mad_wide(x[t], wt[t], part);
+                        const uint64_t F = warp_sum_u64_redux(part);
                         if (lane == 0) p.ent_hash[eb + (int64_t)r * (r + 1) / 2 + a0r + b] = F;
                     }
                 }
             }
+            HP(c_keys += clock64() - c_k0;)
             prev_r = r;
             prev_L = Lr;
+            prev_D = D;
             ++consumed;
-            __syncwarp();   // every lane is done with the stage before the next issue refills it
-        };
-        uint32_t xa[16], xb[16];
-#pragma unroll 1
-        for (int s = 0; s < kHashStages - 1; ++s)
-            if (issue_next(issued & (kHashStages - 1))) ++issued;
-#pragma unroll 1
-        while (consumed < issued) {
-            if (issue_next(issued & (kHashStages - 1))) ++issued;
-            consume(xa, xb);
-            if (consumed < issued) {
-                if (issue_next(issued & (kHashStages - 1))) ++issued;
-                consume(xb, xa);
-            }
+            __syncwarp();   // every lane is done with the stage before a later issue refills it
         }
         next = __shfl_sync(0xffffffffu, next, 0);
-        if (__any_sync(0xffffffffu, dead)) {
-            if (lane == 0) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_INTERNAL);
-            break;
-        }
+        if (__any_sync(0xffffffffu, dead)) break;
     }
+#ifdef AJT_PROF
+    if (lane == 0) {
+        unsigned long long* r = reinterpret_cast<unsigned long long*>(p.ctrl->reserved) + 16;
+        atomicAdd(r + 0, (unsigned long long)(clock64() - c_begin));
+        atomicAdd(r + 1, (unsigned long long)c_wait);
+        atomicAdd(r + 2, (unsigned long long)c_setup);
+        atomicAdd(r + 3, (unsigned long long)c_keys);
+        atomicAdd(r + 4, (unsigned long long)c_issue);
+    }
+#endif
+    if (dead && lane == 0) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_INTERNAL);
 }
 
 // ---------------------------------------------------------------------------------------- K3: keys, sort, select, verify, segments, compact (M2-M6)
@@ -1802,6 +1908,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     p.tl_rec = reinterpret_cast<int4*>(b + ws.tl_rec);
     p.lbad = b + ws.lbad;
     p.grp_rec = reinterpret_cast<int4*>(b + ws.grp_rec);
+    p.unit_rec = reinterpret_cast<int2*>(b + ws.unit_rec);
     p.seg_part = reinterpret_cast<uint64_t*>(b + ws.seg_part);
     p.absorbed = b + ws.absorbed;
     p.owner_tl = reinterpret_cast<int32_t*>(b + ws.owner_tl);
