@@ -1167,55 +1167,120 @@ __device__ __noinline__ int build_segments(bool explicit_masks, const int32_t* m
 }
 
 // M6.  One CTA, one fused scan over the timelines (original order): survivors -> merged index, offsets, origin, traj, first
-// global segment; then owner[].  A lone CTA pays ~0.8 us per dependent global round trip, so every load of the scan is
-// issued up front (8 timelines per thread, nothing conditional) and the owner gather runs 8 deep: three round trips in all.
+// global segment; then owner[].  A lone SM pays ~1-2 us per dependent global round trip and handles only so many memory
+// sectors per cycle, so every global access is coalesced (lane = consecutive timeline) and issued 8 deep, and the scan --
+// which wants 8 CONSECUTIVE timelines per thread -- runs on a copy in shared memory.  Two round trips in all.
+constexpr int kCompactChunk = 8192;
+constexpr int kCompactSmem = kCompactChunk * 16 + kCompactChunk * 4;
 __global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p) {
-    __shared__ int64_t s_w[2][2][32];
+    extern __shared__ __align__(16) uint8_t c_dyn[];
+    __shared__ int64_t s_wa[32], s_wb[32];
     if (fatal(p)) return;
     constexpr int NT = 1024;
-    const int tid = threadIdx.x, n = p.n;
-    int32_t tr[8];
-    const I2 tot = block_scan2<NT, 8>(
-        n,
-        [&](int i) {   // (a survivor's record is garbage for an absorbed timeline: unused)
-            const bool ab = __ldg(p.absorbed + i) != 0;
-            const int64_t L = __ldg(p.offsets + i + 1) - __ldg(p.offsets + i);
-            const int64_t ns = __ldg(reinterpret_cast<const int32_t*>(p.sv_rec + i) + 3);
-            tr[i & 7] = __ldg(p.traj_ids + i);
-            return ab ? I2{0, 0} : I2{((int64_t)1 << 32) | (ns & 0xffffffff), L};
-        },
-        [&](int i, int64_t exa, int64_t exb, int64_t va, int64_t) {
-            if (!va) { p.midx[i] = -1; return; }
-            const int m = (int)(exa >> 32);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = p.n;
+    uint2* const prA = reinterpret_cast<uint2*>(c_dyn);                         // in: {survivor << 24 | segments, length}; out: {merged index, first segment}
+    int64_t* const prB = reinterpret_cast<int64_t*>(c_dyn + kCompactChunk * 8);  // out: merged offset
+    int32_t* const smidx = reinterpret_cast<int32_t*>(c_dyn + kCompactChunk * 16);   // merged index by timeline (n <= chunk)
+    const bool one = n <= kCompactChunk;
+    int64_t base_a = 0, base_b = 0;   // {survivors << 32 | segments}, tokens, before this chunk
+    for (int c0 = 0; c0 < n; c0 += kCompactChunk) {
+        const int cn = min(kCompactChunk, n - c0);
+        int32_t tr[8];
+        uint32_t sv[8];
+        // ---- A: coalesced loads, 8 timelines per thread in flight
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int j = u * NT + tid, i = c0 + j;
+            uint2 v = make_uint2(0u, 0u);
+            tr[u] = 0;
+            if (j < cn) {
+                const bool ab = __ldg(p.absorbed + i) != 0;
+                const int64_t L = __ldg(p.offsets + i + 1) - __ldg(p.offsets + i);
+                const uint32_t ns = (uint32_t)__ldg(reinterpret_cast<const int32_t*>(p.sv_rec + i) + 3);   // (garbage if absorbed: unused)
+                tr[u] = __ldg(p.traj_ids + i);
+                if (!ab) v = make_uint2((1u << 24) | (ns & 0xffffffu), (uint32_t)L);
+            }
+            sv[u] = v.x;
+            prA[j] = v;
+        }
+        __syncthreads();
+        // ---- B: thread t scans timelines 8 t .. 8 t + 7 of the chunk
+        uint2 it[8];
+        int64_t sa = 0, sb = 0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            it[q] = prA[8 * tid + q];
+            sa += ((int64_t)(it[q].x >> 24) << 32) | (it[q].x & 0xffffffu);
+            sb += it[q].y;
+        }
+        int64_t ia = sa, ib = sb;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int64_t ta = __shfl_up_sync(0xffffffffu, ia, o), tb = __shfl_up_sync(0xffffffffu, ib, o);
+            if (lane >= o) { ia += ta; ib += tb; }
+        }
+        if (lane == 31) { s_wa[warp] = ia; s_wb[warp] = ib; }
+        __syncthreads();
+        int64_t wa = s_wa[lane], wb = s_wb[lane], ja = wa, jb = wb;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int64_t ta = __shfl_up_sync(0xffffffffu, ja, o), tb = __shfl_up_sync(0xffffffffu, jb, o);
+            if (lane >= o) { ja += ta; jb += tb; }
+        }
+        int64_t ra = base_a + __shfl_sync(0xffffffffu, ja - wa, warp) + ia - sa;
+        int64_t rb = base_b + __shfl_sync(0xffffffffu, jb - wb, warp) + ib - sb;
+        const int64_t ta = __shfl_sync(0xffffffffu, ja, 31), tb = __shfl_sync(0xffffffffu, jb, 31);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            prA[8 * tid + q] = make_uint2((uint32_t)(ra >> 32), (uint32_t)(ra & 0xffffffff));
+            prB[8 * tid + q] = rb;
+            ra += ((int64_t)(it[q].x >> 24) << 32) | (it[q].x & 0xffffffu);
+            rb += it[q].y;
+        }
+        base_a += ta;
+        base_b += tb;
+        __syncthreads();
+        // ---- C: coalesced outputs
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int j = u * NT + tid, i = c0 + j;
+            if (j >= cn) break;
+            int32_t m = -1;
+            if (sv[u]) {
+                const uint2 e = prA[j];
+                m = (int32_t)e.x;
+                p.merged_origin[m] = i;
+                p.merged_traj[m] = tr[u];
+                p.merged_offsets[m] = prB[j];
+                p.gseg_base[m] = (int32_t)e.y;
+            }
             p.midx[i] = m;
-            p.merged_origin[m] = i;
-            p.merged_traj[m] = tr[i & 7];
-            p.merged_offsets[m] = exb;
-            p.gseg_base[m] = (int32_t)(exa & 0xffffffff);
-        },
-        s_w);
-    const int M = (int)(tot.a >> 32);
-    const int32_t nseg = (int32_t)(tot.a & 0xffffffff);
+            if (one) smidx[i] = m;
+        }
+        __syncthreads();
+    }
+    const int M = (int)(base_a >> 32);
+    const int32_t nseg = (int32_t)(base_a & 0xffffffff);
 #pragma unroll 1
     for (int i0 = tid; i0 < n; i0 += 8 * NT) {
         int32_t o[8];
 #pragma unroll
         for (int u = 0; u < 8; ++u) o[u] = i0 + u * NT < n ? __ldg(p.owner_tl + i0 + u * NT) : 0;
 #pragma unroll
-        for (int u = 0; u < 8; ++u) o[u] = p.midx[o[u]];
+        for (int u = 0; u < 8; ++u) o[u] = one ? smidx[o[u]] : p.midx[o[u]];
 #pragma unroll
         for (int u = 0; u < 8; ++u)
             if (i0 + u * NT < n) p.owner[i0 + u * NT] = o[u];
     }
     if (tid == 0) {
-        p.merged_offsets[M] = tot.b;
+        p.merged_offsets[M] = base_b;
         p.gseg_base[M] = nseg;
         p.counts[0] = M;
-        p.counts[1] = tot.b;
+        p.counts[1] = base_b;
         p.ctrl->M = M;
-        p.ctrl->N_out = tot.b;
+        p.ctrl->N_out = base_b;
         p.ctrl->n_gsegs = nseg;
-        p.ctrl->n_tiles = (int32_t)((tot.b + kTS - 1) >> kTSLog);
+        p.ctrl->n_tiles = (int32_t)((base_b + kTS - 1) >> kTSLog);
     }
 }
 
@@ -1853,6 +1918,8 @@ int merge_dev_facts(int* num_sms) {
             return AJT_ERR_CUDA;
         if (cudaFuncSetAttribute(merge_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kScatSmem) != cudaSuccess)
             return AJT_ERR_CUDA;
+        if (cudaFuncSetAttribute(merge_compact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCompactSmem) != cudaSuccess)
+            return AJT_ERR_CUDA;
         g_dev[dev].num_sms = sms;
         g_dev[dev].ready = true;
     }
@@ -1951,7 +2018,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     AJT_DBG("hash");
     merge_select_kernel<<<num_sms * 4, kSelThreads, sizeof(SelectStage), stream>>>(p);
     AJT_DBG("select");
-    merge_compact_kernel<<<1, 1024, 0, stream>>>(p);
+    merge_compact_kernel<<<1, 1024, kCompactSmem, stream>>>(p);
     const int64_t want = ((n_tokens >> kTSLog) + 1 + 255) / 256 + ((int64_t)n * 32 + 255) / 256;
     merge_plan_kernel<<<(int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8), 256, 0, stream>>>(p);
     AJT_DBG("plan");
