@@ -59,12 +59,7 @@ enum {
 
 enum { AJT_DT_BF16 = 0, AJT_DT_F32 = 1 };
 
-/* ajt_merge_timelines `flags` */
-enum {
-    AJT_MERGE_WEAK_HASH = 1 /* test hook: degrade the prefix hash to 4 bits so that hash-equal,
-                               token-different candidates are common and the exact comparison that
-                               guards every accepted candidate is exercised.  Results are still exact. */
-};
+/* ajt_merge_timelines `flags`: 0 (include/ajt_test.h defines a test hook). */
 
 /* Device status bits (ajt_last_status). */
 enum {
@@ -176,7 +171,10 @@ int ajt_merge_blocks(
     void* workspace, size_t workspace_bytes, ajt_stream_t stream);
 
 /* HOST-buffer variant: same arguments but every array pointer is HOST memory (pinned for speed).
- * `arena` is DEVICE scratch of at least ajt_merge_host_arena_bytes(n, n_tokens) bytes.  Synchronises. */
+ * `arena` is DEVICE scratch of at least ajt_merge_host_arena_bytes(n, n_tokens) bytes; whatever it holds beyond that goes
+ * to the candidate pairs (ajt_merge_workspace_bytes_for_pairs(n, n_tokens, n_pairs) - ajt_merge_workspace_bytes(n, n_tokens)
+ * more bytes hold n_pairs).  Synchronises.  A fatal status is an error of this call: AJT_ERR_CAPACITY for
+ * AJT_STATUS_PROBE_CAPACITY, AJT_ERR_INVALID_ARG for bad offsets / zero-length timelines (status_bits is still filled). */
 size_t ajt_merge_host_arena_bytes(int32_t n, int64_t n_tokens);
 
 int ajt_merge_timelines_host(
@@ -310,9 +308,27 @@ int ajt_segment_counts(const uint8_t* mask /* DEVICE [T] */, const int32_t* seg_
  * The per-token vectors go up first and the batch-wide normalisers are counted on the device; the matrix is cut into up
  * to 16 row slabs whose H2D copy, loss call and D2H copy overlap with their neighbours' (both PCIe directions busy at
  * once); rows with mask 0 are not copied up, since the kernel never reads them.  For that the call creates two helper streams and their events and destroys them before it returns: the only
- * resources the library ever creates.  dlogits / logp rows are those of the device call; loss and stats[3] are the fp64
+ * resources the library ever creates (ajt_policy_loss_fwd_bwd_host2 takes them from a caller-owned context instead).  dlogits / logp rows are those of the device call; loss and stats[3] are the fp64
  * sums of the slabs' fp32 partials.  Pinned host buffers are needed for the overlap.  Synchronises. */
 size_t ajt_loss_host_arena_bytes(int64_t T, int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype);
+
+/* Helper streams and events of the slab pipeline, created once and reused across calls (ajt_policy_loss_fwd_bwd_host2);
+ * the only resources the library ever creates.  One context serves one call at a time. */
+typedef struct ajt_host_ctx* ajt_host_ctx_t;
+int ajt_host_ctx_create(ajt_host_ctx_t* ctx);
+void ajt_host_ctx_destroy(ajt_host_ctx_t ctx);
+
+/* ajt_policy_loss_fwd_bwd_host with two more choices: `dlogits_on_device` != 0 makes `dlogits` a DEVICE buffer
+ * [T, ld_logits] bf16 (16-byte aligned) that receives the gradient, so that nothing but loss / logp / stats / status comes
+ * back over PCIe (what a trainer wants: the backward pass continues on the device); `ctx` (or NULL: created and destroyed
+ * inside the call) carries the helper streams.  Everything else as for ajt_policy_loss_fwd_bwd_host. */
+int ajt_policy_loss_fwd_bwd_host2(
+    const void* logits, const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
+    const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T, int32_t V, int32_t S, int64_t ld_logits,
+    int32_t logits_dtype, const float* seg_denom, float inv_num_segs, float grad_scale,
+    void* dlogits, int32_t dlogits_on_device, float* loss_out /* HOST [1] */, float* logp_out /* HOST [T] or NULL */,
+    float* stats_out /* HOST [4] or NULL */, uint32_t* status_bits /* HOST [1] or NULL */,
+    ajt_host_ctx_t ctx, void* arena /* DEVICE */, size_t arena_bytes, ajt_stream_t stream);
 
 int ajt_policy_loss_fwd_bwd_host(
     const void* logits, const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
@@ -321,12 +337,6 @@ int ajt_policy_loss_fwd_bwd_host(
     void* dlogits /* HOST bf16 */, float* loss_out /* HOST [1] */, float* logp_out /* HOST [T] or NULL */,
     float* stats_out /* HOST [4] or NULL */, uint32_t* status_bits /* HOST [1] or NULL */,
     void* arena /* DEVICE */, size_t arena_bytes, ajt_stream_t stream);
-
-/* Measurement helper ("a micro-benchmark for read-only, write-only and copy HBM ceilings on the same box"):
- * streams `bytes` (multiple of 16, 16-byte aligned DEVICE buffers) with 16-byte accesses.  mode 0: read `src` (dst = a DEVICE
- * word that is practically never written, may alias anything), 1: write zeros to `dst`, 2: copy src -> dst, 3: cudaMemsetAsync
- * of `dst`.  Not part of the method. */
-int ajt_hbm_probe(void* dst, const void* src, size_t bytes, int32_t mode, ajt_stream_t stream);
 
 #ifdef __cplusplus
 }

@@ -248,28 +248,29 @@ def policy_loss(logits, targets, old_logp, adv, mask, seg_ids, S: int, eps_lo: f
 
 
 def pack_loss_inputs(merged_tokens, merged_mask, merged_old_logp, merged_offsets, merged_origin, tl_seg, seg_adv=None):
-    """Per-token loss inputs from merged sequences (reading L-12), sequence by sequence: inside sequence m the
-    row at position q predicts the token at q+1, so targets / mask / old_logp are those of q+1; the last position of every
-    sequence has nothing to predict (0, 0, 0).  seg_ids = dense trajectory id of the surviving timeline; adv = that
-    trajectory's advantage.  Returns (targets int32, mask uint8, old_logp float32 | None, seg_ids int32, adv float32 | None)."""
+    """Per-token loss inputs from merged sequences (reading L-12), sequence by sequence (ajt_oracle_pack in
+    ajt_oracle.c): inside sequence m the row at position q predicts the token at q+1, so targets / mask / old_logp are those
+    of q+1; the last position of every sequence has nothing to predict (0, 0, 0).  seg_ids = dense trajectory id of the
+    surviving timeline; adv = that trajectory's advantage.
+    Returns (targets int32, mask uint8, old_logp float32 | None, seg_ids int32, adv float32 | None)."""
+    merged_offsets = _c(merged_offsets, np.int64)
+    M = max(0, len(merged_offsets) - 1)
     N = int(merged_offsets[-1]) if len(merged_offsets) else 0
     targets = np.zeros(N, np.int32)
     mask = np.zeros(N, np.uint8)
     olp = None if merged_old_logp is None else np.zeros(N, np.float32)
     seg = np.zeros(N, np.int32)
     adv = None if seg_adv is None else np.zeros(N, np.float32)
-    for m in range(len(merged_offsets) - 1):
-        a, b = int(merged_offsets[m]), int(merged_offsets[m + 1])
-        sg = int(tl_seg[int(merged_origin[m])])
-        for q in range(a, b):
-            seg[q] = sg
-            if adv is not None:
-                adv[q] = seg_adv[sg]
-            if q + 1 < b:
-                targets[q] = merged_tokens[q + 1]
-                mask[q] = 1 if merged_mask[q + 1] else 0
-                if olp is not None:
-                    olp[q] = merged_old_logp[q + 1]
+    mt, mm = _c(merged_tokens, np.int32), _c(merged_mask, np.uint8)
+    ml = None if merged_old_logp is None else _c(merged_old_logp, np.float32)
+    mo, ts = _c(merged_origin, np.int32), _c(tl_seg, np.int32)
+    sa = None if seg_adv is None else _c(seg_adv, np.float32)
+    L = lib()
+    L.ajt_oracle_pack.restype = C.c_int
+    rc = L.ajt_oracle_pack(_p(mt), _p(mm), _p(ml), _p(merged_offsets), _p(mo), _p(ts), _p(sa), C.c_int64(M), _p(targets),
+                           _p(mask), _p(olp), _p(seg), _p(adv))
+    if rc != 0:
+        raise ValueError("ajt_oracle_pack: invalid offsets")
     return targets, mask, olp, seg, adv
 
 

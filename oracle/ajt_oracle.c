@@ -500,3 +500,33 @@ int ajt_oracle_merge_blocks(const int64_t* block_ids, const int64_t* block_offse
     free(cur_author); free(cur_src); free(absorbed); free(absorber); free(midx);
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Per-token loss inputs from merged sequences (reading L-12), sequence by sequence: inside sequence m the
+ * row at position q predicts the token at q + 1, so targets / mask / old_logp are those of q + 1; the last position of
+ * every sequence has nothing to predict (0, 0, 0).  seg_ids = dense trajectory id of the surviving timeline; adv = that
+ * trajectory's advantage.  merged_old_logp / old_logp and seg_adv / adv may be NULL in pairs.  The same loops as the
+ * Python function oracle.pack_loss_inputs had (its pins, tests/test_oracle_pack.py, run against this one). */
+int ajt_oracle_pack(const int32_t* merged_tokens, const uint8_t* merged_mask, const float* merged_old_logp,
+                    const int64_t* merged_offsets, const int32_t* merged_origin, const int32_t* tl_seg, const float* seg_adv,
+                    int64_t M, int32_t* targets, uint8_t* mask, float* old_logp, int32_t* seg_ids, float* adv) {
+    for (int64_t m = 0; m < M; ++m) {
+        const int64_t a = merged_offsets[m], b = merged_offsets[m + 1];
+        if (b < a) return -1;
+        const int32_t sg = tl_seg[merged_origin[m]];
+        for (int64_t q = a; q < b; ++q) {
+            seg_ids[q] = sg;
+            if (adv) adv[q] = seg_adv[sg];
+            if (q + 1 < b) {
+                targets[q] = merged_tokens[q + 1];
+                mask[q] = merged_mask[q + 1] ? 1 : 0;
+                if (old_logp) old_logp[q] = merged_old_logp[q + 1];
+            } else {
+                targets[q] = 0;
+                mask[q] = 0;
+                if (old_logp) old_logp[q] = 0.0f;
+            }
+        }
+    }
+    return 0;
+}

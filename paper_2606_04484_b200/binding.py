@@ -27,7 +27,7 @@ _EXPORTS = [
     "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
     "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks_workspace_bytes", "ajt_merge_blocks",
     "ajt_pack_loss_inputs", "ajt_lm_head_workspace_bytes", "ajt_lm_head_logp",
-    "ajt_hbm_probe",
+    "ajt_hbm_probe", "ajt_launch_count", "ajt_host_ctx_create", "ajt_host_ctx_destroy", "ajt_policy_loss_fwd_bwd_host2",
 ]
 
 _lib = None
@@ -74,8 +74,12 @@ def lib():
         L.ajt_loss_host_arena_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32]
         for f in ("ajt_merge_timelines", "ajt_merge_timelines_host", "ajt_policy_loss_fwd_bwd",
                   "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks",
-                  "ajt_pack_loss_inputs", "ajt_lm_head_logp", "ajt_hbm_probe"):
+                  "ajt_pack_loss_inputs", "ajt_lm_head_logp", "ajt_hbm_probe", "ajt_host_ctx_create",
+                  "ajt_policy_loss_fwd_bwd_host2"):
             getattr(L, f).restype = C.c_int
+        L.ajt_launch_count.restype = C.c_uint64
+        L.ajt_host_ctx_destroy.restype = None
+        L.ajt_host_ctx_destroy.argtypes = [C.c_void_p]
         _lib = L
     return _lib
 
@@ -94,6 +98,11 @@ def merge_workspace_bytes(n: int, n_tokens: int) -> int:
 
 def merge_workspace_bytes_for_pairs(n: int, n_tokens: int, n_pairs: int) -> int:
     return int(lib().ajt_merge_workspace_bytes_for_pairs(n, n_tokens, n_pairs))
+
+
+def launch_count() -> int:
+    """Kernels launched by the library in this process so far (include/ajt_test.h)."""
+    return int(lib().ajt_launch_count())
 
 
 def merge_host_arena_bytes(n: int, n_tokens: int) -> int:
@@ -166,8 +175,15 @@ class MergeOutput:
     N_out: int = -1
 
     def finalize(self) -> "MergeOutput":
+        """Synchronises; raises AjtError when the call ended on a fatal status (the outputs are then empty)."""
         c = self.counts.cpu()
         M, No = int(c[0]), int(c[1])
+        st = int(self.workspace[:4].view(torch.int32).cpu()[0]) & 0xFFFFFFFF
+        if st & STATUS_PROBE_CAPACITY:
+            raise AjtError(-3, "ajt_merge_timelines (AJT_STATUS_PROBE_CAPACITY: size the workspace with "
+                               "merge_workspace_bytes_for_pairs)")
+        if st & (STATUS_BAD_OFFSETS | STATUS_ZERO_LEN):
+            raise AjtError(-1, "ajt_merge_timelines (bad offsets or a zero-length timeline)")
         return MergeOutput(self.merged_tokens[:No], self.merged_mask[:No], self.merged_src[:No],
                            None if self.merged_old_logp is None else self.merged_old_logp[:No],
                            self.merged_offsets[:M + 1], self.merged_origin[:M], self.merged_traj[:M], self.owner,
@@ -323,7 +339,8 @@ def pack_loss_inputs(mo, tl_seg: torch.Tensor, S: int, seg_adv: Optional[torch.T
 def merge_timelines_host(tokens, offsets, traj_ids, resp_start=None, mask_in=None, old_logp_in=None,
                          owner_rule: int = OWNER_LONGEST, flags: int = 0, arena: Optional[torch.Tensor] = None,
                          out: Optional[dict] = None, stream=None) -> dict:
-    """ajt_merge_timelines_host: HOST buffers (numpy arrays or CPU torch tensors, pinned for speed)."""
+    """ajt_merge_timelines_host: HOST buffers (numpy arrays or CPU torch tensors, pinned for speed).  Raises AjtError
+    on a fatal status (pair capacity: pass a larger `arena`; bad offsets; zero-length timeline)."""
     _require_cuda()
     n, N = int(len(traj_ids)), int(len(tokens))
     if arena is None:
@@ -544,3 +561,52 @@ def policy_loss_fwd_bwd_host(logits, targets, old_logp, adv, mask, seg_ids, S: i
     if rc != 0:
         raise AjtError(rc, "ajt_policy_loss_fwd_bwd_host")
     return dict(dlogits=dlogits, loss=float(loss[0]), logp=logp, stats=stats, status=int(status.value))
+
+
+class HostCtx:
+    """ajt_host_ctx: the helper streams / events of the host slab pipeline, created once."""
+
+    def __init__(self):
+        _require_cuda()
+        self.h = C.c_void_p(None)
+        rc = lib().ajt_host_ctx_create(C.byref(self.h))
+        if rc != 0:
+            raise AjtError(rc, "ajt_host_ctx_create")
+
+    def close(self):
+        if self.h:
+            lib().ajt_host_ctx_destroy(self.h)
+            self.h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def policy_loss_fwd_bwd_host2(logits, targets, old_logp, adv, mask, seg_ids, S: int, eps_lo: float, eps_hi: float,
+                              dtype: int, dlogits_device: torch.Tensor, V: Optional[int] = None, seg_denom=None,
+                              inv_num_segs: float = 0.0, grad_scale: float = 1.0, want_logp: bool = False,
+                              want_stats: bool = False, ctx: Optional[HostCtx] = None, arena: Optional[torch.Tensor] = None,
+                              stream=None) -> dict:
+    """ajt_policy_loss_fwd_bwd_host2 with the gradient left on the device: HOST inputs, `dlogits_device` a CUDA bf16 [T, ld]
+    tensor; only loss / logp / stats / status come back."""
+    _require_cuda()
+    T, ld = int(logits.shape[0]), int(logits.shape[1])
+    V = ld if V is None else int(V)
+    _check_dev(dlogits_device, torch.bfloat16, "dlogits_device")
+    if arena is None:
+        arena = torch.empty(loss_host_arena_bytes(T, V, S, ld, dtype), dtype=torch.uint8, device="cuda")
+    loss = np.zeros(1, np.float32)
+    logp = np.zeros(max(T, 1), np.float32) if want_logp else None
+    stats = np.zeros(4, np.float32) if want_stats else None
+    status = C.c_uint32(0)
+    rc = lib().ajt_policy_loss_fwd_bwd_host2(
+        _hp(logits), _hp(targets), _hp(old_logp), _hp(adv), _hp(mask), _hp(seg_ids), C.c_float(eps_lo), C.c_float(eps_hi),
+        C.c_int64(T), C.c_int32(V), C.c_int32(S), C.c_int64(ld), C.c_int32(dtype), _hp(seg_denom), C.c_float(inv_num_segs),
+        C.c_float(grad_scale), _dp(dlogits_device), C.c_int32(1), _hp(loss), _hp(logp), _hp(stats), C.byref(status),
+        None if ctx is None else ctx.h, _dp(arena), C.c_size_t(arena.numel()), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_policy_loss_fwd_bwd_host2")
+    return dict(dlogits=dlogits_device, loss=float(loss[0]), logp=logp, stats=stats, status=int(status.value))

@@ -1,10 +1,17 @@
 // Library-level entry points of libajt.so: version, error strings, status read-back and the HOST-buffer
 // variants of the two hot-path calls (stage through a caller-provided device arena; no allocation here).
+#include <atomic>
+
 #include "ajt_common.cuh"
+#include "../../include/ajt_test.h"
 
 namespace {
 inline size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
+std::atomic<unsigned long long> g_launches{0};
 }  // namespace
+
+void ajt::note_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+extern "C" uint64_t ajt_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 extern "C" int ajt_version(void) { return AJT_VERSION_NUM; }
 
@@ -65,9 +72,9 @@ extern "C" int ajt_hbm_probe(void* dst, const void* src, size_t bytes, int32_t m
     if (cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || num_sms < 1) return AJT_ERR_CUDA;
     const size_t n16 = bytes / 16;
     const int grid = num_sms * 32;
-    if (mode == 0) probe_read_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<const uint4*>(src), n16, reinterpret_cast<uint32_t*>(dst));
-    else if (mode == 1) probe_write_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<uint4*>(dst), n16);
-    else if (mode == 2) probe_copy_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<uint4*>(dst), reinterpret_cast<const uint4*>(src), n16);
+    if (mode == 0) AJT_LAUNCH(probe_read_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<const uint4*>(src), n16, reinterpret_cast<uint32_t*>(dst)));
+    else if (mode == 1) AJT_LAUNCH(probe_write_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<uint4*>(dst), n16));
+    else if (mode == 2) AJT_LAUNCH(probe_copy_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<uint4*>(dst), reinterpret_cast<const uint4*>(src), n16));
     else if (cudaMemsetAsync(dst, 0, bytes, s) != cudaSuccess) return AJT_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }
@@ -125,14 +132,63 @@ constexpr int kHostMaxSlabs = 16;
 // Slab pipeline: the per-token vectors go up first and the batch-wide normalisers are counted on the device (reading L-4);
 // the [T, ld] matrix is cut into up to 16 row slabs, and slab i's H2D copy (helper stream 1), its loss call (the caller's
 // stream) and its D2H copy (helper stream 2) overlap with the neighbours', so both PCIe directions stay busy at once.
+struct ajt_host_ctx {
+    cudaStream_t s_up, s_dn;
+    cudaEvent_t ev_up[kHostMaxSlabs], ev_k[kHostMaxSlabs], ev0, ev_end;
+};
+
+extern "C" int ajt_host_ctx_create(ajt_host_ctx_t* out) {
+    if (!out) return AJT_ERR_INVALID_ARG;
+    ajt_host_ctx* c = new (std::nothrow) ajt_host_ctx();
+    if (!c) return AJT_ERR_CAPACITY;
+    bool ok = cudaStreamCreateWithFlags(&c->s_up, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&c->s_dn, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->ev0, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->ev_end, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < kHostMaxSlabs && ok; ++i)
+        ok = cudaEventCreateWithFlags(&c->ev_up[i], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&c->ev_k[i], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) {
+        ajt_host_ctx_destroy(c);
+        return AJT_ERR_CUDA;
+    }
+    *out = c;
+    return AJT_OK;
+}
+
+extern "C" void ajt_host_ctx_destroy(ajt_host_ctx_t c) {
+    if (!c) return;
+    for (int i = 0; i < kHostMaxSlabs; ++i) {
+        if (c->ev_up[i]) cudaEventDestroy(c->ev_up[i]);
+        if (c->ev_k[i]) cudaEventDestroy(c->ev_k[i]);
+    }
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev_end) cudaEventDestroy(c->ev_end);
+    if (c->s_up) cudaStreamDestroy(c->s_up);
+    if (c->s_dn) cudaStreamDestroy(c->s_dn);
+    delete c;
+}
+
 extern "C" int ajt_policy_loss_fwd_bwd_host(const void* logits, const int32_t* targets, const float* old_logp, const float* adv,
                                             const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T,
                                             int32_t V, int32_t S, int64_t ld, int32_t dtype, const float* seg_denom,
                                             float inv_num_segs, float grad_scale, void* dlogits, float* loss_out,
                                             float* logp_out, float* stats_out, uint32_t* status_bits, void* arena,
                                             size_t arena_bytes, ajt_stream_t stream_) {
+    return ajt_policy_loss_fwd_bwd_host2(logits, targets, old_logp, adv, mask, seg_ids, eps_lo, eps_hi, T, V, S, ld, dtype,
+                                         seg_denom, inv_num_segs, grad_scale, dlogits, 0, loss_out, logp_out, stats_out,
+                                         status_bits, nullptr, arena, arena_bytes, stream_);
+}
+
+extern "C" int ajt_policy_loss_fwd_bwd_host2(const void* logits, const int32_t* targets, const float* old_logp, const float* adv,
+                                             const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T,
+                                             int32_t V, int32_t S, int64_t ld, int32_t dtype, const float* seg_denom,
+                                             float inv_num_segs, float grad_scale, void* dlogits, int32_t dlogits_on_device,
+                                             float* loss_out, float* logp_out, float* stats_out, uint32_t* status_bits,
+                                             ajt_host_ctx_t ctx, void* arena, size_t arena_bytes, ajt_stream_t stream_) {
     cudaStream_t s = reinterpret_cast<cudaStream_t>(stream_);
     if (T < 0 || V <= 0 || S <= 0 || ld < V || !arena || !loss_out) return AJT_ERR_INVALID_ARG;
+    if (dlogits_on_device && ((uintptr_t)dlogits & 15)) return AJT_ERR_INVALID_ARG;
     if (dtype != AJT_DT_BF16 && dtype != AJT_DT_F32) return AJT_ERR_INVALID_ARG;
     if (T > 0 && (!logits || !targets || !old_logp || !adv || !mask || !seg_ids || !dlogits)) return AJT_ERR_INVALID_ARG;
     if ((uintptr_t)arena & 255) return AJT_ERR_INVALID_ARG;
@@ -141,7 +197,8 @@ extern "C" int ajt_policy_loss_fwd_bwd_host(const void* logits, const int32_t* t
     uint8_t* d = reinterpret_cast<uint8_t*>(arena);
     const size_t esz = dtype == AJT_DT_F32 ? 4 : 2;
     const size_t ws_bytes = ajt_loss_workspace_bytes(T, V, S);
-    uint8_t* d_dl = dtype == AJT_DT_F32 ? d + a.ws + ws_bytes : d + a.logits;   // bf16: in place
+    // where the kernel writes the gradient: the caller's device buffer, or the arena (bf16: in place over the uploaded rows)
+    uint8_t* d_dl = dlogits_on_device ? reinterpret_cast<uint8_t*>(dlogits) : (dtype == AJT_DT_F32 ? d + a.ws + ws_bytes : d + a.logits);
     // accumulators live in the tail of the stats slot: [loss f32 | ... ] at a.loss, [stats 4 x f32 | acc 5 x f64 | status u32] at a.stats
     float* d_loss = reinterpret_cast<float*>(d + a.loss);
     float* d_stats = reinterpret_cast<float*>(d + a.stats);
@@ -150,8 +207,14 @@ extern "C" int ajt_policy_loss_fwd_bwd_host(const void* logits, const int32_t* t
     float* d_denom = reinterpret_cast<float*>(d + a.denom);
 
     int rc = AJT_OK;
-    cudaStream_t s_up = nullptr, s_dn = nullptr;
-    cudaEvent_t ev_up[kHostMaxSlabs] = {}, ev_k[kHostMaxSlabs] = {}, ev0 = nullptr, ev_end = nullptr;
+    ajt_host_ctx_t own = nullptr;   // helper streams / events: the caller's context, or one made for this call
+    if (!ctx) {
+        rc = ajt_host_ctx_create(&own);
+        if (rc != AJT_OK) return rc;
+        ctx = own;
+    }
+    cudaStream_t s_up = ctx->s_up, s_dn = ctx->s_dn;
+    cudaEvent_t *ev_up = ctx->ev_up, *ev_k = ctx->ev_k, ev0 = ctx->ev0, ev_end = ctx->ev_end;
     const int nslab = (int)(T <= 0 ? 0 : (T < 256 * kHostMaxSlabs ? (T + 255) / 256 : kHostMaxSlabs));
     const int64_t rows_per = nslab ? (T + nslab - 1) / nslab : 0;
 #define AJT_TRY(x) \
@@ -162,14 +225,6 @@ extern "C" int ajt_policy_loss_fwd_bwd_host(const void* logits, const int32_t* t
     do { \
         if ((bytes) > 0) AJT_TRY(cudaMemcpyAsync((dst), (src), (bytes), (kind), (st))); \
     } while (0)
-    AJT_TRY(cudaStreamCreateWithFlags(&s_up, cudaStreamNonBlocking));
-    AJT_TRY(cudaStreamCreateWithFlags(&s_dn, cudaStreamNonBlocking));
-    AJT_TRY(cudaEventCreateWithFlags(&ev0, cudaEventDisableTiming));
-    AJT_TRY(cudaEventCreateWithFlags(&ev_end, cudaEventDisableTiming));
-    for (int i = 0; i < nslab; ++i) {
-        AJT_TRY(cudaEventCreateWithFlags(&ev_up[i], cudaEventDisableTiming));
-        AJT_TRY(cudaEventCreateWithFlags(&ev_k[i], cudaEventDisableTiming));
-    }
     // ---- per-token vectors, normalisers, accumulators (caller's stream)
     AJT_CP(d + a.targets, targets, (size_t)T * 4, cudaMemcpyHostToDevice, s);
     AJT_CP(d + a.old_logp, old_logp, (size_t)T * 4, cudaMemcpyHostToDevice, s);
@@ -208,13 +263,14 @@ extern "C" int ajt_policy_loss_fwd_bwd_host(const void* logits, const int32_t* t
                                      grad_scale, d_dl + (size_t)r0 * ld * 2, d_loss, logp_out ? (float*)(d + a.logp) + r0 : nullptr,
                                      stats_out ? d_stats : nullptr, d + a.ws, ws_bytes, stream_);
         if (rc != AJT_OK) break;
-        host_acc_kernel<<<1, 1, 0, s>>>(d_acc, d_status, d_loss, stats_out ? d_stats : nullptr, (const uint32_t*)(d + a.ws));
+        AJT_LAUNCH(host_acc_kernel<<<1, 1, 0, s>>>(d_acc, d_status, d_loss, stats_out ? d_stats : nullptr, (const uint32_t*)(d + a.ws)));
         AJT_TRY(cudaEventRecord(ev_k[i], s));
         AJT_TRY(cudaStreamWaitEvent(s_dn, ev_k[i], 0));
-        AJT_CP((uint8_t*)dlogits + (size_t)r0 * ld * 2, d_dl + (size_t)r0 * ld * 2, (size_t)R * ld * 2, cudaMemcpyDeviceToHost, s_dn);
+        if (!dlogits_on_device)
+            AJT_CP((uint8_t*)dlogits + (size_t)r0 * ld * 2, d_dl + (size_t)r0 * ld * 2, (size_t)R * ld * 2, cudaMemcpyDeviceToHost, s_dn);
     }
     if (rc == AJT_OK) {
-        host_fin_kernel<<<1, 1, 0, s>>>(d_acc, d_loss, d_stats);
+        AJT_LAUNCH(host_fin_kernel<<<1, 1, 0, s>>>(d_acc, d_loss, d_stats));
         AJT_CP(loss_out, d_loss, 4, cudaMemcpyDeviceToHost, s);
         if (logp_out) AJT_CP(logp_out, d + a.logp, (size_t)T * 4, cudaMemcpyDeviceToHost, s);
         if (stats_out) AJT_CP(stats_out, d_stats, 16, cudaMemcpyDeviceToHost, s);
@@ -225,14 +281,7 @@ extern "C" int ajt_policy_loss_fwd_bwd_host(const void* logits, const int32_t* t
     if (s_up) cudaStreamSynchronize(s_up);
     if (s_dn) cudaStreamSynchronize(s_dn);
     if (cudaStreamSynchronize(s) != cudaSuccess && rc == AJT_OK) rc = AJT_ERR_CUDA;
-    for (int i = 0; i < nslab; ++i) {
-        if (ev_up[i]) cudaEventDestroy(ev_up[i]);
-        if (ev_k[i]) cudaEventDestroy(ev_k[i]);
-    }
-    if (ev0) cudaEventDestroy(ev0);
-    if (ev_end) cudaEventDestroy(ev_end);
-    if (s_up) cudaStreamDestroy(s_up);
-    if (s_dn) cudaStreamDestroy(s_dn);
+    if (own) ajt_host_ctx_destroy(own);
 #undef AJT_CP
 #undef AJT_TRY
     return rc;
@@ -275,8 +324,9 @@ extern "C" int ajt_merge_timelines_host(const int32_t* tokens, const int64_t* of
     if (n < 0 || N < 0 || !arena || !counts || !offsets) return AJT_ERR_INVALID_ARG;
     if ((uintptr_t)arena & 255) return AJT_ERR_INVALID_ARG;
     if ((old_logp_in == nullptr) != (merged_old_logp == nullptr)) return AJT_ERR_INVALID_ARG;
-    const MergeArena a = merge_arena(n, N);
+    MergeArena a = merge_arena(n, N);
     if (arena_bytes < a.total) return AJT_ERR_WORKSPACE_TOO_SMALL;
+    a.ws_bytes += (arena_bytes - a.total) & ~(size_t)255;   // the workspace comes last: a larger arena holds more candidate pairs
     uint8_t* d = reinterpret_cast<uint8_t*>(arena);
 #define AJT_CP(dst, src, bytes, kind) \
     if ((bytes) > 0 && cudaMemcpyAsync((dst), (src), (bytes), (kind), s) != cudaSuccess) return AJT_ERR_CUDA
@@ -297,7 +347,13 @@ extern "C" int ajt_merge_timelines_host(const int32_t* tokens, const int64_t* of
     // the merged sizes are only known on the device: fetch {M, N_out}, then copy exactly that much back
     AJT_CP(counts, d + a.counts, 16, cudaMemcpyDeviceToHost);
     if (status_bits) AJT_CP(status_bits, d + a.ws, 4, cudaMemcpyDeviceToHost);
+    uint32_t st = 0;
+    if (cudaMemcpyAsync(&st, d + a.ws, 4, cudaMemcpyDeviceToHost, s) != cudaSuccess) return AJT_ERR_CUDA;
     if (cudaStreamSynchronize(s) != cudaSuccess) return AJT_ERR_CUDA;
+    // a fatal data-dependent status is an error of this call: the merged outputs would be empty / unspecified
+    if (st & AJT_STATUS_PROBE_CAPACITY) return AJT_ERR_CAPACITY;
+    if (st & (AJT_STATUS_BAD_OFFSETS | AJT_STATUS_ZERO_LEN)) return AJT_ERR_INVALID_ARG;
+    if (st & AJT_STATUS_INTERNAL) return AJT_ERR_CUDA;
     const size_t M = (size_t)counts[0], No = (size_t)counts[1];
     if (M > (size_t)n || No > (size_t)N) return AJT_ERR_CUDA;
     AJT_CP(merged_tokens, d + a.m_tokens, No * 4, cudaMemcpyDeviceToHost);

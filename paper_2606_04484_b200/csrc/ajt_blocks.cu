@@ -396,17 +396,17 @@ extern "C" int ajt_merge_blocks(const int64_t* block_ids, const int64_t* block_o
     const int ntiles = (int)((n_blocks + kScanTile - 1) / kScanTile);
     const int64_t want = (n_blocks + 255) / 256 + 1;
     const int grid_b = (int)(want < (int64_t)num_sms * 8 ? want : (int64_t)num_sms * 8);
-    blocks_prep_kernel<<<grid_b, 256, 0, stream>>>(p, ntiles);
+    AJT_LAUNCH(blocks_prep_kernel<<<grid_b, 256, 0, stream>>>(p, ntiles));
     // Algorithm 1 on the id streams: text-level Match, its own owner rule (the latest extender absorbs)
     const int rc = ajt_merge_timelines(reinterpret_cast<const int32_t*>(block_ids), p.offsets2, traj_ids, nullptr, p.mask2, nullptr,
                                        n, 2 * n_blocks, AJT_OWNER_PAPER, flags, p.ids_out, p.mask2_out, p.src2_out, nullptr,
                                        p.offs2_out, merged_origin, merged_traj, owner, p.counts2, b + ws.inner,
                                        ws.offsets2 - ws.inner, stream_);
     if (rc != AJT_OK) return rc;
-    blocks_info_kernel<<<grid_b, 256, 0, stream>>>(p);
-    blocks_scan_kernel<<<max(1, min(ntiles, num_sms)), 256, 0, stream>>>(p);
-    blocks_offsets_kernel<<<max(1, min((n + 256) / 256, num_sms)), 256, 0, stream>>>(p);
+    AJT_LAUNCH(blocks_info_kernel<<<grid_b, 256, 0, stream>>>(p));
+    AJT_LAUNCH(blocks_scan_kernel<<<max(1, min(ntiles, num_sms)), 256, 0, stream>>>(p));
+    AJT_LAUNCH(blocks_offsets_kernel<<<max(1, min((n + 256) / 256, num_sms)), 256, 0, stream>>>(p));
     const int64_t wantc = (n_tokens + 8 * kCopyTile - 1) / (8 * kCopyTile) + 1;   // 8 warps per CTA, one tile per warp and turn
-    blocks_copy_kernel<<<(int)(wantc < (int64_t)num_sms * 8 ? wantc : (int64_t)num_sms * 8), 256, 0, stream>>>(p);
+    AJT_LAUNCH(blocks_copy_kernel<<<(int)(wantc < (int64_t)num_sms * 8 ? wantc : (int64_t)num_sms * 8), 256, 0, stream>>>(p));
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }

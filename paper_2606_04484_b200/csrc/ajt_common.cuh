@@ -39,6 +39,10 @@ static_assert(sizeof(AjtCtrl) == 256, "AjtCtrl must be 256 bytes");
 
 namespace ajt {
 
+// Kernel launches made by the library in this process (measurement only: ajt_launch_count in ajt_test.h).
+void note_launch();
+#define AJT_LAUNCH(...) do { __VA_ARGS__; ajt::note_launch(); } while (0)
+
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 // ---- mbarrier -------------------------------------------------------------------------------------

@@ -506,10 +506,10 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
         if (ent_out && cudaMemsetAsync(ent_out, 0, (size_t)T * 4, stream) != cudaSuccess) return AJT_ERR_CUDA;
         if (lse_out && cudaMemsetAsync(lse_out, 0, (size_t)T * 4, stream) != cudaSuccess) return AJT_ERR_CUDA;
         const int ntiles = (int)((T + kCompactTile - 1) / kCompactTile);
-        lm_compact_kernel<<<ntiles < num_sms ? ntiles : num_sms, 256, 0, stream>>>(mask, T, reinterpret_cast<uint64_t*>(wsb + ws.tile_state),
-                                                                                 n_rows + 1, row_idx, n_rows);
-        lm_gather_kernel<<<num_sms * 8, 256, 0, stream>>>(reinterpret_cast<const uint4*>(hidden), ld_hidden / 8, d / 8, targets, row_idx, n_rows,
-                                                         reinterpret_cast<uint4*>(wsb + ws.hidden_c), targets_c);
+        AJT_LAUNCH(lm_compact_kernel<<<ntiles < num_sms ? ntiles : num_sms, 256, 0, stream>>>(mask, T, reinterpret_cast<uint64_t*>(wsb + ws.tile_state),
+                                                                                 n_rows + 1, row_idx, n_rows));
+        AJT_LAUNCH(lm_gather_kernel<<<num_sms * 8, 256, 0, stream>>>(reinterpret_cast<const uint4*>(hidden), ld_hidden / 8, d / 8, targets, row_idx, n_rows,
+                                                         reinterpret_cast<uint4*>(wsb + ws.hidden_c), targets_c));
         p.targets = targets_c; p.n_rows = n_rows; p.row_idx = row_idx;
         h_src = wsb + ws.hidden_c;
         h_ld = d;
@@ -531,7 +531,7 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
     if (ncta == 1) {
         if (cudaFuncSetAttribute(lm_head_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<1>::kSmem) != cudaSuccess)
             return AJT_ERR_CUDA;
-        lm_head_kernel<1><<<groups, kLmThreads, LmCfg<1>::kSmem, stream>>>(map_h, map_w, p);
+        AJT_LAUNCH(lm_head_kernel<1><<<groups, kLmThreads, LmCfg<1>::kSmem, stream>>>(map_h, map_w, p));
     } else {
         if (cudaFuncSetAttribute(lm_head_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<2>::kSmem) != cudaSuccess)
             return AJT_ERR_CUDA;
@@ -547,9 +547,10 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
         attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
+        ajt::note_launch();
         if (cudaLaunchKernelEx(&cfg, lm_head_kernel<2>, map_h, map_w, p) != cudaSuccess) return AJT_ERR_CUDA;
     }
     const int64_t want = (T + 255) / 256;
-    lm_head_combine_kernel<<<(int)(want < (int64_t)num_sms * 4 ? want : (int64_t)num_sms * 4), 256, 0, stream>>>(p, nvs);
+    AJT_LAUNCH(lm_head_combine_kernel<<<(int)(want < (int64_t)num_sms * 4 ? want : (int64_t)num_sms * 4), 256, 0, stream>>>(p, nvs));
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }

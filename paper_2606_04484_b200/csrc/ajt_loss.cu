@@ -805,6 +805,7 @@ cudaError_t launch_rows_t(const LossParams& p, int num_sms, cudaStream_t stream)
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+    ajt::note_launch();
     return cudaLaunchKernelEx(&cfg, kern, p);
 }
 
@@ -871,7 +872,7 @@ int loss_call(const void* logits, const int32_t* targets, const float* old_logp,
 
     if (cudaMemsetAsync(p.ctrl, 0, ws.zero_bytes, stream) != cudaSuccess) return AJT_ERR_CUDA;
     const int ntiles = (int)((T + kPrepTile - 1) / kPrepTile);
-    loss_prep_kernel<<<max(1, min(ntiles, num_sms)), 1024, 0, stream>>>(p, ntiles);
+    AJT_LAUNCH(loss_prep_kernel<<<max(1, min(ntiles, num_sms)), 1024, 0, stream>>>(p, ntiles));
 
     const bool aligned = (((uintptr_t)logits | (uintptr_t)dlogits) & 15) == 0 && (ld_logits % 8) == 0 && (V % 8) == 0;
     const bool fast = logits_dtype == AJT_DT_BF16 && aligned && T > 0;
@@ -887,15 +888,15 @@ int loss_call(const void* logits, const int32_t* targets, const float* old_logp,
         by_row = 1;
         const int grid = num_sms * 8;
         if (logits_dtype == AJT_DT_F32) {
-            if (V <= 2048) loss_rows_generic<float, 32><<<grid, 256, 0, stream>>>(p);
-            else loss_rows_generic<float, 256><<<grid, 256, 0, stream>>>(p);
+            if (V <= 2048) AJT_LAUNCH(loss_rows_generic<float, 32><<<grid, 256, 0, stream>>>(p));
+            else AJT_LAUNCH(loss_rows_generic<float, 256><<<grid, 256, 0, stream>>>(p));
         } else {
-            if (V <= 2048) loss_rows_generic<__nv_bfloat16, 32><<<grid, 256, 0, stream>>>(p);
-            else loss_rows_generic<__nv_bfloat16, 256><<<grid, 256, 0, stream>>>(p);
+            if (V <= 2048) AJT_LAUNCH(loss_rows_generic<__nv_bfloat16, 32><<<grid, 256, 0, stream>>>(p));
+            else AJT_LAUNCH(loss_rows_generic<__nv_bfloat16, 256><<<grid, 256, 0, stream>>>(p));
         }
     }
     if (e != cudaSuccess) return AJT_ERR_CUDA;
-    loss_final_kernel<<<1, 1024, 0, stream>>>(p, by_row);
+    AJT_LAUNCH(loss_final_kernel<<<1, 1024, 0, stream>>>(p, by_row));
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }
 }  // namespace
@@ -937,6 +938,6 @@ extern "C" int ajt_segment_counts(const uint8_t* mask, const int32_t* seg_ids, i
     if (T == 0) return AJT_OK;
     const int64_t want = (T + 255) / 256;
     const int grid = (int)(want < (int64_t)num_sms * 8 ? want : (int64_t)num_sms * 8);
-    segment_counts_kernel<<<grid, 256, 0, stream>>>(mask, seg_ids, T, S, seg_denom, status_bits);
+    AJT_LAUNCH(segment_counts_kernel<<<grid, 256, 0, stream>>>(mask, seg_ids, T, S, seg_denom, status_bits));
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }

@@ -45,6 +45,7 @@
 #include <cstdlib>
 
 #include "ajt_common.cuh"
+#include "../../include/ajt_test.h"
 
 namespace {
 
@@ -2011,18 +2012,18 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
         return AJT_OK;
     }
 #define AJT_DBG(name) do { if (getenv("AJT_DEBUG_SYNC")) { cudaError_t e_ = cudaStreamSynchronize(stream); fprintf(stderr, "[ajt] %s: %s\n", name, cudaGetErrorString(e_)); } } while (0)
-    if (n <= kGrpSmemN) merge_group_fast_kernel<<<1, 1024, group_fast_smem(n), stream>>>(p, n + n / 8 + 16);
-    else merge_group_radix_kernel<<<1, 1024, 0, stream>>>(p);
+    if (n <= kGrpSmemN) AJT_LAUNCH(merge_group_fast_kernel<<<1, 1024, group_fast_smem(n), stream>>>(p, n + n / 8 + 16));
+    else AJT_LAUNCH(merge_group_radix_kernel<<<1, 1024, 0, stream>>>(p));
     AJT_DBG("group");
-    merge_hash_kernel<<<num_sms * 2, kHashThreads, kHashSmem, stream>>>(p);
+    AJT_LAUNCH(merge_hash_kernel<<<num_sms * 2, kHashThreads, kHashSmem, stream>>>(p));
     AJT_DBG("hash");
-    merge_select_kernel<<<num_sms * 4, kSelThreads, sizeof(SelectStage), stream>>>(p);
+    AJT_LAUNCH(merge_select_kernel<<<num_sms * 4, kSelThreads, sizeof(SelectStage), stream>>>(p));
     AJT_DBG("select");
-    merge_compact_kernel<<<1, 1024, kCompactSmem, stream>>>(p);
+    AJT_LAUNCH(merge_compact_kernel<<<1, 1024, kCompactSmem, stream>>>(p));
     const int64_t want = ((n_tokens >> kTSLog) + 1 + 255) / 256 + ((int64_t)n * 32 + 255) / 256;
-    merge_plan_kernel<<<(int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8), 256, 0, stream>>>(p);
+    AJT_LAUNCH(merge_plan_kernel<<<(int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8), 256, 0, stream>>>(p));
     AJT_DBG("plan");
-    merge_scatter_kernel<<<num_sms, kScatThreads, kScatSmem, stream>>>(p);
+    AJT_LAUNCH(merge_scatter_kernel<<<num_sms, kScatThreads, kScatSmem, stream>>>(p));
     AJT_DBG("scatter");
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }

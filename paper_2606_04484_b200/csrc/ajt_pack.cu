@@ -144,6 +144,6 @@ extern "C" int ajt_pack_loss_inputs(const int32_t* merged_tokens, const uint8_t*
     p.cap = capacity_tokens; p.S = S; p.targets = targets; p.mask = mask; p.old_logp = old_logp; p.seg_ids = seg_ids; p.adv = adv; p.status = status_bits;
     const int64_t want = (capacity_tokens + 8 * kPackTile - 1) / (8 * kPackTile);
     const int grid = (int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8);
-    pack_loss_inputs_kernel<<<grid, 256, 0, stream>>>(p);
+    AJT_LAUNCH(pack_loss_inputs_kernel<<<grid, 256, 0, stream>>>(p));
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }

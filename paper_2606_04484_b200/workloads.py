@@ -238,33 +238,6 @@ def advantages_group_zscore(seed: int, cfg_index: int, n_traj: int, group: int =
     return adv.astype(np.float32)
 
 
-def shift_for_next_token(merged_tokens: np.ndarray, merged_mask: np.ndarray, merged_old_logp: np.ndarray,
-                         merged_offsets: np.ndarray):
-    """inside each merged sequence targets[q] = tokens[q+1], mask[q] = mask[q+1],
-    old_logp[q] = old_logp[q+1]; the last position of every sequence is masked out.  Pure index plumbing."""
-    N = merged_tokens.shape[0]
-    targets = np.zeros(N, dtype=np.int32)
-    mask = np.zeros(N, dtype=np.uint8)
-    olp = np.zeros(N, dtype=np.float32)
-    if N > 1:
-        targets[:-1] = merged_tokens[1:]
-        mask[:-1] = merged_mask[1:]
-        olp[:-1] = merged_old_logp[1:]
-    last = merged_offsets[1:] - 1
-    last = last[last >= 0]
-    mask[last] = 0
-    targets[last] = 0
-    olp[last] = 0
-    return targets, mask, olp
-
-
-def seg_ids_from_merged(merged_offsets: np.ndarray, merged_traj: np.ndarray):
-    """Segment = trajectory: dense ids 0..S-1 in order of first appearance."""
-    uniq, inv = np.unique(merged_traj, return_inverse=True)
-    lens = np.diff(merged_offsets)
-    return np.repeat(inv.astype(np.int32), lens), int(uniq.shape[0]), uniq
-
-
 @dataclass
 class LossVectors:
     targets: np.ndarray   # int32 [T]

@@ -24,7 +24,8 @@ def gpu_merge(mi, owner_rule, use_explicit_mask=False, flags=0, with_logp=True, 
     lp = torch.from_numpy(mi.old_logp).to(dev) if with_logp else None
     out = ajt.merge_timelines(tokens, offsets, traj, rs, mk, lp, owner_rule=owner_rule, flags=flags)
     status = ajt.last_status(out.workspace)
-    return out.finalize(), status
+    fatal = ajt.STATUS_PROBE_CAPACITY | ajt.STATUS_BAD_OFFSETS | ajt.STATUS_ZERO_LEN
+    return (None if status & fatal else out.finalize()), status
 
 
 def assert_merge_equal(g, r):
@@ -115,3 +116,34 @@ def check_loss(out, ref: "oracle.LossResult", logits_rows_mask, eps_lo, eps_hi, 
                 1e-5 * max(1e-3, float(np.sum(ref.w * np.abs(ref.logp - old_logp[rows]))))
             assert abs(st[3] - ref.stats[3]) <= tol3, (st[3], ref.stats[3], tol3)
     return dict(max_err=float(err.max()) if err.size else 0.0, n_near=int(near.sum()))
+
+
+# ---- pin P-K2 of oracle.pack_loss_inputs: a second formulation of reading L-12 as one global shift (lives with the tests:
+# the product package holds none of the method's arithmetic outside its kernels)
+
+
+def shift_for_next_token(merged_tokens: np.ndarray, merged_mask: np.ndarray, merged_old_logp: np.ndarray,
+                         merged_offsets: np.ndarray):
+    """inside each merged sequence targets[q] = tokens[q+1], mask[q] = mask[q+1],
+    old_logp[q] = old_logp[q+1]; the last position of every sequence is masked out.  Pure index plumbing."""
+    N = merged_tokens.shape[0]
+    targets = np.zeros(N, dtype=np.int32)
+    mask = np.zeros(N, dtype=np.uint8)
+    olp = np.zeros(N, dtype=np.float32)
+    if N > 1:
+        targets[:-1] = merged_tokens[1:]
+        mask[:-1] = merged_mask[1:]
+        olp[:-1] = merged_old_logp[1:]
+    last = merged_offsets[1:] - 1
+    last = last[last >= 0]
+    mask[last] = 0
+    targets[last] = 0
+    olp[last] = 0
+    return targets, mask, olp
+
+
+def seg_ids_from_merged(merged_offsets: np.ndarray, merged_traj: np.ndarray):
+    """Segment = trajectory: dense ids 0..S-1 in order of first appearance."""
+    uniq, inv = np.unique(merged_traj, return_inverse=True)
+    lens = np.diff(merged_offsets)
+    return np.repeat(inv.astype(np.int32), lens), int(uniq.shape[0]), uniq

@@ -16,7 +16,7 @@ import oracle
 import paper_2606_04484_b200 as ajt
 from paper_2606_04484_b200 import harness as H
 from paper_2606_04484_b200 import workloads as W
-from helpers import bf16_bits, check_loss
+from helpers import bf16_bits, check_loss, seg_ids_from_merged, shift_for_next_token
 
 pytestmark = pytest.mark.gpu
 
@@ -91,8 +91,8 @@ def test_bench_microbatch_c2_full():
     fin = mo.finalize()
     r = oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp)
     assert fin.N_out == r.N_out and np.array_equal(fin.merged_tokens.cpu().numpy(), r.merged_tokens)
-    targets, mask, _ = W.shift_for_next_token(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets)
-    seg, S, _ = W.seg_ids_from_merged(r.merged_offsets, r.merged_traj)
+    targets, mask, _ = shift_for_next_token(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets)
+    seg, S, _ = seg_ids_from_merged(r.merged_offsets, r.merged_traj)
     adv = W.advantages_group_zscore(seed, 1, S)[seg].astype(np.float32)
     T, V = 40960, 151936
     Ns_t = ajt.segment_counts(d(mask), d(seg), S)
@@ -182,9 +182,9 @@ def test_c3_chunk_with_real_merge_vectors():
     assert ajt.last_status(mo.workspace) == 0
     fin = mo.finalize()
     cpu = lambda t: t.cpu().numpy()
-    targets, mask, _ = W.shift_for_next_token(cpu(fin.merged_tokens), cpu(fin.merged_mask), cpu(fin.merged_old_logp),
+    targets, mask, _ = shift_for_next_token(cpu(fin.merged_tokens), cpu(fin.merged_mask), cpu(fin.merged_old_logp),
                                               cpu(fin.merged_offsets))
-    seg, S, _ = W.seg_ids_from_merged(cpu(fin.merged_offsets), cpu(fin.merged_traj))
+    seg, S, _ = seg_ids_from_merged(cpu(fin.merged_offsets), cpu(fin.merged_traj))
     adv = W.advantages_group_zscore(W.BASE_SEED + 2, 2, S)[seg].astype(np.float32)
     Ns_t = ajt.segment_counts(d(mask), d(seg), S)
     Ns = Ns_t.cpu().numpy()

@@ -11,7 +11,7 @@ import torch
 import oracle
 import paper_2606_04484_b200 as ajt
 from paper_2606_04484_b200 import workloads as W
-from helpers import check_loss, harness_old_logp, logits_to_oracle
+from helpers import check_loss, harness_old_logp, logits_to_oracle, seg_ids_from_merged, shift_for_next_token
 
 pytestmark = pytest.mark.gpu
 
@@ -154,8 +154,8 @@ def test_c1_loss_over_merged_tokens():
     """configs[0] end to end: merge on the GPU, loss on the merged tokens (fp32 logits, V=1024, adv +-1, eps 0.2)."""
     mi = W.merge_workload("c1")
     r = oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp)
-    targets, mask, _ = W.shift_for_next_token(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets)
-    seg, S, _ = W.seg_ids_from_merged(r.merged_offsets, r.merged_traj)
+    targets, mask, _ = shift_for_next_token(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets)
+    seg, S, _ = seg_ids_from_merged(r.merged_offsets, r.merged_traj)
     advt = W.advantages_pm1(W.BASE_SEED, 0, S)
     T, V = r.N_out, 1024
     g = torch.Generator(device="cuda").manual_seed(W.BASE_SEED)

@@ -207,18 +207,58 @@ def test_empty_and_invalid():
 
 
 def test_probe_capacity_status():
-    # 200 timelines in one group need 20100 keys; the default workspace holds 64*200+4096 = 16896
+    # 200 timelines in one group need 20100 pairs; the default workspace holds 64*200+4096 = 16896: the status bit is set,
+    # counts are {0, 0}, finalize() raises; a workspace sized from the group histogram works (no silent empty merge)
     tls = [[1] * (j + 1) for j in range(200)]
     mi = from_lists(tls, [0] * 200, [0] * 200)
-    g, st = gpu_merge(mi, ajt.OWNER_LONGEST)
-    assert st & ajt.STATUS_PROBE_CAPACITY
     dev = "cuda"
-    big = ajt.merge_workspace_bytes(mi.n, mi.n_tokens) + 32 * 8000
-    out = ajt.merge_timelines(torch.from_numpy(mi.tokens).to(dev), torch.from_numpy(mi.offsets).to(dev),
-                              torch.from_numpy(mi.traj_ids).to(dev), torch.from_numpy(mi.resp_start).to(dev), None,
-                              torch.from_numpy(mi.old_logp).to(dev), workspace_bytes=big)
+    args = (torch.from_numpy(mi.tokens).to(dev), torch.from_numpy(mi.offsets).to(dev), torch.from_numpy(mi.traj_ids).to(dev),
+            torch.from_numpy(mi.resp_start).to(dev), None, torch.from_numpy(mi.old_logp).to(dev))
+    out = ajt.merge_timelines(*args)
+    assert ajt.last_status(out.workspace) & ajt.STATUS_PROBE_CAPACITY
+    assert out.counts.cpu().tolist() == [0, 0]
+    with pytest.raises(ajt.AjtError):
+        out.finalize()
+    n_pairs = 200 * 201 // 2
+    big = ajt.merge_workspace_bytes_for_pairs(mi.n, mi.n_tokens, n_pairs)
+    assert big > ajt.merge_workspace_bytes(mi.n, mi.n_tokens)
+    out = ajt.merge_timelines(*args, workspace_bytes=big)
     assert ajt.last_status(out.workspace) == 0
     assert_merge_equal(out.finalize(), oracle_merge(mi, ajt.OWNER_LONGEST))
+    # the host-buffer call reports the same condition as an error code, and takes the pairs from a larger arena
+    with pytest.raises(ajt.AjtError) as ei:
+        ajt.merge_timelines_host(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp)
+    assert ei.value.code == -3
+    arena = torch.empty(ajt.merge_host_arena_bytes(mi.n, mi.n_tokens) + big, dtype=torch.uint8, device=dev)
+    h = ajt.merge_timelines_host(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp, arena=arena)
+    r = oracle_merge(mi, ajt.OWNER_LONGEST)
+    assert h["status"] == 0 and h["M"] == r.M and np.array_equal(h["merged_tokens"][:r.N_out].numpy(), r.merged_tokens)
+
+
+def test_long_trajectories_over_127_calls():
+    # trajectories averaging more than ~127 LLM calls exceed the default pair capacity; sized from the histogram
+    # they merge exactly.  4 trajectories x 160 calls, appended context, a few rewrites.
+    rng = np.random.default_rng(31)
+    tls, traj = [], []
+    ctx = {g: [int(x) for x in rng.integers(0, 50, size=20)] for g in range(4)}
+    for k in range(160):
+        for g in range(4):
+            if k and rng.random() < 0.05:
+                c = int(rng.integers(0, len(ctx[g])))
+                ctx[g] = ctx[g][:c] + [int(x) for x in rng.integers(50, 99, size=int(rng.integers(1, 30)))]
+            ctx[g] = ctx[g] + [int(x) for x in rng.integers(0, 50, size=int(rng.integers(1, 12)))]
+            tls.append(list(ctx[g]))
+            traj.append(g)
+    mi = from_lists(tls, traj, [max(0, len(t) - 3) for t in tls])
+    n_pairs = 4 * (160 * 161 // 2)
+    dev = "cuda"
+    for rule in RULES:
+        out = ajt.merge_timelines(torch.from_numpy(mi.tokens).to(dev), torch.from_numpy(mi.offsets).to(dev),
+                                  torch.from_numpy(mi.traj_ids).to(dev), torch.from_numpy(mi.resp_start).to(dev), None,
+                                  torch.from_numpy(mi.old_logp).to(dev), owner_rule=rule,
+                                  workspace_bytes=ajt.merge_workspace_bytes_for_pairs(mi.n, mi.n_tokens, n_pairs))
+        assert ajt.last_status(out.workspace) == 0
+        assert_merge_equal(out.finalize(), oracle_merge(mi, rule))
 
 
 def test_host_buffer_variant():

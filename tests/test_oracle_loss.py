@@ -10,6 +10,7 @@ import pytest
 import torch
 
 import oracle
+from helpers import seg_ids_from_merged, shift_for_next_token
 from paper_2606_04484_b200 import workloads as W
 
 
@@ -268,7 +269,7 @@ def test_loss_merged_equals_unmerged(rule):
     rng = np.random.default_rng(12)
     # one logits row per MERGED token; targets = the token itself folded into V; adv per trajectory
     zm = (rng.standard_normal((r.N_out, V)) * 2).astype(np.float32)
-    seg_m, S, uniq = W.seg_ids_from_merged(r.merged_offsets, r.merged_traj)
+    seg_m, S, uniq = seg_ids_from_merged(r.merged_offsets, r.merged_traj)
     adv_traj = rng.standard_normal(S).astype(np.float32)
     ym = (r.merged_tokens % V).astype(np.int32)
     # give the merged old_logp values a plausible scale: old = (random row logp) - handled by using carried values

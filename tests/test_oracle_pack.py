@@ -6,6 +6,7 @@ per sequence, exactly sum_{q>=1} mask[q] log p(x_q | x_<q) computed sequence by 
 import numpy as np
 
 import oracle
+from helpers import seg_ids_from_merged, shift_for_next_token
 from paper_2606_04484_b200 import workloads as W
 
 
@@ -32,8 +33,8 @@ def test_global_shift_formulation():
     uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
     t, m, o, s, _ = oracle.pack_loss_inputs(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets, r.merged_origin,
                                             tl_seg.astype(np.int32))
-    t2, m2, o2 = W.shift_for_next_token(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets)
-    s2, S, _ = W.seg_ids_from_merged(r.merged_offsets, r.merged_traj)
+    t2, m2, o2 = shift_for_next_token(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets)
+    s2, S, _ = seg_ids_from_merged(r.merged_offsets, r.merged_traj)
     assert np.array_equal(t, t2) and np.array_equal(m, m2) and np.array_equal(o, o2) and np.array_equal(s, s2)
     assert S == uniq.shape[0]
 
