@@ -1,17 +1,22 @@
 #!/usr/bin/env python
-"""bench.py — one "step" = one pass of the whole hot path (SURVEY.md §8(a) rows M1-M7 + L0-L4) over one
-synthetic batch of BASELINE.json configs[1] ("single-model GRPO batch"):
+"""bench.py — one "step" = one pass of the whole hot path (SURVEY.md §8(a) rows M1-M7 + L0-L4) over one synthetic batch
+of BASELINE.json configs[2] ("long-horizon agent", the largest single-GPU configuration):
 
-    ajt_merge_timelines      over the batch's 512 timelines (N_in ~ 1.76 M tokens)
-    ajt_policy_loss_fwd_bwd  over one 40,960-row micro-batch of the merged tokens, bf16 logits [40960,151936]
+    ajt_merge_timelines      over the batch's ~7.9k timelines (N_in ~ 69 M tokens, 277 MB)
+    ajt_pack_loss_inputs + ajt_segment_counts   the device-resident bridge (next-token alignment, batch-wide N_s)
+    ajt_policy_loss_fwd_bwd  over one 65,536-row chunk of the merged tokens, bf16 logits [65536,151936] (19.9 GB in,
+                             19.9 GB out), with the chunk's real targets / mask / segments from the merge output
 
-`value` = algorithmic bytes of the step / device time (GB/s), inputs resident in HBM.  `e2e` = the same metric
-through the *_host C-ABI calls with pinned HOST buffers (H2D and D2H inside the timed region).
-`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+`value` = algorithmic bytes of the step / device time (GB/s), inputs resident in HBM.  `e2e` = the same metric through the
+*_host C-ABI calls with pinned HOST buffers (H2D and D2H inside the timed region).  `configs` = one compact record per
+BASELINE.json config (c1, c2, c3, c4 A/B, three c5 cells): merged tokens/s, merge GB/s, logits GB/s, token-reduction
+factor, each as a fraction of the measured and of the nominal HBM rate, and the oracle's merge time on the host cores
+(one thread and all).  `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
 
-Launch: `python bench.py --gpus N --steps K --warmup W`; for N>1 under torch.distributed.run (one rank per GPU,
-weak scaling: every rank runs its own seeded batch, no data-path collective — merging never crosses trajectories
-and loss rows are independent given the per-trajectory normalisers).
+Launch: `python bench.py --gpus N --steps K --warmup W`; for N>1 under torch.distributed.run (one rank per GPU): ONE batch
+is split N ways — trajectory groups go to ranks (paper_2606_04484_b200.shard), every rank merges its share, the batch-wide
+per-trajectory token counts N_s are all-reduced (NCCL) inside the step, every rank runs the loss over one chunk of its own
+merged tokens, and the scalar is all-reduced.
 """
 from __future__ import annotations
 
@@ -29,15 +34,13 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "merge Gtokens/s and policy-loss fwd+bwd logits GB/s (fraction of B200 HBM peak)"
-MB_ROWS = 40960          # loss micro-batch rows (BASELINE.json configs[1]: "~40k merged tokens")
+CHUNK_ROWS = 65536       # BASELINE.json configs[2]: "64k-token chunks of bf16 logits [65536,151936]"
 V = 151936
 EPS = (0.2, 0.28)
+HEADLINE = "c3"
 
-from paper_2606_04484_b200.harness import (NOMINAL_HBM_GBS, loss_bytes as _loss_bytes, measured_peak, merge_bytes)  # noqa: E402
-
-
-def loss_bytes(T: int, Vv: int, n_unmasked: int, b_in: int = 2) -> int:
-    return _loss_bytes(T, Vv, n_unmasked, b_in)
+from paper_2606_04484_b200.harness import (NOMINAL_HBM_GBS, L2Flusher, fill_logits, harness_old_logp, loss_bytes,  # noqa: E402
+                                           measured_peak, merge_bytes, time_calls)
 
 
 # ----------------------------------------------------------------------------------------- clocks sampler
@@ -107,117 +110,110 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sel), "power_w_max": max(pw) if pw else None}
 
 
-# ----------------------------------------------------------------------------------------- workload (harness)
 
 
-def harness_old_logp(torch, logits_t, targets_t, noise):
-    from paper_2606_04484_b200.harness import harness_old_logp as f
-    return f(logits_t, targets_t, noise)
+# ----------------------------------------------------------------------------------------- workload plumbing (no method arithmetic)
+
+CFG_INDEX = {"c1": 0, "c2": 1, "c3": 2, "c4A": 3, "c4B": 3}
+CFG_EPS = {"c1": (0.2, 0.2), "c2": (0.2, 0.28), "c3": (0.2, 0.28), "c4A": (0.2, 0.2), "c4B": (0.2, 0.2)}
+CFG_WHAT = {
+    "c1": "configs[0] tiny: 32 trajectories x 6 turns, vocab 1024, fp32 logits over all merged tokens",
+    "c2": "configs[1] single-model GRPO batch: 64 trajectories x 8 turns, one 40,960-row micro-batch [40960,151936] bf16",
+    "c3": "configs[2] long-horizon agent: 256 trajectories x 20-40 turns, contexts to 32k, one chunk [65536,151936] bf16",
+    "c4A": "configs[3] team, model A (agents 0,1; vocab 151936): one chunk [65536,151936] bf16",
+    "c4B": "configs[3] team, model B (agent 2; vocab 128256): one chunk [65536,128256] bf16",
+}
 
 
-def fill_logits(torch, buf, seed: int, sigma: float = 3.0, slab: int = 2048):
-    from paper_2606_04484_b200.harness import fill_logits as f
-    f(buf, seed, sigma, slab)
+def merge_inputs(W, name: str, seed=None):
+    if name in ("c4A", "c4B"):
+        return W.merge_workload_c4(seed=seed)[name[-1]]
+    return W.merge_workload(name, seed=seed)
 
 
-def loss_side_inputs(W, merged_tokens, merged_mask, merged_old_logp, merged_offsets, merged_traj, seed: int):
-    """Index plumbing from the merge output to the loss call (reading L-12) plus the batch-wide
-    per-trajectory normalisers the caller owns when it streams micro-batches (reading L-4)."""
-    targets, mask, _ = W.shift_for_next_token(merged_tokens, merged_mask, merged_old_logp, merged_offsets)
-    seg, S, _ = W.seg_ids_from_merged(merged_offsets, merged_traj)
-    adv = W.advantages_group_zscore(seed, 1, S)[seg]
-    Ns = np.bincount(seg, weights=mask.astype(np.float64), minlength=S).astype(np.float32)
-    inv = 1.0 / max(1, int((Ns > 0).sum()))
-    return targets, mask, seg, S, adv.astype(np.float32), Ns, float(np.float32(inv))
+def seg_advantages(W, name: str, seed: int, S: int) -> np.ndarray:
+    if name == "c1":
+        return W.advantages_pm1(seed, 0, S).astype(np.float32)
+    return W.advantages_group_zscore(seed, CFG_INDEX[name], S).astype(np.float32)
 
 
-def oracle_step_time(oracle, mi, logits_bits, targets, old_logp, adv, mask, seg, S, Ns, inv, rows: int):
-    """Times the oracle, as it stands, on (full merge) + (the first `rows` rows of the loss micro-batch).
-    Returns (t_merge, t_loss_rows, n_unmasked_in_rows)."""
-    t0 = time.perf_counter()
-    oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp, oracle.OWNER_LONGEST)
-    t1 = time.perf_counter()
-    rid = np.arange(rows, dtype=np.int64)
-    oracle.policy_loss(logits_bits[:rows], targets, old_logp, adv, mask, seg, S, float(np.float32(EPS[0])),
-                       float(np.float32(EPS[1])), seg_denom=Ns, inv_num_segs=inv, row_ids=rid, want_dlogits=True,
-                       logits_is_bf16_bits=True)
-    t2 = time.perf_counter()
-    return t1 - t0, t2 - t1, int(mask[:rows].sum())
+def fracs(gbs: float, peak: float) -> dict:
+    return {"gb_per_s": gbs, "frac_of_measured": gbs / peak, "frac_of_nominal_8tbs": gbs / NOMINAL_HBM_GBS}
 
 
-def extrapolated_gbs(n, N_in, N_out, T, n_unmasked_full, t_merge, t_loss_rows, rows, n_unmasked_rows):
-    """Loss rows are independent: the micro-batch's loss time is extrapolated from the sample at the sample's
-    algorithmic byte rate; the merge is timed in full."""
-    rate = loss_bytes(rows, V, n_unmasked_rows) / max(t_loss_rows, 1e-9)
-    t_step = t_merge + loss_bytes(T, V, n_unmasked_full) / rate
-    return (merge_bytes(n, N_in, N_out) + loss_bytes(T, V, n_unmasked_full)) / t_step / 1e9, t_step
+class Batch:
+    """One batch resident on the device: merge inputs, merge outputs, and the packed per-token loss inputs the bridge
+    derives from them (ajt_pack_loss_inputs + ajt_segment_counts).  All of it through the library's calls."""
+
+    def __init__(self, torch, ajt, W, name, mi, seed, dev, stream, tl_seg=None, S=None):
+        self.torch, self.ajt, self.name, self.mi, self.stream = torch, ajt, name, mi, stream
+        d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+        self.tokens, self.offsets, self.traj, self.rs, self.lp = d(mi.tokens), d(mi.offsets), d(mi.traj_ids), d(mi.resp_start), d(mi.old_logp)
+        if tl_seg is None:
+            uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
+            S = int(uniq.shape[0])
+        self.S = S
+        self.tl_seg_h = tl_seg.astype(np.int32)
+        self.seg_adv_h = seg_advantages(W, name, seed, S)
+        self.tl_seg, self.seg_adv = d(self.tl_seg_h), d(self.seg_adv_h)
+        self.Ns = torch.zeros(S, dtype=torch.float32, device=dev)
+        with torch.cuda.stream(stream):
+            self.mout = ajt.merge_timelines(self.tokens, self.offsets, self.traj, self.rs, None, self.lp,
+                                            owner_rule=ajt.OWNER_LONGEST, stream=stream)
+            self.pk = ajt.pack_loss_inputs(self.mout, self.tl_seg, S, self.seg_adv, stream=stream)
+            stream.synchronize()
+        st = ajt.last_status(self.mout.workspace, stream)
+        assert st == 0, f"{name}: merge status {st}"
+        self.fin = self.mout.finalize()
+        self.n, self.N_in, self.N_out, self.M = mi.n, mi.n_tokens, self.fin.N_out, self.fin.M
+        self.mask_all, self.seg_all = self.pk.mask[:self.N_out], self.pk.seg_ids[:self.N_out]
+        with torch.cuda.stream(stream):
+            ajt.segment_counts(self.mask_all, self.seg_all, S, out=self.Ns, stream=stream)
+            stream.synchronize()
+
+    def merge(self):
+        self.ajt.merge_timelines(self.tokens, self.offsets, self.traj, self.rs, None, self.lp, owner_rule=self.ajt.OWNER_LONGEST,
+                                 out=self.mout, stream=self.stream)
+
+    def bridge(self, accumulate_into=None):
+        self.ajt.pack_loss_inputs(self.mout, self.tl_seg, self.S, self.seg_adv, out=self.pk, stream=self.stream)
+        self.ajt.segment_counts(self.mask_all, self.seg_all, self.S, out=self.Ns, stream=self.stream)
+
+    def rows(self, a: int, b: int) -> dict:
+        pk = self.pk
+        return dict(targets=pk.targets[a:b], mask=pk.mask[a:b], seg=pk.seg_ids[a:b], adv=pk.adv[a:b],
+                    n_unmasked=int(pk.mask[a:b].sum().item()), T=b - a)
+
+    def check_pack_against_oracle(self, oracle, n_seq: int = 24):
+        """The device bridge against oracle.pack_loss_inputs on the first merged sequences (reading L-12)."""
+        f, cpu = self.fin, (lambda t: t.cpu().numpy())
+        m = min(n_seq, f.M)
+        off = cpu(f.merged_offsets[:m + 1])
+        No = int(off[-1])
+        t, mk, lp, sg, av = oracle.pack_loss_inputs(cpu(f.merged_tokens[:No]), cpu(f.merged_mask[:No]), cpu(f.merged_old_logp[:No]),
+                                                    off, cpu(f.merged_origin[:m]), self.tl_seg_h, self.seg_adv_h)
+        pk = self.pk
+        assert np.array_equal(cpu(pk.targets[:No]), t) and np.array_equal(cpu(pk.mask[:No]), mk)
+        assert np.array_equal(cpu(pk.seg_ids[:No]), sg) and np.array_equal(cpu(pk.adv[:No]), av)
+        assert np.array_equal(cpu(pk.old_logp[:No]), lp)
 
 
-# ----------------------------------------------------------------------------------------- reference arm (oracle)
+def noise_for(W, seed: int, key: int, T: int, sigma: float = 0.05) -> np.ndarray:
+    return (W.rng_for(seed, CFG_INDEX.get("c2", 1), 99 + key).standard_normal(T) * sigma).astype(np.float32)
 
 
-def run_reference(args, rank: int):
-    """`--impl reference`: the CPU oracle as it stands, on the box's host cores, same config / metric / unit.
-    Each step = the full merge of the batch + a bounded sample of loss rows (the rest extrapolated; rows are
-    independent).  Under torchrun only rank 0 works."""
-    if rank != 0:
-        return
-    import torch
-
-    import oracle
-    from paper_2606_04484_b200 import workloads as W
-
-    oracle.build()
-    seed = W.BASE_SEED + 1
-    mi = W.merge_workload("c2", seed=seed)
-    r = oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp, oracle.OWNER_LONGEST)
-    targets, mask, seg, S, adv, Ns, inv = loss_side_inputs(W, r.merged_tokens, r.merged_mask, r.merged_old_logp,
-                                                           r.merged_offsets, r.merged_traj, seed)
-    T = min(args.loss_rows, r.N_out)
-    targets, mask, seg, adv = targets[:T], mask[:T], seg[:T], adv[:T]
-    rows_max = 1024
-    g = torch.Generator().manual_seed(seed)
-    logits = (torch.randn((rows_max, V), generator=g) * 3.0).to(torch.bfloat16)
-    noise = (W.rng_for(seed, 1, 99).standard_normal(T) * 0.05).astype(np.float32)
-    old = np.zeros(T, np.float32)
-    old[:rows_max] = harness_old_logp(torch, logits, torch.from_numpy(targets[:rows_max]), noise[:rows_max]).numpy()
-    bits = logits.view(torch.int16).numpy().view(np.uint16)
-    # calibrate: size the per-step sample so that warmup + steps stay within ~2 minutes
-    tm, tl, nu = oracle_step_time(oracle, mi, bits, targets, old, adv, mask, seg, S, Ns, inv, 64)
-    budget = 120.0 / max(1, args.steps + args.warmup)
-    rows = int(min(rows_max, max(64, 64 * max(0.0, budget - tm) / max(tl, 1e-6))))
-    for _ in range(args.warmup):
-        oracle_step_time(oracle, mi, bits, targets, old, adv, mask, seg, S, Ns, inv, rows)
-    t_m = t_l = 0.0
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        a, b, nu = oracle_step_time(oracle, mi, bits, targets, old, adv, mask, seg, S, Ns, inv, rows)
-        t_m += a
-        t_l += b
-    wall = time.perf_counter() - t0
-    K = max(1, args.steps)
-    val, t_step = extrapolated_gbs(mi.n, mi.n_tokens, r.N_out, T, int(mask.sum()), t_m / K, t_l / K, rows, nu)
-    cores = oracle.num_threads()
-    sample = (f"per step: full merge of the batch ({mi.n} timelines, {mi.n_tokens} tokens) + first {rows} of {T} loss rows "
-              f"({nu} unmasked) x V={V}; micro-batch time extrapolated at the sample's byte rate (rows are independent)")
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64 (oracle)", "data": "synthetic",
-            "config": workload_config(mi.n, mi.n_tokens, r.N_out, T, float(mask.mean())),
-            "cpu_baseline": {"value": val, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample,
-                             "measured_wall_s": wall},
-            "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0}
-    print(json.dumps(line), flush=True)
-
-
-def workload_config(n, N_in, N_out, T, rho):
-    return {"workload": "BASELINE.json configs[1] single-model GRPO batch: merge of 64 trajectories x 8 turns "
-                        f"({n} timelines, N_in={N_in}, N_out={N_out}) + policy-loss fwd+bwd over one micro-batch "
-                        f"[{T},{V}] bf16 of the merged tokens (mask density {rho:.3f}), eps 0.2/0.28, group z-score adv",
-            "owner_rule": "longest", "loss_rows": T, "vocab": V, "merge_timelines": n, "N_in": N_in, "N_out": N_out,
-            "l2": "inputs larger than L2: every step streams the 12.4 GB logits micro-batch (two buffers alternate), "
-                  "which also evicts the 7 MB merge input between merge calls"}
+def oracle_merge_times(oracle, mi) -> dict:
+    """The brute-force merge oracle on the host cores: one thread, then all of them."""
+    allc = oracle.num_threads()
+    out = {}
+    for nm, nt in (("one_thread", 1), ("all_cores", allc)):
+        oracle.set_threads(nt)
+        t0 = time.perf_counter()
+        oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp, oracle.OWNER_LONGEST)
+        out[nm + "_ms"] = (time.perf_counter() - t0) * 1e3
+    oracle.set_threads(allc)
+    out["cores"] = allc
+    return out
 
 
 # ----------------------------------------------------------------------------------------- our arm (CUDA)
@@ -228,6 +224,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     import torch.distributed as dist
 
     import paper_2606_04484_b200 as ajt
+    from paper_2606_04484_b200 import shard as SH
     from paper_2606_04484_b200 import workloads as W
 
     if not torch.cuda.is_available():
@@ -237,90 +234,72 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     ajt.lib()  # fail loudly if libajt.so is missing
-
-    # ---- inputs (seeded, synthetic; weak scaling: every rank owns its own batch)
-    seed = W.BASE_SEED + 1 + 1000 * rank
-    mi = W.merge_workload("c2", seed=seed)
-    d = lambda a: torch.from_numpy(a).to(dev)
-    tokens, offsets, traj, rs, lp = d(mi.tokens), d(mi.offsets), d(mi.traj_ids), d(mi.resp_start), d(mi.old_logp)
+    peak, peak_src = measured_peak()
     stream = torch.cuda.Stream(dev)
-    with torch.cuda.stream(stream):
-        mout = ajt.merge_timelines(tokens, offsets, traj, rs, None, lp, owner_rule=ajt.OWNER_LONGEST)
-        stream.synchronize()
-        assert ajt.last_status(mout.workspace) == 0
-        fin = mout.finalize()
-    n, N_in, N_out, M = mi.n, mi.n_tokens, fin.N_out, fin.M
-    cpu = lambda t: t.cpu().numpy()
-    targets, mask, seg, S, adv, Ns, inv = loss_side_inputs(W, cpu(fin.merged_tokens), cpu(fin.merged_mask),
-                                                           cpu(fin.merged_old_logp), cpu(fin.merged_offsets),
-                                                           cpu(fin.merged_traj), seed)
-    T = min(args.loss_rows, N_out)
-    n_mb = 2 if N_out >= 2 * T else 1
-    Ns_d = d(Ns)
-    mbs = []
-    for k in range(n_mb):
-        sl = slice(k * T, (k + 1) * T)
-        logits = torch.empty((T, V), dtype=torch.bfloat16, device=dev)
-        fill_logits(torch, logits, seed * 7 + k)
-        tg = d(targets[sl].copy())
-        noise = (W.rng_for(seed, 1, 99 + k).standard_normal(T) * 0.05).astype(np.float32)
-        old = harness_old_logp(torch, logits, tg, noise)
-        mbs.append(dict(logits=logits, targets=tg, old=old, adv=d(adv[sl].copy()), mask=d(mask[sl].copy()),
-                        seg=d(seg[sl].copy()), n_unmasked=int(mask[sl].sum())))
-    dlogits = torch.empty((T, V), dtype=torch.bfloat16, device=dev)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+
+    # ---- the batch (seeded, synthetic).  N > 1: ONE batch split by trajectory groups, every rank keeps its share
+    seed = W.BASE_SEED + CFG_INDEX[HEADLINE]
+    mi_full = merge_inputs(W, HEADLINE, seed)
+    uniq, tl_seg_full = np.unique(mi_full.traj_ids, return_inverse=True)
+    S = int(uniq.shape[0])
+    if world > 1:
+        sh = SH.shard_merge_inputs(mi_full.tokens, mi_full.offsets, mi_full.traj_ids, mi_full.resp_start, None, mi_full.old_logp,
+                                   rank=rank, world=world)
+        mi = W.MergeInputs(sh.tokens, sh.offsets, sh.traj_ids, sh.resp_start, sh.old_logp)
+        tl_seg = tl_seg_full[sh.index]
+    else:
+        mi, tl_seg = mi_full, tl_seg_full
+    B = Batch(torch, ajt, W, HEADLINE, mi, seed, dev, stream, tl_seg=tl_seg, S=S)
+    T = min(args.loss_rows, B.N_out)
+    n_ch = 2 if B.N_out >= 2 * T else 1
+    big_rows = 131072 if (world == 1 and not args.no_configs) else T   # the largest configs[4] cell shares the buffers
+    logits_big = torch.empty((big_rows, V), dtype=torch.bfloat16, device=dev)
+    dlogits_big = torch.empty((big_rows, V), dtype=torch.bfloat16, device=dev)
+    fill_logits(logits_big, seed * 7 + rank)
+    logits, dlogits = logits_big[:T], dlogits_big[:T]
+    chunks = []
+    for k in range(n_ch):
+        r = B.rows(k * T, (k + 1) * T)
+        r["old"] = harness_old_logp(logits, r["targets"], noise_for(W, seed, k, T))   # input synthesis: new logp + N(0, 0.05)
+        chunks.append(r)
+    Ns_loc = B.Ns                                      # this rank's per-trajectory counts; all-reduced inside the step
+    Ns_glob = torch.zeros_like(Ns_loc)
+    loss_acc = torch.zeros(1, dtype=torch.float64, device=dev)
     lout = None
-    # The stages are chained on the device: the merge's outputs feed ajt_pack_loss_inputs (next-token alignment, segment ids,
-    # advantages: reading L-12), ajt_segment_counts gives the batch-wide N_s (reading L-4), and the loss call reads the
-    # micro-batch's rows of those arrays.  Nothing goes through the host inside a step.  (`old` was synthesised in the set-up
-    # from the same targets: input synthesis, BASELINE.json configs.)
-    uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
-    assert int(uniq.shape[0]) == S
-    tl_seg_d = d(tl_seg.astype(np.int32))
-    seg_adv_d = d(W.advantages_group_zscore(seed, 1, S).astype(np.float32))
-    with torch.cuda.stream(stream):
-        pk = ajt.pack_loss_inputs(mout, tl_seg_d, S, seg_adv_d, stream=stream)
-        stream.synchronize()
-    for k in range(n_mb):       # the device chain reproduces the set-up's host arrays bit for bit
-        sl = slice(k * T, (k + 1) * T)
-        assert torch.equal(pk.targets[sl], mbs[k]["targets"]) and torch.equal(pk.mask[sl], mbs[k]["mask"])
-        assert torch.equal(pk.seg_ids[sl], mbs[k]["seg"]) and torch.equal(pk.adv[sl], mbs[k]["adv"])
-        mbs[k].update(targets=pk.targets[sl], mask=pk.mask[sl], seg=pk.seg_ids[sl], adv=pk.adv[sl])
-    pk_mask_all, pk_seg_all = pk.mask[:N_out], pk.seg_ids[:N_out]
 
     def step(k: int, ev=None):
         nonlocal lout
-        mb = mbs[k % n_mb]
+        ch = chunks[k % n_ch]
         if ev:
             ev[0].record(stream)
-        ajt.merge_timelines(tokens, offsets, traj, rs, None, lp, owner_rule=ajt.OWNER_LONGEST, out=mout, stream=stream)
+        B.merge()
         if ev:
             ev[1].record(stream)
-        ajt.pack_loss_inputs(mout, tl_seg_d, S, seg_adv_d, out=pk, stream=stream)
-        ajt.segment_counts(pk_mask_all, pk_seg_all, S, out=Ns_d, stream=stream)
-        if ev:
-            ev[3].record(stream)
-        lout = ajt.policy_loss_fwd_bwd(mb["logits"], mb["targets"], mb["old"], mb["adv"], mb["mask"], mb["seg"], S, EPS[0],
-                                       EPS[1], seg_denom=Ns_d, inv_num_segs=inv, dlogits=dlogits, out=lout, stream=stream)
+        B.bridge()
+        Ns_glob.copy_(Ns_loc)
+        if world > 1:
+            dist.all_reduce(Ns_glob)                   # N_s over the whole batch (kilobytes)
         if ev:
             ev[2].record(stream)
+        lout = ajt.policy_loss_fwd_bwd(logits, ch["targets"], ch["old"], ch["adv"], ch["mask"], ch["seg"], S, EPS[0], EPS[1],
+                                       seg_denom=Ns_glob, inv_num_segs=0.0, dlogits=dlogits, out=lout, stream=stream)
+        if ev:
+            ev[3].record(stream)
+        if world > 1:
+            loss_acc.copy_(lout.loss.double())
+            dist.all_reduce(loss_acc)                  # the scalar (one double)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    def max_over_ranks(x: float) -> float:
+    def reduce_ranks(x: float, op) -> float:
         if world == 1:
             return x
         t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t[0])
-
-    def sum_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        dist.all_reduce(t, op=op)
         return float(t[0])
 
     K, Wm = args.steps, args.warmup
@@ -334,6 +313,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
+        l0 = ajt.launch_count()
         tw0 = time.time()
         e0.record(stream)
         for k in range(K):
@@ -341,20 +321,21 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         e1.record(stream)
         barrier()
         tw1 = time.time()
-    total_ms = max_over_ranks(e0.elapsed_time(e1))
+        launches = ajt.launch_count() - l0
+    total_ms = reduce_ranks(e0.elapsed_time(e1), dist.ReduceOp.MAX if world > 1 else None)
     merge_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
-    bridge_ms = float(np.mean([e[1].elapsed_time(e[3]) for e in evs]))
-    loss_ms = float(np.mean([e[3].elapsed_time(e[2]) for e in evs]))
-    assert ajt.last_status(mout.workspace) == 0 and ajt.last_status(lout.workspace) == 0
+    bridge_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    loss_ms = float(np.mean([e[2].elapsed_time(e[3]) for e in evs]))
+    assert ajt.last_status(B.mout.workspace) == 0 and ajt.last_status(lout.workspace) == 0
     clocks = sampler.summary(tw0, tw1)
 
-    b_merge = merge_bytes(n, N_in, N_out)
-    b_loss = [loss_bytes(T, V, mb["n_unmasked"]) for mb in mbs]
-    step_bytes = float(np.mean([b_merge + b_loss[k % n_mb] for k in range(K)]))
-    loss_b = float(np.mean([b_loss[k % n_mb] for k in range(K)]))
+    b_merge = merge_bytes(B.n, B.N_in, B.N_out)
+    b_loss = [loss_bytes(T, V, ch["n_unmasked"]) for ch in chunks]
+    step_bytes = float(np.mean([b_merge + b_loss[k % n_ch] for k in range(K)]))
+    loss_b = float(np.mean([b_loss[k % n_ch] for k in range(K)]))
     ms_per_step = total_ms / K
-    value = sum_over_ranks(step_bytes) / (ms_per_step * 1e-3) / 1e9
-    peak, peak_src = measured_peak()
+    value = reduce_ranks(step_bytes, dist.ReduceOp.SUM if world > 1 else None) / (ms_per_step * 1e-3) / 1e9
+    rho = float(np.mean([ch["n_unmasked"] for ch in chunks]) / T)
 
     # ---- HBM ceilings of this box, measured now with the library's probe kernels; dlogits is scratch here
     ceilings = None
@@ -374,52 +355,62 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                     best = min(best, a0.elapsed_time(a1))
             return moved / (best * 1e-3) / 1e9
 
-        ceilings = {"read_gb_per_s": probe(0, sink, mbs[0]["logits"], nb), "write_gb_per_s": probe(1, dlogits, None, nb),
-                    "memset_gb_per_s": probe(3, dlogits, None, nb), "copy_gb_per_s": probe(2, dlogits, mbs[0]["logits"], 2 * nb),
-                    "bytes": nb, "how": "ajt_hbm_probe (16-byte loads / stores over the 12.4 GB logits / dlogits buffers, best of 4)"}
+        ceilings = {"read_gb_per_s": probe(0, sink, logits, nb), "write_gb_per_s": probe(1, dlogits, None, nb),
+                    "memset_gb_per_s": probe(3, dlogits, None, nb), "copy_gb_per_s": probe(2, dlogits, logits, 2 * nb),
+                    "bytes": nb, "how": "ajt_hbm_probe (16-byte loads / stores over the logits / dlogits chunk buffers, best of 4)"}
 
     # ---- e2e: the *_host C-ABI calls, pinned HOST buffers, H2D + D2H inside the timed region
     e2e = None
     if not args.no_e2e:
-        e2e = run_e2e(torch, ajt, mi, mbs[0], S, Ns, inv, T, dev, stream, K, Wm, b_merge + b_loss[0], barrier,
-                      max_over_ranks, sum_over_ranks)
+        e2e = run_e2e(torch, ajt, mi, B, chunks[0], logits, dlogits, S, T, dev, stream, K, Wm, b_merge, barrier, reduce_ranks,
+                      dist, world)
     sampler.stop()
 
-    cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu:
-        cpu_baseline = run_cpu_baseline(torch, mi, mbs[0], targets[:T], mask[:T], seg[:T], adv[:T], S, Ns, inv, T, n, N_in,
-                                        N_out)
+    cpu_baseline, cfg_records = None, None
+    if rank == 0 and not args.no_cpu:
+        cpu_baseline = run_cpu_baseline(torch, B, chunks[0], logits, S, T)
+    if rank == 0 and world == 1 and not args.no_configs:
+        cfg_records = run_config_records(torch, ajt, W, B, chunks[0], logits_big, dlogits_big, dev, stream, peak,
+                                         dict(merge_ms=merge_ms, loss_ms=loss_ms, T=T, rho=rho), with_oracle=not args.no_cpu)
 
     if rank == 0:
-        traffic = None
+        shape_key = f"loss_rows_kernel[{T}x{V},rho={rho:.2f}]"
+        traffic, traffic_note = None, None
         tp = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tp):
             try:
                 with open(tp) as f:
-                    traffic = json.load(f).get("loss_rows_kernel_dram_bytes_per_launch")
+                    tj = json.load(f)
+                ent = tj.get("shapes", {}).get(f"{T}x{V}")
+                if ent:
+                    traffic, traffic_note = ent.get("dram_bytes_per_launch"), ent.get("note")
             except Exception:
                 traffic = None
         ach = loss_b / (loss_ms * 1e-3) / 1e9
         mg = b_merge / (merge_ms * 1e-3) / 1e9
         line = {
             "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": K, "warmup": Wm,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak" if world == 1 else "strong",
+            "vs_baseline": None,
             "dtype": "f32 (bf16 logits/dlogits in HBM, fp64 scalar; merge int32/u64)", "data": "synthetic",
-            "config": workload_config(n, N_in, N_out, T, float(np.mean([mb["n_unmasked"] for mb in mbs]) / T)),
-            "merge": {"ms": merge_ms, "merged_gtokens_per_s": N_out / (merge_ms * 1e-3) / 1e9,
-                      "input_gtokens_per_s": N_in / (merge_ms * 1e-3) / 1e9, "gb_per_s": mg, "frac_of_measured": mg / peak,
-                      "frac_of_nominal_8tbs": mg / NOMINAL_HBM_GBS, "token_reduction_factor": N_in / N_out, "M": M,
-                      "algorithmic_bytes": b_merge},
+            "config": workload_config(mi_full.n, mi_full.n_tokens, B, T, rho, world),
+            "merge_c3": {"ms": merge_ms, "merged_gtokens_per_s": B.N_out / (merge_ms * 1e-3) / 1e9,
+                         "input_gtokens_per_s": B.N_in / (merge_ms * 1e-3) / 1e9, **fracs(mg, peak),
+                         "token_reduction_factor": B.N_in / B.N_out, "M": B.M, "n": B.n, "N_in": B.N_in, "N_out": B.N_out,
+                         "algorithmic_bytes": b_merge, "target": "north_star: >= 0.40 of the nominal 8 TB/s"},
             "bridge": {"ms": bridge_ms, "what": "ajt_pack_loss_inputs over the N_out merged tokens + ajt_segment_counts "
-                       "(device-resident chain between the stages; its bytes are not counted in `value`)"},
+                       "(device-resident chain between the stages" + (", then the NCCL all-reduce of N_s" if world > 1 else "") +
+                       "; its bytes are not counted in `value`)"},
             "loss": {"ms": loss_ms, "logits_gb_per_s": ach, "frac_of_measured": ach / peak,
                      "frac_of_nominal_8tbs": ach / NOMINAL_HBM_GBS, "algorithmic_bytes": loss_b,
-                     "dense_2TV_gb_per_s": 4.0 * T * V / (loss_ms * 1e-3) / 1e9},
-            "roofline": {"bound": "hbm", "kernel": "loss_rows_kernel (timed as the ajt_policy_loss_fwd_bwd call: prep + rows + "
-                         "final launches; rows is >99% of it, profiles/)", "achieved": ach, "peak": peak, "unit": "GB/s",
-                         "frac": ach / peak, "traffic": traffic, "peak_source": peak_src},
-            "hbm_ceilings": ceilings, "clocks": clocks, "gpu_launches": K * (6 + 1 + 1 + 3),   # merge 6, pack 1, segment counts 1, loss 3 (prep, rows, final)
-            "e2e": e2e, "cpu_baseline": cpu_baseline,
+                     "dense_2TV_gb_per_s": 4.0 * T * V / (loss_ms * 1e-3) / 1e9, "mask_density": rho},
+            "roofline": {"bound": "hbm", "kernel": shape_key + " (timed as the ajt_policy_loss_fwd_bwd call: prep + rows + final "
+                         "launches; rows is >99% of it, profiles/)", "achieved": ach, "peak": peak, "unit": "GB/s",
+                         "frac": ach / peak, "traffic": traffic, "traffic_note": traffic_note, "peak_source": peak_src},
+            "hbm_ceilings": ceilings, "clocks": clocks, "gpu_launches": int(launches),
+            "gpu_launches_how": "counted by the library (ajt_launch_count before / after the timed region): merge 6, pack 1, "
+                                "segment counts 1, loss 3 per step",
+            "e2e": e2e, "cpu_baseline": cpu_baseline, "configs": cfg_records,
             "paper_context": "paper reports only end-to-end actor-update 2160 s -> 346 s (6.25x) with merging on AppWorld, "
                              "8-GPU node at most, GPU model and precision not stated (PAPER.md:373,395); not comparable",
         }
@@ -429,18 +420,50 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         dist.destroy_process_group()
 
 
-def run_e2e(torch, ajt, mi, mb, S, Ns, inv, T, dev, stream, K, Wm, step_bytes, barrier, max_over_ranks, sum_over_ranks):
-    """Same step through ajt_merge_timelines_host + ajt_policy_loss_fwd_bwd_host: every input starts in pinned HOST
-    memory and every output ends there; the copies run inside the timed region."""
+def workload_config(n, N_in, B, T, rho, world):
+    return {"workload": "BASELINE.json configs[2] long-horizon agent (the largest single-GPU configuration): merge of 256 "
+                        f"trajectories x 20-40 turns ({n} timelines, N_in={N_in}, contexts to 32k tokens, Zipf(1.1) tokens) + "
+                        f"policy-loss fwd+bwd over one chunk [{T},{V}] bf16 of the merged tokens with the merge's own targets / "
+                        f"mask / segments (mask density {rho:.3f}), eps 0.2/0.28, group z-score advantages"
+                        + (f"; the batch is split over {world} ranks by trajectory group, this record describes rank 0's share "
+                           f"(n={B.n}, N_in={B.N_in})" if world > 1 else ""),
+            "owner_rule": "longest", "loss_rows": T, "vocab": V, "merge_timelines": n, "N_in": N_in, "N_out": B.N_out,
+            "parallelism": "single GPU" if world == 1 else f"dp{world}: groups -> ranks, all-reduce of N_s and of the scalar",
+            "l2": "inputs larger than L2: every step streams the 277 MB token array and a 19.9 GB logits chunk (126 MB L2)"}
+
+
+def mem_available_gb() -> float:
+    try:
+        with open("/proc/meminfo") as f:
+            for ln in f:
+                if ln.startswith("MemAvailable:"):
+                    return float(ln.split()[1]) / 1e6
+    except Exception:
+        pass
+    return 0.0
+
+
+def run_e2e(torch, ajt, mi, B, ch, logits, dlogits, S, T, dev, stream, K, Wm, b_merge, barrier, reduce_ranks, dist, world):
+    """Same step through ajt_merge_timelines_host + ajt_policy_loss_fwd_bwd_host2: every input starts in pinned HOST memory;
+    the merge's outputs and the loss / status come back to the host; the gradient stays on the device (where the backward
+    pass continues).  The copies run inside the timed region.  The logits chunk needs T x V x 2 bytes of pinned host memory:
+    on a box without that much the leg uses as many rows as fit and says so."""
+    Te = T
+    need_gb = T * V * 2 / 1e9 + 4.0
+    if mem_available_gb() < need_gb + 8.0:
+        Te = max(1024, min(T, int((mem_available_gb() - 12.0) * 1e9 / (V * 2)) // 1024 * 1024))
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_tok, h_off, h_traj, h_rs, h_lp = pin(mi.tokens), pin(mi.offsets), pin(mi.traj_ids), pin(mi.resp_start), pin(mi.old_logp)
-    h_logits = torch.empty((T, V), dtype=torch.bfloat16, pin_memory=True)
-    h_logits.copy_(mb["logits"])
-    h_dlogits = torch.empty((T, V), dtype=torch.bfloat16, pin_memory=True)
-    h_vec = {k: mb[k].cpu().pin_memory() for k in ("targets", "old", "adv", "mask", "seg")}
-    h_Ns = pin(Ns)
+    h_logits = torch.empty((Te, V), dtype=torch.bfloat16, pin_memory=True)
+    h_logits.copy_(logits[:Te])
+    h_vec = {k: ch[k][:Te].cpu().pin_memory() for k in ("targets", "old", "adv", "mask", "seg")}
+    Ns = B.Ns.clone()
+    if world > 1:
+        dist.all_reduce(Ns)
+    h_Ns = Ns.cpu().pin_memory()
     m_arena = torch.empty(ajt.merge_host_arena_bytes(mi.n, mi.n_tokens), dtype=torch.uint8, device=dev)
-    l_arena = torch.empty(ajt.loss_host_arena_bytes(T, V, S, V, ajt.DT_BF16), dtype=torch.uint8, device=dev)
+    l_arena = torch.empty(ajt.loss_host_arena_bytes(Te, V, S, V, ajt.DT_BF16), dtype=torch.uint8, device=dev)
+    ctx = ajt.HostCtx()
     m_out = None
     res = {}
 
@@ -451,11 +474,11 @@ def run_e2e(torch, ajt, mi, mb, S, Ns, inv, T, dev, stream, K, Wm, step_bytes, b
         m_out = {k: r[k] for k in ("merged_tokens", "merged_mask", "merged_src", "merged_old_logp", "merged_offsets",
                                    "merged_origin", "merged_traj", "owner")}
         res["merge"] = r
-        res["loss"] = ajt.policy_loss_fwd_bwd_host(h_logits, h_vec["targets"], h_vec["old"], h_vec["adv"], h_vec["mask"],
-                                                   h_vec["seg"], S, EPS[0], EPS[1], ajt.DT_BF16, seg_denom=h_Ns,
-                                                   inv_num_segs=inv, dlogits=h_dlogits, arena=l_arena, stream=stream)
+        res["loss"] = ajt.policy_loss_fwd_bwd_host2(h_logits, h_vec["targets"], h_vec["old"], h_vec["adv"], h_vec["mask"],
+                                                    h_vec["seg"], S, EPS[0], EPS[1], ajt.DT_BF16, dlogits[:Te], seg_denom=h_Ns,
+                                                    inv_num_segs=0.0, want_logp=True, ctx=ctx, arena=l_arena, stream=stream)
 
-    Ke = max(1, min(K, args_e2e_steps(K)))
+    Ke = max(1, min(K, 5))   # each e2e step moves ~10 GB over PCIe
     with torch.cuda.stream(stream):
         for _ in range(min(Wm, 2)):
             step()
@@ -466,37 +489,42 @@ def run_e2e(torch, ajt, mi, mb, S, Ns, inv, T, dev, stream, K, Wm, step_bytes, b
             step()
         e1.record(stream)
         barrier()
-    ms = max_over_ranks(e0.elapsed_time(e1)) / Ke
+    ms = reduce_ranks(e0.elapsed_time(e1), dist.ReduceOp.MAX if world > 1 else None) / Ke
+    ctx.close()
     assert res["merge"]["status"] == 0 and res["loss"]["status"] == 0
     No, M, n, N = res["merge"]["N_out"], res["merge"]["M"], mi.n, mi.n_tokens
-    n_up = int(mb["n_unmasked"])   # the host call uploads only the rows the kernel reads (mask != 0)
-    h2d = 4 * N + 8 * (n + 1) + 4 * n + 4 * n + 4 * N + n_up * V * 2 + 17 * T + 4 * S
-    d2h = No * (4 + 1 + 4 + 4) + 8 * (M + 1) + 4 * M + 4 * M + 4 * n + 16 + 4 + T * V * 2 + 4 + 4
-    return {"value": sum_over_ranks(float(step_bytes)) / (ms * 1e-3) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": int(h2d),
-            "d2h_bytes_per_step": int(d2h), "ms_per_step": ms, "steps": Ke,
-            "api": "ajt_merge_timelines_host + ajt_policy_loss_fwd_bwd_host (pinned host buffers)",
+    n_up = int(h_vec["mask"].sum().item())   # the host call uploads only the rows the kernel reads (mask != 0)
+    step_bytes = b_merge + loss_bytes(Te, V, n_up)
+    h2d = 4 * N + 8 * (n + 1) + 4 * n + 4 * n + 4 * N + n_up * V * 2 + 17 * Te + 4 * S
+    d2h = No * (4 + 1 + 4 + 4) + 8 * (M + 1) + 4 * M + 4 * M + 4 * n + 16 + 4 + 4 + 4 * Te + 4
+    return {"value": reduce_ranks(float(step_bytes), dist.ReduceOp.SUM if world > 1 else None) / (ms * 1e-3) / 1e9, "unit": "GB/s",
+            "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": ms, "steps": Ke, "loss_rows": Te,
+            "api": "ajt_merge_timelines_host + ajt_policy_loss_fwd_bwd_host2 (pinned host buffers; merged sequences, loss, "
+                   "log-probs and status return to the host, dlogits stay on the device for the backward pass)",
+            "note": None if Te == T else f"host memory holds {Te} of the chunk's {T} logits rows pinned; the loss leg ran on those",
             "pcie_gb_per_s": (h2d + d2h) / (ms * 1e-3) / 1e9, "loss": res["loss"]["loss"]}
 
 
-def args_e2e_steps(K: int) -> int:
-    return max(1, min(K, 5))   # each e2e step moves ~25 GB over PCIe (~0.5-1 s)
-
-
-def run_cpu_baseline(torch, mi, mb, targets, mask, seg, adv, S, Ns, inv, T, n, N_in, N_out):
-    """The oracle as it stands on the GPU box's host cores, on a bounded sample (~10-30 s of CPU work): the full
-    merge of the batch + loss rows in slabs of 2048 until ~20 s are spent (the whole micro-batch if it gets there)."""
+def run_cpu_baseline(torch, B, ch, logits, S, T):
+    """The oracle as it stands on the GPU box's host cores, on a bounded sample (~10-30 s of CPU work): the full merge of
+    the batch + loss rows of the chunk in slabs of 1024 until ~15 s are spent; the rest of the chunk is extrapolated at the
+    sample's byte rate (rows are independent)."""
     import oracle
 
     oracle.build()
-    slab = 2048
-    old = mb["old"].cpu().numpy().astype(np.float32)
+    mi = B.mi
     t0 = time.perf_counter()
     oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp, oracle.OWNER_LONGEST)
     tm = time.perf_counter() - t0
-    tl, rows, nu = 0.0, 0, 0
-    while rows < T and tl < 20.0:
+    B.check_pack_against_oracle(oracle)
+    cpu = lambda t: t.cpu().numpy()
+    targets, mask, seg, adv, old = cpu(ch["targets"]), cpu(ch["mask"]), cpu(ch["seg"]), cpu(ch["adv"]), cpu(ch["old"])
+    Ns = cpu(B.Ns)
+    inv = float(np.float32(1.0 / max(1, int((Ns > 0).sum()))))
+    slab, tl, rows, nu = 1024, 0.0, 0, 0
+    while rows < T and tl < 15.0:
         b = min(T, rows + slab)
-        bits = mb["logits"][rows:b].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+        bits = logits[rows:b].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
         rid = np.arange(rows, b, dtype=np.int64)
         t0 = time.perf_counter()
         oracle.policy_loss(bits, targets, old, adv, mask, seg, S, float(np.float32(EPS[0])), float(np.float32(EPS[1])),
@@ -504,12 +532,181 @@ def run_cpu_baseline(torch, mi, mb, targets, mask, seg, adv, S, Ns, inv, T, n, N
         tl += time.perf_counter() - t0
         nu += int(mask[rows:b].sum())
         rows = b
-    val, t_step = extrapolated_gbs(n, N_in, N_out, T, int(mask.sum()), tm, tl, rows, nu)
-    how = "no extrapolation" if rows == T else "rest of the micro-batch extrapolated at the sample's byte rate"
+    rate = loss_bytes(rows, V, nu) / max(tl, 1e-9)
+    b_all = loss_bytes(T, V, int(mask.sum()))
+    t_step = tm + b_all / rate
+    val = (merge_bytes(B.n, B.N_in, B.N_out) + b_all) / t_step / 1e9
+    how = "no extrapolation" if rows == T else "rest of the chunk extrapolated at the sample's byte rate"
     return {"value": val, "unit": "GB/s", "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"full merge of the batch ({n} timelines, {N_in} tokens: {tm * 1e3:.1f} ms) + first {rows} of {T} loss rows "
+            "sample": f"full merge of the batch ({B.n} timelines, {B.N_in} tokens: {tm * 1e3:.0f} ms) + first {rows} of {T} loss rows "
                       f"({nu} unmasked) x V={V} in {tl:.2f} s, fp64 dlogits included; {how}",
             "est_ms_per_step": t_step * 1e3, "merge_ms": tm * 1e3}
+
+
+def run_config_records(torch, ajt, W, B3, ch3, logits_big, dlogits_big, dev, stream, peak, head, with_oracle=True):
+    """One compact record per BASELINE.json config (north_star "Report throughput ..."; SURVEY.md §8(d) "Reported per
+    config"): merge ms / merged tokens per s / GB/s / token-reduction factor, loss ms / logits GB/s, fractions of the measured
+    and nominal HBM rate, and the merge oracle's time on the host cores with one thread and with all of them.  Calls whose
+    inputs fit in the 126 MB L2 are timed cold (a 256 MB write before every repetition)."""
+    oracle = None
+    if with_oracle:
+        import oracle as _o
+        _o.build()
+        oracle = _o
+    flush = L2Flusher(dev)
+    L2 = 126 << 20
+    recs = {}
+
+    def time_med(fn, cold):
+        ms = time_calls(fn, stream, reps=5, warmup=2, flush=flush if cold else None)
+        return float(np.median(ms))
+
+    def loss_rec(lg, dl, targets, old, adv, mask, seg, S, Vv, eps, seg_denom=None):
+        T = int(lg.shape[0])
+        b_in = 2 if lg.dtype == torch.bfloat16 else 4
+        nu = int(mask.sum().item())
+        lo = None
+
+        def call():
+            nonlocal lo
+            lo = ajt.policy_loss_fwd_bwd(lg, targets, old, adv, mask, seg, S, eps[0], eps[1], seg_denom=seg_denom, inv_num_segs=0.0,
+                                         V=Vv, dlogits=dl, out=lo, stream=stream)
+        cold = T * Vv * b_in < L2
+        ms = time_med(call, cold)
+        assert ajt.last_status(lo.workspace, stream) == 0
+        b = loss_bytes(T, Vv, nu, b_in)
+        return {"T": T, "V": Vv, "dtype": "bf16" if b_in == 2 else "f32", "mask_density": nu / max(1, T), "ms": ms,
+                "algorithmic_bytes": b, **{("logits_" + k if k == "gb_per_s" else k): v for k, v in fracs(b / ms / 1e6, peak).items()},
+                "l2": "cold" if cold else "larger than L2"}
+
+    def merge_rec(Bx, ms=None):
+        cold = 4 * Bx.N_in * 2 < L2
+        if ms is None:
+            ms = time_med(Bx.merge, cold)
+        b = merge_bytes(Bx.n, Bx.N_in, Bx.N_out)
+        r = {"n": Bx.n, "N_in": Bx.N_in, "N_out": Bx.N_out, "M": Bx.M, "token_reduction_factor": Bx.N_in / max(1, Bx.N_out),
+             "ms": ms, "merged_gtokens_per_s": Bx.N_out / ms / 1e6, "input_gtokens_per_s": Bx.N_in / ms / 1e6, "algorithmic_bytes": b,
+             **fracs(b / ms / 1e6, peak), "l2": "cold" if cold else "larger than L2"}
+        if oracle is not None:
+            r["oracle_merge"] = oracle_merge_times(oracle, Bx.mi)
+        return r
+
+    # c3: the headline step's own measurements
+    recs["c3"] = {"what": CFG_WHAT["c3"], "merge": merge_rec(B3, head["merge_ms"]),
+                  "loss": {"T": head["T"], "V": V, "dtype": "bf16", "mask_density": head["rho"], "ms": head["loss_ms"],
+                           "algorithmic_bytes": loss_bytes(head["T"], V, ch3["n_unmasked"]),
+                           **{("logits_" + k if k == "gb_per_s" else k): v
+                              for k, v in fracs(loss_bytes(head["T"], V, ch3["n_unmasked"]) / head["loss_ms"] / 1e6, peak).items()},
+                           "l2": "larger than L2"}}
+    for name in ("c1", "c2", "c4A", "c4B"):
+        seed = W.BASE_SEED + CFG_INDEX[name]
+        Bx = Batch(torch, ajt, W, name, merge_inputs(W, name, seed), seed, dev, stream)
+        rec = {"what": CFG_WHAT[name], "merge": merge_rec(Bx)}
+        if name == "c1":
+            T = Bx.N_out
+            lg = torch.empty((T, 1024), dtype=torch.float32, device=dev)
+            g = torch.Generator(device=dev).manual_seed(seed)
+            lg.copy_(torch.randn((T, 1024), generator=g, device=dev) * 2.0)
+            dl, Vv = torch.empty((T, 1024), dtype=torch.bfloat16, device=dev), 1024
+        else:
+            T = min({"c2": 40960}.get(name, CHUNK_ROWS), Bx.N_out)
+            Vv = 128256 if name == "c4B" else V
+            lg, dl = logits_big[:T], dlogits_big[:T]
+        r = Bx.rows(0, T)
+        old = harness_old_logp(lg[:, :Vv] if lg.shape[1] != Vv else lg, r["targets"], noise_for(W, seed, 0, T))
+        rec["loss"] = loss_rec(lg, dl, r["targets"], old, r["adv"], r["mask"], r["seg"], Bx.S, Vv, CFG_EPS[name], seg_denom=Bx.Ns)
+        recs[name] = rec
+        del Bx
+    # c5: three cells of the loss sweep (smallest; V = 32,000 at mask density 0.7; largest)
+    for cell, (T, Vv, rho, S) in enumerate(((4096, 32000, 0.3, 8), (16384, 32000, 0.7, 64), (131072, V, 0.7, 512))):
+        if T > logits_big.shape[0]:
+            continue
+        lv = W.loss_sweep_vectors(T, Vv, S, rho, cell=cell)
+        dd = lambda a: torch.from_numpy(a).to(dev)
+        lg, dl = logits_big[:T], dlogits_big[:T]
+        tg = dd(lv.targets)
+        old = harness_old_logp(lg[:, :Vv] if Vv != V else lg, tg, lv.noise)
+        rec = loss_rec(lg, dl, tg, old, dd(lv.adv), dd(lv.mask), dd(lv.seg_ids), S, Vv, (0.2, 0.28))
+        rec["S"] = S
+        recs[f"c5[{T}x{Vv},rho={rho}]"] = {"what": "configs[4] loss sweep cell", "loss": rec}
+    return recs
+
+
+# ----------------------------------------------------------------------------------------- reference arm (oracle)
+
+
+def run_reference(args, rank: int):
+    """`--impl reference`: the CPU oracle as it stands, on the box's host cores, same config / metric / unit.  Each step =
+    the full merge of the batch + a bounded sample of the chunk's loss rows (the rest extrapolated: rows are independent).
+    Under torchrun only rank 0 works."""
+    if rank != 0:
+        return
+    import torch
+
+    import oracle
+    from paper_2606_04484_b200 import workloads as W
+
+    oracle.build()
+    seed = W.BASE_SEED + CFG_INDEX[HEADLINE]
+    mi = merge_inputs(W, HEADLINE, seed)
+    r = oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp, oracle.OWNER_LONGEST)
+    uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
+    S = int(uniq.shape[0])
+    seg_adv = seg_advantages(W, HEADLINE, seed, S)
+    targets, mask, _, seg, adv = oracle.pack_loss_inputs(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets,
+                                                         r.merged_origin, tl_seg.astype(np.int32), seg_adv)
+    Ns = np.bincount(seg, weights=mask.astype(np.float64), minlength=S).astype(np.float32)   # the oracle's step 4 input
+    inv = float(np.float32(1.0 / max(1, int((Ns > 0).sum()))))
+    T = min(args.loss_rows, r.N_out)
+    n_unm = int(mask[:T].sum())
+    rows_max = 512
+    g = torch.Generator().manual_seed(seed)
+    logits = (torch.randn((rows_max, V), generator=g) * 3.0).to(torch.bfloat16)
+    old = np.zeros(T, np.float32)
+    old[:rows_max] = harness_old_logp(logits, torch.from_numpy(targets[:rows_max]), noise_for(W, seed, 0, rows_max)).numpy()
+    bits = logits.view(torch.int16).numpy().view(np.uint16)
+
+    def one_step(rows):
+        t0 = time.perf_counter()
+        oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp, oracle.OWNER_LONGEST)
+        t1 = time.perf_counter()
+        oracle.policy_loss(bits[:rows], targets[:T], old, adv[:T], mask[:T], seg[:T], S, float(np.float32(EPS[0])),
+                           float(np.float32(EPS[1])), seg_denom=Ns, inv_num_segs=inv, row_ids=np.arange(rows, dtype=np.int64),
+                           want_dlogits=True, logits_is_bf16_bits=True)
+        return t1 - t0, time.perf_counter() - t1, int(mask[:rows].sum())
+
+    tm, tl, nu = one_step(32)
+    budget = 120.0 / max(1, args.steps + args.warmup)   # warm-up + steps stay within ~2 minutes
+    rows = int(min(rows_max, max(32, 32 * max(0.0, budget - tm) / max(tl, 1e-6))))
+    for _ in range(args.warmup):
+        one_step(rows)
+    t_m = t_l = 0.0
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        a, b, nu = one_step(rows)
+        t_m += a
+        t_l += b
+    wall = time.perf_counter() - t0
+    K = max(1, args.steps)
+    rate = loss_bytes(rows, V, nu) / max(t_l / K, 1e-9)
+    b_all = loss_bytes(T, V, n_unm)
+    t_step = t_m / K + b_all / rate
+    val = (merge_bytes(mi.n, mi.n_tokens, r.N_out) + b_all) / t_step / 1e9
+    cores = oracle.num_threads()
+    sample = (f"per step: full merge of the batch ({mi.n} timelines, {mi.n_tokens} tokens) + first {rows} of {T} loss rows "
+              f"({nu} unmasked) x V={V}; the chunk's time is extrapolated at the sample's byte rate (rows are independent)")
+
+    class _B:   # what workload_config reads
+        n, N_in, N_out = mi.n, mi.n_tokens, r.N_out
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64 (oracle)", "data": "synthetic",
+            "config": workload_config(mi.n, mi.n_tokens, _B, T, n_unm / T, 1),
+            "cpu_baseline": {"value": val, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample,
+                             "measured_wall_s": wall},
+            "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
 
 
 def main():
@@ -518,10 +715,11 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--loss-rows", type=int, default=MB_ROWS, help="rows of the loss micro-batch (profiling runs only; "
-                    "the default is the workload BASELINE.json names)")
+    ap.add_argument("--loss-rows", type=int, default=CHUNK_ROWS, help="rows of the loss chunk (profiling runs only; the default "
+                    "is the workload BASELINE.json names)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
-    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle legs (cpu_baseline, oracle merge times)")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config records")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
