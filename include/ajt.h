@@ -204,6 +204,16 @@ int ajt_pack_loss_inputs(
     int32_t* targets, uint8_t* mask, float* old_logp, int32_t* seg_ids, float* adv,
     uint32_t* status_bits, ajt_stream_t stream);
 
+/* Token-budget packing of the merged sequences into micro-batches, on the device ("the packed merged sequences",
+ * BASELINE.json north_star): consecutive sequences are taken in order while the rows of the
+ * micro-batch stay <= budget (a sequence longer than the budget gets a micro-batch of its own).  Micro-batch b is
+ * sequences mb_seq[b] .. mb_seq[b+1] = rows mb_row[b] .. mb_row[b+1] of the arrays ajt_pack_loss_inputs writes, so a loss
+ * call per micro-batch is a row range of them.  merged_offsets / counts: the merge call's (DEVICE).  mb_seq / mb_row:
+ * DEVICE [capacity], n_mb DEVICE [1]; entries up to n_mb (inclusive: the closing entry {M, N_out}) are written when
+ * n_mb < capacity (size them M + 1).  Enqueues on `stream`. */
+int ajt_pack_microbatches(const int64_t* merged_offsets, const int64_t* counts, int64_t budget, int32_t capacity,
+                          int32_t* mb_seq, int64_t* mb_row, int32_t* n_mb, ajt_stream_t stream);
+
 /* ------------------------------------------------------------------------------------------------
  * Stage (b): token-level clipped policy-gradient loss, forward and backward w.r.t. the logits.
  * Definition, for t in [0,T):

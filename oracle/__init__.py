@@ -16,7 +16,9 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "ajt_oracle.c")
-_SO = os.path.join(_HERE, "libajt_oracle.so")
+# AJT_ORACLE_SANITIZE=1 (tests/test_oracle_sanitize.py): a second build with -fsanitize=address,undefined next to the normal one
+_SAN = os.environ.get("AJT_ORACLE_SANITIZE") == "1"
+_SO = os.path.join(_HERE, "libajt_oracle_san.so" if _SAN else "libajt_oracle.so")
 
 OWNER_LONGEST = 0   # BASELINE.json north_star: longest surviving extender, then lowest index
 OWNER_PAPER = 1     # Algorithm 1 taken literally: the latest extender
@@ -29,7 +31,8 @@ _lib = None
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (building the checker is not using it)."""
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _SO, _SRC, "-lm"])
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"] if _SAN else ["-O2"]
+        subprocess.check_call(["gcc"] + flags + ["-fopenmp", "-shared", "-fPIC", "-o", _SO, _SRC, "-lm"])
     return _SO
 
 
@@ -272,6 +275,25 @@ def pack_loss_inputs(merged_tokens, merged_mask, merged_old_logp, merged_offsets
     if rc != 0:
         raise ValueError("ajt_oracle_pack: invalid offsets")
     return targets, mask, olp, seg, adv
+
+
+def pack_microbatches(lengths, budget: int):
+    """Token-budget packing of consecutive merged sequences ("packed merged sequences", BASELINE.json north_star; DESIGN.md
+    reading L-12): walk the sequences in order, open a new micro-batch whenever the next sequence would push the current one
+    over `budget` rows (a sequence longer than the budget gets a micro-batch of its own).  Returns the list of
+    (first_sequence, one_past_last_sequence)."""
+    if budget < 1:
+        raise ValueError("budget must be >= 1")
+    out, a, used = [], 0, 0
+    for k, L in enumerate(lengths):
+        L = int(L)
+        if used > 0 and used + L > budget:
+            out.append((a, k))
+            a, used = k, 0
+        used += L
+    if len(lengths) > a:
+        out.append((a, len(lengths)))
+    return out
 
 
 def lm_head_logp(hidden_bits, weight_bits, targets, mask=None, round_logits_bf16: bool = False):

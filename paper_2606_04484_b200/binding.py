@@ -26,7 +26,7 @@ _EXPORTS = [
     "ajt_merge_workspace_bytes", "ajt_merge_workspace_bytes_for_pairs", "ajt_merge_timelines", "ajt_merge_host_arena_bytes", "ajt_merge_timelines_host",
     "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
     "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks_workspace_bytes", "ajt_merge_blocks",
-    "ajt_pack_loss_inputs", "ajt_lm_head_workspace_bytes", "ajt_lm_head_logp",
+    "ajt_pack_loss_inputs", "ajt_pack_microbatches", "ajt_lm_head_workspace_bytes", "ajt_lm_head_logp",
     "ajt_hbm_probe", "ajt_launch_count", "ajt_host_ctx_create", "ajt_host_ctx_destroy", "ajt_policy_loss_fwd_bwd_host2",
 ]
 
@@ -74,7 +74,7 @@ def lib():
         L.ajt_loss_host_arena_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32]
         for f in ("ajt_merge_timelines", "ajt_merge_timelines_host", "ajt_policy_loss_fwd_bwd",
                   "ajt_policy_loss_fwd_bwd_host", "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks",
-                  "ajt_pack_loss_inputs", "ajt_lm_head_logp", "ajt_hbm_probe", "ajt_host_ctx_create",
+                  "ajt_pack_loss_inputs", "ajt_pack_microbatches", "ajt_lm_head_logp", "ajt_hbm_probe", "ajt_host_ctx_create",
                   "ajt_policy_loss_fwd_bwd_host2"):
             getattr(L, f).restype = C.c_int
         L.ajt_launch_count.restype = C.c_uint64
@@ -334,6 +334,25 @@ def pack_loss_inputs(mo, tl_seg: torch.Tensor, S: int, seg_adv: Optional[torch.T
     if rc != 0:
         raise AjtError(rc, "ajt_pack_loss_inputs")
     return out
+
+
+def pack_microbatches(mo, budget: int, stream=None):
+    """ajt_pack_microbatches (include/ajt.h): token-budget packing of the merged sequences.  Returns device tensors
+    (mb_seq int32 [n+2], mb_row int64 [n+2], n_mb int32 [1]); entries 0 .. n_mb are defined."""
+    _require_cuda()
+    counts = mo.counts
+    if counts.numel() == 3:
+        counts = torch.stack((counts[0], counts[2]))
+    cap = int(mo.merged_offsets.numel()) + 1
+    dev = mo.merged_offsets.device
+    mb_seq = torch.empty(cap, dtype=torch.int32, device=dev)
+    mb_row = torch.empty(cap, dtype=torch.int64, device=dev)
+    n_mb = torch.zeros(1, dtype=torch.int32, device=dev)
+    rc = lib().ajt_pack_microbatches(_dp(mo.merged_offsets), _dp(counts), C.c_int64(int(budget)), C.c_int32(cap), _dp(mb_seq),
+                                     _dp(mb_row), _dp(n_mb), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_pack_microbatches")
+    return mb_seq, mb_row, n_mb
 
 
 def merge_timelines_host(tokens, offsets, traj_ids, resp_start=None, mask_in=None, old_logp_in=None,

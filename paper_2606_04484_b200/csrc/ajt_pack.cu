@@ -120,7 +120,57 @@ __global__ void __launch_bounds__(256) pack_loss_inputs_kernel(const PackParams 
     }
 }
 
+// Token-budget packing (north_star "packed merged sequences"): consecutive merged sequences go into
+// micro-batches of at most `budget` rows, greedily and in order (a sequence longer than the budget gets a micro-batch of
+// its own).  The recurrence is sequential in the sequences, so one CTA stages the offsets in shared memory (coalesced) and
+// one thread walks them; M is a few thousand at most in the configs (micro-seconds).
+constexpr int kMbStage = 4096;
+__global__ void __launch_bounds__(1024) pack_microbatches_kernel(const int64_t* __restrict__ merged_offsets, const int64_t* __restrict__ counts,
+                                                                 int64_t budget, int32_t cap, int32_t* __restrict__ mb_seq,
+                                                                 int64_t* __restrict__ mb_row, int32_t* __restrict__ n_mb) {
+    __shared__ int64_t s_off[kMbStage + 1];
+    __shared__ int64_t s_used;
+    __shared__ int s_nmb;
+    const int64_t M = counts[0];
+    if (threadIdx.x == 0) { s_used = 0; s_nmb = 0; }
+    __syncthreads();
+    for (int64_t m0 = 0; m0 < M; m0 += kMbStage) {
+        const int cn = (int)min((int64_t)kMbStage, M - m0);
+        for (int x = threadIdx.x; x <= cn; x += blockDim.x) s_off[x] = merged_offsets[m0 + x];
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int64_t used = s_used;
+            int nmb = s_nmb;
+            for (int x = 0; x < cn; ++x) {
+                const int64_t L = s_off[x + 1] - s_off[x];
+                if (nmb == 0 || (used > 0 && used + L > budget)) {   // sequence m0 + x opens a micro-batch
+                    if (nmb < cap) { mb_seq[nmb] = (int32_t)(m0 + x); mb_row[nmb] = s_off[x]; }
+                    ++nmb;
+                    used = 0;
+                }
+                used += L;
+            }
+            s_used = used;
+            s_nmb = nmb;
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const int nmb = s_nmb;
+        if (nmb < cap) { mb_seq[nmb] = (int32_t)M; mb_row[nmb] = counts[1]; }   // the closing entry
+        *n_mb = nmb;
+    }
+}
+
 }  // namespace
+
+extern "C" int ajt_pack_microbatches(const int64_t* merged_offsets, const int64_t* counts, int64_t budget, int32_t capacity,
+                                     int32_t* mb_seq, int64_t* mb_row, int32_t* n_mb, ajt_stream_t stream_) {
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (!merged_offsets || !counts || !mb_seq || !mb_row || !n_mb || budget < 1 || capacity < 1) return AJT_ERR_INVALID_ARG;
+    AJT_LAUNCH(pack_microbatches_kernel<<<1, 1024, 0, stream>>>(merged_offsets, counts, budget, capacity, mb_seq, mb_row, n_mb));
+    return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
+}
 
 extern "C" int ajt_pack_loss_inputs(const int32_t* merged_tokens, const uint8_t* merged_mask, const float* merged_old_logp,
                                     const int64_t* merged_offsets, const int32_t* merged_origin, const int32_t* tl_seg,

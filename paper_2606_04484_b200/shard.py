@@ -14,7 +14,7 @@ process group uses.
 from __future__ import annotations
 
 from dataclasses import dataclass
-from typing import List, Optional, Sequence, Tuple
+from typing import Optional, Sequence, Tuple
 
 import numpy as np
 import torch
@@ -107,24 +107,6 @@ def split_rows(T: int, world: int) -> np.ndarray:
     """Row boundaries int64 [world + 1] of an even contiguous split of T packed rows (token-budget sharding: the
     rows of one trajectory may straddle two ranks, which is what `allreduce_seg_denom` is for)."""
     return (np.arange(world + 1, dtype=np.int64) * int(T)) // world
-
-
-def pack_sequences(lengths: Sequence[int], budget: int) -> List[Tuple[int, int]]:
-    """Consecutive merged sequences -> micro-batches of at most `budget` rows (a sequence longer than the budget
-    gets a micro-batch of its own).  Returns [(first_sequence, one_past_last_sequence)] covering all sequences in
-    order ("packed merged sequences", BASELINE.json north_star)."""
-    if budget < 1:
-        raise ValueError("budget must be >= 1")
-    out, a, used = [], 0, 0
-    for k, L in enumerate(lengths):
-        L = int(L)
-        if used > 0 and used + L > budget:
-            out.append((a, k))
-            a, used = k, 0
-        used += L
-    if len(lengths) > a:
-        out.append((a, len(lengths)))
-    return out
 
 
 def allreduce_seg_denom(seg_denom: torch.Tensor, group=None) -> torch.Tensor:

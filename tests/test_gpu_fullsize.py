@@ -209,6 +209,68 @@ def test_c3_chunk_with_real_merge_vectors():
     anysize_properties(out, d(mk), V)
 
 
+@pytest.mark.parametrize("model,V", [("A", 151936), ("B", 128256)])
+def test_c4_chunks_with_real_merge_vectors(model, V):
+    """configs[3]: each model's own merge (GPU) -> ajt_pack_loss_inputs (GPU, checked against the oracle's pack over the WHOLE
+    batch) -> one 64k-row chunk [65536, V] with eps 0.2 / 0.2 and batch-wide normalisers; sampled rows against the oracle."""
+    seed = W.BASE_SEED + 3
+    mi = W.merge_workload_c4(seed=seed)[model]
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    mo = ajt.merge_timelines(d(mi.tokens), d(mi.offsets), d(mi.traj_ids), d(mi.resp_start), None, d(mi.old_logp))
+    assert ajt.last_status(mo.workspace) == 0
+    uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
+    S = int(uniq.shape[0])
+    seg_adv = W.advantages_group_zscore(seed, 3, S).astype(np.float32)
+    pk = ajt.pack_loss_inputs(mo, d(tl_seg.astype(np.int32)), S, d(seg_adv))
+    fin = mo.finalize()
+    r = oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp)
+    targets, mask, olp, seg, adv = oracle.pack_loss_inputs(r.merged_tokens, r.merged_mask, r.merged_old_logp, r.merged_offsets,
+                                                           r.merged_origin, tl_seg.astype(np.int32), seg_adv)
+    No = r.N_out
+    cpu = lambda t: t.cpu().numpy()
+    assert fin.N_out == No and np.array_equal(cpu(pk.targets[:No]), targets) and np.array_equal(cpu(pk.mask[:No]), mask)
+    assert np.array_equal(cpu(pk.seg_ids[:No]), seg) and np.array_equal(cpu(pk.adv[:No]), adv)
+    Ns_t = ajt.segment_counts(pk.mask[:No], pk.seg_ids[:No], S)
+    Ns = Ns_t.cpu().numpy()
+    assert np.array_equal(Ns, np.bincount(seg, weights=mask.astype(np.float64), minlength=S).astype(np.float32))
+    inv = float(np.float32(1.0) / np.float32((Ns > 0).sum()))
+    T, k = 65536, 3
+    sl = slice(k * T, (k + 1) * T)
+    logits = torch.empty((T, V), dtype=torch.bfloat16, device="cuda")
+    H.fill_logits(logits, 91 + V % 7)
+    noise = (W.rng_for(seed, 3, 99).standard_normal(T) * 0.05).astype(np.float32)
+    old_t = H.harness_old_logp(logits, pk.targets[sl], noise)
+    out = ajt.policy_loss_fwd_bwd(logits, pk.targets[sl], old_t, pk.adv[sl], pk.mask[sl], pk.seg_ids[sl], S, 0.2, 0.2,
+                                  seg_denom=Ns_t, inv_num_segs=0.0, want_logp=True)
+    torch.cuda.synchronize()
+    assert ajt.last_status(out.workspace) == 0
+    tg, mk, sg, av, old = targets[sl], mask[sl], seg[sl], adv[sl], old_t.cpu().numpy()
+    rows = sample_rows(mk, 32, 3)
+    e = float(np.float32(0.2))
+    ref = oracle.policy_loss(bf16_bits(logits[torch.from_numpy(rows).cuda()]), tg, old, av, mk, sg, S, e, e, seg_denom=Ns,
+                             inv_num_segs=inv, row_ids=rows, logits_is_bf16_bits=True)
+    check_loss(out, ref, mk, 0.2, 0.2, av, old, 1.0, V, row_ids=rows, check_scalar=False)
+    anysize_properties(out, pk.mask[sl], V)
+
+
+@pytest.mark.parametrize("T", [4096, 16384, 65536, 131072])
+@pytest.mark.parametrize("V", [32000, 128256, 151936])
+@pytest.mark.parametrize("rho", [0.3, 0.7])
+def test_every_sweep_cell_sampled(T, V, rho):
+    """configs[4], all 24 (T, V, mask density) cells (S rotates over 8 / 64 / 512): sampled rows element by element against
+    the oracle, masked rows exactly zero, every gradient row sums to zero, the masked-token count."""
+    cell = (T // 4096) % 5 + (V // 1000) % 7 + int(rho * 10)
+    S = (8, 64, 512)[cell % 3]
+    lv, logits, (tg, old_t, adv_t, mask_t, seg_t) = _sweep_cell(T, V, S, rho, cell=cell)
+    out = ajt.policy_loss_fwd_bwd(logits, tg, old_t, adv_t, mask_t, seg_t, lv.S, EPS[0], EPS[1], want_logp=True, want_stats=True)
+    torch.cuda.synchronize()
+    assert ajt.last_status(out.workspace) == 0
+    vec = (lv.targets, old_t.cpu().numpy(), lv.adv, lv.mask, lv.seg_ids)
+    check_sampled(out, logits, vec, lv.S, sample_rows(lv.mask, 16, 7))
+    anysize_properties(out, mask_t, V)
+    assert float(out.stats[0]) == float(lv.mask.sum())
+
+
 def test_lm_head_full_size_sampled_rows():
     """ajt_lm_head_logp at the size sweep `h1` times (40,960 x 4,096 x 151,936: CTA pairs, 9 waves of row blocks, 4 vocabulary
     ranges of 149 tiles): sampled rows against the fp64 oracle computed row by row; every row finite and a valid log-prob."""

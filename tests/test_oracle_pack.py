@@ -55,3 +55,22 @@ def test_alignment_scores_each_sequence():
         direct += sum(float(table[x[q - 1], x[q]]) for q in range(1, len(x)) if mm[q])
     assert abs(packed - direct) < 1e-12
     assert int(m.sum()) == sum(int(msk[off[k] + 1:off[k + 1]].sum()) for k in range(4))
+
+
+def test_pack_microbatches_hand_and_properties():
+    # P-K4 hand example (budget 10): 5+5 fits, the third 5 opens a batch, 20 is alone (longer than the budget), 1+1 close
+    assert oracle.pack_microbatches([5, 5, 5, 20, 1, 1], 10) == [(0, 2), (2, 3), (3, 4), (4, 6)]
+    assert oracle.pack_microbatches([], 10) == []
+    assert oracle.pack_microbatches([3], 10) == [(0, 1)]
+    # P-K5 what "greedy, in order" fixes on random inputs: the batches tile the sequences in order; a batch is within the
+    # budget unless it is a single sequence; and it is maximal (the next sequence would not have fitted)
+    rng = np.random.default_rng(5)
+    for _ in range(200):
+        L = [int(x) for x in rng.integers(1, 40, size=int(rng.integers(1, 60)))]
+        B = int(rng.integers(1, 80))
+        mb = oracle.pack_microbatches(L, B)
+        assert mb[0][0] == 0 and mb[-1][1] == len(L) and all(mb[i][1] == mb[i + 1][0] for i in range(len(mb) - 1))
+        for a, b in mb:
+            assert b > a and (sum(L[a:b]) <= B or b - a == 1)
+            if b < len(L):
+                assert sum(L[a:b]) + L[b] > B

@@ -108,13 +108,6 @@ def test_shard_keeps_input_order_and_content():
             assert p.resp_start[k] == mi.resp_start[j] and p.traj_ids[k] == mi.traj_ids[j]
 
 
-def test_pack_sequences():
-    assert SH.pack_sequences([5, 5, 5, 20, 1, 1], 10) == [(0, 2), (2, 3), (3, 4), (4, 6)]
-    assert SH.pack_sequences([], 10) == []
-    assert SH.pack_sequences([3], 10) == [(0, 1)]
-    b = SH.split_rows(10, 3)
-    assert b[0] == 0 and b[-1] == 10 and np.all(np.diff(b) >= 3)
-
 
 def test_sharded_merge_equals_unsharded(two_rank_run):
     import oracle
