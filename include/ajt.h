@@ -286,7 +286,9 @@ int ajt_policy_loss_fwd_bwd_ext(
  * produced by tcgen05.mma (bf16 x bf16 -> fp32 in tensor memory) and reduced on the fly.  Arithmetic: fp32.
  * Requires d % 64 == 0, ld % 8 == 0 and 16-byte aligned bases (AJT_ERR_UNSUPPORTED otherwise).
  * With a mask the unmasked rows are compacted first (their hidden rows gathered into the workspace), so masked rows cost
- * no flops.  Workspace: ajt_lm_head_workspace_bytes(T, d, V) bytes of DEVICE memory, 256-byte aligned. */
+ * no flops.  Workspace: ajt_lm_head_workspace_bytes(T, d, V) bytes of DEVICE memory, 256-byte aligned; its first word is the
+ * call's status word (ajt_last_status): AJT_STATUS_BAD_TARGET when an unmasked row's target is outside [0, V) (that row
+ * returns 0, 0, 0). */
 enum {
     AJT_LM_ROUND_LOGITS_BF16 = 1 /* round every logit to bf16 (RNE) before the softmax: the log-probs then agree with what
                                     ajt_policy_loss_fwd_bwd computes from the same logits STORED in bf16 (to fp32 rounding of

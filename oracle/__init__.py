@@ -198,7 +198,7 @@ class LossResult:
 def policy_loss(logits, targets, old_logp, adv, mask, seg_ids, S: int, eps_lo: float, eps_hi: float,
                 seg_denom=None, inv_num_segs: float = 0.0, grad_scale: float = 1.0,
                 row_ids=None, want_dlogits: bool = True, logits_is_bf16_bits: bool = False,
-                ref_logp=None, kl_coef: float = 0.0, extended: bool = False) -> LossResult:
+                ref_logp=None, kl_coef: float = 0.0, extended: bool = False, clip_c: float = 0.0) -> LossResult:
     """fp64 loss oracle (DESIGN.md O-L).  `logits` is float32 [R,V], or uint16 [R,V] holding bf16 bit
     patterns when logits_is_bf16_bits.  Per-token vectors have length T (all tokens of the call);
     `row_ids` (int64 [R]) says which tokens the given logits rows are (None => R == T)."""
@@ -232,20 +232,21 @@ def policy_loss(logits, targets, old_logp, adv, mask, seg_ids, S: int, eps_lo: f
                                C.c_double(grad_scale), _p(loss), _p(logp), _p(w), _p(g), _p(Lt), _p(dl), _p(stats))
     if rc != 0:
         raise ValueError(f"ajt_oracle_loss: invalid input (rc={rc})")
-    if extended or ref_logp is not None:
+    if extended or ref_logp is not None or clip_c != 0.0:
         # steps 8-9 (KL against a reference policy, entropy): a second call of the extended entry point
         ref = _c(ref_logp, np.float32)
         k3 = np.zeros(max(R, 1), np.float64)
         ent = np.zeros(max(R, 1), np.float64)
         ext = np.zeros(2, np.float64)
         stats[:] = 0.0
-        rc = lib().ajt_oracle_loss_ex(_p(logits), C.c_int32(dt), C.c_int64(R), C.c_int32(V), C.c_int64(V), _p(row_ids),
+        lib().ajt_oracle_loss_ex2.restype = C.c_int
+        rc = lib().ajt_oracle_loss_ex2(_p(logits), C.c_int32(dt), C.c_int64(R), C.c_int32(V), C.c_int64(V), _p(row_ids),
                                       _p(targets), _p(old_logp), _p(adv), _p(mask), _p(seg_ids), C.c_int64(T), C.c_int32(S),
                                       C.c_double(eps_lo), C.c_double(eps_hi), _p(seg_denom), C.c_double(inv_num_segs),
                                       C.c_double(grad_scale), _p(loss), _p(logp), _p(w), _p(g), _p(Lt), _p(dl), _p(stats),
-                                      _p(ref), C.c_double(kl_coef), _p(k3), _p(ent), _p(ext))
+                                      _p(ref), C.c_double(kl_coef), _p(k3), _p(ent), _p(ext), C.c_double(clip_c))
         if rc != 0:
-            raise ValueError(f"ajt_oracle_loss_ex: invalid input (rc={rc})")
+            raise ValueError(f"ajt_oracle_loss_ex2: invalid input (rc={rc})")
         return LossResult(float(loss[0]), logp[:R], w[:R], g[:R], Lt[:R], dl, stats, k3[:R], ent[:R], ext)
     return LossResult(float(loss[0]), logp[:R], w[:R], g[:R], Lt[:R], dl, stats)
 

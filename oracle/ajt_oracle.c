@@ -199,14 +199,16 @@ static double load_logit(const void* logits, int dtype, int64_t idx) {
  *           g_t += grad_scale w_t kl_coef (1 - exp(d_t)) [k3_t < 10]
  *   step 9  H_t = lse_t - sum_v p_tv z_tv  (entropy of the row's softmax; reported, no gradient)
  * ref_logp NULL or kl_coef 0 switches step 8 off.  k3[R], ent[R] optional; ext[2] += {sum w_t k3_t, sum w_t H_t}.
+ *   step 3b (optional, clip_c > 0; reading L-18: the three-parameter "dual-clip" bound of SURVEY.md §8(f) f1): for A_t < 0
+ *           the surrogate is capped, L_t = min(L_t, -A_t c); where the cap is strictly active (r_t > c) the gradient is zero.
  */
 static int loss_impl(const void* logits, int32_t dtype, int64_t R, int32_t V, int64_t ld, const int64_t* row_ids,
                      const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
                      const int32_t* seg_ids, int64_t T, int32_t S,
                      double eps_lo, double eps_hi, const float* seg_denom, double inv_num_segs, double grad_scale,
                      double* loss_partial, double* logp, double* w, double* g, double* Lt, double* dlogits,
-                     double* stats, const float* ref_logp, double kl_coef, double* k3, double* ent, double* ext) {
-    if (R < 0 || T < 0 || V <= 0 || S <= 0 || ld < V || eps_lo < 0 || eps_hi < 0) return -1;
+                     double* stats, const float* ref_logp, double kl_coef, double* k3, double* ent, double* ext, double clip_c) {
+    if (R < 0 || T < 0 || V <= 0 || S <= 0 || ld < V || eps_lo < 0 || eps_hi < 0 || clip_c < 0) return -1;
     if (dtype != 0 && dtype != 1) return -1;
 
     /* Step 4: N_s = sum_{t: s_t = s} m_t (or seg_denom[s]);  S' = #{s: N_s > 0} (or 1/inv_num_segs). */
@@ -265,6 +267,13 @@ static int loss_impl(const void* logits, int32_t dtype, int64_t R, int32_t V, in
         double a1 = ratio * A, a2 = rc * A;
         double L = -(a1 < a2 ? a1 : a2);
 
+        /* Step 3b: dual-clip cap for negative advantages, L = min(L, -A c). */
+        int cap = 0;
+        if (clip_c > 0.0 && A < 0.0) {
+            double L3 = -A * clip_c;
+            if (L3 < L) { L = L3; cap = 1; }
+        }
+
         /* Step 4: w = m / (N_s S'). */
         double wt = (Ns[sg] > 0.0) ? inv_Sp / Ns[sg] : 0.0;
 
@@ -272,7 +281,7 @@ static int loss_impl(const void* logits, int32_t dtype, int64_t R, int32_t V, in
          * g = grad_scale w (-A r) [pass]; dlogits_v = g (1[v=y] - p_v). */
         int clip_hi = (A > 0.0 && ratio > 1.0 + eps_hi);
         int clip_lo = (A < 0.0 && ratio < 1.0 - eps_lo);
-        double gt = (clip_hi || clip_lo) ? 0.0 : grad_scale * wt * (-A * ratio);
+        double gt = (clip_hi || clip_lo || cap) ? 0.0 : grad_scale * wt * (-A * ratio);
 
         /* Step 8: low-variance KL estimator against the reference policy's log-prob of the same token. */
         double k3t = 0.0;
@@ -330,7 +339,7 @@ int ajt_oracle_loss(const void* logits, int32_t dtype, int64_t R, int32_t V, int
                     double* loss_partial, double* logp, double* w, double* g, double* Lt, double* dlogits,
                     double* stats) {
     return loss_impl(logits, dtype, R, V, ld, row_ids, targets, old_logp, adv, mask, seg_ids, T, S, eps_lo, eps_hi, seg_denom,
-                     inv_num_segs, grad_scale, loss_partial, logp, w, g, Lt, dlogits, stats, NULL, 0.0, NULL, NULL, NULL);
+                     inv_num_segs, grad_scale, loss_partial, logp, w, g, Lt, dlogits, stats, NULL, 0.0, NULL, NULL, NULL, 0.0);
 }
 
 int ajt_oracle_loss_ex(const void* logits, int32_t dtype, int64_t R, int32_t V, int64_t ld, const int64_t* row_ids,
@@ -340,7 +349,17 @@ int ajt_oracle_loss_ex(const void* logits, int32_t dtype, int64_t R, int32_t V, 
                        double* loss_partial, double* logp, double* w, double* g, double* Lt, double* dlogits,
                        double* stats, const float* ref_logp, double kl_coef, double* k3, double* ent, double* ext) {
     return loss_impl(logits, dtype, R, V, ld, row_ids, targets, old_logp, adv, mask, seg_ids, T, S, eps_lo, eps_hi, seg_denom,
-                     inv_num_segs, grad_scale, loss_partial, logp, w, g, Lt, dlogits, stats, ref_logp, kl_coef, k3, ent, ext);
+                     inv_num_segs, grad_scale, loss_partial, logp, w, g, Lt, dlogits, stats, ref_logp, kl_coef, k3, ent, ext, 0.0);
+}
+
+int ajt_oracle_loss_ex2(const void* logits, int32_t dtype, int64_t R, int32_t V, int64_t ld, const int64_t* row_ids,
+                        const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
+                        const int32_t* seg_ids, int64_t T, int32_t S,
+                        double eps_lo, double eps_hi, const float* seg_denom, double inv_num_segs, double grad_scale,
+                        double* loss_partial, double* logp, double* w, double* g, double* Lt, double* dlogits,
+                        double* stats, const float* ref_logp, double kl_coef, double* k3, double* ent, double* ext, double clip_c) {
+    return loss_impl(logits, dtype, R, V, ld, row_ids, targets, old_logp, adv, mask, seg_ids, T, S, eps_lo, eps_hi, seg_denom,
+                     inv_num_segs, grad_scale, loss_partial, logp, w, g, Lt, dlogits, stats, ref_logp, kl_coef, k3, ent, ext, clip_c);
 }
 
 /* Round an fp64 value to bf16 (round-to-nearest-even), returned as fp64 (reading L-10:

@@ -50,6 +50,7 @@ struct LmParams {
     float* logp_out;
     float* ent_out;
     float* lse_out;
+    uint32_t* status;            // first word of the workspace: AJT_STATUS_BAD_TARGET when a processed row's target is outside [0, V)
 };
 
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
@@ -339,6 +340,11 @@ __global__ void __launch_bounds__(256) lm_head_combine_kernel(const LmParams p, 
             H = logS - U / S;
             lse = M + logS;
         }
+        const int y = p.targets[t];
+        if (y < 0 || y >= p.V) {   // no column matched: report it instead of returning -inf (the row's outputs are 0)
+            atomicOr(p.status, (uint32_t)AJT_STATUS_BAD_TARGET);
+            lp = 0.f; H = 0.f; lse = 0.f;
+        }
         const int64_t o = p.row_idx ? (int64_t)p.row_idx[t] : t;
         p.logp_out[o] = lp;
         if (p.ent_out) p.ent_out[o] = H;
@@ -444,11 +450,12 @@ bool make_map(EncodeTiledFn fn, CUtensorMap* map, const void* base, int64_t rows
 }  // namespace
 
 namespace {
-struct LmWs { size_t part, n_rows, tile_state, row_idx, targets_c, hidden_c, total; };
+struct LmWs { size_t status, part, n_rows, tile_state, row_idx, targets_c, hidden_c, total; };
 inline size_t lm_a256(size_t x) { return (x + 255) & ~(size_t)255; }
 LmWs lm_ws_layout(int64_t T, int32_t d) {
     LmWs w;
     size_t o = 0;
+    w.status = o; o += 256;                                  // status word first (ajt_last_status)
     w.part = o; o += lm_a256((size_t)T * kVS * sizeof(float4));
     w.n_rows = o; o += 256;                                  // {n_rows, ticket}
     w.tile_state = o; o += lm_a256((size_t)((T + kCompactTile - 1) / kCompactTile + 1) * 8);
@@ -494,6 +501,8 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
     LmParams p;
     p.targets = targets; p.mask = mask; p.T = T; p.d = d; p.V = V;
     p.n_rows = nullptr; p.row_idx = nullptr;
+    p.status = reinterpret_cast<uint32_t*>(wsb + ws.status);
+    if (cudaMemsetAsync(p.status, 0, 256, stream) != cudaSuccess) return AJT_ERR_CUDA;
     p.round_bf16 = (flags & AJT_LM_ROUND_LOGITS_BF16) ? 1 : 0;
     const void* h_src = hidden;
     int64_t h_ld = ld_hidden;

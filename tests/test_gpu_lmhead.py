@@ -100,3 +100,26 @@ def test_unsupported_shapes_are_rejected():
     W = torch.zeros((16, 48), dtype=torch.bfloat16, device="cuda")
     with pytest.raises(ajt.AjtError):
         ajt.lm_head_logp(H, W, torch.zeros(8, dtype=torch.int32, device="cuda"))
+
+
+def test_bad_target_sets_status_word():
+    # an out-of-range target must not silently give logp = -inf; the status word reports it, the row returns 0
+    g = torch.Generator(device="cuda").manual_seed(9)
+    T, d, V = 200, 128, 1000
+    Hh = torch.randn((T, d), generator=g, device="cuda").to(torch.bfloat16)
+    Ww = (torch.randn((V, d), generator=g, device="cuda") * 0.05).to(torch.bfloat16)
+    y = torch.randint(0, V, (T,), generator=g, device="cuda", dtype=torch.int32)
+    ws = torch.empty(int(ajt.lib().ajt_lm_head_workspace_bytes(T, d, V)) + 256, dtype=torch.uint8, device="cuda")
+    lp, en = ajt.lm_head_logp(Hh, Ww, y, workspace=ws)
+    torch.cuda.synchronize()
+    assert ajt.last_status(ws) == 0 and bool(torch.isfinite(lp).all())
+    y2 = y.clone()
+    y2[17] = V + 5
+    y2[150] = -1
+    lp2, en2 = ajt.lm_head_logp(Hh, Ww, y2, workspace=ws)
+    torch.cuda.synchronize()
+    assert ajt.last_status(ws) & ajt.STATUS_BAD_TARGET
+    assert float(lp2[17]) == 0.0 and float(lp2[150]) == 0.0 and bool(torch.isfinite(lp2).all())
+    keep = torch.ones(T, dtype=torch.bool, device="cuda")
+    keep[17] = keep[150] = False
+    assert torch.equal(lp2[keep], lp[keep])

@@ -386,3 +386,63 @@ def test_extended_against_torch_autograd(T, V, S):
     r = oracle.policy_loss(z, y, old, adv, mask, seg, S, eps_lo, eps_hi, ref_logp=ref, kl_coef=kl_coef)
     np.testing.assert_allclose(r.loss, float(total), rtol=1e-12, atol=1e-14)
     np.testing.assert_allclose(r.dlogits, zt.grad.numpy(), rtol=1e-9, atol=1e-14)
+
+
+# ---- step 3b: the three-parameter dual-clip bound c (reading L-18)
+
+
+def _dual_clip_case(rstar, A, c, eps=(0.2, 0.28)):
+    """One token, one segment, ratio set exactly: old_logp = logp - log r*."""
+    V = 7
+    z = np.linspace(-1.0, 1.5, V).astype(np.float32)[None, :]
+    y = np.array([3], np.int32)
+    lse = np.log(np.exp(z.astype(np.float64)).sum())
+    logp = float(z[0, 3]) - lse
+    old = np.array([logp - np.log(rstar)], np.float32)
+    return oracle.policy_loss(z, y, old, np.array([A], np.float32), np.ones(1, np.uint8), np.zeros(1, np.int32), 1, eps[0], eps[1],
+                              clip_c=c), float(np.exp(logp - float(old[0])))
+
+
+def test_dual_clip_closed_form():
+    # P-L10: for A < 0 the loss is -A min(max(r, 1 - eps_lo), c); the gradient vanishes exactly where r > c (and where r < 1 - eps_lo);
+    # for A >= 0 the bound changes nothing
+    c = 3.0
+    for rstar in (0.5, 0.9, 1.5, 2.9, 3.1, 6.0):
+        res, r = _dual_clip_case(rstar, -2.0, c)
+        assert abs(res.Lt[0] - 2.0 * min(max(r, 0.8), c)) < 1e-12
+        assert (res.g[0] == 0.0) == (r > c or r < 0.8)
+        plain, _ = _dual_clip_case(rstar, -2.0, 0.0)
+        if r <= c:
+            assert res.Lt[0] == plain.Lt[0] and res.g[0] == plain.g[0]
+        pos, _ = _dual_clip_case(rstar, 2.0, c)
+        pos0, _ = _dual_clip_case(rstar, 2.0, 0.0)
+        assert pos.Lt[0] == pos0.Lt[0] and pos.g[0] == pos0.g[0]
+
+
+def test_dual_clip_against_torch_autograd():
+    # P-L11: an independent torch fp64 graph of the published form: max(-A r, -A clip(r)) capped by -A c where A < 0
+    rng = np.random.default_rng(12)
+    T, V, S, c = 40, 11, 3, 2.5
+    z = rng.standard_normal((T, V)).astype(np.float32) * 2
+    y = rng.integers(0, V, size=T).astype(np.int32)
+    adv = rng.standard_normal(T).astype(np.float32)
+    mask = (rng.random(T) < 0.8).astype(np.uint8)
+    seg = rng.integers(0, S, size=T).astype(np.int32)
+    zt = torch.tensor(z, dtype=torch.float64, requires_grad=True)
+    lp = torch.log_softmax(zt, dim=-1).gather(1, torch.tensor(y, dtype=torch.int64)[:, None])[:, 0]
+    old = (lp.detach().numpy() + rng.standard_normal(T) * 0.8).astype(np.float32)     # wide ratios: the cap fires
+    r = torch.exp(lp - torch.tensor(old, dtype=torch.float64))
+    A = torch.tensor(adv, dtype=torch.float64)
+    l1 = torch.maximum(-A * r, -A * torch.clamp(r, 1 - 0.2, 1 + 0.28))
+    l = torch.where(A < 0, torch.minimum(l1, -A * c), l1)
+    m = torch.tensor(mask, dtype=torch.float64)
+    sg = torch.tensor(seg, dtype=torch.int64)
+    Ns = torch.zeros(S, dtype=torch.float64).index_add_(0, sg, m)
+    live = (Ns > 0).sum()
+    w = torch.where(Ns[sg] > 0, m / (Ns[sg] * live), torch.zeros_like(m))
+    loss = (w * l).sum()
+    loss.backward()
+    res = oracle.policy_loss(z, y, old, adv, mask, seg, S, 0.2, 0.28, clip_c=c)
+    assert abs(res.loss - float(loss)) < 1e-12
+    assert np.abs(res.dlogits - zt.grad.numpy()).max() < 1e-12
+    assert (np.exp(res.logp - old) > c)[(adv < 0) & (mask > 0)].any()      # the case is exercised
