@@ -262,7 +262,10 @@ int ajt_policy_loss_fwd_bwd(
  *           switched off by ref_logp = NULL or kl_coef = 0 (then k3_t = 0).
  *   step 9  entropy of each unmasked row's softmax (the policy entropy the paper monitors),
  *             H_t = lse_t - sum_v p_tv z_tv,   reported only (no gradient).
- * Extra arguments: ref_logp DEVICE [T] or NULL; kl_coef >= 0; k3_out, ent_out DEVICE [T] or NULL (k3_t, H_t where
+ *   step 3b the optional three-parameter "dual-clip" bound (reading L-18): clip_c > 1 caps the surrogate
+ *           of negative-advantage tokens, L_t = min(L_t, -A_t clip_c), with zero gradient where the cap is active
+ *           (r_t > clip_c); clip_c = 0 switches it off.  (stats_out does not count capped tokens.)
+ * Extra arguments: ref_logp DEVICE [T] or NULL; kl_coef >= 0; clip_c >= 0; k3_out, ent_out DEVICE [T] or NULL (k3_t, H_t where
  * mask_t = 1, 0 elsewhere); ext_out DEVICE [2], required: {sum_t w_t k3_t, sum_t w_t H_t} of this call.
  * Everything else (arguments, workspace, layouts, error behaviour, paths) is as for ajt_policy_loss_fwd_bwd; with
  * ref_logp = NULL the loss, dlogits, logp_out and stats_out are bit-identical to that call's. */
@@ -270,7 +273,7 @@ int ajt_policy_loss_fwd_bwd_ext(
     const void* logits, const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
     const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T, int32_t V, int32_t S, int64_t ld_logits,
     int32_t logits_dtype, const float* seg_denom, float inv_num_segs, float grad_scale,
-    const float* ref_logp, float kl_coef,
+    const float* ref_logp, float kl_coef, float clip_c,
     void* dlogits, float* loss_out, float* logp_out, float* stats_out,
     float* k3_out, float* ent_out, float* ext_out,
     void* workspace, size_t workspace_bytes, ajt_stream_t stream);

@@ -454,9 +454,9 @@ def policy_loss_fwd_bwd_ext(logits: torch.Tensor, targets: torch.Tensor, old_log
                             seg_denom: Optional[torch.Tensor] = None, inv_num_segs: float = 0.0, grad_scale: float = 1.0,
                             V: Optional[int] = None, dlogits: Optional[torch.Tensor] = None, want_logp: bool = False,
                             want_stats: bool = False, want_rows: bool = True, out: Optional[LossOutput] = None,
-                            stream=None) -> LossOutput:
-    """ajt_policy_loss_fwd_bwd_ext (include/ajt.h): the loss call plus the KL term against `ref_logp` (low_var_kl) and
-    the per-row entropy, from the same single read of each row."""
+                            stream=None, clip_c: float = 0.0) -> LossOutput:
+    """ajt_policy_loss_fwd_bwd_ext (include/ajt.h): the loss call plus the KL term against `ref_logp` (low_var_kl), the
+    per-row entropy and the optional dual-clip bound `clip_c`, from the same single read of each row."""
     _require_cuda()
     if logits.dim() != 2 or not logits.is_cuda or logits.stride(1) != 1:
         raise TypeError("logits: expected a 2-D CUDA tensor with unit column stride")
@@ -490,7 +490,7 @@ def policy_loss_fwd_bwd_ext(logits: torch.Tensor, targets: torch.Tensor, old_log
     rc = lib().ajt_policy_loss_fwd_bwd_ext(
         _dp(logits), _dp(targets), _dp(old_logp), _dp(adv), _dp(mask), _dp(seg_ids),
         C.c_float(eps_lo), C.c_float(eps_hi), C.c_int64(T), C.c_int32(V), C.c_int32(S), C.c_int64(ld), C.c_int32(dt),
-        _dp(seg_denom), C.c_float(inv_num_segs), C.c_float(grad_scale), _dp(ref_logp), C.c_float(kl_coef),
+        _dp(seg_denom), C.c_float(inv_num_segs), C.c_float(grad_scale), _dp(ref_logp), C.c_float(kl_coef), C.c_float(clip_c),
         _dp(out.dlogits), _dp(out.loss), _dp(out.logp), _dp(out.stats), _dp(out.k3), _dp(out.ent), _dp(out.ext),
         _dp(out.workspace), C.c_size_t(out.workspace.numel()), _stream(stream))
     if rc != 0:

@@ -67,6 +67,7 @@ struct LossParams {
     float* stats_out;
     const float* ref_logp;  // extended form (steps 8-9): reference-policy log-probs [T] or NULL
     float kl_coef;
+    float clip_c;           // extended form, step 3b: dual-clip bound for negative advantages (0: off)
     float* ext_out;         // [2] {sum w_t k3_t, sum w_t H_t} or NULL
     float* k3_out;          // [T] or NULL
     float* ent_out;         // [T] or NULL
@@ -234,7 +235,7 @@ struct TokScalars {
 // M = max_v z, S = sum_v exp(z_v - M) (so 1 <= S <= V), zy = z[y].  DESIGN.md O-L steps 1-6.
 __device__ __forceinline__ TokScalars token_scalars(float M, float S, float zy, float old, float A, float w,
                                                     float eps_lo, float eps_hi, float grad_scale, bool use_kl = false,
-                                                    float ref = 0.f, float kl_coef = 0.f) {
+                                                    float ref = 0.f, float kl_coef = 0.f, float clip_c = 0.f) {
     TokScalars o;
     const float logS = logf(S);
     o.lse = M + logS;
@@ -247,8 +248,11 @@ __device__ __forceinline__ TokScalars token_scalars(float M, float S, float zy, 
     const bool hi = (A > 0.f) && (r > 1.f + eps_hi);
     const bool lo = (A < 0.f) && (r < 1.f - eps_lo);
     const float rc = fminf(fmaxf(r, 1.f - eps_lo), 1.f + eps_hi);
-    const float L = -fminf(r * A, rc * A);
-    o.g = (hi || lo) ? 0.f : grad_scale * w * (-A * r);
+    float L = -fminf(r * A, rc * A);
+    // step 3b (reading L-18): the dual-clip cap for negative advantages, L = min(L, -A c); no gradient where it is active
+    const bool cap = clip_c > 0.f && A < 0.f && -A * clip_c < L;
+    if (cap) L = -A * clip_c;
+    o.g = (hi || lo || cap) ? 0.f : grad_scale * w * (-A * r);
     o.wl = (double)w * (double)L;
     o.wkl = (double)w * (-(double)d);
     o.clip = (hi ? 1 : 0) | (lo ? 2 : 0);
@@ -531,7 +535,7 @@ __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams
                 S = warp_sum(pv.y * exp_diff(pv.x, M) + pw.y * exp_diff(pw.x, M));
             }
             const TokScalars ts = token_scalars(M, S, zy, old, A, w, p.eps_lo, p.eps_hi, p.grad_scale,
-                                                EXT && p.ref_logp != nullptr && p.kl_coef != 0.f, ref, p.kl_coef);
+                                                EXT && p.ref_logp != nullptr && p.kl_coef != 0.f, ref, p.kl_coef, EXT ? p.clip_c : 0.f);
             if (tid == 0 && rank == 0) {
                 p.row_val[kidx] = ts.wl;
                 p.row_kl[kidx] = ts.wkl;
@@ -655,7 +659,7 @@ __global__ void __launch_bounds__(256) loss_rows_generic(const LossParams p) {
             float g = 0.f, lse = 0.f;
             if (act) {
                 const TokScalars ts = token_scalars(m, s, zy, old, A, w, p.eps_lo, p.eps_hi, p.grad_scale,
-                                                    p.ext && p.ref_logp != nullptr && p.kl_coef != 0.f, ref, p.kl_coef);
+                                                    p.ext && p.ref_logp != nullptr && p.kl_coef != 0.f, ref, p.kl_coef, p.ext ? p.clip_c : 0.f);
                 g = ts.g;
                 lse = ts.lse;
                 if (gl == 0) {
@@ -828,6 +832,7 @@ struct LossExt {   // steps 8-9 (ajt_policy_loss_fwd_bwd_ext)
     const float* ref_logp;
     float kl_coef;
     float *k3_out, *ent_out, *ext_out;
+    float clip_c;
 };
 
 int loss_call(const void* logits, const int32_t* targets, const float* old_logp, const float* adv, const uint8_t* mask,
@@ -836,7 +841,7 @@ int loss_call(const void* logits, const int32_t* targets, const float* old_logp,
               float* logp_out, float* stats_out, const LossExt& x, void* workspace, size_t workspace_bytes,
               ajt_stream_t stream_) {
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
-    if (x.on && (!x.ext_out || !(x.kl_coef >= 0.f))) return AJT_ERR_INVALID_ARG;
+    if (x.on && (!x.ext_out || !(x.kl_coef >= 0.f) || !(x.clip_c >= 0.f))) return AJT_ERR_INVALID_ARG;
     if (T < 0 || V <= 0 || S <= 0 || ld_logits < V || T >= ((int64_t)1 << 31)) return AJT_ERR_INVALID_ARG;
     if (!(eps_lo >= 0.f) || !(eps_hi >= 0.f) || inv_num_segs < 0.f) return AJT_ERR_INVALID_ARG;
     if (logits_dtype != AJT_DT_BF16 && logits_dtype != AJT_DT_F32) return AJT_ERR_INVALID_ARG;
@@ -865,7 +870,7 @@ int loss_call(const void* logits, const int32_t* targets, const float* old_logp,
     p.row_val = reinterpret_cast<double*>(wsb + ws.row_val);
     p.row_kl = reinterpret_cast<double*>(wsb + ws.row_kl);
     p.row_clip = wsb + ws.row_clip;
-    p.ext = x.on; p.ref_logp = x.ref_logp; p.kl_coef = x.kl_coef; p.k3_out = x.k3_out; p.ent_out = x.ent_out; p.ext_out = x.ext_out;
+    p.ext = x.on; p.ref_logp = x.ref_logp; p.kl_coef = x.kl_coef; p.clip_c = x.clip_c; p.k3_out = x.k3_out; p.ent_out = x.ent_out; p.ext_out = x.ext_out;
     p.rec_r = reinterpret_cast<float*>(wsb + ws.rec_r);
     p.row_k3 = reinterpret_cast<double*>(wsb + ws.row_k3);
     p.row_ent = reinterpret_cast<double*>(wsb + ws.row_ent);
@@ -906,7 +911,7 @@ extern "C" int ajt_policy_loss_fwd_bwd(const void* logits, const int32_t* target
                                        int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype, const float* seg_denom,
                                        float inv_num_segs, float grad_scale, void* dlogits, float* loss_out, float* logp_out,
                                        float* stats_out, void* workspace, size_t workspace_bytes, ajt_stream_t stream) {
-    const LossExt x = {0, nullptr, 0.f, nullptr, nullptr, nullptr};
+    const LossExt x = {0, nullptr, 0.f, nullptr, nullptr, nullptr, 0.f};
     return loss_call(logits, targets, old_logp, adv, mask, seg_ids, eps_lo, eps_hi, T, V, S, ld_logits, logits_dtype, seg_denom,
                      inv_num_segs, grad_scale, dlogits, loss_out, logp_out, stats_out, x, workspace, workspace_bytes, stream);
 }
@@ -915,10 +920,10 @@ extern "C" int ajt_policy_loss_fwd_bwd_ext(const void* logits, const int32_t* ta
                                            const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T,
                                            int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype, const float* seg_denom,
                                            float inv_num_segs, float grad_scale, const float* ref_logp, float kl_coef,
-                                           void* dlogits, float* loss_out, float* logp_out, float* stats_out, float* k3_out,
-                                           float* ent_out, float* ext_out, void* workspace, size_t workspace_bytes,
+                                           float clip_c, void* dlogits, float* loss_out, float* logp_out, float* stats_out,
+                                           float* k3_out, float* ent_out, float* ext_out, void* workspace, size_t workspace_bytes,
                                            ajt_stream_t stream) {
-    const LossExt x = {1, ref_logp, kl_coef, k3_out, ent_out, ext_out};
+    const LossExt x = {1, ref_logp, kl_coef, k3_out, ent_out, ext_out, clip_c};
     return loss_call(logits, targets, old_logp, adv, mask, seg_ids, eps_lo, eps_hi, T, V, S, ld_logits, logits_dtype, seg_denom,
                      inv_num_segs, grad_scale, dlogits, loss_out, logp_out, stats_out, x, workspace, workspace_bytes, stream);
 }

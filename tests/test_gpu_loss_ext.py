@@ -143,3 +143,38 @@ def test_ext_argument_errors():
     lv, logits, targets, old, adv, mask, seg = make_case(8, 32000, 2, 1.0, torch.bfloat16, 3.0, 3)
     with pytest.raises(ajt.AjtError):
         ajt.policy_loss_fwd_bwd_ext(logits, targets, old, adv, mask, seg, lv.S, 0.2, 0.2, ref_logp=old, kl_coef=-1.0)
+
+
+@pytest.mark.parametrize("T,V", [(300, 1000), (257, 151936)])
+def test_dual_clip_bound_matches_oracle(T, V):
+    # step 3b (reading L-18): wide ratio noise so that r > c occurs on negative-advantage tokens; both kernel families
+    rng = np.random.default_rng(17)
+    S, c = 5, 2.0
+    g = torch.Generator(device="cuda").manual_seed(23)
+    logits = (torch.randn((T, V), generator=g, device="cuda") * 3.0).to(torch.bfloat16)
+    y = rng.integers(0, V, size=T).astype(np.int32)
+    adv = rng.standard_normal(T).astype(np.float32)
+    mask = (rng.random(T) < 0.8).astype(np.uint8)
+    seg = rng.integers(0, S, size=T).astype(np.int32)
+    dev = lambda a: torch.from_numpy(a).cuda()
+    lp = torch.log_softmax(logits.float(), dim=-1).gather(1, dev(y).long()[:, None])[:, 0]
+    old = (lp.cpu().numpy() + rng.standard_normal(T).astype(np.float32)).astype(np.float32)
+    out = ajt.policy_loss_fwd_bwd_ext(logits, dev(y), dev(old), dev(adv), dev(mask), dev(seg), S, 0.2, 0.28, clip_c=c, want_logp=True)
+    torch.cuda.synchronize()
+    assert ajt.last_status(out.workspace) == 0
+    bits = logits.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+    e = (float(np.float32(0.2)), float(np.float32(0.28)))
+    ref = oracle.policy_loss(bits, y, old, adv, mask, seg, S, e[0], e[1], logits_is_bf16_bits=True, clip_c=c)
+    r = np.exp(ref.logp - old)
+    capped = (adv < 0) & (mask > 0) & (r > c)
+    assert capped.any()
+    near = np.abs(r - c) < 1e-4     # fp32 and fp64 may land on different sides of the cap there
+    d_gpu = out.dlogits[:, :V].float().cpu().numpy().astype(np.float64)
+    ok = (mask > 0) & ~near
+    err = np.abs(d_gpu[ok] - ref.dlogits[ok])
+    assert (err <= 2.0 ** -8 * np.abs(ref.dlogits[ok]) + 1e-10).all()
+    assert not d_gpu[capped & ~near].any()
+    l1 = float(np.sum(ref.w * np.abs(ref.Lt)))
+    assert abs(float(out.loss[0]) - ref.loss) <= 1e-5 * l1 + 1e-7 * abs(ref.loss)
+    plain = ajt.policy_loss_fwd_bwd_ext(logits, dev(y), dev(old), dev(adv), dev(mask), dev(seg), S, 0.2, 0.28)
+    assert float(plain.loss[0]) != float(out.loss[0])
