@@ -325,6 +325,49 @@ def lm_head_logp(hidden_bits, weight_bits, targets, mask=None, round_logits_bf16
     return logp, ent
 
 
+def lm_head_loss_bwd(hidden_bits, weight_bits, targets, old_logp, adv, mask, seg_ids, S: int, eps_lo: float, eps_hi: float,
+                     seg_denom=None, inv_num_segs: float = 0.0, grad_scale: float = 1.0, round_dz_bf16: bool = False):
+    """The policy loss straight from the hidden states and its gradients w.r.t. both of them (SURVEY.md §8(f)
+    f3, backward half; the actor update of PAPER.md:136).  The plain chain rule through z_t = W h_t:
+        steps 1-6 of O-L on z (fp64 from the exact bf16 inputs; NOT rounded to bf16: reading H-1) give loss and, per row,
+        dZ_tv = g_t (1[v = y_t] - p_tv);   dH = dZ W  ([T,V] x [V,d]);   dW = dZ^T H  ([V,T] x [T,d])
+    round_dz_bf16: dZ is rounded to bf16 (RNE) before the two products, as a tensor-core path that feeds dZ as a bf16 operand
+    does (reading H-4) -- the variant the kernel is compared with element by element; the unrounded one is the definition.
+    Returns dict(loss, logp[T], lse[T], g[T], dH[T,d], dW[V,d]) in fp64.  CPU-sized inputs only (one [T,V] fp64 matrix)."""
+    def f64(bits):
+        b = np.ascontiguousarray(bits, np.uint16).astype(np.uint32) << 16
+        return b.view(np.float32).astype(np.float64)
+    H, W = f64(hidden_bits), f64(weight_bits)
+    T, V = H.shape[0], W.shape[0]
+    y = np.asarray(targets, np.int64)
+    m = (np.asarray(mask) != 0).astype(np.float64)
+    sg = np.asarray(seg_ids, np.int64)
+    old, A = np.asarray(old_logp, np.float64), np.asarray(adv, np.float64)
+    z = H @ W.T                                                   # library matmul as a step
+    zmax = z.max(axis=1)
+    lse = zmax + np.log(np.exp(z - zmax[:, None]).sum(axis=1))    # step 1
+    logp = z[np.arange(T), y] - lse
+    p = np.exp(z - lse[:, None])
+    r = np.exp(logp - old)                                        # step 2
+    rc = np.clip(r, 1.0 - eps_lo, 1.0 + eps_hi)
+    L = -np.minimum(r * A, rc * A)                                # step 3
+    Ns = np.zeros(S, np.float64)                                  # step 4
+    np.add.at(Ns, sg, m)
+    if seg_denom is not None:
+        Ns = np.asarray(seg_denom, np.float64)
+    inv = inv_num_segs if inv_num_segs != 0.0 else (1.0 / max(1, int((Ns > 0).sum())) if (Ns > 0).any() else 0.0)
+    w = np.where(Ns[sg] > 0, m * inv / np.where(Ns[sg] > 0, Ns[sg], 1.0), 0.0)
+    loss = float(np.sum(w * L))                                   # step 5
+    hi = (A > 0) & (r > 1.0 + eps_hi)                             # step 6
+    lo = (A < 0) & (r < 1.0 - eps_lo)
+    g = np.where(hi | lo, 0.0, grad_scale * w * (-A * r))
+    dZ = -g[:, None] * p
+    dZ[np.arange(T), y] += g
+    if round_dz_bf16:
+        dZ = round_bf16(dZ)
+    return dict(loss=loss, logp=logp * m, lse=lse * m, g=g, dH=dZ @ W, dW=dZ.T @ H, w=w, Lt=L)
+
+
 def round_bf16(x: np.ndarray) -> np.ndarray:
     """fp64 -> nearest bf16 (ties to even), as fp64."""
     a = np.ascontiguousarray(x, np.float64)
