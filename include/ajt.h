@@ -306,6 +306,26 @@ int ajt_lm_head_logp(const void* hidden, const void* weight, const int32_t* targ
                      float* lse_out /* or NULL */, uint32_t flags /* AJT_LM_* */, void* workspace, size_t workspace_bytes,
                      ajt_stream_t stream);
 
+/* The policy loss straight from the hidden states, forward AND backward ("policy gradient ... loss terms
+ * are computed"): with z_t = W h_t and steps 1-6 of ajt_policy_loss_fwd_bwd on z,
+ *   loss = sum_t w_t L_t;   dZ_tv = g_t (1[v = y_t] - exp(z_tv - lse_t));   dH = dZ W  [T, d] bf16;   dW (+)= dZ^T H  [V, d] fp32
+ * The [T, V] logits are never written: tiles of 256 x 256 are recomputed by tcgen05.mma and turned into dZ in the epilogue;
+ * dZ is staged in bf16 (round to nearest even: the operand precision of the two follow-on tensor-core products, reading
+ * H-4) 4,096 unmasked rows at a time in the workspace, and dH / dW come out of the same TMA / tcgen05 mainloop.  Masked
+ * rows (mask NULL: none) cost no flops; their dH rows are zero.  seg_denom DEVICE [S] or NULL (then N_s is counted from
+ * this call's tokens), inv_num_segs as for ajt_policy_loss_fwd_bwd.  accumulate_dw != 0 adds to dW instead of overwriting.
+ * loss_out DEVICE [1]; logp_out DEVICE [T] or NULL.  flags: AJT_LM_*.  Requires d % 64 == 0, ld_hidden / ld_weight / ld_dh
+ * % 8 == 0, ld_dw % 4 == 0, 16-byte aligned bases.  Workspace: ajt_lm_head_bwd_workspace_bytes(T, d, V, S) bytes (its first
+ * word is the status word: AJT_STATUS_BAD_TARGET, AJT_STATUS_BAD_SEG).  Enqueues on `stream`. */
+size_t ajt_lm_head_bwd_workspace_bytes(int64_t T, int32_t d, int32_t V, int32_t S);
+
+int ajt_lm_head_loss_bwd(const void* hidden, const void* weight, const int32_t* targets, const float* old_logp, const float* adv,
+                         const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T, int32_t d, int32_t V,
+                         int32_t S, int64_t ld_hidden, int64_t ld_weight, const float* seg_denom, float inv_num_segs,
+                         float grad_scale, void* dH, int64_t ld_dh, float* dW, int64_t ld_dw, int32_t accumulate_dw,
+                         float* loss_out, float* logp_out, uint32_t flags, void* workspace, size_t workspace_bytes,
+                         ajt_stream_t stream);
+
 /* Batch-wide per-trajectory normalisers for callers that stream the batch through several loss calls
  * (micro-batches, 64k-row chunks, or rows of one trajectory spread over several GPUs; reading L-4;
  * "masked per-trajectory mean", BASELINE.json north_star):

@@ -26,7 +26,8 @@ _EXPORTS = [
     "ajt_merge_workspace_bytes", "ajt_merge_workspace_bytes_for_pairs", "ajt_merge_timelines", "ajt_merge_host_arena_bytes", "ajt_merge_timelines_host",
     "ajt_loss_workspace_bytes", "ajt_policy_loss_fwd_bwd", "ajt_loss_host_arena_bytes", "ajt_policy_loss_fwd_bwd_host",
     "ajt_segment_counts", "ajt_policy_loss_fwd_bwd_ext", "ajt_merge_blocks_workspace_bytes", "ajt_merge_blocks",
-    "ajt_pack_loss_inputs", "ajt_pack_microbatches", "ajt_lm_head_workspace_bytes", "ajt_lm_head_logp",
+    "ajt_pack_loss_inputs", "ajt_pack_microbatches", "ajt_lm_head_workspace_bytes", "ajt_lm_head_bwd_workspace_bytes",
+    "ajt_lm_head_loss_bwd", "ajt_lm_head_logp",
     "ajt_hbm_probe", "ajt_launch_count", "ajt_host_ctx_create", "ajt_host_ctx_destroy", "ajt_policy_loss_fwd_bwd_host2",
 ]
 
@@ -66,6 +67,9 @@ def lib():
         L.ajt_merge_workspace_bytes_for_pairs.argtypes = [C.c_int32, C.c_int64, C.c_int64]
         L.ajt_lm_head_workspace_bytes.restype = C.c_size_t
         L.ajt_lm_head_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
+        L.ajt_lm_head_bwd_workspace_bytes.restype = C.c_size_t
+        L.ajt_lm_head_bwd_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
+        L.ajt_lm_head_loss_bwd.restype = C.c_int
         L.ajt_merge_blocks_workspace_bytes.restype = C.c_size_t
         L.ajt_merge_blocks_workspace_bytes.argtypes = [C.c_int32, C.c_int64]
         L.ajt_loss_workspace_bytes.restype = C.c_size_t
@@ -527,6 +531,44 @@ def lm_head_logp(hidden: torch.Tensor, weight: torch.Tensor, targets: torch.Tens
     if want_lse:
         return logp[:T], (None if ent is None else ent[:T]), lse[:T]
     return logp[:T], (None if ent is None else ent[:T])
+
+
+def lm_head_loss_bwd(hidden: torch.Tensor, weight: torch.Tensor, targets: torch.Tensor, old_logp: torch.Tensor, adv: torch.Tensor,
+                     mask: Optional[torch.Tensor], seg_ids: torch.Tensor, S: int, eps_lo: float, eps_hi: float,
+                     seg_denom: Optional[torch.Tensor] = None, inv_num_segs: float = 0.0, grad_scale: float = 1.0,
+                     dW: Optional[torch.Tensor] = None, accumulate_dw: bool = False, round_logits_bf16: bool = False,
+                     workspace: Optional[torch.Tensor] = None, stream=None) -> dict:
+    """ajt_lm_head_loss_bwd (include/ajt.h): loss, dH (bf16 [T, d]) and dW (fp32 [V, d]) from hidden states and head weights."""
+    _require_cuda()
+    _check_dev(hidden, torch.bfloat16, "hidden")
+    _check_dev(weight, torch.bfloat16, "weight")
+    _check_dev(targets, torch.int32, "targets")
+    _check_dev(old_logp, torch.float32, "old_logp")
+    _check_dev(adv, torch.float32, "adv")
+    _check_dev(mask, torch.uint8, "mask")
+    _check_dev(seg_ids, torch.int32, "seg_ids")
+    _check_dev(seg_denom, torch.float32, "seg_denom")
+    T, d = int(hidden.shape[0]), int(hidden.shape[1])
+    V = int(weight.shape[0])
+    dev = hidden.device
+    dH = torch.empty((T, d), dtype=torch.bfloat16, device=dev)
+    if dW is None:
+        dW = torch.empty((V, d), dtype=torch.float32, device=dev)
+        accumulate_dw = False
+    _check_dev(dW, torch.float32, "dW")
+    loss = torch.empty(1, dtype=torch.float32, device=dev)
+    logp = torch.empty(max(T, 1), dtype=torch.float32, device=dev)
+    if workspace is None:
+        workspace = torch.empty(int(lib().ajt_lm_head_bwd_workspace_bytes(T, d, V, S)) + 256, dtype=torch.uint8, device=dev)
+    rc = lib().ajt_lm_head_loss_bwd(_dp(hidden), _dp(weight), _dp(targets), _dp(old_logp), _dp(adv), _dp(mask), _dp(seg_ids),
+                                    C.c_float(eps_lo), C.c_float(eps_hi), C.c_int64(T), C.c_int32(d), C.c_int32(V), C.c_int32(S),
+                                    C.c_int64(d), C.c_int64(d), _dp(seg_denom), C.c_float(inv_num_segs), C.c_float(grad_scale),
+                                    _dp(dH), C.c_int64(d), _dp(dW), C.c_int64(d), C.c_int32(1 if accumulate_dw else 0), _dp(loss),
+                                    _dp(logp), C.c_uint32(1 if round_logits_bf16 else 0), _dp(workspace),
+                                    C.c_size_t(workspace.numel()), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_lm_head_loss_bwd")
+    return dict(loss=loss, dH=dH, dW=dW, logp=logp[:T], workspace=workspace)
 
 
 def hbm_probe(dst: Optional[torch.Tensor], src: Optional[torch.Tensor], nbytes: int, mode: int, stream=None) -> None:

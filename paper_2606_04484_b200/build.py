@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = ["ajt_api.cu", "ajt_loss.cu", "ajt_merge.cu", "ajt_blocks.cu", "ajt_pack.cu", "ajt_lmhead.cu"]
-HEADERS = ["ajt_common.cuh", os.path.join("..", "..", "include", "ajt.h")]
+HEADERS = ["ajt_common.cuh", "ajt_token.cuh", os.path.join("..", "..", "include", "ajt.h"), os.path.join("..", "..", "include", "ajt_test.h")]
 LIB = os.path.join(HERE, "libajt.so")
 
 NVCC_FLAGS = ["-Wno-deprecated-gpu-targets", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -13,6 +13,7 @@
 #include <cuda.h>
 
 #include "ajt_common.cuh"
+#include "ajt_token.cuh"
 
 namespace {
 
@@ -51,7 +52,22 @@ struct LmParams {
     float* ent_out;
     float* lse_out;
     uint32_t* status;            // first word of the workspace: AJT_STATUS_BAD_TARGET when a processed row's target is outside [0, V)
+    // ---- backward (ajt_lm_head_loss_bwd): the same mainloop with other epilogues
+    int64_t row0;                // first (compacted) row of the chunk this launch works on; rows are counted from it
+    const float* g_row;          // kDz: [rows] d loss / d logp of every (compacted) row (0: nothing to propagate)
+    const float* lse_row;        // kDz: [rows] log-sum-exp of the row's logits (forward pass)
+    __nv_bfloat16* dz;           // kDz: [chunk rows, ld_dz] dZ of the chunk, row-major
+    __nv_bfloat16* dzt;          // kDz: [ld_dz, ld_dzt] its transpose (vocabulary-major)
+    int64_t ld_dz, ld_dzt;
+    __nv_bfloat16* out_bf16;     // kStoreBf16: [*, ld_out] rows scattered through row_idx (dH)
+    float* out_f32;              // kAccF32: [n_out_rows, ld_out] += (dW)
+    int64_t ld_out;
+    int64_t n_out_rows;          // kAccF32: rows that exist (the operand is zero-padded beyond)
 };
+// Epilogue of the tile kernel.  kReduce: the forward pass (online log-sum-exp / entropy / target gather).  kDz: the tile of
+// logits becomes dZ = g (1[v = y] - exp(z - lse)) in bf16, stored row-major and transposed.  kStoreBf16 / kAccF32: a plain
+// product A B^T written as bf16 rows (dH) or added to an fp32 matrix (dW).
+enum { kReduce = 0, kDz = 1, kStoreBf16 = 2, kAccF32 = 3 };
 
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
@@ -130,7 +146,7 @@ __device__ __forceinline__ bool item_of(const LmParams& p, int n_mtiles, int it,
 }
 
 // Row blocks are 128 * NCTA rows.
-template <int NCTA>
+template <int NCTA, int MODE>
 __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_constant__ CUtensorMap map_h,
                                                                 const __grid_constant__ CUtensorMap map_w, const LmParams p) {
     using Cfg = LmCfg<NCTA>;
@@ -145,7 +161,14 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = NCTA > 1 ? cluster_ctarank() : 0u;
     const int nk = p.d / kBK;
-    const int64_t Teff = p.n_rows ? (int64_t)*p.n_rows : p.T;   // rows actually present (masked rows compacted away)
+    // rows actually present: all of them, or (masked rows compacted away) the device-side count; a backward launch works on the
+    // chunk of p.T rows that starts at row0 and has nothing to do beyond the count
+    int64_t Teff = p.n_rows ? (int64_t)*p.n_rows : p.T;
+    if (MODE != kReduce) {
+        const int64_t left = p.n_rows ? Teff - p.row0 : p.T;   // unmasked rows from this chunk on
+        if (left <= 0) return;   // uniform over the grid: before any barrier / tensor-memory allocation
+        Teff = MODE == kAccF32 ? p.T : (left < p.T ? left : p.T);
+    }
     const int n_mtiles = (int)((Teff + kBM * NCTA - 1) / (kBM * NCTA));
     const int n_groups = (int)gridDim.x / NCTA;
     const int n_items = (int)(((int64_t)n_mtiles * p.nvs + n_groups - 1) / n_groups);
@@ -245,9 +268,89 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
             if (!item_of<NCTA>(p, n_mtiles, it, mt, vs)) continue;
             const int64_t row = (int64_t)(mt * NCTA + (int)rank) * kBM + rloc;
             const bool live = row < Teff;
+            const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
+            if (MODE != kReduce) {
+                // ---- backward epilogues: one row of the tile per thread, 32 columns at a time
+                int y = -1;
+                float g = 0.f, klse = 0.f;
+                int64_t orow = row;
+                if (MODE == kDz && live) {
+                    y = p.targets[p.row0 + row];
+                    g = p.g_row[p.row0 + row];
+                    klse = -p.lse_row[p.row0 + row] * kLog2e;
+                }
+                if (MODE == kStoreBf16 && live && p.row_idx) orow = p.row_idx[p.row0 + row];
+                for (int n0 = v0; n0 < v1; n0 += kBN) {
+                    mbar_wait(&tfull[as], aph);
+                    tc_fence_after();
+                    const uint32_t tacc = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * kBN);
+#pragma unroll 1
+                    for (int c = 0; c < kBN; c += 32) {
+                        uint32_t v[32];
+                        tmem_ld32(tacc + (uint32_t)c, v);
+                        const int col0 = n0 + c;
+                        if (MODE == kDz) {
+                            uint32_t w2[16];
+#pragma unroll
+                            for (int e = 0; e < 32; e += 2) {
+                                float x0 = __uint_as_float(v[e]), x1 = __uint_as_float(v[e + 1]);
+                                if (p.round_bf16) {
+                                    x0 = __bfloat162float(__float2bfloat16_rn(x0));
+                                    x1 = __bfloat162float(__float2bfloat16_rn(x1));
+                                }
+                                float d0 = -g * ex2(fmaf(x0, kLog2e, klse)), d1 = -g * ex2(fmaf(x1, kLog2e, klse));
+                                if (col0 + e == y) d0 += g;
+                                if (col0 + e + 1 == y) d1 += g;
+                                if (col0 + e >= p.V || g == 0.f) d0 = 0.f;        // padding columns of the operand are zeros
+                                if (col0 + e + 1 >= p.V || g == 0.f) d1 = 0.f;
+                                w2[e >> 1] = pack_bf16x2(d0, d1);
+                            }
+                            // row-major: this thread's 32 columns are 64 contiguous bytes (rows beyond the chunk do not exist)
+                            if (row < p.T) {
+                                uint4* dst = reinterpret_cast<uint4*>(p.dz + row * p.ld_dz + col0);
+#pragma unroll
+                                for (int q = 0; q < 4; ++q) dst[q] = make_uint4(w2[4 * q], w2[4 * q + 1], w2[4 * q + 2], w2[4 * q + 3]);
+                                // transposed: for one column the warp's 32 rows are 64 contiguous bytes
+                                unsigned short* dt = reinterpret_cast<unsigned short*>(p.dzt) + (int64_t)col0 * p.ld_dzt + row;
+#pragma unroll
+                                for (int e = 0; e < 32; ++e)
+                                    dt[(int64_t)e * p.ld_dzt] = (unsigned short)((e & 1) ? (w2[e >> 1] >> 16) : (w2[e >> 1] & 0xffffu));
+                            }
+                        } else if (MODE == kStoreBf16) {
+                            if (live && col0 < p.V) {
+                                uint4* dst = reinterpret_cast<uint4*>(p.out_bf16 + orow * p.ld_out + col0);
+#pragma unroll
+                                for (int q = 0; q < 4; ++q)
+                                    dst[q] = make_uint4(pack_bf16x2(__uint_as_float(v[8 * q]), __uint_as_float(v[8 * q + 1])),
+                                                        pack_bf16x2(__uint_as_float(v[8 * q + 2]), __uint_as_float(v[8 * q + 3])),
+                                                        pack_bf16x2(__uint_as_float(v[8 * q + 4]), __uint_as_float(v[8 * q + 5])),
+                                                        pack_bf16x2(__uint_as_float(v[8 * q + 6]), __uint_as_float(v[8 * q + 7])));
+                            }
+                        } else {   // kAccF32
+                            if (row < p.n_out_rows && col0 < p.V) {
+                                float4* dst = reinterpret_cast<float4*>(p.out_f32 + row * p.ld_out + col0);
+#pragma unroll
+                                for (int q = 0; q < 8; ++q) {
+                                    float4 a = dst[q];
+                                    a.x += __uint_as_float(v[4 * q]); a.y += __uint_as_float(v[4 * q + 1]);
+                                    a.z += __uint_as_float(v[4 * q + 2]); a.w += __uint_as_float(v[4 * q + 3]);
+                                    dst[q] = a;
+                                }
+                            }
+                        }
+                    }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) {
+                        if (NCTA == 1) mbar_arrive(&tempty[as]);
+                        else mbar_arrive_remote(&tempty[as], 0);
+                    }
+                    if (++as == 2) { as = 0; aph ^= 1u; }
+                }
+                continue;
+            }
             const int y = live ? p.targets[row] : -1;
             float m = -INFINITY, s = 0.f, u = 0.f, zy = -INFINITY;
-            const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
             for (int n0 = v0; n0 < v1; n0 += kBN) {
                 mbar_wait(&tfull[as], aph);
                 tc_fence_after();
@@ -538,11 +641,11 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
 
     // ranges beyond nvs are empty (v0 >= V): their CTAs have nothing to do, and the combine reads nvs partials per row
     if (ncta == 1) {
-        if (cudaFuncSetAttribute(lm_head_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<1>::kSmem) != cudaSuccess)
+        if (cudaFuncSetAttribute(lm_head_kernel<1, kReduce>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<1>::kSmem) != cudaSuccess)
             return AJT_ERR_CUDA;
-        AJT_LAUNCH(lm_head_kernel<1><<<groups, kLmThreads, LmCfg<1>::kSmem, stream>>>(map_h, map_w, p));
+        AJT_LAUNCH(lm_head_kernel<1, kReduce><<<groups, kLmThreads, LmCfg<1>::kSmem, stream>>>(map_h, map_w, p));
     } else {
-        if (cudaFuncSetAttribute(lm_head_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<2>::kSmem) != cudaSuccess)
+        if (cudaFuncSetAttribute(lm_head_kernel<2, kReduce>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<2>::kSmem) != cudaSuccess)
             return AJT_ERR_CUDA;
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3((unsigned)(groups * 2));
@@ -557,9 +660,275 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
         cfg.attrs = attr;
         cfg.numAttrs = 1;
         ajt::note_launch();
-        if (cudaLaunchKernelEx(&cfg, lm_head_kernel<2>, map_h, map_w, p) != cudaSuccess) return AJT_ERR_CUDA;
+        if (cudaLaunchKernelEx(&cfg, lm_head_kernel<2, kReduce>, map_h, map_w, p) != cudaSuccess) return AJT_ERR_CUDA;
     }
     const int64_t want = (T + 255) / 256;
     AJT_LAUNCH(lm_head_combine_kernel<<<(int)(want < (int64_t)num_sms * 4 ? want : (int64_t)num_sms * 4), 256, 0, stream>>>(p, nvs));
+    return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
+}
+
+// ================================================================================================ backward
+//
+// ajt_lm_head_loss_bwd: loss, dH and dW straight from the hidden states.  The [T, V] logits are recomputed
+// tile by tile on the tensor cores and turned into dZ = g (1[v = y] - exp(z - lse)) in the epilogue; the two follow-on
+// contractions dH = dZ W and dW = dZ^T H run through the SAME TMA / tcgen05 mainloop with a store / accumulate epilogue.
+// dZ cannot stay on chip between them: its consumers' accumulators (rows x d fp32 for dH, V x d fp32 for dW) are 30-1000x the
+// tensor memory of the whole GPU, so dZ is staged in bf16, a CHUNK of rows at a time (row-major for dH, transposed for dW),
+// in the workspace.  Per chunk of R compacted rows: [R, V] bf16 is written twice and read once each: 4 R V bytes of traffic
+// against 6 R V d flops (d = 4096: 0.016 % of the time at the roofs).  Masked rows cost nothing (they are compacted away).
+namespace {
+
+constexpr int kBwdChunk = 4096;   // rows of dZ staged at a time (multiple of 256)
+
+// d loss / d logp of every compacted row k (original row t = row_idx[k], or k), the row's lse, and the loss: steps 2-6 of O-L
+// on the forward pass's log-probs (ajt_token.cuh).  Block partials in fp64, summed in block order by the last kernel.
+__global__ void __launch_bounds__(256) lm_token_grad_kernel(const float* __restrict__ logp, const float* __restrict__ lse,
+                                                            const float* __restrict__ old_logp, const float* __restrict__ adv,
+                                                            const int32_t* __restrict__ seg_ids, const float* __restrict__ seg_denom,
+                                                            const int32_t* __restrict__ row_idx, const int32_t* __restrict__ n_rows,
+                                                            int64_t T, int32_t S, float inv_num_segs, float eps_lo, float eps_hi,
+                                                            float grad_scale, float* __restrict__ g_row, float* __restrict__ lse_row,
+                                                            double* __restrict__ partials, uint32_t* status) {
+    __shared__ double s_red[8];
+    __shared__ float s_inv;
+    if (threadIdx.x == 0) s_inv = inv_num_segs;
+    if (inv_num_segs == 0.f) {   // 1 / S' from the normalisers (reading L-3): every block counts the live trajectories itself
+        int live = 0;
+        for (int x = threadIdx.x; x < S; x += 256) live += seg_denom[x] > 0.f ? 1 : 0;
+        live = __reduce_add_sync(0xffffffffu, live);
+        __shared__ int s_live[8];
+        if ((threadIdx.x & 31) == 0) s_live[threadIdx.x >> 5] = live;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int tot = 0;
+            for (int w = 0; w < 8; ++w) tot += s_live[w];
+            s_inv = tot > 0 ? 1.f / (float)tot : 0.f;
+        }
+    }
+    __syncthreads();
+    const int64_t Teff = n_rows ? (int64_t)*n_rows : T;
+    const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    double wl = 0.0;
+    if (k < T) {
+        float g = 0.f, ls = 0.f;
+        if (k < Teff) {
+            const int64_t t = row_idx ? (int64_t)row_idx[k] : k;
+            const int sg = seg_ids[t];
+            if (sg < 0 || sg >= S) {
+                atomicOr(status, (uint32_t)AJT_STATUS_BAD_SEG);
+            } else {
+                const float Ns = seg_denom[sg];
+                const float w = Ns > 0.f ? s_inv / Ns : 0.f;
+                const TokScalars ts = token_scalars(0.f, 1.f, logp[t], old_logp[t], adv[t], w, eps_lo, eps_hi, grad_scale);
+                g = ts.g;
+                wl = ts.wl;
+                ls = lse[t];
+            }
+        }
+        g_row[k] = g;
+        lse_row[k] = ls;
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) wl += __shfl_xor_sync(0xffffffffu, wl, o);
+    if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = wl;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tot = 0.0;
+        for (int w = 0; w < 8; ++w) tot += s_red[w];
+        partials[blockIdx.x] = tot;
+    }
+}
+__global__ void lm_loss_sum_kernel(const double* partials, int n, float* loss_out) {
+    double tot = 0.0;
+    for (int i = 0; i < n; ++i) tot += partials[i];
+    *loss_out = (float)tot;
+}
+
+// out[c, r] = in[r, c] for r < rows, c < cols (zeros elsewhere up to out_rows x ld_out): 64 x 64 tiles through shared memory.
+// `n_rows` (DEVICE, or NULL): rows that exist in `in` counted from row0; rows beyond are written as zeros.
+__global__ void __launch_bounds__(256) lm_transpose_kernel(const __nv_bfloat16* __restrict__ in, int64_t ld_in, int64_t rows, int64_t cols,
+                                                           __nv_bfloat16* __restrict__ out, int64_t ld_out, int64_t out_rows, int64_t out_cols,
+                                                           const int32_t* __restrict__ n_rows, int64_t row0) {
+    __shared__ __nv_bfloat16 tile[64][66];
+    if (n_rows) rows = min(rows, max((int64_t)0, (int64_t)*n_rows - row0));
+    const int64_t r0 = (int64_t)blockIdx.y * 64, c0 = (int64_t)blockIdx.x * 64;   // tile of `in`: rows r0.., cols c0..
+    for (int x = threadIdx.x; x < 64 * 64; x += 256) {
+        const int rr = x >> 6, cc = x & 63;
+        const int64_t r = r0 + rr, c = c0 + cc;
+        tile[rr][cc] = (r < rows && c < cols) ? in[r * ld_in + c] : __float2bfloat16(0.f);
+    }
+    __syncthreads();
+    for (int x = threadIdx.x; x < 64 * 64; x += 256) {
+        const int cc = x >> 6, rr = x & 63;
+        const int64_t r = r0 + rr, c = c0 + cc;
+        if (c < out_rows && r < out_cols) out[c * ld_out + r] = tile[rr][cc];
+    }
+}
+
+struct LmBwdWs { size_t fwd, logp, lse, g_row, lse_row, ns, partials, ones, wt, dz, dzt, hct, total; };
+LmBwdWs lm_bwd_ws_layout(int64_t T, int32_t d, int32_t V, int32_t S) {
+    LmBwdWs w;
+    size_t o = 0;
+    const size_t Vp = ((size_t)V + 255) / 256 * 256, R = kBwdChunk;
+    w.fwd = o; o += lm_a256(lm_ws_layout(T, d).total);
+    w.logp = o; o += lm_a256((size_t)T * 4);
+    w.lse = o; o += lm_a256((size_t)T * 4);
+    w.g_row = o; o += lm_a256((size_t)T * 4);
+    w.lse_row = o; o += lm_a256((size_t)T * 4);
+    w.ns = o; o += lm_a256((size_t)S * 4);
+    w.partials = o; o += lm_a256(((size_t)T / 256 + 2) * 8);
+    w.ones = o; o += lm_a256((size_t)T);
+    w.wt = o; o += lm_a256((size_t)d * Vp * 2);
+    w.dz = o; o += lm_a256(R * Vp * 2);
+    w.dzt = o; o += lm_a256(Vp * R * 2);
+    w.hct = o; o += lm_a256((size_t)d * R * 2);
+    w.total = o;
+    return w;
+}
+
+// one launch of the tile kernel: C[M, N] (epilogue MODE) from A [M, K] and B [N, K], both K-major bf16
+template <int MODE>
+int lm_launch(EncodeTiledFn encode, int num_sms, const void* A, int64_t M, int64_t lda, const void* Bm, int64_t N, int64_t ldb, int64_t K,
+              LmParams p, bool ranges, cudaStream_t stream) {
+    constexpr int ncta = 2;
+    CUtensorMap map_a, map_b;
+    if (!make_map(encode, &map_a, A, M, (int32_t)K, lda, kBM) || !make_map(encode, &map_b, Bm, N, (int32_t)K, ldb, kBN / ncta)) return AJT_ERR_CUDA;
+    p.T = M; p.d = (int32_t)K; p.V = (int32_t)N;
+    if (ranges) {   // the forward's decomposition: 4 vocabulary ranges walked tile by tile
+        p.nvs = N >= kVS * kBN ? kVS : 1;
+        p.vs_len = (int32_t)((((N + p.nvs - 1) / p.nvs + kBN - 1) / kBN) * kBN);
+    } else {        // one output tile per work item
+        p.nvs = (int32_t)((N + kBN - 1) / kBN);
+        p.vs_len = kBN;
+    }
+    const int64_t n_mtiles = (M + kBM * ncta - 1) / (kBM * ncta);
+    int groups = num_sms / ncta;
+    if ((int64_t)groups > n_mtiles * p.nvs) groups = (int)(n_mtiles * p.nvs);
+    if (cudaFuncSetAttribute(lm_head_kernel<ncta, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<ncta>::kSmem) != cudaSuccess)
+        return AJT_ERR_CUDA;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(groups * 2));
+    cfg.blockDim = dim3(kLmThreads);
+    cfg.dynamicSmemBytes = LmCfg<ncta>::kSmem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ajt::note_launch();
+    return cudaLaunchKernelEx(&cfg, lm_head_kernel<ncta, MODE>, map_a, map_b, p) == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
+}
+
+}  // namespace
+
+extern "C" size_t ajt_lm_head_bwd_workspace_bytes(int64_t T, int32_t d, int32_t V, int32_t S) {
+    if (T < 0 || d <= 0 || V <= 0 || S <= 0) return 0;
+    return lm_bwd_ws_layout(T, d, V, S).total;
+}
+
+extern "C" int ajt_lm_head_loss_bwd(const void* hidden, const void* weight, const int32_t* targets, const float* old_logp,
+                                    const float* adv, const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi,
+                                    int64_t T, int32_t d, int32_t V, int32_t S, int64_t ld_hidden, int64_t ld_weight,
+                                    const float* seg_denom, float inv_num_segs, float grad_scale, void* dH, int64_t ld_dh,
+                                    float* dW, int64_t ld_dw, int32_t accumulate_dw, float* loss_out, float* logp_out,
+                                    uint32_t flags, void* workspace, size_t workspace_bytes, ajt_stream_t stream_) {
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (T < 0 || d <= 0 || V <= 0 || S <= 0 || !workspace || !loss_out) return AJT_ERR_INVALID_ARG;
+    if (T > 0 && (!hidden || !weight || !targets || !old_logp || !adv || !seg_ids || !dH || !dW)) return AJT_ERR_INVALID_ARG;
+    if (!(eps_lo >= 0.f) || !(eps_hi >= 0.f) || inv_num_segs < 0.f) return AJT_ERR_INVALID_ARG;
+    if ((d % 64) || (ld_hidden % 8) || (ld_weight % 8) || (ld_dh % 8) || (ld_dw % 4) || ld_dh < d || ld_dw < d) return AJT_ERR_UNSUPPORTED;
+    if (((uintptr_t)hidden | (uintptr_t)weight | (uintptr_t)dH | (uintptr_t)dW) & 15) return AJT_ERR_UNSUPPORTED;
+    if ((uintptr_t)workspace & 255) return AJT_ERR_INVALID_ARG;
+    if (T >= ((int64_t)1 << 31)) return AJT_ERR_INVALID_ARG;
+    const LmBwdWs ws = lm_bwd_ws_layout(T, d, V, S);
+    if (workspace_bytes < ws.total) return AJT_ERR_WORKSPACE_TOO_SMALL;
+    uint8_t* b = reinterpret_cast<uint8_t*>(workspace);
+    int dev = 0, num_sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AJT_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || num_sms < kVS) return AJT_ERR_CUDA;
+    static EncodeTiledFn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return AJT_ERR_CUDA;
+        encode = reinterpret_cast<EncodeTiledFn>(fn);
+    }
+    if (T == 0) {
+        if (cudaMemsetAsync(loss_out, 0, 4, stream) != cudaSuccess) return AJT_ERR_CUDA;
+        if (!accumulate_dw && cudaMemsetAsync(dW, 0, (size_t)V * ld_dw * 4, stream) != cudaSuccess) return AJT_ERR_CUDA;
+        return AJT_OK;
+    }
+    float* logp = reinterpret_cast<float*>(b + ws.logp);
+    float* lse = reinterpret_cast<float*>(b + ws.lse);
+    float* g_row = reinterpret_cast<float*>(b + ws.g_row);
+    float* lse_row = reinterpret_cast<float*>(b + ws.lse_row);
+    float* ns = reinterpret_cast<float*>(b + ws.ns);
+    double* partials = reinterpret_cast<double*>(b + ws.partials);
+    __nv_bfloat16* wt = reinterpret_cast<__nv_bfloat16*>(b + ws.wt);
+    __nv_bfloat16* dz = reinterpret_cast<__nv_bfloat16*>(b + ws.dz);
+    __nv_bfloat16* dzt = reinterpret_cast<__nv_bfloat16*>(b + ws.dzt);
+    __nv_bfloat16* hct = reinterpret_cast<__nv_bfloat16*>(b + ws.hct);
+    uint32_t* status = reinterpret_cast<uint32_t*>(b + ws.fwd);   // the forward's status word is the call's
+    const int64_t Vp = ((int64_t)V + 255) / 256 * 256, R = kBwdChunk;
+
+    // ---- forward half: log-probs and log-sum-exp of every unmasked row (compacts the unmasked rows into the workspace)
+    int rc = ajt_lm_head_logp(hidden, weight, targets, mask, T, d, V, ld_hidden, ld_weight, logp, nullptr, lse, flags, b + ws.fwd,
+                              lm_a256(lm_ws_layout(T, d).total), stream_);
+    if (rc != AJT_OK) return rc;
+    if (logp_out && cudaMemcpyAsync(logp_out, logp, (size_t)T * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return AJT_ERR_CUDA;
+    const LmWs fw = lm_ws_layout(T, d);
+    const int32_t* n_rows = mask ? reinterpret_cast<const int32_t*>(b + ws.fwd + fw.n_rows) : nullptr;
+    const int32_t* row_idx = mask ? reinterpret_cast<const int32_t*>(b + ws.fwd + fw.row_idx) : nullptr;
+    const int32_t* targets_c = mask ? reinterpret_cast<const int32_t*>(b + ws.fwd + fw.targets_c) : targets;
+    const __nv_bfloat16* hc = mask ? reinterpret_cast<const __nv_bfloat16*>(b + ws.fwd + fw.hidden_c) : reinterpret_cast<const __nv_bfloat16*>(hidden);
+    const int64_t ld_hc = mask ? d : ld_hidden;
+    // ---- per-trajectory normalisers, then d loss / d logp per compacted row and the loss
+    if (!seg_denom) {
+        const uint8_t* mk = mask;
+        if (!mk) {
+            if (cudaMemsetAsync(b + ws.ones, 1, (size_t)T, stream) != cudaSuccess) return AJT_ERR_CUDA;
+            mk = b + ws.ones;
+        }
+        rc = ajt_segment_counts(mk, seg_ids, T, S, 0, ns, nullptr, stream_);
+        if (rc != AJT_OK) return rc;
+        seg_denom = ns;
+    }
+    const int nblk = (int)((T + 255) / 256);
+    AJT_LAUNCH(lm_token_grad_kernel<<<nblk, 256, 0, stream>>>(logp, lse, old_logp, adv, seg_ids, seg_denom, row_idx, n_rows, T, S, inv_num_segs,
+                                                   eps_lo, eps_hi, grad_scale, g_row, lse_row, partials, status));
+    AJT_LAUNCH(lm_loss_sum_kernel<<<1, 1, 0, stream>>>(partials, nblk, loss_out));
+    // ---- outputs start from zero (masked rows of dH stay zero); W^T once
+    if (cudaMemsetAsync(dH, 0, (size_t)T * ld_dh * 2, stream) != cudaSuccess) return AJT_ERR_CUDA;
+    if (!accumulate_dw && cudaMemsetAsync(dW, 0, (size_t)V * ld_dw * 4, stream) != cudaSuccess) return AJT_ERR_CUDA;
+    AJT_LAUNCH(lm_transpose_kernel<<<dim3((unsigned)((d + 63) / 64), (unsigned)((Vp + 63) / 64)), 256, 0, stream>>>(
+        reinterpret_cast<const __nv_bfloat16*>(weight), ld_weight, V, d, wt, Vp, d, Vp, nullptr, 0));
+    // the staging buffers never hold anything but finite numbers (a chunk may leave parts of them untouched)
+    if (cudaMemsetAsync(dz, 0, (size_t)R * Vp * 2, stream) != cudaSuccess || cudaMemsetAsync(dzt, 0, (size_t)Vp * R * 2, stream) != cudaSuccess)
+        return AJT_ERR_CUDA;
+    LmParams p = {};
+    p.targets = targets_c; p.n_rows = n_rows; p.row_idx = row_idx; p.round_bf16 = (flags & AJT_LM_ROUND_LOGITS_BF16) ? 1 : 0;
+    p.status = status; p.g_row = g_row; p.lse_row = lse_row; p.dz = dz; p.dzt = dzt; p.ld_dz = Vp; p.ld_dzt = R;
+    p.out_bf16 = reinterpret_cast<__nv_bfloat16*>(dH); p.out_f32 = dW; p.n_out_rows = V;
+    for (int64_t c0 = 0; c0 < T; c0 += R) {   // chunks beyond the number of unmasked rows (known on the device only) exit at once
+        const int64_t rows = T - c0 < R ? T - c0 : R;
+        p.row0 = c0;
+        // dZ of the chunk (row-major and transposed) from recomputed logits tiles
+        rc = lm_launch<kDz>(encode, num_sms, hc + c0 * ld_hc, rows, ld_hc, weight, V, ld_weight, d, p, true, stream);
+        if (rc != AJT_OK) return rc;
+        // H_chunk^T (rows beyond the unmasked count: zeros)
+        AJT_LAUNCH(lm_transpose_kernel<<<dim3((unsigned)((d + 63) / 64), (unsigned)(R / 64)), 256, 0, stream>>>(hc + c0 * ld_hc, ld_hc, rows, d, hct, R, d, R,
+                                                                                              n_rows, c0));
+        // dH_chunk = dZ_chunk W  (rows scattered to their original positions)
+        p.ld_out = ld_dh;
+        rc = lm_launch<kStoreBf16>(encode, num_sms, dz, rows, Vp, wt, d, Vp, Vp, p, false, stream);
+        if (rc != AJT_OK) return rc;
+        // dW += dZ_chunk^T H_chunk
+        p.ld_out = ld_dw;
+        rc = lm_launch<kAccF32>(encode, num_sms, dzt, Vp, R, hct, d, R, R, p, false, stream);
+        if (rc != AJT_OK) return rc;
+    }
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }
