@@ -293,6 +293,84 @@ def test_lm_head_full_size_sampled_rows():
     assert np.abs(ent[rt].cpu().numpy().astype(np.float64) - re).max() <= 5e-5
 
 
+def test_lm_head_loss_bwd_full_width_against_oracle():
+    """ajt_lm_head_loss_bwd at the full hidden size and vocabulary (d = 4,096, V = 151,936: 594 vocabulary tiles, 4 ranges, CTA
+    pairs) on 512 rows, where the fp64 oracle (O-HB) still computes everything: loss, dH and dW element by element."""
+    T, d, V, S = 512, 4096, 151936, 6
+    g = torch.Generator(device="cuda").manual_seed(5)
+    rng = np.random.default_rng(5)
+    Hh = torch.randn((T, d), generator=g, device="cuda").to(torch.bfloat16)
+    Ww = (torch.randn((V, d), generator=g, device="cuda") * 0.02).to(torch.bfloat16)
+    y = torch.randint(0, V, (T,), generator=g, device="cuda", dtype=torch.int32)
+    adv = torch.from_numpy(rng.standard_normal(T).astype(np.float32)).cuda()
+    mask = torch.from_numpy((rng.random(T) < 0.6).astype(np.uint8)).cuda()
+    seg = torch.from_numpy(np.sort(rng.integers(0, S, size=T)).astype(np.int32)).cuda()
+    lp, _ = ajt.lm_head_logp(Hh, Ww, y)
+    old = (lp + torch.from_numpy((rng.standard_normal(T) * 0.1).astype(np.float32)).cuda()).contiguous()
+    out = ajt.lm_head_loss_bwd(Hh, Ww, y, old, adv, mask, seg, S, 0.2, 0.28)
+    torch.cuda.synchronize()
+    assert ajt.last_status(out["workspace"]) == 0
+    e = (float(np.float32(0.2)), float(np.float32(0.28)))
+    ref = oracle.lm_head_loss_bwd(bf16_bits(Hh), bf16_bits(Ww), y.cpu().numpy(), old.cpu().numpy(), adv.cpu().numpy(),
+                                  mask.cpu().numpy(), seg.cpu().numpy(), S, e[0], e[1], round_dz_bf16=True)
+    l1 = float(np.sum(ref["w"] * np.abs(ref["Lt"])))
+    assert abs(float(out["loss"][0]) - ref["loss"]) <= 1e-5 * l1 + 1e-7 * abs(ref["loss"])
+    dH, dW = out["dH"].float().cpu().numpy().astype(np.float64), out["dW"].cpu().numpy().astype(np.float64)
+    sH, sW = np.abs(ref["dH"]).max(), np.abs(ref["dW"]).max()
+    assert np.abs(dH - ref["dH"]).max() <= 2.0 ** -7 * sH
+    assert np.abs(dW - ref["dW"]).max() <= 2e-3 * sW
+
+
+def test_lm_head_loss_bwd_bench_size_properties():
+    """The size the sweep times (40,960 x 4,096 x 151,936, mask density ~0.34: 4 chunks of staged dZ): sampled dH rows against
+    the oracle computed row by row (the row's own 151,936 logits in fp64), masked rows exactly zero, and two identities of
+    the exact gradients that tie dW to them at any size: sum_v dW_v = 0 (every dZ row sums to zero) and <dW, W> = sum_t <dH_t, h_t>."""
+    T, d, V, S = 40960, 4096, 151936, 64
+    g = torch.Generator(device="cuda").manual_seed(6)
+    rng = np.random.default_rng(6)
+    Hh = torch.randn((T, d), generator=g, device="cuda").to(torch.bfloat16)
+    Ww = (torch.randn((V, d), generator=g, device="cuda") * 0.02).to(torch.bfloat16)
+    lv = W.loss_sweep_vectors(T, V, S, 0.35, cell=9)
+    dd = lambda a: torch.from_numpy(a).cuda()
+    y, adv, mask, seg = dd(lv.targets), dd(lv.adv), dd(lv.mask), dd(lv.seg_ids)
+    lp, _ = ajt.lm_head_logp(Hh, Ww, y, mask)
+    old = (lp + dd(lv.noise)).contiguous()
+    out = ajt.lm_head_loss_bwd(Hh, Ww, y, old, adv, mask, seg, S, 0.2, 0.28)
+    torch.cuda.synchronize()
+    assert ajt.last_status(out["workspace"]) == 0
+    dH, dW = out["dH"], out["dW"]
+    assert bool(torch.isfinite(dW).all()) and bool(torch.isfinite(dH.float()).all())
+    assert not bool(dH[mask == 0].any())
+    # identities of the exact gradients
+    colsum = dW.double().sum(dim=0)
+    assert float(colsum.abs().max()) <= 1e-3 * float(dW.double().abs().sum(dim=0).max())
+    lhs = float((dW.double() * Ww.double()).sum())
+    rhs = float((dH.double() * Hh.double()).sum())
+    scale = float((dH.double().abs() * Hh.double().abs()).sum())
+    assert abs(lhs - rhs) <= 2.0 ** -8 * scale
+    # sampled rows, oracle row by row: z_t = W h_t in fp64, steps 1-6, dH_t = dZ_t W
+    Ns = np.bincount(lv.seg_ids, weights=lv.mask.astype(np.float64), minlength=S)
+    inv = 1.0 / max(1, int((Ns > 0).sum()))
+    Wf = Ww.double().cpu().numpy()
+    oldh, e = old.cpu().numpy().astype(np.float64), (float(np.float32(0.2)), float(np.float32(0.28)))
+    on = np.nonzero(lv.mask)[0]
+    for t in [int(on[0]), int(on[-1])] + [int(x) for x in rng.choice(on, size=6, replace=False)]:
+        h = Hh[t].double().cpu().numpy()
+        z = Wf @ h
+        lse = z.max() + np.log(np.exp(z - z.max()).sum())
+        logp = z[lv.targets[t]] - lse
+        r = np.exp(logp - oldh[t])
+        A = float(lv.adv[t])
+        passes = not ((A > 0 and r > 1 + e[1]) or (A < 0 and r < 1 - e[0]))
+        w = inv / Ns[lv.seg_ids[t]]
+        gt = w * (-A * r) if passes else 0.0
+        dz = -gt * np.exp(z - lse)
+        dz[lv.targets[t]] += gt
+        ref = oracle.round_bf16(dz) @ Wf
+        got = dH[t].double().cpu().numpy()
+        assert np.abs(got - ref).max() <= 2.0 ** -7 * np.abs(ref).max() + 1e-30, t
+
+
 def test_merge_blocks_full_size_b3():
     """ajt_merge_blocks on the full b3 workload (7,805 timelines, 253,556 blocks, 145.6 M tokens), bit-exact in every output."""
     from test_gpu_blocks import as_dict, run
