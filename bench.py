@@ -376,16 +376,14 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     if rank == 0:
         shape_key = f"loss_rows_kernel[{T}x{V},rho={rho:.2f}]"
         traffic, traffic_note = None, None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tp):
-            try:
-                with open(tp) as f:
-                    tj = json.load(f)
-                ent = tj.get("shapes", {}).get(f"{T}x{V}")
-                if ent:
-                    traffic, traffic_note = ent.get("dram_bytes_per_launch"), ent.get("note")
-            except Exception:
-                traffic = None
+        try:   # DRAM bytes of one rows-kernel launch at this shape, from the committed ncu --set full capture
+            import csv
+            with open(os.path.join(ROOT, "profiles", "r02_traffic.csv")) as f:
+                for row in csv.DictReader(f):
+                    if row["kernel"] == "loss_rows_kernel" and row["shape"] == f"{T}x{V}":
+                        traffic, traffic_note = float(row["dram_bytes_per_launch"]), row["note"]
+        except Exception:
+            traffic = None
         ach = loss_b / (loss_ms * 1e-3) / 1e9
         mg = b_merge / (merge_ms * 1e-3) / 1e9
         line = {
@@ -629,7 +627,58 @@ def run_config_records(torch, ajt, W, B3, ch3, logits_big, dlogits_big, dev, str
         rec = loss_rec(lg, dl, tg, old, dd(lv.adv), dd(lv.mask), dd(lv.seg_ids), S, Vv, (0.2, 0.28))
         rec["S"] = S
         recs[f"c5[{T}x{Vv},rho={rho}]"] = {"what": "configs[4] loss sweep cell", "loss": rec}
+    # f3: log-probs and the loss with its gradients straight from hidden states, the one tensor-core stage
+    try:
+        recs["lm_head[40960x4096x151936]"] = lm_head_record(torch, ajt, W, dev, stream)
+    except Exception as e:   # measurement extra: never takes the bench line down
+        recs["lm_head[40960x4096x151936]"] = {"error": repr(e)[:200]}
     return recs
+
+
+def lm_head_record(torch, ajt, W, dev, stream):
+    """ajt_lm_head_logp (forward) and ajt_lm_head_loss_bwd (loss + dH + dW) at 40,960 x 4,096 x 151,936 with the mask of a
+    configs[4] cell (density ~0.35): TFLOP/s over the unmasked rows (2 T d V forward; 8 T d V for the whole backward call,
+    which recomputes the logits tiles), against the measured cuBLAS bf16 rates of MEASURED_PEAKS.json."""
+    T, d, Vv, S = 40960, 4096, V, 64
+    g = torch.Generator(device=dev).manual_seed(6)
+    Hh = torch.randn((T, d), generator=g, device=dev).to(torch.bfloat16)
+    Ww = (torch.randn((Vv, d), generator=g, device=dev) * 0.02).to(torch.bfloat16)
+    lv = W.loss_sweep_vectors(T, Vv, S, 0.35, cell=9)
+    dd = lambda a: torch.from_numpy(a).to(dev)
+    y, adv, mask, seg = dd(lv.targets), dd(lv.adv), dd(lv.mask), dd(lv.seg_ids)
+    with torch.cuda.stream(stream):
+        lp, _ = ajt.lm_head_logp(Hh, Ww, y, mask, stream=stream)
+        stream.synchronize()
+    old = (lp + dd(lv.noise)).contiguous()
+    dW = torch.zeros((Vv, d), dtype=torch.float32, device=dev)
+    st = {"ws": None}
+
+    def bwd():
+        o = ajt.lm_head_loss_bwd(Hh, Ww, y, old, adv, mask, seg, S, EPS[0], EPS[1], dW=dW, accumulate_dw=False, workspace=st["ws"],
+                                 stream=stream)
+        st["ws"] = o["workspace"]
+
+    def fwd():
+        ajt.lm_head_logp(Hh, Ww, y, mask, stream=stream)
+
+    ms_b = float(np.median(time_calls(bwd, stream, reps=3, warmup=1)))
+    ms_f = float(np.median(time_calls(fwd, stream, reps=3, warmup=1)))
+    Tu = int(lv.mask.sum())
+    burst = sust = None
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            mp = json.load(f)
+        burst, sust = float(mp["bf16_tflops"]), float(mp["bf16_tflops_sustained"])
+    except Exception:
+        pass
+    tf_f, tf_b = 2.0 * Tu * d * Vv / ms_f / 1e9, 8.0 * Tu * d * Vv / ms_b / 1e9
+    return {"what": "SURVEY.md §8(f) f3: LM head fused with the loss, forward and backward (tcgen05 / TMEM / TMA); bound: tensor",
+            "rows": T, "unmasked_rows": Tu, "d": d, "V": Vv,
+            "forward": {"ms": ms_f, "tflops": tf_f, "frac_of_bf16_burst": tf_f / burst if burst else None,
+                        "frac_of_bf16_sustained": tf_f / sust if sust else None},
+            "loss_fwd_bwd": {"ms": ms_b, "tflops": tf_b, "frac_of_bf16_burst": tf_b / burst if burst else None,
+                             "frac_of_bf16_sustained": tf_b / sust if sust else None,
+                             "flops": "8 T d V: logits tiles twice (forward, recomputed for dZ), dH = dZ W, dW = dZ^T H"}}
 
 
 # ----------------------------------------------------------------------------------------- reference arm (oracle)
@@ -659,25 +708,31 @@ def run_reference(args, rank: int):
     inv = float(np.float32(1.0 / max(1, int((Ns > 0).sum()))))
     T = min(args.loss_rows, r.N_out)
     n_unm = int(mask[:T].sum())
-    rows_max = 512
+    rows_max = min(2048, T)
     g = torch.Generator().manual_seed(seed)
     logits = (torch.randn((rows_max, V), generator=g) * 3.0).to(torch.bfloat16)
+    # the sample is every (T / rows_max)-th row of the chunk, so it carries the chunk's own mix of prompt (masked) and
+    # response rows; a leading slab would hold prompt rows only
+    rid_all = np.unique(np.linspace(0, T - 1, rows_max).astype(np.int64))
+    rows_max = int(rid_all.shape[0])
     old = np.zeros(T, np.float32)
-    old[:rows_max] = harness_old_logp(logits, torch.from_numpy(targets[:rows_max]), noise_for(W, seed, 0, rows_max)).numpy()
+    old[rid_all] = harness_old_logp(logits[:rows_max], torch.from_numpy(targets[rid_all]), noise_for(W, seed, 0, rows_max)).numpy()
     bits = logits.view(torch.int16).numpy().view(np.uint16)
 
     def one_step(rows):
+        pick = np.unique(np.linspace(0, rows_max - 1, rows).astype(np.int64))   # evenly spaced among the sampled rows
+        rid, bt = rid_all[pick], np.ascontiguousarray(bits[pick])
         t0 = time.perf_counter()
         oracle.merge_timelines(mi.tokens, mi.offsets, mi.traj_ids, mi.resp_start, None, mi.old_logp, oracle.OWNER_LONGEST)
         t1 = time.perf_counter()
-        oracle.policy_loss(bits[:rows], targets[:T], old, adv[:T], mask[:T], seg[:T], S, float(np.float32(EPS[0])),
-                           float(np.float32(EPS[1])), seg_denom=Ns, inv_num_segs=inv, row_ids=np.arange(rows, dtype=np.int64),
+        oracle.policy_loss(bt, targets[:T], old, adv[:T], mask[:T], seg[:T], S, float(np.float32(EPS[0])),
+                           float(np.float32(EPS[1])), seg_denom=Ns, inv_num_segs=inv, row_ids=rid,
                            want_dlogits=True, logits_is_bf16_bits=True)
-        return t1 - t0, time.perf_counter() - t1, int(mask[:rows].sum())
+        return t1 - t0, time.perf_counter() - t1, int(mask[rid].sum())
 
-    tm, tl, nu = one_step(32)
+    tm, tl, nu = one_step(min(256, rows_max))
     budget = 120.0 / max(1, args.steps + args.warmup)   # warm-up + steps stay within ~2 minutes
-    rows = int(min(rows_max, max(32, 32 * max(0.0, budget - tm) / max(tl, 1e-6))))
+    rows = int(min(rows_max, max(32, 256 * max(0.0, budget - tm) / max(tl, 1e-6))))
     for _ in range(args.warmup):
         one_step(rows)
     t_m = t_l = 0.0
@@ -693,8 +748,8 @@ def run_reference(args, rank: int):
     t_step = t_m / K + b_all / rate
     val = (merge_bytes(mi.n, mi.n_tokens, r.N_out) + b_all) / t_step / 1e9
     cores = oracle.num_threads()
-    sample = (f"per step: full merge of the batch ({mi.n} timelines, {mi.n_tokens} tokens) + first {rows} of {T} loss rows "
-              f"({nu} unmasked) x V={V}; the chunk's time is extrapolated at the sample's byte rate (rows are independent)")
+    sample = (f"per step: full merge of the batch ({mi.n} timelines, {mi.n_tokens} tokens) + {rows} of the chunk's {T} loss rows, evenly "
+              f"spaced ({nu} unmasked) x V={V}; the chunk's time is extrapolated at the sample's byte rate (rows are independent)")
 
     class _B:   # what workload_config reads
         n, N_in, N_out = mi.n, mi.n_tokens, r.N_out

@@ -42,5 +42,45 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+SASS_MNEMONICS = ["UTCHMMA", "UTCBAR", "LDTM", "UTMALDG", "UBLKCP", "SYNCS", "UCGABAR", "ELECT", "FENCE", "REDUX", "MATCH", "MUFU.EX2",
+                  "IMAD.WIDE", "LDG.E.128", "STG.E.128", "LDS.128", "STS.128", "ATOMG", "ATOMS", "BAR.SYNC", "HMMA", "LDL", "STL"]
+
+
+def sass_census() -> str:
+    """Per-kernel count of the SASS mnemonics that show which hardware path a kernel uses (`cuobjdump -sass libajt.so`):
+    UTCHMMA / UTCBAR / LDTM = tcgen05.mma / commit / ld (TMEM), UTMALDG = TMA tensor load, UBLKCP = 1-D bulk async copy,
+    SYNCS = mbarrier, UCGABAR = cluster barrier, REDUX = warp reduce, MUFU.EX2 = exp2, LDL / STL = local-memory traffic
+    (spills or indexed register arrays).  Returns a markdown table."""
+    import collections
+    import re
+
+    build()
+    cuobjdump = os.path.join(os.path.dirname(os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")), "cuobjdump")
+    text = subprocess.run([cuobjdump, "-sass", LIB], capture_output=True, text=True, check=True).stdout
+    per, cur = collections.OrderedDict(), None
+    for line in text.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            cur = per.setdefault(m.group(1), collections.Counter())
+            continue
+        m = re.match(r"\s+/\*[0-9a-f]+\*/\s+(?:@!?U?P\w+\s+)?([A-Z][A-Z0-9_.]*)", line)
+        if m and cur is not None:
+            cur["instructions"] += 1
+            for p in SASS_MNEMONICS:
+                if m.group(1).startswith(p):
+                    cur[p] += 1
+    names = subprocess.run(["c++filt"], input="\n".join(per), capture_output=True, text=True).stdout.splitlines()
+    cols = ["instructions"] + [p for p in SASS_MNEMONICS if any(c[p] for c in per.values())]
+    out = ["| kernel | " + " | ".join(cols) + " |", "|---|" + "---:|" * len(cols)]
+    for (_, c), n in zip(per.items(), names):
+        n = re.sub(r"\(anonymous namespace\)::", "", n)
+        n = re.sub(r"\(.*", "", n).replace("void ", "")
+        out.append(f"| `{n}` | " + " | ".join(str(c[k]) if c[k] else "" for k in cols) + " |")
+    return "\n".join(out)
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--sass-census" in sys.argv:
+        print(sass_census())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -729,16 +729,58 @@ __global__ void __launch_bounds__(256) segment_counts_kernel(const uint8_t* __re
                                                              uint32_t* __restrict__ status) {
     const int lane = threadIdx.x & 31;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    const int64_t Tpad = (T + 31) & ~(int64_t)31;   // whole warps stay converged for match.any
-    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < Tpad; t += stride) {
-        bool act = t < T && mask[t] != 0;
-        const int sg = act ? seg_ids[t] : 0;
-        if (act && (unsigned)sg >= (unsigned)S) {
-            if (status) atomicOr(status, (uint32_t)AJT_STATUS_BAD_SEG);
-            act = false;
+    const int64_t gtid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // Vector body: 4 positions per thread and iteration (one 4-byte mask load, one 16-byte segment-id load), whenever both
+    // arrays reach their alignment at the same position h; segments are long runs, so a warp's 128 positions almost always
+    // carry one id and cost one atomic.  Counts are integers below 2^24, so the float adds are exact in any order.
+    int64_t h = (4 - (int64_t)(reinterpret_cast<uintptr_t>(mask) & 3)) & 3;
+    const bool vec = ((reinterpret_cast<uintptr_t>(seg_ids) >> 2) + (uintptr_t)h) % 4 == 0;
+    if (!vec) h = T;
+    if (h > T) h = T;
+    const int64_t nq = vec ? (T - h) / 4 : 0;
+    const int64_t nq_pad = (nq + 31) & ~(int64_t)31;
+    for (int64_t q = gtid; q < nq_pad; q += stride) {
+        int sg = -1, cnt = 0;
+        if (q < nq) {
+            const uint32_t m4 = *reinterpret_cast<const uint32_t*>(mask + h + 4 * q);
+            if (m4) {
+                const int4 s4 = *reinterpret_cast<const int4*>(seg_ids + h + 4 * q);
+                const int sv[4] = {s4.x, s4.y, s4.z, s4.w};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    if (!((m4 >> (8 * i)) & 0xffu)) continue;
+                    if ((unsigned)sv[i] >= (unsigned)S) {
+                        if (status) atomicOr(status, (uint32_t)AJT_STATUS_BAD_SEG);
+                        continue;
+                    }
+                    if (sg < 0) sg = sv[i];
+                    if (sv[i] == sg) ++cnt;
+                    else atomicAdd(&denom[sv[i]], 1.0f);
+                }
+            }
         }
-        const unsigned peers = __match_any_sync(0xffffffffu, act ? sg : -1 - lane);
-        if (act && lane == __ffs(peers) - 1) atomicAdd(&denom[sg], (float)__popc(peers));
+        const unsigned have = __ballot_sync(0xffffffffu, cnt > 0);
+        if (!have) continue;
+        const int s0 = __shfl_sync(0xffffffffu, sg, __ffs(have) - 1);
+        if (__all_sync(0xffffffffu, cnt == 0 || sg == s0)) {
+            const int tot = __reduce_add_sync(0xffffffffu, cnt);
+            if (lane == 0) atomicAdd(&denom[s0], (float)tot);
+        } else if (cnt > 0) {
+            atomicAdd(&denom[sg], (float)cnt);
+        }
+    }
+    // scalar head / tail (and the whole range when the two alignments never meet)
+    const int64_t t_tail = vec ? h + 4 * nq : 0;
+    const int64_t n_sc = vec ? h + (T - t_tail) : T;
+    for (int64_t i = gtid; i < n_sc; i += stride) {
+        const int64_t t = (vec && i >= h) ? t_tail + (i - h) : i;
+        if (mask[t] == 0) continue;
+        const int sg = seg_ids[t];
+        if ((unsigned)sg >= (unsigned)S) {
+            if (status) atomicOr(status, (uint32_t)AJT_STATUS_BAD_SEG);
+            continue;
+        }
+        atomicAdd(&denom[sg], 1.0f);
     }
 }
 

@@ -41,9 +41,6 @@
 //   K5 merge_scatter_kernel     M7  warp per output tile: one record lookup, then plain coalesced copies -- lane l moves
 //                                   positions l + 32 j of the tile: tokens from the survivor, mask / src constants of the
 //                                   segment, old_logp from the supplying member -- whatever the alignment of the sources
-#include <cstdio>
-#include <cstdlib>
-
 #include "ajt_common.cuh"
 #include "../../include/ajt_test.h"
 
@@ -426,16 +423,6 @@ __device__ __forceinline__ void emit_units(int2* unit_rec, const uint32_t* ub, i
 // ---------------------------------------------------------------------------------------- K1: group (M1)
 
 constexpr uint32_t kEmpty = 0xFFFFFFFFu;
-#ifdef AJT_PROF
-__device__ __forceinline__ uint64_t gtimer() { uint64_t t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define AJT_TICK(k) do { __syncthreads(); if (threadIdx.x == 0) reinterpret_cast<unsigned long long*>(p.ctrl->reserved)[k] = gtimer(); } while (0)
-#define AJT_TMAX(k) do { if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned long long*>(p.ctrl->reserved) + (k), (unsigned long long)gtimer()); } while (0)
-#define AJT_TMIN(k) do { if (threadIdx.x == 0) atomicMin(reinterpret_cast<unsigned long long*>(p.ctrl->reserved) + (k), (unsigned long long)gtimer()); } while (0)
-#else
-#define AJT_TICK(k) do { } while (0)
-#define AJT_TMAX(k) do { } while (0)
-#define AJT_TMIN(k) do { } while (0)
-#endif
 
 // n <= kGrpSmemN.  Dynamic shared memory (H = hash-table slots, passed by the host; G <= n groups):
 //   B1 [H+2] u32  table keys              -> members per group -> group starts (sorted position, exclusive scan)
@@ -470,7 +457,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
 #pragma unroll 1
     for (int g = tid; g < n + 2; g += 1024) { B4[g] = 0; B5[g] = 0; }
     __syncthreads();
-    AJT_TICK(0);
     // ---- validate offsets; trajectory id -> table slot; the thread that claims a slot numbers the group
     uint32_t bad = 0;
 #pragma unroll 1
@@ -518,7 +504,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
         return;
     }
     const int G = (int)s_ng;
-    AJT_TICK(1);
     // ---- the table keys are done: B1 becomes the per-group member count
 #pragma unroll 1
     for (int i = tid; i < n; i += 1024) B6[i] = B2[B6[i]];
@@ -532,10 +517,8 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
         atomicMax(&B5[g], B3[i + 1] - B3[i]);
     }
     __syncthreads();
-    AJT_TICK(2);
     block_scan<1024, 8>(
         G + 1, [&](int g) { return g < G ? B1[g] : 0u; }, [&](int g, int64_t ex, int64_t) { B1[g] = (uint32_t)ex; }, s_w);
-    AJT_TICK(3);
     // ---- place the members (any order inside a group) ...
 #pragma unroll 1
     for (int i = tid; i < n; i += 1024) {
@@ -543,7 +526,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
         B7[B1[g] + atomicAdd(&B4[g], 1u)] = (uint16_t)i;
     }
     __syncthreads();
-    AJT_TICK(12);
     // ---- ... and put them in input order, one warp per group: a bitonic network over the lanes for groups of up to 32
     // (15 shuffles), ranking by counting (members are read as broadcasts) for larger ones
 #pragma unroll 1
@@ -598,7 +580,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
         }
     }
     __syncthreads();
-    AJT_TICK(4);
     // ---- key slots and hash units by group (two scans), hash slices by sorted position (one scan)
     const int64_t E = block_scan<1024, 8>(
         G + 1, [&](int g) { const int64_t k = g < G ? B1[g + 1] - B1[g] : 0; return k * (k + 1) / 2; },
@@ -610,7 +591,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
         if (tid == 0) group_fail(p, (uint32_t)AJT_STATUS_PROBE_CAPACITY);
         return;
     }
-    AJT_TICK(5);
     const int64_t nslice = block_scan<1024, 8>(
         n,
         [&](int pos) {
@@ -621,7 +601,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
     // ---- records by sorted position: coalesced stores.  A lone SM cannot afford 7,862 scattered 8-byte loads (one sector
     // each, ~15 us), so the token offsets come from the 32-bit copies kept since the first phase whenever N < 2^32.
     const bool off32 = p.N < ((int64_t)1 << 32);
-    AJT_TICK(15);
 #pragma unroll 2
     for (int pos = tid; pos < n; pos += 1024) {
         const uint32_t i = B8[pos], g = B6[i], gs = B1[g], r = (uint32_t)pos - gs;
@@ -631,7 +610,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
         p.goff[pos] = off32 ? (int64_t)B3[i] : __ldg(p.offsets + i);
         p.lbad[pos] = 0;
     }
-    AJT_TICK(6);
 #pragma unroll 1
     for (int g = tid; g <= G; g += 1024)
         p.grp_rec[g] = make_int4((int)B1[g], g < G ? (int)(B1[g + 1] - B1[g]) : 0, (int)B4[g], (int)B5[g]);
@@ -642,7 +620,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
         p.ctrl->n_hash_segs = (int32_t)nslice;
         p.ctrl->n_units = (int32_t)U;
     }
-    AJT_TICK(7);
 }
 
 // The same for any n: a stable LSD radix sort of (traj_id - min, index) and block scans, through arrays in the workspace.
@@ -841,12 +818,6 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
     }
     __syncwarp();
     uint32_t phases = 0;   // bit s: the parity stage s completes next
-#ifdef AJT_PROF
-    long long c_wait = 0, c_setup = 0, c_keys = 0, c_issue = 0; const long long c_begin = clock64();
-#define HP(x) x
-#else
-#define HP(x)
-#endif
     const int U = p.ctrl->n_units;
     const int32_t* __restrict__ tokens = p.tokens;
     const int64_t N = p.N;
@@ -858,7 +829,6 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
     next = __shfl_sync(0xffffffffu, next, 0);
     while (next < U) {
         const int u = next;
-        HP(const long long c_u0 = clock64();)
         if (lane == 0) next = atomicAdd(&p.ctrl->unit_ticket, 1);   // needed only after this unit: the round trip is hidden
         const int2 ur = __ldg(p.unit_rec + u);                      // {group, slice}: largest units first
         const int4 gr = __ldg(p.grp_rec + ur.x);
@@ -933,16 +903,11 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
         unsigned fvalid = 0;    // ranks whose Fk belongs to the latest member
         issue_next();
         issue_next();           // two members ahead: the predecessor's stage stays intact while a member is compared with it
-        HP(c_setup += clock64() - c_u0;)
 #pragma unroll 1
         while (consumed < issued) {
-            HP(const long long c_i0 = clock64();)
             issue_next();
-            HP(c_issue += clock64() - c_i0;)
             const int st = consumed & (kHashStages - 1);
-            HP(const long long c_w0 = clock64();)
             if (!mbar_wait_bounded(&full[st], (phases >> st) & 1u)) dead = true;   // never in practice: a lost copy must not hang the GPU
-            HP(c_wait += clock64() - c_w0;)
             phases ^= 1u << st;
             int r, Lr, sbr, D;
             asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r), "=r"(Lr), "=r"(sbr), "=r"(D) : "r"(sdesc + 16 * st));
@@ -982,7 +947,6 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
             const uint64_t tot = warp_sum_u64_redux(ac0 + ac1);
             if (lane == 0) p.seg_part[sbr + w] = tot;
             // keys: the prefixes (L_a of an earlier member, or L_r itself) that end inside this slice
-            HP(const long long c_k0 = clock64();)
             if (!same) fvalid = 0;
             unsigned m0 = end0 & (r >= 31 ? 0xffffffffu : (2u << r) - 1u);
             if (m0) m0 &= __ballot_sync(0xffffffffu, L0 <= Lr);
@@ -1025,7 +989,6 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
                     }
                 }
             }
-            HP(c_keys += clock64() - c_k0;)
             prev_r = r;
             prev_L = Lr;
             prev_D = D;
@@ -1035,16 +998,6 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
         next = __shfl_sync(0xffffffffu, next, 0);
         if (__any_sync(0xffffffffu, dead)) break;
     }
-#ifdef AJT_PROF
-    if (lane == 0) {
-        unsigned long long* r = reinterpret_cast<unsigned long long*>(p.ctrl->reserved) + 16;
-        atomicAdd(r + 0, (unsigned long long)(clock64() - c_begin));
-        atomicAdd(r + 1, (unsigned long long)c_wait);
-        atomicAdd(r + 2, (unsigned long long)c_setup);
-        atomicAdd(r + 3, (unsigned long long)c_keys);
-        atomicAdd(r + 4, (unsigned long long)c_issue);
-    }
-#endif
     if (dead && lane == 0) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_INTERNAL);
 }
 
@@ -1297,9 +1250,6 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
     const bool longest = p.owner_rule == AJT_OWNER_LONGEST;
     const bool explicit_masks = p.mask_in != nullptr;
     if (tid == 0) sm.coll = 0;
-#ifdef AJT_PROF
-    if (tid == 0 && reinterpret_cast<unsigned long long*>(p.ctrl->reserved)[8] == 0) reinterpret_cast<unsigned long long*>(p.ctrl->reserved)[8] = gtimer();
-#endif
     for (int g = blockIdx.x; g < G; g += gridDim.x) {
         const int4 gr = __ldg(p.grp_rec + g);
         const int gs = gr.x, k = gr.y, eb = gr.z;
@@ -1579,7 +1529,6 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
         }
         __syncthreads();
     }
-    AJT_TMAX(9);
     if (tid == 0 && sm.coll) {
         atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_HASH_COLLISION);
         p.ctrl->collision = 1;
@@ -1660,14 +1609,6 @@ __device__ __forceinline__ GSeg load_gseg(const GSeg* g) {
     o.src = b.z;
     o.aux = b.w;
     return o;
-}
-__device__ __forceinline__ void stg32_stream(void* ptr, uint32_t v) {
-    asm volatile("st.global.L1::no_allocate.u32 [%0], %1;" ::"l"(ptr), "r"(v) : "memory");
-}
-__device__ __forceinline__ uint32_t ldg32_stream(const void* ptr) {
-    uint32_t v;
-    asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(ptr));
-    return v;
 }
 
 // One tile moved position by position through registers, walking the segment records from the tile's first one: the path
@@ -2011,19 +1952,13 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
         if (cudaMemsetAsync(merged_offsets, 0, sizeof(int64_t), stream) != cudaSuccess) return AJT_ERR_CUDA;
         return AJT_OK;
     }
-#define AJT_DBG(name) do { if (getenv("AJT_DEBUG_SYNC")) { cudaError_t e_ = cudaStreamSynchronize(stream); fprintf(stderr, "[ajt] %s: %s\n", name, cudaGetErrorString(e_)); } } while (0)
     if (n <= kGrpSmemN) AJT_LAUNCH(merge_group_fast_kernel<<<1, 1024, group_fast_smem(n), stream>>>(p, n + n / 8 + 16));
     else AJT_LAUNCH(merge_group_radix_kernel<<<1, 1024, 0, stream>>>(p));
-    AJT_DBG("group");
     AJT_LAUNCH(merge_hash_kernel<<<num_sms * 2, kHashThreads, kHashSmem, stream>>>(p));
-    AJT_DBG("hash");
     AJT_LAUNCH(merge_select_kernel<<<num_sms * 4, kSelThreads, sizeof(SelectStage), stream>>>(p));
-    AJT_DBG("select");
     AJT_LAUNCH(merge_compact_kernel<<<1, 1024, kCompactSmem, stream>>>(p));
     const int64_t want = ((n_tokens >> kTSLog) + 1 + 255) / 256 + ((int64_t)n * 32 + 255) / 256;
     AJT_LAUNCH(merge_plan_kernel<<<(int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8), 256, 0, stream>>>(p));
-    AJT_DBG("plan");
     AJT_LAUNCH(merge_scatter_kernel<<<num_sms, kScatThreads, kScatSmem, stream>>>(p));
-    AJT_DBG("scatter");
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }

@@ -234,3 +234,14 @@ def test_segment_counts():
     assert int(st[0]) & ajt.STATUS_BAD_SEG
     assert got.sum().item() == want.sum() - 1
     assert ajt.segment_counts(mk[:0], sg[:0], 3).cpu().tolist() == [0.0, 0.0, 0.0]
+    # slices at every alignment of the two arrays (vector body with a scalar head and tail, or the scalar path alone when the
+    # 4-byte mask and 16-byte segment-id alignments never meet), short ranges, and views whose storage offsets differ
+    for a in range(0, 9):
+        for n in (0, 1, 3, 5, 131, 4099, T - 9):
+            w = np.bincount(seg[a:a + n], weights=mask[a:a + n].astype(np.float64), minlength=S).astype(np.float32)
+            assert np.array_equal(ajt.segment_counts(mk[a:a + n], sg[a:a + n], S).cpu().numpy(), w), (a, n)
+    mk_off = torch.zeros(T + 3, dtype=torch.uint8, device="cuda")[3:]
+    mk_off.copy_(mk)
+    assert np.array_equal(ajt.segment_counts(mk_off, sg, S).cpu().numpy(), want)
+    assert np.array_equal(ajt.segment_counts(mk_off[2:], sg[2:], S).cpu().numpy(),
+                          np.bincount(seg[2:], weights=mask[2:].astype(np.float64), minlength=S).astype(np.float32))
