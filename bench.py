@@ -388,7 +388,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         mg = b_merge / (merge_ms * 1e-3) / 1e9
         line = {
             "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": K, "warmup": Wm,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak" if world == 1 else "strong",
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None,
             "dtype": "f32 (bf16 logits/dlogits in HBM, fp64 scalar; merge int32/u64)", "data": "synthetic",
             "config": workload_config(mi_full.n, mi_full.n_tokens, B, T, rho, world),

@@ -1,4 +1,4 @@
-"""Measurement harness shared by bench.py and sweep.py: algorithmic byte counts, input synthesis on the device, CUDA-event
+"""Measurement harness used by bench.py and the full-size tests: algorithmic byte counts, input synthesis on the device, CUDA-event
 timing with an L2 flush.  None of the method's steps is computed here (the one softmax below only SYNTHESISES the
 `old_logp` input as "new logp + noise", BASELINE.json configs), and nothing here touches the oracle."""
 from __future__ import annotations

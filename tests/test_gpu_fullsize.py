@@ -1,4 +1,4 @@
-"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py / sweep.py time.
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
 
 The oracle cannot produce [T,V] fp64 gradients for 40k-131k rows of a 151,936-wide vocabulary, so at these sizes:
   * sampled rows (first, last, random unmasked, random masked) are checked element by element against the oracle,
@@ -272,7 +272,7 @@ def test_every_sweep_cell_sampled(T, V, rho):
 
 
 def test_lm_head_full_size_sampled_rows():
-    """ajt_lm_head_logp at the size sweep `h1` times (40,960 x 4,096 x 151,936: CTA pairs, 9 waves of row blocks, 4 vocabulary
+    """ajt_lm_head_logp at the size bench.py's LM-head record times (40,960 x 4,096 x 151,936: CTA pairs, 9 waves of row blocks, 4 vocabulary
     ranges of 149 tiles): sampled rows against the fp64 oracle computed row by row; every row finite and a valid log-prob."""
     T, d, V = 40960, 4096, 151936
     g = torch.Generator(device="cuda").manual_seed(41)
@@ -322,7 +322,7 @@ def test_lm_head_loss_bwd_full_width_against_oracle():
 
 
 def test_lm_head_loss_bwd_bench_size_properties():
-    """The size the sweep times (40,960 x 4,096 x 151,936, mask density ~0.34: 4 chunks of staged dZ): sampled dH rows against
+    """The size bench.py's LM-head record times (40,960 x 4,096 x 151,936, mask density ~0.34: 4 chunks of staged dZ): sampled dH rows against
     the oracle computed row by row (the row's own 151,936 logits in fp64), masked rows exactly zero, and two identities of
     the exact gradients that tie dW to them at any size: sum_v dW_v = 0 (every dZ row sums to zero) and <dW, W> = sum_t <dH_t, h_t>."""
     T, d, V, S = 40960, 4096, 151936, 64
