@@ -21,7 +21,7 @@ struct AjtCtrl {
     // merge
     int32_t n_groups;
     int32_t n_entries;    // sum_g k_g (k_g+1)/2
-    int32_t n_hash_segs;  // hash slices: sum over timelines of grouped (k >= 2) groups of ceil(L / 512)
+    int32_t n_hash_segs;  // hash slices: sum over timelines of grouped (k >= 2) groups of ceil(L / 508)
     int32_t M;
     int64_t N_out;
     int32_t collision;    // informational: a hash-equal candidate failed the exact comparison in the select pass
@@ -29,9 +29,9 @@ struct AjtCtrl {
     int32_t tile_counter; // loss prep: dynamic tile ticket (ordered, so a tile's predecessors have always started)
     int32_t done_counter; // loss prep: CTAs finished (the last one finalises 1/S')
     // merge (round 2)
-    int32_t n_units;      // hash units: sum over grouped groups of ceil(max L / 512)
+    int32_t n_units;      // hash units: (chunk of ranks, block of slices) pairs
     int32_t unit_ticket;  // hash pass: dynamic unit ticket
-    int32_t sel_done;     // select pass: CTAs finished (the last one compacts)
+    int32_t n_chunks;     // chunks of consecutive ranks of grouped groups
     int32_t n_gsegs;      // scatter segments (constant-source runs of the merged output)
     uint32_t reserved[44];
 };

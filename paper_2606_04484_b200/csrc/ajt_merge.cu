@@ -48,8 +48,10 @@ namespace {
 
 using namespace ajt;
 
-constexpr int kSl = 512;           // hash slice: 512 token positions = 16 per lane
-constexpr int kSlLog = 9;
+constexpr int kSl = 508;           // hash slice: 508 token positions; with up to 3 elements of misalignment a slice is
+                                   // exactly 128 aligned 16-byte vectors = 4 per lane
+__host__ __device__ __forceinline__ int slices_of(int L) { return (L + kSl - 1) / kSl; }
+__host__ __device__ __forceinline__ int slice_at(int pos) { return pos / kSl; }
 constexpr int kTS = 512;           // scatter tile: 512 output positions = 16 per lane
 constexpr int kTSLog = 9;
 constexpr uint32_t kW = 0x9E3779B1u;   // odd multiplier of the prefix hash's 32-bit position weights
@@ -59,9 +61,10 @@ constexpr uint32_t cpow32(uint32_t b, uint32_t e) {
         if (e & 1) r *= b;
     return r;
 }
-constexpr uint32_t kW3 = kW * kW * kW;
-constexpr uint32_t kW32 = cpow32(kW, 32);
-constexpr uint32_t kW512 = cpow32(kW, 512);
+constexpr uint32_t kW128 = cpow32(kW, 128);
+constexpr uint32_t kWSl = cpow32(kW, kSl);
+constexpr uint32_t kWinv = cpow32(kW, 0x7fffffffu);   // W^-1 mod 2^32 (the odd residues have exponent 2^30)
+static_assert(kW * kWinv == 1u, "inverse of the hash multiplier");
 constexpr uint32_t kFatal = AJT_STATUS_BAD_OFFSETS | AJT_STATUS_ZERO_LEN | AJT_STATUS_PROBE_CAPACITY;
 constexpr int kSelThreads = 256;
 constexpr int kSelSmemKeys = 2048;  // groups with more keys than this sort through global memory
@@ -107,10 +110,11 @@ struct MergeParams {
     int32_t* perm;         // [n] sorted position -> timeline index (groups contiguous, input order inside a group)
     int32_t* glen;         // [n] sorted position -> timeline length
     int64_t* goff;         // [n] sorted position -> token offset
-    int4* tl_rec;          // [n] BY SORTED POSITION: {first hash slice, group start (sorted position), rank in group, first key slot}
+    int4* tl_rec;          // [n] BY SORTED POSITION: {first hash slice, group start (sorted position), members of the group, first key slot of the timeline}
     uint8_t* lbad;         // [n] BY SORTED POSITION: the member differs from its in-group predecessor on that one's positions (exact)
     int4* grp_rec;         // [G+1] {group start, members, first key slot, first hash unit}
-    int2* unit_rec;        // [slice_cap] hash units {group, slice}, the largest (lowest slices) first
+    int2* unit_rec;        // [slice_cap] hash units {chunk, slice block}, the largest (lowest slices) first
+    int4* chunk_rec;       // [n+1] chunks of consecutive ranks of a group: {group start (sorted position), first rank, members of the group, first key slot of the group}
     uint64_t* seg_part;    // [slice_cap] per (member, slice) hash totals, then exclusive prefixes per member
     uint64_t* ent_hash;    // [E_cap] key slot (r, a), a = 0..r: in-slice partial, then the final prefix hash
     uint32_t* ent_dig;     // [E_cap] global sort path: digests / order ping-pong
@@ -134,7 +138,7 @@ struct MergeParams {
 };
 
 struct MergeWs {
-    size_t ctrl, gbuf[6], perm, glen, goff, tl_rec, lbad, grp_rec, unit_rec, seg_part, absorbed, owner_tl, midx, sel[8],
+    size_t ctrl, gbuf[6], perm, glen, goff, tl_rec, lbad, grp_rec, unit_rec, chunk_rec, seg_part, absorbed, owner_tl, midx, sel[8],
         sel_q, mem_list, sv_rec, rseg, gseg_base, gseg, tile_seg, ent;
 };
 __host__ inline size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -152,6 +156,7 @@ __host__ MergeWs merge_ws_layout(int32_t n, int64_t N) {
     w.lbad = o; o += a256((size_t)n + 2);
     w.grp_rec = o; o += n16;
     w.unit_rec = o; o += a256(sc * 8);
+    w.chunk_rec = o; o += n16;
     w.seg_part = o; o += a256(sc * 8);
     w.absorbed = o; o += a256((size_t)n + 2);
     w.owner_tl = o; o += n4; w.midx = o; o += n4;
@@ -169,6 +174,13 @@ __host__ MergeWs merge_ws_layout(int32_t n, int64_t N) {
 constexpr size_t kEntBytes = 32;  // per key slot: hash 8, dig 4, idx 4, tmp_dig 4, tmp_idx 4 = 24 used; ajt.h promises 32 per pair
 
 __device__ __forceinline__ bool fatal(const MergeParams& p) { return (p.ctrl->status & kFatal) != 0; }
+// Programmatic dependent launch: kernels 2..6 of the pipeline are launched while their predecessor still runs, so their CTAs
+// are resident (launch latency, shared-memory carve-out, parameter loads) when it ends.  Nothing the predecessor wrote is
+// read before pdl_wait(), which returns once the predecessor grid has completed and its writes are visible.
+__device__ __forceinline__ void pdl_wait() {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
 
 __device__ __forceinline__ uint32_t digest32(uint64_t h, int32_t len) {
     uint64_t z = h ^ ((uint64_t)(uint32_t)len * 0xD6E8FEB86659FD93ull);
@@ -176,15 +188,6 @@ __device__ __forceinline__ uint32_t digest32(uint64_t h, int32_t len) {
     z *= 0xD6E8FEB86659FD93ull;
     z ^= z >> 32;
     return (uint32_t)z;
-}
-__device__ __forceinline__ uint64_t mad_wide(uint32_t a, uint32_t b, uint64_t c) { return (uint64_t)a * b + c; }
-// Sum of a 64-bit value over the warp (mod 2^64) with three REDUX instead of ten shuffles: 22 + 22 + 20-bit slices, whose
-// 32-term sums fit 32 bits.
-__device__ __forceinline__ uint64_t warp_sum_u64_redux(uint64_t v) {
-    const uint32_t a = (uint32_t)v & 0x3fffffu, b = (uint32_t)(v >> 22) & 0x3fffffu, c = (uint32_t)(v >> 44);
-    const uint32_t sa = __reduce_add_sync(0xffffffffu, a), sb = __reduce_add_sync(0xffffffffu, b);
-    const uint32_t sc = __reduce_add_sync(0xffffffffu, c);
-    return (uint64_t)sa + ((uint64_t)sb << 22) + ((uint64_t)sc << 44);
 }
 __device__ __forceinline__ int64_t shfl_i64(int64_t v, int src) {
     const uint32_t lo = __shfl_sync(0xffffffffu, (uint32_t)v, src), hi = __shfl_sync(0xffffffffu, (uint32_t)((uint64_t)v >> 32), src);
@@ -352,73 +355,8 @@ __device__ __forceinline__ void group_fail(const MergeParams& p, uint32_t bits) 
     p.merged_offsets[0] = 0;
 }
 
-// Hash units in the order the hash pass takes them: slice 0 of every group, then slice 1, ... (a unit's work is the number
-// of members that reach its slice, so the longest units go first and the tail of the pass is made of short ones); slices
-// from 128 on follow group by group.  ub[g] = first unit of group g in group-major numbering (exclusive scan, ub[G] = U).
-// One CTA of 1024 threads; s_cnt / s_C: 130 words of shared scratch each.
-constexpr int kUnitRows = 128;
-__device__ __forceinline__ void emit_units(int2* unit_rec, const uint32_t* ub, int G, uint32_t* s_cnt, uint32_t* s_C) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int w = tid; w <= kUnitRows + 1; w += 1024) { s_cnt[w] = 0; s_C[w] = 0; }
-    __syncthreads();
-    for (int g = tid; g < G; g += 1024) {
-        const uint32_t un = ub[g + 1] - ub[g];
-        if (un) atomicAdd(&s_cnt[min(un, (uint32_t)kUnitRows)], 1u);   // histogram of units per group, capped
-        if (un > (uint32_t)kUnitRows) s_cnt[kUnitRows + 1] = 1;        // some group has slices beyond the rows
-    }
-    __syncthreads();
-    if (warp == 0) {   // row w holds the groups with more than w units: suffix sums of the histogram, then their running total
-        uint32_t h[4], c[4], sfx = 0;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) h[j] = s_cnt[4 * lane + j + 1];   // groups with exactly 4 lane + j + 1 units
-#pragma unroll
-        for (int j = 3; j >= 0; --j) { sfx += h[j]; c[j] = sfx; }      // within the lane
-        uint32_t inc = sfx;                                            // + the lanes above
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_down_sync(0xffffffffu, inc, o);
-            if (lane + o < 32) inc += t;
-        }
-        const uint32_t above = inc - sfx;
-        uint32_t rowsum = 0;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) { c[j] += above; rowsum += c[j]; }   // c[j] = groups with more than 4 lane + j units
-        uint32_t pre = rowsum;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(0xffffffffu, pre, o);
-            if (lane >= o) pre += t;
-        }
-        uint32_t run = pre - rowsum;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) { s_C[4 * lane + j] = run; run += c[j]; }
-        if (lane == 31) s_C[kUnitRows] = run;
-    }
-    __syncthreads();
-    for (int w = warp; w < kUnitRows; w += 32) {
-        const uint32_t base = s_C[w];
-        if (s_C[w + 1] == base) break;   // no group has more than w units, nor any later row
-        uint32_t run = 0;
-        for (int g0 = 0; g0 < G; g0 += 32) {
-            const int g = g0 + lane;
-            const bool has = g < G && ub[g + 1] - ub[g] > (uint32_t)w;
-            const unsigned bal = __ballot_sync(0xffffffffu, has);
-            if (has) unit_rec[base + run + __popc(bal & ((1u << lane) - 1u))] = make_int2(g, w);
-            run += __popc(bal);
-        }
-    }
-    // slices from kUnitRows on (timelines beyond 64k tokens): group-major after the rows; one warp, running offset
-    if (warp == 0 && s_cnt[kUnitRows + 1]) {
-        uint32_t run = s_C[kUnitRows];
-        for (int g = 0; g < G; ++g) {
-            const uint32_t un = ub[g + 1] - ub[g];
-            if (un > (uint32_t)kUnitRows) {
-                for (uint32_t x = kUnitRows + lane; x < un; x += 32) unit_rec[run + x - kUnitRows] = make_int2(g, (int)x);
-                run += un - kUnitRows;
-            }
-        }
-    }
-}
+constexpr int kChunk = 8;      // hash units: a group's members are cut into chunks of this many consecutive ranks ...
+constexpr int kSliceBlk = 1;   // ... and a chunk's slices into blocks of this many: one warp's critical path is ~9 member-slices
 
 // ---------------------------------------------------------------------------------------- K1: group (M1)
 
@@ -439,7 +377,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
     extern __shared__ __align__(16) uint8_t g_dyn[];
     __shared__ int64_t s_w[2][2][32];
     __shared__ uint32_t s_bad, s_ng;
-    __shared__ uint32_t s_cnt[kUnitRows + 2], s_C[kUnitRows + 2];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = p.n;
     uint32_t* const B1 = reinterpret_cast<uint32_t*>(g_dyn);
     uint16_t* const B2 = reinterpret_cast<uint16_t*>(B1 + (H + 2));
@@ -514,7 +451,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
     for (int i = tid; i < n; i += 1024) {
         const uint32_t g = B6[i];
         atomicAdd(&B1[g], 1u);
-        atomicMax(&B5[g], B3[i + 1] - B3[i]);
     }
     __syncthreads();
     block_scan<1024, 8>(
@@ -584,9 +520,6 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
     const int64_t E = block_scan<1024, 8>(
         G + 1, [&](int g) { const int64_t k = g < G ? B1[g + 1] - B1[g] : 0; return k * (k + 1) / 2; },
         [&](int g, int64_t ex, int64_t) { B4[g] = (uint32_t)min(ex, (int64_t)INT32_MAX); }, s_w);
-    const int64_t U = block_scan<1024, 8>(
-        G + 1, [&](int g) { return g < G && B1[g + 1] - B1[g] >= 2 ? (B5[g] + kSl - 1) >> kSlLog : 0u; },
-        [&](int g, int64_t ex, int64_t) { B5[g] = (uint32_t)ex; }, s_w);
     if (E > (int64_t)p.E_cap) {   // (slices and units always fit: the workspace is sized for their worst case)
         if (tid == 0) group_fail(p, (uint32_t)AJT_STATUS_PROBE_CAPACITY);
         return;
@@ -595,7 +528,7 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
         n,
         [&](int pos) {
             const uint32_t i = B8[pos], g = B6[i];
-            return B1[g + 1] - B1[g] < 2 ? 0u : (B3[i + 1] - B3[i] + kSl - 1) >> kSlLog;
+            return B1[g + 1] - B1[g] < 2 ? 0u : (uint32_t)slices_of((int)(B3[i + 1] - B3[i]));
         },
         [&](int pos, int64_t ex, int64_t) { B9[pos] = (uint32_t)ex; }, s_w);
     // ---- records by sorted position: coalesced stores.  A lone SM cannot afford 7,862 scattered 8-byte loads (one sector
@@ -604,7 +537,7 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
 #pragma unroll 2
     for (int pos = tid; pos < n; pos += 1024) {
         const uint32_t i = B8[pos], g = B6[i], gs = B1[g], r = (uint32_t)pos - gs;
-        p.tl_rec[pos] = make_int4((int)B9[pos], (int)gs, (int)r, (int)(B4[g] + r * (r + 1) / 2u));
+        p.tl_rec[pos] = make_int4((int)B9[pos], (int)gs, (int)(B1[g + 1] - gs), (int)(B4[g] + r * (r + 1) / 2u));
         p.perm[pos] = (int32_t)i;
         p.glen[pos] = (int32_t)(B3[i + 1] - B3[i]);
         p.goff[pos] = off32 ? (int64_t)B3[i] : __ldg(p.offsets + i);
@@ -612,13 +545,11 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
     }
 #pragma unroll 1
     for (int g = tid; g <= G; g += 1024)
-        p.grp_rec[g] = make_int4((int)B1[g], g < G ? (int)(B1[g + 1] - B1[g]) : 0, (int)B4[g], (int)B5[g]);
-    emit_units(p.unit_rec, B5, G, s_cnt, s_C);
+        p.grp_rec[g] = make_int4((int)B1[g], g < G ? (int)(B1[g + 1] - B1[g]) : 0, (int)B4[g], 0);
     if (tid == 0) {
         p.ctrl->n_groups = G;
         p.ctrl->n_entries = (int32_t)E;
         p.ctrl->n_hash_segs = (int32_t)nslice;
-        p.ctrl->n_units = (int32_t)U;
     }
 }
 
@@ -628,11 +559,9 @@ __global__ void __launch_bounds__(1024) merge_group_radix_kernel(const MergePara
     __shared__ int64_t s_w[2][2][32];
     __shared__ int s_min, s_max;
     __shared__ uint32_t s_bad;
-    __shared__ uint32_t s_cnt[kUnitRows + 2], s_C[kUnitRows + 2];
     const int tid = threadIdx.x, n = p.n;
     uint32_t* kb[2] = {p.gbuf[0], p.gbuf[1]};
     uint32_t* vb[2] = {p.gbuf[2], p.gbuf[3]};
-    uint32_t* gun = p.gbuf[4];                                   // [g] hash units of group g, then their exclusive scan
     int32_t* tln = reinterpret_cast<int32_t*>(p.gbuf[5]);        // [i] length of timeline i
     if (tid < (int)(sizeof(AjtCtrl) / 4)) reinterpret_cast<uint32_t*>(p.ctrl)[tid] = 0;   // fresh control block
     if (tid == 0) { s_min = INT32_MAX; s_max = INT32_MIN; s_bad = 0; }
@@ -694,44 +623,77 @@ __global__ void __launch_bounds__(1024) merge_group_radix_kernel(const MergePara
     const int64_t E = block_scan<1024, 4>(
         G, [&](int g) { const int64_t k = gsv[g + 1] - gsv[g]; return k * (k + 1) / 2; },
         [&](int g, int64_t ex, int64_t) { gent[g] = (uint32_t)min(ex, (int64_t)INT32_MAX); }, s_w);
-    // hash units of a group = slices up to its longest member (none for singleton groups)
-    const int64_t U = block_scan<1024, 1>(
-        G,
-        [&](int g) {
-            const int k = (int)(gsv[g + 1] - gsv[g]);
-            if (k < 2) return (int64_t)0;
-            int mx = 0;
-            for (int x = 0; x < k; ++x) mx = max(mx, tln[val[gsv[g] + x]]);
-            return (int64_t)((mx + kSl - 1) >> kSlLog);
-        },
-        [&](int g, int64_t ex, int64_t) { gun[g] = (uint32_t)ex; }, s_w);
-    if (tid == 0) { gent[G] = (uint32_t)min(E, (int64_t)INT32_MAX); gun[G] = (uint32_t)U; }
+    if (tid == 0) gent[G] = (uint32_t)min(E, (int64_t)INT32_MAX);
     // hash slices: numbered in GROUP order, by sorted position
     const int64_t nslice = block_scan<1024, 4>(
-        n, [&](int pos) { const int g = (int)gid[pos]; return gsv[g + 1] - gsv[g] < 2 ? 0 : (tln[val[pos]] + kSl - 1) >> kSlLog; },
+        n, [&](int pos) { const int g = (int)gid[pos]; return gsv[g + 1] - gsv[g] < 2 ? 0 : slices_of((int)tln[val[pos]]); },
         [&](int pos, int64_t ex, int64_t) {
             const int i = (int)val[pos], g = (int)gid[pos];
             const int gs = (int)gsv[g], r = pos - gs;
-            p.tl_rec[pos] = make_int4((int)ex, gs, r, (int)(gent[g] + (uint32_t)r * (uint32_t)(r + 1) / 2u));
+            p.tl_rec[pos] = make_int4((int)ex, gs, (int)(gsv[g + 1] - gsv[g]), (int)(gent[g] + (uint32_t)r * (uint32_t)(r + 1) / 2u));
             p.perm[pos] = i;
             p.glen[pos] = tln[i];
             p.goff[pos] = __ldg(p.offsets + i);
             p.lbad[pos] = 0;
         },
         s_w);
-    if (E > (int64_t)p.E_cap || nslice > (int64_t)p.slice_cap || U > (int64_t)p.slice_cap) {
+    if (E > (int64_t)p.E_cap || nslice > (int64_t)p.slice_cap) {   // (units <= slices)
         if (tid == 0) group_fail(p, (uint32_t)AJT_STATUS_PROBE_CAPACITY);
         return;
     }
     for (int g = tid; g <= G; g += 1024)
-        p.grp_rec[g] = make_int4((int)gsv[g], g < G ? (int)(gsv[g + 1] - gsv[g]) : 0, (int)gent[g], (int)gun[g]);
-    __syncthreads();
-    emit_units(p.unit_rec, gun, G, s_cnt, s_C);
+        p.grp_rec[g] = make_int4((int)gsv[g], g < G ? (int)(gsv[g + 1] - gsv[g]) : 0, (int)gent[g], 0);
     if (tid == 0) {
         p.ctrl->n_groups = G;
         p.ctrl->n_entries = (int32_t)E;
         p.ctrl->n_hash_segs = (int32_t)nslice;
-        p.ctrl->n_units = (int32_t)U;
+    }
+}
+
+// ---------------------------------------------------------------------------------------- K1b: hash units
+
+// Hash units, in parallel over the whole GPU (the group kernel is one SM): thread per sorted position; the thread of a rank
+// that is a multiple of kChunk in a group of at least two opens a chunk {group start, first rank, members, first key slot} and
+// one unit per block of kSliceBlk slices up to the chunk's longest member.  Chunk ids and unit slots come from two counters
+// (one atomic per warp each); units are short (<= kChunk + 1 member-slices per slice), so their order does not matter.
+__global__ void __launch_bounds__(256) merge_units_kernel(const MergeParams p) {
+    pdl_wait();
+    if (fatal(p)) return;
+    const int lane = threadIdx.x & 31, n = p.n;
+    const int npad = (n + 31) & ~31;
+    for (int pos = blockIdx.x * blockDim.x + threadIdx.x; pos < npad; pos += gridDim.x * blockDim.x) {
+        int4 t = make_int4(0, 0, 0, 0);
+        if (pos < n) t = __ldg(p.tl_rec + pos);
+        const int gs = t.y, k = t.z, r = pos - gs;
+        const bool open = pos < n && k >= 2 && r % kChunk == 0;
+        int cnt = 0;
+        if (open) {
+            int mx = 0;
+            for (int x = 0; x < min(kChunk, k - r); ++x) mx = max(mx, __ldg(p.glen + pos + x));
+            cnt = (slices_of(mx) + kSliceBlk - 1) / kSliceBlk;
+        }
+        const unsigned om = __ballot_sync(0xffffffffu, open);
+        if (om == 0) continue;
+        int inc = cnt;   // inclusive scan of the unit counts over the warp
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += v;
+        }
+        const int tot = __shfl_sync(0xffffffffu, inc, 31);
+        int cb = 0, ub = 0;
+        if (lane == 0) {
+            cb = atomicAdd(&p.ctrl->n_chunks, __popc(om));
+            ub = atomicAdd(&p.ctrl->n_units, tot);
+        }
+        cb = __shfl_sync(0xffffffffu, cb, 0);
+        ub = __shfl_sync(0xffffffffu, ub, 0);
+        if (open) {
+            const int c = cb + __popc(om & ((1u << lane) - 1u));
+            p.chunk_rec[c] = make_int4(gs, r, k, t.w - (int)((uint32_t)r * (uint32_t)(r + 1) / 2u));
+            int2* const ur = p.unit_rec + ub + inc - cnt;
+            for (int j = 0; j < cnt; ++j) ur[j] = make_int2(c, j);
+        }
     }
 }
 
@@ -758,8 +720,6 @@ struct PowTab {
         for (int i = 0; i < N; ++i) { v[i] = r; r *= base; }
     }
 };
-__constant__ PowTab<128> c_w512 = PowTab<128>(kW512);   // W^(512 j): slice j of a timeline (64k tokens before the slow path)
-__constant__ PowTab<32> c_w1 = PowTab<32>(kW);          // W^lane
 
 // Last index i in [0, n) with key(i) <= x, for a non-decreasing key with key(0) <= x: warp-cooperative 32-ary search
 // (2 dependent loads for n <= 1024 instead of 10).
@@ -792,29 +752,51 @@ __device__ __forceinline__ uint32_t lds32(uint32_t saddr) {
 __device__ __forceinline__ void sts32(uint32_t saddr, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory"); }
 
 constexpr int kHashThreads = 256;
-constexpr int kHashStages = 4;
-constexpr int kStageBytes = kSl * 4 + 32;                           // 512 tokens + one 16-byte vector of misalignment (+ pad)
-constexpr int kHashWarpBytes = kHashStages * kStageBytes + 128;     // + 4 mbarriers (32 B, padded to 64) + 4 descriptors
+constexpr int kHashStages = 3;          // the member in flight, the member at work, its predecessor
+constexpr int kSlotBytes = 2048;                                    // 128 aligned vectors: the slice + its misalignment
+constexpr int kStageBytes = 16 + kSlotBytes + 16;                   // a zero vector on either side (reads at e + delta, |delta| <= 3)
+constexpr int kHashWarpBytes = kHashStages * kStageBytes + 128;     // + mbarriers (padded to 64 B) + descriptors
 constexpr int kHashSmem = (kHashThreads / 32) * kHashWarpBytes + 128;
+__constant__ PowTab<128> c_wsl = PowTab<128>(kWSl);     // W^(508 j): slice j of a timeline (65k tokens before the slow path)
+__constant__ PowTab<4> c_winv = PowTab<4>(kWinv);       // W^-D: undoes the misalignment of a member in its slot
 
-// Warp per hash unit = (group, slice of 512 positions).  Lane l holds positions S0 + l + 32 t (t < 16) of EVERY member: a
-// member's slice arrives as ONE bulk async copy (TMA, 1-D) of the 16-byte-aligned superset of its bytes, launched by the
-// lane that holds the member's facts and counted on a warp-private mbarrier, and is read with conflict-free 32-bit
-// shared-memory loads at the member's own misalignment.  So the weights are per unit, and member r is compared with member
-// r - 1 stage against stage (a stage is refilled two members behind).  The kernel is bound by instruction issue (~200 per
-// member-slice), not by memory: everything per member that can be computed 32 members at a time is.
-__global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const MergeParams p) {
+__device__ __forceinline__ uint4 lds128(uint32_t saddr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(saddr));
+    return v;
+}
+
+// Warp per hash unit = (chunk of <= kChunk consecutive ranks of a group, block of kSliceBlk slices of 508 positions), taken
+// from an atomic ticket, largest first.  The chunk's members -- preceded by the last member of the previous chunk, which is
+// only there to be compared with -- sit one per lane; for every slice of the block the warp streams the members that reach
+// it, in rank order.  A member's slice arrives as ONE bulk async copy (TMA, 1-D) of the 16-byte-aligned superset of its
+// bytes -- exactly 128 vectors, whatever the member's misalignment D -- launched by the lane that holds the member and
+// counted on a warp-private mbarrier.  Lane l owns vectors l + 32 t (t < 4) of EVERY slot, i.e. slot elements
+// e = 4 (l + 32 t) + i: four conflict-free 16-byte shared-memory loads per member.  The hash is a polynomial in the ring mod
+// 2^32, F(p) = sum_{q<p} x_q W^q: a lane's weights belong to the SLOT elements and never change, and the member's shift
+// (slice start, misalignment) is one multiplication by W^(S0 - D) after the warp reduction (one REDUX: the sum wraps mod 2^32
+// by itself).  Elements outside the member (before D, behind its end) are zeroed in shared memory on arrival, and every
+// slot sits between two zero vectors, so member r is compared with member r - 1 slot against slot at an element shift
+// delta = D' - D without masks; when the two agree over a whole slice the slice total is inherited and nothing is
+// multiplied at all.  Slices in which a member or its predecessor ends take a masked path.  Why chunks: one warp works
+// through its members one after the other (~2 us each), so a unit of 40 members would take as long as the whole kernel.
+__global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const MergeParams p) {
+    pdl_wait();
     extern __shared__ __align__(128) uint8_t h_dyn[];
     if (fatal(p)) return;
     const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
     uint8_t* const wbuf = reinterpret_cast<uint8_t*>(((uintptr_t)h_dyn + 127) & ~(uintptr_t)127) + (size_t)wic * kHashWarpBytes;
     uint64_t* const full = reinterpret_cast<uint64_t*>(wbuf + kHashStages * kStageBytes);
     const uint32_t sdesc = smem_u32(wbuf + kHashStages * kStageBytes + 64);
-    const uint32_t sbuf = smem_u32(wbuf);
+    const uint32_t sbuf = smem_u32(wbuf) + 16;   // element 0 of stage 0
     if (lane == 0) {
 #pragma unroll
         for (int s = 0; s < kHashStages; ++s) mbar_init(&full[s], 1);
         fence_mbar_init();
+    }
+    if (lane < 2 * kHashStages) {   // the zero vectors around every slot (never written again)
+        const uint32_t a = smem_u32(wbuf) + (lane >> 1) * kStageBytes + (lane & 1) * (16 + kSlotBytes);
+        asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
     }
     __syncwarp();
     uint32_t phases = 0;   // bit s: the parity stage s completes next
@@ -822,7 +804,17 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
     const int32_t* __restrict__ tokens = p.tokens;
     const int64_t N = p.N;
     const int mis = p.mis;
-    const uint32_t lw = c_w1.v[lane] * kW3;   // W^(lane + 3)
+    // weights of this lane's vectors: slot elements e = 4 (lane + 32 t) + i weigh W^e = bt[t] W^i (Horner inside a vector)
+    uint32_t bt[4];
+    bt[0] = pow32(kW, 4u * (uint32_t)lane);
+#pragma unroll
+    for (int t = 1; t < 4; ++t) bt[t] = bt[t - 1] * kW128;
+    auto dot = [&](const uint32_t* y) {
+        uint32_t g = 0;
+#pragma unroll
+        for (int t = 0; t < 4; ++t) g += (((y[4 * t + 3] * kW + y[4 * t + 2]) * kW + y[4 * t + 1]) * kW + y[4 * t]) * bt[t];
+        return g;
+    };
     bool dead = false;
     int next = 0;
     if (lane == 0) next = atomicAdd(&p.ctrl->unit_ticket, 1);
@@ -830,169 +822,206 @@ __global__ void __launch_bounds__(kHashThreads, 2) merge_hash_kernel(const Merge
     while (next < U) {
         const int u = next;
         if (lane == 0) next = atomicAdd(&p.ctrl->unit_ticket, 1);   // needed only after this unit: the round trip is hidden
-        const int2 ur = __ldg(p.unit_rec + u);                      // {group, slice}: largest units first
-        const int4 gr = __ldg(p.grp_rec + ur.x);
-        const int gs = gr.x, k = gr.y, w = ur.y;
-        const int64_t eb = gr.z;
-        const int S0 = w << kSlLog;                 // first position of the slice
+        const int2 ur = __ldg(p.unit_rec + u);                      // {chunk, slice block}: largest units first
+        const int4 cr = __ldg(p.chunk_rec + ur.x);                  // {group start, first rank, members of the group, first key slot}
+        const int gs = cr.x, k = cr.z;
+        const int64_t eb = cr.w;
+        const int rlo = cr.y - (cr.y > 0 ? 1 : 0);                  // lane i holds rank rlo + i: the predecessor of the chunk first
+        const int rhi = min(k, cr.y + kChunk);
         const int32_t* __restrict__ gln = p.glen + gs;
-        const int64_t* __restrict__ gof = p.goff + gs;
-        // lane weights of positions S0 + lane + 32 t: the same for every member
-        uint32_t wt[16];
-        wt[0] = (w < 128 ? c_w512.v[w] : pow32(kW512, (uint32_t)w)) * lw;
-#pragma unroll
-        for (int t = 1; t < 16; ++t) wt[t] = wt[t - 1] * kW32;
-        // ---- the members, 32 ranks at a time; each lane works out its own member's copy once
-        int ic0 = 0, iL = 0, isb = 0, iD = 0, inv = 0;
-        int64_t ig0 = 0;
-        unsigned ireach = 0, iedge = 0;
-        auto load_chunk = [&]() {
-            const bool v = ic0 + lane < k;
-            iL = v ? __ldg(gln + ic0 + lane) : 0;
-            const int64_t off = v ? __ldg(gof + ic0 + lane) : 0;
-            isb = v ? __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + ic0 + lane)) : 0;
-            iD = (int)((off + mis) & 3);                    // slot of position S0 in the 16-byte grid
-            ig0 = off + S0 - iD;                             // element index of the first aligned vector
-            inv = (min(iL - S0, kSl) + iD + 3) >> 2;         // vectors holding positions < min(L, S0 + 512)
-            ireach = __ballot_sync(0xffffffffu, iL > S0);
-            iedge = __ballot_sync(0xffffffffu, iL > S0 && !(ig0 >= 0 && ig0 + 4 * (int64_t)inv <= N));
-        };
-        load_chunk();
-        const int L0 = iL;   // lengths of the first 32 ranks: where prefixes end
-        const unsigned end0 = __ballot_sync(0xffffffffu, L0 > 0 && ((L0 - 1) >> kSlLog) == w);
-        bool more = true;
-        int issued = 0, consumed = 0;
-        // launches the next member's copy into stage `issued & 3` (if there is one)
+        // ---- each lane's member: facts that do not depend on the slice
+        const bool mine = rlo + lane < rhi;
+        const int iL = mine ? __ldg(gln + rlo + lane) : 0;
+        const int64_t ioff = mine ? __ldg(p.goff + gs + rlo + lane) : 0;
+        const int isb = mine ? __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + rlo + lane)) : 0;
+        const int iD0 = (int)((ioff + mis) & 3);
+        const int L0 = lane < k ? __ldg(gln + lane) : 0;   // lengths of the group's first 32 ranks: where prefixes end
+        const int w_end = min(slices_of(__reduce_max_sync(0xffffffffu, lane > 0 || cr.y == 0 ? iL : 0)), (ur.y + 1) * kSliceBlk);
+        // ---- the sequence of (slice, member) pairs: producer side
+        int pw = ur.y * kSliceBlk;                                 // slice of the next copy
+        unsigned preach = __ballot_sync(0xffffffffu, iL > pw * kSl);
+        int istage = 0, issued = 0, consumed = 0, st = 0, pst = 0;
+        // launches the next member's copy into stage `istage` (if there is one)
         auto issue_next = [&]() {
-            while (ireach == 0) {
-                if (!more) return;
-                ic0 += 32;
-                if (ic0 >= k) { more = false; return; }
-                load_chunk();
+            while (preach == 0) {
+                if (++pw >= w_end) { pw = w_end; return; }
+                preach = __ballot_sync(0xffffffffu, iL > pw * kSl);
             }
-            const int b = __ffs(ireach) - 1;
-            ireach &= ireach - 1;
-            const int stage = issued & (kHashStages - 1);
-            if ((iedge >> b) & 1u) {   // first / last vectors of the token array: element-wise, inside the array only
-                const int64_t g0 = shfl_i64(ig0, b);
-                const int nv = __shfl_sync(0xffffffffu, inv, b);
-                for (int e = lane; e < 4 * nv; e += 32) {
-                    const int64_t gi = g0 + e;
+            const int b = __ffs(preach) - 1;
+            preach &= preach - 1;
+            const int S0 = pw * kSl;
+            // the member's slot in this slice (computed by every lane for its own member; lane b's counts)
+            const int D = (iD0 + S0) & 3;                         // slot element of position S0
+            const int64_t g0 = ioff + S0 - D;                     // array index of slot element 0
+            const int nv = (min(iL - S0, kSl) + D + 3) >> 2;      // vectors holding positions < min(L, S0 + 508): at most 128
+            const bool edge = !(g0 >= 0 && g0 + 4 * (int64_t)nv <= N);
+            const int stage = istage;
+            if (__shfl_sync(0xffffffffu, (int)edge, b)) {   // first / last vectors of the token array: element-wise, inside the array only
+                const int64_t gb = shfl_i64(g0, b);
+                const int nvb = __shfl_sync(0xffffffffu, nv, b);
+                for (int e = lane; e < 4 * nvb; e += 32) {
+                    const int64_t gi = gb + e;
                     sts32(sbuf + stage * kStageBytes + 4 * e, gi >= 0 && gi < N ? (uint32_t)tokens[gi] : 0u);
                 }
                 __syncwarp();
             }
             if (lane == b) {   // the descriptor is published by the barrier's release / acquire
-                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(sdesc + 16 * stage), "r"(ic0 + b), "r"(iL), "r"(isb), "r"(iD) : "memory");
-                if ((iedge >> b) & 1u) {
+                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(sdesc + 16 * stage), "r"((rlo + b) | (D << 28)), "r"(iL), "r"(isb), "r"(pw) : "memory");
+                if (edge) {
                     mbar_arrive(&full[stage]);
                 } else {
-                    mbar_arrive_expect_tx(&full[stage], 16u * (uint32_t)inv);
-                    bulk_load(wbuf + stage * kStageBytes, tokens + ig0, 16u * (uint32_t)inv, &full[stage]);
+                    mbar_arrive_expect_tx(&full[stage], 16u * (uint32_t)nv);
+                    fence_proxy_async_smem();   // the stage's last user zeroed a few of its elements with ordinary stores
+                    bulk_load(wbuf + 16 + stage * kStageBytes, tokens + g0, 16u * (uint32_t)nv, &full[stage]);
                 }
             }
             ++issued;
+            if (++istage == kHashStages) istage = 0;
         };
-        bool end_hi = false;   // does a member of rank >= 32 end in this slice?  (groups of more than 32 only)
-        for (int a0 = 32; a0 < k && !end_hi; a0 += 32) {
-            const int La = a0 + lane < k ? __ldg(gln + a0 + lane) : 0;
-            end_hi = __any_sync(0xffffffffu, La > 0 && ((La - 1) >> kSlLog) == w);
-        }
+        int cw = -1;            // slice of the member at work
+        int S0 = 0;
+        uint32_t wS0 = 0;
+        unsigned end0 = 0;
+        bool end_hi = false;
         int prev_r = -2, prev_L = 0, prev_D = 0;
-        uint64_t Fk = 0;        // lane a: the partial of the prefix ending at member a's last token, for the latest member
+        uint32_t prev_tot = 0;
+        bool prev_hashed = false;
+        uint32_t Fk = 0;        // lane a: the partial of the prefix ending at member a's last token, for the latest member
         unsigned fvalid = 0;    // ranks whose Fk belongs to the latest member
-        issue_next();
-        issue_next();           // two members ahead: the predecessor's stage stays intact while a member is compared with it
+        issue_next();           // one member ahead: the predecessor's stage stays intact while a member is compared with it
 #pragma unroll 1
         while (consumed < issued) {
             issue_next();
-            const int st = consumed & (kHashStages - 1);
             if (!mbar_wait_bounded(&full[st], (phases >> st) & 1u)) dead = true;   // never in practice: a lost copy must not hang the GPU
             phases ^= 1u << st;
-            int r, Lr, sbr, D;
-            asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r), "=r"(Lr), "=r"(sbr), "=r"(D) : "r"(sdesc + 16 * st));
-            const uint32_t a0 = sbuf + st * kStageBytes + 4 * (D + lane);
-            uint32_t x[16];
-#pragma unroll
-            for (int t = 0; t < 16; ++t) x[t] = lds32(a0 + 128 * t);
-            if (Lr < S0 + kSl) {   // the member ends in this slice: nothing beyond its last token
-                const int rem = Lr - S0 - lane;
-#pragma unroll
-                for (int t = 0; t < 16; ++t)
-                    if (32 * t >= rem) x[t] = 0;
-            }
-            uint64_t ac0 = (uint64_t)x[0] * wt[0], ac1 = (uint64_t)x[1] * wt[1];
-#pragma unroll
-            for (int t = 2; t < 16; t += 2) {
-                ac0 = mad_wide(x[t], wt[t], ac0);
-                ac1 = mad_wide(x[t + 1], wt[t + 1], ac1);
-            }
-            // exact comparison with the in-group predecessor on its positions (M5, first half)
-            bool same = false;   // the two agree on every position of the slice below prev_L
-            if (prev_r == r - 1) {
-                uint32_t diff = 0;
-                const uint32_t pa0 = sbuf + ((consumed - 1) & (kHashStages - 1)) * kStageBytes + 4 * (prev_D + lane);
-                if (prev_L >= S0 + kSl) {
-#pragma unroll
-                    for (int t = 0; t < 16; ++t) diff |= x[t] ^ lds32(pa0 + 128 * t);
-                } else {
-                    const int rem = prev_L - S0 - lane;
-#pragma unroll
-                    for (int t = 0; t < 16; ++t)
-                        if (32 * t < rem) diff |= x[t] ^ lds32(pa0 + 128 * t);
+            int rD, Lr, sbr, w;
+            asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(rD), "=r"(Lr), "=r"(sbr), "=r"(w) : "r"(sdesc + 16 * st));
+            const int r = rD & 0x0fffffff, D = rD >> 28;
+            if (w != cw) {   // a new slice: nothing carries over
+                cw = w;
+                S0 = w * kSl;
+                wS0 = w < 128 ? c_wsl.v[w] : pow32(kWSl, (uint32_t)w);   // W^S0
+                end0 = __ballot_sync(0xffffffffu, L0 > 0 && slice_at(L0 - 1) == w);
+                end_hi = false;   // does a member of rank >= 32 end in this slice?  (groups of more than 32 only)
+                for (int a0 = 32; a0 < k && !end_hi; a0 += 32) {
+                    const int La = a0 + lane < k ? __ldg(gln + a0 + lane) : 0;
+                    end_hi = __any_sync(0xffffffffu, La > 0 && slice_at(La - 1) == w);
                 }
-                same = !__any_sync(0xffffffffu, diff != 0);
-                if (!same && lane == 0) p.lbad[gs + r] = 1;
+                prev_r = -2;
+                fvalid = 0;
             }
-            const uint64_t tot = warp_sum_u64_redux(ac0 + ac1);
-            if (lane == 0) p.seg_part[sbr + w] = tot;
-            // keys: the prefixes (L_a of an earlier member, or L_r itself) that end inside this slice
-            if (!same) fvalid = 0;
-            unsigned m0 = end0 & (r >= 31 ? 0xffffffffu : (2u << r) - 1u);
-            if (m0) m0 &= __ballot_sync(0xffffffffu, L0 <= Lr);
-            for (; m0; m0 &= m0 - 1) {
-                const int b = __ffs(m0) - 1;
-                const int Lb = __shfl_sync(0xffffffffu, L0, b);
-                uint64_t F;
-                if (((fvalid >> b) & 1u) && Lb <= prev_L) {
-                    F = (uint64_t)shfl_i64((int64_t)Fk, b);   // member r - 1 has the same tokens up to there
+            const uint32_t slot = sbuf + st * kStageBytes;
+            const int len = min(Lr - S0, kSl);           // positions of the member in this slice
+            const int nq = (len + D + 3) >> 2;
+            // zero what is not the member's: elements [0, D) and [D + len, end of the last vector) -- for a whole slice up to
+            // the end of the slot (with D = 0 the copy is 127 vectors and the 128th holds an earlier member's data)
+            if (lane < D) sts32(slot + 4 * lane, 0u);
+            if (lane < 4 && D + len + lane < (len == kSl ? kSlotBytes / 4 : 4 * nq)) sts32(slot + 4 * (D + len + lane), 0u);
+            __syncwarp();
+            if (r < cr.y) {   // the previous chunk's last member: here to be compared with, nothing else
+                prev_r = r; prev_L = Lr; prev_D = D; prev_hashed = false;
+            } else {
+                const bool have_prev = prev_r == r - 1;
+                const int plen = min(prev_L - S0, kSl);
+                const uint32_t pslot = sbuf + pst * kStageBytes;
+                const int delta = prev_D - D;                 // position p: own element p + D, predecessor's element p + D + delta
+                uint32_t y[16];
+                bool same = false;   // the two agree on every position of the slice below prev_L
+                if (len == kSl && (!have_prev || plen == kSl)) {
+                    // ---- whole slices: no masks anywhere
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) {
+                        const uint4 v = lds128(slot + 16 * (lane + 32 * t));
+                        y[4 * t] = v.x; y[4 * t + 1] = v.y; y[4 * t + 2] = v.z; y[4 * t + 3] = v.w;
+                    }
+                    if (have_prev) {
+                        uint32_t diff = 0;
+                        if (delta == 0) {
+#pragma unroll
+                            for (int t = 0; t < 4; ++t) {
+                                const uint4 z = lds128(pslot + 16 * (lane + 32 * t));
+                                diff |= (y[4 * t] ^ z.x) | (y[4 * t + 1] ^ z.y) | (y[4 * t + 2] ^ z.z) | (y[4 * t + 3] ^ z.w);
+                            }
+                        } else {
+                            const uint32_t pa = pslot + 4 * delta + 16 * lane;
+#pragma unroll
+                            for (int t = 0; t < 4; ++t)
+#pragma unroll
+                                for (int i = 0; i < 4; ++i) diff |= y[4 * t + i] ^ lds32(pa + 512 * t + 4 * i);
+                        }
+                        same = !__any_sync(0xffffffffu, diff != 0);
+                    }
                 } else {
-                    if (b == r) {
-                        F = tot;   // its own last token: everything beyond is zero already
+                    // ---- the member or its predecessor ends in this slice: element by element
+                    const int cmp = have_prev ? min(len, plen) : 0;   // positions to compare
+                    uint32_t diff = 0;
+#pragma unroll
+                    for (int t = 0; t < 4; ++t)
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const int e = 4 * (lane + 32 * t) + i, pos = e - D;
+                            const uint32_t v = pos >= 0 && pos < len ? lds32(slot + 4 * e) : 0u;
+                            y[4 * t + i] = v;
+                            if (pos >= 0 && pos < cmp) diff |= v ^ lds32(pslot + 4 * (e + delta));
+                        }
+                    if (have_prev) same = !__any_sync(0xffffffffu, diff != 0);
+                }
+                if (have_prev && !same && lane == 0) p.lbad[gs + r] = 1;
+                const uint32_t fD = wS0 * c_winv.v[D];   // W^(S0 - D)
+                uint32_t tot;
+                if (have_prev && same && prev_hashed && len == kSl && plen == kSl) tot = prev_tot;   // the same 508 tokens
+                else tot = __reduce_add_sync(0xffffffffu, dot(y)) * fD;
+                if (lane == 0) p.seg_part[sbr + w] = tot;
+                // keys: the prefixes (L_a of an earlier member, or L_r itself) that end inside this slice
+                if (!same) fvalid = 0;
+                unsigned m0 = end0 & (r >= 31 ? 0xffffffffu : (2u << r) - 1u);
+                if (m0) m0 &= __ballot_sync(0xffffffffu, L0 <= Lr);
+                for (; m0; m0 &= m0 - 1) {
+                    const int b = __ffs(m0) - 1;
+                    const int Lb = __shfl_sync(0xffffffffu, L0, b);
+                    uint32_t F;
+                    if (((fvalid >> b) & 1u) && Lb <= prev_L) {
+                        F = __shfl_sync(0xffffffffu, Fk, b);   // member r - 1 has the same tokens up to there
                     } else {
-                        const int rem = Lb - S0 - lane;   // tokens 32 t < rem are inside the prefix
-                        uint64_t part = 0;
+                        if (b == r) {
+                            F = tot;   // its own last token: everything beyond is zero already
+                        } else {
+                            const int rem = Lb - S0 + D - 4 * lane;   // slot elements 128 t + i < rem are inside the prefix
+                            uint32_t z[16];
 #pragma unroll
-                        for (int t = 0; t < 16; ++t)
-                            if (32 * t < rem) part = mad_wide(x[t], wt[t], part);
-                        F = warp_sum_u64_redux(part);
+                            for (int j = 0; j < 16; ++j) z[j] = 128 * (j >> 2) + (j & 3) < rem ? y[j] : 0u;
+                            F = __reduce_add_sync(0xffffffffu, dot(z)) * fD;
+                        }
+                        if (lane == b) Fk = F;
+                        fvalid |= 1u << b;
                     }
-                    if (lane == b) Fk = F;
-                    fvalid |= 1u << b;
+                    if (lane == 0) p.ent_hash[eb + (int64_t)r * (r + 1) / 2 + b] = F;
                 }
-                if (lane == 0) p.ent_hash[eb + (int64_t)r * (r + 1) / 2 + b] = F;
-            }
-            if (end_hi && r >= 32) {   // groups of more than 32: ends of ranks >= 32, no caching
-                for (int a0r = 32; a0r <= r; a0r += 32) {
-                    const int a = a0r + lane;
-                    const int La = a < k ? __ldg(gln + a) : 0;
-                    const bool hit = a <= r && La > 0 && La <= Lr && ((La - 1) >> kSlLog) == w;
-                    for (unsigned m = __ballot_sync(0xffffffffu, hit); m; m &= m - 1) {
-                        const int b = __ffs(m) - 1;
-                        const int rem = __shfl_sync(0xffffffffu, La, b) - S0 - lane;
-                        uint64_t part = 0;
+                if (end_hi && r >= 32) {   // groups of more than 32: ends of ranks >= 32, no caching
+                    for (int a0r = 32; a0r <= r; a0r += 32) {
+                        const int a = a0r + lane;
+                        const int La = a < k ? __ldg(gln + a) : 0;
+                        const bool hit = a <= r && La > 0 && La <= Lr && slice_at(La - 1) == w;
+                        for (unsigned m = __ballot_sync(0xffffffffu, hit); m; m &= m - 1) {
+                            const int b = __ffs(m) - 1;
+                            const int rem = __shfl_sync(0xffffffffu, La, b) - S0 + D - 4 * lane;
+                            uint32_t z[16];
 #pragma unroll
-                        for (int t = 0; t < 16; ++t)
-                            if (32 * t < rem) part = mad_wide(x[t], wt[t], part);
-                        const uint64_t F = warp_sum_u64_redux(part);
-                        if (lane == 0) p.ent_hash[eb + (int64_t)r * (r + 1) / 2 + a0r + b] = F;
+                            for (int j = 0; j < 16; ++j) z[j] = 128 * (j >> 2) + (j & 3) < rem ? y[j] : 0u;
+                            const uint32_t F = __reduce_add_sync(0xffffffffu, dot(z)) * fD;
+                            if (lane == 0) p.ent_hash[eb + (int64_t)r * (r + 1) / 2 + a0r + b] = F;
+                        }
                     }
                 }
+                prev_r = r;
+                prev_L = Lr;
+                prev_D = D;
+                prev_tot = tot;
+                prev_hashed = true;
             }
-            prev_r = r;
-            prev_L = Lr;
-            prev_D = D;
             ++consumed;
+            pst = st;
+            if (++st == kHashStages) st = 0;
             __syncwarp();   // every lane is done with the stage before a later issue refills it
         }
         next = __shfl_sync(0xffffffffu, next, 0);
@@ -1127,6 +1156,7 @@ __device__ __noinline__ int build_segments(bool explicit_masks, const int32_t* m
 constexpr int kCompactChunk = 8192;
 constexpr int kCompactSmem = kCompactChunk * 16 + kCompactChunk * 4;
 __global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p) {
+    pdl_wait();
     extern __shared__ __align__(16) uint8_t c_dyn[];
     __shared__ int64_t s_wa[32], s_wb[32];
     if (fatal(p)) return;
@@ -1239,6 +1269,7 @@ __global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p
 }
 
 __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const MergeParams p) {
+    pdl_wait();
     __shared__ SelectSmem sm;
     extern __shared__ __align__(16) uint8_t sel_dyn[];
     SelectStage& sg = *reinterpret_cast<SelectStage*>(sel_dyn);
@@ -1284,7 +1315,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
             }
             for (int x = tid; x < c; x += NT) sg.eh[x] = p.ent_hash[eb + x];
             __syncthreads();
-            const int sb0 = sg.sb[0], nsl = sg.sb[k - 1] + ((sg.L[k - 1] + kSl - 1) >> kSlLog) - sb0;
+            const int sb0 = sg.sb[0], nsl = sg.sb[k - 1] + slices_of(sg.L[k - 1]) - sb0;
             fast = nsl <= kSelSlices;
             if (fast) {   // round trip 3: the slice totals (contiguous: slices are numbered in group order), response starts
                 for (int x = tid; x < nsl; x += NT) sg.sp[x] = p.seg_part[sb0 + x];
@@ -1311,7 +1342,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
         // ---- M2 (end): per member, exclusive prefix over its slice totals (in place), one warp per member
         for (int r = warp; r < k; r += NT / 32) {
             const int sb = sb_of(r);
-            const int ns = (gln[r] + kSl - 1) >> kSlLog;
+            const int ns = slices_of(gln[r]);
             uint64_t carry = 0;
             for (int s0 = 0; s0 < ns; s0 += 32) {
                 const int s = s0 + lane;
@@ -1343,7 +1374,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
             const int32_t Lp = gln[a];
             uint32_t dg = 0xFFFFFFFFu;
             if (Lp <= gln[r]) {
-                uint64_t h = eh[x] + sp[sb_of(r) + ((Lp - 1) >> kSlLog)];
+                uint64_t h = (eh[x] + sp[sb_of(r) + slice_at(Lp - 1)]) & 0xFFFFFFFFull;   // the hash lives in the ring mod 2^32
                 if (weak) h &= 0xFull;
                 eh[x] = h;
                 dg = digest32(h, Lp);
@@ -1540,6 +1571,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
 // (a) one warp per merged sequence: its relative segments -> global segment records at output positions;
 // (b) one thread per output tile: the segment that holds the tile's first position.
 __global__ void __launch_bounds__(256) merge_plan_kernel(const MergeParams p) {
+    pdl_wait();
     if (fatal(p)) return;
     const int lane = threadIdx.x & 31;
     const int wglobal = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
@@ -1680,6 +1712,7 @@ static_assert(kScatWarpBytes % 128 == 0, "warp regions stay 128-byte aligned");
 // the output's alignment into a staging copy of the four output rows (32-bit shared-memory accesses, conflict-free) and one
 // lane sends them off with four bulk stores.  Requests of kilobytes instead of 128 bytes: what it takes to fill HBM.
 __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const MergeParams p) {
+    pdl_wait();
     extern __shared__ __align__(128) uint8_t sc_dyn[];
     if (fatal(p)) return;
     const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
@@ -1868,6 +1901,22 @@ int merge_dev_facts(int* num_sms) {
     *num_sms = g_dev[dev].num_sms;
     return AJT_OK;
 }
+
+template <class K>
+cudaError_t launch_dependent(K kern, int grid, int block, size_t smem, cudaStream_t stream, const MergeParams& p) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ajt::note_launch();
+    return cudaLaunchKernelEx(&cfg, kern, p);
+}
 }  // namespace
 
 extern "C" size_t ajt_merge_workspace_bytes(int32_t n, int64_t n_tokens) {
@@ -1918,6 +1967,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     p.lbad = b + ws.lbad;
     p.grp_rec = reinterpret_cast<int4*>(b + ws.grp_rec);
     p.unit_rec = reinterpret_cast<int2*>(b + ws.unit_rec);
+    p.chunk_rec = reinterpret_cast<int4*>(b + ws.chunk_rec);
     p.seg_part = reinterpret_cast<uint64_t*>(b + ws.seg_part);
     p.absorbed = b + ws.absorbed;
     p.owner_tl = reinterpret_cast<int32_t*>(b + ws.owner_tl);
@@ -1954,11 +2004,16 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     }
     if (n <= kGrpSmemN) AJT_LAUNCH(merge_group_fast_kernel<<<1, 1024, group_fast_smem(n), stream>>>(p, n + n / 8 + 16));
     else AJT_LAUNCH(merge_group_radix_kernel<<<1, 1024, 0, stream>>>(p));
-    AJT_LAUNCH(merge_hash_kernel<<<num_sms * 2, kHashThreads, kHashSmem, stream>>>(p));
-    AJT_LAUNCH(merge_select_kernel<<<num_sms * 4, kSelThreads, sizeof(SelectStage), stream>>>(p));
-    AJT_LAUNCH(merge_compact_kernel<<<1, 1024, kCompactSmem, stream>>>(p));
+    // kernels 2..6 are launched as programmatic dependents: resident and waiting when their predecessor ends
     const int64_t want = ((n_tokens >> kTSLog) + 1 + 255) / 256 + ((int64_t)n * 32 + 255) / 256;
-    AJT_LAUNCH(merge_plan_kernel<<<(int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8), 256, 0, stream>>>(p));
-    AJT_LAUNCH(merge_scatter_kernel<<<num_sms, kScatThreads, kScatSmem, stream>>>(p));
+    const int plan_grid = (int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8);
+    const int64_t uwant = ((int64_t)n + 255) / 256;
+    if (launch_dependent(merge_units_kernel, (int)(uwant < (int64_t)num_sms * 4 ? uwant : (int64_t)num_sms * 4), 256, 0, stream, p) != cudaSuccess ||
+        launch_dependent(merge_hash_kernel, num_sms * 3, kHashThreads, kHashSmem, stream, p) != cudaSuccess ||
+        launch_dependent(merge_select_kernel, num_sms * 4, kSelThreads, sizeof(SelectStage), stream, p) != cudaSuccess ||
+        launch_dependent(merge_compact_kernel, 1, 1024, kCompactSmem, stream, p) != cudaSuccess ||
+        launch_dependent(merge_plan_kernel, plan_grid, 256, 0, stream, p) != cudaSuccess ||
+        launch_dependent(merge_scatter_kernel, num_sms, kScatThreads, kScatSmem, stream, p) != cudaSuccess)
+        return AJT_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }
