@@ -356,7 +356,8 @@ __device__ __forceinline__ void group_fail(const MergeParams& p, uint32_t bits) 
 }
 
 constexpr int kChunk = 8;      // hash units: a group's members are cut into chunks of this many consecutive ranks ...
-constexpr int kSliceBlk = 1;   // ... and a chunk's slices into blocks of this many: one warp's critical path is ~9 member-slices
+constexpr int kSliceBlk = 1;   // ... and every slice of a chunk is a unit of its own: one warp's critical path is ~9 member-slices
+static_assert(kSliceBlk == 1, "the hash kernel takes one slice per unit");
 
 // ---------------------------------------------------------------------------------------- K1: group (M1)
 
@@ -822,67 +823,60 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
     while (next < U) {
         const int u = next;
         if (lane == 0) next = atomicAdd(&p.ctrl->unit_ticket, 1);   // needed only after this unit: the round trip is hidden
-        const int2 ur = __ldg(p.unit_rec + u);                      // {chunk, slice block}: largest units first
+        const int2 ur = __ldg(p.unit_rec + u);                      // {chunk, slice}
         const int4 cr = __ldg(p.chunk_rec + ur.x);                  // {group start, first rank, members of the group, first key slot}
-        const int gs = cr.x, k = cr.z;
-        const int64_t eb = cr.w;
+        const int gs = cr.x, k = cr.z, w = ur.y;
         const int rlo = cr.y - (cr.y > 0 ? 1 : 0);                  // lane i holds rank rlo + i: the predecessor of the chunk first
         const int rhi = min(k, cr.y + kChunk);
         const int32_t* __restrict__ gln = p.glen + gs;
-        // ---- each lane's member: facts that do not depend on the slice
+        const int S0 = w * kSl;                                     // first position of the slice
+        // ---- each lane's member and its slot in this slice
         const bool mine = rlo + lane < rhi;
-        const int iL = mine ? __ldg(gln + rlo + lane) : 0;
-        const int64_t ioff = mine ? __ldg(p.goff + gs + rlo + lane) : 0;
-        const int isb = mine ? __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + rlo + lane)) : 0;
-        const int iD0 = (int)((ioff + mis) & 3);
+        const int myr = rlo + lane;
+        const int iL = mine ? __ldg(gln + myr) : 0;
+        const int64_t ioff = mine ? __ldg(p.goff + gs + myr) : 0;
+        const int isb = mine ? __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + myr)) : 0;
         const int L0 = lane < k ? __ldg(gln + lane) : 0;   // lengths of the group's first 32 ranks: where prefixes end
-        const int w_end = min(slices_of(__reduce_max_sync(0xffffffffu, lane > 0 || cr.y == 0 ? iL : 0)), (ur.y + 1) * kSliceBlk);
-        // ---- the sequence of (slice, member) pairs: producer side
-        int pw = ur.y * kSliceBlk;                                 // slice of the next copy
-        unsigned preach = __ballot_sync(0xffffffffu, iL > pw * kSl);
-        int istage = 0, issued = 0, consumed = 0, st = 0, pst = 0;
+        const int iD = (int)((ioff + mis + S0) & 3);               // slot element of position S0
+        const int64_t ig0 = ioff + S0 - iD;                        // array index of slot element 0
+        const int inv = (min(iL - S0, kSl) + iD + 3) >> 2;         // vectors holding positions < min(L, S0 + 508): at most 128
+        const bool iedge = !(ig0 >= 0 && ig0 + 4 * (int64_t)inv <= N);
+        uint64_t* const my_tot = p.seg_part + isb + w;             // where this member's slice total goes
+        uint64_t* const my_keys = p.ent_hash + (int64_t)cr.w + (int64_t)myr * (myr + 1) / 2;   // its key slots (myr, a), a <= myr
+        unsigned preach = __ballot_sync(0xffffffffu, iL > S0);     // members still to be fetched / still to be worked on
+        unsigned creach = preach;
+        const unsigned edges = __ballot_sync(0xffffffffu, iedge) & preach;
+        const uint32_t wS0 = w < 128 ? c_wsl.v[w] : pow32(kWSl, (uint32_t)w);   // W^S0
+        const uint32_t fD_mine = wS0 * c_winv.v[iD];               // W^(S0 - D)
+        const unsigned end0 = __ballot_sync(0xffffffffu, L0 > 0 && slice_at(L0 - 1) == w);
+        bool end_hi = false;   // does a member of rank >= 32 end in this slice?  (groups of more than 32 only)
+        for (int a0 = 32; a0 < k && !end_hi; a0 += 32) {
+            const int La = a0 + lane < k ? __ldg(gln + a0 + lane) : 0;
+            end_hi = __any_sync(0xffffffffu, La > 0 && slice_at(La - 1) == w);
+        }
+        int istage = 0, st = 0, pst = 0;
         // launches the next member's copy into stage `istage` (if there is one)
         auto issue_next = [&]() {
-            while (preach == 0) {
-                if (++pw >= w_end) { pw = w_end; return; }
-                preach = __ballot_sync(0xffffffffu, iL > pw * kSl);
-            }
+            if (preach == 0) return;
             const int b = __ffs(preach) - 1;
             preach &= preach - 1;
-            const int S0 = pw * kSl;
-            // the member's slot in this slice (computed by every lane for its own member; lane b's counts)
-            const int D = (iD0 + S0) & 3;                         // slot element of position S0
-            const int64_t g0 = ioff + S0 - D;                     // array index of slot element 0
-            const int nv = (min(iL - S0, kSl) + D + 3) >> 2;      // vectors holding positions < min(L, S0 + 508): at most 128
-            const bool edge = !(g0 >= 0 && g0 + 4 * (int64_t)nv <= N);
             const int stage = istage;
-            if (__shfl_sync(0xffffffffu, (int)edge, b)) {   // first / last vectors of the token array: element-wise, inside the array only
-                const int64_t gb = shfl_i64(g0, b);
-                const int nvb = __shfl_sync(0xffffffffu, nv, b);
+            if ((edges >> b) & 1u) {   // first / last vectors of the token array: element-wise, inside the array only
+                const int64_t gb = shfl_i64(ig0, b);
+                const int nvb = __shfl_sync(0xffffffffu, inv, b);
                 for (int e = lane; e < 4 * nvb; e += 32) {
                     const int64_t gi = gb + e;
                     sts32(sbuf + stage * kStageBytes + 4 * e, gi >= 0 && gi < N ? (uint32_t)tokens[gi] : 0u);
                 }
                 __syncwarp();
+                if (lane == b) mbar_arrive(&full[stage]);
+            } else if (lane == b) {
+                mbar_arrive_expect_tx(&full[stage], 16u * (uint32_t)inv);
+                fence_proxy_async_smem();   // the stage's last user zeroed a few of its elements with ordinary stores
+                bulk_load(wbuf + 16 + stage * kStageBytes, tokens + ig0, 16u * (uint32_t)inv, &full[stage]);
             }
-            if (lane == b) {   // the descriptor is published by the barrier's release / acquire
-                asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(sdesc + 16 * stage), "r"((rlo + b) | (D << 28)), "r"(iL), "r"(isb), "r"(pw) : "memory");
-                if (edge) {
-                    mbar_arrive(&full[stage]);
-                } else {
-                    mbar_arrive_expect_tx(&full[stage], 16u * (uint32_t)nv);
-                    fence_proxy_async_smem();   // the stage's last user zeroed a few of its elements with ordinary stores
-                    bulk_load(wbuf + 16 + stage * kStageBytes, tokens + g0, 16u * (uint32_t)nv, &full[stage]);
-                }
-            }
-            ++issued;
             if (++istage == kHashStages) istage = 0;
         };
-        int cw = -1;            // slice of the member at work
-        int S0 = 0;
-        uint32_t wS0 = 0;
-        unsigned end0 = 0;
-        bool end_hi = false;
         int prev_r = -2, prev_L = 0, prev_D = 0;
         uint32_t prev_tot = 0;
         bool prev_hashed = false;
@@ -890,36 +884,23 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
         unsigned fvalid = 0;    // ranks whose Fk belongs to the latest member
         issue_next();           // one member ahead: the predecessor's stage stays intact while a member is compared with it
 #pragma unroll 1
-        while (consumed < issued) {
+        while (creach) {
             issue_next();
+            const int b = __ffs(creach) - 1;   // the member at work sits in lane b
+            creach &= creach - 1;
+            const int r = rlo + b;
+            const int Lr = __shfl_sync(0xffffffffu, iL, b), D = __shfl_sync(0xffffffffu, iD, b);
             if (!mbar_wait_bounded(&full[st], (phases >> st) & 1u)) dead = true;   // never in practice: a lost copy must not hang the GPU
             phases ^= 1u << st;
-            int rD, Lr, sbr, w;
-            asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(rD), "=r"(Lr), "=r"(sbr), "=r"(w) : "r"(sdesc + 16 * st));
-            const int r = rD & 0x0fffffff, D = rD >> 28;
-            if (w != cw) {   // a new slice: nothing carries over
-                cw = w;
-                S0 = w * kSl;
-                wS0 = w < 128 ? c_wsl.v[w] : pow32(kWSl, (uint32_t)w);   // W^S0
-                end0 = __ballot_sync(0xffffffffu, L0 > 0 && slice_at(L0 - 1) == w);
-                end_hi = false;   // does a member of rank >= 32 end in this slice?  (groups of more than 32 only)
-                for (int a0 = 32; a0 < k && !end_hi; a0 += 32) {
-                    const int La = a0 + lane < k ? __ldg(gln + a0 + lane) : 0;
-                    end_hi = __any_sync(0xffffffffu, La > 0 && slice_at(La - 1) == w);
-                }
-                prev_r = -2;
-                fvalid = 0;
-            }
             const uint32_t slot = sbuf + st * kStageBytes;
             const int len = min(Lr - S0, kSl);           // positions of the member in this slice
-            const int nq = (len + D + 3) >> 2;
             // zero what is not the member's: elements [0, D) and [D + len, end of the last vector) -- for a whole slice up to
             // the end of the slot (with D = 0 the copy is 127 vectors and the 128th holds an earlier member's data)
             if (lane < D) sts32(slot + 4 * lane, 0u);
-            if (lane < 4 && D + len + lane < (len == kSl ? kSlotBytes / 4 : 4 * nq)) sts32(slot + 4 * (D + len + lane), 0u);
+            if (lane < 4 && D + len + lane < (len == kSl ? kSlotBytes / 4 : (len + D + 3) & ~3)) sts32(slot + 4 * (D + len + lane), 0u);
             __syncwarp();
             if (r < cr.y) {   // the previous chunk's last member: here to be compared with, nothing else
-                prev_r = r; prev_L = Lr; prev_D = D; prev_hashed = false;
+                prev_hashed = false;
             } else {
                 const bool have_prev = prev_r == r - 1;
                 const int plen = min(prev_L - S0, kSl);
@@ -966,36 +947,38 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
                         }
                     if (have_prev) same = !__any_sync(0xffffffffu, diff != 0);
                 }
-                if (have_prev && !same && lane == 0) p.lbad[gs + r] = 1;
-                const uint32_t fD = wS0 * c_winv.v[D];   // W^(S0 - D)
+                if (have_prev && !same && lane == b) p.lbad[gs + r] = 1;
+                const uint32_t fD = __shfl_sync(0xffffffffu, fD_mine, b);
                 uint32_t tot;
                 if (have_prev && same && prev_hashed && len == kSl && plen == kSl) tot = prev_tot;   // the same 508 tokens
                 else tot = __reduce_add_sync(0xffffffffu, dot(y)) * fD;
-                if (lane == 0) p.seg_part[sbr + w] = tot;
+                if (lane == b) *my_tot = tot;
                 // keys: the prefixes (L_a of an earlier member, or L_r itself) that end inside this slice
                 if (!same) fvalid = 0;
-                unsigned m0 = end0 & (r >= 31 ? 0xffffffffu : (2u << r) - 1u);
-                if (m0) m0 &= __ballot_sync(0xffffffffu, L0 <= Lr);
-                for (; m0; m0 &= m0 - 1) {
-                    const int b = __ffs(m0) - 1;
-                    const int Lb = __shfl_sync(0xffffffffu, L0, b);
-                    uint32_t F;
-                    if (((fvalid >> b) & 1u) && Lb <= prev_L) {
-                        F = __shfl_sync(0xffffffffu, Fk, b);   // member r - 1 has the same tokens up to there
-                    } else {
-                        if (b == r) {
-                            F = tot;   // its own last token: everything beyond is zero already
+                if (end0) {
+                    unsigned m0 = end0 & (r >= 31 ? 0xffffffffu : (2u << r) - 1u);
+                    if (m0) m0 &= __ballot_sync(0xffffffffu, L0 <= Lr);
+                    for (; m0; m0 &= m0 - 1) {
+                        const int a = __ffs(m0) - 1;
+                        const int La = __shfl_sync(0xffffffffu, L0, a);
+                        uint32_t F;
+                        if (((fvalid >> a) & 1u) && La <= prev_L) {
+                            F = __shfl_sync(0xffffffffu, Fk, a);   // member r - 1 has the same tokens up to there
                         } else {
-                            const int rem = Lb - S0 + D - 4 * lane;   // slot elements 128 t + i < rem are inside the prefix
-                            uint32_t z[16];
+                            if (a == r) {
+                                F = tot;   // its own last token: everything beyond is zero already
+                            } else {
+                                const int rem = La - S0 + D - 4 * lane;   // slot elements 128 t + i < rem are inside the prefix
+                                uint32_t z[16];
 #pragma unroll
-                            for (int j = 0; j < 16; ++j) z[j] = 128 * (j >> 2) + (j & 3) < rem ? y[j] : 0u;
-                            F = __reduce_add_sync(0xffffffffu, dot(z)) * fD;
+                                for (int j = 0; j < 16; ++j) z[j] = 128 * (j >> 2) + (j & 3) < rem ? y[j] : 0u;
+                                F = __reduce_add_sync(0xffffffffu, dot(z)) * fD;
+                            }
+                            if (lane == a) Fk = F;
+                            fvalid |= 1u << a;
                         }
-                        if (lane == b) Fk = F;
-                        fvalid |= 1u << b;
+                        if (lane == b) my_keys[a] = F;
                     }
-                    if (lane == 0) p.ent_hash[eb + (int64_t)r * (r + 1) / 2 + b] = F;
                 }
                 if (end_hi && r >= 32) {   // groups of more than 32: ends of ranks >= 32, no caching
                     for (int a0r = 32; a0r <= r; a0r += 32) {
@@ -1003,23 +986,22 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
                         const int La = a < k ? __ldg(gln + a) : 0;
                         const bool hit = a <= r && La > 0 && La <= Lr && slice_at(La - 1) == w;
                         for (unsigned m = __ballot_sync(0xffffffffu, hit); m; m &= m - 1) {
-                            const int b = __ffs(m) - 1;
-                            const int rem = __shfl_sync(0xffffffffu, La, b) - S0 + D - 4 * lane;
+                            const int a1 = __ffs(m) - 1;
+                            const int rem = __shfl_sync(0xffffffffu, La, a1) - S0 + D - 4 * lane;
                             uint32_t z[16];
 #pragma unroll
                             for (int j = 0; j < 16; ++j) z[j] = 128 * (j >> 2) + (j & 3) < rem ? y[j] : 0u;
                             const uint32_t F = __reduce_add_sync(0xffffffffu, dot(z)) * fD;
-                            if (lane == 0) p.ent_hash[eb + (int64_t)r * (r + 1) / 2 + a0r + b] = F;
+                            if (lane == b) my_keys[a0r + a1] = F;
                         }
                     }
                 }
-                prev_r = r;
-                prev_L = Lr;
-                prev_D = D;
                 prev_tot = tot;
                 prev_hashed = true;
             }
-            ++consumed;
+            prev_r = r;
+            prev_L = Lr;
+            prev_D = D;
             pst = st;
             if (++st == kHashStages) st = 0;
             __syncwarp();   // every lane is done with the stage before a later issue refills it
