@@ -1681,9 +1681,10 @@ __device__ __noinline__ void scatter_tile_walk(const ScatPtrs p, int t, int64_t 
     }
 }
 
-constexpr int kScatThreads = 256;
+constexpr int kScatThreads = 384;                                   // 12 warps: what the shared memory of one SM holds
 constexpr int kScatInBytes = 2560;                                   // one input array of a tile: 2 KB + 16-byte slack of up to 8 pieces
-constexpr int kScatOutBytes = 3 * kTS * 4 + kTS;                     // tokens, src, old_logp, mask of one tile
+constexpr int kScatOutBytes = 2 * kTS * 4;                           // realigned tokens and old_logp of one tile (src and mask are constants
+                                                                     // per piece: they go out straight from registers)
 constexpr int kScatWarpBytes = 2 * 2 * kScatInBytes + 2 * kScatOutBytes + 2 * 8 * 32 + 128;   // 2 stages in, 2 out, piece tables, barriers
 constexpr int kScatSmem = (kScatThreads / 32) * kScatWarpBytes + 128;
 static_assert(kScatWarpBytes % 128 == 0, "warp regions stay 128-byte aligned");
@@ -1705,7 +1706,7 @@ __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const Me
     const int mis_t = p.mis, mis_l = (int)(((uintptr_t)p.old_logp_in >> 2) & 3);
     uint8_t* const wb = reinterpret_cast<uint8_t*>(((uintptr_t)sc_dyn + 127) & ~(uintptr_t)127) + (size_t)wic * kScatWarpBytes;
     uint8_t* const in_base = wb;                                            // [stage][tok | lp]
-    uint8_t* const out_base = wb + 4 * kScatInBytes;                        // [stage][tok | src | lp | mask]
+    uint8_t* const out_base = wb + 4 * kScatInBytes;                        // [stage][tok | lp]
     int4* const tbl = reinterpret_cast<int4*>(wb + 4 * kScatInBytes + 2 * kScatOutBytes);   // [stage][8 pieces][2]
     uint64_t* const full = reinterpret_cast<uint64_t*>(wb + 4 * kScatInBytes + 2 * kScatOutBytes + 2 * 8 * 32);
     const ScatPtrs sp = {p.tokens, p.old_logp_in, p.offsets, p.mask_in, p.mem_list, p.gseg, p.tile_seg,
@@ -1787,7 +1788,7 @@ __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const Me
             const int64_t dt = (int64_t)t << kTSLog;
             const uint32_t in_tok = smem_u32(in_base + st * 2 * kScatInBytes), in_lp = in_tok + kScatInBytes;
             uint8_t* const ob = out_base + st * kScatOutBytes;
-            const uint32_t out_tok = smem_u32(ob), out_src = out_tok + 4 * kTS, out_lp = out_tok + 8 * kTS, out_mask = out_tok + 12 * kTS;
+            const uint32_t out_tok = smem_u32(ob), out_lp = out_tok + 4 * kTS;
             if (lane == 0) bulk_wait_read<1>();   // the stores of two tiles ago have read this staging copy
             __syncwarp();
             if (!mbar_wait_bounded(&full[st], (phases >> st) & 1u)) dead = true;
@@ -1809,11 +1810,10 @@ __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const Me
                     }
                 }
                 const uint32_t sv = (uint32_t)e1.x, mk = e1.x >= 0 ? 0x01010101u : 0u;
+                uint4* const gs4 = reinterpret_cast<uint4*>(p.merged_src + dt) + lane;   // 512 contiguous bytes per instruction
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(out_src + 16 * lane + 512 * j), "r"(sv) : "memory");
-                    sts32(out_mask + 4 * lane + 128 * j, mk);
-                }
+                for (int j = 0; j < 4; ++j) gs4[32 * j] = make_uint4(sv, sv, sv, sv);
+                reinterpret_cast<uint4*>(p.merged_mask + dt)[lane] = make_uint4(mk, mk, mk, mk);
             } else {
 #pragma unroll 1
                 for (int pi = 0; pi < np_cur; ++pi) {
@@ -1821,9 +1821,9 @@ __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const Me
                     const uint32_t sv = (uint32_t)e1.x;
                     for (int q = e0.x + lane; q < e0.y; q += 32) {
                         sts32(out_tok + 4 * q, lds32(in_tok + 4 * (e0.z + q - e0.x)));
-                        sts32(out_src + 4 * q, sv);
                         if (want_lp) sts32(out_lp + 4 * q, e0.w >= 0 ? lds32(in_lp + 4 * (e0.w + q - e0.x)) : 0u);
-                        asm volatile("st.shared.u8 [%0], %1;" ::"r"(out_mask + q), "r"(e1.x >= 0 ? 1u : 0u) : "memory");
+                        p.merged_src[dt + q] = (int32_t)sv;
+                        p.merged_mask[dt + q] = e1.x >= 0 ? (uint8_t)1 : (uint8_t)0;
                     }
                 }
             }
@@ -1831,9 +1831,7 @@ __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const Me
             __syncwarp();
             if (lane == 0) {
                 bulk_store(p.merged_tokens + dt, ob, 4 * kTS);
-                bulk_store(p.merged_src + dt, ob + 4 * kTS, 4 * kTS);
-                if (want_lp) bulk_store(p.merged_old_logp + dt, ob + 8 * kTS, 4 * kTS);
-                bulk_store(p.merged_mask + dt, ob + 12 * kTS, kTS);
+                if (want_lp) bulk_store(p.merged_old_logp + dt, ob + 4 * kTS, 4 * kTS);
             }
         }
         if (lane == 0) bulk_commit();   // one group per tile, empty for a walked one: "two tiles ago" is then always group - 2
