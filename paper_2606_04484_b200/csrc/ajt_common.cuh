@@ -33,7 +33,8 @@ struct AjtCtrl {
     int32_t unit_ticket;  // hash pass: dynamic unit ticket
     int32_t n_chunks;     // chunks of consecutive ranks of grouped groups
     int32_t n_gsegs;      // scatter segments (constant-source runs of the merged output)
-    uint32_t reserved[44];
+    int32_t scat_ticket;  // scatter pass: dynamic tile ticket
+    uint32_t reserved[43];
 };
 static_assert(sizeof(AjtCtrl) == 256, "AjtCtrl must be 256 bytes");
 

@@ -1681,11 +1681,9 @@ __device__ __noinline__ void scatter_tile_walk(const ScatPtrs p, int t, int64_t 
     }
 }
 
-constexpr int kScatThreads = 384;                                   // 12 warps: what the shared memory of one SM holds
+constexpr int kScatThreads = 640;                                   // 20 warps: what the shared memory of one SM holds
 constexpr int kScatInBytes = 2560;                                   // one input array of a tile: 2 KB + 16-byte slack of up to 8 pieces
-constexpr int kScatOutBytes = 2 * kTS * 4;                           // realigned tokens and old_logp of one tile (src and mask are constants
-                                                                     // per piece: they go out straight from registers)
-constexpr int kScatWarpBytes = 2 * 2 * kScatInBytes + 2 * kScatOutBytes + 2 * 8 * 32 + 128;   // 2 stages in, 2 out, piece tables, barriers
+constexpr int kScatWarpBytes = 2 * 2 * kScatInBytes + 2 * 8 * 32 + 128;   // 2 input stages (tokens, old_logp), piece tables, barriers
 constexpr int kScatSmem = (kScatThreads / 32) * kScatWarpBytes + 128;
 static_assert(kScatWarpBytes % 128 == 0, "warp regions stay 128-byte aligned");
 
@@ -1706,9 +1704,8 @@ __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const Me
     const int mis_t = p.mis, mis_l = (int)(((uintptr_t)p.old_logp_in >> 2) & 3);
     uint8_t* const wb = reinterpret_cast<uint8_t*>(((uintptr_t)sc_dyn + 127) & ~(uintptr_t)127) + (size_t)wic * kScatWarpBytes;
     uint8_t* const in_base = wb;                                            // [stage][tok | lp]
-    uint8_t* const out_base = wb + 4 * kScatInBytes;                        // [stage][tok | lp]
-    int4* const tbl = reinterpret_cast<int4*>(wb + 4 * kScatInBytes + 2 * kScatOutBytes);   // [stage][8 pieces][2]
-    uint64_t* const full = reinterpret_cast<uint64_t*>(wb + 4 * kScatInBytes + 2 * kScatOutBytes + 2 * 8 * 32);
+    int4* const tbl = reinterpret_cast<int4*>(wb + 4 * kScatInBytes);   // [stage][8 pieces][2]
+    uint64_t* const full = reinterpret_cast<uint64_t*>(wb + 4 * kScatInBytes + 2 * 8 * 32);
     const ScatPtrs sp = {p.tokens, p.old_logp_in, p.offsets, p.mask_in, p.mem_list, p.gseg, p.tile_seg,
                          p.merged_tokens, p.merged_mask, p.merged_src, p.merged_old_logp};
     if (lane == 0) {
@@ -1769,48 +1766,55 @@ __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const Me
     };
     const bool out_ok = ((((uintptr_t)p.merged_tokens | (uintptr_t)p.merged_src | (uintptr_t)p.merged_old_logp | (uintptr_t)p.merged_mask) & 15) == 0);
     if (wglobal >= ntiles) return;
-    GSeg rec = load_rec(wglobal);
-    int np_cur = out_ok ? plan(wglobal, 0, rec) : -1;
-    if (wglobal + nwarps < ntiles) rec = load_rec(wglobal + nwarps);
+    // Tiles: the first three of a warp are fixed (wglobal, + nwarps, + 2 nwarps), the rest come from a ticket, three tiles
+    // ahead of the one at work -- tiles cut into several pieces take longer than plain ones, and a fixed stride leaves the
+    // last warp 30 % behind the median.  tA: at work; tB: its copies are in flight; tC: its segment record is being loaded.
+    int tA = wglobal, tB = wglobal + nwarps, tC = wglobal + 2 * nwarps, pend = 0;
+    if (lane == 0) pend = atomicAdd(&p.ctrl->scat_ticket, 1) + 3 * nwarps;
+    GSeg rec = load_rec(tA);
+    int np_cur = out_ok ? plan(tA, 0, rec) : -1;
+    if (tB < ntiles) rec = load_rec(tB);
     int it = 0;
     bool dead = false;
 #pragma unroll 1
-    for (int t = wglobal; t < ntiles; t += nwarps, ++it) {
+    for (; tA < ntiles; ++it) {
+        const int t = tA;
         const int st = it & 1;
         int np_next = -1;
-        if (t + nwarps < ntiles) {   // next tile: its copies fly while this one is rewritten; the tile after: its record
-            if (out_ok) np_next = plan(t + nwarps, st ^ 1, rec);
-            if (t + 2 * nwarps < ntiles) rec = load_rec(t + 2 * nwarps);
+        if (tB < ntiles) {   // next tile: its copies fly while this one is rewritten; the tile after: its record
+            if (out_ok) np_next = plan(tB, st ^ 1, rec);
+            if (tC < ntiles) rec = load_rec(tC);
         }
         if (np_cur < 0) {
             scatter_tile_walk(sp, t, N_out);
         } else {
             const int64_t dt = (int64_t)t << kTSLog;
             const uint32_t in_tok = smem_u32(in_base + st * 2 * kScatInBytes), in_lp = in_tok + kScatInBytes;
-            uint8_t* const ob = out_base + st * kScatOutBytes;
-            const uint32_t out_tok = smem_u32(ob), out_lp = out_tok + 4 * kTS;
-            if (lane == 0) bulk_wait_read<1>();   // the stores of two tiles ago have read this staging copy
-            __syncwarp();
             if (!mbar_wait_bounded(&full[st], (phases >> st) & 1u)) dead = true;
             phases ^= 1u << st;
             if (np_cur == 1) {
+                // one source: lane l writes positions 4 l + 128 j .. + 3 (16-byte stores, 512 contiguous bytes per instruction),
+                // read from the input stage at the source's own misalignment
                 const int4 e0 = tbl[(st * 8) * 2], e1 = tbl[(st * 8) * 2 + 1];
-                const uint32_t a0 = in_tok + 4 * (e0.z + lane), o0 = out_tok + 4 * lane;
+                const uint32_t a0 = in_tok + 4 * (e0.z + 4 * lane);
+                uint4* const gt4 = reinterpret_cast<uint4*>(p.merged_tokens + dt) + lane;
 #pragma unroll
-                for (int j = 0; j < 16; ++j) sts32(o0 + 128 * j, lds32(a0 + 128 * j));
+                for (int j = 0; j < 4; ++j)
+                    gt4[32 * j] = make_uint4(lds32(a0 + 512 * j), lds32(a0 + 512 * j + 4), lds32(a0 + 512 * j + 8), lds32(a0 + 512 * j + 12));
                 if (want_lp) {
+                    uint4* const gl4 = reinterpret_cast<uint4*>(p.merged_old_logp + dt) + lane;
                     if (e0.w >= 0) {
-                        const uint32_t b0 = in_lp + 4 * (e0.w + lane), q0 = out_lp + 4 * lane;
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) sts32(q0 + 128 * j, lds32(b0 + 128 * j));
-                    } else {
+                        const uint32_t b0 = in_lp + 4 * (e0.w + 4 * lane);
 #pragma unroll
                         for (int j = 0; j < 4; ++j)
-                            asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(out_lp + 16 * lane + 512 * j), "r"(0u) : "memory");
+                            gl4[32 * j] = make_uint4(lds32(b0 + 512 * j), lds32(b0 + 512 * j + 4), lds32(b0 + 512 * j + 8), lds32(b0 + 512 * j + 12));
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) gl4[32 * j] = make_uint4(0u, 0u, 0u, 0u);
                     }
                 }
                 const uint32_t sv = (uint32_t)e1.x, mk = e1.x >= 0 ? 0x01010101u : 0u;
-                uint4* const gs4 = reinterpret_cast<uint4*>(p.merged_src + dt) + lane;   // 512 contiguous bytes per instruction
+                uint4* const gs4 = reinterpret_cast<uint4*>(p.merged_src + dt) + lane;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) gs4[32 * j] = make_uint4(sv, sv, sv, sv);
                 reinterpret_cast<uint4*>(p.merged_mask + dt)[lane] = make_uint4(mk, mk, mk, mk);
@@ -1818,27 +1822,22 @@ __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const Me
 #pragma unroll 1
                 for (int pi = 0; pi < np_cur; ++pi) {
                     const int4 e0 = tbl[(st * 8 + pi) * 2], e1 = tbl[(st * 8 + pi) * 2 + 1];
-                    const uint32_t sv = (uint32_t)e1.x;
                     for (int q = e0.x + lane; q < e0.y; q += 32) {
-                        sts32(out_tok + 4 * q, lds32(in_tok + 4 * (e0.z + q - e0.x)));
-                        if (want_lp) sts32(out_lp + 4 * q, e0.w >= 0 ? lds32(in_lp + 4 * (e0.w + q - e0.x)) : 0u);
-                        p.merged_src[dt + q] = (int32_t)sv;
+                        p.merged_tokens[dt + q] = (int32_t)lds32(in_tok + 4 * (e0.z + q - e0.x));
+                        if (want_lp) p.merged_old_logp[dt + q] = e0.w >= 0 ? __uint_as_float(lds32(in_lp + 4 * (e0.w + q - e0.x))) : 0.f;
+                        p.merged_src[dt + q] = e1.x;
                         p.merged_mask[dt + q] = e1.x >= 0 ? (uint8_t)1 : (uint8_t)0;
                     }
                 }
             }
-            fence_proxy_async_smem();   // the staging copy was written through the generic proxy, the bulk stores read it through the async one
-            __syncwarp();
-            if (lane == 0) {
-                bulk_store(p.merged_tokens + dt, ob, 4 * kTS);
-                if (want_lp) bulk_store(p.merged_old_logp + dt, ob + 4 * kTS, 4 * kTS);
-            }
         }
-        if (lane == 0) bulk_commit();   // one group per tile, empty for a walked one: "two tiles ago" is then always group - 2
         np_cur = np_next;
+        tA = tB;
+        tB = tC;
+        tC = __shfl_sync(0xffffffffu, pend, 0);
+        if (lane == 0) pend = atomicAdd(&p.ctrl->scat_ticket, 1) + 3 * nwarps;
         if (__any_sync(0xffffffffu, dead)) break;
     }
-    if (lane == 0) bulk_wait<0>();
     if (dead && lane == 0) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_INTERNAL);
 }
 }  // namespace
