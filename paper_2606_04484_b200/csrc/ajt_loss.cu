@@ -73,6 +73,7 @@ struct LossParams {
     float* k3_out;          // [T] or NULL
     float* ent_out;         // [T] or NULL
     int32_t ext;            // 1: extended kernels (KL term and / or entropy requested)
+    int32_t zero_rows;      // 1: the prep kernel zeroes logp_out / k3_out / ent_out of every row
     // workspace
     AjtCtrl* ctrl;
     uint64_t* tile_state;  // [ntiles] prep scan: bit 63 valid, bits 32..62 active rows of the tile, bits 0..31 masked rows
@@ -134,6 +135,11 @@ __global__ void __launch_bounds__(1024) loss_prep_kernel(const LossParams p, int
         if (tile >= ntiles) break;
         const int64_t t = (int64_t)tile * kPrepTile + tid;
         const bool in = t < p.T;
+        if (in && p.zero_rows) {   // per-row outputs: masked rows read 0; the rows kernel then writes the unmasked ones
+            if (p.logp_out) p.logp_out[t] = 0.f;
+            if (p.k3_out) p.k3_out[t] = 0.f;
+            if (p.ent_out) p.ent_out[t] = 0.f;
+        }
         bool act = in && p.mask[t] != 0;
         int sg = act ? p.seg_ids[t] : 0;
         if (act && (unsigned)sg >= (unsigned)p.S) {
@@ -264,6 +270,7 @@ __device__ __forceinline__ void rebase(float m, float M, float& s, float& u) {
 template <int NCH, int CSIZE, bool EXT>
 __global__ void __launch_bounds__(kThreads, 1) loss_rows_kernel(const LossParams p) {
     extern __shared__ __align__(1024) uint8_t smem[];
+    pdl_wait();
     uint8_t* ring = smem;
     uint8_t* zbuf = smem + (size_t)kSlots * kChunkBytes;
     uint64_t* full = reinterpret_cast<uint64_t*>(zbuf + kChunkBytes);
@@ -546,6 +553,7 @@ __device__ __forceinline__ float ld_logit<__nv_bfloat16>(const __nv_bfloat16* p,
 // second and third hit L1/L2.  Used for fp32 logits (config c1), V % 8 != 0, unaligned pointers, V > 155648.
 template <typename TIn, int G>
 __global__ void __launch_bounds__(256) loss_rows_generic(const LossParams p) {
+    pdl_wait();
     constexpr int kGroups = 256 / G;
     __shared__ float s_red[3][kGroups][8];
     const int tid = threadIdx.x, gl = tid % G, gi = tid / G, lane = tid & 31, wig = gl >> 5;
@@ -656,6 +664,7 @@ __global__ void __launch_bounds__(256) loss_rows_generic(const LossParams p) {
 
 // Fixed-order fp64 reduction: thread i sums elements i, i+1024, ...; then a shared-memory tree.
 __global__ void __launch_bounds__(1024) loss_final_kernel(const LossParams p, int by_row) {
+    pdl_wait();
     __shared__ double s_a[1024], s_b[1024];
     __shared__ int s_c[2][1024];
     const int tid = threadIdx.x;
@@ -789,20 +798,7 @@ cudaError_t launch_rows_t(const LossParams& p, int num_sms, cudaStream_t stream)
     auto kern = loss_rows_kernel<NCH, CSIZE, EXT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmemBytes);
     if (e != cudaSuccess) return e;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)((num_sms / CSIZE) * CSIZE));
-    cfg.blockDim = dim3(kThreads);
-    cfg.dynamicSmemBytes = kRowsSmemBytes;
-    cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = CSIZE;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    ajt::note_launch();
-    return cudaLaunchKernelEx(&cfg, kern, p);
+    return launch_dependent(kern, (num_sms / CSIZE) * CSIZE, kThreads, kRowsSmemBytes, stream, CSIZE, p);
 }
 
 template <int NCH, int CSIZE>
@@ -867,33 +863,31 @@ int loss_call(const void* logits, const int32_t* targets, const float* old_logp,
     p.row_k3 = reinterpret_cast<double*>(wsb + ws.row_k3);
     p.row_ent = reinterpret_cast<double*>(wsb + ws.row_ent);
 
+    const bool aligned = (((uintptr_t)logits | (uintptr_t)dlogits) & 15) == 0 && (ld_logits % 8) == 0 && (V % 8) == 0;
+    const bool fast = logits_dtype == AJT_DT_BF16 && aligned && T > 0 && V <= 2 * 16 * kChunkElems - 16;
+    p.zero_rows = fast ? 1 : 0;   // the fast kernels write the per-row outputs of unmasked rows only
     if (cudaMemsetAsync(p.ctrl, 0, ws.zero_bytes, stream) != cudaSuccess) return AJT_ERR_CUDA;
     const int ntiles = (int)((T + kPrepTile - 1) / kPrepTile);
     AJT_LAUNCH(loss_prep_kernel<<<max(1, min(ntiles, num_sms)), 1024, 0, stream>>>(p, ntiles));
 
-    const bool aligned = (((uintptr_t)logits | (uintptr_t)dlogits) & 15) == 0 && (ld_logits % 8) == 0 && (V % 8) == 0;
-    const bool fast = logits_dtype == AJT_DT_BF16 && aligned && T > 0;
     cudaError_t e = cudaSuccess;
     int by_row = 0;
-    if (fast && logp_out && cudaMemsetAsync(logp_out, 0, (size_t)T * sizeof(float), stream) != cudaSuccess) return AJT_ERR_CUDA;
-    if (fast && x.on && x.k3_out && cudaMemsetAsync(x.k3_out, 0, (size_t)T * sizeof(float), stream) != cudaSuccess) return AJT_ERR_CUDA;
-    if (fast && x.on && x.ent_out && cudaMemsetAsync(x.ent_out, 0, (size_t)T * sizeof(float), stream) != cudaSuccess) return AJT_ERR_CUDA;
     if (fast && V <= 8 * kChunkElems) e = launch_rows<8, 1>(p, num_sms, stream);
     else if (fast && V <= 16 * kChunkElems) e = launch_rows<16, 1>(p, num_sms, stream);
-    else if (fast && V <= 2 * 16 * kChunkElems - 16) e = launch_rows<16, 2>(p, num_sms, stream);
+    else if (fast) e = launch_rows<16, 2>(p, num_sms, stream);
     else if (T > 0) {
         by_row = 1;
         const int grid = num_sms * 8;
         if (logits_dtype == AJT_DT_F32) {
-            if (V <= 2048) AJT_LAUNCH(loss_rows_generic<float, 32><<<grid, 256, 0, stream>>>(p));
-            else AJT_LAUNCH(loss_rows_generic<float, 256><<<grid, 256, 0, stream>>>(p));
+            if (V <= 2048) e = launch_dependent(loss_rows_generic<float, 32>, grid, 256, 0, stream, 1, p);
+            else e = launch_dependent(loss_rows_generic<float, 256>, grid, 256, 0, stream, 1, p);
         } else {
-            if (V <= 2048) AJT_LAUNCH(loss_rows_generic<__nv_bfloat16, 32><<<grid, 256, 0, stream>>>(p));
-            else AJT_LAUNCH(loss_rows_generic<__nv_bfloat16, 256><<<grid, 256, 0, stream>>>(p));
+            if (V <= 2048) e = launch_dependent(loss_rows_generic<__nv_bfloat16, 32>, grid, 256, 0, stream, 1, p);
+            else e = launch_dependent(loss_rows_generic<__nv_bfloat16, 256>, grid, 256, 0, stream, 1, p);
         }
     }
     if (e != cudaSuccess) return AJT_ERR_CUDA;
-    AJT_LAUNCH(loss_final_kernel<<<1, 1024, 0, stream>>>(p, by_row));
+    if (launch_dependent(loss_final_kernel, 1, 1024, 0, stream, 1, p, by_row) != cudaSuccess) return AJT_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }
 }  // namespace

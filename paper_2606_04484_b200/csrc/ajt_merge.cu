@@ -174,13 +174,6 @@ __host__ MergeWs merge_ws_layout(int32_t n, int64_t N) {
 constexpr size_t kEntBytes = 32;  // per key slot: hash 8, dig 4, idx 4, tmp_dig 4, tmp_idx 4 = 24 used; ajt.h promises 32 per pair
 
 __device__ __forceinline__ bool fatal(const MergeParams& p) { return (p.ctrl->status & kFatal) != 0; }
-// Programmatic dependent launch: kernels 2..6 of the pipeline are launched while their predecessor still runs, so their CTAs
-// are resident (launch latency, shared-memory carve-out, parameter loads) when it ends.  Nothing the predecessor wrote is
-// read before pdl_wait(), which returns once the predecessor grid has completed and its writes are visible.
-__device__ __forceinline__ void pdl_wait() {
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-}
 
 __device__ __forceinline__ uint32_t digest32(uint64_t h, int32_t len) {
     uint64_t z = h ^ ((uint64_t)(uint32_t)len * 0xD6E8FEB86659FD93ull);
@@ -1881,21 +1874,6 @@ int merge_dev_facts(int* num_sms) {
     return AJT_OK;
 }
 
-template <class K>
-cudaError_t launch_dependent(K kern, int grid, int block, size_t smem, cudaStream_t stream, const MergeParams& p) {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3((unsigned)block);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    ajt::note_launch();
-    return cudaLaunchKernelEx(&cfg, kern, p);
-}
 }  // namespace
 
 extern "C" size_t ajt_merge_workspace_bytes(int32_t n, int64_t n_tokens) {
@@ -1987,12 +1965,12 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     const int64_t want = ((n_tokens >> kTSLog) + 1 + 255) / 256 + ((int64_t)n * 32 + 255) / 256;
     const int plan_grid = (int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8);
     const int64_t uwant = ((int64_t)n + 255) / 256;
-    if (launch_dependent(merge_units_kernel, (int)(uwant < (int64_t)num_sms * 4 ? uwant : (int64_t)num_sms * 4), 256, 0, stream, p) != cudaSuccess ||
-        launch_dependent(merge_hash_kernel, num_sms * 3, kHashThreads, kHashSmem, stream, p) != cudaSuccess ||
-        launch_dependent(merge_select_kernel, num_sms * 4, kSelThreads, sizeof(SelectStage), stream, p) != cudaSuccess ||
-        launch_dependent(merge_compact_kernel, 1, 1024, kCompactSmem, stream, p) != cudaSuccess ||
-        launch_dependent(merge_plan_kernel, plan_grid, 256, 0, stream, p) != cudaSuccess ||
-        launch_dependent(merge_scatter_kernel, num_sms, kScatThreads, kScatSmem, stream, p) != cudaSuccess)
+    if (launch_dependent(merge_units_kernel, (int)(uwant < (int64_t)num_sms * 4 ? uwant : (int64_t)num_sms * 4), 256, 0, stream, 1, p) != cudaSuccess ||
+        launch_dependent(merge_hash_kernel, num_sms * 3, kHashThreads, kHashSmem, stream, 1, p) != cudaSuccess ||
+        launch_dependent(merge_select_kernel, num_sms * 4, kSelThreads, sizeof(SelectStage), stream, 1, p) != cudaSuccess ||
+        launch_dependent(merge_compact_kernel, 1, 1024, kCompactSmem, stream, 1, p) != cudaSuccess ||
+        launch_dependent(merge_plan_kernel, plan_grid, 256, 0, stream, 1, p) != cudaSuccess ||
+        launch_dependent(merge_scatter_kernel, num_sms, kScatThreads, kScatSmem, stream, 1, p) != cudaSuccess)
         return AJT_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }
