@@ -19,7 +19,7 @@ namespace {
 
 using namespace ajt;
 
-constexpr int kBM = 128, kBN = 256, kBK = 64, kVS = 4;
+constexpr int kBM = 128, kBN = 256, kBK = 64, kVS = 16;
 constexpr int kABytes = kBM * kBK * 2;
 constexpr int kLmThreads = 192;   // warp 0: TMA producer, warp 1: MMA issuer + TMEM owner, warps 2-5: epilogue
 constexpr float kLog2e = 1.4426950408889634f;
@@ -134,14 +134,31 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
+// How many vocabulary ranges to cut the columns into, given the row blocks there really are (known only on the device when
+// masked rows were compacted away) and the G work groups of the launch: every group walks `rounds` items of `len` column
+// tiles each, so the launch takes ~ rounds x len tile times; the fewest ranges with the smallest product win.  (61 row
+// blocks on 74 groups: 4 ranges = 4 rounds x 149 tiles, 6 ranges = 5 x 99: 17 % less.)  Host and device, forward kernel and
+// combine kernel all call this with the same arguments.
+__host__ __device__ inline void choose_ranges(int64_t n_mtiles, int G, int V, int& nvs, int& vs_len) {
+    const int ncol = (V + kBN - 1) / kBN;
+    int64_t best = INT64_MAX;
+    nvs = 1;
+    vs_len = ncol * kBN;
+    for (int s = 1; s <= kVS && s <= ncol; ++s) {
+        const int len = (ncol + s - 1) / s, se = (ncol + len - 1) / len;   // se <= s ranges are not empty
+        const int64_t rounds = (n_mtiles * se + G - 1) / G, cost = rounds * len;
+        if (cost < best) { best = cost; nvs = se; vs_len = len * kBN; }
+    }
+}
+
 // Work unit u = (row block u / nvs, vocabulary range u % nvs); work group g (a CTA, or a CTA pair) takes units g, g + G, ...
 // Groups that run together hold neighbouring units: a few row blocks times all ranges, so the W ranges are shared through L2.
 template <int NCTA>
-__device__ __forceinline__ bool item_of(const LmParams& p, int n_mtiles, int it, int& mt, int& vs) {
+__device__ __forceinline__ bool item_of(int nvs, int n_mtiles, int it, int& mt, int& vs) {
     const int G = (int)gridDim.x / NCTA, g = (int)blockIdx.x / NCTA;
     const int64_t u = (int64_t)it * G + g;
-    mt = (int)(u / p.nvs);
-    vs = (int)(u % p.nvs);
+    mt = (int)(u / nvs);
+    vs = (int)(u % nvs);
     return mt < n_mtiles;
 }
 
@@ -171,7 +188,9 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
     }
     const int n_mtiles = (int)((Teff + kBM * NCTA - 1) / (kBM * NCTA));
     const int n_groups = (int)gridDim.x / NCTA;
-    const int n_items = (int)(((int64_t)n_mtiles * p.nvs + n_groups - 1) / n_groups);
+    int nvs = p.nvs, vs_len = p.vs_len;
+    if (nvs == 0) choose_ranges(n_mtiles, n_groups, p.V, nvs, vs_len);   // ranges fitted to the rows there are
+    const int n_items = (int)(((int64_t)n_mtiles * nvs + n_groups - 1) / n_groups);
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < kStages; ++i) {
@@ -205,8 +224,8 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
             uint32_t ph = 0;
             for (int it = 0; it < n_items; ++it) {
                 int mt, vs;
-                if (!item_of<NCTA>(p, n_mtiles, it, mt, vs)) continue;
-                const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
+                if (!item_of<NCTA>(nvs, n_mtiles, it, mt, vs)) continue;
+                const int v0 = vs * vs_len, v1 = min(p.V, v0 + vs_len);
                 const int row0 = (mt * NCTA + (int)rank) * kBM;
                 for (int n0 = v0; n0 < v1; n0 += kBN) {
                     for (int k = 0; k < nk; ++k) {
@@ -233,8 +252,8 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
             uint32_t ph = 0, aph = 0;
             for (int it = 0; it < n_items; ++it) {
                 int mt, vs;
-                if (!item_of<NCTA>(p, n_mtiles, it, mt, vs)) continue;
-                const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
+                if (!item_of<NCTA>(nvs, n_mtiles, it, mt, vs)) continue;
+                const int v0 = vs * vs_len, v1 = min(p.V, v0 + vs_len);
                 for (int n0 = v0; n0 < v1; n0 += kBN) {
                     mbar_wait(&tempty[as], aph ^ 1u);
                     tc_fence_after();
@@ -265,10 +284,10 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
         uint32_t aph = 0;
         for (int it = 0; it < n_items; ++it) {
             int mt, vs;
-            if (!item_of<NCTA>(p, n_mtiles, it, mt, vs)) continue;
+            if (!item_of<NCTA>(nvs, n_mtiles, it, mt, vs)) continue;
             const int64_t row = (int64_t)(mt * NCTA + (int)rank) * kBM + rloc;
             const bool live = row < Teff;
-            const int v0 = vs * p.vs_len, v1 = min(p.V, v0 + p.vs_len);
+            const int v0 = vs * vs_len, v1 = min(p.V, v0 + vs_len);
             if (MODE != kReduce) {
                 // ---- backward epilogues: one row of the tile per thread, 32 columns at a time
                 int y = -1;
@@ -418,25 +437,27 @@ __global__ void __launch_bounds__(kLmThreads, 1) lm_head_kernel(const __grid_con
 
 // Folds the range partials of every processed row and writes the outputs at the row's ORIGINAL position (the outputs of
 // masked rows were zeroed beforehand when the rows were compacted).
-__global__ void __launch_bounds__(256) lm_head_combine_kernel(const LmParams p, int nvs) {
+__global__ void __launch_bounds__(256) lm_head_combine_kernel(const LmParams p, int groups, int ncta) {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     const int64_t Teff = p.n_rows ? (int64_t)*p.n_rows : p.T;
+    int nvs, vs_len;   // the ranges the tile kernel chose: same function, same arguments
+    choose_ranges((Teff + kBM * ncta - 1) / (kBM * ncta), groups, p.V, nvs, vs_len);
     for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < Teff; t += stride) {
         float lp = 0.f, H = 0.f, lse = 0.f;
         {
-            float4 q[kVS];
+            const float4* q = p.part + t * kVS;
             float M = -INFINITY, zy = -INFINITY;
             for (int k = 0; k < nvs; ++k) {
-                q[k] = p.part[t * kVS + k];
                 M = fmaxf(M, q[k].x);
                 zy = fmaxf(zy, q[k].w);   // exactly one range holds the target; the others left -inf
             }
             float S = 0.f, U = 0.f;
             for (int k = 0; k < nvs; ++k) {
-                const float f = q[k].x == -INFINITY ? 0.f : ex2((q[k].x - M) * kLog2e);
-                const float dm = q[k].x == -INFINITY ? 0.f : q[k].x - M;
-                U += f * fmaf(dm, q[k].y, q[k].z);
-                S += f * q[k].y;
+                const float4 v = q[k];
+                const float f = v.x == -INFINITY ? 0.f : ex2((v.x - M) * kLog2e);
+                const float dm = v.x == -INFINITY ? 0.f : v.x - M;
+                U += f * fmaf(dm, v.y, v.z);
+                S += f * v.y;
             }
             const float logS = logf(S);
             lp = (zy - M) - logS;
@@ -631,15 +652,13 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
         return AJT_ERR_CUDA;
 
     const int64_t n_mtiles = (T + kBM * ncta - 1) / (kBM * ncta);   // row blocks of 128 * ncta rows (upper bound when rows are compacted)
-    const int nvs = V >= kVS * kBN ? kVS : 1;   // small vocabularies: one range
-    p.nvs = nvs;
-    p.vs_len = (((V + nvs - 1) / nvs + kBN - 1) / kBN) * kBN;
+    p.nvs = 0;                                  // the kernel fits the vocabulary ranges to the rows there really are
+    p.vs_len = 0;
     int groups = num_sms / ncta;                // one work group per SM (pair of SMs)
-    if ((int64_t)groups > n_mtiles * nvs) groups = (int)(n_mtiles * nvs);
+    if ((int64_t)groups > n_mtiles * kVS) groups = (int)(n_mtiles * kVS);
     p.part = reinterpret_cast<float4*>(wsb + ws.part);
     p.logp_out = logp_out; p.ent_out = ent_out; p.lse_out = lse_out;
 
-    // ranges beyond nvs are empty (v0 >= V): their CTAs have nothing to do, and the combine reads nvs partials per row
     if (ncta == 1) {
         if (cudaFuncSetAttribute(lm_head_kernel<1, kReduce>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<1>::kSmem) != cudaSuccess)
             return AJT_ERR_CUDA;
@@ -663,7 +682,7 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
         if (cudaLaunchKernelEx(&cfg, lm_head_kernel<2, kReduce>, map_h, map_w, p) != cudaSuccess) return AJT_ERR_CUDA;
     }
     const int64_t want = (T + 255) / 256;
-    AJT_LAUNCH(lm_head_combine_kernel<<<(int)(want < (int64_t)num_sms * 4 ? want : (int64_t)num_sms * 4), 256, 0, stream>>>(p, nvs));
+    AJT_LAUNCH(lm_head_combine_kernel<<<(int)(want < (int64_t)num_sms * 4 ? want : (int64_t)num_sms * 4), 256, 0, stream>>>(p, groups, ncta));
     return cudaGetLastError() == cudaSuccess ? AJT_OK : AJT_ERR_CUDA;
 }
 
@@ -678,7 +697,7 @@ extern "C" int ajt_lm_head_logp(const void* hidden, const void* weight, const in
 // against 6 R V d flops (d = 4096: 0.016 % of the time at the roofs).  Masked rows cost nothing (they are compacted away).
 namespace {
 
-constexpr int kBwdChunk = 4096;   // rows of dZ staged at a time (multiple of 256)
+constexpr int kBwdChunk = 4096;   // rows of dZ staged at a time (multiple of 256); 9,472 (8 full rounds of dH tiles) measured 5 % slower
 
 // d loss / d logp of every compacted row k (original row t = row_idx[k], or k), the row's lse, and the loss: steps 2-6 of O-L
 // on the forward pass's log-probs (ajt_token.cuh).  Block partials in fp64, summed in block order by the last kernel.
@@ -794,16 +813,16 @@ int lm_launch(EncodeTiledFn encode, int num_sms, const void* A, int64_t M, int64
     CUtensorMap map_a, map_b;
     if (!make_map(encode, &map_a, A, M, (int32_t)K, lda, kBM) || !make_map(encode, &map_b, Bm, N, (int32_t)K, ldb, kBN / ncta)) return AJT_ERR_CUDA;
     p.T = M; p.d = (int32_t)K; p.V = (int32_t)N;
-    if (ranges) {   // the forward's decomposition: 4 vocabulary ranges walked tile by tile
-        p.nvs = N >= kVS * kBN ? kVS : 1;
-        p.vs_len = (int32_t)((((N + p.nvs - 1) / p.nvs + kBN - 1) / kBN) * kBN);
+    if (ranges) {   // the forward's decomposition: vocabulary ranges walked tile by tile
+        p.nvs = 0;   // fitted on the device
+        p.vs_len = 0;
     } else {        // one output tile per work item
         p.nvs = (int32_t)((N + kBN - 1) / kBN);
         p.vs_len = kBN;
     }
     const int64_t n_mtiles = (M + kBM * ncta - 1) / (kBM * ncta);
     int groups = num_sms / ncta;
-    if ((int64_t)groups > n_mtiles * p.nvs) groups = (int)(n_mtiles * p.nvs);
+    if ((int64_t)groups > n_mtiles * (p.nvs ? p.nvs : kVS)) groups = (int)(n_mtiles * (p.nvs ? p.nvs : kVS));
     if (cudaFuncSetAttribute(lm_head_kernel<ncta, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LmCfg<ncta>::kSmem) != cudaSuccess)
         return AJT_ERR_CUDA;
     cudaLaunchConfig_t cfg = {};
