@@ -1405,12 +1405,12 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
             sk = dd[cur];   // after 4 passes cur == 0: digests are back in ent_dig (sorted), order in ent_idx
             sv = kk[cur];
         }
-        // visit(dg, fn): fn(le) for every key slot of this group whose digest is dg (the equal-key run)
+        // visit(dg, fn): one warp; fn(le) for every key slot of this group whose digest is dg (the equal-key run), a lane each
         auto visit = [&](uint32_t dg, auto fn) {
             if (small) {
                 const uint32_t b = dg >> (32 - kSelBucketBits);
                 const uint32_t x1 = sm.start[b], x0 = b ? sm.start[b - 1] : 0u;
-                for (uint32_t x = x0; x < x1; ++x) {
+                for (uint32_t x = x0 + lane; x < x1; x += 32) {
                     const uint32_t le = sm.sorted[x];
                     if (sm.dig[le] == dg) fn(le);
                 }
@@ -1420,7 +1420,12 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
                     const int mid = (lo + hi) >> 1;
                     if (sk[mid] < dg) lo = mid + 1; else hi = mid;
                 }
-                for (int x = lo; x < c && sk[x] == dg; ++x) fn(sv[x]);
+                for (int x0 = lo;; x0 += 32) {
+                    const int x = x0 + lane;
+                    const bool in = x < c && sk[x] == dg;
+                    if (in) fn(sv[x]);
+                    if (!__all_sync(0xffffffffu, in)) break;
+                }
             }
         };
         // Verification rounds.  pick(b) proposes a candidate for every undecided member (or decides it); proposals that no
@@ -1443,7 +1448,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
         };
         // ---- M4 + M5: survivors and the Algorithm-1 owner = the latest extender
         while (true) {
-            for (int b = tid; b < k; b += NT) {
+            for (int b = warp; b < k; b += NT / 32) {   // a warp per member: the lanes share its equal-key run
                 if (own[b] != -2) continue;
                 const uint64_t H = eh[b * (b + 1) / 2 + b];   // full key of member b
                 const int32_t L = gln[b];
@@ -1458,9 +1463,12 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
                     if (gln[a] != L || eh[le] != H) return;
                     best = rb;
                 });
-                if (best < 0) own[b] = -1;
-                else if (badc[best] == badc[b]) own[b] = best;   // every link b+1 .. best was verified by the hash pass
-                else vq[atomicAdd(&sm.qn, 1)] = make_int2(b, best);
+                best = __reduce_max_sync(0xffffffffu, best);
+                if (lane == 0) {
+                    if (best < 0) own[b] = -1;
+                    else if (badc[best] == badc[b]) own[b] = best;   // every link b+1 .. best was verified by the hash pass
+                    else vq[atomicAdd(&sm.qn, 1)] = make_int2(b, best);
+                }
             }
             if (run_queue([&](int b, int cd) { own[b] = cd; }, [&](int b, int cd) { lim[b] = cd; }) == 0) break;
         }
@@ -1469,7 +1477,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
             for (int b = tid; b < k; b += NT) { fin[b] = own[b] >= 0 ? -2 : -1; exL[b] = INT32_MAX; exR[b] = -1; }
             __syncthreads();
             while (true) {
-                for (int b = tid; b < k; b += NT) {
+                for (int b = warp; b < k; b += NT / 32) {
                     if (fin[b] != -2) continue;
                     const uint64_t H = eh[b * (b + 1) / 2 + b];
                     const int32_t L = gln[b];
@@ -1489,9 +1497,14 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
                         best = rb;
                         bestL = Li;
                     });
-                    if (best < 0 || best == own[b]) fin[b] = own[b];                // the Algorithm-1 owner is verified already
-                    else if (badc[best] == badc[b]) fin[b] = best;
-                    else vq[atomicAdd(&sm.qn, 1)] = make_int2(b, best);
+                    // the longest over the lanes, then the lowest rank among those
+                    const int32_t topL = __reduce_max_sync(0xffffffffu, bestL);
+                    best = (int)__reduce_min_sync(0xffffffffu, best >= 0 && bestL == topL ? (unsigned)best : 0xFFFFFFFFu);
+                    if (lane == 0) {
+                        if (best < 0 || best == own[b]) fin[b] = own[b];            // the Algorithm-1 owner is verified already
+                        else if (badc[best] == badc[b]) fin[b] = best;
+                        else vq[atomicAdd(&sm.qn, 1)] = make_int2(b, best);
+                    }
                 }
                 if (run_queue([&](int b, int cd) { fin[b] = cd; }, [&](int b, int cd) { exL[b] = gln[cd]; exR[b] = cd; }) == 0) break;
             }
