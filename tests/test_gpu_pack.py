@@ -123,3 +123,58 @@ def test_hbm_probe_modes():
     assert not bool(b.any()) and not bool(a.any())
     with pytest.raises(ajt.AjtError):
         ajt.hbm_probe(b, None, 4 * n + 4, 1)      # not a multiple of 16 bytes
+
+
+def test_chain_captured_in_a_cuda_graph_replays_bit_exactly():
+    """include/ajt.h: the device-pointer calls only enqueue on the caller's stream (no synchronisation, no cooperative launch;
+    kernels 2.. of a call are programmatic dependents of their predecessor), so merge -> pack -> segment counts -> loss can be
+    captured once and replayed.  The replay on NEW inputs of the same shapes must equal the eager calls on them bit for bit."""
+    mi = W.merge_workload("c2")
+    uniq, tl_seg = np.unique(mi.traj_ids, return_inverse=True)
+    S = int(uniq.shape[0])
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    tokens, offsets, traj, rs, lp = d(mi.tokens), d(mi.offsets), d(mi.traj_ids), d(mi.resp_start), d(mi.old_logp)
+    tls, adv = d(tl_seg.astype(np.int32)), d(W.advantages_group_zscore(W.BASE_SEED, 1, S))
+    T, V = 1500, 4096
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    logits = (torch.randn((T, V), generator=gen, device="cuda") * 2).to(torch.bfloat16)
+    old = torch.full((T,), -8.5, device="cuda")
+    stream = torch.cuda.Stream()
+    st = {}
+
+    def chain():
+        st["mo"] = ajt.merge_timelines(tokens, offsets, traj, rs, None, lp, out=st.get("mo"), stream=stream)
+        st["pk"] = ajt.pack_loss_inputs(st["mo"], tls, S, adv, out=st.get("pk"), stream=stream)
+        pk = st["pk"]
+        st["Ns"] = ajt.segment_counts(pk.mask[:T], pk.seg_ids[:T], S, out=st.get("Ns"), stream=stream)
+        st["lo"] = ajt.policy_loss_fwd_bwd(logits, pk.targets[:T], old, pk.adv[:T], pk.mask[:T], pk.seg_ids[:T], S, 0.2, 0.28,
+                                           seg_denom=st["Ns"], out=st.get("lo"), stream=stream)
+
+    with torch.cuda.stream(stream):
+        chain()                      # eager once: allocates every output and workspace
+        stream.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=stream):
+            chain()
+        # new inputs, same shapes: the token values go through a bijection (same prefix structure, other contents), the
+        # log-probs are halved, the logits redrawn
+        tok2 = (mi.tokens.astype(np.int64) * 7 + 3) % 151939   # 151939 is prime: a bijection on [0, 151939)
+        mi2 = W.MergeInputs(tok2.astype(np.int32), mi.offsets, mi.traj_ids, mi.resp_start, (mi.old_logp * 0.5).astype(np.float32))
+        tokens.copy_(d(mi2.tokens)); lp.copy_(d(mi2.old_logp))
+        logits.copy_((torch.randn((T, V), generator=gen, device="cuda") * 2).to(torch.bfloat16))
+        g.replay()
+        stream.synchronize()
+        got = {k: v.clone() for k, v in dict(tok=st["mo"].merged_tokens, mask=st["mo"].merged_mask, src=st["mo"].merged_src,
+                                             cnt=st["mo"].counts, dl=st["lo"].dlogits, loss=st["lo"].loss, tg=st["pk"].targets).items()}
+        st.clear()
+        chain()                      # eager on the same new inputs
+        stream.synchronize()
+    want = dict(tok=st["mo"].merged_tokens, mask=st["mo"].merged_mask, src=st["mo"].merged_src, cnt=st["mo"].counts,
+                dl=st["lo"].dlogits, loss=st["lo"].loss, tg=st["pk"].targets)
+    N = int(want["cnt"][1])
+    assert N > 0 and torch.equal(got["cnt"], want["cnt"])
+    for k in ("tok", "mask", "src", "tg"):
+        assert torch.equal(got[k][:N], want[k][:N]), k
+    assert torch.equal(got["dl"], want["dl"]) and torch.equal(got["loss"], want["loss"])
+    r = oracle.merge_timelines(mi2.tokens, mi2.offsets, mi2.traj_ids, mi2.resp_start, None, mi2.old_logp)
+    assert N == r.N_out and np.array_equal(got["tok"][:N].cpu().numpy(), r.merged_tokens)
