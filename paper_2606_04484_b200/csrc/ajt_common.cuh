@@ -31,7 +31,7 @@ struct AjtCtrl {
     // merge (round 2)
     int32_t n_units;      // hash units: (chunk of ranks, block of slices) pairs
     int32_t unit_ticket;  // hash pass: dynamic unit ticket
-    int32_t n_chunks;     // chunks of consecutive ranks of grouped groups
+    int32_t unused0;
     int32_t n_gsegs;      // scatter segments (constant-source runs of the merged output)
     int32_t scat_ticket;  // scatter pass: dynamic tile ticket
     uint32_t reserved[43];

@@ -113,8 +113,7 @@ struct MergeParams {
     int4* tl_rec;          // [n] BY SORTED POSITION: {first hash slice, group start (sorted position), members of the group, first key slot of the timeline}
     uint8_t* lbad;         // [n] BY SORTED POSITION: the member differs from its in-group predecessor on that one's positions (exact)
     int4* grp_rec;         // [G+1] {group start, members, first key slot, first hash unit}
-    int2* unit_rec;        // [slice_cap] hash units {chunk, slice block}, the largest (lowest slices) first
-    int4* chunk_rec;       // [n+1] chunks of consecutive ranks of a group: {group start (sorted position), first rank, members of the group, first key slot of the group}
+    int4* unit_rec;        // [slice_cap] hash units {group start (sorted position), first rank of the chunk, members of the group, slice}
     uint64_t* seg_part;    // [slice_cap] per (member, slice) hash totals, then exclusive prefixes per member
     uint64_t* ent_hash;    // [E_cap] key slot (r, a), a = 0..r: in-slice partial, then the final prefix hash
     uint32_t* ent_dig;     // [E_cap] global sort path: digests / order ping-pong
@@ -138,7 +137,7 @@ struct MergeParams {
 };
 
 struct MergeWs {
-    size_t ctrl, gbuf[6], perm, glen, goff, tl_rec, lbad, grp_rec, unit_rec, chunk_rec, seg_part, absorbed, owner_tl, midx, sel[8],
+    size_t ctrl, gbuf[6], perm, glen, goff, tl_rec, lbad, grp_rec, unit_rec, seg_part, absorbed, owner_tl, midx, sel[8],
         sel_q, mem_list, sv_rec, rseg, gseg_base, gseg, tile_seg, ent;
 };
 __host__ inline size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -155,8 +154,7 @@ __host__ MergeWs merge_ws_layout(int32_t n, int64_t N) {
     w.tl_rec = o; o += n16;
     w.lbad = o; o += a256((size_t)n + 2);
     w.grp_rec = o; o += n16;
-    w.unit_rec = o; o += a256(sc * 8);
-    w.chunk_rec = o; o += n16;
+    w.unit_rec = o; o += a256(sc * 16);
     w.seg_part = o; o += a256(sc * 8);
     w.absorbed = o; o += a256((size_t)n + 2);
     w.owner_tl = o; o += n4; w.midx = o; o += n4;
@@ -647,9 +645,9 @@ __global__ void __launch_bounds__(1024) merge_group_radix_kernel(const MergePara
 // ---------------------------------------------------------------------------------------- K1b: hash units
 
 // Hash units, in parallel over the whole GPU (the group kernel is one SM): thread per sorted position; the thread of a rank
-// that is a multiple of kChunk in a group of at least two opens a chunk {group start, first rank, members, first key slot} and
-// one unit per block of kSliceBlk slices up to the chunk's longest member.  Chunk ids and unit slots come from two counters
-// (one atomic per warp each); units are short (<= kChunk + 1 member-slices per slice), so their order does not matter.
+// that is a multiple of kChunk in a group of at least two emits one unit {group start, first rank, members of the group, slice}
+// per slice up to the longest member of its chunk.  Unit slots come from one counter (one atomic per warp); units are short
+// (<= kChunk + 1 member-slices), so their order does not matter.
 __global__ void __launch_bounds__(256) merge_units_kernel(const MergeParams p) {
     pdl_wait();
     if (fatal(p)) return;
@@ -664,10 +662,9 @@ __global__ void __launch_bounds__(256) merge_units_kernel(const MergeParams p) {
         if (open) {
             int mx = 0;
             for (int x = 0; x < min(kChunk, k - r); ++x) mx = max(mx, __ldg(p.glen + pos + x));
-            cnt = (slices_of(mx) + kSliceBlk - 1) / kSliceBlk;
+            cnt = slices_of(mx);
         }
-        const unsigned om = __ballot_sync(0xffffffffu, open);
-        if (om == 0) continue;
+        if (!__any_sync(0xffffffffu, open)) continue;
         int inc = cnt;   // inclusive scan of the unit counts over the warp
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -675,18 +672,12 @@ __global__ void __launch_bounds__(256) merge_units_kernel(const MergeParams p) {
             if (lane >= o) inc += v;
         }
         const int tot = __shfl_sync(0xffffffffu, inc, 31);
-        int cb = 0, ub = 0;
-        if (lane == 0) {
-            cb = atomicAdd(&p.ctrl->n_chunks, __popc(om));
-            ub = atomicAdd(&p.ctrl->n_units, tot);
-        }
-        cb = __shfl_sync(0xffffffffu, cb, 0);
+        int ub = 0;
+        if (lane == 0) ub = atomicAdd(&p.ctrl->n_units, tot);
         ub = __shfl_sync(0xffffffffu, ub, 0);
         if (open) {
-            const int c = cb + __popc(om & ((1u << lane) - 1u));
-            p.chunk_rec[c] = make_int4(gs, r, k, t.w - (int)((uint32_t)r * (uint32_t)(r + 1) / 2u));
-            int2* const ur = p.unit_rec + ub + inc - cnt;
-            for (int j = 0; j < cnt; ++j) ur[j] = make_int2(c, j);
+            int4* const ur = p.unit_rec + ub + inc - cnt;
+            for (int j = 0; j < cnt; ++j) ur[j] = make_int4(gs, r, k, j);
         }
     }
 }
@@ -816,11 +807,10 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
     while (next < U) {
         const int u = next;
         if (lane == 0) next = atomicAdd(&p.ctrl->unit_ticket, 1);   // needed only after this unit: the round trip is hidden
-        const int2 ur = __ldg(p.unit_rec + u);                      // {chunk, slice}
-        const int4 cr = __ldg(p.chunk_rec + ur.x);                  // {group start, first rank, members of the group, first key slot}
-        const int gs = cr.x, k = cr.z, w = ur.y;
-        const int rlo = cr.y - (cr.y > 0 ? 1 : 0);                  // lane i holds rank rlo + i: the predecessor of the chunk first
-        const int rhi = min(k, cr.y + kChunk);
+        const int4 ur = __ldg(p.unit_rec + u);                      // {group start, first rank, members of the group, slice}
+        const int gs = ur.x, r0 = ur.y, k = ur.z, w = ur.w;
+        const int rlo = r0 - (r0 > 0 ? 1 : 0);                      // lane i holds rank rlo + i: the predecessor of the chunk first
+        const int rhi = min(k, r0 + kChunk);
         const int32_t* __restrict__ gln = p.glen + gs;
         const int S0 = w * kSl;                                     // first position of the slice
         // ---- each lane's member and its slot in this slice
@@ -828,14 +818,14 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
         const int myr = rlo + lane;
         const int iL = mine ? __ldg(gln + myr) : 0;
         const int64_t ioff = mine ? __ldg(p.goff + gs + myr) : 0;
-        const int isb = mine ? __ldg(reinterpret_cast<const int32_t*>(p.tl_rec + gs + myr)) : 0;
+        const int4 trec = mine ? __ldg(p.tl_rec + gs + myr) : make_int4(0, 0, 0, 0);   // .x first slice, .w first key slot
         const int L0 = lane < k ? __ldg(gln + lane) : 0;   // lengths of the group's first 32 ranks: where prefixes end
         const int iD = (int)((ioff + mis + S0) & 3);               // slot element of position S0
         const int64_t ig0 = ioff + S0 - iD;                        // array index of slot element 0
         const int inv = (min(iL - S0, kSl) + iD + 3) >> 2;         // vectors holding positions < min(L, S0 + 508): at most 128
         const bool iedge = !(ig0 >= 0 && ig0 + 4 * (int64_t)inv <= N);
-        uint64_t* const my_tot = p.seg_part + isb + w;             // where this member's slice total goes
-        uint64_t* const my_keys = p.ent_hash + (int64_t)cr.w + (int64_t)myr * (myr + 1) / 2;   // its key slots (myr, a), a <= myr
+        uint64_t* const my_tot = p.seg_part + trec.x + w;          // where this member's slice total goes
+        uint64_t* const my_keys = p.ent_hash + trec.w;             // its key slots (myr, a), a <= myr
         unsigned preach = __ballot_sync(0xffffffffu, iL > S0);     // members still to be fetched / still to be worked on
         unsigned creach = preach;
         const unsigned edges = __ballot_sync(0xffffffffu, iedge) & preach;
@@ -892,7 +882,7 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
             if (lane < D) sts32(slot + 4 * lane, 0u);
             if (lane < 4 && D + len + lane < (len == kSl ? kSlotBytes / 4 : (len + D + 3) & ~3)) sts32(slot + 4 * (D + len + lane), 0u);
             __syncwarp();
-            if (r < cr.y) {   // the previous chunk's last member: here to be compared with, nothing else
+            if (r < r0) {   // the previous chunk's last member: here to be compared with, nothing else
                 prev_hashed = false;
             } else {
                 const bool have_prev = prev_r == r - 1;
@@ -1936,8 +1926,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     p.tl_rec = reinterpret_cast<int4*>(b + ws.tl_rec);
     p.lbad = b + ws.lbad;
     p.grp_rec = reinterpret_cast<int4*>(b + ws.grp_rec);
-    p.unit_rec = reinterpret_cast<int2*>(b + ws.unit_rec);
-    p.chunk_rec = reinterpret_cast<int4*>(b + ws.chunk_rec);
+    p.unit_rec = reinterpret_cast<int4*>(b + ws.unit_rec);
     p.seg_part = reinterpret_cast<uint64_t*>(b + ws.seg_part);
     p.absorbed = b + ws.absorbed;
     p.owner_tl = reinterpret_cast<int32_t*>(b + ws.owner_tl);
