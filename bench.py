@@ -406,7 +406,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                          "launches; rows is >99% of it, profiles/)", "achieved": ach, "peak": peak, "unit": "GB/s",
                          "frac": ach / peak, "traffic": traffic, "traffic_note": traffic_note, "peak_source": peak_src},
             "hbm_ceilings": ceilings, "clocks": clocks, "gpu_launches": int(launches),
-            "gpu_launches_how": "counted by the library (ajt_launch_count before / after the timed region): merge 6, pack 1, "
+            "gpu_launches_how": "counted by the library (ajt_launch_count before / after the timed region): merge 7, pack 1, "
                                 "segment counts 1, loss 3 per step",
             "e2e": e2e, "cpu_baseline": cpu_baseline, "configs": cfg_records,
             "paper_context": "paper reports only end-to-end actor-update 2160 s -> 346 s (6.25x) with merging on AppWorld, "

@@ -33,7 +33,7 @@ struct AjtCtrl {
     int32_t unit_ticket;  // hash pass: dynamic unit ticket
     int32_t unused0;
     int32_t n_gsegs;      // scatter segments (constant-source runs of the merged output)
-    int32_t scat_ticket;  // scatter pass: dynamic tile ticket
+    int32_t unused1;
     uint32_t reserved[43];
 };
 static_assert(sizeof(AjtCtrl) == 256, "AjtCtrl must be 256 bytes");

@@ -1762,11 +1762,12 @@ __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const Me
     };
     const bool out_ok = ((((uintptr_t)p.merged_tokens | (uintptr_t)p.merged_src | (uintptr_t)p.merged_old_logp | (uintptr_t)p.merged_mask) & 15) == 0);
     if (wglobal >= ntiles) return;
-    // Tiles: the first three of a warp are fixed (wglobal, + nwarps, + 2 nwarps), the rest come from a ticket, three tiles
-    // ahead of the one at work -- tiles cut into several pieces take longer than plain ones, and a fixed stride leaves the
-    // last warp 30 % behind the median.  tA: at work; tB: its copies are in flight; tC: its segment record is being loaded.
+    // Tiles go round the warps with a fixed stride.  (Handing them out by an atomic ticket evens out the warps' finishing
+    // times -- tiles cut into several pieces take longer -- but 45 k same-address atomics cost more than that: 256 against
+    // 235 us for the whole merge inside the bench step.)  tA: at work; tB: its copies are in flight; tC: its segment record
+    // is being loaded.
     int tA = wglobal, tB = wglobal + nwarps, tC = wglobal + 2 * nwarps, pend = 0;
-    if (lane == 0) pend = atomicAdd(&p.ctrl->scat_ticket, 1) + 3 * nwarps;
+    pend = wglobal + 3 * nwarps;
     GSeg rec = load_rec(tA);
     int np_cur = out_ok ? plan(tA, 0, rec) : -1;
     if (tB < ntiles) rec = load_rec(tB);
@@ -1830,8 +1831,8 @@ __global__ void __launch_bounds__(kScatThreads, 1) merge_scatter_kernel(const Me
         np_cur = np_next;
         tA = tB;
         tB = tC;
-        tC = __shfl_sync(0xffffffffu, pend, 0);
-        if (lane == 0) pend = atomicAdd(&p.ctrl->scat_ticket, 1) + 3 * nwarps;
+        tC = pend;
+        pend += nwarps;
         if (__any_sync(0xffffffffu, dead)) break;
     }
     if (dead && lane == 0) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_INTERNAL);
