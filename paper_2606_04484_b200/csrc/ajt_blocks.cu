@@ -9,7 +9,7 @@
 // mask from block k of that member (lines 12-14), else from s itself.
 //
 //   blocks_prep_kernel     offsets in id-words, mask per id-word                                     tiny
-//   (6 launches of the token-level merge on 8 B per block)
+//   (7 launches of the token-level merge on 8 B per block)
 //   blocks_info_kernel     per merged block: supplying timeline, source block, length, author        tiny (per block)
 //   blocks_scan_kernel     single-pass exclusive scan of the block lengths -> token offsets          tiny
 //   blocks_offsets_kernel  merged_offsets / merged_block_offsets / counts                            tiny

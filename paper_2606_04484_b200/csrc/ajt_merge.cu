@@ -1,46 +1,45 @@
 // Stage (a): timeline merging (Algorithm 1) on flat token streams, sm_100a.
 //
-// Definition: DESIGN.md "O-M".  Pipeline (rows M1-M7 of the scope table), 5 launches on one
-// stream, no host round trip, no cooperative launch (the call can be captured in a CUDA graph):
-//   K1 merge_group_fast_kernel  M1  one CTA, everything in shared memory (n <= 7936): trajectory ids go through a hash
-//                                   table (atomicCAS), groups are laid out by a scan over its slots, members are placed with
-//                                   an atomic cursor and ranked by counting (in-group order = input order).  Emits, by
-//                                   SORTED POSITION, {timeline, length, token offset, first hash slice, rank, first key
-//                                   slot}, and one record per HASH UNIT = (group, slice of 512 token positions).
-//                                   merge_group_radix_kernel (stable LSD radix sort through the workspace) does the same
-//                                   for larger batches.
-//   K2 merge_hash_kernel        M2  warp per hash unit (dynamic ticket): the warp streams the SAME 512 positions of every
-//                                   member of the group, in order, through a warp-private 4-stage cp.async ring (16-byte
-//                                   async copies of the aligned superset, whatever the member's alignment).  The prefix
-//                                   hash F_i(p) = sum_{q<p} x_q w(q) mod 2^64, w(q) = W^(q+3) mod 2^32, is a sum over
-//                                   positions, hence a monoid: the lane weights depend on the positions only and are
-//                                   computed once per unit; every lane keeps its partial and lanes are combined with
-//                                   three REDUX where a value leaves the warp: the slice total of every member, and one key
-//                                   per (member r, earlier member a with L_a <= L_r) whose prefix end L_a - 1 lies in this
-//                                   slice (probe keys; a = r gives the full key).
-//                               M5  (first half) member r is compared EXACTLY with member r - 1 on the way, register
-//                                   against register (both slices pass through the same lanes): a difference marks the
-//                                   link r-1 -> r broken.  Every token is loaded once; nothing is re-read.
-//   K3 merge_select_kernel      M2  (end) one CTA per group: exclusive prefix of each member's slice totals -> final keys
-//                               M3  segmented radix sort of the group's (hash, length) keys by a 32-bit digest: one MSD
-//                                   pass on the top 11 bits in shared memory (<= 2048 keys), 4 LSD passes through global
-//                                   memory above that
-//                               M4  per timeline: its equal-key run gives the hash-equal extenders; survivor flag,
-//                                   Algorithm-1 owner (latest extender), under LONGEST the longest surviving extender
-//                               M5  (second half) a candidate is ACCEPTED only if an unbroken chain of verified links
-//                                   leads to it (prefix-of is transitive) or after an exact warp-cooperative token
-//                                   comparison (128-bit loads when the two are co-aligned); a hash-equal candidate that
-//                                   fails is skipped (AJT_STATUS_HASH_COLLISION, informational).  Results are exact
-//                                   whatever the hash does (AJT_MERGE_WEAK_HASH degrades it to 4 bits to test this).
-//                                   Then per survivor: its member list and its SEGMENTS (maximal runs of positions with
-//                                   one source of mask / log-prob), warp-cooperatively.
-//                               M6  the last CTA to finish scans the timelines once: survivors in original order ->
-//                                   merged_offsets / origin / traj, owner, first segment of every merged sequence
-//   K4 merge_plan_kernel        M7  segments rebased to output positions (one 32-byte record each), and for every tile
-//                                   of 512 OUTPUT positions the first segment that touches it
-//   K5 merge_scatter_kernel     M7  warp per output tile: one record lookup, then plain coalesced copies -- lane l moves
-//                                   positions l + 32 j of the tile: tokens from the survivor, mask / src constants of the
-//                                   segment, old_logp from the supplying member -- whatever the alignment of the sources
+// Definition: DESIGN.md "O-M".  Pipeline (rows M1-M7 of the scope table), 7 launches on one
+// stream, no host round trip, no cooperative launch (the call can be captured in a CUDA graph); kernels 2-7 are programmatic
+// dependents of their predecessor (griddepcontrol), so their launch latency overlaps its tail:
+//   K1  merge_group_fast_kernel  M1  one CTA, everything in shared memory (n <= 7936): trajectory ids go through a hash
+//                                    table (atomicCAS), groups are laid out by a scan over its slots, members are placed
+//                                    with an atomic cursor and put in input order by a bitonic network per warp.  Emits, by
+//                                    SORTED POSITION, {timeline, length, token offset, first hash slice, group start, group
+//                                    size, first key slot}.  merge_group_radix_kernel (stable LSD radix sort through the
+//                                    workspace) does the same for larger batches.
+//   K1b merge_units_kernel       M1  the hash pass's work list, built over the whole GPU: chunks of 8 consecutive ranks of a
+//                                    group x slices of 508 positions up to the chunk's longest member.
+//   K2  merge_hash_kernel        M2  warp per unit (dynamic ticket): the warp streams the SAME 508 positions of the chunk's
+//                                    members, in rank order, through a warp-private ring of 2 KB slots, one bulk async copy
+//                                    (TMA, 1-D) of the aligned superset each.  Prefix hash in the ring mod 2^32,
+//                                    F_i(p) = sum_{q<p} x_q W^q: weights per slot element, one REDUX per slice total, the
+//                                    member's shift applied afterwards; keys = masked partial sums where an earlier
+//                                    member's length falls into the slice.
+//                                M5  (first half) member r is compared EXACTLY with member r - 1 on the way, slot against
+//                                    slot: a difference marks the link r-1 -> r broken.  Every token is loaded from DRAM
+//                                    once.
+//   K3  merge_select_kernel      M2  (end) one CTA per group: exclusive prefix of each member's slice totals -> final keys
+//                                M3  segmented radix sort of the group's (hash, length) keys by a 32-bit digest: one MSD
+//                                    pass on the top 11 bits in shared memory (<= 2048 keys), 4 LSD passes through global
+//                                    memory above that
+//                                M4  per timeline: its equal-key run gives the hash-equal extenders; survivor flag,
+//                                    Algorithm-1 owner (latest extender), under LONGEST the longest surviving extender
+//                                M5  (second half) a candidate is ACCEPTED only if an unbroken chain of verified links
+//                                    leads to it (prefix-of is transitive) or after an exact warp-cooperative token
+//                                    comparison; a hash-equal candidate that fails is skipped
+//                                    (AJT_STATUS_HASH_COLLISION, informational).  Results are exact whatever the hash
+//                                    does (AJT_MERGE_WEAK_HASH degrades it to 4 bits to test this).  Then per survivor:
+//                                    its member list and its SEGMENTS (maximal runs of positions with one source of mask /
+//                                    log-prob), warp-cooperatively.
+//   K4  merge_compact_kernel     M6  one CTA scans the timelines once: survivors in original order -> merged_offsets /
+//                                    origin / traj, owner, first segment of every merged sequence
+//   K5  merge_plan_kernel        M7  segments rebased to output positions (one 32-byte record each), and for every tile
+//                                    of 512 OUTPUT positions the first segment that touches it
+//   K6  merge_scatter_kernel     M7  warp per output tile: bulk async copies of the tile's source pieces into shared
+//                                    memory, then 16-byte stores of tokens / old_logp / src / mask straight from registers
+//                                    -- whatever the alignment of the sources
 #include "ajt_common.cuh"
 #include "../../include/ajt_test.h"
 
