@@ -662,6 +662,116 @@ __global__ void __launch_bounds__(256) loss_rows_generic(const LossParams p) {
 
 // ------------------------------------------------------------------------------------------------ K8
 
+// fp32 logits with V <= 2048 (configs[0]): ONE read of every unmasked row.  A warp per row; lane l keeps vectors l + 32 j
+// (j < NV = ceil(V / 128)) of the row in registers as float4, so the maximum, the sum of exponentials (kept in place of the
+// logits) and the gradient all come from the same 16-byte loads, and dlogits leave as 8-byte stores (256 contiguous bytes per
+// instruction).  Same per-row outputs as loss_rows_generic (by_row layout for the final kernel).
+template <int NV>
+__global__ void __launch_bounds__(256) loss_rows_f32_regs(const LossParams p) {
+    pdl_wait();
+    const int lane = threadIdx.x & 31;
+    const int64_t wglobal = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    const float* logits = reinterpret_cast<const float*>(p.logits);
+    __nv_bfloat16* dlogits = reinterpret_cast<__nv_bfloat16*>(p.dlogits);
+    const float inv_S = p.ctrl->inv_num_segs;
+    const int V = p.V, nvec = V >> 2;
+    for (int64_t row = wglobal; row < p.T; row += nwarps) {
+        const bool act = p.mask[row] != 0;
+        uint2* const drow = reinterpret_cast<uint2*>(dlogits + row * p.ld);
+        if (!act) {
+#pragma unroll
+            for (int j = 0; j < NV; ++j)
+                if (lane + 32 * j < nvec) drow[lane + 32 * j] = make_uint2(0u, 0u);
+            if (lane == 0) {
+                p.row_val[row] = 0.0;
+                p.row_kl[row] = 0.0;
+                p.row_clip[row] = 0;
+                if (p.logp_out) p.logp_out[row] = 0.f;
+                if (p.ext) {
+                    p.row_k3[row] = 0.0;
+                    p.row_ent[row] = 0.0;
+                    if (p.k3_out) p.k3_out[row] = 0.f;
+                    if (p.ent_out) p.ent_out[row] = 0.f;
+                }
+            }
+            continue;
+        }
+        const float4* const zrow = reinterpret_cast<const float4*>(logits + row * p.ld);
+        float4 x[NV];
+#pragma unroll
+        for (int j = 0; j < NV; ++j)
+            x[j] = lane + 32 * j < nvec ? __ldg(zrow + lane + 32 * j) : make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
+        const float ref = p.ext && p.ref_logp ? p.ref_logp[row] : 0.f;
+        const int y = p.targets[row], sg = p.seg_ids[row];
+        const float old = p.old_logp[row], A = p.adv[row];
+        const bool ybad = (unsigned)y >= (unsigned)V, sbad = (unsigned)sg >= (unsigned)p.S;
+        const float denom = sbad ? 0.f : (p.seg_denom ? p.seg_denom[sg] : (float)p.seg_cnt[sg]);
+        const float w = (denom > 0.f && !ybad) ? inv_S / denom : 0.f;
+        float m = -INFINITY;
+#pragma unroll
+        for (int j = 0; j < NV; ++j) m = fmaxf(m, fmaxf(fmaxf(x[j].x, x[j].y), fmaxf(x[j].z, x[j].w)));
+        m = warp_max(m);
+        // the target's logit sits in exactly one lane's registers
+        float zy = 0.f;
+#pragma unroll
+        for (int j = 0; j < NV; ++j) {
+            const int v0 = 4 * (lane + 32 * j);
+            if (!ybad && y >= v0 && y < v0 + 4) zy = y == v0 ? x[j].x : y == v0 + 1 ? x[j].y : y == v0 + 2 ? x[j].z : x[j].w;
+        }
+        zy = warp_sum(zy);
+        float s = 0.f, u = 0.f;   // x becomes e^{z - m}; u = sum e^{z-m} (z-m): entropy of the row (extended form)
+#pragma unroll
+        for (int j = 0; j < NV; ++j) {
+            float* f = reinterpret_cast<float*>(&x[j]);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float t = f[i] - m;
+                const float e = ex2(t * kLog2e);   // padding lanes: e^{-inf} = 0
+                s += e;
+                if (p.ext && e > 0.f) u = fmaf(e, t, u);
+                f[i] = e;
+            }
+        }
+        s = warp_sum(s);
+        u = warp_sum(u);
+        const TokScalars ts = token_scalars(m, s, zy, old, A, w, p.eps_lo, p.eps_hi, p.grad_scale,
+                                            p.ext && p.ref_logp != nullptr && p.kl_coef != 0.f, ref, p.kl_coef, p.ext ? p.clip_c : 0.f);
+        if (lane == 0) {
+            p.row_val[row] = ts.wl;
+            p.row_kl[row] = ts.wkl;
+            p.row_clip[row] = (uint8_t)(w > 0.f ? ts.clip : 0);
+            if (p.logp_out) p.logp_out[row] = ybad ? 0.f : ts.logp;
+            if (ybad) atomicOr(&p.ctrl->status, (uint32_t)AJT_STATUS_BAD_TARGET);
+            if (p.ext) {
+                const float H = ybad ? 0.f : ts.logS - u / s;
+                p.row_k3[row] = ts.wk3;
+                p.row_ent[row] = (double)w * (double)H;
+                if (p.k3_out) p.k3_out[row] = ybad ? 0.f : ts.k3;
+                if (p.ent_out) p.ent_out[row] = H;
+            }
+        }
+        const float g = ts.g;
+        if (g != 0.f) {
+            const float coef = -g * ex2((m - ts.lse) * kLog2e);   // p_v = e^{z_v - m} e^{m - lse}
+#pragma unroll
+            for (int j = 0; j < NV; ++j) {
+                if (lane + 32 * j >= nvec) continue;
+                const int v0 = 4 * (lane + 32 * j);
+                float d0 = coef * x[j].x, d1 = coef * x[j].y, d2 = coef * x[j].z, d3 = coef * x[j].w;
+                if (y == v0) d0 += g;
+                if (y == v0 + 1) d1 += g;
+                if (y == v0 + 2) d2 += g;
+                if (y == v0 + 3) d3 += g;
+                drow[lane + 32 * j] = make_uint2(pack_bf16x2(d0, d1), pack_bf16x2(d2, d3));
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < NV; ++j)
+                if (lane + 32 * j < nvec) drow[lane + 32 * j] = make_uint2(0u, 0u);
+        }
+    }
+}
+
 // Fixed-order fp64 reduction: thread i sums elements i, i+1024, ...; then a shared-memory tree.
 __global__ void __launch_bounds__(1024) loss_final_kernel(const LossParams p, int by_row) {
     pdl_wait();
@@ -878,7 +988,12 @@ int loss_call(const void* logits, const int32_t* targets, const float* old_logp,
     else if (T > 0) {
         by_row = 1;
         const int grid = num_sms * 8;
-        if (logits_dtype == AJT_DT_F32) {
+        const bool f32_regs = logits_dtype == AJT_DT_F32 && V <= 2048 && (V % 4) == 0 && (ld_logits % 4) == 0 &&
+                              ((uintptr_t)logits & 15) == 0 && ((uintptr_t)dlogits & 7) == 0;
+        if (f32_regs) {
+            e = V <= 1024 ? launch_dependent(loss_rows_f32_regs<8>, grid, 256, 0, stream, 1, p)
+                          : launch_dependent(loss_rows_f32_regs<16>, grid, 256, 0, stream, 1, p);
+        } else if (logits_dtype == AJT_DT_F32) {
             if (V <= 2048) e = launch_dependent(loss_rows_generic<float, 32>, grid, 256, 0, stream, 1, p);
             else e = launch_dependent(loss_rows_generic<float, 256>, grid, 256, 0, stream, 1, p);
         } else {

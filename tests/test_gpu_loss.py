@@ -58,7 +58,11 @@ def test_fast_path_bf16(T, V, S, rho):
 
 
 @pytest.mark.parametrize("T,V,S,rho,dtype", [
-    (3000, 1024, 32, 0.45, torch.float32),    # config c1's shape: fp32 logits, V=1024 (warp-per-row generic)
+    (3000, 1024, 32, 0.45, torch.float32),    # config c1's shape: fp32 logits, V=1024: the one-read register kernel, 8 vectors per lane
+    (700, 2048, 8, 0.6, torch.float32),       # fp32 one-read kernel, 16 vectors per lane (its largest V)
+    (500, 1000, 4, 0.5, torch.float32),       # fp32 one-read kernel, V not a multiple of 128: lanes without a vector
+    (300, 36, 3, 0.7, torch.float32),         # fp32 one-read kernel, fewer vectors than lanes
+    (300, 1002, 4, 0.7, torch.float32),       # fp32, V % 4 != 0 -> generic, warp per row
     (300, 5000, 4, 0.7, torch.float32),       # fp32, CTA-per-row generic
     (300, 1001, 4, 0.7, torch.bfloat16),      # odd V -> generic, warp per row
     (200, 151937, 4, 0.7, torch.bfloat16),    # odd V -> generic, CTA per row
@@ -87,6 +91,8 @@ def test_row_stride_and_inplace():
     run_and_check(300, 32000, 4, 0.7, torch.bfloat16, ld=32000 + 64)
     run_and_check(300, 151936, 4, 0.7, torch.bfloat16, inplace=True)
     run_and_check(200, 1001, 4, 0.7, torch.bfloat16, ld=1010)
+    run_and_check(200, 1024, 4, 0.7, torch.float32, ld=1040, sigma=2.0)   # fp32 one-read kernel with a row stride
+    run_and_check(200, 1024, 4, 0.7, torch.float32, ld=1026, sigma=2.0)   # stride not a multiple of 4: generic kernel
 
 
 def test_padding_columns_untouched():
@@ -122,6 +128,12 @@ def test_bad_target_and_segment_set_status():
     s2 = seg.clone(); s2[7] = -1
     out = ajt.policy_loss_fwd_bwd(logits, targets, old, adv, mask, s2, lv.S, 0.2, 0.2)
     assert ajt.last_status(out.workspace) & ajt.STATUS_BAD_SEG
+    # the fp32 one-read kernel reports them too, and the bad row contributes nothing
+    lv, logits, targets, old, adv, mask, seg = make_case(64, 1024, 4, 1.0, torch.float32, 2.0, 12)
+    t2 = targets.clone(); t2[5] = 1024
+    out = ajt.policy_loss_fwd_bwd(logits, t2, old, adv, mask, seg, lv.S, 0.2, 0.2)
+    assert ajt.last_status(out.workspace) & ajt.STATUS_BAD_TARGET
+    assert torch.all(out.dlogits[5] == 0)
 
 
 def test_chunked_equals_unchunked():

@@ -92,7 +92,9 @@ def test_ext_fast_path(T, V, S, rho):
 
 
 @pytest.mark.parametrize("T,V,S,rho,dtype", [
-    (3000, 1024, 32, 0.45, torch.float32),    # c1's shape: fp32 logits, warp-per-row generic
+    (3000, 1024, 32, 0.45, torch.float32),    # c1's shape: fp32 logits, one-read register kernel
+    (500, 2048, 6, 0.6, torch.float32),       # one-read register kernel, 16 vectors per lane
+    (300, 1002, 4, 0.7, torch.float32),       # fp32 generic, warp per row
     (300, 5000, 4, 0.7, torch.float32),       # fp32, CTA-per-row generic
     (200, 151937, 4, 0.7, torch.bfloat16),    # odd V -> generic
 ])
