@@ -306,6 +306,26 @@ int ajt_lm_head_logp(const void* hidden, const void* weight, const int32_t* targ
                      float* lse_out /* or NULL */, uint32_t flags /* AJT_LM_* */, void* workspace, size_t workspace_bytes,
                      ajt_stream_t stream);
 
+/* ajt_policy_loss_fwd_bwd for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same computation, the same kernels and the same results as ajt_policy_loss_fwd_bwd
+ * (BASELINE.json north_star; DESIGN.md "O-L" steps 1-7), but the call's scratch lives in a file-scope
+ * device array of the library instead of a caller-provided workspace.  The call allocates nothing (no cudaMalloc / cudaFree,
+ * no allocating library routine).  Inputs and outputs are the caller's, exactly as for ajt_policy_loss_fwd_bwd.
+ *   Limit: the scratch is ajt_loss_static_scratch_bytes() = 4 MiB per GPU (held by every GPU that loads the library until
+ *   the process exits); a call needs ajt_loss_workspace_bytes(T, V, S) bytes of it (69 bytes per row + 4 S + ~1 KB: e.g.
+ *   T = 40,960 rows with S = 4,096).  Larger calls return AJT_ERR_CAPACITY and launch nothing: use the workspace call.
+ *   Sharing: every call on a device uses the same array, which keeps the previous call's contents; the call clears what must
+ *   start at zero on `stream`.  Two such calls that overlap on one GPU (different streams, no dependency) RACE: order them.
+ *   status_out: DEVICE [1] or NULL: the call's AJT_STATUS_* word, copied on `stream` (there is no workspace to pass to
+ *   ajt_last_status).  Enqueues on `stream`, does not synchronise. */
+size_t ajt_loss_static_scratch_bytes(void);
+
+int ajt_policy_loss_fwd_bwd_static(const void* logits, const int32_t* targets, const float* old_logp, const float* adv,
+                                   const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T, int32_t V,
+                                   int32_t S, int64_t ld_logits, int32_t logits_dtype, const float* seg_denom, float inv_num_segs,
+                                   float grad_scale, void* dlogits, float* loss_out, float* logp_out /* or NULL */,
+                                   float* stats_out /* or NULL */, uint32_t* status_out /* or NULL */, ajt_stream_t stream);
+
 /* The policy loss straight from the hidden states, forward AND backward ("policy gradient ... loss terms
  * are computed"): with z_t = W h_t and steps 1-6 of ajt_policy_loss_fwd_bwd on z,
  *   loss = sum_t w_t L_t;   dZ_tv = g_t (1[v = y_t] - exp(z_tv - lse_t));   dH = dZ W  [T, d] bf16;   dW (+)= dZ^T H  [V, d] fp32

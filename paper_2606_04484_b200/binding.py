@@ -29,6 +29,7 @@ _EXPORTS = [
     "ajt_pack_loss_inputs", "ajt_pack_microbatches", "ajt_lm_head_workspace_bytes", "ajt_lm_head_bwd_workspace_bytes",
     "ajt_lm_head_loss_bwd", "ajt_lm_head_logp",
     "ajt_hbm_probe", "ajt_launch_count", "ajt_host_ctx_create", "ajt_host_ctx_destroy", "ajt_policy_loss_fwd_bwd_host2",
+    "ajt_loss_static_scratch_bytes", "ajt_policy_loss_fwd_bwd_static",
 ]
 
 _lib = None
@@ -450,6 +451,52 @@ def policy_loss_fwd_bwd(logits: torch.Tensor, targets: torch.Tensor, old_logp: t
     if rc != 0:
         raise AjtError(rc, "ajt_policy_loss_fwd_bwd")
     return out
+
+
+def loss_static_scratch_bytes() -> int:
+    L = lib()
+    L.ajt_loss_static_scratch_bytes.restype = C.c_size_t
+    return int(L.ajt_loss_static_scratch_bytes())
+
+
+def policy_loss_fwd_bwd_static(logits: torch.Tensor, targets: torch.Tensor, old_logp: torch.Tensor, adv: torch.Tensor,
+                               mask: torch.Tensor, seg_ids: torch.Tensor, S: int, eps_lo: float, eps_hi: float,
+                               dlogits: torch.Tensor, loss: torch.Tensor, logp: Optional[torch.Tensor] = None,
+                               stats: Optional[torch.Tensor] = None, status: Optional[torch.Tensor] = None,
+                               seg_denom: Optional[torch.Tensor] = None, inv_num_segs: float = 0.0, grad_scale: float = 1.0,
+                               V: Optional[int] = None, stream=None) -> None:
+    """ajt_policy_loss_fwd_bwd_static (include/ajt.h): the loss call with its scratch in the library's static device array.
+    Allocates nothing: every output tensor is the caller's."""
+    _require_cuda()
+    if logits.dim() != 2 or not logits.is_cuda or logits.stride(1) != 1:
+        raise TypeError("logits: expected a 2-D CUDA tensor with unit column stride")
+    if logits.dtype == torch.bfloat16:
+        dt = DT_BF16
+    elif logits.dtype == torch.float32:
+        dt = DT_F32
+    else:
+        raise TypeError("logits: bf16 or f32 only")
+    T, ld = int(logits.shape[0]), int(logits.stride(0)) if logits.shape[0] > 1 else int(logits.shape[1])
+    V = int(logits.shape[1]) if V is None else int(V)
+    _check_dev(targets, torch.int32, "targets")
+    _check_dev(old_logp, torch.float32, "old_logp")
+    _check_dev(adv, torch.float32, "adv")
+    _check_dev(mask, torch.uint8, "mask")
+    _check_dev(seg_ids, torch.int32, "seg_ids")
+    _check_dev(seg_denom, torch.float32, "seg_denom")
+    _check_dev(loss, torch.float32, "loss")
+    _check_dev(logp, torch.float32, "logp")
+    _check_dev(stats, torch.float32, "stats")
+    _check_dev(status, torch.int32, "status")
+    if dlogits.dtype != torch.bfloat16 or not dlogits.is_cuda:
+        raise TypeError("dlogits: expected a CUDA bf16 tensor")
+    rc = lib().ajt_policy_loss_fwd_bwd_static(
+        _dp(logits), _dp(targets), _dp(old_logp), _dp(adv), _dp(mask), _dp(seg_ids),
+        C.c_float(eps_lo), C.c_float(eps_hi), C.c_int64(T), C.c_int32(V), C.c_int32(S), C.c_int64(ld), C.c_int32(dt),
+        _dp(seg_denom), C.c_float(inv_num_segs), C.c_float(grad_scale), _dp(dlogits), _dp(loss), _dp(logp), _dp(stats),
+        _dp(status), _stream(stream))
+    if rc != 0:
+        raise AjtError(rc, "ajt_policy_loss_fwd_bwd_static")
 
 
 def policy_loss_fwd_bwd_ext(logits: torch.Tensor, targets: torch.Tensor, old_logp: torch.Tensor, adv: torch.Tensor,

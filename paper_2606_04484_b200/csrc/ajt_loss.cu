@@ -15,6 +15,8 @@
 //   K8  loss_final_kernel  fixed-order fp64 reduction of the per-row terms -> loss, stats      [L4]
 #include <math.h>
 
+#include <mutex>
+
 #include "ajt_common.cuh"
 #include "ajt_token.cuh"
 
@@ -1027,6 +1029,55 @@ extern "C" int ajt_policy_loss_fwd_bwd_ext(const void* logits, const int32_t* ta
     const LossExt x = {1, ref_logp, kl_coef, k3_out, ent_out, ext_out, clip_c};
     return loss_call(logits, targets, old_logp, adv, mask, seg_ids, eps_lo, eps_hi, T, V, S, ld_logits, logits_dtype, seg_denom,
                      inv_num_segs, grad_scale, dlogits, loss_out, logp_out, stats_out, x, workspace, workspace_bytes, stream);
+}
+
+// ---- the loss call for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+// cudaMalloc): the same kernels with their scratch in a file-scope device array instead of a caller-provided workspace.
+// Every GPU that loads the library holds the array until exit.  Host code never passes the symbol itself to a kernel (in host
+// code its name is a host-side stand-in, not a device address): its device address is looked up once per device with
+// cudaGetSymbolAddress, that device being current.  The array keeps the last call's contents; what must start at zero (control
+// block, tile states, per-segment counts) is cleared by loss_call's memset on the caller's stream as in every loss call.
+constexpr size_t kStaticWsBytes = (size_t)4 << 20;   // 4 MiB: e.g. T = 40,960 rows with S = 4,096 (69 bytes per row + 4 S + 768)
+static __device__ __align__(256) uint8_t g_loss_static_ws[kStaticWsBytes];
+namespace {
+constexpr int kStaticMaxDev = 64;
+void* g_static_ws_addr[kStaticMaxDev];   // device address of g_loss_static_ws on device i, once looked up
+std::mutex g_static_ws_mu;
+}  // namespace
+
+extern "C" size_t ajt_loss_static_scratch_bytes(void) { return kStaticWsBytes; }
+
+extern "C" int ajt_policy_loss_fwd_bwd_static(const void* logits, const int32_t* targets, const float* old_logp, const float* adv,
+                                              const uint8_t* mask, const int32_t* seg_ids, float eps_lo, float eps_hi, int64_t T,
+                                              int32_t V, int32_t S, int64_t ld_logits, int32_t logits_dtype,
+                                              const float* seg_denom, float inv_num_segs, float grad_scale, void* dlogits,
+                                              float* loss_out, float* logp_out, float* stats_out, uint32_t* status_out,
+                                              ajt_stream_t stream) {
+    if (T < 0 || S <= 0) return AJT_ERR_INVALID_ARG;
+    if (loss_ws_layout(T, S).total > kStaticWsBytes) return AJT_ERR_CAPACITY;   // beyond the static scratch: use the workspace call
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return AJT_ERR_CUDA;
+    if (dev < 0 || dev >= kStaticMaxDev) return AJT_ERR_UNSUPPORTED;
+    void* ws = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_static_ws_mu);
+        if (!g_static_ws_addr[dev]) {   // once per device, with that device current
+            void* a = nullptr;
+            if (cudaGetSymbolAddress(&a, g_loss_static_ws) != cudaSuccess || !a) return AJT_ERR_CUDA;
+            g_static_ws_addr[dev] = a;
+        }
+        ws = g_static_ws_addr[dev];
+    }
+    const LossExt x = {0, nullptr, 0.f, nullptr, nullptr, nullptr, 0.f};
+    const int rc = loss_call(logits, targets, old_logp, adv, mask, seg_ids, eps_lo, eps_hi, T, V, S, ld_logits, logits_dtype,
+                             seg_denom, inv_num_segs, grad_scale, dlogits, loss_out, logp_out, stats_out, x, ws, kStaticWsBytes,
+                             stream);
+    if (rc != AJT_OK) return rc;
+    if (status_out &&   // the status word is the first word of the scratch: handed to the caller on the same stream
+        cudaMemcpyAsync(status_out, ws, sizeof(uint32_t), cudaMemcpyDeviceToDevice, reinterpret_cast<cudaStream_t>(stream)) !=
+            cudaSuccess)
+        return AJT_ERR_CUDA;
+    return AJT_OK;
 }
 
 extern "C" int ajt_segment_counts(const uint8_t* mask, const int32_t* seg_ids, int64_t T, int32_t S, int32_t accumulate,
