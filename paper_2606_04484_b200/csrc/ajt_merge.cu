@@ -47,7 +47,9 @@ namespace {
 
 using namespace ajt;
 
-constexpr int kSl = 508;           // hash slice: 508 token positions; with up to 3 elements of misalignment a slice is
+constexpr int kVT = 4;              // 16-byte vectors of a hash slot per lane (8 = 4 KB slots of 1,020 positions: 127 registers,
+                                   // 2 CTAs per SM, hash pass 70 instead of 72-76 us, the merge inside the bench step unchanged)
+constexpr int kSl = 128 * kVT - 4;           // hash slice: 508 token positions; with up to 3 elements of misalignment a slice is
                                    // exactly 128 aligned 16-byte vectors = 4 per lane
 __host__ __device__ __forceinline__ int slices_of(int L) { return (L + kSl - 1) / kSl; }
 __host__ __device__ __forceinline__ int slice_at(int pos) { return pos / kSl; }
@@ -737,7 +739,7 @@ __device__ __forceinline__ void sts32(uint32_t saddr, uint32_t v) { asm volatile
 
 constexpr int kHashThreads = 256;
 constexpr int kHashStages = 3;          // the member in flight, the member at work, its predecessor
-constexpr int kSlotBytes = 2048;                                    // 128 aligned vectors: the slice + its misalignment
+constexpr int kSlotBytes = 512 * kVT;                                    // 128 aligned vectors: the slice + its misalignment
 constexpr int kStageBytes = 16 + kSlotBytes + 16;                   // a zero vector on either side (reads at e + delta, |delta| <= 3)
 constexpr int kHashWarpBytes = kHashStages * kStageBytes + 128;     // + mbarriers (padded to 64 B) + descriptors
 constexpr int kHashSmem = (kHashThreads / 32) * kHashWarpBytes + 128;
@@ -764,7 +766,7 @@ __device__ __forceinline__ uint4 lds128(uint32_t saddr) {
 // delta = D' - D without masks; when the two agree over a whole slice the slice total is inherited and nothing is
 // multiplied at all.  Slices in which a member or its predecessor ends take a masked path.  Why chunks: one warp works
 // through its members one after the other (~2 us each), so a unit of 40 members would take as long as the whole kernel.
-__global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const MergeParams p) {
+__global__ void __launch_bounds__(kHashThreads, kVT > 4 ? 2 : 3) merge_hash_kernel(const MergeParams p) {
     pdl_wait();
     extern __shared__ __align__(128) uint8_t h_dyn[];
     if (fatal(p)) return;
@@ -789,14 +791,14 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
     const int64_t N = p.N;
     const int mis = p.mis;
     // weights of this lane's vectors: slot elements e = 4 (lane + 32 t) + i weigh W^e = bt[t] W^i (Horner inside a vector)
-    uint32_t bt[4];
+    uint32_t bt[kVT];
     bt[0] = pow32(kW, 4u * (uint32_t)lane);
 #pragma unroll
-    for (int t = 1; t < 4; ++t) bt[t] = bt[t - 1] * kW128;
+    for (int t = 1; t < kVT; ++t) bt[t] = bt[t - 1] * kW128;
     auto dot = [&](const uint32_t* y) {
         uint32_t g = 0;
 #pragma unroll
-        for (int t = 0; t < 4; ++t) g += (((y[4 * t + 3] * kW + y[4 * t + 2]) * kW + y[4 * t + 1]) * kW + y[4 * t]) * bt[t];
+        for (int t = 0; t < kVT; ++t) g += (((y[4 * t + 3] * kW + y[4 * t + 2]) * kW + y[4 * t + 1]) * kW + y[4 * t]) * bt[t];
         return g;
     };
     bool dead = false;
@@ -888,12 +890,12 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
                 const int plen = min(prev_L - S0, kSl);
                 const uint32_t pslot = sbuf + pst * kStageBytes;
                 const int delta = prev_D - D;                 // position p: own element p + D, predecessor's element p + D + delta
-                uint32_t y[16];
+                uint32_t y[4 * kVT];
                 bool same = false;   // the two agree on every position of the slice below prev_L
                 if (len == kSl && (!have_prev || plen == kSl)) {
                     // ---- whole slices: no masks anywhere
 #pragma unroll
-                    for (int t = 0; t < 4; ++t) {
+                    for (int t = 0; t < kVT; ++t) {
                         const uint4 v = lds128(slot + 16 * (lane + 32 * t));
                         y[4 * t] = v.x; y[4 * t + 1] = v.y; y[4 * t + 2] = v.z; y[4 * t + 3] = v.w;
                     }
@@ -901,14 +903,14 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
                         uint32_t diff = 0;
                         if (delta == 0) {
 #pragma unroll
-                            for (int t = 0; t < 4; ++t) {
+                            for (int t = 0; t < kVT; ++t) {
                                 const uint4 z = lds128(pslot + 16 * (lane + 32 * t));
                                 diff |= (y[4 * t] ^ z.x) | (y[4 * t + 1] ^ z.y) | (y[4 * t + 2] ^ z.z) | (y[4 * t + 3] ^ z.w);
                             }
                         } else {
                             const uint32_t pa = pslot + 4 * delta + 16 * lane;
 #pragma unroll
-                            for (int t = 0; t < 4; ++t)
+                            for (int t = 0; t < kVT; ++t)
 #pragma unroll
                                 for (int i = 0; i < 4; ++i) diff |= y[4 * t + i] ^ lds32(pa + 512 * t + 4 * i);
                         }
@@ -919,7 +921,7 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
                     const int cmp = have_prev ? min(len, plen) : 0;   // positions to compare
                     uint32_t diff = 0;
 #pragma unroll
-                    for (int t = 0; t < 4; ++t)
+                    for (int t = 0; t < kVT; ++t)
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
                             const int e = 4 * (lane + 32 * t) + i, pos = e - D;
@@ -951,9 +953,9 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
                                 F = tot;   // its own last token: everything beyond is zero already
                             } else {
                                 const int rem = La - S0 + D - 4 * lane;   // slot elements 128 t + i < rem are inside the prefix
-                                uint32_t z[16];
+                                uint32_t z[4 * kVT];
 #pragma unroll
-                                for (int j = 0; j < 16; ++j) z[j] = 128 * (j >> 2) + (j & 3) < rem ? y[j] : 0u;
+                                for (int j = 0; j < 4 * kVT; ++j) z[j] = 128 * (j >> 2) + (j & 3) < rem ? y[j] : 0u;
                                 F = __reduce_add_sync(0xffffffffu, dot(z)) * fD;
                             }
                             if (lane == a) Fk = F;
@@ -970,9 +972,9 @@ __global__ void __launch_bounds__(kHashThreads, 3) merge_hash_kernel(const Merge
                         for (unsigned m = __ballot_sync(0xffffffffu, hit); m; m &= m - 1) {
                             const int a1 = __ffs(m) - 1;
                             const int rem = __shfl_sync(0xffffffffu, La, a1) - S0 + D - 4 * lane;
-                            uint32_t z[16];
+                            uint32_t z[4 * kVT];
 #pragma unroll
-                            for (int j = 0; j < 16; ++j) z[j] = 128 * (j >> 2) + (j & 3) < rem ? y[j] : 0u;
+                            for (int j = 0; j < 4 * kVT; ++j) z[j] = 128 * (j >> 2) + (j & 3) < rem ? y[j] : 0u;
                             const uint32_t F = __reduce_add_sync(0xffffffffu, dot(z)) * fD;
                             if (lane == b) my_keys[a0r + a1] = F;
                         }
@@ -1986,7 +1988,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     const int plan_grid = (int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8);
     const int64_t uwant = ((int64_t)n + 255) / 256;
     if (launch_dependent(merge_units_kernel, (int)(uwant < (int64_t)num_sms * 4 ? uwant : (int64_t)num_sms * 4), 256, 0, stream, 1, p) != cudaSuccess ||
-        launch_dependent(merge_hash_kernel, num_sms * 3, kHashThreads, kHashSmem, stream, 1, p) != cudaSuccess ||
+        launch_dependent(merge_hash_kernel, num_sms * (kVT > 4 ? 2 : 3), kHashThreads, kHashSmem, stream, 1, p) != cudaSuccess ||
         launch_dependent(merge_select_kernel, num_sms * 4, kSelThreads, sizeof(SelectStage), stream, 1, p) != cudaSuccess ||
         launch_dependent(merge_compact_kernel, 1, 1024, kCompactSmem, stream, 1, p) != cudaSuccess ||
         launch_dependent(merge_plan_kernel, plan_grid, 256, 0, stream, 1, p) != cudaSuccess ||
