@@ -137,6 +137,20 @@ def seg_advantages(W, name: str, seed: int, S: int) -> np.ndarray:
     return W.advantages_group_zscore(seed, CFG_INDEX[name], S).astype(np.float32)
 
 
+def loss_traffic(T: int, Vv: int):
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE loss rows-kernel launch at shape [T, Vv], from the
+    committed ncu --set full captures (profiles/r02_traffic.csv; the commands are in profiles/r02_README.md), or None."""
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "r02_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["kernel"].startswith("loss_rows") and row["shape"] == f"{T}x{Vv}":
+                    return float(row["dram_bytes_per_launch"]), row["note"]
+    except Exception:
+        pass
+    return None, None
+
+
 def fracs(gbs: float, peak: float) -> dict:
     return {"gb_per_s": gbs, "frac_of_measured": gbs / peak, "frac_of_nominal_8tbs": gbs / NOMINAL_HBM_GBS}
 
@@ -375,15 +389,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
 
     if rank == 0:
         shape_key = f"loss_rows_kernel[{T}x{V},rho={rho:.2f}]"
-        traffic, traffic_note = None, None
-        try:   # DRAM bytes of one rows-kernel launch at this shape, from the committed ncu --set full capture
-            import csv
-            with open(os.path.join(ROOT, "profiles", "r02_traffic.csv")) as f:
-                for row in csv.DictReader(f):
-                    if row["kernel"] == "loss_rows_kernel" and row["shape"] == f"{T}x{V}":
-                        traffic, traffic_note = float(row["dram_bytes_per_launch"]), row["note"]
-        except Exception:
-            traffic = None
+        traffic, traffic_note = loss_traffic(T, V)
         ach = loss_b / (loss_ms * 1e-3) / 1e9
         mg = b_merge / (merge_ms * 1e-3) / 1e9
         line = {
@@ -575,7 +581,7 @@ def run_config_records(torch, ajt, W, B3, ch3, logits_big, dlogits_big, dev, str
         b = loss_bytes(T, Vv, nu, b_in)
         return {"T": T, "V": Vv, "dtype": "bf16" if b_in == 2 else "f32", "mask_density": nu / max(1, T), "ms": ms,
                 "algorithmic_bytes": b, **{("logits_" + k if k == "gb_per_s" else k): v for k, v in fracs(b / ms / 1e6, peak).items()},
-                "l2": "cold" if cold else "larger than L2"}
+                "l2": "cold" if cold else "larger than L2", "traffic": loss_traffic(T, Vv)[0]}
 
     def merge_rec(Bx, ms=None):
         cold = 4 * Bx.N_in * 2 < L2
@@ -595,7 +601,7 @@ def run_config_records(torch, ajt, W, B3, ch3, logits_big, dlogits_big, dev, str
                            "algorithmic_bytes": loss_bytes(head["T"], V, ch3["n_unmasked"]),
                            **{("logits_" + k if k == "gb_per_s" else k): v
                               for k, v in fracs(loss_bytes(head["T"], V, ch3["n_unmasked"]) / head["loss_ms"] / 1e6, peak).items()},
-                           "l2": "larger than L2"}}
+                           "l2": "larger than L2", "traffic": loss_traffic(head["T"], V)[0]}}
     for name in ("c1", "c2", "c4A", "c4B"):
         seed = W.BASE_SEED + CFG_INDEX[name]
         Bx = Batch(torch, ajt, W, name, merge_inputs(W, name, seed), seed, dev, stream)
