@@ -1554,12 +1554,12 @@ __global__ void __launch_bounds__(256) merge_plan_kernel(const MergeParams p) {
     if (fatal(p)) return;
     const int lane = threadIdx.x & 31;
     const int wglobal = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
-    const int M = p.ctrl->M, ntiles = p.ctrl->n_tiles;
+    const int M = p.ctrl->M;
     const int64_t N_out = p.ctrl->N_out;
     for (int m = wglobal; m < M; m += nwarps) {
         const int s = __ldg(p.merged_origin + m);
         const int4 sr = __ldg(p.sv_rec + s);
-        const int64_t mo = __ldg(p.merged_offsets + m), so = __ldg(p.offsets + s);
+        const int64_t mo = __ldg(p.merged_offsets + m), mo1 = __ldg(p.merged_offsets + m + 1), so = __ldg(p.offsets + s);
         const int gb = __ldg(p.gseg_base + m);
         for (int li = lane; li < sr.w; li += 32) {
             const int2 rs = __ldg(p.rseg + sr.z + li);
@@ -1573,28 +1573,23 @@ __global__ void __launch_bounds__(256) merge_plan_kernel(const MergeParams p) {
             else o.lp_delta = 0;
             p.gseg[gb + li] = o;
         }
+        // the tiles whose first position lies in this sequence: a lane each; the last relative segment that starts at or
+        // before it (the sequence's segment list was read a moment ago: these searches hit L1)
+        const int64_t t0 = (mo + kTS - 1) >> kTSLog, t1 = (mo1 + kTS - 1) >> kTSLog;   // tiles t0 .. t1 - 1 start in [mo, mo1)
+        for (int64_t t = t0 + lane; t < t1; t += 32) {
+            const int64_t pr = (t << kTSLog) - mo;
+            int a = 0, b = sr.w - 1;
+            while (a < b) {
+                const int mid = (a + b + 1) >> 1;
+                if ((int64_t)__ldg(p.rseg + sr.z + mid).x <= pr) a = mid; else b = mid - 1;
+            }
+            p.tile_seg[t] = gb + a;
+        }
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         GSeg o;
         o.out_start = N_out; o.tok_delta = 0; o.lp_delta = 0; o.src = kSrcNone; o.aux = 0;
         p.gseg[p.ctrl->n_gsegs] = o;
-    }
-    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < ntiles; t += gridDim.x * blockDim.x) {
-        const int64_t d = (int64_t)t << kTSLog;
-        int lo = 0, hi = M - 1;   // last merged sequence that starts at or before d
-        while (lo < hi) {
-            const int mid = (lo + hi + 1) >> 1;
-            if (__ldg(p.merged_offsets + mid) <= d) lo = mid; else hi = mid - 1;
-        }
-        const int s = __ldg(p.merged_origin + lo);
-        const int4 sr = __ldg(p.sv_rec + s);
-        const int64_t pr = d - __ldg(p.merged_offsets + lo);
-        int a = 0, b = sr.w - 1;   // last relative segment that starts at or before pr
-        while (a < b) {
-            const int mid = (a + b + 1) >> 1;
-            if ((int64_t)__ldg(p.rseg + sr.z + mid).x <= pr) a = mid; else b = mid - 1;
-        }
-        p.tile_seg[t] = __ldg(p.gseg_base + lo) + a;
     }
 }
 
@@ -1984,7 +1979,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     if (n <= kGrpSmemN) AJT_LAUNCH(merge_group_fast_kernel<<<1, 1024, group_fast_smem(n), stream>>>(p, n + n / 8 + 16));
     else AJT_LAUNCH(merge_group_radix_kernel<<<1, 1024, 0, stream>>>(p));
     // kernels 2..6 are launched as programmatic dependents: resident and waiting when their predecessor ends
-    const int64_t want = ((n_tokens >> kTSLog) + 1 + 255) / 256 + ((int64_t)n * 32 + 255) / 256;
+    const int64_t want = ((int64_t)n * 32 + 255) / 256;   // a warp per merged sequence (at most n)
     const int plan_grid = (int)(want < (int64_t)num_sms * 8 ? (want < 1 ? 1 : want) : (int64_t)num_sms * 8);
     const int64_t uwant = ((int64_t)n + 255) / 256;
     if (launch_dependent(merge_units_kernel, (int)(uwant < (int64_t)num_sms * 4 ? uwant : (int64_t)num_sms * 4), 256, 0, stream, 1, p) != cudaSuccess ||
