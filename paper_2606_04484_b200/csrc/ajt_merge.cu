@@ -135,6 +135,7 @@ struct MergeParams {
     int32_t E_cap;
     int32_t slice_cap;
     int32_t mis;           // (address of tokens / 4) mod 4: element misalignment of the token array vs 16 bytes
+    int32_t slim;          // the group kernel left {timeline | group << 16, first slice} in sel_q: the units kernel writes the records
 };
 
 struct MergeWs {
@@ -524,17 +525,12 @@ __global__ void __launch_bounds__(1024) merge_group_fast_kernel(const MergeParam
             return B1[g + 1] - B1[g] < 2 ? 0u : (uint32_t)slices_of((int)(B3[i + 1] - B3[i]));
         },
         [&](int pos, int64_t ex, int64_t) { B9[pos] = (uint32_t)ex; }, s_w);
-    // ---- records by sorted position: coalesced stores.  A lone SM cannot afford 7,862 scattered 8-byte loads (one sector
-    // each, ~15 us), so the token offsets come from the 32-bit copies kept since the first phase whenever N < 2^32.
-    const bool off32 = p.N < ((int64_t)1 << 32);
+    // ---- by sorted position: {timeline | group << 16, first hash slice}, 8 bytes.  One SM stores slowly (the full 37-byte
+    // records cost 8 us here), so merge_units_kernel expands these into tl_rec / perm / glen / goff / lbad over the whole GPU.
 #pragma unroll 2
     for (int pos = tid; pos < n; pos += 1024) {
-        const uint32_t i = B8[pos], g = B6[i], gs = B1[g], r = (uint32_t)pos - gs;
-        p.tl_rec[pos] = make_int4((int)B9[pos], (int)gs, (int)(B1[g + 1] - gs), (int)(B4[g] + r * (r + 1) / 2u));
-        p.perm[pos] = (int32_t)i;
-        p.glen[pos] = (int32_t)(B3[i + 1] - B3[i]);
-        p.goff[pos] = off32 ? (int64_t)B3[i] : __ldg(p.offsets + i);
-        p.lbad[pos] = 0;
+        const uint32_t i = B8[pos], g = B6[i];
+        p.sel_q[pos] = make_int2((int)(i | (g << 16)), (int)B9[pos]);   // n <= 7936 < 2^13: both fit 16 bits
     }
 #pragma unroll 1
     for (int g = tid; g <= G; g += 1024)
@@ -656,15 +652,49 @@ __global__ void __launch_bounds__(256) merge_units_kernel(const MergeParams p) {
     const int npad = (n + 31) & ~31;
     for (int pos = blockIdx.x * blockDim.x + threadIdx.x; pos < npad; pos += gridDim.x * blockDim.x) {
         int4 t = make_int4(0, 0, 0, 0);
-        if (pos < n) t = __ldg(p.tl_rec + pos);
-        const int gs = t.y, k = t.z, r = pos - gs;
-        const bool open = pos < n && k >= 2 && r % kChunk == 0;
         int cnt = 0;
-        if (open) {
+        bool open = false;
+        if (p.slim) {
+            // expand the group kernel's slim record into the per-position records, and take the lengths from the offsets
+            int2 sr = make_int2(0, 0);
+            int4 gr = make_int4(0, 0, 0, 0);
+            if (pos < n) {
+                sr = __ldg(p.sel_q + pos);
+                gr = __ldg(p.grp_rec + ((uint32_t)sr.x >> 16));   // {group start, members, first key slot}
+            }
+            const int i = sr.x & 0xffff, gs = gr.x, k = gr.y, r = pos - gs;
+            open = pos < n && k >= 2 && r % kChunk == 0;
+            int64_t o0 = 0, o1 = 0;
+            if (pos < n) { o0 = __ldg(p.offsets + i); o1 = __ldg(p.offsets + i + 1); }
             int mx = 0;
-            for (int x = 0; x < min(kChunk, k - r); ++x) mx = max(mx, __ldg(p.glen + pos + x));
-            cnt = slices_of(mx);
+            if (open) {   // the chunk's other members: their lengths straight from the offsets (their records are being written now)
+                int ix[kChunk];
+#pragma unroll
+                for (int x = 1; x < kChunk; ++x) ix[x] = x < k - r ? (__ldg(p.sel_q + pos + x).x & 0xffff) : -1;
+#pragma unroll
+                for (int x = 1; x < kChunk; ++x)
+                    if (ix[x] >= 0) mx = max(mx, (int)(__ldg(p.offsets + ix[x] + 1) - __ldg(p.offsets + ix[x])));
+            }
+            if (pos < n) {
+                t = make_int4(sr.y, gs, k, gr.z + (int)((uint32_t)r * (uint32_t)(r + 1) / 2u));
+                p.tl_rec[pos] = t;
+                p.perm[pos] = i;
+                p.glen[pos] = (int32_t)(o1 - o0);
+                p.goff[pos] = o0;
+                p.lbad[pos] = 0;
+            }
+            if (open) cnt = slices_of(max(mx, (int)(o1 - o0)));
+        } else {
+            if (pos < n) t = __ldg(p.tl_rec + pos);
+            const int k = t.z, r = pos - t.y;
+            open = pos < n && k >= 2 && r % kChunk == 0;
+            if (open) {
+                int mx = 0;
+                for (int x = 0; x < min(kChunk, k - r); ++x) mx = max(mx, __ldg(p.glen + pos + x));
+                cnt = slices_of(mx);
+            }
         }
+        const int gs = t.y, k = t.z, r = pos - gs;
         if (!__any_sync(0xffffffffu, open)) continue;
         int inc = cnt;   // inclusive scan of the unit counts over the warp
 #pragma unroll
@@ -1969,6 +1999,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     if (sc > (int64_t)INT32_MAX) return AJT_ERR_UNSUPPORTED;
     p.slice_cap = (int32_t)sc;
     p.mis = (int32_t)(((uintptr_t)tokens >> 2) & 3);
+    p.slim = n <= kGrpSmemN ? 1 : 0;
 
     if (n == 0) {
         if (cudaMemsetAsync(p.ctrl, 0, sizeof(AjtCtrl), stream) != cudaSuccess) return AJT_ERR_CUDA;
