@@ -1150,7 +1150,7 @@ __device__ __noinline__ int build_segments(bool explicit_masks, const int32_t* m
 // sectors per cycle, so every global access is coalesced (lane = consecutive timeline) and issued 8 deep, and the scan --
 // which wants 8 CONSECUTIVE timelines per thread -- runs on a copy in shared memory.  Two round trips in all.
 constexpr int kCompactChunk = 8192;
-constexpr int kCompactSmem = kCompactChunk * 16 + kCompactChunk * 4;
+constexpr int kCompactSmem = kCompactChunk * 16;
 __global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p) {
     pdl_wait();
     extern __shared__ __align__(16) uint8_t c_dyn[];
@@ -1160,8 +1160,6 @@ __global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = p.n;
     uint2* const prA = reinterpret_cast<uint2*>(c_dyn);                         // in: {survivor << 24 | segments, length}; out: {merged index, first segment}
     int64_t* const prB = reinterpret_cast<int64_t*>(c_dyn + kCompactChunk * 8);  // out: merged offset
-    int32_t* const smidx = reinterpret_cast<int32_t*>(c_dyn + kCompactChunk * 16);   // merged index by timeline (n <= chunk)
-    const bool one = n <= kCompactChunk;
     int64_t base_a = 0, base_b = 0;   // {survivors << 32 | segments}, tokens, before this chunk
     for (int c0 = 0; c0 < n; c0 += kCompactChunk) {
         const int cn = min(kCompactChunk, n - c0);
@@ -1235,23 +1233,12 @@ __global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p
                 p.gseg_base[m] = (int32_t)e.y;
             }
             p.midx[i] = m;
-            if (one) smidx[i] = m;
         }
         __syncthreads();
     }
     const int M = (int)(base_a >> 32);
     const int32_t nseg = (int32_t)(base_a & 0xffffffff);
-#pragma unroll 1
-    for (int i0 = tid; i0 < n; i0 += 8 * NT) {
-        int32_t o[8];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) o[u] = i0 + u * NT < n ? __ldg(p.owner_tl + i0 + u * NT) : 0;
-#pragma unroll
-        for (int u = 0; u < 8; ++u) o[u] = one ? smidx[o[u]] : p.midx[o[u]];
-#pragma unroll
-        for (int u = 0; u < 8; ++u)
-            if (i0 + u * NT < n) p.owner[i0 + u * NT] = o[u];
-    }
+    // (owner[] = merged index of every timeline's owner is a gather over all timelines: merge_plan_kernel does it GPU-wide)
     if (tid == 0) {
         p.merged_offsets[M] = base_b;
         p.gseg_base[M] = nseg;
@@ -1621,6 +1608,9 @@ __global__ void __launch_bounds__(256) merge_plan_kernel(const MergeParams p) {
         o.out_start = N_out; o.tok_delta = 0; o.lp_delta = 0; o.src = kSrcNone; o.aux = 0;
         p.gseg[p.ctrl->n_gsegs] = o;
     }
+    // owner[j] = merged index of the timeline that owns j (index map, reading M-12)
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < p.n; j += gridDim.x * blockDim.x)
+        p.owner[j] = __ldg(p.midx + __ldg(p.owner_tl + j));
 }
 
 // ---------------------------------------------------------------------------------------- K5: scatter (M7)
