@@ -121,7 +121,7 @@ struct MergeParams {
     uint32_t* ent_idx;     // [E_cap]
     uint32_t* tmp_dig;     // [E_cap]
     uint32_t* tmp_idx;     // [E_cap]
-    uint8_t* absorbed;     // [n] by timeline
+    uint2* cinfo;          // [n] by timeline, for the compaction: {1 << 24 | segments, length} of a survivor, {0, 0} of an absorbed one
     int32_t* owner_tl;     // [n] owning timeline (itself for survivors)
     int32_t* midx;         // [n] merged index of survivors, -1 otherwise
     int32_t* sel[8];       // [n] each, by sorted position: decision state of groups larger than kSelCacheK
@@ -158,7 +158,7 @@ __host__ MergeWs merge_ws_layout(int32_t n, int64_t N) {
     w.grp_rec = o; o += n16;
     w.unit_rec = o; o += a256(sc * 16);
     w.seg_part = o; o += a256(sc * 8);
-    w.absorbed = o; o += a256((size_t)n + 2);
+    w.absorbed = o; o += n8;   // (cinfo)
     w.owner_tl = o; o += n4; w.midx = o; o += n4;
     for (int k = 0; k < 8; ++k) { w.sel[k] = o; o += n4; }
     w.sel_q = o; o += n8;
@@ -1163,21 +1163,13 @@ __global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p
     int64_t base_a = 0, base_b = 0;   // {survivors << 32 | segments}, tokens, before this chunk
     for (int c0 = 0; c0 < n; c0 += kCompactChunk) {
         const int cn = min(kCompactChunk, n - c0);
-        int32_t tr[8];
         uint32_t sv[8];
-        // ---- A: coalesced loads, 8 timelines per thread in flight
+        // ---- A: coalesced loads, 8 timelines per thread in flight: one 8-byte record each, written by the select pass
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
             const int j = u * NT + tid, i = c0 + j;
             uint2 v = make_uint2(0u, 0u);
-            tr[u] = 0;
-            if (j < cn) {
-                const bool ab = __ldg(p.absorbed + i) != 0;
-                const int64_t L = __ldg(p.offsets + i + 1) - __ldg(p.offsets + i);
-                const uint32_t ns = (uint32_t)__ldg(reinterpret_cast<const int32_t*>(p.sv_rec + i) + 3);   // (garbage if absorbed: unused)
-                tr[u] = __ldg(p.traj_ids + i);
-                if (!ab) v = make_uint2((1u << 24) | (ns & 0xffffffu), (uint32_t)L);
-            }
+            if (j < cn) v = __ldg(p.cinfo + i);
             sv[u] = v.x;
             prA[j] = v;
         }
@@ -1228,7 +1220,6 @@ __global__ void __launch_bounds__(1024) merge_compact_kernel(const MergeParams p
                 const uint2 e = prA[j];
                 m = (int32_t)e.x;
                 p.merged_origin[m] = i;
-                p.merged_traj[m] = tr[u];
                 p.merged_offsets[m] = prB[j];
                 p.gseg_base[m] = (int32_t)e.y;
             }
@@ -1275,12 +1266,15 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
                 const int i = __ldg(p.perm + gs), L = __ldg(p.glen + gs);
                 const int rs = explicit_masks ? 0 : min(max(__ldg(p.resp_start + i), 0), L);
                 if (lane == 0) {
-                    p.absorbed[i] = 0; p.owner_tl[i] = i; mem[0] = i;
+                    p.owner_tl[i] = i; mem[0] = i;
                     p.sel[3][gs] = L; p.sel[4][gs] = rs;
                 }
                 __syncwarp();
                 const int sc = build_segments(explicit_masks, mem, p.sel[3] + gs, p.sel[4] + gs, 1, rs_out);
-                if (lane == 0) p.sv_rec[i] = make_int4(gs, 1, 2 * gs, sc);
+                if (lane == 0) {
+                    p.sv_rec[i] = make_int4(gs, 1, 2 * gs, sc);
+                    p.cinfo[i] = make_uint2((1u << 24) | (uint32_t)sc, (uint32_t)L);
+                }
             }
             continue;
         }
@@ -1523,7 +1517,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
         // ---- outputs by timeline; members of every survivor, ascending
         for (int b = tid; b < k; b += NT) {
             const int j = gl[b], o = own[b] < 0 ? b : own[b];
-            p.absorbed[j] = own[b] >= 0;
+            if (own[b] >= 0) p.cinfo[j] = make_uint2(0u, 0u);
             p.owner_tl[j] = gl[o];
             atomicAdd(&mcnt[o], 1);
         }
@@ -1552,7 +1546,10 @@ __global__ void __launch_bounds__(kSelThreads, 2) merge_select_kernel(const Merg
             if (own[b] >= 0) continue;
             const int mb = mbase[b], mc = mcnt[b];
             const int sc = build_segments(explicit_masks, mj + mb, mL + mb, mR + mb, mc, rs_out + 2 * mb);
-            if (lane == 0) p.sv_rec[gl[b]] = make_int4(gs + mb, mc, 2 * (gs + mb), sc);
+            if (lane == 0) {
+                p.sv_rec[gl[b]] = make_int4(gs + mb, mc, 2 * (gs + mb), sc);
+                p.cinfo[gl[b]] = make_uint2((1u << 24) | (uint32_t)sc, (uint32_t)gln[b]);
+            }
         }
         __syncthreads();
     }
@@ -1578,6 +1575,7 @@ __global__ void __launch_bounds__(256) merge_plan_kernel(const MergeParams p) {
         const int4 sr = __ldg(p.sv_rec + s);
         const int64_t mo = __ldg(p.merged_offsets + m), mo1 = __ldg(p.merged_offsets + m + 1), so = __ldg(p.offsets + s);
         const int gb = __ldg(p.gseg_base + m);
+        if (lane == 0) p.merged_traj[m] = __ldg(p.traj_ids + s);
         for (int li = lane; li < sr.w; li += 32) {
             const int2 rs = __ldg(p.rseg + sr.z + li);
             GSeg o;
@@ -1963,7 +1961,7 @@ extern "C" int ajt_merge_timelines(const int32_t* tokens, const int64_t* offsets
     p.grp_rec = reinterpret_cast<int4*>(b + ws.grp_rec);
     p.unit_rec = reinterpret_cast<int4*>(b + ws.unit_rec);
     p.seg_part = reinterpret_cast<uint64_t*>(b + ws.seg_part);
-    p.absorbed = b + ws.absorbed;
+    p.cinfo = reinterpret_cast<uint2*>(b + ws.absorbed);
     p.owner_tl = reinterpret_cast<int32_t*>(b + ws.owner_tl);
     p.midx = reinterpret_cast<int32_t*>(b + ws.midx);
     for (int k = 0; k < 8; ++k) p.sel[k] = reinterpret_cast<int32_t*>(b + ws.sel[k]);
