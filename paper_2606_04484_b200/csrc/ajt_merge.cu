@@ -1705,7 +1705,7 @@ __device__ __noinline__ void scatter_tile_walk(const ScatPtrs p, int t, int64_t 
     }
 }
 
-constexpr int kScatThreads = 640;                                   // 20 warps: what the shared memory of one SM holds
+constexpr int kScatThreads = 512;                                   // 16 warps: 118 registers without spills (20 warps fit the shared memory but spill at 96)
 constexpr int kScatInBytes = 2560;                                   // one input array of a tile: 2 KB + 16-byte slack of up to 8 pieces
 constexpr int kScatWarpBytes = 2 * 2 * kScatInBytes + 2 * 8 * 32 + 128;   // 2 input stages (tokens, old_logp), piece tables, barriers
 constexpr int kScatSmem = (kScatThreads / 32) * kScatWarpBytes + 128;
