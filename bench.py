@@ -407,7 +407,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                        "; its bytes are not counted in `value`)"},
             "loss": {"ms": loss_ms, "logits_gb_per_s": ach, "frac_of_measured": ach / peak,
                      "frac_of_nominal_8tbs": ach / NOMINAL_HBM_GBS, "algorithmic_bytes": loss_b,
-                     "dense_2TV_gb_per_s": 4.0 * T * V / (loss_ms * 1e-3) / 1e9, "mask_density": rho},
+                     "dense_2TV_gb_per_s": 4.0 * T * V / (loss_ms * 1e-3) / 1e9, "mask_density": rho,
+                     "chunks_in_batch": int((B.N_out + T - 1) // T),
+                     "batch_loss_s_extrapolated": float((B.N_out + T - 1) // T) * loss_ms * 1e-3,
+                     "extrapolation": "the batch's merged tokens in chunks of loss_rows x this call's time (chunks are "
+                                      "independent given the batch-wide N_s; SURVEY.md 8(d) configs[2])"},
             "roofline": {"bound": "hbm", "kernel": shape_key + " (timed as the ajt_policy_loss_fwd_bwd call: prep + rows + final "
                          "launches; rows is >99% of it, profiles/)", "achieved": ach, "peak": peak, "unit": "GB/s",
                          "frac": ach / peak, "traffic": traffic, "traffic_note": traffic_note, "peak_source": peak_src},
